@@ -1,0 +1,143 @@
+/*
+ * dvx.h - C ABI of libdvx: the single-pass compositional sparse-voxel tile rasterizer of
+ * "Driving Voxels" (arxiv/paper_2606_23031), forward and backward, for one NVIDIA B200 (sm_100a).
+ *
+ * What the calls compute (PAPER.md = the paper text; R# = readings listed in DESIGN.md section 3):
+ *   render   : Algorithm 1 "Scene Rendering with Segmented Volume Rendering" over
+ *              one static world-frame octree O_bg and N rigid actor octrees O_i under poses T_t^i
+ *              (PAPER.md:63, :73-75), per-ray ray-OBB intervals sorted front to back (PAPER.md:101-105,
+ *              :295), accumulation function F over Morton-ordered per-tile voxel lists with the state
+ *              S = (C, D, T, tau_curr), T_final returned as alpha (Eq. 2, :111).
+ *   backward : "Gradients flow through each voxel segment independently": gradients of the
+ *              8 corner raw densities v_geo and of the per-voxel SH colour coefficients.
+ *
+ * Conventions
+ *   - Plain C.  No exception, abort, exit or print ever crosses this boundary; every call returns a
+ *     dvx_status (0 = DVX_OK, negative = error) and dvx_last_error() gives the text of the last failure.
+ *   - "DEVICE" pointers are CUDA device pointers on the context's device, owned by the caller and only
+ *     borrowed by the library; "HOST" pointers are ordinary host memory, read before the call returns.
+ *   - All GPU work is enqueued on the context's stream.  dvx_render synchronises that stream once
+ *     internally (it has to learn the number of (tile, voxel) pairs to size the sort); dvx_backward does
+ *     not synchronise.  The caller synchronises before reading outputs.
+ *   - There is no CPU fallback: without a CUDA device dvx_create fails with DVX_ERR_CUDA.
+ */
+#ifndef DVX_H_
+#define DVX_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef int32_t dvx_status;
+#define DVX_OK 0
+#define DVX_ERR_INVALID_ARG (-1)     /* null pointer, n_actors > 64, sh_degree > 3, k_samples not in [1,8], bad camera, pose not rigid */
+#define DVX_ERR_BAD_OCTREE (-2)      /* level not in [1,16], code bits below the level not zero, duplicate or nested leaves */
+#define DVX_ERR_OOM (-3)             /* the allocator returned NULL */
+#define DVX_ERR_CUDA (-4)            /* CUDA runtime error (sticky); text via dvx_last_error */
+#define DVX_ERR_NOT_IMPLEMENTED (-5)
+
+#define DVX_MAX_ACTORS 64
+#define DVX_MAX_LEVEL 16
+#define DVX_TILE 16 /* 16x16 pixel tiles (BASELINE.json north_star (1)) */
+
+typedef struct dvx_ctx dvx_ctx;       /* opaque: device, stream, scratch cache */
+typedef struct dvx_octree dvx_octree; /* opaque: borrowed array pointers + cached per-octant rank tables (step 0) */
+typedef struct dvx_frame dvx_frame;   /* opaque: what dvx_backward needs from one dvx_render call */
+
+/* Device memory comes from the caller (the PyTorch caching allocator in practice).  Both NULL = cudaMalloc/cudaFree. */
+typedef void *(*dvx_alloc_fn)(size_t bytes, void *user);
+typedef void (*dvx_free_fn)(void *ptr, void *user);
+
+/* device: CUDA ordinal.  cuda_stream: a cudaStream_t (NULL = the legacy default stream). */
+dvx_status dvx_create(int device, void *cuda_stream, dvx_alloc_fn alloc, dvx_free_fn free_, void *user, dvx_ctx **out);
+void dvx_destroy(dvx_ctx *ctx);
+
+/* One leaf-only octree.  All three arrays are DEVICE pointers, borrowed until dvx_octree_destroy;
+ * geo and sh may change in place between renders (they are re-read every frame), code may not (see refresh). */
+typedef struct {
+  uint32_t n_voxels;    /* V >= 0 */
+  uint32_t sh_degree;   /* 0..3; C_sh = (deg+1)^2 basis functions */
+  float center[3];      /* w_c: cube centre in the octree's own frame */
+  float side;           /* w_s: root cube edge length (> 0) */
+  const uint64_t *code; /* [V] bits 48-52 = level l in [1,16]; bits 0-47 = Morton path left-aligned: 3-bit group
+                           m in [0,l) at bits [45-3m,47-3m] = 4 x_m + 2 y_m + z_m, x_m = bit (l-1-m) of the cell
+                           coordinate i; groups m >= l are zero (R14a) */
+  const float *geo;     /* [V][8] raw corner densities, corner c = 4 b_x + 2 b_y + b_z (R7); 32-byte aligned */
+  const float *sh;      /* [V][C_sh][3] SH colour coefficients (R8); 16-byte aligned */
+} dvx_octree_desc;
+
+/* Validates the leaf set and builds the per-octant rank tables (hot-path step 0: rank of every voxel under the key
+ * morton48 XOR q*0x249249249249, q = 4 s_x + 2 s_y + s_z, s_a = (d_a < 0); R14b).  Synchronises the stream. */
+dvx_status dvx_octree_create(dvx_ctx *ctx, const dvx_octree_desc *desc, dvx_octree **out);
+/* The leaf set (code / n_voxels) changed: revalidate and rebuild the rank tables. */
+dvx_status dvx_octree_refresh_structure(dvx_ctx *ctx, dvx_octree *tree, const dvx_octree_desc *desc);
+void dvx_octree_destroy(dvx_ctx *ctx, dvx_octree *tree);
+
+/* Pinhole camera (R10): pixel centres at half-integers; camera axes x right, y down, z forward. */
+typedef struct {
+  uint32_t width, height;
+  float fx, fy, cx, cy;
+  float c2w[12]; /* row-major 3x4 [R_c | o_c] */
+  float near_;   /* tau starts here (R11), > 0 */
+  float far_;    /* tau_max */
+} dvx_camera;
+
+typedef struct {
+  uint32_t k_samples;  /* K midpoint samples per clipped ray-voxel segment, 1..8 (R6) */
+  uint32_t activation; /* 0 = exp (default), 1 = exp-linear with theta = 1.1 (R5) */
+  float t_stop;        /* early termination T < t_stop, tested after every voxel (R3); 0 disables */
+  uint32_t flags;      /* DVX_FLAG_* */
+} dvx_render_opts;
+#define DVX_FLAG_COUNTERS 1u /* maintain q_test / q_hit / pairs_eff (slower; off in timed runs) */
+#define DVX_FLAG_NAIVE 2u    /* debug: per-thread in-order walker instead of the cooperative tile kernel */
+
+typedef struct {
+  float *rgb;   /* DEVICE [H][W][3] */
+  float *depth; /* DEVICE [H][W]  D = sum T_j alpha_j (a_j+b_j)/2, Euclidean ray distance (R9) */
+  float *alpha; /* DEVICE [H][W]  1 - T_final */
+} dvx_image;
+
+/* Steps 1-4 of the hot path.  poses_l2w: HOST [N][12] row-major [R_i | t_i] local->world;
+ * box_half: HOST [N][3] half extents of the oriented box in the actor frame.  opts NULL = defaults
+ * (K=8, exp, t_stop=1e-4, flags 0).  saved: if non-NULL receives a frame handle for dvx_backward / introspection
+ * (release with dvx_frame_release); NULL = inference, nothing kept. */
+dvx_status dvx_render(dvx_ctx *ctx, const dvx_camera *cam, const dvx_octree *static_tree, uint32_t n_actors,
+                      const dvx_octree *const *actors, const float *poses_l2w, const float *box_half,
+                      const dvx_render_opts *opts, dvx_image out, dvx_frame **saved);
+
+typedef struct {
+  float *dgeo; /* DEVICE [V][8]       same shape as geo; ACCUMULATED (+=); may be NULL (skipped) */
+  float *dsh;  /* DEVICE [V][C_sh][3] same shape as sh;  ACCUMULATED (+=); may be NULL (skipped) */
+} dvx_grad;
+
+/* Step 5.  dL_drgb DEVICE [H][W][3]; dL_ddepth / dL_dalpha DEVICE [H][W] or NULL (= zero).
+ * static_grad for the static octree, actor_grads HOST array [N] of DEVICE pointers, same order as in dvx_render.
+ * No gradient flows to geometry (camera, poses, voxel positions) nor through the per-voxel view direction. */
+dvx_status dvx_backward(dvx_ctx *ctx, dvx_frame *saved, const float *dL_drgb, const float *dL_ddepth,
+                        const float *dL_dalpha, dvx_grad static_grad, const dvx_grad *actor_grads);
+void dvx_frame_release(dvx_ctx *ctx, dvx_frame *frame);
+
+/* Introspection for the parity tests and the benchmark (each synchronises the stream).
+ * dvx_debug_tile_list: the sorted voxel list (voxel indices within octree `octree`, 0 = static, i = actor i-1) of
+ * tile `tile` (row-major tile index) for ray-direction octant `octant`; ids_host HOST [capacity]; *n_out = full length. */
+dvx_status dvx_debug_tile_list(dvx_ctx *ctx, const dvx_frame *frame, uint32_t tile, uint32_t octree, uint32_t octant,
+                               uint32_t *ids_host, uint32_t capacity, uint32_t *n_out);
+/* v_vis: voxels surviving culling; pairs: (tile, octant, voxel) pairs sorted; the last three need DVX_FLAG_COUNTERS. */
+dvx_status dvx_frame_counters(dvx_ctx *ctx, const dvx_frame *frame, uint64_t *v_vis, uint64_t *pairs,
+                              uint64_t *pairs_eff, uint64_t *q_test, uint64_t *q_hit);
+/* Device milliseconds of the stages of the frame's dvx_render call: [0] preprocess (step 1), [1] key generation +
+ * sort + ranges (step 2), [2] compositing (steps 3+4); after dvx_backward also [3] backward (step 5). HOST out[4]. */
+dvx_status dvx_frame_stage_ms(dvx_ctx *ctx, const dvx_frame *frame, float *ms_out4);
+const char *dvx_last_error(const dvx_ctx *ctx);
+
+/* Stand-alone entry to hot-path step 2's sort (tests and sort-throughput measurement): sorts n (key, value) pairs by
+ * the low key_bits bits of the key, ascending, stable.  keys / vals DEVICE arrays, sorted in place. */
+dvx_status dvx_sort_pairs(dvx_ctx *ctx, uint64_t *keys, uint32_t *vals, uint64_t n, uint32_t key_bits);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DVX_H_ */

@@ -1,0 +1,277 @@
+"""Thin ctypes binding of libdvx.so (include/dvx.h): argument marshalling only.
+
+Every step of the hot path runs in the CUDA kernels behind the C ABI; PyTorch is used for device memory
+(``torch.empty`` through the allocator callbacks) and the stream.  There is no CPU fallback: importing works
+anywhere (so the symbol table can be checked), but creating a ``Context`` without a CUDA device raises.
+"""
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libdvx.so")
+
+DVX_OK = 0
+ERRORS = {-1: "DVX_ERR_INVALID_ARG", -2: "DVX_ERR_BAD_OCTREE", -3: "DVX_ERR_OOM", -4: "DVX_ERR_CUDA",
+          -5: "DVX_ERR_NOT_IMPLEMENTED"}
+FLAG_COUNTERS = 1
+FLAG_NAIVE = 2
+
+EXPORTS = ["dvx_create", "dvx_destroy", "dvx_octree_create", "dvx_octree_refresh_structure", "dvx_octree_destroy",
+           "dvx_render", "dvx_backward", "dvx_frame_release", "dvx_debug_tile_list", "dvx_frame_counters",
+           "dvx_frame_stage_ms", "dvx_last_error", "dvx_sort_pairs"]
+
+
+class DvxError(RuntimeError):
+    def __init__(self, status, text):
+        super().__init__("%s (%d): %s" % (ERRORS.get(status, "?"), status, text))
+        self.status = status
+
+
+class OctreeDesc(C.Structure):
+    _fields_ = [("n_voxels", C.c_uint32), ("sh_degree", C.c_uint32), ("center", C.c_float * 3), ("side", C.c_float),
+                ("code", C.c_void_p), ("geo", C.c_void_p), ("sh", C.c_void_p)]
+
+
+class Camera(C.Structure):
+    _fields_ = [("width", C.c_uint32), ("height", C.c_uint32), ("fx", C.c_float), ("fy", C.c_float), ("cx", C.c_float),
+                ("cy", C.c_float), ("c2w", C.c_float * 12), ("near_", C.c_float), ("far_", C.c_float)]
+
+
+class RenderOpts(C.Structure):
+    _fields_ = [("k_samples", C.c_uint32), ("activation", C.c_uint32), ("t_stop", C.c_float), ("flags", C.c_uint32)]
+
+
+class Image(C.Structure):
+    _fields_ = [("rgb", C.c_void_p), ("depth", C.c_void_p), ("alpha", C.c_void_p)]
+
+
+class Grad(C.Structure):
+    _fields_ = [("dgeo", C.c_void_p), ("dsh", C.c_void_p)]
+
+
+ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_size_t, C.c_void_p)
+FREE_FN = C.CFUNCTYPE(None, C.c_void_p, C.c_void_p)
+
+_lib = None
+
+
+def load():
+    """dlopen libdvx.so (built in-tree by paper_2606_23031_b200.build) and declare the signatures."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise ImportError("libdvx.so is missing: run `python -m paper_2606_23031_b200.build` (there is no CPU fallback)")
+    lib = C.CDLL(LIB_PATH)
+    P = C.c_void_p
+    lib.dvx_create.argtypes = [C.c_int, P, ALLOC_FN, FREE_FN, P, C.POINTER(P)]
+    lib.dvx_destroy.argtypes = [P]
+    lib.dvx_destroy.restype = None
+    lib.dvx_octree_create.argtypes = [P, C.POINTER(OctreeDesc), C.POINTER(P)]
+    lib.dvx_octree_refresh_structure.argtypes = [P, P, C.POINTER(OctreeDesc)]
+    lib.dvx_octree_destroy.argtypes = [P, P]
+    lib.dvx_octree_destroy.restype = None
+    lib.dvx_render.argtypes = [P, C.POINTER(Camera), P, C.c_uint32, C.POINTER(P), P, P, C.POINTER(RenderOpts), Image,
+                               C.POINTER(P)]
+    lib.dvx_backward.argtypes = [P, P, P, P, P, Grad, C.POINTER(Grad)]
+    lib.dvx_frame_release.argtypes = [P, P]
+    lib.dvx_frame_release.restype = None
+    lib.dvx_debug_tile_list.argtypes = [P, P, C.c_uint32, C.c_uint32, C.c_uint32, P, C.c_uint32, C.POINTER(C.c_uint32)]
+    lib.dvx_frame_counters.argtypes = [P, P] + [C.POINTER(C.c_uint64)] * 5
+    lib.dvx_frame_stage_ms.argtypes = [P, P, C.POINTER(C.c_float)]
+    lib.dvx_last_error.argtypes = [P]
+    lib.dvx_last_error.restype = C.c_char_p
+    lib.dvx_sort_pairs.argtypes = [P, P, P, C.c_uint64, C.c_uint32]
+    for name in EXPORTS:
+        if name not in ("dvx_destroy", "dvx_octree_destroy", "dvx_frame_release", "dvx_last_error"):
+            getattr(lib, name).restype = C.c_int32
+    _lib = lib
+    return lib
+
+
+class Context:
+    """dvx_create on a CUDA device; device scratch comes from the PyTorch caching allocator."""
+
+    def __init__(self, device=0, stream=None, torch_alloc=True):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("libdvx needs a CUDA device (sm_100a); there is no CPU fallback")
+        self.lib = load()
+        self.torch = torch
+        self.device = torch.device("cuda", device)
+        self._blocks = {}
+        self._alloc_cb = ALLOC_FN(self._alloc)
+        self._free_cb = FREE_FN(self._free)
+        self.stream = stream
+        handle = C.c_void_p()
+        with torch.cuda.device(self.device):
+            st = stream.cuda_stream if stream is not None else torch.cuda.current_stream().cuda_stream
+        self._stream_ptr = st
+        if torch_alloc:
+            rc = self.lib.dvx_create(device, C.c_void_p(st), self._alloc_cb, self._free_cb, None, C.byref(handle))
+        else:
+            rc = self.lib.dvx_create(device, C.c_void_p(st), ALLOC_FN(0), FREE_FN(0), None, C.byref(handle))
+        if rc != DVX_OK:
+            raise DvxError(rc, "dvx_create failed")
+        self.h = handle
+
+    def _alloc(self, nbytes, _user):
+        try:
+            t = self.torch.empty(int(nbytes), dtype=self.torch.uint8, device=self.device)
+        except Exception:  # out of memory -> NULL -> DVX_ERR_OOM
+            return None
+        self._blocks[t.data_ptr()] = t
+        return t.data_ptr()
+
+    def _free(self, ptr, _user):
+        self._blocks.pop(ptr, None)
+
+    def check(self, rc):
+        if rc != DVX_OK:
+            raise DvxError(rc, self.lib.dvx_last_error(self.h).decode())
+
+    def close(self):
+        if self.h:
+            self.lib.dvx_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # ------------------------------------------------------------------ octrees
+    def octree(self, code, geo, sh, center, side, sh_degree):
+        return Octree(self, code, geo, sh, center, side, sh_degree)
+
+    # ------------------------------------------------------------------ render / backward
+    def render(self, cam, static, actors=(), poses=None, box_half=None, k_samples=8, activation=0, t_stop=1e-4, flags=0,
+               save=True, out=None):
+        """dvx_render.  cam: binding.Camera; poses [N,12] / box_half [N,3] host float32 arrays.
+        Returns (rgb [H,W,3], depth [H,W], alpha [H,W], Frame or None)."""
+        torch = self.torch
+        H, W = cam.height, cam.width
+        if out is None:
+            rgb = torch.empty((H, W, 3), dtype=torch.float32, device=self.device)
+            depth = torch.empty((H, W), dtype=torch.float32, device=self.device)
+            alpha = torch.empty((H, W), dtype=torch.float32, device=self.device)
+        else:
+            rgb, depth, alpha = out
+        n = len(actors)
+        handles = (C.c_void_p * max(n, 1))(*[a.h for a in actors])
+        poses = np.ascontiguousarray(np.zeros((0, 12)) if poses is None else poses, dtype=np.float32).reshape(-1)
+        half = np.ascontiguousarray(np.zeros((0, 3)) if box_half is None else box_half, dtype=np.float32).reshape(-1)
+        assert poses.size == 12 * n and half.size == 3 * n
+        opts = RenderOpts(k_samples, activation, t_stop, flags)
+        img = Image(rgb.data_ptr(), depth.data_ptr(), alpha.data_ptr())
+        fh = C.c_void_p()
+        rc = self.lib.dvx_render(self.h, C.byref(cam), static.h, n, handles, poses.ctypes.data_as(C.c_void_p),
+                                 half.ctypes.data_as(C.c_void_p), C.byref(opts), img, C.byref(fh) if save else None)
+        self.check(rc)
+        frame = Frame(self, fh, [static] + list(actors)) if save else None
+        return rgb, depth, alpha, frame
+
+
+class Octree:
+    """dvx_octree_create over caller-owned CUDA tensors (kept alive here)."""
+
+    def __init__(self, ctx, code, geo, sh, center, side, sh_degree):
+        torch = ctx.torch
+        self.ctx = ctx
+        self.code = code.contiguous()
+        self.geo = geo.contiguous()
+        self.sh = sh.contiguous()
+        assert self.code.dtype in (torch.int64, torch.uint64) and self.geo.dtype == torch.float32 and self.sh.dtype == torch.float32
+        self.n_voxels = int(self.code.shape[0])
+        self.sh_degree = int(sh_degree)
+        self.n_sh = (self.sh_degree + 1) ** 2
+        self.desc = OctreeDesc(self.n_voxels, self.sh_degree, (C.c_float * 3)(*[float(x) for x in center]), float(side),
+                               self.code.data_ptr() if self.n_voxels else None,
+                               self.geo.data_ptr() if self.n_voxels else None,
+                               self.sh.data_ptr() if self.n_voxels else None)
+        h = C.c_void_p()
+        ctx.check(ctx.lib.dvx_octree_create(ctx.h, C.byref(self.desc), C.byref(h)))
+        self.h = h
+
+    def close(self):
+        if self.h and self.ctx.h:
+            self.ctx.lib.dvx_octree_destroy(self.ctx.h, self.h)
+        self.h = None
+
+
+class Frame:
+    def __init__(self, ctx, h, trees):
+        self.ctx, self.h, self.trees = ctx, h, trees
+
+    def backward(self, dL_drgb, dL_ddepth=None, dL_dalpha=None, grads=None):
+        """dvx_backward.  grads: list of (dgeo, dsh) tensors per octree (accumulated into); None = fresh zeros.
+        Returns the list of (dgeo, dsh)."""
+        ctx, torch = self.ctx, self.ctx.torch
+        if grads is None:
+            grads = [(torch.zeros((t.n_voxels, 8), dtype=torch.float32, device=ctx.device),
+                      torch.zeros((t.n_voxels, t.n_sh, 3), dtype=torch.float32, device=ctx.device)) for t in self.trees]
+        g = [Grad(a.data_ptr() if a is not None else None, b.data_ptr() if b is not None else None) for a, b in grads]
+        n = len(self.trees) - 1
+        arr = (Grad * max(n, 1))(*g[1:])
+        ptr = lambda t: None if t is None else t.data_ptr()
+        ctx.check(ctx.lib.dvx_backward(ctx.h, self.h, ptr(dL_drgb), ptr(dL_ddepth), ptr(dL_dalpha), g[0], arr))
+        return grads
+
+    def tile_list(self, tile, octree, octant):
+        ctx = self.ctx
+        n = C.c_uint32()
+        ctx.check(ctx.lib.dvx_debug_tile_list(ctx.h, self.h, tile, octree, octant, None, 0, C.byref(n)))
+        ids = np.zeros(max(n.value, 1), dtype=np.uint32)
+        ctx.check(ctx.lib.dvx_debug_tile_list(ctx.h, self.h, tile, octree, octant, ids.ctypes.data_as(C.c_void_p), n.value,
+                                              C.byref(n)))
+        return ids[:n.value]
+
+    def counters(self):
+        ctx = self.ctx
+        v = [C.c_uint64() for _ in range(5)]
+        ctx.check(ctx.lib.dvx_frame_counters(ctx.h, self.h, *[C.byref(x) for x in v]))
+        return dict(zip(("v_vis", "pairs", "pairs_eff", "q_test", "q_hit"), [x.value for x in v]))
+
+    def stage_ms(self):
+        ctx = self.ctx
+        ms = (C.c_float * 4)()
+        ctx.check(ctx.lib.dvx_frame_stage_ms(ctx.h, self.h, ms))
+        return dict(zip(("preprocess", "sort", "composite", "backward"), list(ms)))
+
+    def release(self):
+        if self.h and self.ctx.h:
+            self.ctx.lib.dvx_frame_release(self.ctx.h, self.h)
+        self.h = None
+
+
+def camera_from(cam):
+    """dvx_scenes.Camera (or anything with the same attributes) -> binding.Camera."""
+    return Camera(cam.width, cam.height, cam.fx, cam.fy, cam.cx, cam.cy,
+                  (C.c_float * 12)(*[float(x) for x in np.asarray(cam.c2w).reshape(12)]), cam.near, cam.far)
+
+
+class SceneOnDevice:
+    """Uploads a dvx_scenes.Scene (host numpy) to the GPU and creates the octree handles."""
+
+    def __init__(self, ctx, scene):
+        torch = ctx.torch
+        self.ctx, self.scene = ctx, scene
+        self.trees = []
+        for t in scene.octrees:
+            code = torch.from_numpy(np.ascontiguousarray(t.code).view(np.int64)).to(ctx.device)
+            geo = torch.from_numpy(np.ascontiguousarray(t.geo, dtype=np.float32)).to(ctx.device)
+            sh = torch.from_numpy(np.ascontiguousarray(t.sh, dtype=np.float32)).to(ctx.device)
+            self.trees.append(ctx.octree(code, geo, sh, t.center, t.side, t.sh_degree))
+        self.poses = np.ascontiguousarray(scene.poses, dtype=np.float32)
+        self.box_half = np.ascontiguousarray(scene.box_half, dtype=np.float32)
+        self.cams = [camera_from(c) for c in scene.cameras]
+
+    def render(self, cam_index=0, save=True, flags=0, out=None, **opt):
+        s = self.scene
+        kw = dict(k_samples=s.k_samples, activation=s.activation, t_stop=s.t_stop)
+        kw.update(opt)
+        return self.ctx.render(self.cams[cam_index], self.trees[0], self.trees[1:], self.poses, self.box_half, flags=flags,
+                               save=save, out=out, **kw)

@@ -1,0 +1,514 @@
+// dvx_api.cu - the C ABI of include/dvx.h: argument checks, per-frame host set-up, scratch cache, stage sequencing.
+// No arithmetic of the rendering method lives here except the per-tree frame set-up (poses composed in fp64).
+#include <math.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <string>
+#include <vector>
+
+#include "dvx_internal.cuh"
+
+struct dvx_ctx {
+  int device = 0;
+  cudaStream_t st = nullptr;
+  dvx_alloc_fn alloc = nullptr;
+  dvx_free_fn free_ = nullptr;
+  void *user = nullptr;
+  struct Block { void *p; size_t bytes; };
+  std::vector<Block> cache;  // released scratch blocks, reused stream-ordered
+  std::vector<Block> all;    // every block ever obtained (freed in dvx_destroy)
+  unsigned long long *h_counters = nullptr;  // pinned
+  std::string err;
+};
+
+struct dvx_octree {
+  dvx_octree_desc d;
+  uint32_t *rank = nullptr;  // [8][V]
+  size_t rank_bytes = 0;
+};
+
+struct dvx_frame {
+  FrameParams p;
+  std::vector<TreeFrame> trees_h;
+  struct Buf { void *p = nullptr; size_t bytes = 0; };
+  Buf trees_d, fvox, pxrect, octmask, actor_mask, ids, range_beg, range_end, counters, sv_rgbd, sv_T, sv_nused;
+  uint64_t n_pairs = 0, v_vis = 0;
+  cudaEvent_t ev[7] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+  bool did_backward = false;
+};
+
+namespace {
+
+dvx_status fail(dvx_ctx *ctx, dvx_status code, const char *msg) {
+  if (ctx) ctx->err = msg;
+  return code;
+}
+dvx_status cuda_fail(dvx_ctx *ctx, cudaError_t e, const char *where) {
+  if (ctx) ctx->err = std::string(where) + ": " + cudaGetErrorString(e);
+  return DVX_ERR_CUDA;
+}
+#define CU(call)                                          \
+  do {                                                    \
+    cudaError_t e_ = (call);                              \
+    if (e_ != cudaSuccess) return cuda_fail(ctx, e_, #call); \
+  } while (0)
+
+void *ctx_alloc(dvx_ctx *ctx, size_t bytes) {
+  if (bytes == 0) bytes = 256;
+  bytes = (bytes + 255) & ~(size_t)255;
+  int best = -1;
+  for (size_t i = 0; i < ctx->cache.size(); ++i) {
+    size_t b = ctx->cache[i].bytes;
+    if (b >= bytes && b <= 2 * bytes + 4096 && (best < 0 || b < ctx->cache[best].bytes)) best = (int)i;
+  }
+  if (best >= 0) {
+    void *p = ctx->cache[best].p;
+    ctx->cache.erase(ctx->cache.begin() + best);
+    return p;
+  }
+  void *p = nullptr;
+  if (ctx->alloc) {
+    p = ctx->alloc(bytes, ctx->user);
+  } else if (cudaMalloc(&p, bytes) != cudaSuccess) {
+    cudaGetLastError();
+    p = nullptr;
+  }
+  if (p) ctx->all.push_back({p, bytes});
+  return p;
+}
+void ctx_release(dvx_ctx *ctx, void *p) {
+  if (!p) return;
+  for (auto &b : ctx->all)
+    if (b.p == p) {
+      ctx->cache.push_back(b);
+      return;
+    }
+}
+bool buf_alloc(dvx_ctx *ctx, dvx_frame::Buf &b, size_t bytes) {
+  b.p = ctx_alloc(ctx, bytes);
+  b.bytes = bytes;
+  return b.p != nullptr;
+}
+
+uint32_t bits_for(uint64_t n_values) {  // bits needed to hold values 0..n_values-1 (at least 1)
+  uint32_t b = 1;
+  while (b < 63 && (1ull << b) < n_values) ++b;
+  return b;
+}
+
+void frame_free(dvx_ctx *ctx, dvx_frame *f) {
+  if (!f) return;
+  dvx_frame::Buf *bs[] = {&f->trees_d, &f->fvox, &f->pxrect, &f->octmask, &f->actor_mask, &f->ids,
+                          &f->range_beg, &f->range_end, &f->counters, &f->sv_rgbd, &f->sv_T, &f->sv_nused};
+  for (auto *b : bs) ctx_release(ctx, b->p);
+  for (auto &e : f->ev)
+    if (e) cudaEventDestroy(e);
+  delete f;
+}
+
+dvx_status build_rank_tables(dvx_ctx *ctx, dvx_octree *t) {
+  const uint32_t V = t->d.n_voxels;
+  if (t->rank) { ctx_release(ctx, t->rank); t->rank = nullptr; }
+  if (V == 0) return DVX_OK;
+  t->rank_bytes = (size_t)8 * V * sizeof(uint32_t);
+  t->rank = (uint32_t *)ctx_alloc(ctx, t->rank_bytes);
+  uint64_t *ka = (uint64_t *)ctx_alloc(ctx, (size_t)V * 8), *kb = (uint64_t *)ctx_alloc(ctx, (size_t)V * 8);
+  uint32_t *va = (uint32_t *)ctx_alloc(ctx, (size_t)V * 4), *vb = (uint32_t *)ctx_alloc(ctx, (size_t)V * 4);
+  void *scr = ctx_alloc(ctx, dvx_sort_scratch_bytes(V));
+  uint32_t *bad = (uint32_t *)ctx_alloc(ctx, 256);
+  dvx_status rc = DVX_OK;
+  if (!t->rank || !ka || !kb || !va || !vb || !scr || !bad) {
+    rc = fail(ctx, DVX_ERR_OOM, "dvx_octree_create: allocator returned NULL");
+  } else {
+    cudaMemsetAsync(bad, 0, 4, ctx->st);
+    for (int q = 0; q < 8; ++q) {
+      dvx_rank_keys_launch(t->d.code, V, q, ka, va, ctx->st);
+      int which = dvx_sort_launch(ka, va, kb, vb, V, 48, scr, ctx->st);
+      const uint64_t *sk = which ? kb : ka;
+      const uint32_t *perm = which ? vb : va;
+      if (q == 0) dvx_validate_launch(sk, perm, t->d.code, V, bad, ctx->st);
+      dvx_rank_scatter_launch(perm, V, t->rank + (size_t)q * V, ctx->st);
+    }
+    uint32_t h_bad = 0;
+    cudaError_t e = cudaMemcpyAsync(&h_bad, bad, 4, cudaMemcpyDeviceToHost, ctx->st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->st);
+    if (e != cudaSuccess) rc = cuda_fail(ctx, e, "dvx_octree_create");
+    else if (h_bad) rc = fail(ctx, DVX_ERR_BAD_OCTREE, "dvx_octree_create: invalid level, non-zero bits below the level, or duplicate/nested leaves");
+  }
+  ctx_release(ctx, ka); ctx_release(ctx, kb); ctx_release(ctx, va); ctx_release(ctx, vb);
+  ctx_release(ctx, scr); ctx_release(ctx, bad);
+  if (rc != DVX_OK && t->rank) { ctx_release(ctx, t->rank); t->rank = nullptr; }
+  return rc;
+}
+
+dvx_status check_desc(dvx_ctx *ctx, const dvx_octree_desc *d) {
+  if (!d) return fail(ctx, DVX_ERR_INVALID_ARG, "octree desc is NULL");
+  if (d->sh_degree > 3) return fail(ctx, DVX_ERR_INVALID_ARG, "sh_degree > 3");
+  if (!(d->side > 0.f) || !isfinite(d->side)) return fail(ctx, DVX_ERR_INVALID_ARG, "side must be positive");
+  if (d->n_voxels && (!d->code || !d->geo || !d->sh)) return fail(ctx, DVX_ERR_INVALID_ARG, "octree array pointer is NULL");
+  if (((uintptr_t)d->geo & 31) || ((uintptr_t)d->sh & 15) || ((uintptr_t)d->code & 7))
+    return fail(ctx, DVX_ERR_INVALID_ARG, "octree arrays must be aligned (code 8, geo 32, sh 16 bytes)");
+  return DVX_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+dvx_status dvx_create(int device, void *cuda_stream, dvx_alloc_fn alloc, dvx_free_fn free_, void *user, dvx_ctx **out) {
+  if (!out) return DVX_ERR_INVALID_ARG;
+  *out = nullptr;
+  if ((alloc == nullptr) != (free_ == nullptr)) return DVX_ERR_INVALID_ARG;
+  int n = 0;
+  if (cudaGetDeviceCount(&n) != cudaSuccess || device < 0 || device >= n) {
+    cudaGetLastError();
+    return DVX_ERR_CUDA;  // no CPU fallback
+  }
+  if (cudaSetDevice(device) != cudaSuccess) return DVX_ERR_CUDA;
+  dvx_ctx *ctx = new dvx_ctx();
+  ctx->device = device;
+  ctx->st = (cudaStream_t)cuda_stream;
+  ctx->alloc = alloc; ctx->free_ = free_; ctx->user = user;
+  if (cudaMallocHost((void **)&ctx->h_counters, CNT_N * sizeof(unsigned long long)) != cudaSuccess) {
+    delete ctx;
+    return DVX_ERR_CUDA;
+  }
+  *out = ctx;
+  return DVX_OK;
+}
+
+void dvx_destroy(dvx_ctx *ctx) {
+  if (!ctx) return;
+  cudaSetDevice(ctx->device);
+  cudaStreamSynchronize(ctx->st);
+  for (auto &b : ctx->all) {
+    if (ctx->free_) ctx->free_(b.p, ctx->user);
+    else cudaFree(b.p);
+  }
+  cudaFreeHost(ctx->h_counters);
+  delete ctx;
+}
+
+const char *dvx_last_error(const dvx_ctx *ctx) { return ctx ? ctx->err.c_str() : "context is NULL"; }
+
+dvx_status dvx_octree_create(dvx_ctx *ctx, const dvx_octree_desc *desc, dvx_octree **out) {
+  if (!ctx || !out) return fail(ctx, DVX_ERR_INVALID_ARG, "NULL argument");
+  *out = nullptr;
+  dvx_status rc = check_desc(ctx, desc);
+  if (rc != DVX_OK) return rc;
+  cudaSetDevice(ctx->device);
+  dvx_octree *t = new dvx_octree();
+  t->d = *desc;
+  rc = build_rank_tables(ctx, t);
+  if (rc != DVX_OK) { delete t; return rc; }
+  *out = t;
+  return DVX_OK;
+}
+
+dvx_status dvx_octree_refresh_structure(dvx_ctx *ctx, dvx_octree *tree, const dvx_octree_desc *desc) {
+  if (!ctx || !tree) return fail(ctx, DVX_ERR_INVALID_ARG, "NULL argument");
+  dvx_status rc = check_desc(ctx, desc);
+  if (rc != DVX_OK) return rc;
+  cudaSetDevice(ctx->device);
+  tree->d = *desc;
+  return build_rank_tables(ctx, tree);
+}
+
+void dvx_octree_destroy(dvx_ctx *ctx, dvx_octree *tree) {
+  if (!ctx || !tree) return;
+  ctx_release(ctx, tree->rank);
+  delete tree;
+}
+
+}  // extern "C"
+
+// ------------------------------------------------------------------------------------------------ render
+namespace {
+
+// Per-tree frame set-up in fp64: o_l = R_o^T (o_c - t_o), N = R_o^T R_c  (r_local = (T_t^i)^-1 r).
+void setup_tree(TreeFrame &T, const dvx_octree *t, uint32_t base, bool actor, const float *pose, const float *half,
+                const dvx_camera *cam) {
+  memset(&T, 0, sizeof(T));
+  T.code = t->d.code; T.geo = t->d.geo; T.sh = t->d.sh; T.rank = t->rank;
+  T.n_voxels = t->d.n_voxels; T.n_sh = (t->d.sh_degree + 1) * (t->d.sh_degree + 1);
+  T.base = base; T.is_actor = actor ? 1u : 0u;
+  for (int a = 0; a < 3; ++a) T.lo[a] = (double)t->d.center[a] - 0.5 * (double)t->d.side;
+  T.cell = (double)t->d.side / 65536.0;
+  double R[9] = {1, 0, 0, 0, 1, 0, 0, 0, 1}, tr[3] = {0, 0, 0};
+  if (actor)
+    for (int r = 0; r < 3; ++r) {
+      for (int c = 0; c < 3; ++c) R[3 * r + c] = pose[4 * r + c];
+      tr[r] = pose[4 * r + 3];
+    }
+  for (int a = 0; a < 3; ++a) {
+    double o = 0;
+    for (int r = 0; r < 3; ++r) o += R[3 * r + a] * ((double)cam->c2w[4 * r + 3] - tr[r]);
+    T.o_l[a] = o;
+    T.ol_f[a] = (float)o;
+    for (int c = 0; c < 3; ++c) {
+      double n = 0;
+      for (int r = 0; r < 3; ++r) n += R[3 * r + a] * (double)cam->c2w[4 * r + c];
+      T.N[3 * a + c] = (float)n;
+    }
+    T.half[a] = actor ? half[a] : INFINITY;
+  }
+}
+
+bool rigid(const float *m, int stride) {  // rows of a 3x3 inside a row-major matrix with `stride` columns
+  for (int i = 0; i < 3; ++i)
+    for (int j = 0; j < 3; ++j) {
+      double d = 0;
+      for (int k = 0; k < 3; ++k) d += (double)m[stride * k + i] * (double)m[stride * k + j];
+      if (!(fabs(d - (i == j ? 1.0 : 0.0)) < 1e-4)) return false;
+    }
+  return true;
+}
+
+}  // namespace
+
+extern "C" {
+
+dvx_status dvx_render(dvx_ctx *ctx, const dvx_camera *cam, const dvx_octree *static_tree, uint32_t n_actors,
+                      const dvx_octree *const *actors, const float *poses_l2w, const float *box_half,
+                      const dvx_render_opts *opts, dvx_image out, dvx_frame **saved) {
+  if (saved) *saved = nullptr;
+  if (!ctx) return DVX_ERR_INVALID_ARG;
+  if (!cam || !static_tree || !out.rgb || !out.depth || !out.alpha) return fail(ctx, DVX_ERR_INVALID_ARG, "NULL argument");
+  if (n_actors > DVX_MAX_ACTORS) return fail(ctx, DVX_ERR_INVALID_ARG, "n_actors > 64");
+  if (n_actors && (!actors || !poses_l2w || !box_half)) return fail(ctx, DVX_ERR_INVALID_ARG, "actor arrays are NULL");
+  dvx_render_opts o = {8u, 0u, 1e-4f, 0u};
+  if (opts) o = *opts;
+  if (o.k_samples < 1 || o.k_samples > 8) return fail(ctx, DVX_ERR_INVALID_ARG, "k_samples must be in [1,8]");
+  if (o.activation > 1) return fail(ctx, DVX_ERR_INVALID_ARG, "unknown activation");
+  if (!(o.t_stop >= 0.f)) return fail(ctx, DVX_ERR_INVALID_ARG, "t_stop must be >= 0");
+  if (cam->width == 0 || cam->height == 0 || cam->width > 65535 || cam->height > 65535 || !(cam->fx > 0.f) ||
+      !(cam->fy > 0.f) || !(cam->near_ > 0.f) || !(cam->far_ > cam->near_))
+    return fail(ctx, DVX_ERR_INVALID_ARG, "bad camera (size, focal length, near/far)");
+  if (!rigid(cam->c2w, 4)) return fail(ctx, DVX_ERR_INVALID_ARG, "camera rotation is not orthonormal");
+  for (uint32_t i = 0; i < n_actors; ++i) {
+    if (!actors[i]) return fail(ctx, DVX_ERR_INVALID_ARG, "actor handle is NULL");
+    if (!rigid(poses_l2w + 12 * i, 4)) return fail(ctx, DVX_ERR_INVALID_ARG, "actor pose is not rigid (R^T R != I to 1e-4)");
+    for (int a = 0; a < 3; ++a)
+      if (!(box_half[3 * i + a] >= 0.f)) return fail(ctx, DVX_ERR_INVALID_ARG, "negative box half extent");
+  }
+  cudaSetDevice(ctx->device);
+  cudaStream_t st = ctx->st;
+
+  dvx_frame *f = new dvx_frame();
+  FrameParams &p = f->p;
+  memset(&p, 0, sizeof(p));
+  p.width = cam->width; p.height = cam->height;
+  p.tiles_x = (cam->width + DVX_TILE - 1) / DVX_TILE; p.tiles_y = (cam->height + DVX_TILE - 1) / DVX_TILE;
+  p.n_tiles = p.tiles_x * p.tiles_y; p.n_trees = 1 + n_actors;
+  p.fx = cam->fx; p.fy = cam->fy; p.cx = cam->cx; p.cy = cam->cy; p.near_ = cam->near_; p.far_ = cam->far_;
+  {  // every point of a ray at tau >= near has z_cam >= near * min_pixels cos(angle to the axis) > zclip
+    double mc = 1.0;
+    const double us[2] = {0.5, (double)cam->width - 0.5}, vs[2] = {0.5, (double)cam->height - 0.5};
+    for (double uu : us)
+      for (double vv : vs) {
+        double x = (uu - cam->cx) / cam->fx, y = (vv - cam->cy) / cam->fy;
+        mc = fmin(mc, 1.0 / sqrt(x * x + y * y + 1.0));
+      }
+    p.zclip = (float)(0.5 * (double)cam->near_ * mc);
+  }
+  p.k_samples = o.k_samples; p.activation = o.activation; p.flags = o.flags; p.t_stop = o.t_stop;
+  f->trees_h.resize(p.n_trees);
+  uint64_t vtot = 0, vmax = 1;
+  for (uint32_t t = 0; t < p.n_trees; ++t) {
+    const dvx_octree *tr = t == 0 ? static_tree : actors[t - 1];
+    setup_tree(f->trees_h[t], tr, (uint32_t)vtot, t > 0, t ? poses_l2w + 12 * (t - 1) : nullptr,
+               t ? box_half + 3 * (t - 1) : nullptr, cam);
+    vtot += tr->d.n_voxels;
+    if (tr->d.n_voxels > vmax) vmax = tr->d.n_voxels;
+  }
+  if (vtot >= 0xFFFFFFFFull) { frame_free(ctx, f); return fail(ctx, DVX_ERR_INVALID_ARG, "more than 2^32-2 voxels in total"); }
+  p.v_total = (uint32_t)vtot;
+  p.rank_bits = bits_for(vmax);
+  p.n_buckets = p.n_tiles * p.n_trees * 8u;
+  const uint32_t key_bits = p.rank_bits + bits_for(p.n_buckets);
+  const size_t npix = (size_t)p.width * p.height;
+
+  bool ok = buf_alloc(ctx, f->trees_d, sizeof(TreeFrame) * p.n_trees) && buf_alloc(ctx, f->fvox, sizeof(FrameVox) * (size_t)p.v_total) &&
+            buf_alloc(ctx, f->pxrect, sizeof(ushort4) * (size_t)p.v_total) && buf_alloc(ctx, f->octmask, (size_t)p.n_tiles * p.n_trees) &&
+            buf_alloc(ctx, f->actor_mask, sizeof(unsigned long long) * p.n_tiles) &&
+            buf_alloc(ctx, f->range_beg, sizeof(uint32_t) * (size_t)p.n_buckets) &&
+            buf_alloc(ctx, f->range_end, sizeof(uint32_t) * (size_t)p.n_buckets) &&
+            buf_alloc(ctx, f->counters, sizeof(unsigned long long) * CNT_N);
+  if (ok && saved)
+    ok = buf_alloc(ctx, f->sv_rgbd, npix * 16) && buf_alloc(ctx, f->sv_T, npix * 4) && buf_alloc(ctx, f->sv_nused, npix * 4);
+  if (!ok) { frame_free(ctx, f); return fail(ctx, DVX_ERR_OOM, "dvx_render: allocator returned NULL"); }
+  for (auto &e : f->ev) CU(cudaEventCreate(&e));
+
+  TreeFrame *trees_d = (TreeFrame *)f->trees_d.p;
+  unsigned long long *counters = (unsigned long long *)f->counters.p;
+  CU(cudaMemcpyAsync(trees_d, f->trees_h.data(), sizeof(TreeFrame) * p.n_trees, cudaMemcpyHostToDevice, st));
+  CU(cudaMemsetAsync(counters, 0, sizeof(unsigned long long) * CNT_N, st));
+  // ---- step 1
+  CU(cudaEventRecord(f->ev[0], st));
+  dvx_tree_setup_launch(p, trees_d, st);
+  dvx_tile_masks_launch(p, trees_d, (uint8_t *)f->octmask.p, (unsigned long long *)f->actor_mask.p, st);
+  dvx_preprocess_launch(p, trees_d, (const uint8_t *)f->octmask.p, (FrameVox *)f->fvox.p, (ushort4 *)f->pxrect.p, counters, st);
+  CU(cudaEventRecord(f->ev[1], st));
+  CU(cudaMemcpyAsync(ctx->h_counters, counters, sizeof(unsigned long long) * CNT_N, cudaMemcpyDeviceToHost, st));
+  CU(cudaStreamSynchronize(st));
+  f->n_pairs = ctx->h_counters[CNT_PAIRS];
+  f->v_vis = ctx->h_counters[CNT_VVIS];
+  if (f->n_pairs >= 0xFFFFFFFFull) { frame_free(ctx, f); return fail(ctx, DVX_ERR_INVALID_ARG, "more than 2^32-2 (tile, voxel) pairs"); }
+  // ---- step 2
+  const uint64_t P = f->n_pairs;
+  uint64_t *ka = (uint64_t *)ctx_alloc(ctx, P * 8), *kb = (uint64_t *)ctx_alloc(ctx, P * 8);
+  uint32_t *va = (uint32_t *)ctx_alloc(ctx, P * 4), *vb = (uint32_t *)ctx_alloc(ctx, P * 4);
+  void *scr = ctx_alloc(ctx, dvx_sort_scratch_bytes(P));
+  if (!ka || !kb || !va || !vb || !scr) {
+    ctx_release(ctx, ka); ctx_release(ctx, kb); ctx_release(ctx, va); ctx_release(ctx, vb); ctx_release(ctx, scr);
+    frame_free(ctx, f);
+    return fail(ctx, DVX_ERR_OOM, "dvx_render: allocator returned NULL");
+  }
+  CU(cudaEventRecord(f->ev[2], st));
+  dvx_emit_pairs_launch(p, trees_d, (const uint8_t *)f->octmask.p, (const ushort4 *)f->pxrect.p, ka, va, P, counters, st);
+  int which = dvx_sort_launch(ka, va, kb, vb, P, key_bits, scr, st);
+  CU(cudaMemsetAsync(f->range_beg.p, 0, sizeof(uint32_t) * (size_t)p.n_buckets, st));
+  CU(cudaMemsetAsync(f->range_end.p, 0, sizeof(uint32_t) * (size_t)p.n_buckets, st));
+  dvx_ranges_launch(which ? kb : ka, P, p.rank_bits, (uint32_t *)f->range_beg.p, (uint32_t *)f->range_end.p, st);
+  CU(cudaEventRecord(f->ev[3], st));
+  f->ids.p = which ? vb : va;
+  f->ids.bytes = P * 4;
+  ctx_release(ctx, ka); ctx_release(ctx, kb); ctx_release(ctx, which ? va : vb); ctx_release(ctx, scr);
+  // ---- steps 3 + 4
+  CompositeArgs A;
+  memset(&A, 0, sizeof(A));
+  A.p = p; A.trees = trees_d; A.fvox = (const FrameVox *)f->fvox.p; A.pxrect = (const ushort4 *)f->pxrect.p;
+  A.ids = (const uint32_t *)f->ids.p; A.range_beg = (const uint32_t *)f->range_beg.p; A.range_end = (const uint32_t *)f->range_end.p;
+  A.actor_mask = (const unsigned long long *)f->actor_mask.p;
+  A.rgb = out.rgb; A.depth = out.depth; A.alpha = out.alpha;
+  A.sv_rgbd = (float *)f->sv_rgbd.p; A.sv_T = (float *)f->sv_T.p; A.sv_nused = (uint32_t *)f->sv_nused.p;
+  A.counters = counters;
+  dvx_composite_launch(A, false, st);
+  CU(cudaEventRecord(f->ev[4], st));
+  CU(cudaGetLastError());
+  if (saved) *saved = f;
+  else frame_free(ctx, f);
+  return DVX_OK;
+}
+
+dvx_status dvx_backward(dvx_ctx *ctx, dvx_frame *f, const float *dL_drgb, const float *dL_ddepth, const float *dL_dalpha,
+                        dvx_grad static_grad, const dvx_grad *actor_grads) {
+  if (!ctx) return DVX_ERR_INVALID_ARG;
+  if (!f || !dL_drgb) return fail(ctx, DVX_ERR_INVALID_ARG, "NULL argument");
+  if (!f->sv_rgbd.p) return fail(ctx, DVX_ERR_INVALID_ARG, "frame holds no saved state");
+  const FrameParams &p = f->p;
+  if (p.n_trees > 1 && !actor_grads) return fail(ctx, DVX_ERR_INVALID_ARG, "actor_grads is NULL");
+  cudaSetDevice(ctx->device);
+  cudaStream_t st = ctx->st;
+  for (uint32_t t = 0; t < p.n_trees; ++t) {
+    const dvx_grad g = t == 0 ? static_grad : actor_grads[t - 1];
+    f->trees_h[t].dgeo = g.dgeo;
+    f->trees_h[t].dsh = g.dsh;
+  }
+  float *drgb = (float *)ctx_alloc(ctx, (size_t)p.v_total * 16);
+  if (!drgb) return fail(ctx, DVX_ERR_OOM, "dvx_backward: allocator returned NULL");
+  TreeFrame *trees_d = (TreeFrame *)f->trees_d.p;
+  // box_rect was filled on the device; only the gradient pointers change, so patch those fields
+  for (uint32_t t = 0; t < p.n_trees; ++t)
+    CU(cudaMemcpyAsync((char *)(trees_d + t) + offsetof(TreeFrame, dgeo), &f->trees_h[t].dgeo, 2 * sizeof(float *),
+                       cudaMemcpyHostToDevice, st));
+  CU(cudaEventRecord(f->ev[5], st));
+  CU(cudaMemsetAsync(drgb, 0, (size_t)p.v_total * 16, st));
+  CompositeArgs A;
+  memset(&A, 0, sizeof(A));
+  A.p = p; A.trees = trees_d; A.fvox = (const FrameVox *)f->fvox.p; A.pxrect = (const ushort4 *)f->pxrect.p;
+  A.ids = (const uint32_t *)f->ids.p; A.range_beg = (const uint32_t *)f->range_beg.p; A.range_end = (const uint32_t *)f->range_end.p;
+  A.actor_mask = (const unsigned long long *)f->actor_mask.p;
+  A.sv_rgbd = (float *)f->sv_rgbd.p; A.sv_T = (float *)f->sv_T.p; A.sv_nused = (uint32_t *)f->sv_nused.p;
+  A.counters = (unsigned long long *)f->counters.p;
+  A.g_rgb = dL_drgb; A.g_depth = dL_ddepth; A.g_alpha = dL_dalpha; A.drgb = drgb;
+  dvx_composite_launch(A, true, st);
+  dvx_sh_backward_launch(p, trees_d, A.fvox, A.pxrect, drgb, st);
+  CU(cudaEventRecord(f->ev[6], st));
+  CU(cudaGetLastError());
+  ctx_release(ctx, drgb);
+  f->did_backward = true;
+  return DVX_OK;
+}
+
+void dvx_frame_release(dvx_ctx *ctx, dvx_frame *frame) {
+  if (ctx && frame) frame_free(ctx, frame);
+}
+
+dvx_status dvx_debug_tile_list(dvx_ctx *ctx, const dvx_frame *f, uint32_t tile, uint32_t octree, uint32_t octant,
+                               uint32_t *ids_host, uint32_t capacity, uint32_t *n_out) {
+  if (!ctx) return DVX_ERR_INVALID_ARG;
+  if (!f || !n_out || (capacity && !ids_host)) return fail(ctx, DVX_ERR_INVALID_ARG, "NULL argument");
+  if (tile >= f->p.n_tiles || octree >= f->p.n_trees || octant >= 8) return fail(ctx, DVX_ERR_INVALID_ARG, "index out of range");
+  cudaSetDevice(ctx->device);
+  size_t b = ((size_t)tile * f->p.n_trees + octree) * 8 + octant;
+  uint32_t be[2];
+  CU(cudaMemcpyAsync(&be[0], (const uint32_t *)f->range_beg.p + b, 4, cudaMemcpyDeviceToHost, ctx->st));
+  CU(cudaMemcpyAsync(&be[1], (const uint32_t *)f->range_end.p + b, 4, cudaMemcpyDeviceToHost, ctx->st));
+  CU(cudaStreamSynchronize(ctx->st));
+  uint32_t n = be[1] - be[0];
+  *n_out = n;
+  uint32_t m = n < capacity ? n : capacity;
+  if (m) {
+    CU(cudaMemcpyAsync(ids_host, (const uint32_t *)f->ids.p + be[0], (size_t)m * 4, cudaMemcpyDeviceToHost, ctx->st));
+    CU(cudaStreamSynchronize(ctx->st));
+    for (uint32_t i = 0; i < m; ++i) ids_host[i] -= f->trees_h[octree].base;
+  }
+  return DVX_OK;
+}
+
+dvx_status dvx_frame_counters(dvx_ctx *ctx, const dvx_frame *f, uint64_t *v_vis, uint64_t *pairs, uint64_t *pairs_eff,
+                              uint64_t *q_test, uint64_t *q_hit) {
+  if (!ctx) return DVX_ERR_INVALID_ARG;
+  if (!f) return fail(ctx, DVX_ERR_INVALID_ARG, "NULL argument");
+  cudaSetDevice(ctx->device);
+  unsigned long long h[CNT_N];
+  CU(cudaMemcpyAsync(h, f->counters.p, sizeof(h), cudaMemcpyDeviceToHost, ctx->st));
+  CU(cudaStreamSynchronize(ctx->st));
+  if (v_vis) *v_vis = h[CNT_VVIS];
+  if (pairs) *pairs = h[CNT_PAIRS];
+  if (pairs_eff) *pairs_eff = h[CNT_PAIRS_EFF];
+  if (q_test) *q_test = h[CNT_QTEST];
+  if (q_hit) *q_hit = h[CNT_QHIT];
+  return DVX_OK;
+}
+
+dvx_status dvx_frame_stage_ms(dvx_ctx *ctx, const dvx_frame *f, float *ms) {
+  if (!ctx) return DVX_ERR_INVALID_ARG;
+  if (!f || !ms) return fail(ctx, DVX_ERR_INVALID_ARG, "NULL argument");
+  cudaSetDevice(ctx->device);
+  CU(cudaStreamSynchronize(ctx->st));
+  ms[0] = ms[1] = ms[2] = ms[3] = 0.f;
+  CU(cudaEventElapsedTime(&ms[0], f->ev[0], f->ev[1]));
+  CU(cudaEventElapsedTime(&ms[1], f->ev[2], f->ev[3]));
+  CU(cudaEventElapsedTime(&ms[2], f->ev[3], f->ev[4]));
+  if (f->did_backward) CU(cudaEventElapsedTime(&ms[3], f->ev[5], f->ev[6]));
+  return DVX_OK;
+}
+
+dvx_status dvx_sort_pairs(dvx_ctx *ctx, uint64_t *keys, uint32_t *vals, uint64_t n, uint32_t key_bits) {
+  if (!ctx) return DVX_ERR_INVALID_ARG;
+  if (n && (!keys || !vals)) return fail(ctx, DVX_ERR_INVALID_ARG, "NULL argument");
+  if (key_bits < 1 || key_bits > 64 || n >= 0xFFFFFFFFull) return fail(ctx, DVX_ERR_INVALID_ARG, "key_bits must be in [1,64], n < 2^32-1");
+  if (n == 0) return DVX_OK;
+  cudaSetDevice(ctx->device);
+  uint64_t *kb = (uint64_t *)ctx_alloc(ctx, n * 8);
+  uint32_t *vb = (uint32_t *)ctx_alloc(ctx, n * 4);
+  void *scr = ctx_alloc(ctx, dvx_sort_scratch_bytes(n));
+  dvx_status rc = DVX_OK;
+  if (!kb || !vb || !scr) rc = fail(ctx, DVX_ERR_OOM, "dvx_sort_pairs: allocator returned NULL");
+  else {
+    int which = dvx_sort_launch(keys, vals, kb, vb, n, key_bits, scr, ctx->st);
+    if (which) {
+      cudaMemcpyAsync(keys, kb, n * 8, cudaMemcpyDeviceToDevice, ctx->st);
+      cudaMemcpyAsync(vals, vb, n * 4, cudaMemcpyDeviceToDevice, ctx->st);
+    }
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) rc = cuda_fail(ctx, e, "dvx_sort_pairs");
+  }
+  ctx_release(ctx, kb); ctx_release(ctx, vb); ctx_release(ctx, scr);
+  return rc;
+}
+
+}  // extern "C"

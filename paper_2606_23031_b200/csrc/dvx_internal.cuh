@@ -1,0 +1,93 @@
+// dvx_internal.cuh - structures and launch prototypes shared by the translation units of libdvx.
+// Nothing here is visible through include/dvx.h.  Notation follows the paper and DESIGN.md.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include "../../include/dvx.h"
+
+#define DVX_MAX_TREES (DVX_MAX_ACTORS + 1)
+
+// One octree as the kernels of one frame see it (device array of n_trees entries; [0] = static O_bg).
+struct TreeFrame {
+  const uint64_t *code;  // [V]        R14a
+  const float *geo;      // [V][8]     raw corner densities v_geo
+  const float *sh;       // [V][n_sh][3]
+  const uint32_t *rank;  // [8][V]     step-0 tables: rank of voxel v under octant q at rank[q*V + v]
+  float *dgeo;           // backward only
+  float *dsh;            // backward only
+  uint32_t n_voxels, n_sh, base, is_actor;  // base = first global voxel id of this tree
+  double lo[3];          // cube min corner w_c - w_s/2 (tree frame)
+  double cell;           // w_s / 2^16 : edge of a level-16 cell
+  double o_l[3];         // camera origin in the tree frame: R_o^T (o_c - t_o)
+  float ol_f[3];         // the same rounded to fp32 (ray-OBB test only)
+  float N[9];            // R_o^T R_c: d_l[a] = N[3a] x' + N[3a+1] y' + N[3a+2];  p_cam[c] = sum_a N[3a+c] rel[a]
+  float half[3];         // OBB half extents (actors)
+  int box_rect[4];       // pixel rectangle of the OBB (x0,y0,x1,y1 inclusive; x1<x0 = not visible); set on device
+};
+
+struct FrameParams {
+  uint32_t width, height, tiles_x, tiles_y, n_tiles, n_trees;
+  float fx, fy, cx, cy, near_, far_, zclip;
+  uint32_t k_samples, activation, flags;
+  float t_stop;
+  uint32_t rank_bits;   // sort key = (bucket << rank_bits) | rank ; bucket = (tile*n_trees + tree)*8 + octant
+  uint32_t v_total;     // sum of n_voxels
+  uint32_t n_buckets;   // n_tiles * n_trees * 8
+};
+
+// Per visible voxel, per frame (32 bytes, indexed by global voxel id).
+struct __align__(16) FrameVox {
+  float rel[3];   // voxel min corner minus camera origin, tree frame (computed in fp64, rounded once)
+  float s;        // voxel edge length
+  float rgb[3];   // max(0, 1/2 + sum_i Y_i(dir_v) k_i)  (R8)
+  uint32_t meta;  // bits 0-2: colour channel clamped at 0 (gradient blocked)
+};
+
+enum { CNT_PAIRS = 0, CNT_VVIS = 1, CNT_QTEST = 2, CNT_QHIT = 3, CNT_PAIRS_EFF = 4, CNT_OVERFLOW = 5, CNT_EMIT = 6, CNT_N = 8 };
+
+struct CompositeArgs {
+  FrameParams p;
+  const TreeFrame *trees;
+  const FrameVox *fvox;
+  const ushort4 *pxrect;       // [v_total] pixel rectangle of each voxel (x0,y0,x1,y1 inclusive)
+  const uint32_t *ids;         // [P] sorted global voxel ids
+  const uint32_t *range_beg;   // [n_buckets]
+  const uint32_t *range_end;   // [n_buckets]
+  const unsigned long long *actor_mask;  // [n_tiles]
+  float *rgb, *depth, *alpha;  // caller's images
+  float *sv_rgbd;              // [H*W][4] saved C_final, D_final (frame-owned; may be NULL when nothing is saved)
+  float *sv_T;                 // [H*W]
+  uint32_t *sv_nused;          // [H*W]
+  unsigned long long *counters;
+  // backward
+  const float *g_rgb, *g_depth, *g_alpha;
+  float *drgb;                 // [v_total][4] scratch: dL/drgb_v
+};
+
+// ---- dvx_sort.cu
+size_t dvx_sort_scratch_bytes(uint64_t n);
+// Sorts by bits [0,key_bits) ascending, stable.  Result lands in keys_a/vals_a or keys_b/vals_b; returns 0 or 1 (which).
+int dvx_sort_launch(uint64_t *keys_a, uint32_t *vals_a, uint64_t *keys_b, uint32_t *vals_b, uint64_t n, uint32_t key_bits,
+                    void *scratch, cudaStream_t st);
+void dvx_scan_u32_launch(uint32_t *data, uint64_t n, uint32_t *scratch, cudaStream_t st);  // exclusive, in place
+
+// ---- dvx_preprocess.cu
+void dvx_rank_keys_launch(const uint64_t *code, uint32_t n, int q, uint64_t *keys, uint32_t *vals, cudaStream_t st);
+void dvx_rank_scatter_launch(const uint32_t *perm, uint32_t n, uint32_t *rank, cudaStream_t st);
+void dvx_validate_launch(const uint64_t *code_sorted_keys, const uint32_t *perm, const uint64_t *code, uint32_t n,
+                         uint32_t *bad_flag, cudaStream_t st);
+void dvx_tree_setup_launch(const FrameParams &p, TreeFrame *trees, cudaStream_t st);
+void dvx_tile_masks_launch(const FrameParams &p, const TreeFrame *trees, uint8_t *octmask, unsigned long long *actor_mask,
+                           cudaStream_t st);
+void dvx_preprocess_launch(const FrameParams &p, const TreeFrame *trees, const uint8_t *octmask, FrameVox *fvox,
+                           ushort4 *pxrect, unsigned long long *counters, cudaStream_t st);
+void dvx_emit_pairs_launch(const FrameParams &p, const TreeFrame *trees, const uint8_t *octmask, const ushort4 *pxrect,
+                           uint64_t *keys, uint32_t *vals, unsigned long long capacity, unsigned long long *counters,
+                           cudaStream_t st);
+void dvx_ranges_launch(const uint64_t *keys, uint64_t n, uint32_t rank_bits, uint32_t *range_beg, uint32_t *range_end,
+                       cudaStream_t st);
+void dvx_sh_backward_launch(const FrameParams &p, const TreeFrame *trees, const FrameVox *fvox, const ushort4 *pxrect,
+                            const float *drgb, cudaStream_t st);
+
+// ---- dvx_composite.cu
+void dvx_composite_launch(const CompositeArgs &a, bool backward, cudaStream_t st);

@@ -1,0 +1,356 @@
+// dvx_preprocess.cu - hot-path steps 0, 1 and the non-sort parts of step 2:
+//   step 0  per-octree, per-octant rank tables under the key morton48 XOR q*0x249249249249 (R14b)
+//   step 1  per-voxel projection under the octree's rigid transform, pixel/tile rectangle, frustum + OBB cull,
+//           per-voxel view-dependent colour (R8)
+//   step 2  (tile, octant, voxel) key generation and per-bucket ranges (the radix sort itself is dvx_sort.cu)
+//   step 5b per-voxel SH post-pass of the backward
+#include "dvx_device.cuh"
+
+namespace {
+
+constexpr int PRE_THREADS = 256;
+
+__device__ __forceinline__ int find_tree(const uint32_t *s_base, int n_trees, uint32_t g) {
+  int t = 0;
+  while (t + 1 < n_trees && g >= s_base[t + 1]) ++t;
+  return t;
+}
+
+// ------------------------------------------------------------------ step 0
+__global__ void rank_keys_kernel(const uint64_t *code, uint32_t n, uint64_t flip, uint64_t *keys, uint32_t *vals) {
+  uint32_t v = blockIdx.x * blockDim.x + threadIdx.x;
+  if (v >= n) return;
+  keys[v] = (code[v] & 0xFFFFFFFFFFFFull) ^ flip;
+  vals[v] = v;
+}
+__global__ void rank_scatter_kernel(const uint32_t *perm, uint32_t n, uint32_t *rank) {
+  uint32_t r = blockIdx.x * blockDim.x + threadIdx.x;
+  if (r < n) rank[perm[r]] = r;
+}
+// Leaf-set validation on the q = 0 order: level in [1,16], bits below the level zero, no leaf equal to or nested in
+// its successor (ancestors sort immediately before their descendants because of the zero padding).
+__global__ void validate_kernel(const uint64_t *skeys, const uint32_t *perm, const uint64_t *code, uint32_t n,
+                                uint32_t *bad) {
+  uint32_t r = blockIdx.x * blockDim.x + threadIdx.x;
+  if (r >= n) return;
+  uint64_t c = code[perm[r]];
+  uint32_t l = (uint32_t)(c >> 48) & 31u;
+  bool ok = (c >> 53) == 0 && l >= 1 && l <= DVX_MAX_LEVEL;
+  if (ok) {
+    uint32_t sh = 3u * (DVX_MAX_LEVEL - l);
+    uint64_t path = c & 0xFFFFFFFFFFFFull;
+    if (sh && (path & ((1ull << sh) - 1ull))) ok = false;
+    if (ok && r + 1 < n && ((skeys[r + 1] >> sh) == (path >> sh))) ok = false;  // duplicate or descendant follows
+  }
+  if (!ok) atomicOr(bad, 1u);
+}
+
+// ------------------------------------------------------------------ per-frame set-up
+// One thread per tree: pixel rectangle of the actor's oriented box.
+__global__ void tree_setup_kernel(FrameParams p, TreeFrame *trees) {
+  int t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= (int)p.n_trees) return;
+  TreeFrame &T = trees[t];
+  if (!T.is_actor) {
+    T.box_rect[0] = 0; T.box_rect[1] = 0; T.box_rect[2] = (int)p.width - 1; T.box_rect[3] = (int)p.height - 1;
+    return;
+  }
+  float pc[8][3];
+  for (int c = 0; c < 8; ++c) {
+    float rel[3];
+    for (int a = 0; a < 3; ++a) {
+      double x = ((c >> (2 - a)) & 1) ? (double)T.half[a] : -(double)T.half[a];
+      rel[a] = (float)(x - T.o_l[a]);
+    }
+    for (int cc = 0; cc < 3; ++cc) pc[c][cc] = T.N[cc] * rel[0] + T.N[3 + cc] * rel[1] + T.N[6 + cc] * rel[2];
+  }
+  int x0, y0, x1, y1;
+  if (dvx_pixel_rect(pc, p, x0, y0, x1, y1)) {
+    T.box_rect[0] = x0; T.box_rect[1] = y0; T.box_rect[2] = x1; T.box_rect[3] = y1;
+  } else {
+    T.box_rect[0] = 1; T.box_rect[1] = 1; T.box_rect[2] = 0; T.box_rect[3] = 0;
+  }
+}
+
+// One thread per tile: for every tree the set of ray-direction octants present among the tile's pixels (R12), and the
+// 64-bit mask of actors whose box footprint touches the tile.
+__global__ void tile_masks_kernel(FrameParams p, const TreeFrame *trees, uint8_t *octmask, unsigned long long *actor_mask) {
+  int tile = blockIdx.x * blockDim.x + threadIdx.x;
+  if (tile >= (int)p.n_tiles) return;
+  int tx = tile % p.tiles_x, ty = tile / p.tiles_x;
+  int u0 = tx * DVX_TILE, v0 = ty * DVX_TILE;
+  int u1 = min(u0 + DVX_TILE, (int)p.width) - 1, v1 = min(v0 + DVX_TILE, (int)p.height) - 1;
+  float xs[2] = {dvx_cam_x(p, u0), dvx_cam_x(p, u1)}, ys[2] = {dvx_cam_y(p, v0), dvx_cam_y(p, v1)};
+  unsigned long long am = 0;
+  for (int t = 0; t < (int)p.n_trees; ++t) {
+    const TreeFrame &T = trees[t];
+    uint8_t m = 0;
+    bool overlap = T.box_rect[2] >= u0 && T.box_rect[0] <= u1 && T.box_rect[3] >= v0 && T.box_rect[1] <= v1;
+    if (overlap) {
+      int sset[3];  // bit 0: some pixel has s_a = 0 (d_a >= 0); bit 1: some pixel has s_a = 1
+      for (int a = 0; a < 3; ++a) {
+        int s = 0;
+        for (int i = 0; i < 2; ++i)
+          for (int j = 0; j < 2; ++j) s |= (dvx_dir_comp(T.N, a, xs[i], ys[j]) < 0.f) ? 2 : 1;
+        sset[a] = s;
+      }
+      for (int q = 0; q < 8; ++q) {
+        int sx = (q >> 2) & 1, sy = (q >> 1) & 1, sz = q & 1;
+        if (((sset[0] >> sx) & 1) && ((sset[1] >> sy) & 1) && ((sset[2] >> sz) & 1)) m |= (uint8_t)(1u << q);
+      }
+      if (T.is_actor) am |= 1ull << (t - 1);
+    }
+    octmask[(size_t)tile * p.n_trees + t] = m;
+  }
+  actor_mask[tile] = am;
+}
+
+// ------------------------------------------------------------------ step 1
+__device__ __forceinline__ bool voxel_rect(const FrameParams &p, const TreeFrame &T, uint64_t code, float rel_out[3],
+                                           float &s_out, int &x0, int &y0, int &x1, int &y1) {
+  uint32_t X, Y, Z, l;
+  dvx_decode16(code, X, Y, Z, l);
+  const double s = T.cell * (double)(1u << (DVX_MAX_LEVEL - l));
+  double mn[3] = {T.lo[0] + T.cell * (double)X, T.lo[1] + T.cell * (double)Y, T.lo[2] + T.cell * (double)Z};
+  double bmn[3], bmx[3];
+#pragma unroll
+  for (int a = 0; a < 3; ++a) {
+    rel_out[a] = (float)(mn[a] - T.o_l[a]);
+    bmn[a] = mn[a];
+    bmx[a] = mn[a] + s;
+    if (T.is_actor) {  // actor voxels only matter inside the box (R18)
+      bmn[a] = fmax(bmn[a], -(double)T.half[a]);
+      bmx[a] = fmin(bmx[a], (double)T.half[a]);
+    }
+  }
+  s_out = (float)s;
+  if (!(bmx[0] >= bmn[0]) || !(bmx[1] >= bmn[1]) || !(bmx[2] >= bmn[2])) return false;
+  float pc[8][3];
+#pragma unroll
+  for (int c = 0; c < 8; ++c) {
+    float r0 = (float)(((c & 4) ? bmx[0] : bmn[0]) - T.o_l[0]);
+    float r1 = (float)(((c & 2) ? bmx[1] : bmn[1]) - T.o_l[1]);
+    float r2 = (float)(((c & 1) ? bmx[2] : bmn[2]) - T.o_l[2]);
+#pragma unroll
+    for (int cc = 0; cc < 3; ++cc) pc[c][cc] = T.N[cc] * r0 + T.N[3 + cc] * r1 + T.N[6 + cc] * r2;
+  }
+  return dvx_pixel_rect(pc, p, x0, y0, x1, y1);
+}
+
+__device__ __forceinline__ uint32_t count_pairs(const FrameParams &p, const uint8_t *octmask, int t, int x0, int y0,
+                                                int x1, int y1) {
+  uint32_t n = 0;
+  for (int ty = y0 >> 4; ty <= (y1 >> 4); ++ty)
+    for (int tx = x0 >> 4; tx <= (x1 >> 4); ++tx)
+      n += __popc((uint32_t)octmask[(size_t)(ty * p.tiles_x + tx) * p.n_trees + t]);
+  return n;
+}
+
+__global__ void __launch_bounds__(PRE_THREADS) preprocess_kernel(FrameParams p, const TreeFrame *trees,
+                                                                 const uint8_t *octmask, FrameVox *fvox,
+                                                                 ushort4 *pxrect, unsigned long long *counters) {
+  __shared__ uint32_t s_base[DVX_MAX_TREES + 1];
+  for (int i = threadIdx.x; i < (int)p.n_trees; i += blockDim.x) s_base[i] = trees[i].base;
+  __syncthreads();
+  uint32_t g = blockIdx.x * blockDim.x + threadIdx.x;
+  uint32_t npairs = 0, vis = 0;
+  if (g < p.v_total) {
+    int t = find_tree(s_base, p.n_trees, g);
+    const TreeFrame &T = trees[t];
+    uint32_t v = g - s_base[t];
+    float rel[3], s;
+    int x0, y0, x1, y1;
+    bool ok = voxel_rect(p, T, T.code[v], rel, s, x0, y0, x1, y1);
+    if (ok) npairs = count_pairs(p, octmask, t, x0, y0, x1, y1);
+    if (npairs == 0) {
+      pxrect[g] = make_ushort4(0xFFFF, 0xFFFF, 0, 0);
+    } else {
+      vis = 1;
+      pxrect[g] = make_ushort4((unsigned short)x0, (unsigned short)y0, (unsigned short)x1, (unsigned short)y1);
+      // O7 / R8: one colour per voxel per camera, direction camera origin -> voxel centre in the tree's frame
+      float dx = rel[0] + 0.5f * s, dy = rel[1] + 0.5f * s, dz = rel[2] + 0.5f * s;
+      float inv = rsqrtf(dx * dx + dy * dy + dz * dz);
+      float Y[16];
+      dvx_sh_basis(dx * inv, dy * inv, dz * inv, Y, (int)T.n_sh);
+      float acc[3] = {0.5f, 0.5f, 0.5f};
+      const float *k = T.sh + (size_t)v * T.n_sh * 3;
+      if (T.n_sh == 16) {
+        const float4 *k4 = reinterpret_cast<const float4 *>(k);
+        float kk[48];
+#pragma unroll
+        for (int i = 0; i < 12; ++i) {
+          float4 q = __ldg(k4 + i);
+          kk[4 * i] = q.x; kk[4 * i + 1] = q.y; kk[4 * i + 2] = q.z; kk[4 * i + 3] = q.w;
+        }
+#pragma unroll
+        for (int i = 0; i < 16; ++i) {
+          acc[0] += Y[i] * kk[3 * i]; acc[1] += Y[i] * kk[3 * i + 1]; acc[2] += Y[i] * kk[3 * i + 2];
+        }
+      } else {
+        for (int i = 0; i < (int)T.n_sh; ++i) {
+          acc[0] += Y[i] * __ldg(k + 3 * i); acc[1] += Y[i] * __ldg(k + 3 * i + 1); acc[2] += Y[i] * __ldg(k + 3 * i + 2);
+        }
+      }
+      FrameVox fv;
+      fv.rel[0] = rel[0]; fv.rel[1] = rel[1]; fv.rel[2] = rel[2]; fv.s = s;
+      uint32_t meta = 0;
+#pragma unroll
+      for (int ch = 0; ch < 3; ++ch) {
+        if (!(acc[ch] > 0.f)) { meta |= 1u << ch; acc[ch] = 0.f; }
+        fv.rgb[ch] = acc[ch];
+      }
+      fv.meta = meta;
+      fvox[g] = fv;
+    }
+  }
+  // warp-aggregated totals
+  for (int o = 16; o > 0; o >>= 1) {
+    npairs += __shfl_xor_sync(0xffffffffu, npairs, o);
+    vis += __shfl_xor_sync(0xffffffffu, vis, o);
+  }
+  if ((threadIdx.x & 31) == 0 && (npairs | vis)) {
+    atomicAdd(&counters[CNT_PAIRS], (unsigned long long)npairs);
+    atomicAdd(&counters[CNT_VVIS], (unsigned long long)vis);
+  }
+}
+
+// ------------------------------------------------------------------ step 2: key generation
+// key = (bucket << rank_bits) | rank_q(v), bucket = (tile*n_trees + tree)*8 + q; value = global voxel id.
+// Every key is unique, so the order in which pairs are emitted does not matter: slots are handed out with one
+// warp-aggregated atomic per warp.
+__global__ void __launch_bounds__(PRE_THREADS) emit_pairs_kernel(FrameParams p, const TreeFrame *trees,
+                                                                 const uint8_t *octmask, const ushort4 *pxrect,
+                                                                 uint64_t *keys, uint32_t *vals,
+                                                                 unsigned long long capacity,
+                                                                 unsigned long long *counters) {
+  __shared__ uint32_t s_base[DVX_MAX_TREES + 1];
+  for (int i = threadIdx.x; i < (int)p.n_trees; i += blockDim.x) s_base[i] = trees[i].base;
+  __syncthreads();
+  uint32_t g = blockIdx.x * blockDim.x + threadIdx.x;
+  const int lane = threadIdx.x & 31;
+  uint32_t n = 0;
+  int t = 0;
+  ushort4 r = make_ushort4(0xFFFF, 0xFFFF, 0, 0);
+  if (g < p.v_total) {
+    r = pxrect[g];
+    if (r.x <= r.z) {
+      t = find_tree(s_base, p.n_trees, g);
+      n = count_pairs(p, octmask, t, r.x, r.y, r.z, r.w);
+    }
+  }
+  // warp exclusive scan of n, one atomic for the warp
+  uint32_t inc = n;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    uint32_t x = __shfl_up_sync(0xffffffffu, inc, o);
+    if (lane >= o) inc += x;
+  }
+  uint32_t total = __shfl_sync(0xffffffffu, inc, 31);
+  unsigned long long wbase = 0;
+  if (lane == 31 && total) wbase = atomicAdd(&counters[CNT_EMIT], (unsigned long long)total);
+  wbase = __shfl_sync(0xffffffffu, wbase, 31);
+  if (n == 0) return;
+  unsigned long long pos = wbase + (inc - n);
+  if (pos + n > capacity) {
+    atomicOr((unsigned int *)&counters[CNT_OVERFLOW], 1u);
+    return;
+  }
+  const TreeFrame &T = trees[t];
+  const uint32_t v = g - s_base[t];
+  for (int ty = r.y >> 4; ty <= (r.w >> 4); ++ty)
+    for (int tx = r.x >> 4; tx <= (r.z >> 4); ++tx) {
+      uint32_t tile = ty * p.tiles_x + tx;
+      uint32_t m = octmask[(size_t)tile * p.n_trees + t];
+      while (m) {
+        int q = __ffs(m) - 1;
+        m &= m - 1;
+        uint64_t bucket = ((uint64_t)tile * p.n_trees + t) * 8u + q;
+        keys[pos] = (bucket << p.rank_bits) | (uint64_t)__ldg(T.rank + (size_t)q * T.n_voxels + v);
+        vals[pos] = g;
+        ++pos;
+      }
+    }
+}
+
+// range[bucket] = [begin, end) in the sorted pair array, by boundary detection (buffers pre-zeroed: empty = [0,0))
+__global__ void ranges_kernel(const uint64_t *keys, uint64_t n, uint32_t rank_bits, uint32_t *range_beg,
+                              uint32_t *range_end) {
+  uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  uint64_t b = keys[i] >> rank_bits;
+  if (i == 0 || (keys[i - 1] >> rank_bits) != b) range_beg[b] = (uint32_t)i;
+  if (i + 1 == n || (keys[i + 1] >> rank_bits) != b) range_end[b] = (uint32_t)(i + 1);
+}
+
+// ------------------------------------------------------------------ step 5b: dL/dk_{v,i} = Y_i(dir_v) dL/drgb_v
+__global__ void __launch_bounds__(PRE_THREADS) sh_backward_kernel(FrameParams p, const TreeFrame *trees,
+                                                                  const FrameVox *fvox, const ushort4 *pxrect,
+                                                                  const float *drgb) {
+  __shared__ uint32_t s_base[DVX_MAX_TREES + 1];
+  for (int i = threadIdx.x; i < (int)p.n_trees; i += blockDim.x) s_base[i] = trees[i].base;
+  __syncthreads();
+  uint32_t g = blockIdx.x * blockDim.x + threadIdx.x;
+  if (g >= p.v_total) return;
+  ushort4 r = pxrect[g];
+  if (r.x > r.z) return;
+  float4 d = reinterpret_cast<const float4 *>(drgb)[g];
+  if (d.x == 0.f && d.y == 0.f && d.z == 0.f) return;
+  int t = find_tree(s_base, p.n_trees, g);
+  const TreeFrame &T = trees[t];
+  if (!T.dsh) return;
+  FrameVox fv = fvox[g];
+  float dx = fv.rel[0] + 0.5f * fv.s, dy = fv.rel[1] + 0.5f * fv.s, dz = fv.rel[2] + 0.5f * fv.s;
+  float inv = rsqrtf(dx * dx + dy * dy + dz * dz);
+  float Y[16];
+  dvx_sh_basis(dx * inv, dy * inv, dz * inv, Y, (int)T.n_sh);
+  float gch[3] = {(fv.meta & 1u) ? 0.f : d.x, (fv.meta & 2u) ? 0.f : d.y, (fv.meta & 4u) ? 0.f : d.z};
+  float *out = T.dsh + (size_t)(g - s_base[t]) * T.n_sh * 3;
+  for (int i = 0; i < (int)T.n_sh; ++i) {
+    out[3 * i] += Y[i] * gch[0];
+    out[3 * i + 1] += Y[i] * gch[1];
+    out[3 * i + 2] += Y[i] * gch[2];
+  }
+}
+
+inline unsigned blocks_for(uint64_t n, int threads) { return (unsigned)((n + threads - 1) / threads); }
+
+}  // namespace
+
+void dvx_rank_keys_launch(const uint64_t *code, uint32_t n, int q, uint64_t *keys, uint32_t *vals, cudaStream_t st) {
+  if (n) rank_keys_kernel<<<blocks_for(n, 256), 256, 0, st>>>(code, n, (uint64_t)q * 0x249249249249ull, keys, vals);
+}
+void dvx_rank_scatter_launch(const uint32_t *perm, uint32_t n, uint32_t *rank, cudaStream_t st) {
+  if (n) rank_scatter_kernel<<<blocks_for(n, 256), 256, 0, st>>>(perm, n, rank);
+}
+void dvx_validate_launch(const uint64_t *skeys, const uint32_t *perm, const uint64_t *code, uint32_t n,
+                         uint32_t *bad_flag, cudaStream_t st) {
+  if (n) validate_kernel<<<blocks_for(n, 256), 256, 0, st>>>(skeys, perm, code, n, bad_flag);
+}
+void dvx_tree_setup_launch(const FrameParams &p, TreeFrame *trees, cudaStream_t st) {
+  tree_setup_kernel<<<1, 128, 0, st>>>(p, trees);
+}
+void dvx_tile_masks_launch(const FrameParams &p, const TreeFrame *trees, uint8_t *octmask, unsigned long long *actor_mask,
+                           cudaStream_t st) {
+  tile_masks_kernel<<<blocks_for(p.n_tiles, 128), 128, 0, st>>>(p, trees, octmask, actor_mask);
+}
+void dvx_preprocess_launch(const FrameParams &p, const TreeFrame *trees, const uint8_t *octmask, FrameVox *fvox,
+                           ushort4 *pxrect, unsigned long long *counters, cudaStream_t st) {
+  if (p.v_total)
+    preprocess_kernel<<<blocks_for(p.v_total, PRE_THREADS), PRE_THREADS, 0, st>>>(p, trees, octmask, fvox, pxrect, counters);
+}
+void dvx_emit_pairs_launch(const FrameParams &p, const TreeFrame *trees, const uint8_t *octmask, const ushort4 *pxrect,
+                           uint64_t *keys, uint32_t *vals, unsigned long long capacity, unsigned long long *counters,
+                           cudaStream_t st) {
+  if (p.v_total)
+    emit_pairs_kernel<<<blocks_for(p.v_total, PRE_THREADS), PRE_THREADS, 0, st>>>(p, trees, octmask, pxrect, keys, vals,
+                                                                                   capacity, counters);
+}
+void dvx_ranges_launch(const uint64_t *keys, uint64_t n, uint32_t rank_bits, uint32_t *range_beg, uint32_t *range_end,
+                       cudaStream_t st) {
+  if (n) ranges_kernel<<<blocks_for(n, 256), 256, 0, st>>>(keys, n, rank_bits, range_beg, range_end);
+}
+void dvx_sh_backward_launch(const FrameParams &p, const TreeFrame *trees, const FrameVox *fvox, const ushort4 *pxrect,
+                            const float *drgb, cudaStream_t st) {
+  if (p.v_total)
+    sh_backward_kernel<<<blocks_for(p.v_total, PRE_THREADS), PRE_THREADS, 0, st>>>(p, trees, fvox, pxrect, drgb);
+}

@@ -1,0 +1,201 @@
+// dvx_sort.cu - hot-path step 2: LSD radix sort of (64-bit key, 32-bit value) pairs, plus the exclusive scan it needs.
+// "per-tile key generation and radix sort in direction-dependent Morton order" (BASELINE.json north_star (2));
+// the paper only says the traversal is "Morton-ordered".  HBM-bound: per 8-bit pass the keys are
+// read twice and written once (histogram kernel + scatter kernel), values read once and written once.
+#include "dvx_internal.cuh"
+
+namespace {
+
+constexpr int SORT_THREADS = 256;
+constexpr int SORT_ITEMS = 16;                         // keys per thread
+constexpr int SORT_TILE = SORT_THREADS * SORT_ITEMS;   // 4096 keys per block
+constexpr int SORT_WARPS = SORT_THREADS / 32;
+constexpr int RADIX = 256;
+
+constexpr int SCAN_THREADS = 512;
+constexpr int SCAN_ITEMS = 8;
+constexpr int SCAN_TILE = SCAN_THREADS * SCAN_ITEMS;   // 4096
+
+// ------------------------------------------------------------------ exclusive scan (reduce-then-scan, recursive)
+__device__ __forceinline__ uint32_t warp_incl_scan(uint32_t v) {
+  const int lane = threadIdx.x & 31;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    uint32_t t = __shfl_up_sync(0xffffffffu, v, o);
+    if (lane >= o) v += t;
+  }
+  return v;
+}
+
+// block-wide exclusive scan of one value per thread; returns the exclusive prefix, *total = block sum
+__device__ __forceinline__ uint32_t block_excl_scan(uint32_t v, uint32_t *total) {
+  __shared__ uint32_t wsum[32];
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = blockDim.x >> 5;
+  uint32_t inc = warp_incl_scan(v);
+  if (lane == 31) wsum[w] = inc;
+  __syncthreads();
+  if (w == 0) {
+    uint32_t s = lane < nw ? wsum[lane] : 0;
+    uint32_t si = warp_incl_scan(s);
+    wsum[lane] = si - s;
+    if (lane == 31) wsum[31] = si;  // nw <= 16 here, so slot 31 is free for the total
+  }
+  __syncthreads();
+  uint32_t r = wsum[w] + inc - v;
+  *total = wsum[31];
+  __syncthreads();
+  return r;
+}
+
+__global__ void scan_block_sums(const uint32_t *data, uint64_t n, uint32_t *sums) {
+  uint64_t base = (uint64_t)blockIdx.x * SCAN_TILE;
+  uint32_t s = 0;
+#pragma unroll
+  for (int i = 0; i < SCAN_ITEMS; ++i) {
+    uint64_t idx = base + (uint64_t)i * SCAN_THREADS + threadIdx.x;
+    if (idx < n) s += data[idx];
+  }
+  uint32_t total;
+  block_excl_scan(s, &total);
+  if (threadIdx.x == 0) sums[blockIdx.x] = total;
+}
+
+__global__ void scan_apply(uint32_t *data, uint64_t n, const uint32_t *block_off) {
+  uint64_t base = (uint64_t)blockIdx.x * SCAN_TILE + (uint64_t)threadIdx.x * SCAN_ITEMS;
+  uint32_t v[SCAN_ITEMS], s = 0;
+#pragma unroll
+  for (int i = 0; i < SCAN_ITEMS; ++i) {
+    v[i] = (base + i < n) ? data[base + i] : 0;
+    s += v[i];
+  }
+  uint32_t total;
+  uint32_t off = block_excl_scan(s, &total) + (block_off ? block_off[blockIdx.x] : 0);
+#pragma unroll
+  for (int i = 0; i < SCAN_ITEMS; ++i) {
+    if (base + i < n) data[base + i] = off;
+    off += v[i];
+  }
+}
+
+// ------------------------------------------------------------------ radix pass
+__global__ void __launch_bounds__(SORT_THREADS) radix_hist(const uint64_t *keys, uint64_t n, uint32_t shift,
+                                                            uint32_t *block_hist, uint32_t n_blocks) {
+  __shared__ uint32_t h[RADIX];
+  h[threadIdx.x] = 0;
+  __syncthreads();
+  uint64_t base = (uint64_t)blockIdx.x * SORT_TILE;
+#pragma unroll 4
+  for (int i = 0; i < SORT_ITEMS; ++i) {
+    uint64_t idx = base + (uint64_t)i * SORT_THREADS + threadIdx.x;
+    if (idx < n) atomicAdd(&h[(uint32_t)(keys[idx] >> shift) & (RADIX - 1)], 1u);
+  }
+  __syncthreads();
+  block_hist[(uint64_t)threadIdx.x * n_blocks + blockIdx.x] = h[threadIdx.x];  // digit-major for the scan
+}
+
+__global__ void __launch_bounds__(SORT_THREADS) radix_scatter(const uint64_t *__restrict__ keys_in,
+                                                               const uint32_t *__restrict__ vals_in,
+                                                               uint64_t *__restrict__ keys_out, uint32_t *__restrict__ vals_out,
+                                                               uint64_t n, uint32_t shift, const uint32_t *__restrict__ offs,
+                                                               uint32_t n_blocks) {
+  __shared__ uint32_t cnt[SORT_WARPS][RADIX];
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  for (int d = lane; d < RADIX; d += 32) cnt[w][d] = 0;
+  __syncwarp();
+  // warp w owns the contiguous keys [w*512, (w+1)*512) of the tile, in 16 steps of 32: order inside the tile is kept
+  const uint64_t wbase = (uint64_t)blockIdx.x * SORT_TILE + (uint64_t)w * (32 * SORT_ITEMS);
+  uint64_t key[SORT_ITEMS];
+  uint16_t rnk[SORT_ITEMS];
+#pragma unroll
+  for (int i = 0; i < SORT_ITEMS; ++i) {
+    uint64_t idx = wbase + (uint64_t)i * 32 + lane;
+    bool valid = idx < n;
+    key[i] = valid ? keys_in[idx] : 0;
+    uint32_t d = valid ? ((uint32_t)(key[i] >> shift) & (RADIX - 1)) : RADIX;  // RADIX = "no key"
+    uint32_t peers = __match_any_sync(0xffffffffu, d);
+    uint32_t before = __popc(peers & ((1u << lane) - 1u));
+    int leader = __ffs(peers) - 1;
+    uint32_t old = 0;
+    if (valid && lane == leader) {
+      old = cnt[w][d];
+      cnt[w][d] = old + __popc(peers);
+    }
+    old = __shfl_sync(0xffffffffu, old, leader);
+    rnk[i] = (uint16_t)(old + before);
+    __syncwarp();
+  }
+  __syncthreads();
+  {  // digit d = threadIdx.x: exclusive prefix over the warps, plus this block's global base for the digit
+    const int d = threadIdx.x;
+    uint32_t run = offs[(uint64_t)d * n_blocks + blockIdx.x];
+#pragma unroll
+    for (int ww = 0; ww < SORT_WARPS; ++ww) {
+      uint32_t c = cnt[ww][d];
+      cnt[ww][d] = run;
+      run += c;
+    }
+  }
+  __syncthreads();
+#pragma unroll
+  for (int i = 0; i < SORT_ITEMS; ++i) {
+    uint64_t idx = wbase + (uint64_t)i * 32 + lane;
+    if (idx < n) {
+      uint32_t d = (uint32_t)(key[i] >> shift) & (RADIX - 1);
+      uint32_t pos = cnt[w][d] + rnk[i];
+      keys_out[pos] = key[i];
+      vals_out[pos] = vals_in[idx];
+    }
+  }
+}
+
+inline uint64_t ceil_div(uint64_t a, uint64_t b) { return (a + b - 1) / b; }
+
+}  // namespace
+
+// scratch for a scan of n counters: the chain of block-sum levels
+static size_t scan_scratch_elems(uint64_t n) {
+  size_t tot = 0;
+  while (n > SCAN_TILE) {
+    n = ceil_div(n, SCAN_TILE);
+    tot += n;
+  }
+  return tot + 1;
+}
+
+void dvx_scan_u32_launch(uint32_t *data, uint64_t n, uint32_t *scratch, cudaStream_t st) {
+  if (n == 0) return;
+  uint64_t nb = ceil_div(n, SCAN_TILE);
+  if (nb == 1) {
+    scan_apply<<<1, SCAN_THREADS, 0, st>>>(data, n, nullptr);
+    return;
+  }
+  scan_block_sums<<<(unsigned)nb, SCAN_THREADS, 0, st>>>(data, n, scratch);
+  dvx_scan_u32_launch(scratch, nb, scratch + nb, st);
+  scan_apply<<<(unsigned)nb, SCAN_THREADS, 0, st>>>(data, n, scratch);
+}
+
+size_t dvx_sort_scratch_bytes(uint64_t n) {
+  uint64_t nb = ceil_div(n ? n : 1, SORT_TILE);
+  uint64_t hist = nb * RADIX;
+  return (hist + scan_scratch_elems(hist) + 64) * sizeof(uint32_t);
+}
+
+int dvx_sort_launch(uint64_t *keys_a, uint32_t *vals_a, uint64_t *keys_b, uint32_t *vals_b, uint64_t n, uint32_t key_bits,
+                    void *scratch, cudaStream_t st) {
+  if (n == 0) return 0;
+  uint32_t nb = (uint32_t)ceil_div(n, SORT_TILE);
+  uint32_t *hist = (uint32_t *)scratch;
+  uint32_t *scan_scr = hist + (uint64_t)nb * RADIX;
+  int passes = (int)((key_bits + 7) / 8);
+  if (passes < 1) passes = 1;
+  int cur = 0;
+  for (int p = 0; p < passes; ++p) {
+    uint64_t *kin = cur ? keys_b : keys_a, *kout = cur ? keys_a : keys_b;
+    uint32_t *vin = cur ? vals_b : vals_a, *vout = cur ? vals_a : vals_b;
+    radix_hist<<<nb, SORT_THREADS, 0, st>>>(kin, n, 8u * p, hist, nb);
+    dvx_scan_u32_launch(hist, (uint64_t)nb * RADIX, scan_scr, st);
+    radix_scatter<<<nb, SORT_THREADS, 0, st>>>(kin, vin, kout, vout, n, 8u * p, hist, nb);
+    cur ^= 1;
+  }
+  return cur;
+}

@@ -1,0 +1,115 @@
+"""GPU-vs-oracle parity through the C ABI (tolerances of BASELINE.json north_star, R16)."""
+import numpy as np
+import pytest
+
+import dvx_scenes as S
+from oracle import oracle as O
+
+pytestmark = pytest.mark.gpu
+
+RGB_TOL = 2e-4      # fp32 RGB / alpha: max abs error
+DEPTH_REL = 1e-4    # depth: |dD| <= 1e-4 * max(|D_ref|, 1 m)
+GRAD_REL, GRAD_ABS = 1e-3, 1e-6
+
+
+@pytest.fixture(scope="module")
+def ctx():
+    import paper_2606_23031_b200 as dvx
+    c = dvx.Context(0)
+    yield c
+    c.close()
+
+
+def _check_images(rgb, depth, alpha, ref, mask=None):
+    rgb, depth, alpha = rgb.cpu().numpy().astype(np.float64), depth.cpu().numpy().astype(np.float64), alpha.cpu().numpy().astype(np.float64)
+    m = np.ones(depth.shape, bool) if mask is None else mask.astype(bool)
+    e_rgb = np.abs(rgb - ref["rgb"])[m].max()
+    e_a = np.abs(alpha - ref["alpha"])[m].max()
+    e_d = (np.abs(depth - ref["depth"]) / np.maximum(np.abs(ref["depth"]), 1.0))[m].max()
+    assert e_rgb <= RGB_TOL, "rgb max abs error %g" % e_rgb
+    assert e_a <= RGB_TOL, "alpha max abs error %g" % e_a
+    assert e_d <= DEPTH_REL, "depth rel error %g" % e_d
+    return e_rgb, e_a, e_d
+
+
+def _check_grads(got, ref, what):
+    got = got.cpu().numpy().astype(np.float64)
+    err = np.abs(got - ref)
+    bound = GRAD_REL * np.abs(ref) + GRAD_ABS
+    worst = (err - bound).max() if err.size else 0.0
+    assert worst <= 0, "%s: %d entries out of tolerance, worst excess %g (|ref| max %g)" % (what, int((err > bound).sum()), worst, np.abs(ref).max())
+    nref = np.linalg.norm(ref)
+    return np.linalg.norm(got - ref) / nref if nref > 0 else 0.0
+
+
+def test_sort_pairs_matches_numpy(ctx):
+    import torch
+    rng = np.random.default_rng(7)
+    for n, bits in ((1, 8), (33, 13), (4096, 20), (4097, 33), (100003, 46), (1 << 20, 64)):
+        keys = rng.integers(0, 1 << min(bits, 63), size=n, dtype=np.uint64)
+        if bits == 64:
+            keys |= rng.integers(0, 2, size=n, dtype=np.uint64) << np.uint64(63)
+        keys[: n // 3] = keys[n // 3: 2 * (n // 3)]  # duplicates: stability is visible in the values
+        vals = np.arange(n, dtype=np.uint32)
+        k = torch.from_numpy(keys.view(np.int64)).cuda()
+        v = torch.from_numpy(vals.view(np.int32)).cuda()
+        ctx.check(ctx.lib.dvx_sort_pairs(ctx.h, k.data_ptr(), v.data_ptr(), n, bits))
+        torch.cuda.synchronize()
+        order = np.argsort(keys, kind="stable")
+        assert np.array_equal(k.cpu().numpy().view(np.uint64), keys[order])
+        assert np.array_equal(v.cpu().numpy().view(np.uint32), vals[order])
+
+
+def test_t2_t3_config1_images_and_gradients(ctx, config1):
+    """Config 1: every pixel and every gradient entry against the pure brute-force oracle."""
+    import paper_2606_23031_b200 as dvx
+    import torch
+    sc = config1
+    gin = sc.image_grads(rgb_std=1e-2, depth_std=1e-3, alpha_std=1e-2)
+    ref = O.render(sc, mode=0, grads_in=gin)
+    dev = dvx.SceneOnDevice(ctx, sc)
+    for flags in (dvx.FLAG_NAIVE, 0):
+        rgb, depth, alpha, frame = dev.render(flags=flags)
+        torch.cuda.synchronize()
+        _check_images(rgb, depth, alpha, ref)
+        g = [torch.from_numpy(gin[k]).cuda() for k in ("rgb", "depth", "alpha")]
+        grads = frame.backward(g[0], g[1], g[2])
+        torch.cuda.synchronize()
+        for t in range(len(sc.octrees)):
+            _check_grads(grads[t][0], ref["dgeo"][t], "dgeo[%d]" % t)
+            _check_grads(grads[t][1], ref["dsh"][t], "dsh[%d]" % t)
+        # accumulate semantics (R17): a second backward into the same buffers doubles them
+        frame.backward(g[0], g[1], g[2], grads=grads)
+        torch.cuda.synchronize()
+        _check_grads(grads[0][0] * 0.5, ref["dgeo"][0], "dgeo[0] accumulated")
+        frame.release()
+
+
+def test_t1_config1_tile_order(ctx, config1):
+    """Per-tile sorted voxel order, bit-exact: the oracle's hit list H (sorted by the R14b key) must be a subsequence of
+    the library's list, and the library's list must itself ascend in the key."""
+    import paper_2606_23031_b200 as dvx
+    sc = config1
+    dev = dvx.SceneOnDevice(ctx, sc)
+    _, _, _, frame = dev.render()
+    cam = sc.cameras[0]
+    tw, th = (cam.width + 15) // 16, (cam.height + 15) // 16
+    n_checked = 0
+    for ty in range(th):
+        for tx in range(tw):
+            for tree in range(len(sc.octrees)):
+                for q in range(8):
+                    got = frame.tile_list(ty * tw + tx, tree, q)
+                    if len(got):
+                        keys = O.order_key(sc.octrees[tree].code[got], q)
+                        assert np.all(keys[1:] > keys[:-1]), "list not strictly ascending in the R14b key"
+                    want = O.tile_hit_list(sc, tx, ty, tree, q)
+                    if len(want) == 0:
+                        continue
+                    pos = {int(v): i for i, v in enumerate(got)}
+                    idx = [pos.get(int(v), -1) for v in want]
+                    assert min(idx) >= 0, "tile (%d,%d) tree %d octant %d: hit voxel missing from the list" % (tx, ty, tree, q)
+                    assert all(a < b for a, b in zip(idx, idx[1:]))
+                    n_checked += len(want)
+    assert n_checked > 1000
+    frame.release()
