@@ -1,0 +1,332 @@
+#!/usr/bin/env python
+"""bench.py - throughput of the DrivingVoxels hot path (steps 1-5 behind include/dvx.h) on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 3] [--impl reference]
+
+One "step" = one pass of the whole hot path over one synthetic frame: dvx_render (projection + binning, key
+generation + radix sort, ray-OBB schedule, compositing) followed by dvx_backward (replay + atomics + SH post-pass).
+Workload at N=1: BASELINE.json configs[2] ("PandaSet-shaped frame", 1920x1080, 4 M + 10x50 k voxels, SH degree 3,
+K = 8), the configuration the metric is quoted on.  Prints ONE JSON line.
+The path does not shard (BASELINE.json north_star: one GPU, no collectives): --gpus N runs N independent replicas.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "fwd+bwd megapixels/s at 1920x1080 (1 B200)"
+UNIT = "MP/s"
+SMI_QUERY = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+             "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=3, help="BASELINE.json config number 1..5 (default 3 = the headline workload)")
+    ap.add_argument("--impl", default="dvx", choices=["dvx", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing leg (profiling runs)")
+    ap.add_argument("--cpu-tiles", type=int, default=0, help="tiles in the CPU-oracle sample (0 = pick for about 10-30 s)")
+    ap.add_argument("--fwd-only", action="store_true", help="profiling aid: time dvx_render alone")
+    return ap.parse_args()
+
+
+def workload_name(n):
+    return {1: "config1_tiny_128x96", 2: "config2_small_960x540", 3: "config3_pandaset_shaped_1920x1080_4M+10x50k_sh3_K8",
+            4: "config4_crowded_1920x1080_500k+40x25k_sh3_K8", 5: "config5_training_batch_6x1920x1080_8M+20x50k_sh3_K8"}[n]
+
+
+# ----------------------------------------------------------------------------------------------- clocks
+class ClockSampler:
+    """nvidia-smi sampled every 200 ms DURING the timed region (B200_PROFILING.md clocks line)."""
+
+    def __init__(self, index):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        self.p = None
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), "--query-gpu=" + SMI_QUERY, "--format=csv,noheader,nounits",
+                                       "-lms", "200"], stdout=self.f, stderr=subprocess.DEVNULL)
+        except OSError:
+            self.p = None
+
+    def stop(self):
+        if self.p is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.p.kill()
+        self.f.flush()
+        rows = [r.split(",") for r in open(self.f.name).read().strip().splitlines() if r.strip()]
+        os.unlink(self.f.name)
+        sm, smax, reasons, power = [], [], set(), []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in rows:
+            try:
+                sm.append(float(r[1])); smax.append(float(r[2])); power.append(float(r[3]))
+            except (ValueError, IndexError):
+                continue
+            for name, val in zip(names, r[5:9]):
+                if val.strip().lower() == "active":
+                    reasons.add(name)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(smax)), "reasons": sorted(reasons),
+                "samples": len(sm), "power_w_max": max(power)}
+
+
+# ----------------------------------------------------------------------------------------------- CPU oracle leg
+def oracle_sample(scene, n_tiles_sample, backward, seed=7):
+    """Times the oracle (tile-culled mode, validated bit-identical to brute force by pin P13), as it stands, on a seeded
+    sample of whole 16x16 tiles of camera 0.  Returns dict(seconds_binning, seconds_sample, pixels, mp_s_full_frame)."""
+    from oracle import oracle as O
+    cam = scene.cameras[0]
+    H, W = cam.height, cam.width
+    tw, th = (W + 15) // 16, (H + 15) // 16
+    rng = np.random.default_rng(seed)
+    tiles = rng.choice(tw * th, size=min(n_tiles_sample, tw * th), replace=False)
+    mask = np.zeros((H, W), dtype=np.uint8)
+    for t in tiles:
+        ty, tx = divmod(int(t), tw)
+        mask[ty * 16:(ty + 1) * 16, tx * 16:(tx + 1) * 16] = 1
+    gin = scene.image_grads(rgb_std=1e-2) if backward else None
+    t0 = time.perf_counter()
+    O.render(scene, mode=1, mask=np.zeros((H, W), dtype=np.uint8))       # binning of the whole frame, no pixel rendered
+    t_bin = time.perf_counter() - t0
+    t0 = time.perf_counter()
+    O.render(scene, mode=1, mask=mask, grads_in=gin)
+    t_all = time.perf_counter() - t0
+    npx = int(mask.sum())
+    t_px = max(t_all - t_bin, 1e-9)
+    full = t_bin + t_px * (W * H / npx)
+    return {"seconds_binning": t_bin, "seconds_sample": t_all, "pixels": npx, "tiles": int(len(tiles)),
+            "mp_s_full_frame": W * H / full / 1e6, "threads": O.num_threads()}
+
+
+def pick_cpu_tiles(scene, backward):
+    """Sizes the sample for roughly 15 s of CPU work from a 4-tile probe."""
+    probe = oracle_sample(scene, 4, backward, seed=11)
+    per_tile = max((probe["seconds_sample"] - probe["seconds_binning"]) / 4, 1e-3)
+    return int(min(max(15.0 / per_tile, 8), 2048))
+
+
+def run_reference(args, scene):
+    """--impl reference: the oracle as it stands on the host cores, each step a bounded sample of the workload."""
+    n_tiles = args.cpu_tiles or max(4, pick_cpu_tiles(scene, True) // max(args.steps + args.warmup, 1))
+    vals = []
+    for it in range(args.warmup + args.steps):
+        r = oracle_sample(scene, n_tiles, True, seed=100 + it)
+        if it >= args.warmup:
+            vals.append(r)
+    mp = float(np.mean([r["mp_s_full_frame"] for r in vals]))
+    cam = scene.cameras[0]
+    ms = cam.width * cam.height / (mp * 1e6) * 1e3
+    sample = "%d seeded 16x16 tiles (%d px) of camera 0 per step, fwd+bwd, tile-culled oracle; full-frame time = binning + per-pixel time x W*H" % (
+        vals[0]["tiles"], vals[0]["pixels"])
+    line = {"impl": "reference", "metric": METRIC, "value": mp, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic", "config": {"workload": workload_name(args.config), "inputs_exceed_l2": True},
+            "cpu_baseline": {"value": mp, "unit": UNIT, "cores": vals[0]["threads"], "kind": "oracle", "sample": sample},
+            "e2e": {"value": mp, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+# ----------------------------------------------------------------------------------------------- GPU arm
+def measured_peaks():
+    """Roofline denominators: MEASURED_PEAKS.json (driver-written) or the fallback B200_PROFILING.md states."""
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        d = json.load(open(path))
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json)", d
+    except (OSError, ValueError, KeyError):
+        return 6650.0, "fallback (B200_PROFILING.md)", {}
+
+
+def algorithmic_bytes(scene, W, H, cnt, touched):
+    """bytes the method must move, from the run's own counters.  cnt: v_vis (per frame), pairs_eff."""
+    n_sh = scene.static.n_sh
+    rec = 8 + 32 + 12 * n_sh                    # key + 8 corner densities + SH coefficients of one voxel record
+    px = W * H
+    b = {}
+    b["min_fwd"] = cnt["v_vis"] * rec + 20 * px
+    b["min_fwdbwd"] = b["min_fwd"] + 12 * px + touched * (2 * 32 + 2 * 12 * n_sh)
+    # per kernel (what a tile-sort rasterizer of this method streams): id + per-frame voxel record + corners
+    b["composite_fwd"] = cnt["pairs_eff"] * (4 + 32 + 32) + 20 * px + 24 * px
+    b["composite_bwd"] = cnt["pairs_eff"] * (4 + 32 + 32) + px * (12 + 24) + touched * (2 * 32 + 2 * 16)
+    return b
+
+
+def run_dvx(args):
+    import torch
+    import torch.distributed as dist
+    import dvx_scenes
+    import paper_2606_23031_b200 as dvx
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: libdvx has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    scene = dvx_scenes.make_config(args.config)
+    ctx = dvx.Context(local)
+    dev = dvx.SceneOnDevice(ctx, scene)
+    n_cams = len(scene.cameras)
+    cam0 = scene.cameras[0]
+    W, H = cam0.width, cam0.height
+    px_step = n_cams * W * H
+    grads = dev.zero_grads()
+    g_dev = [torch.from_numpy(scene.image_grads(c, rgb_std=1e-2)["rgb"]).to(ctx.device) for c in range(n_cams)]
+    g_host = [g.cpu().pin_memory() for g in g_dev]
+    out_dev = (torch.empty((H, W, 3), dtype=torch.float32, device=ctx.device), torch.empty((H, W), dtype=torch.float32, device=ctx.device),
+               torch.empty((H, W), dtype=torch.float32, device=ctx.device))
+    out_host = tuple(t.cpu().pin_memory() for t in out_dev)
+
+    def step(host=False, keep=None, bwd=True):
+        for c in range(n_cams):
+            _, _, _, fr = dev.render(c, save=bwd, out=out_host if host else out_dev, host=host)
+            if bwd:
+                fr.backward(g_host[c] if host else g_dev[c], grads=grads, host=host)
+                if keep is not None:
+                    keep.append(fr)
+                else:
+                    fr.release()
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def timed(n, **kw):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        e0.record()
+        for _ in range(n):
+            step(**kw)
+        e1.record()
+        barrier()
+        ms = e0.elapsed_time(e1)
+        if world > 1:
+            t = torch.tensor([ms], device=ctx.device)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ms = float(t.item())
+        return ms
+
+    # ---- untimed: counters of this workload (one frame per camera, counting build of the kernels)
+    cnt = {"v_vis": 0, "pairs": 0, "pairs_eff": 0, "q_test": 0, "q_hit": 0}
+    for c in range(n_cams):
+        _, _, _, fr = dev.render(c, save=True, flags=dvx.FLAG_COUNTERS)
+        for k, v in fr.counters().items():
+            cnt[k] += v
+        fr.release()
+    if cnt["pairs_eff"] == 0:
+        cnt["pairs_eff"] = cnt["pairs"]
+    for _ in range(args.warmup):
+        step(bwd=not args.fwd_only)
+    torch.cuda.synchronize()
+    touched = int(sum(int((g[0] != 0).any(dim=1).sum().item()) for g in grads))
+
+    # ---- timed region 1: device-resident inputs
+    keep = []
+    l0 = ctx.lib.dvx_launch_count()
+    sampler = ClockSampler(local) if rank == 0 else None
+    ms_total = timed(args.steps, keep=keep, bwd=not args.fwd_only)
+    launches = int(ctx.lib.dvx_launch_count() - l0)
+    stage = {}
+    for fr in keep:
+        for k, v in fr.stage_ms().items():
+            stage[k] = stage.get(k, 0.0) + v / args.steps
+        fr.release()
+    keep = None
+    # ---- forward only (reported beside the headline)
+    for _ in range(2):
+        step(bwd=False)
+    ms_fwd = timed(args.steps, bwd=False)
+    # ---- timed region 2: end to end through the host-buffer entry points (pinned host <-> device copies inside)
+    for _ in range(2):
+        step(host=True, bwd=not args.fwd_only)
+    ms_e2e = timed(args.steps, host=True, bwd=not args.fwd_only)
+    clocks = sampler.stop() if sampler else None
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+    ms_step = ms_total / args.steps
+    value = world * px_step / (ms_step * 1e-3) / 1e6
+    fwd_value = world * px_step / (ms_fwd / args.steps * 1e-3) / 1e6
+    e2e_value = world * px_step / (ms_e2e / args.steps * 1e-3) / 1e6
+    peak, peak_src, peaks = measured_peaks()
+    ab = algorithmic_bytes(scene, W, H, {k: v / 1 for k, v in cnt.items()}, touched)
+    dom = "composite_bwd" if not args.fwd_only else "composite_fwd"
+    dom_ms = stage.get("backward_composite" if not args.fwd_only else "composite", 0.0)
+    dom_bytes = ab[dom]
+    achieved = dom_bytes / (dom_ms * 1e-3) / 1e9 if dom_ms > 0 else 0.0
+    ncu_traffic = None
+    try:  # per-launch DRAM bytes of the dominant kernel from the committed ncu --set full capture, if present
+        ncu_traffic = json.load(open(os.path.join(ROOT, "profiles", "traffic.json"))).get(dom)
+    except (OSError, ValueError):
+        pass
+    hbm_frac_step = ab["min_fwdbwd" if not args.fwd_only else "min_fwd"] / (ms_step * 1e-3) / 1e9 / peak
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+        "data": "synthetic",
+        "config": {"workload": workload_name(args.config), "cameras": n_cams, "k_samples": scene.k_samples, "sh_degree": scene.static.sh_degree,
+                   "voxels": int(sum(t.n_voxels for t in scene.octrees)), "actors": len(scene.actors),
+                   "l2_policy": "inputs larger than L2 (voxel records + gradient buffers >> 126 MB)", "replicas": world,
+                   "passes": "fwd" if args.fwd_only else "fwd+bwd"},
+        "fwd_value": fwd_value, "fwd_ms": ms_fwd / args.steps,
+        "hbm_roofline_frac_step": hbm_frac_step,
+        "stage_ms": stage, "counters": dict(cnt, touched_voxels=touched),
+        "algorithmic_bytes": ab,
+        "roofline": {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
+                     "frac": achieved / peak if peak else None, "traffic": ncu_traffic, "peak_source": peak_src,
+                     "bytes_per_launch": dom_bytes, "ms_per_launch": dom_ms},
+        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": (0 if args.fwd_only else 12 * px_step),
+                "d2h_bytes_per_step": 20 * px_step, "ms_per_step": ms_e2e / args.steps},
+        "gpu_launches": launches, "clocks": clocks,
+    }
+    if not args.no_cpu_baseline and world == 1:
+        n_tiles = args.cpu_tiles or pick_cpu_tiles(scene, True)
+        r = oracle_sample(scene, n_tiles, True)
+        line["cpu_baseline"] = {"value": r["mp_s_full_frame"], "unit": UNIT, "cores": r["threads"], "kind": "oracle",
+                                "sample": "%d seeded 16x16 tiles (%d px) of camera 0, fwd+bwd, tile-culled oracle (pin P13); "
+                                          "full-frame time = whole-frame binning (%.1f s) + per-pixel time x W*H" % (
+                                              r["tiles"], r["pixels"], r["seconds_binning"])}
+    else:
+        line["cpu_baseline"] = None
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        if int(os.environ.get("RANK", "0")) != 0:
+            return
+        import dvx_scenes
+        run_reference(args, dvx_scenes.make_config(args.config))
+        return
+    run_dvx(args)
+
+
+if __name__ == "__main__":
+    main()

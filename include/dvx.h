@@ -120,6 +120,18 @@ dvx_status dvx_backward(dvx_ctx *ctx, dvx_frame *saved, const float *dL_drgb, co
                         const float *dL_dalpha, dvx_grad static_grad, const dvx_grad *actor_grads);
 void dvx_frame_release(dvx_ctx *ctx, dvx_frame *frame);
 
+/* The same two calls with HOST image buffers (pinned memory recommended), for end-to-end use from a host
+ * data pipeline: dvx_render_host renders into device staging owned by the context and enqueues the device->host
+ * copies of RGB, depth and alpha (out_host.* are HOST pointers; valid after the stream is synchronised);
+ * dvx_backward_host enqueues the host->device copies of the incoming image gradients (HOST pointers; depth / alpha
+ * may be NULL) and then runs step 5.  Octree arrays and gradient buffers stay DEVICE pointers (they are model
+ * state that lives in HBM across steps).  Bytes moved per call: 20 W H out, 12 W H (+4 W H each for depth/alpha) in. */
+dvx_status dvx_render_host(dvx_ctx *ctx, const dvx_camera *cam, const dvx_octree *static_tree, uint32_t n_actors,
+                           const dvx_octree *const *actors, const float *poses_l2w, const float *box_half,
+                           const dvx_render_opts *opts, dvx_image out_host, dvx_frame **saved);
+dvx_status dvx_backward_host(dvx_ctx *ctx, dvx_frame *saved, const float *dL_drgb_host, const float *dL_ddepth_host,
+                             const float *dL_dalpha_host, dvx_grad static_grad, const dvx_grad *actor_grads);
+
 /* Introspection for the parity tests and the benchmark (each synchronises the stream).
  * dvx_debug_tile_list: the sorted voxel list (voxel indices within octree `octree`, 0 = static, i = actor i-1) of
  * tile `tile` (row-major tile index) for ray-direction octant `octant`; ids_host HOST [capacity]; *n_out = full length. */
@@ -128,9 +140,13 @@ dvx_status dvx_debug_tile_list(dvx_ctx *ctx, const dvx_frame *frame, uint32_t ti
 /* v_vis: voxels surviving culling; pairs: (tile, octant, voxel) pairs sorted; the last three need DVX_FLAG_COUNTERS. */
 dvx_status dvx_frame_counters(dvx_ctx *ctx, const dvx_frame *frame, uint64_t *v_vis, uint64_t *pairs,
                               uint64_t *pairs_eff, uint64_t *q_test, uint64_t *q_hit);
-/* Device milliseconds of the stages of the frame's dvx_render call: [0] preprocess (step 1), [1] key generation +
- * sort + ranges (step 2), [2] compositing (steps 3+4); after dvx_backward also [3] backward (step 5). HOST out[4]. */
-dvx_status dvx_frame_stage_ms(dvx_ctx *ctx, const dvx_frame *frame, float *ms_out4);
+/* Device milliseconds (CUDA events on the context's stream) of the stages of the frame's dvx_render call:
+ * [0] preprocess (step 1), [1] key generation + sort + ranges (step 2), [2] compositing kernel (steps 3+4);
+ * after dvx_backward also [3] all of step 5, [4] its compositing-replay kernel alone, [5] its per-voxel SH
+ * post-pass alone.  [6], [7] reserved (0).  HOST out[8].  Synchronises the stream. */
+dvx_status dvx_frame_stage_ms(dvx_ctx *ctx, const dvx_frame *frame, float *ms_out8);
+/* Kernels launched by the library in this process so far (all contexts). */
+uint64_t dvx_launch_count(void);
 const char *dvx_last_error(const dvx_ctx *ctx);
 
 /* Stand-alone entry to hot-path step 2's sort (tests and sort-throughput measurement): sorts n (key, value) pairs by

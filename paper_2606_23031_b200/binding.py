@@ -20,7 +20,8 @@ FLAG_NAIVE = 2
 
 EXPORTS = ["dvx_create", "dvx_destroy", "dvx_octree_create", "dvx_octree_refresh_structure", "dvx_octree_destroy",
            "dvx_render", "dvx_backward", "dvx_frame_release", "dvx_debug_tile_list", "dvx_frame_counters",
-           "dvx_frame_stage_ms", "dvx_last_error", "dvx_sort_pairs"]
+           "dvx_frame_stage_ms", "dvx_last_error", "dvx_sort_pairs", "dvx_launch_count", "dvx_render_host",
+           "dvx_backward_host"]
 
 
 class DvxError(RuntimeError):
@@ -84,9 +85,13 @@ def load():
     lib.dvx_last_error.argtypes = [P]
     lib.dvx_last_error.restype = C.c_char_p
     lib.dvx_sort_pairs.argtypes = [P, P, P, C.c_uint64, C.c_uint32]
+    lib.dvx_launch_count.argtypes = []
+    lib.dvx_render_host.argtypes = lib.dvx_render.argtypes
+    lib.dvx_backward_host.argtypes = lib.dvx_backward.argtypes
     for name in EXPORTS:
-        if name not in ("dvx_destroy", "dvx_octree_destroy", "dvx_frame_release", "dvx_last_error"):
+        if name not in ("dvx_destroy", "dvx_octree_destroy", "dvx_frame_release", "dvx_last_error", "dvx_launch_count"):
             getattr(lib, name).restype = C.c_int32
+    lib.dvx_launch_count.restype = C.c_uint64
     _lib = lib
     return lib
 
@@ -149,11 +154,15 @@ class Context:
 
     # ------------------------------------------------------------------ render / backward
     def render(self, cam, static, actors=(), poses=None, box_half=None, k_samples=8, activation=0, t_stop=1e-4, flags=0,
-               save=True, out=None):
-        """dvx_render.  cam: binding.Camera; poses [N,12] / box_half [N,3] host float32 arrays.
+               save=True, out=None, host=False):
+        """dvx_render (host=False: device image tensors) or dvx_render_host (host=True: ``out`` must be three pinned
+        CPU tensors).  cam: binding.Camera; poses [N,12] / box_half [N,3] host float32 arrays.
         Returns (rgb [H,W,3], depth [H,W], alpha [H,W], Frame or None)."""
         torch = self.torch
         H, W = cam.height, cam.width
+        if host and out is None:
+            out = (torch.empty((H, W, 3), dtype=torch.float32).pin_memory(), torch.empty((H, W), dtype=torch.float32).pin_memory(),
+                   torch.empty((H, W), dtype=torch.float32).pin_memory())
         if out is None:
             rgb = torch.empty((H, W, 3), dtype=torch.float32, device=self.device)
             depth = torch.empty((H, W), dtype=torch.float32, device=self.device)
@@ -168,8 +177,9 @@ class Context:
         opts = RenderOpts(k_samples, activation, t_stop, flags)
         img = Image(rgb.data_ptr(), depth.data_ptr(), alpha.data_ptr())
         fh = C.c_void_p()
-        rc = self.lib.dvx_render(self.h, C.byref(cam), static.h, n, handles, poses.ctypes.data_as(C.c_void_p),
-                                 half.ctypes.data_as(C.c_void_p), C.byref(opts), img, C.byref(fh) if save else None)
+        fn = self.lib.dvx_render_host if host else self.lib.dvx_render
+        rc = fn(self.h, C.byref(cam), static.h, n, handles, poses.ctypes.data_as(C.c_void_p),
+                half.ctypes.data_as(C.c_void_p), C.byref(opts), img, C.byref(fh) if save else None)
         self.check(rc)
         frame = Frame(self, fh, [static] + list(actors)) if save else None
         return rgb, depth, alpha, frame
@@ -206,8 +216,9 @@ class Frame:
     def __init__(self, ctx, h, trees):
         self.ctx, self.h, self.trees = ctx, h, trees
 
-    def backward(self, dL_drgb, dL_ddepth=None, dL_dalpha=None, grads=None):
-        """dvx_backward.  grads: list of (dgeo, dsh) tensors per octree (accumulated into); None = fresh zeros.
+    def backward(self, dL_drgb, dL_ddepth=None, dL_dalpha=None, grads=None, host=False):
+        """dvx_backward (device image gradients) or dvx_backward_host (host=True: pinned CPU tensors).
+        grads: list of (dgeo, dsh) tensors per octree (accumulated into); None = fresh zeros.
         Returns the list of (dgeo, dsh)."""
         ctx, torch = self.ctx, self.ctx.torch
         if grads is None:
@@ -217,7 +228,8 @@ class Frame:
         n = len(self.trees) - 1
         arr = (Grad * max(n, 1))(*g[1:])
         ptr = lambda t: None if t is None else t.data_ptr()
-        ctx.check(ctx.lib.dvx_backward(ctx.h, self.h, ptr(dL_drgb), ptr(dL_ddepth), ptr(dL_dalpha), g[0], arr))
+        fn = ctx.lib.dvx_backward_host if host else ctx.lib.dvx_backward
+        ctx.check(fn(ctx.h, self.h, ptr(dL_drgb), ptr(dL_ddepth), ptr(dL_dalpha), g[0], arr))
         return grads
 
     def tile_list(self, tile, octree, octant):
@@ -237,9 +249,9 @@ class Frame:
 
     def stage_ms(self):
         ctx = self.ctx
-        ms = (C.c_float * 4)()
+        ms = (C.c_float * 8)()
         ctx.check(ctx.lib.dvx_frame_stage_ms(ctx.h, self.h, ms))
-        return dict(zip(("preprocess", "sort", "composite", "backward"), list(ms)))
+        return dict(zip(("preprocess", "sort", "composite", "backward", "backward_composite", "backward_sh"), list(ms)[:6]))
 
     def release(self):
         if self.h and self.ctx.h:
@@ -269,9 +281,14 @@ class SceneOnDevice:
         self.box_half = np.ascontiguousarray(scene.box_half, dtype=np.float32)
         self.cams = [camera_from(c) for c in scene.cameras]
 
-    def render(self, cam_index=0, save=True, flags=0, out=None, **opt):
+    def render(self, cam_index=0, save=True, flags=0, out=None, host=False, **opt):
         s = self.scene
         kw = dict(k_samples=s.k_samples, activation=s.activation, t_stop=s.t_stop)
         kw.update(opt)
         return self.ctx.render(self.cams[cam_index], self.trees[0], self.trees[1:], self.poses, self.box_half, flags=flags,
-                               save=save, out=out, **kw)
+                               save=save, out=out, host=host, **kw)
+
+    def zero_grads(self):
+        torch = self.ctx.torch
+        return [(torch.zeros((t.n_voxels, 8), dtype=torch.float32, device=self.ctx.device),
+                 torch.zeros((t.n_voxels, t.n_sh, 3), dtype=torch.float32, device=self.ctx.device)) for t in self.trees]

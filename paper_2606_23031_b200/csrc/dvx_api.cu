@@ -9,6 +9,8 @@
 
 #include "dvx_internal.cuh"
 
+unsigned long long g_dvx_launches = 0;
+
 struct dvx_ctx {
   int device = 0;
   cudaStream_t st = nullptr;
@@ -34,7 +36,7 @@ struct dvx_frame {
   struct Buf { void *p = nullptr; size_t bytes = 0; };
   Buf trees_d, fvox, pxrect, octmask, actor_mask, ids, range_beg, range_end, counters, sv_rgbd, sv_T, sv_nused;
   uint64_t n_pairs = 0, v_vis = 0;
-  cudaEvent_t ev[7] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+  cudaEvent_t ev[9] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
   bool did_backward = false;
 };
 
@@ -423,7 +425,9 @@ dvx_status dvx_backward(dvx_ctx *ctx, dvx_frame *f, const float *dL_drgb, const 
   A.sv_rgbd = (float *)f->sv_rgbd.p; A.sv_T = (float *)f->sv_T.p; A.sv_nused = (uint32_t *)f->sv_nused.p;
   A.counters = (unsigned long long *)f->counters.p;
   A.g_rgb = dL_drgb; A.g_depth = dL_ddepth; A.g_alpha = dL_dalpha; A.drgb = drgb;
+  CU(cudaEventRecord(f->ev[7], st));
   dvx_composite_launch(A, true, st);
+  CU(cudaEventRecord(f->ev[8], st));
   dvx_sh_backward_launch(p, trees_d, A.fvox, A.pxrect, drgb, st);
   CU(cudaEventRecord(f->ev[6], st));
   CU(cudaGetLastError());
@@ -479,12 +483,58 @@ dvx_status dvx_frame_stage_ms(dvx_ctx *ctx, const dvx_frame *f, float *ms) {
   if (!f || !ms) return fail(ctx, DVX_ERR_INVALID_ARG, "NULL argument");
   cudaSetDevice(ctx->device);
   CU(cudaStreamSynchronize(ctx->st));
-  ms[0] = ms[1] = ms[2] = ms[3] = 0.f;
+  for (int i = 0; i < 8; ++i) ms[i] = 0.f;
   CU(cudaEventElapsedTime(&ms[0], f->ev[0], f->ev[1]));
   CU(cudaEventElapsedTime(&ms[1], f->ev[2], f->ev[3]));
   CU(cudaEventElapsedTime(&ms[2], f->ev[3], f->ev[4]));
-  if (f->did_backward) CU(cudaEventElapsedTime(&ms[3], f->ev[5], f->ev[6]));
+  if (f->did_backward) {
+    CU(cudaEventElapsedTime(&ms[3], f->ev[5], f->ev[6]));
+    CU(cudaEventElapsedTime(&ms[4], f->ev[7], f->ev[8]));
+    CU(cudaEventElapsedTime(&ms[5], f->ev[8], f->ev[6]));
+  }
   return DVX_OK;
+}
+
+uint64_t dvx_launch_count(void) { return (uint64_t)g_dvx_launches; }
+
+dvx_status dvx_render_host(dvx_ctx *ctx, const dvx_camera *cam, const dvx_octree *static_tree, uint32_t n_actors,
+                           const dvx_octree *const *actors, const float *poses_l2w, const float *box_half,
+                           const dvx_render_opts *opts, dvx_image out_host, dvx_frame **saved) {
+  if (saved) *saved = nullptr;
+  if (!ctx) return DVX_ERR_INVALID_ARG;
+  if (!cam || !out_host.rgb || !out_host.depth || !out_host.alpha) return fail(ctx, DVX_ERR_INVALID_ARG, "NULL argument");
+  cudaSetDevice(ctx->device);
+  const size_t npix = (size_t)cam->width * cam->height;
+  float *stage = (float *)ctx_alloc(ctx, npix * 20);
+  if (!stage) return fail(ctx, DVX_ERR_OOM, "dvx_render_host: allocator returned NULL");
+  dvx_image dev = {stage, stage + 3 * npix, stage + 4 * npix};
+  dvx_status rc = dvx_render(ctx, cam, static_tree, n_actors, actors, poses_l2w, box_half, opts, dev, saved);
+  if (rc == DVX_OK) {
+    cudaError_t e = cudaMemcpyAsync(out_host.rgb, dev.rgb, npix * 12, cudaMemcpyDeviceToHost, ctx->st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(out_host.depth, dev.depth, npix * 4, cudaMemcpyDeviceToHost, ctx->st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(out_host.alpha, dev.alpha, npix * 4, cudaMemcpyDeviceToHost, ctx->st);
+    if (e != cudaSuccess) rc = cuda_fail(ctx, e, "dvx_render_host: cudaMemcpyAsync");
+  }
+  ctx_release(ctx, stage);  // stream-ordered reuse: later users of the block are enqueued after the copies
+  return rc;
+}
+
+dvx_status dvx_backward_host(dvx_ctx *ctx, dvx_frame *f, const float *g_rgb_h, const float *g_depth_h, const float *g_alpha_h,
+                             dvx_grad static_grad, const dvx_grad *actor_grads) {
+  if (!ctx) return DVX_ERR_INVALID_ARG;
+  if (!f || !g_rgb_h) return fail(ctx, DVX_ERR_INVALID_ARG, "NULL argument");
+  cudaSetDevice(ctx->device);
+  const size_t npix = (size_t)f->p.width * f->p.height;
+  float *stage = (float *)ctx_alloc(ctx, npix * 20);
+  if (!stage) return fail(ctx, DVX_ERR_OOM, "dvx_backward_host: allocator returned NULL");
+  float *d_rgb = stage, *d_depth = g_depth_h ? stage + 3 * npix : nullptr, *d_alpha = g_alpha_h ? stage + 4 * npix : nullptr;
+  cudaError_t e = cudaMemcpyAsync(d_rgb, g_rgb_h, npix * 12, cudaMemcpyHostToDevice, ctx->st);
+  if (e == cudaSuccess && d_depth) e = cudaMemcpyAsync(d_depth, g_depth_h, npix * 4, cudaMemcpyHostToDevice, ctx->st);
+  if (e == cudaSuccess && d_alpha) e = cudaMemcpyAsync(d_alpha, g_alpha_h, npix * 4, cudaMemcpyHostToDevice, ctx->st);
+  dvx_status rc = e == cudaSuccess ? dvx_backward(ctx, f, d_rgb, d_depth, d_alpha, static_grad, actor_grads)
+                                   : cuda_fail(ctx, e, "dvx_backward_host: cudaMemcpyAsync");
+  ctx_release(ctx, stage);
+  return rc;
 }
 
 dvx_status dvx_sort_pairs(dvx_ctx *ctx, uint64_t *keys, uint32_t *vals, uint64_t n, uint32_t key_bits) {

@@ -291,8 +291,6 @@ __global__ void __launch_bounds__(TILE_THREADS) composite_naive_kernel(const Com
 
 void dvx_composite_launch(const CompositeArgs &a, bool backward, cudaStream_t st) {
   if (a.p.n_tiles == 0) return;
-  if (backward)
-    composite_naive_kernel<true><<<a.p.n_tiles, TILE_THREADS, 0, st>>>(a);
-  else
-    composite_naive_kernel<false><<<a.p.n_tiles, TILE_THREADS, 0, st>>>(a);
+    if (backward) { DVX_COUNT_LAUNCH(1); composite_naive_kernel<true><<<a.p.n_tiles, TILE_THREADS, 0, st>>>(a); }
+    else { DVX_COUNT_LAUNCH(1); composite_naive_kernel<false><<<a.p.n_tiles, TILE_THREADS, 0, st>>>(a); }
 }

@@ -64,6 +64,10 @@ struct CompositeArgs {
   float *drgb;                 // [v_total][4] scratch: dL/drgb_v
 };
 
+// Number of kernels launched by this library since it was loaded (bench.py's gpu_launches claim).
+extern unsigned long long g_dvx_launches;
+#define DVX_COUNT_LAUNCH(n) (g_dvx_launches += (unsigned long long)(n))
+
 // ---- dvx_sort.cu
 size_t dvx_sort_scratch_bytes(uint64_t n);
 // Sorts by bits [0,key_bits) ascending, stable.  Result lands in keys_a/vals_a or keys_b/vals_b; returns 0 or 1 (which).

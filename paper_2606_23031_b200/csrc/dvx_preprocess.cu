@@ -317,40 +317,37 @@ inline unsigned blocks_for(uint64_t n, int threads) { return (unsigned)((n + thr
 }  // namespace
 
 void dvx_rank_keys_launch(const uint64_t *code, uint32_t n, int q, uint64_t *keys, uint32_t *vals, cudaStream_t st) {
-  if (n) rank_keys_kernel<<<blocks_for(n, 256), 256, 0, st>>>(code, n, (uint64_t)q * 0x249249249249ull, keys, vals);
+  if (n) { DVX_COUNT_LAUNCH(1); rank_keys_kernel<<<blocks_for(n, 256), 256, 0, st>>>(code, n, (uint64_t)q * 0x249249249249ull, keys, vals); }
 }
 void dvx_rank_scatter_launch(const uint32_t *perm, uint32_t n, uint32_t *rank, cudaStream_t st) {
-  if (n) rank_scatter_kernel<<<blocks_for(n, 256), 256, 0, st>>>(perm, n, rank);
+  if (n) { DVX_COUNT_LAUNCH(1); rank_scatter_kernel<<<blocks_for(n, 256), 256, 0, st>>>(perm, n, rank); }
 }
 void dvx_validate_launch(const uint64_t *skeys, const uint32_t *perm, const uint64_t *code, uint32_t n,
                          uint32_t *bad_flag, cudaStream_t st) {
-  if (n) validate_kernel<<<blocks_for(n, 256), 256, 0, st>>>(skeys, perm, code, n, bad_flag);
+  if (n) { DVX_COUNT_LAUNCH(1); validate_kernel<<<blocks_for(n, 256), 256, 0, st>>>(skeys, perm, code, n, bad_flag); }
 }
 void dvx_tree_setup_launch(const FrameParams &p, TreeFrame *trees, cudaStream_t st) {
-  tree_setup_kernel<<<1, 128, 0, st>>>(p, trees);
+  { DVX_COUNT_LAUNCH(1); tree_setup_kernel<<<1, 128, 0, st>>>(p, trees); }
 }
 void dvx_tile_masks_launch(const FrameParams &p, const TreeFrame *trees, uint8_t *octmask, unsigned long long *actor_mask,
                            cudaStream_t st) {
-  tile_masks_kernel<<<blocks_for(p.n_tiles, 128), 128, 0, st>>>(p, trees, octmask, actor_mask);
+  { DVX_COUNT_LAUNCH(1); tile_masks_kernel<<<blocks_for(p.n_tiles, 128), 128, 0, st>>>(p, trees, octmask, actor_mask); }
 }
 void dvx_preprocess_launch(const FrameParams &p, const TreeFrame *trees, const uint8_t *octmask, FrameVox *fvox,
                            ushort4 *pxrect, unsigned long long *counters, cudaStream_t st) {
-  if (p.v_total)
-    preprocess_kernel<<<blocks_for(p.v_total, PRE_THREADS), PRE_THREADS, 0, st>>>(p, trees, octmask, fvox, pxrect, counters);
+    if (p.v_total) { DVX_COUNT_LAUNCH(1); preprocess_kernel<<<blocks_for(p.v_total, PRE_THREADS), PRE_THREADS, 0, st>>>(p, trees, octmask, fvox, pxrect, counters); }
 }
 void dvx_emit_pairs_launch(const FrameParams &p, const TreeFrame *trees, const uint8_t *octmask, const ushort4 *pxrect,
                            uint64_t *keys, uint32_t *vals, unsigned long long capacity, unsigned long long *counters,
                            cudaStream_t st) {
-  if (p.v_total)
-    emit_pairs_kernel<<<blocks_for(p.v_total, PRE_THREADS), PRE_THREADS, 0, st>>>(p, trees, octmask, pxrect, keys, vals,
-                                                                                   capacity, counters);
+    if (p.v_total) { DVX_COUNT_LAUNCH(1); emit_pairs_kernel<<<blocks_for(p.v_total, PRE_THREADS), PRE_THREADS, 0, st>>>(p, trees, octmask, pxrect, keys, vals,
+                                                                                   capacity, counters); }
 }
 void dvx_ranges_launch(const uint64_t *keys, uint64_t n, uint32_t rank_bits, uint32_t *range_beg, uint32_t *range_end,
                        cudaStream_t st) {
-  if (n) ranges_kernel<<<blocks_for(n, 256), 256, 0, st>>>(keys, n, rank_bits, range_beg, range_end);
+  if (n) { DVX_COUNT_LAUNCH(1); ranges_kernel<<<blocks_for(n, 256), 256, 0, st>>>(keys, n, rank_bits, range_beg, range_end); }
 }
 void dvx_sh_backward_launch(const FrameParams &p, const TreeFrame *trees, const FrameVox *fvox, const ushort4 *pxrect,
                             const float *drgb, cudaStream_t st) {
-  if (p.v_total)
-    sh_backward_kernel<<<blocks_for(p.v_total, PRE_THREADS), PRE_THREADS, 0, st>>>(p, trees, fvox, pxrect, drgb);
+    if (p.v_total) { DVX_COUNT_LAUNCH(1); sh_backward_kernel<<<blocks_for(p.v_total, PRE_THREADS), PRE_THREADS, 0, st>>>(p, trees, fvox, pxrect, drgb); }
 }

@@ -166,12 +166,12 @@ void dvx_scan_u32_launch(uint32_t *data, uint64_t n, uint32_t *scratch, cudaStre
   if (n == 0) return;
   uint64_t nb = ceil_div(n, SCAN_TILE);
   if (nb == 1) {
-    scan_apply<<<1, SCAN_THREADS, 0, st>>>(data, n, nullptr);
+    { DVX_COUNT_LAUNCH(1); scan_apply<<<1, SCAN_THREADS, 0, st>>>(data, n, nullptr); }
     return;
   }
-  scan_block_sums<<<(unsigned)nb, SCAN_THREADS, 0, st>>>(data, n, scratch);
+  { DVX_COUNT_LAUNCH(1); scan_block_sums<<<(unsigned)nb, SCAN_THREADS, 0, st>>>(data, n, scratch); }
   dvx_scan_u32_launch(scratch, nb, scratch + nb, st);
-  scan_apply<<<(unsigned)nb, SCAN_THREADS, 0, st>>>(data, n, scratch);
+  { DVX_COUNT_LAUNCH(1); scan_apply<<<(unsigned)nb, SCAN_THREADS, 0, st>>>(data, n, scratch); }
 }
 
 size_t dvx_sort_scratch_bytes(uint64_t n) {
@@ -192,9 +192,9 @@ int dvx_sort_launch(uint64_t *keys_a, uint32_t *vals_a, uint64_t *keys_b, uint32
   for (int p = 0; p < passes; ++p) {
     uint64_t *kin = cur ? keys_b : keys_a, *kout = cur ? keys_a : keys_b;
     uint32_t *vin = cur ? vals_b : vals_a, *vout = cur ? vals_a : vals_b;
-    radix_hist<<<nb, SORT_THREADS, 0, st>>>(kin, n, 8u * p, hist, nb);
+    { DVX_COUNT_LAUNCH(1); radix_hist<<<nb, SORT_THREADS, 0, st>>>(kin, n, 8u * p, hist, nb); }
     dvx_scan_u32_launch(hist, (uint64_t)nb * RADIX, scan_scr, st);
-    radix_scatter<<<nb, SORT_THREADS, 0, st>>>(kin, vin, kout, vout, n, 8u * p, hist, nb);
+    { DVX_COUNT_LAUNCH(1); radix_scatter<<<nb, SORT_THREADS, 0, st>>>(kin, vin, kout, vout, n, 8u * p, hist, nb); }
     cur ^= 1;
   }
   return cur;

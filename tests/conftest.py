@@ -16,3 +16,9 @@ def pytest_configure(config):
 def config1():
     import dvx_scenes
     return dvx_scenes.make_config(1)
+
+
+@pytest.fixture(scope="session")
+def config3():
+    import dvx_scenes
+    return dvx_scenes.make_config(3)

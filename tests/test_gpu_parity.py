@@ -113,3 +113,140 @@ def test_t1_config1_tile_order(ctx, config1):
                     n_checked += len(want)
     assert n_checked > 1000
     frame.release()
+
+
+# ----------------------------------------------------------------------------------------------- larger configs
+def _tile_mask(cam, n_tiles, seed):
+    tw, th = (cam.width + 15) // 16, (cam.height + 15) // 16
+    rng = np.random.default_rng(seed)
+    tiles = rng.choice(tw * th, size=min(n_tiles, tw * th), replace=False)
+    mask = np.zeros((cam.height, cam.width), dtype=np.uint8)
+    for t in tiles:
+        ty, tx = divmod(int(t), tw)
+        mask[ty * 16:(ty + 1) * 16, tx * 16:(tx + 1) * 16] = 1
+    return mask, tiles
+
+
+def _sampled_parity(ctx, sc, n_tiles, seed, backward):
+    """Full-size launch (the configuration bench.py times); compared on seeded whole tiles the oracle (tile-culled mode,
+    pin P13) renders pixel by pixel.  Gradients: dL/dimage is zeroed outside the sample on both sides, so every gradient
+    entry is compared."""
+    import paper_2606_23031_b200 as dvx
+    import torch
+    cam = sc.cameras[0]
+    mask, _ = _tile_mask(cam, n_tiles, seed)
+    gin = None
+    if backward:
+        gin = sc.image_grads(rgb_std=1e-2)
+        gin["rgb"] = gin["rgb"] * mask[:, :, None].astype(np.float32)
+    ref = O.render(sc, mode=1, mask=mask, grads_in=gin)
+    dev = dvx.SceneOnDevice(ctx, sc)
+    rgb, depth, alpha, frame = dev.render()
+    torch.cuda.synchronize()
+    errs = _check_images(rgb, depth, alpha, ref, mask)
+    if backward:
+        grads = frame.backward(torch.from_numpy(gin["rgb"]).cuda())
+        torch.cuda.synchronize()
+        for t in range(len(sc.octrees)):
+            _check_grads(grads[t][0], ref["dgeo"][t], "dgeo[%d]" % t)
+            _check_grads(grads[t][1], ref["dsh"][t], "dsh[%d]" % t)
+    frame.release()
+    for t in dev.trees:
+        t.close()
+    return errs
+
+
+def test_t2_config2_forward_sampled_tiles(ctx):
+    _sampled_parity(ctx, S.make_config(2), 192, 21, backward=False)
+
+
+def test_t2_t3_config3_fwd_bwd_sampled_tiles(ctx, config3):
+    _sampled_parity(ctx, config3, 96, 31, backward=True)
+
+
+def test_t2_t3_config4_crowded_fwd_bwd_sampled_tiles(ctx):
+    sc = S.make_config(4)
+    # sample tiles where boxes overlap the rays: restrict the draw to the lower-middle band where the traffic is
+    _sampled_parity(ctx, sc, 96, 41, backward=True)
+
+
+def test_t1_config2_tile_order_sampled(ctx):
+    """T1 on seeded tiles of config 2 (brute-force hit lists are slow: 12 tiles)."""
+    import paper_2606_23031_b200 as dvx
+    sc = S.make_config(2)
+    dev = dvx.SceneOnDevice(ctx, sc)
+    _, _, _, frame = dev.render()
+    cam = sc.cameras[0]
+    tw = (cam.width + 15) // 16
+    _, tiles = _tile_mask(cam, 12, 51)
+    n_checked = 0
+    for tile in tiles:
+        ty, tx = divmod(int(tile), tw)
+        for tree in range(len(sc.octrees)):
+            for q in range(8):
+                got = frame.tile_list(int(tile), tree, q)
+                if len(got) == 0:
+                    continue
+                keys = O.order_key(sc.octrees[tree].code[got], q)
+                assert np.all(keys[1:] > keys[:-1])
+                want = O.tile_hit_list(sc, tx, ty, tree, q)
+                pos = {int(v): i for i, v in enumerate(got)}
+                idx = [pos.get(int(v), -1) for v in want]
+                assert len(idx) == 0 or min(idx) >= 0, "hit voxel missing from the tile list"
+                assert all(a < b for a, b in zip(idx, idx[1:]))
+                n_checked += len(want)
+    assert n_checked > 100
+    frame.release()
+
+
+def test_t4_api_errors_and_inference_path(ctx, config1):
+    import ctypes as C
+    import paper_2606_23031_b200 as dvx
+    import torch
+    sc = config1
+    dev = dvx.SceneOnDevice(ctx, sc)
+    # saved = NULL path renders the same image and keeps nothing
+    rgb0, d0, a0, fr = dev.render(save=True)
+    rgb1, d1, a1, none = dev.render(save=False)
+    torch.cuda.synchronize()
+    assert none is None and torch.equal(rgb0, rgb1) and torch.equal(d0, d1) and torch.equal(a0, a1)
+    # host-buffer entry points give the same bits
+    rgbh, dh, ah, frh = dev.render(save=True, host=True)
+    torch.cuda.synchronize()
+    assert torch.equal(rgbh, rgb0.cpu()) and torch.equal(dh, d0.cpu()) and torch.equal(ah, a0.cpu())
+    gin = sc.image_grads(rgb_std=1e-2)
+    g_dev = torch.from_numpy(gin["rgb"]).cuda()
+    ga = fr.backward(g_dev)
+    gb = frh.backward(torch.from_numpy(gin["rgb"]).pin_memory(), host=True)
+    torch.cuda.synchronize()
+    ref = ga[0][0].abs().max().item()
+    assert (ga[0][0] - gb[0][0]).abs().max().item() <= 1e-5 * ref + 1e-7   # float-atomic order is free (R17)
+    fr.release(); frh.release()
+    # invalid arguments -> DVX_ERR_INVALID_ARG, never a crash
+    for kw in (dict(k_samples=0), dict(k_samples=9), dict(activation=2), dict(t_stop=-1.0)):
+        with pytest.raises(dvx.DvxError) as e:
+            dev.render(**kw)
+        assert e.value.status == -1
+    bad_pose = dev.poses.copy(); bad_pose[0, 0] *= 1.5
+    with pytest.raises(dvx.DvxError) as e:
+        ctx.render(dev.cams[0], dev.trees[0], dev.trees[1:], bad_pose, dev.box_half)
+    assert e.value.status == -1
+    cam = dvx.camera_from(sc.cameras[0]); cam.fx = 0.0
+    with pytest.raises(dvx.DvxError):
+        ctx.render(cam, dev.trees[0], dev.trees[1:], dev.poses, dev.box_half)
+    # bad octrees -> DVX_ERR_BAD_OCTREE (duplicate leaf; nested leaf; bits below the level)
+    t = sc.static
+    code = t.code.copy(); code[1] = code[0]
+    for bad in (code, np.concatenate([t.code[:4], [np.uint64((np.uint64(5) << np.uint64(48)) | (t.code[0] & np.uint64(0xFFFFFFFFFFFF) & ~np.uint64((1 << 33) - 1)))]]).astype(np.uint64)):
+        n = len(bad)
+        with pytest.raises(dvx.DvxError) as e:
+            ctx.octree(torch.from_numpy(bad.view(np.int64)).cuda(), torch.zeros((n, 8), device="cuda"),
+                       torch.zeros((n, 1, 3), device="cuda"), t.center, t.side, 0)
+        assert e.value.status == -2, e.value
+    # empty actor list and empty octree are legal
+    empty = ctx.octree(torch.zeros(0, dtype=torch.int64, device="cuda"), torch.zeros((0, 8), device="cuda"),
+                       torch.zeros((0, 1, 3), device="cuda"), (0, 0, 0), 1.0, 0)
+    r, d, a, f2 = ctx.render(dev.cams[0], empty)
+    torch.cuda.synchronize()
+    assert float(a.abs().max()) == 0.0 and float(r.abs().max()) == 0.0
+    f2.release()
