@@ -247,10 +247,12 @@ void setup_tree(TreeFrame &T, const dvx_octree *t, uint32_t base, bool actor, co
     double o = 0;
     for (int r = 0; r < 3; ++r) o += R[3 * r + a] * ((double)cam->c2w[4 * r + 3] - tr[r]);
     T.o_l[a] = o;
+    T.rel0[a] = T.lo[a] - o;
     T.ol_f[a] = (float)o;
     for (int c = 0; c < 3; ++c) {
       double n = 0;
       for (int r = 0; r < 3; ++r) n += R[3 * r + a] * (double)cam->c2w[4 * r + c];
+      T.Nd[3 * a + c] = n;
       T.N[3 * a + c] = (float)n;
     }
     T.half[a] = actor ? half[a] : INFINITY;
@@ -304,6 +306,7 @@ dvx_status dvx_render(dvx_ctx *ctx, const dvx_camera *cam, const dvx_octree *sta
   p.tiles_x = (cam->width + DVX_TILE - 1) / DVX_TILE; p.tiles_y = (cam->height + DVX_TILE - 1) / DVX_TILE;
   p.n_tiles = p.tiles_x * p.tiles_y; p.n_trees = 1 + n_actors;
   p.fx = cam->fx; p.fy = cam->fy; p.cx = cam->cx; p.cy = cam->cy; p.near_ = cam->near_; p.far_ = cam->far_;
+  p.inv_fx = 1.0 / (double)cam->fx; p.inv_fy = 1.0 / (double)cam->fy; p.cx_d = (double)cam->cx; p.cy_d = (double)cam->cy;
   {  // every point of a ray at tau >= near has z_cam >= near * min_pixels cos(angle to the axis) > zclip
     double mc = 1.0;
     const double us[2] = {0.5, (double)cam->width - 0.5}, vs[2] = {0.5, (double)cam->height - 0.5};

@@ -19,7 +19,9 @@ struct TreeFrame {
   double lo[3];          // cube min corner w_c - w_s/2 (tree frame)
   double cell;           // w_s / 2^16 : edge of a level-16 cell
   double o_l[3];         // camera origin in the tree frame: R_o^T (o_c - t_o)
-  float ol_f[3];         // the same rounded to fp32 (ray-OBB test only)
+  double rel0[3];        // lo - o_l: cube min corner relative to the camera origin (tree frame)
+  double Nd[9];          // R_o^T R_c in fp64 (N below is its fp32 rounding)
+  float ol_f[3];         // o_l rounded to fp32 (debug walker's ray-OBB test only)
   float N[9];            // R_o^T R_c: d_l[a] = N[3a] x' + N[3a+1] y' + N[3a+2];  p_cam[c] = sum_a N[3a+c] rel[a]
   float half[3];         // OBB half extents (actors)
   int box_rect[4];       // pixel rectangle of the OBB (x0,y0,x1,y1 inclusive; x1<x0 = not visible); set on device
@@ -28,6 +30,7 @@ struct TreeFrame {
 struct FrameParams {
   uint32_t width, height, tiles_x, tiles_y, n_tiles, n_trees;
   float fx, fy, cx, cy, near_, far_, zclip;
+  double inv_fx, inv_fy, cx_d, cy_d;  // fp64 copies for the per-pixel ray set-up of the tile kernel
   uint32_t k_samples, activation, flags;
   float t_stop;
   uint32_t rank_bits;   // sort key = (bucket << rank_bits) | rank ; bucket = (tile*n_trees + tree)*8 + octant
@@ -93,5 +96,10 @@ void dvx_ranges_launch(const uint64_t *keys, uint64_t n, uint32_t rank_bits, uin
 void dvx_sh_backward_launch(const FrameParams &p, const TreeFrame *trees, const FrameVox *fvox, const ushort4 *pxrect,
                             const float *drgb, cudaStream_t st);
 
-// ---- dvx_composite.cu
-void dvx_composite_launch(const CompositeArgs &a, bool backward, cudaStream_t st);
+// ---- dvx_composite_tile.cu (production) / dvx_composite_naive.cu (DVX_FLAG_NAIVE: one thread walks one ray, debug)
+void dvx_composite_tile_launch(const CompositeArgs &a, bool backward, cudaStream_t st);
+void dvx_composite_naive_launch(const CompositeArgs &a, bool backward, cudaStream_t st);
+inline void dvx_composite_launch(const CompositeArgs &a, bool backward, cudaStream_t st) {
+  if (a.p.flags & DVX_FLAG_NAIVE) dvx_composite_naive_launch(a, backward, st);
+  else dvx_composite_tile_launch(a, backward, st);
+}
