@@ -119,7 +119,7 @@ def pick_cpu_tiles(scene, backward):
     """Sizes the sample for roughly 15 s of CPU work from a 4-tile probe."""
     probe = oracle_sample(scene, 4, backward, seed=11)
     per_tile = max((probe["seconds_sample"] - probe["seconds_binning"]) / 4, 1e-3)
-    return int(min(max(15.0 / per_tile, 8), 2048))
+    return int(min(max(15.0 / per_tile, 8), 8160))
 
 
 def run_reference(args, scene):
@@ -197,15 +197,12 @@ def run_dvx(args):
                torch.empty((H, W), dtype=torch.float32, device=ctx.device))
     out_host = tuple(t.cpu().pin_memory() for t in out_dev)
 
-    def step(host=False, keep=None, bwd=True):
+    def step(host=False, bwd=True):
         for c in range(n_cams):
             _, _, _, fr = dev.render(c, save=bwd, out=out_host if host else out_dev, host=host)
             if bwd:
                 fr.backward(g_host[c] if host else g_dev[c], grads=grads, host=host)
-                if keep is not None:
-                    keep.append(fr)
-                else:
-                    fr.release()
+                fr.release()
 
     def barrier():
         torch.cuda.synchronize()
@@ -243,17 +240,13 @@ def run_dvx(args):
     touched = int(sum(int((g[0] != 0).any(dim=1).sum().item()) for g in grads))
 
     # ---- timed region 1: device-resident inputs
-    keep = []
+    ctx.stage_ms_collect()                       # drop the stage times of the warm-up frames
     l0 = ctx.lib.dvx_launch_count()
     sampler = ClockSampler(local) if rank == 0 else None
-    ms_total = timed(args.steps, keep=keep, bwd=not args.fwd_only)
+    ms_total = timed(args.steps, bwd=not args.fwd_only)
     launches = int(ctx.lib.dvx_launch_count() - l0)
-    stage = {}
-    for fr in keep:
-        for k, v in fr.stage_ms().items():
-            stage[k] = stage.get(k, 0.0) + v / args.steps
-        fr.release()
-    keep = None
+    sums, n_frames = ctx.stage_ms_collect()      # CUDA-event stage times of exactly the timed steps (on the ctx stream)
+    stage = {k: v / args.steps for k, v in sums.items()}
     # ---- forward only (reported beside the headline)
     for _ in range(2):
         step(bwd=False)

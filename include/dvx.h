@@ -145,6 +145,10 @@ dvx_status dvx_frame_counters(dvx_ctx *ctx, const dvx_frame *frame, uint64_t *v_
  * after dvx_backward also [3] all of step 5, [4] its compositing-replay kernel alone, [5] its per-voxel SH
  * post-pass alone.  [6], [7] reserved (0).  HOST out[8].  Synchronises the stream. */
 dvx_status dvx_frame_stage_ms(dvx_ctx *ctx, const dvx_frame *frame, float *ms_out8);
+/* The same six stage times SUMMED over every frame released (or rendered with saved = NULL) since the last call;
+ * *n_frames = how many.  Lets a benchmark time the stages of the very steps it measures without keeping frames alive.
+ * HOST ms_out8[8], HOST n_frames.  Synchronises the stream. */
+dvx_status dvx_stage_ms_collect(dvx_ctx *ctx, float *ms_out8, uint32_t *n_frames);
 /* Kernels launched by the library in this process so far (all contexts). */
 uint64_t dvx_launch_count(void);
 const char *dvx_last_error(const dvx_ctx *ctx);

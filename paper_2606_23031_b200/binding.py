@@ -15,12 +15,13 @@ LIB_PATH = os.path.join(_HERE, "libdvx.so")
 DVX_OK = 0
 ERRORS = {-1: "DVX_ERR_INVALID_ARG", -2: "DVX_ERR_BAD_OCTREE", -3: "DVX_ERR_OOM", -4: "DVX_ERR_CUDA",
           -5: "DVX_ERR_NOT_IMPLEMENTED"}
+STAGES = ("preprocess", "sort", "composite", "backward", "backward_composite", "backward_sh")
 FLAG_COUNTERS = 1
 FLAG_NAIVE = 2
 
 EXPORTS = ["dvx_create", "dvx_destroy", "dvx_octree_create", "dvx_octree_refresh_structure", "dvx_octree_destroy",
            "dvx_render", "dvx_backward", "dvx_frame_release", "dvx_debug_tile_list", "dvx_frame_counters",
-           "dvx_frame_stage_ms", "dvx_last_error", "dvx_sort_pairs", "dvx_launch_count", "dvx_render_host",
+           "dvx_frame_stage_ms", "dvx_last_error", "dvx_sort_pairs", "dvx_launch_count", "dvx_stage_ms_collect", "dvx_render_host",
            "dvx_backward_host"]
 
 
@@ -86,6 +87,7 @@ def load():
     lib.dvx_last_error.restype = C.c_char_p
     lib.dvx_sort_pairs.argtypes = [P, P, P, C.c_uint64, C.c_uint32]
     lib.dvx_launch_count.argtypes = []
+    lib.dvx_stage_ms_collect.argtypes = [P, C.POINTER(C.c_float), C.POINTER(C.c_uint32)]
     lib.dvx_render_host.argtypes = lib.dvx_render.argtypes
     lib.dvx_backward_host.argtypes = lib.dvx_backward.argtypes
     for name in EXPORTS:
@@ -132,6 +134,13 @@ class Context:
 
     def _free(self, ptr, _user):
         self._blocks.pop(ptr, None)
+
+    def stage_ms_collect(self):
+        """Sum of the stage times of all frames released since the last call -> (dict of ms sums, n_frames)."""
+        ms = (C.c_float * 8)()
+        n = C.c_uint32()
+        self.check(self.lib.dvx_stage_ms_collect(self.h, ms, C.byref(n)))
+        return dict(zip(STAGES, list(ms)[:6])), n.value
 
     def check(self, rc):
         if rc != DVX_OK:

@@ -11,7 +11,14 @@
 
 unsigned long long g_dvx_launches = 0;
 
+// The CUDA events of one render (+ backward) call.  Owned by the context and recycled, so the steady state creates none.
+struct EventSet {
+  cudaEvent_t ev[9] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+  bool rendered = false, did_backward = false;
+};
+
 struct dvx_ctx {
+  std::vector<EventSet *> ev_free, ev_pending;  // pending: released frames whose times dvx_stage_ms_collect has not summed yet
   int device = 0;
   cudaStream_t st = nullptr;
   dvx_alloc_fn alloc = nullptr;
@@ -36,7 +43,9 @@ struct dvx_frame {
   struct Buf { void *p = nullptr; size_t bytes = 0; };
   Buf trees_d, fvox, pxrect, octmask, actor_mask, ids, range_beg, range_end, counters, sv_rgbd, sv_T, sv_nused;
   uint64_t n_pairs = 0, v_vis = 0;
-  cudaEvent_t ev[9] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+  EventSet *es = nullptr;
+  cudaEvent_t *ev = nullptr;  // = es->ev
+  Buf eff_end;
   bool did_backward = false;
 };
 
@@ -104,8 +113,19 @@ void frame_free(dvx_ctx *ctx, dvx_frame *f) {
   dvx_frame::Buf *bs[] = {&f->trees_d, &f->fvox, &f->pxrect, &f->octmask, &f->actor_mask, &f->ids,
                           &f->range_beg, &f->range_end, &f->counters, &f->sv_rgbd, &f->sv_T, &f->sv_nused};
   for (auto *b : bs) ctx_release(ctx, b->p);
-  for (auto &e : f->ev)
-    if (e) cudaEventDestroy(e);
+  ctx_release(ctx, f->eff_end.p);
+  if (f->es) {
+    f->es->did_backward = f->did_backward;
+    if (f->es->rendered) {
+      ctx->ev_pending.push_back(f->es);
+      if (ctx->ev_pending.size() > 256) {  // nobody collects: recycle the oldest
+        ctx->ev_free.push_back(ctx->ev_pending.front());
+        ctx->ev_pending.erase(ctx->ev_pending.begin());
+      }
+    } else {
+      ctx->ev_free.push_back(f->es);
+    }
+  }
   delete f;
 }
 
@@ -189,6 +209,11 @@ void dvx_destroy(dvx_ctx *ctx) {
     else cudaFree(b.p);
   }
   cudaFreeHost(ctx->h_counters);
+  for (auto *v : {&ctx->ev_free, &ctx->ev_pending})
+    for (EventSet *es : *v) {
+      for (auto &e : es->ev) cudaEventDestroy(e);
+      delete es;
+    }
   delete ctx;
 }
 
@@ -237,6 +262,7 @@ void setup_tree(TreeFrame &T, const dvx_octree *t, uint32_t base, bool actor, co
   T.base = base; T.is_actor = actor ? 1u : 0u;
   for (int a = 0; a < 3; ++a) T.lo[a] = (double)t->d.center[a] - 0.5 * (double)t->d.side;
   T.cell = (double)t->d.side / 65536.0;
+  T.inv_cell_f = (float)(65536.0 / (double)t->d.side);
   double R[9] = {1, 0, 0, 0, 1, 0, 0, 0, 1}, tr[3] = {0, 0, 0};
   if (actor)
     for (int r = 0; r < 3; ++r) {
@@ -318,6 +344,7 @@ dvx_status dvx_render(dvx_ctx *ctx, const dvx_camera *cam, const dvx_octree *sta
     p.zclip = (float)(0.5 * (double)cam->near_ * mc);
   }
   p.k_samples = o.k_samples; p.activation = o.activation; p.flags = o.flags; p.t_stop = o.t_stop;
+  p.inv_k = 1.0f / (float)o.k_samples;
   f->trees_h.resize(p.n_trees);
   uint64_t vtot = 0, vmax = 1;
   for (uint32_t t = 0; t < p.n_trees; ++t) {
@@ -343,7 +370,21 @@ dvx_status dvx_render(dvx_ctx *ctx, const dvx_camera *cam, const dvx_octree *sta
   if (ok && saved)
     ok = buf_alloc(ctx, f->sv_rgbd, npix * 16) && buf_alloc(ctx, f->sv_T, npix * 4) && buf_alloc(ctx, f->sv_nused, npix * 4);
   if (!ok) { frame_free(ctx, f); return fail(ctx, DVX_ERR_OOM, "dvx_render: allocator returned NULL"); }
-  for (auto &e : f->ev) CU(cudaEventCreate(&e));
+  if (!ctx->ev_free.empty()) {
+    f->es = ctx->ev_free.back();
+    ctx->ev_free.pop_back();
+  } else {
+    f->es = new EventSet();
+    for (auto &e : f->es->ev)
+      if (cudaEventCreate(&e) != cudaSuccess) {
+        for (auto &e2 : f->es->ev) if (e2) cudaEventDestroy(e2);
+        delete f->es; f->es = nullptr;
+        frame_free(ctx, f);
+        return fail(ctx, DVX_ERR_CUDA, "cudaEventCreate failed");
+      }
+  }
+  f->es->rendered = false; f->es->did_backward = false;
+  f->ev = f->es->ev;
 
   TreeFrame *trees_d = (TreeFrame *)f->trees_d.p;
   unsigned long long *counters = (unsigned long long *)f->counters.p;
@@ -389,8 +430,14 @@ dvx_status dvx_render(dvx_ctx *ctx, const dvx_camera *cam, const dvx_octree *sta
   A.rgb = out.rgb; A.depth = out.depth; A.alpha = out.alpha;
   A.sv_rgbd = (float *)f->sv_rgbd.p; A.sv_T = (float *)f->sv_T.p; A.sv_nused = (uint32_t *)f->sv_nused.p;
   A.counters = counters;
+  if (p.flags & DVX_FLAG_COUNTERS) {
+    if (!buf_alloc(ctx, f->eff_end, sizeof(uint32_t) * (size_t)p.n_buckets)) { frame_free(ctx, f); return fail(ctx, DVX_ERR_OOM, "dvx_render: allocator returned NULL"); }
+    CU(cudaMemsetAsync(f->eff_end.p, 0, sizeof(uint32_t) * (size_t)p.n_buckets, st));
+    A.eff_end = (uint32_t *)f->eff_end.p;
+  }
   dvx_composite_launch(A, false, st);
   CU(cudaEventRecord(f->ev[4], st));
+  f->es->rendered = true;
   CU(cudaGetLastError());
   if (saved) *saved = f;
   else frame_free(ctx, f);
@@ -475,7 +522,19 @@ dvx_status dvx_frame_counters(dvx_ctx *ctx, const dvx_frame *f, uint64_t *v_vis,
   CU(cudaStreamSynchronize(ctx->st));
   if (v_vis) *v_vis = h[CNT_VVIS];
   if (pairs) *pairs = h[CNT_PAIRS];
-  if (pairs_eff) *pairs_eff = h[CNT_PAIRS_EFF];
+  if (pairs_eff) {
+    *pairs_eff = 0;
+    if (f->eff_end.p) {  // sum over buckets of (furthest streamed position - begin)
+      std::vector<uint32_t> beg(f->p.n_buckets), eff(f->p.n_buckets);
+      CU(cudaMemcpyAsync(beg.data(), f->range_beg.p, 4 * (size_t)f->p.n_buckets, cudaMemcpyDeviceToHost, ctx->st));
+      CU(cudaMemcpyAsync(eff.data(), f->eff_end.p, 4 * (size_t)f->p.n_buckets, cudaMemcpyDeviceToHost, ctx->st));
+      CU(cudaStreamSynchronize(ctx->st));
+      uint64_t tot = 0;
+      for (size_t b = 0; b < beg.size(); ++b)
+        if (eff[b] > beg[b]) tot += eff[b] - beg[b];
+      *pairs_eff = tot;
+    }
+  }
   if (q_test) *q_test = h[CNT_QTEST];
   if (q_hit) *q_hit = h[CNT_QHIT];
   return DVX_OK;
@@ -495,6 +554,27 @@ dvx_status dvx_frame_stage_ms(dvx_ctx *ctx, const dvx_frame *f, float *ms) {
     CU(cudaEventElapsedTime(&ms[4], f->ev[7], f->ev[8]));
     CU(cudaEventElapsedTime(&ms[5], f->ev[8], f->ev[6]));
   }
+  return DVX_OK;
+}
+
+dvx_status dvx_stage_ms_collect(dvx_ctx *ctx, float *ms, uint32_t *n_frames) {
+  if (!ctx) return DVX_ERR_INVALID_ARG;
+  if (!ms || !n_frames) return fail(ctx, DVX_ERR_INVALID_ARG, "NULL argument");
+  cudaSetDevice(ctx->device);
+  CU(cudaStreamSynchronize(ctx->st));
+  for (int i = 0; i < 8; ++i) ms[i] = 0.f;
+  *n_frames = (uint32_t)ctx->ev_pending.size();
+  static const int pairs[6][2] = {{0, 1}, {2, 3}, {3, 4}, {5, 6}, {7, 8}, {8, 6}};
+  for (EventSet *es : ctx->ev_pending) {
+    for (int i = 0; i < 6; ++i) {
+      if (i >= 3 && !es->did_backward) break;
+      float t = 0.f;
+      if (cudaEventElapsedTime(&t, es->ev[pairs[i][0]], es->ev[pairs[i][1]]) == cudaSuccess) ms[i] += t;
+      else cudaGetLastError();
+    }
+    ctx->ev_free.push_back(es);
+  }
+  ctx->ev_pending.clear();
   return DVX_OK;
 }
 

@@ -3,22 +3,25 @@
 //   step 4  Algorithm 1: F over Morton-ordered per-tile voxel lists, segment by segment, carrying
 //           S = (C, D, T, tau_curr); trilinear raw density, K midpoint samples, activation,
 //           alpha = 1 - exp(-sum sigma dt), blend weighted by T
-//   step 5  the matching backward, segment-reduced over the warp before the vector atomics
+//   step 5  the matching backward, run-reduced over the warp before the vector atomics
 //
-// One CTA per 16x16 tile, one warp per 8x4 pixel block, one lane per pixel.  The work of a warp is split into three
-// kinds of phases so that the expensive arithmetic always runs on full warps:
-//   A  geometry   the warp walks the tile's sorted list 32 entries at a time (lane = entry: coalesced id load, gather of
-//                 the per-frame voxel record, pixel-rectangle pre-filter by ballot); for every surviving entry all lanes
-//                 (= pixels) run the ray-AABB slab test, clip to their current interval of Algorithm 1 and apply the
-//                 gating rule; hits are appended to a per-warp queue in shared memory as (voxel, pixel, a, b) items,
-//                 ordered by list position - which is each pixel's own front-to-back order.
+// One CTA per 16x16 tile, one warp per 8x4 pixel block, one lane per pixel.  The work of a warp is split into phases so
+// that the expensive arithmetic always runs on full warps:
+//   A  geometry   the warp walks the tile's sorted list 32 entries at a time.  First lane = entry: coalesced id load,
+//                 pixel-rectangle pre-filter, Morton decode and - in fp64, once per (warp, entry) - the voxel centre
+//                 split into its distance t0 along the warp's reference direction d0 and the small remainder m0.
+//                 Then lane = pixel: for every surviving entry the slab test runs on small, well-conditioned numbers
+//                 (x(tau) - c = s' d + (t0 e - m0), s' = tau - t0, e = d - d0), is clipped to the pixel's current interval
+//                 of Algorithm 1 (R1) and gated; hits go to a per-warp ring in shared memory as items, ordered by list
+//                 position = each pixel's own front-to-back order.
 //   B  integrate  as soon as 32 items are queued: lane = item.  The trilinear raw density restricted to a ray segment
-//                 is a cubic in the segment parameter, so the 8 corner values are folded into 4 coefficients once and
-//                 each of the K samples costs a Horner evaluation and one ex2.  tau_v goes back to the queue.
-//   C  blend      lane = pixel again: every pixel consumes its own items of the batch in order (T, C, D update and the
-//                 T < t_stop test after every voxel, R3).  In the backward this phase produces dL/dtau_v and T alpha g_C
-//                 per item, and a second lane = item phase (B2) turns them into corner gradients, reduces runs of items
-//                 of the same voxel with shuffles and issues one 16-byte vector atomic per 4 floats.
+//                 is a cubic in the segment parameter: the 8 corner values fold into 4 coefficients once, each of the
+//                 K samples is a Horner evaluation and one ex2.
+//   C  blend      lane = pixel again: every pixel consumes its own items of the batch in order (a per-lane bit mask of
+//                 ring positions): T, C, D update and the T < t_stop test after every voxel (R3).  In the backward this
+//                 phase produces dL/dtau_v and T alpha g_C per item, and a second lane = item phase (B2) turns them
+//                 into corner gradients, reduces runs of items of the same voxel with shuffles and issues 16-byte
+//                 vector reductions (red.global.add.v4.f32).
 // Gating (which list entry ends a pixel's current background / actor interval) is purely geometric, so phase A never
 // needs T; early termination only removes pixels from later batches.
 #include "dvx_ray.cuh"
@@ -27,20 +30,32 @@ namespace {
 
 constexpr int TILE_THREADS = 256;
 constexpr int TILE_WARPS = TILE_THREADS / 32;
-constexpr int QCAP = 64;              // queue capacity per warp: at most 31 left-over items + 32 of one entry
+constexpr int QCAP = 64;              // ring capacity per warp: at most 31 left-over items + 32 of one entry
 constexpr uint32_t NONE = 0xFFFFFFFFu;
 constexpr float LOG2E = 1.4426950408889634f;
 
+// One list entry as phase A (lane = pixel) sees it, staged by the lane that owns the entry.
+struct __align__(16) EntryRec {
+  float t0;       // distance of the voxel centre along the warp's reference direction d0
+  float m0[3];    // centre - t0 d0 (tree frame)
+  float hs;       // half edge length
+  uint32_t id;    // global voxel id
+  uint32_t level;
+  uint32_t pad;
+};
+
 template <bool BWD>
 struct WarpQueue {
-  uint32_t id[QCAP];     // item: global voxel id
-  uint32_t meta[QCAP];   // item: pixel lane | tree << 8
-  float a[QCAP], b[QCAP];  // item: clipped sub-segment [a,b] (O4)
-  float tau[QCAP];       // phase B: tau_v;  backward phase C overwrites it with dL/dtau_v
-  uint32_t e_id[QCAP];   // entry (one list element hit by >= 1 pixel): voxel id, hit-lane mask, index of its first item
-  uint32_t e_mask[QCAP];
-  uint32_t e_base[QCAP];
-  float wg[BWD ? QCAP * 3 : 1];  // backward phase C: T alpha g_C per item, zero where the colour clamp is active
+  EntryRec ent[32];
+  // items (ring of QCAP)
+  uint32_t id[QCAP];
+  uint32_t meta[QCAP];     // pixel lane | tree << 8 | level << 16
+  float ca[QCAP], cb[QCAP];  // clipped sub-segment, relative to t0 (O4, R1)
+  float w[3][QCAP];        // x(tau) - centre = s' d + w
+  float d[3][QCAP];        // ray direction in the tree frame
+  float mid[QCAP];         // (a + b) / 2, absolute ray distance (depth, R9)
+  float tau[QCAP];         // phase B: tau_v;  backward phase C overwrites it with dL/dtau_v
+  float wg[BWD ? 3 : 1][QCAP];  // backward phase C: T alpha g_C per item, zero where the colour clamp is active
 };
 
 struct Pix {
@@ -51,12 +66,22 @@ struct Pix {
   uint32_t n_stop;
 };
 
-struct WarpCtx {
-  int lane, u0, v0;     // u0,v0: pixel of lane 0 of this warp
-  uint32_t lt;          // lanes below this one
-};
-
 __device__ __forceinline__ uint32_t warp_min_u32(uint32_t v) { return __reduce_min_sync(0xffffffffu, v); }
+__device__ __forceinline__ float ex2_approx(float x) {
+  float y;
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+__device__ __forceinline__ double shfl_double(double v, int src) {
+  int lo = __double2loint(v), hi = __double2hiint(v);
+  lo = __shfl_sync(0xffffffffu, lo, src);
+  hi = __shfl_sync(0xffffffffu, hi, src);
+  return __hiloint2double(hi, lo);
+}
+__device__ __forceinline__ double rcp_double(double x) {  // 1/x to ~1e-14 relative: fp32 seed + one Newton step
+  double r = (double)__frcp_rn((float)x);
+  return r * (2.0 - x * r);
+}
 
 // ---- phase B arithmetic -------------------------------------------------------------------------------------------
 // Coefficients of raw(lambda) = trilinear(g, p + q lambda), lambda in [0,1]; corner c = 4 b_x + 2 b_y + b_z (R7).
@@ -88,45 +113,42 @@ struct ItemGeom {
   float delta;       // (b - a) / K
 };
 
-// O6 for one queued item: K-point midpoint rule on [a,b].  Returns tau_v; with GRAD also the moments
-// M_j = sum_k act'(raw_k) lambda_k^j (j = 0..3) from which phase B2 rebuilds sum_k act'(raw_k) w_c(u_k) for all corners.
-template <bool GRAD>
-__device__ __forceinline__ float integrate_item(const CompositeArgs &A, const WarpCtx &W, uint32_t id, uint32_t meta, float a,
-                                                float b, ItemGeom &G, float M[4]) {
-  const TreeFrame &T = A.trees[meta >> 8];
-  const int pl = (int)(meta & 31u);
-  const float xp = dvx_cam_x(A.p, W.u0 + (pl & 7)), yp = dvx_cam_y(A.p, W.v0 + (pl >> 3));
-  const float rn = rsqrtf(xp * xp + yp * yp + 1.0f);
-  const float4 f0 = __ldg(reinterpret_cast<const float4 *>(A.fvox + id));
+// O6 for one queued item (ring slot `at`): K-point midpoint rule on the clipped segment.  Returns tau_v; with GRAD also
+// the moments M_j = sum_k act'(raw_k) lambda_k^j (j = 0..3), from which phase B2 rebuilds sum_k act'(raw_k) w_c(u_k).
+template <bool BWD>
+__device__ __forceinline__ float integrate_item(const CompositeArgs &A, const WarpQueue<BWD> &Q, int at, uint32_t id,
+                                                uint32_t meta, ItemGeom &G, float M[4]) {
+  const TreeFrame &T = A.trees[(meta >> 8) & 0xFFu];
+  const uint32_t level = meta >> 16;
   const float4 *gp = reinterpret_cast<const float4 *>(T.geo + (size_t)(id - T.base) * 8);
   const float4 g0 = __ldg(gp), g1 = __ldg(gp + 1);
   const float g[8] = {g0.x, g0.y, g0.z, g0.w, g1.x, g1.y, g1.z, g1.w};
-  const float rel[3] = {f0.x, f0.y, f0.z};
-  const float inv_s = 1.0f / f0.w;
-  const float len = b - a;
+  // 1 / edge length = (1 / level-16 cell) * 2^(level - 16): exact power-of-two scaling
+  const float inv_s = T.inv_cell_f * __uint_as_float((111u + level) << 23);
+  const float ca = Q.ca[at], cb = Q.cb[at];
 #pragma unroll
   for (int ax = 0; ax < 3; ++ax) {
-    const float d = dvx_dir_comp(T.N, ax, xp, yp) * rn;
-    const float pa = __saturatef((a * d - rel[ax]) * inv_s);   // u clamped to [0,1]^3 (O6)
-    const float pb = __saturatef((b * d - rel[ax]) * inv_s);
+    const float d = Q.d[ax][at], w = Q.w[ax][at];
+    const float pa = __saturatef(fmaf(fmaf(ca, d, w), inv_s, 0.5f));   // u clamped to [0,1]^3 (O6)
+    const float pb = __saturatef(fmaf(fmaf(cb, d, w), inv_s, 0.5f));
     G.p[ax] = pa;
     G.q[ax] = pb - pa;
   }
   float c[4];
   cubic_coeffs(g, G.p, G.q, c);
   const uint32_t K = A.p.k_samples, kind = A.p.activation;
-  const float invK = 1.0f / (float)K;
-  G.delta = len * invK;
+  const float invK = A.p.inv_k;
+  G.delta = (cb - ca) * invK;
   float S = 0.f;
-  if (GRAD) M[0] = M[1] = M[2] = M[3] = 0.f;
+  if (BWD) M[0] = M[1] = M[2] = M[3] = 0.f;
+  float lam = 0.5f * invK;
   if (kind == 0) {  // exp: sigma = ex2(raw * log2 e), act' = act
     const float c0 = c[0] * LOG2E, c1 = c[1] * LOG2E, c2 = c[2] * LOG2E, c3 = c[3] * LOG2E;
-    float lam = 0.5f * invK;
 #pragma unroll 8
     for (uint32_t k = 0; k < K; ++k) {
-      const float sig = exp2f(fmaf(fmaf(fmaf(c3, lam, c2), lam, c1), lam, c0));
+      const float sig = ex2_approx(fmaf(fmaf(fmaf(c3, lam, c2), lam, c1), lam, c0));
       S += sig;
-      if (GRAD) {
+      if (BWD) {
         M[0] += sig;
         float t = sig * lam; M[1] += t;
         t *= lam; M[2] += t;
@@ -135,11 +157,10 @@ __device__ __forceinline__ float integrate_item(const CompositeArgs &A, const Wa
       lam += invK;
     }
   } else {
-    float lam = 0.5f * invK;
     for (uint32_t k = 0; k < K; ++k) {
       const float raw = fmaf(fmaf(fmaf(c[3], lam, c[2]), lam, c[1]), lam, c[0]);
       S += act_fn(raw, kind);
-      if (GRAD) {
+      if (BWD) {
         const float ds = dact_fn(raw, kind);
         M[0] += ds;
         float t = ds * lam; M[1] += t;
@@ -185,86 +206,76 @@ __device__ __forceinline__ void red_add_v4(float *addr, float x, float y, float 
   asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(addr), "f"(x), "f"(y), "f"(z), "f"(w) : "memory");
 }
 
-// ---- phases B, C (and B2) over the first min(n_items, 32) queued items; the rest is shifted to the queue front ----
+// ---- phases B, C (and B2) over the first min(n_items, 32) queued items of the ring ------------------------------------
+// Ring slot of the i-th queued item: (head + i) & (QCAP-1).  my_bits: bit i set <=> queued item i belongs to this pixel.
 template <bool BWD>
-__device__ __forceinline__ void flush_batch(const CompositeArgs &A, const WarpCtx &W, WarpQueue<BWD> &Q, int &n_items,
-                                            int &n_ent, Pix &S) {
-  const int lane = W.lane;
+__device__ __forceinline__ void flush_batch(const CompositeArgs &A, int lane, WarpQueue<BWD> &Q, int &n_items, int &head,
+                                            unsigned long long &my_bits, Pix &S) {
   const int count = n_items < 32 ? n_items : 32;
   __syncwarp();
   // -- B: lane = item
   ItemGeom G;
   float M[4];
   uint32_t my_id = NONE, my_meta = 0;
+  const int at_b = (head + lane) & (QCAP - 1);
   if (lane < count) {
-    my_id = Q.id[lane];
-    my_meta = Q.meta[lane];
-    Q.tau[lane] = integrate_item<BWD>(A, W, my_id, my_meta, Q.a[lane], Q.b[lane], G, M);
+    my_id = Q.id[at_b];
+    my_meta = Q.meta[at_b];
+    Q.tau[at_b] = integrate_item<BWD>(A, Q, at_b, my_id, my_meta, G, M);
   }
   __syncwarp();
-  // -- C: lane = pixel; entries in list order, i.e. in this pixel's front-to-back order
-  int j = 0;
-  uint32_t strad_mask = 0;  // hit lanes of an entry cut by the batch boundary that were NOT consumed
-  bool strad = false;
-  for (; j < n_ent; ++j) {
-    const int base = (int)Q.e_base[j];
-    if (base >= count) break;
-    const uint32_t mask = Q.e_mask[j];
-    const bool mine = (mask >> lane) & 1u;
-    const int pos = base + __popc(mask & W.lt);
-    const bool in_batch = mine && pos < count;
-    if (base + __popc(mask) > count) {  // the entry straddles the boundary: keep the lanes beyond it for the next batch
-      strad = true;
-      strad_mask = mask & ~__ballot_sync(0xffffffffu, in_batch);
-    }
-    if (in_batch) {
-      if (!S.done) {
-        const float4 f1 = __ldg(reinterpret_cast<const float4 *>(A.fvox + Q.e_id[j]) + 1);
-        const float tau = Q.tau[pos];
-        const float ca = Q.a[pos], cb = Q.b[pos];
-        const float e = exp2f(-tau * LOG2E);
-        const float alpha = tau < 1e-3f ? tau * fmaf(-0.5f, tau, 1.0f) : 1.0f - e;  // 1 - exp(-tau) without cancellation
-        const float w = S.T * alpha;
-        const float mid = 0.5f * (ca + cb);
-        if (!BWD) {
-          S.C0 = fmaf(w, f1.x, S.C0); S.C1 = fmaf(w, f1.y, S.C1); S.C2 = fmaf(w, f1.z, S.C2);
-          S.D = fmaf(w, mid, S.D);
-        } else {
-          const float X = S.gC0 * f1.x + S.gC1 * f1.y + S.gC2 * f1.z + S.gD * mid;
-          S.Xpre = fmaf(w, X, S.Xpre);
-          Q.tau[pos] = S.T * e * X - (S.Xtot - S.Xpre) + S.gA * S.T_final;  // dL/dtau_v
-          const uint32_t cm = __float_as_uint(f1.w);
-          Q.wg[3 * pos + 0] = (cm & 1u) ? 0.f : w * S.gC0;
-          Q.wg[3 * pos + 1] = (cm & 2u) ? 0.f : w * S.gC1;
-          Q.wg[3 * pos + 2] = (cm & 4u) ? 0.f : w * S.gC2;
-        }
-        S.T *= e;
-        S.n_used++;
-        if (!BWD) {
-          if (S.T < A.p.t_stop) S.done = true;  // R3: tested after every voxel
-        } else {
-          if (S.n_used >= S.n_stop) S.done = true;
-        }
-      } else if (BWD) {  // queued before this pixel finished its replay: contributes nothing
-        Q.tau[pos] = 0.f;
-        Q.wg[3 * pos + 0] = 0.f; Q.wg[3 * pos + 1] = 0.f; Q.wg[3 * pos + 2] = 0.f;
+  // -- C: lane = pixel; its own items of the batch in queue order = front-to-back order along its ray
+  uint32_t mine = (uint32_t)my_bits;
+  if (count < 32) mine &= (1u << count) - 1u;
+  while (mine) {
+    const int i = __ffs(mine) - 1;
+    mine &= mine - 1;
+    const int at = (head + i) & (QCAP - 1);
+    if (!S.done) {
+      const float4 f1 = __ldg(reinterpret_cast<const float4 *>(A.fvox + Q.id[at]) + 1);
+      const float tau = Q.tau[at];
+      const float mid = Q.mid[at];
+      const float e = ex2_approx(-tau * LOG2E);
+      const float alpha = tau < 1e-3f ? tau * fmaf(-0.5f, tau, 1.0f) : 1.0f - e;  // 1 - exp(-tau) without cancellation
+      const float w = S.T * alpha;
+      if (!BWD) {
+        S.C0 = fmaf(w, f1.x, S.C0); S.C1 = fmaf(w, f1.y, S.C1); S.C2 = fmaf(w, f1.z, S.C2);
+        S.D = fmaf(w, mid, S.D);
+      } else {
+        const float X = S.gC0 * f1.x + S.gC1 * f1.y + S.gC2 * f1.z + S.gD * mid;
+        S.Xpre = fmaf(w, X, S.Xpre);
+        Q.tau[at] = S.T * e * X - (S.Xtot - S.Xpre) + S.gA * S.T_final;  // dL/dtau_v
+        const uint32_t cm = __float_as_uint(f1.w);
+        Q.wg[0][at] = (cm & 1u) ? 0.f : w * S.gC0;
+        Q.wg[1][at] = (cm & 2u) ? 0.f : w * S.gC1;
+        Q.wg[2][at] = (cm & 4u) ? 0.f : w * S.gC2;
       }
+      S.T *= e;
+      S.n_used++;
+      if (!BWD) {
+        if (S.T < A.p.t_stop) S.done = true;  // R3: tested after every voxel
+      } else {
+        if (S.n_used >= S.n_stop) S.done = true;
+      }
+    } else if (BWD) {  // queued before this pixel finished its replay: contributes nothing
+      Q.tau[at] = 0.f;
+      Q.wg[0][at] = 0.f; Q.wg[1][at] = 0.f; Q.wg[2][at] = 0.f;
     }
   }
-  const int j_keep = strad ? j - 1 : j;  // first entry that stays in the queue
+  my_bits >>= count;
   __syncwarp();
-  // -- B2 (backward): lane = item again; corner gradients, run-reduced by voxel, vector atomics
+  // -- B2 (backward): lane = item again; corner gradients, run-reduced by voxel, vector reductions
   if (BWD) {
     float val[11];
 #pragma unroll
     for (int c = 0; c < 11; ++c) val[c] = 0.f;
     if (lane < count) {
-      const float dtau = Q.tau[lane] * G.delta;
+      const float dtau = Q.tau[at_b] * G.delta;
       float cs[8];
       corner_sums(G, M, cs);
 #pragma unroll
       for (int c = 0; c < 8; ++c) val[c] = dtau * cs[c];
-      val[8] = Q.wg[3 * lane]; val[9] = Q.wg[3 * lane + 1]; val[10] = Q.wg[3 * lane + 2];
+      val[8] = Q.wg[0][at_b]; val[9] = Q.wg[1][at_b]; val[10] = Q.wg[2][at_b];
     }
     // items of one voxel are contiguous: segmented suffix sums, the first lane of each run ends up with the run total
 #pragma unroll
@@ -279,7 +290,7 @@ __device__ __forceinline__ void flush_batch(const CompositeArgs &A, const WarpCt
     }
     const uint32_t prev = __shfl_up_sync(0xffffffffu, my_id, 1);
     if (my_id != NONE && (lane == 0 || prev != my_id)) {
-      const TreeFrame &T = A.trees[my_meta >> 8];
+      const TreeFrame &T = A.trees[(my_meta >> 8) & 0xFFu];
       if (T.dgeo) {
         float *dg = T.dgeo + (size_t)(my_id - T.base) * 8;
         red_add_v4(dg, val[0], val[1], val[2], val[3]);
@@ -287,28 +298,10 @@ __device__ __forceinline__ void flush_batch(const CompositeArgs &A, const WarpCt
       }
       red_add_v4(A.drgb + (size_t)my_id * 4, val[8], val[9], val[10], 0.f);
     }
+    __syncwarp();
   }
-  // -- shift what is left to the queue front
-  const int rem = n_items - count;
-  const int ent_left = n_ent - j_keep;
-  uint32_t t_id = 0, t_meta = 0, t_eid = 0, t_emask = 0, t_ebase = 0;
-  float t_a = 0.f, t_b = 0.f;
-  if (lane < rem) {
-    t_id = Q.id[count + lane]; t_meta = Q.meta[count + lane]; t_a = Q.a[count + lane]; t_b = Q.b[count + lane];
-  }
-  if (lane < ent_left) {
-    t_eid = Q.e_id[j_keep + lane];
-    t_emask = Q.e_mask[j_keep + lane];
-    t_ebase = Q.e_base[j_keep + lane];
-    if (lane == 0 && strad) { t_emask = strad_mask; t_ebase = 0; }
-    else t_ebase -= (uint32_t)count;
-  }
-  __syncwarp();
-  if (lane < rem) { Q.id[lane] = t_id; Q.meta[lane] = t_meta; Q.a[lane] = t_a; Q.b[lane] = t_b; }
-  if (lane < ent_left) { Q.e_id[lane] = t_eid; Q.e_mask[lane] = t_emask; Q.e_base[lane] = t_ebase; }
-  __syncwarp();
-  n_items = rem;
-  n_ent = ent_left;
+  head = (head + count) & (QCAP - 1);
+  n_items -= count;
 }
 
 // ---- the kernel ------------------------------------------------------------------------------------------------------
@@ -318,14 +311,12 @@ __global__ void __launch_bounds__(TILE_THREADS, 2) composite_tile_kernel(const C
   const FrameParams &p = A.p;
   const int tile = blockIdx.x;
   const int warp = threadIdx.x >> 5;
-  WarpCtx W;
-  W.lane = threadIdx.x & 31;
-  W.lt = (1u << W.lane) - 1u;
-  W.u0 = (tile % p.tiles_x) * DVX_TILE + (warp & 1) * 8;
-  W.v0 = (tile / p.tiles_x) * DVX_TILE + (warp >> 1) * 4;
+  const int lane = threadIdx.x & 31;
+  const uint32_t lt = (1u << lane) - 1u;
+  const int wu0 = (tile % p.tiles_x) * DVX_TILE + (warp & 1) * 8;   // pixel of lane 0 of this warp
+  const int wv0 = (tile / p.tiles_x) * DVX_TILE + (warp >> 1) * 4;
   WarpQueue<BWD> &Q = s_queue[warp];
-  const int lane = W.lane;
-  const int u = W.u0 + (lane & 7), v = W.v0 + (lane >> 3);
+  const int u = wu0 + (lane & 7), v = wv0 + (lane >> 3);
   const bool inside = u < (int)p.width && v < (int)p.height;
   const size_t pix = (size_t)v * p.width + u;
   const bool counters = (p.flags & DVX_FLAG_COUNTERS) != 0;
@@ -343,8 +334,10 @@ __global__ void __launch_bounds__(TILE_THREADS, 2) composite_tile_kernel(const C
     S.n_stop = A.sv_nused[pix];
     if (S.n_stop == 0) S.done = true;
   }
-  const float xp = dvx_cam_x(p, u), yp = dvx_cam_y(p, v);
-  const float rn = rsqrtf(xp * xp + yp * yp + 1.0f);
+  // O1 in fp64 (once per pixel): d_cam = ((u+1/2-cx)/fx, (v+1/2-cy)/fy, 1) / |.|
+  const double xd = ((double)u + 0.5 - p.cx_d) * p.inv_fx, yd = ((double)v + 0.5 - p.cy_d) * p.inv_fy;
+  const double rnd = rsqrt(xd * xd + yd * yd + 1.0);
+  const float xp = dvx_cam_x(p, u), yp = dvx_cam_y(p, v);  // fp32 copy: only the octant decision uses it (R12)
 
   // ---- step 3: intervals of the actors in this tile's mask, insertion-sorted by (tau_in, actor index) (O2, O3)
   float h_in[DVX_MAX_ACTORS], h_out[DVX_MAX_ACTORS];
@@ -357,17 +350,29 @@ __global__ void __launch_bounds__(TILE_THREADS, 2) composite_tile_kernel(const C
       am &= am - 1;
       if (S.done) continue;
       const TreeFrame &T = A.trees[1 + i];
-      Ray r; int q;
-      make_ray(T.N, xp, yp, rn, r, q);
-      float tin, tout;
-      if (ray_box(T, r, p.near_, p.far_, tin, tout)) {
-        int j = m++;
-        while (j > 0 && h_in[j - 1] > tin) {  // ties keep the lower actor index first
-          h_in[j] = h_in[j - 1]; h_out[j] = h_out[j - 1]; h_idx[j] = h_idx[j - 1];
-          --j;
+      double lo = -1.0e300, hi = 1.0e300;
+      bool miss = false;
+#pragma unroll
+      for (int a = 0; a < 3; ++a) {
+        const double da = (T.Nd[3 * a] * xd + T.Nd[3 * a + 1] * yd + T.Nd[3 * a + 2]) * rnd;
+        const double o = T.o_l[a], hh = (double)T.half[a];
+        if (da == 0.0) {
+          miss = miss || !(o >= -hh && o < hh);
+        } else {
+          const double inv = rcp_double(da);
+          const double t1 = (-hh - o) * inv, t2 = (hh - o) * inv;
+          lo = fmax(lo, fmin(t1, t2));
+          hi = fmin(hi, fmax(t1, t2));
         }
-        h_in[j] = tin; h_out[j] = tout; h_idx[j] = (unsigned char)i;
       }
+      if (miss || !(hi > fmax(lo, (double)p.near_))) continue;
+      const float tin = (float)fmax(lo, (double)p.near_), tout = (float)fmin(hi, (double)p.far_);
+      int j = m++;
+      while (j > 0 && h_in[j - 1] > tin) {  // ties keep the lower actor index first
+        h_in[j] = h_in[j - 1]; h_out[j] = h_out[j - 1]; h_idx[j] = h_idx[j - 1];
+        --j;
+      }
+      h_in[j] = tin; h_out[j] = tout; h_idx[j] = (unsigned char)i;
     }
   }
 
@@ -376,12 +381,13 @@ __global__ void __launch_bounds__(TILE_THREADS, 2) composite_tile_kernel(const C
   int h = 0;             // next entry of the hit list
   int stage = 0;         // 0: background before hit h (or the final background), 1: actor of hit h, 2: finished
   uint32_t cur0 = NONE;  // this pixel's cursor in the static list of its octant (persists across background intervals)
-  int n_items = 0, n_ent = 0;
+  int n_items = 0, head = 0;
+  unsigned long long my_bits = 0;
   unsigned long long q_test = 0;
-  const uint32_t wu0 = (uint32_t)W.u0, wv0 = (uint32_t)W.v0, wu1 = wu0 + 7u, wv1 = wv0 + 3u;
-
+  const uint32_t ru0 = (uint32_t)wu0, rv0 = (uint32_t)wv0, ru1 = ru0 + 7u, rv1 = rv0 + 3u;
   uint32_t seg_tree = NONE;  // pending segment of this lane: tree and interval [lo, hi]
   float lo = 0.f, hi = 0.f;
+
   for (;;) {
     // -- this lane's next non-empty segment of Algorithm 1 (kept until the warp serves its tree)
     if (S.done) seg_tree = NONE;
@@ -390,27 +396,40 @@ __global__ void __launch_bounds__(TILE_THREADS, 2) composite_tile_kernel(const C
         if (h < m) {
           const float tin = h_in[h];
           stage = 1;
-          if (tin > cur) { seg_tree = 0; lo = cur; hi = tin; break; }           // background before object entry
+          if (tin > cur) { seg_tree = 0; lo = cur; hi = tin; }              // background before object entry
         } else {
           stage = 2;
-          if (p.far_ > cur) { seg_tree = 0; lo = cur; hi = p.far_; break; }     // remaining background
+          if (p.far_ > cur) { seg_tree = 0; lo = cur; hi = p.far_; }        // remaining background
         }
       } else {
         const float tin = h_in[h], tout = h_out[h];
         const float l = fmaxf(tin, cur);
-        const uint32_t t = 1u + h_idx[h];
+        const uint32_t ta = 1u + h_idx[h];
         cur = fmaxf(cur, tout);
         ++h;
         stage = 0;
-        if (tout > l) { seg_tree = t; lo = l; hi = tout; break; }                // object in its canonical local space
+        if (tout > l) { seg_tree = ta; lo = l; hi = tout; }                  // object in its canonical local space
       }
     }
     const uint32_t t = warp_min_u32(seg_tree);
     if (t == NONE) break;
     const bool part = seg_tree == t;
     const TreeFrame &T = A.trees[t];
-    Ray r; int q = 0;
-    make_ray(T.N, xp, yp, rn, r, q);
+    // ray of this pixel in the frame of tree t: fp64 direction, its fp32 rounding, reciprocal, octant, and the small
+    // difference e to the warp's reference direction d0 (= the direction of lane 0's pixel)
+    float d[3], inv[3], kinv[3], e[3];
+    double d0[3];
+    int q = 0;
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+      const double da = (T.Nd[3 * a] * xd + T.Nd[3 * a + 1] * yd + T.Nd[3 * a + 2]) * rnd;
+      d0[a] = shfl_double(da, 0);
+      e[a] = (float)(da - d0[a]);
+      d[a] = (float)da;
+      q |= (dvx_dir_comp(T.N, a, xp, yp) < 0.f) ? (4 >> a) : 0;  // R12: s_a = (d_a < 0), same fp32 formula as step 1
+      inv[a] = d[a] != 0.f ? 1.0f / d[a] : 1.0e30f;               // axis-parallel: +-1e30 puts the slab at -+infinity
+      kinv[a] = fabsf(inv[a]);
+    }
     uint32_t omask = __reduce_or_sync(0xffffffffu, part ? (1u << q) : 0u);
     while (omask) {
       const int qq = __ffs(omask) - 1;
@@ -423,57 +442,83 @@ __global__ void __launch_bounds__(TILE_THREADS, 2) composite_tile_kernel(const C
       uint32_t pos = warp_min_u32(active ? c_l : NONE);
       while (pos < end && __any_sync(0xffffffffu, active)) {
         const uint32_t n = min(32u, end - pos);
-        uint32_t id = 0;
-        float4 f0 = make_float4(0.f, 0.f, 0.f, 0.f);
+        // -- lane = entry: pre-filter and fp64 centre decomposition
         bool c = false;
         if ((uint32_t)lane < n) {
-          id = __ldg(A.ids + pos + lane);
+          const uint32_t id = __ldg(A.ids + pos + lane);
           const ushort4 rc = __ldg(A.pxrect + id);
-          f0 = __ldg(reinterpret_cast<const float4 *>(A.fvox + id));
-          c = rc.x <= wu1 && rc.z >= wu0 && rc.y <= wv1 && rc.w >= wv0;
+          c = rc.x <= ru1 && rc.z >= ru0 && rc.y <= rv1 && rc.w >= rv0;
+          if (c) {
+            uint32_t X, Y, Z, lv;
+            dvx_decode16(__ldg(T.code + (id - T.base)), X, Y, Z, lv);
+            const uint32_t size = 1u << (DVX_MAX_LEVEL - lv);
+            const double hc = 0.5 * T.cell;
+            const double cx = fma(hc, (double)(2u * X + size), T.rel0[0]);
+            const double cy = fma(hc, (double)(2u * Y + size), T.rel0[1]);
+            const double cz = fma(hc, (double)(2u * Z + size), T.rel0[2]);
+            const float t0 = (float)(cx * d0[0] + cy * d0[1] + cz * d0[2]);
+            const double t0d = (double)t0;
+            EntryRec rec;
+            rec.t0 = t0;
+            rec.m0[0] = (float)(cx - t0d * d0[0]); rec.m0[1] = (float)(cy - t0d * d0[1]); rec.m0[2] = (float)(cz - t0d * d0[2]);
+            rec.hs = (float)(hc * (double)size);
+            rec.id = id; rec.level = lv; rec.pad = 0;
+            Q.ent[lane] = rec;
+          }
         }
         uint32_t cand = __ballot_sync(0xffffffffu, c);
+        __syncwarp();
+        // -- lane = pixel
         while (cand) {
           const int j = __ffs(cand) - 1;
           cand &= cand - 1;
-          const uint32_t e = pos + j;
-          const uint32_t id_e = __shfl_sync(0xffffffffu, id, j);
-          const float rel[3] = {__shfl_sync(0xffffffffu, f0.x, j), __shfl_sync(0xffffffffu, f0.y, j),
-                                __shfl_sync(0xffffffffu, f0.z, j)};
-          const float s = __shfl_sync(0xffffffffu, f0.w, j);
+          const uint32_t ei = pos + j;
+          const float4 r0 = *reinterpret_cast<const float4 *>(&Q.ent[j]);          // t0, m0
+          const uint4 r1 = *(reinterpret_cast<const uint4 *>(&Q.ent[j]) + 1);      // hs, id, level
+          const float hs = __uint_as_float(r1.x);
           bool emit = false;
-          float ca = 0.f, cb = 0.f;
-          if (active && c_l <= e) {
-            float a, b;
+          float ca = 0.f, cb = 0.f, w0 = 0.f, w1 = 0.f, w2 = 0.f;
+          if (active && c_l <= ei) {
             if (counters) ++q_test;
-            if (slab_rel(r, rel, s, a, b) && b > a) {
-              if (a >= hi) {            // the voxel starts at or beyond the interval end: gate here
-                active = false; c_l = e;
+            w0 = fmaf(r0.x, e[0], -r0.y); w1 = fmaf(r0.x, e[1], -r0.z); w2 = fmaf(r0.x, e[2], -r0.w);
+            const float c0 = w0 * inv[0], c1 = w1 * inv[1], c2 = w2 * inv[2];
+            const float sa = fmaxf(fmaxf(fmaf(-hs, kinv[0], -c0), fmaf(-hs, kinv[1], -c1)), fmaf(-hs, kinv[2], -c2));
+            const float sb = fminf(fminf(fmaf(hs, kinv[0], -c0), fmaf(hs, kinv[1], -c1)), fmaf(hs, kinv[2], -c2));
+            if (sb > sa) {
+              const float lo_r = lo - r0.x, hi_r = hi - r0.x;
+              if (sa >= hi_r) {           // the voxel starts at or beyond the interval end: gate here
+                active = false; c_l = ei;
               } else {
-                ca = fmaxf(a, lo); cb = fminf(b, hi);   // R1: clip to the interval
+                ca = fmaxf(sa, lo_r); cb = fminf(sb, hi_r);   // R1: clip to the interval
                 emit = cb > ca;
-                if (b > hi) { active = false; c_l = e; }  // sticks out: it may own a second piece after the box
+                if (sb > hi_r) { active = false; c_l = ei; }  // sticks out: it may own a second piece after the box
               }
             }
           }
           const uint32_t mk = __ballot_sync(0xffffffffu, emit);
           if (mk) {
-            if (lane == 0) { Q.e_id[n_ent] = id_e; Q.e_mask[n_ent] = mk; Q.e_base[n_ent] = (uint32_t)n_items; }
             if (emit) {
-              const int at = n_items + __popc(mk & W.lt);
-              Q.id[at] = id_e; Q.meta[at] = (uint32_t)lane | (t << 8); Q.a[at] = ca; Q.b[at] = cb;
+              const int rel_at = n_items + __popc(mk & lt);
+              const int at = (head + rel_at) & (QCAP - 1);
+              Q.id[at] = r1.y; Q.meta[at] = (uint32_t)lane | (t << 8) | (r1.z << 16);
+              Q.ca[at] = ca; Q.cb[at] = cb;
+              Q.w[0][at] = w0; Q.w[1][at] = w1; Q.w[2][at] = w2;
+              Q.d[0][at] = d[0]; Q.d[1][at] = d[1]; Q.d[2][at] = d[2];
+              Q.mid[at] = r0.x + 0.5f * (ca + cb);
+              my_bits |= 1ull << rel_at;
             }
-            ++n_ent;
             n_items += __popc(mk);
             if (n_items >= 32) {
-              flush_batch<BWD>(A, W, Q, n_items, n_ent, S);
+              flush_batch<BWD>(A, lane, Q, n_items, head, my_bits, S);
               active = active && !S.done;
             }
           }
           if (!__any_sync(0xffffffffu, active)) break;
         }
+        __syncwarp();
         pos += 32;
       }
+      if (counters && A.eff_end && lane == 0) atomicMax(A.eff_end + bucket, min(pos, end));
       if (part && q == qq) {
         if (active) c_l = end;          // walked off the list: nothing left for later intervals either
         if (t == 0) cur0 = c_l;
@@ -481,7 +526,7 @@ __global__ void __launch_bounds__(TILE_THREADS, 2) composite_tile_kernel(const C
     }
     if (part) seg_tree = NONE;          // served
   }
-  while (n_items > 0) flush_batch<BWD>(A, W, Q, n_items, n_ent, S);
+  while (n_items > 0) flush_batch<BWD>(A, lane, Q, n_items, head, my_bits, S);
 
   if (!BWD && inside) {
     A.rgb[3 * pix] = S.C0; A.rgb[3 * pix + 1] = S.C1; A.rgb[3 * pix + 2] = S.C2;

@@ -22,6 +22,7 @@ struct TreeFrame {
   double rel0[3];        // lo - o_l: cube min corner relative to the camera origin (tree frame)
   double Nd[9];          // R_o^T R_c in fp64 (N below is its fp32 rounding)
   float ol_f[3];         // o_l rounded to fp32 (debug walker's ray-OBB test only)
+  float inv_cell_f;      // 1 / cell rounded to fp32
   float N[9];            // R_o^T R_c: d_l[a] = N[3a] x' + N[3a+1] y' + N[3a+2];  p_cam[c] = sum_a N[3a+c] rel[a]
   float half[3];         // OBB half extents (actors)
   int box_rect[4];       // pixel rectangle of the OBB (x0,y0,x1,y1 inclusive; x1<x0 = not visible); set on device
@@ -32,7 +33,7 @@ struct FrameParams {
   float fx, fy, cx, cy, near_, far_, zclip;
   double inv_fx, inv_fy, cx_d, cy_d;  // fp64 copies for the per-pixel ray set-up of the tile kernel
   uint32_t k_samples, activation, flags;
-  float t_stop;
+  float t_stop, inv_k;  // inv_k = 1 / k_samples
   uint32_t rank_bits;   // sort key = (bucket << rank_bits) | rank ; bucket = (tile*n_trees + tree)*8 + octant
   uint32_t v_total;     // sum of n_voxels
   uint32_t n_buckets;   // n_tiles * n_trees * 8
@@ -62,6 +63,7 @@ struct CompositeArgs {
   float *sv_T;                 // [H*W]
   uint32_t *sv_nused;          // [H*W]
   unsigned long long *counters;
+  uint32_t *eff_end;           // [n_buckets] furthest list position any warp streamed (DVX_FLAG_COUNTERS only, else NULL)
   // backward
   const float *g_rgb, *g_depth, *g_alpha;
   float *drgb;                 // [v_total][4] scratch: dL/drgb_v
