@@ -30,6 +30,9 @@ namespace {
 
 constexpr int TILE_THREADS = 256;
 constexpr int TILE_WARPS = TILE_THREADS / 32;
+#ifndef DVX_TILE_MIN_CTAS
+#define DVX_TILE_MIN_CTAS 3
+#endif
 constexpr int QCAP = 64;              // ring capacity per warp: at most 31 left-over items + 32 of one entry
 constexpr uint32_t NONE = 0xFFFFFFFFu;
 constexpr float LOG2E = 1.4426950408889634f;
@@ -44,17 +47,22 @@ struct __align__(16) EntryRec {
   uint32_t pad;
 };
 
+// One queued (pixel, voxel) hit: 48 bytes, written with three 16-byte stores in phase A.
+struct __align__(16) Item {
+  uint32_t id;        // global voxel id
+  uint32_t meta;      // pixel lane | tree << 8 | level << 16
+  float ca, cb;       // clipped sub-segment, relative to t0 (O4, R1)
+  float w[3];         // x(tau) - centre = s' d + w
+  float mid;          // (a + b) / 2, absolute ray distance (depth, R9)
+  float d[3];         // ray direction in the tree frame
+  float tau;          // phase B: tau_v;  backward phase C overwrites it with dL/dtau_v
+};
+
 template <bool BWD>
 struct WarpQueue {
   EntryRec ent[32];
-  // items (ring of QCAP)
-  uint32_t id[QCAP];
-  uint32_t meta[QCAP];     // pixel lane | tree << 8 | level << 16
-  float ca[QCAP], cb[QCAP];  // clipped sub-segment, relative to t0 (O4, R1)
-  float w[3][QCAP];        // x(tau) - centre = s' d + w
-  float d[3][QCAP];        // ray direction in the tree frame
-  float mid[QCAP];         // (a + b) / 2, absolute ray distance (depth, R9)
-  float tau[QCAP];         // phase B: tau_v;  backward phase C overwrites it with dL/dtau_v
+  Item item[QCAP];              // ring
+  double d0[3];                 // the warp's reference direction for the list being served
   float wg[BWD ? 3 : 1][QCAP];  // backward phase C: T alpha g_C per item, zero where the colour clamp is active
 };
 
@@ -116,8 +124,10 @@ struct ItemGeom {
 // O6 for one queued item (ring slot `at`): K-point midpoint rule on the clipped segment.  Returns tau_v; with GRAD also
 // the moments M_j = sum_k act'(raw_k) lambda_k^j (j = 0..3), from which phase B2 rebuilds sum_k act'(raw_k) w_c(u_k).
 template <bool BWD>
-__device__ __forceinline__ float integrate_item(const CompositeArgs &A, const WarpQueue<BWD> &Q, int at, uint32_t id,
-                                                uint32_t meta, ItemGeom &G, float M[4]) {
+__device__ __forceinline__ float integrate_item(const CompositeArgs &A, const WarpQueue<BWD> &Q, int at, uint32_t &id,
+                                                uint32_t &meta, ItemGeom &G, float M[4]) {
+  id = Q.item[at].id;
+  meta = Q.item[at].meta;
   const TreeFrame &T = A.trees[(meta >> 8) & 0xFFu];
   const uint32_t level = meta >> 16;
   const float4 *gp = reinterpret_cast<const float4 *>(T.geo + (size_t)(id - T.base) * 8);
@@ -125,10 +135,14 @@ __device__ __forceinline__ float integrate_item(const CompositeArgs &A, const Wa
   const float g[8] = {g0.x, g0.y, g0.z, g0.w, g1.x, g1.y, g1.z, g1.w};
   // 1 / edge length = (1 / level-16 cell) * 2^(level - 16): exact power-of-two scaling
   const float inv_s = T.inv_cell_f * __uint_as_float((111u + level) << 23);
-  const float ca = Q.ca[at], cb = Q.cb[at];
+  const float4 i0 = *reinterpret_cast<const float4 *>(&Q.item[at]);        // id, meta, ca, cb
+  const float4 i1 = *(reinterpret_cast<const float4 *>(&Q.item[at]) + 1);  // w, mid
+  const float4 i2 = *(reinterpret_cast<const float4 *>(&Q.item[at]) + 2);  // d, tau
+  const float ca = i0.z, cb = i0.w;
+  const float dd[3] = {i2.x, i2.y, i2.z}, ww[3] = {i1.x, i1.y, i1.z};
 #pragma unroll
   for (int ax = 0; ax < 3; ++ax) {
-    const float d = Q.d[ax][at], w = Q.w[ax][at];
+    const float d = dd[ax], w = ww[ax];
     const float pa = __saturatef(fmaf(fmaf(ca, d, w), inv_s, 0.5f));   // u clamped to [0,1]^3 (O6)
     const float pb = __saturatef(fmaf(fmaf(cb, d, w), inv_s, 0.5f));
     G.p[ax] = pa;
@@ -142,9 +156,23 @@ __device__ __forceinline__ float integrate_item(const CompositeArgs &A, const Wa
   float S = 0.f;
   if (BWD) M[0] = M[1] = M[2] = M[3] = 0.f;
   float lam = 0.5f * invK;
-  if (kind == 0) {  // exp: sigma = ex2(raw * log2 e), act' = act
+  if (kind == 0 && K == 8) {  // the configured case: exp, 8 samples at lambda = (k + 1/2) / 8 as immediates
     const float c0 = c[0] * LOG2E, c1 = c[1] * LOG2E, c2 = c[2] * LOG2E, c3 = c[3] * LOG2E;
-#pragma unroll 8
+#pragma unroll
+    for (int k = 0; k < 8; ++k) {
+      const float l8 = (float)(2 * k + 1) * 0.0625f;
+      const float sig = ex2_approx(fmaf(fmaf(fmaf(c3, l8, c2), l8, c1), l8, c0));
+      S += sig;
+      if (BWD) {
+        M[0] += sig;
+        float t = sig * l8; M[1] += t;
+        t *= l8; M[2] += t;
+        t *= l8; M[3] += t;
+      }
+    }
+  } else if (kind == 0) {  // exp: sigma = ex2(raw * log2 e), act' = act
+    const float c0 = c[0] * LOG2E, c1 = c[1] * LOG2E, c2 = c[2] * LOG2E, c3 = c[3] * LOG2E;
+#pragma unroll 4
     for (uint32_t k = 0; k < K; ++k) {
       const float sig = ex2_approx(fmaf(fmaf(fmaf(c3, lam, c2), lam, c1), lam, c0));
       S += sig;
@@ -218,11 +246,7 @@ __device__ __forceinline__ void flush_batch(const CompositeArgs &A, int lane, Wa
   float M[4];
   uint32_t my_id = NONE, my_meta = 0;
   const int at_b = (head + lane) & (QCAP - 1);
-  if (lane < count) {
-    my_id = Q.id[at_b];
-    my_meta = Q.meta[at_b];
-    Q.tau[at_b] = integrate_item<BWD>(A, Q, at_b, my_id, my_meta, G, M);
-  }
+  if (lane < count) Q.item[at_b].tau = integrate_item<BWD>(A, Q, at_b, my_id, my_meta, G, M);
   __syncwarp();
   // -- C: lane = pixel; its own items of the batch in queue order = front-to-back order along its ray
   uint32_t mine = (uint32_t)my_bits;
@@ -232,9 +256,9 @@ __device__ __forceinline__ void flush_batch(const CompositeArgs &A, int lane, Wa
     mine &= mine - 1;
     const int at = (head + i) & (QCAP - 1);
     if (!S.done) {
-      const float4 f1 = __ldg(reinterpret_cast<const float4 *>(A.fvox + Q.id[at]) + 1);
-      const float tau = Q.tau[at];
-      const float mid = Q.mid[at];
+      const float4 f1 = __ldg(reinterpret_cast<const float4 *>(A.fvox + Q.item[at].id) + 1);
+      const float tau = Q.item[at].tau;
+      const float mid = Q.item[at].mid;
       const float e = ex2_approx(-tau * LOG2E);
       const float alpha = tau < 1e-3f ? tau * fmaf(-0.5f, tau, 1.0f) : 1.0f - e;  // 1 - exp(-tau) without cancellation
       const float w = S.T * alpha;
@@ -244,7 +268,7 @@ __device__ __forceinline__ void flush_batch(const CompositeArgs &A, int lane, Wa
       } else {
         const float X = S.gC0 * f1.x + S.gC1 * f1.y + S.gC2 * f1.z + S.gD * mid;
         S.Xpre = fmaf(w, X, S.Xpre);
-        Q.tau[at] = S.T * e * X - (S.Xtot - S.Xpre) + S.gA * S.T_final;  // dL/dtau_v
+        Q.item[at].tau = S.T * e * X - (S.Xtot - S.Xpre) + S.gA * S.T_final;  // dL/dtau_v
         const uint32_t cm = __float_as_uint(f1.w);
         Q.wg[0][at] = (cm & 1u) ? 0.f : w * S.gC0;
         Q.wg[1][at] = (cm & 2u) ? 0.f : w * S.gC1;
@@ -258,7 +282,7 @@ __device__ __forceinline__ void flush_batch(const CompositeArgs &A, int lane, Wa
         if (S.n_used >= S.n_stop) S.done = true;
       }
     } else if (BWD) {  // queued before this pixel finished its replay: contributes nothing
-      Q.tau[at] = 0.f;
+      Q.item[at].tau = 0.f;
       Q.wg[0][at] = 0.f; Q.wg[1][at] = 0.f; Q.wg[2][at] = 0.f;
     }
   }
@@ -270,7 +294,7 @@ __device__ __forceinline__ void flush_batch(const CompositeArgs &A, int lane, Wa
 #pragma unroll
     for (int c = 0; c < 11; ++c) val[c] = 0.f;
     if (lane < count) {
-      const float dtau = Q.tau[at_b] * G.delta;
+      const float dtau = Q.item[at_b].tau * G.delta;
       float cs[8];
       corner_sums(G, M, cs);
 #pragma unroll
@@ -305,8 +329,16 @@ __device__ __forceinline__ void flush_batch(const CompositeArgs &A, int lane, Wa
 }
 
 // ---- the kernel ------------------------------------------------------------------------------------------------------
-template <bool BWD>
-__global__ void __launch_bounds__(TILE_THREADS, 2) composite_tile_kernel(const CompositeArgs A) {
+// Per-pixel ray in fp64 (O1): d_cam = ((u+1/2-cx)/fx, (v+1/2-cy)/fy, 1) / |.|.  Recomputed where needed (once per served
+// list) instead of being held in six registers.
+__device__ __forceinline__ void pixel_ray_d(const FrameParams &p, int u, int v, double &xd, double &yd, double &rnd) {
+  xd = ((double)u + 0.5 - p.cx_d) * p.inv_fx;
+  yd = ((double)v + 0.5 - p.cy_d) * p.inv_fy;
+  rnd = rsqrt(xd * xd + yd * yd + 1.0);
+}
+
+template <bool BWD, bool CNT>
+__global__ void __launch_bounds__(TILE_THREADS, DVX_TILE_MIN_CTAS) composite_tile_kernel(const CompositeArgs A) {
   __shared__ WarpQueue<BWD> s_queue[TILE_WARPS];
   const FrameParams &p = A.p;
   const int tile = blockIdx.x;
@@ -319,7 +351,6 @@ __global__ void __launch_bounds__(TILE_THREADS, 2) composite_tile_kernel(const C
   const int u = wu0 + (lane & 7), v = wv0 + (lane >> 3);
   const bool inside = u < (int)p.width && v < (int)p.height;
   const size_t pix = (size_t)v * p.width + u;
-  const bool counters = (p.flags & DVX_FLAG_COUNTERS) != 0;
 
   Pix S;
   S.C0 = S.C1 = S.C2 = 0.f; S.D = 0.f; S.T = 1.f; S.n_used = 0; S.done = !inside;
@@ -334,10 +365,6 @@ __global__ void __launch_bounds__(TILE_THREADS, 2) composite_tile_kernel(const C
     S.n_stop = A.sv_nused[pix];
     if (S.n_stop == 0) S.done = true;
   }
-  // O1 in fp64 (once per pixel): d_cam = ((u+1/2-cx)/fx, (v+1/2-cy)/fy, 1) / |.|
-  const double xd = ((double)u + 0.5 - p.cx_d) * p.inv_fx, yd = ((double)v + 0.5 - p.cy_d) * p.inv_fy;
-  const double rnd = rsqrt(xd * xd + yd * yd + 1.0);
-  const float xp = dvx_cam_x(p, u), yp = dvx_cam_y(p, v);  // fp32 copy: only the octant decision uses it (R12)
 
   // ---- step 3: intervals of the actors in this tile's mask, insertion-sorted by (tau_in, actor index) (O2, O3)
   float h_in[DVX_MAX_ACTORS], h_out[DVX_MAX_ACTORS];
@@ -345,34 +372,38 @@ __global__ void __launch_bounds__(TILE_THREADS, 2) composite_tile_kernel(const C
   int m = 0;
   {
     unsigned long long am = A.actor_mask[tile];
-    while (am) {
-      const int i = __ffsll((long long)am) - 1;
-      am &= am - 1;
-      if (S.done) continue;
-      const TreeFrame &T = A.trees[1 + i];
-      double lo = -1.0e300, hi = 1.0e300;
-      bool miss = false;
+    if (am) {
+      double xd, yd, rnd;
+      pixel_ray_d(p, u, v, xd, yd, rnd);
+      while (am) {
+        const int i = __ffsll((long long)am) - 1;
+        am &= am - 1;
+        if (S.done) continue;
+        const TreeFrame &T = A.trees[1 + i];
+        double lo = -1.0e300, hi = 1.0e300;
+        bool miss = false;
 #pragma unroll
-      for (int a = 0; a < 3; ++a) {
-        const double da = (T.Nd[3 * a] * xd + T.Nd[3 * a + 1] * yd + T.Nd[3 * a + 2]) * rnd;
-        const double o = T.o_l[a], hh = (double)T.half[a];
-        if (da == 0.0) {
-          miss = miss || !(o >= -hh && o < hh);
-        } else {
-          const double inv = rcp_double(da);
-          const double t1 = (-hh - o) * inv, t2 = (hh - o) * inv;
-          lo = fmax(lo, fmin(t1, t2));
-          hi = fmin(hi, fmax(t1, t2));
+        for (int a = 0; a < 3; ++a) {
+          const double da = (T.Nd[3 * a] * xd + T.Nd[3 * a + 1] * yd + T.Nd[3 * a + 2]) * rnd;
+          const double o = T.o_l[a], hh = (double)T.half[a];
+          if (da == 0.0) {
+            miss = miss || !(o >= -hh && o < hh);
+          } else {
+            const double inv = rcp_double(da);
+            const double t1 = (-hh - o) * inv, t2 = (hh - o) * inv;
+            lo = fmax(lo, fmin(t1, t2));
+            hi = fmin(hi, fmax(t1, t2));
+          }
         }
+        if (miss || !(hi > fmax(lo, (double)p.near_))) continue;
+        const float tin = (float)fmax(lo, (double)p.near_), tout = (float)fmin(hi, (double)p.far_);
+        int j = m++;
+        while (j > 0 && h_in[j - 1] > tin) {  // ties keep the lower actor index first
+          h_in[j] = h_in[j - 1]; h_out[j] = h_out[j - 1]; h_idx[j] = h_idx[j - 1];
+          --j;
+        }
+        h_in[j] = tin; h_out[j] = tout; h_idx[j] = (unsigned char)i;
       }
-      if (miss || !(hi > fmax(lo, (double)p.near_))) continue;
-      const float tin = (float)fmax(lo, (double)p.near_), tout = (float)fmin(hi, (double)p.far_);
-      int j = m++;
-      while (j > 0 && h_in[j - 1] > tin) {  // ties keep the lower actor index first
-        h_in[j] = h_in[j - 1]; h_out[j] = h_out[j - 1]; h_idx[j] = h_idx[j - 1];
-        --j;
-      }
-      h_in[j] = tin; h_out[j] = tout; h_idx[j] = (unsigned char)i;
     }
   }
 
@@ -416,19 +447,25 @@ __global__ void __launch_bounds__(TILE_THREADS, 2) composite_tile_kernel(const C
     const bool part = seg_tree == t;
     const TreeFrame &T = A.trees[t];
     // ray of this pixel in the frame of tree t: fp64 direction, its fp32 rounding, reciprocal, octant, and the small
-    // difference e to the warp's reference direction d0 (= the direction of lane 0's pixel)
-    float d[3], inv[3], kinv[3], e[3];
-    double d0[3];
+    // difference e to the warp's reference direction d0 (= the direction of lane 0's pixel, kept in shared memory)
+    float d[3], inv[3], e[3];
     int q = 0;
+    {
+      double xd, yd, rnd;
+      pixel_ray_d(p, u, v, xd, yd, rnd);
+      const float xp = dvx_cam_x(p, u), yp = dvx_cam_y(p, v);  // fp32 copy: only the octant decision uses it (R12)
+      __syncwarp();
 #pragma unroll
-    for (int a = 0; a < 3; ++a) {
-      const double da = (T.Nd[3 * a] * xd + T.Nd[3 * a + 1] * yd + T.Nd[3 * a + 2]) * rnd;
-      d0[a] = shfl_double(da, 0);
-      e[a] = (float)(da - d0[a]);
-      d[a] = (float)da;
-      q |= (dvx_dir_comp(T.N, a, xp, yp) < 0.f) ? (4 >> a) : 0;  // R12: s_a = (d_a < 0), same fp32 formula as step 1
-      inv[a] = d[a] != 0.f ? 1.0f / d[a] : 1.0e30f;               // axis-parallel: +-1e30 puts the slab at -+infinity
-      kinv[a] = fabsf(inv[a]);
+      for (int a = 0; a < 3; ++a) {
+        const double da = (T.Nd[3 * a] * xd + T.Nd[3 * a + 1] * yd + T.Nd[3 * a + 2]) * rnd;
+        const double d0a = shfl_double(da, 0);
+        if (lane == 0) Q.d0[a] = d0a;
+        e[a] = (float)(da - d0a);
+        d[a] = (float)da;
+        q |= (dvx_dir_comp(T.N, a, xp, yp) < 0.f) ? (4 >> a) : 0;  // R12: s_a = (d_a < 0), same fp32 formula as step 1
+        inv[a] = d[a] != 0.f ? 1.0f / d[a] : 1.0e30f;               // axis-parallel: +-1e30 puts the slab at -+infinity
+      }
+      __syncwarp();
     }
     uint32_t omask = __reduce_or_sync(0xffffffffu, part ? (1u << q) : 0u);
     while (omask) {
@@ -436,11 +473,11 @@ __global__ void __launch_bounds__(TILE_THREADS, 2) composite_tile_kernel(const C
       omask &= omask - 1;
       const size_t bucket = ((size_t)tile * p.n_trees + t) * 8 + qq;
       const uint32_t beg = __ldg(A.range_beg + bucket), end = __ldg(A.range_end + bucket);
-      bool active = part && q == qq;
+      uint32_t active = (part && q == qq) ? 1u : 0u;
       uint32_t c_l = beg;
       if (t == 0 && cur0 != NONE) c_l = cur0;
       uint32_t pos = warp_min_u32(active ? c_l : NONE);
-      while (pos < end && __any_sync(0xffffffffu, active)) {
+      while (pos < end && __any_sync(0xffffffffu, active != 0u)) {
         const uint32_t n = min(32u, end - pos);
         // -- lane = entry: pre-filter and fp64 centre decomposition
         bool c = false;
@@ -453,14 +490,15 @@ __global__ void __launch_bounds__(TILE_THREADS, 2) composite_tile_kernel(const C
             dvx_decode16(__ldg(T.code + (id - T.base)), X, Y, Z, lv);
             const uint32_t size = 1u << (DVX_MAX_LEVEL - lv);
             const double hc = 0.5 * T.cell;
+            const double d0x = Q.d0[0], d0y = Q.d0[1], d0z = Q.d0[2];
             const double cx = fma(hc, (double)(2u * X + size), T.rel0[0]);
             const double cy = fma(hc, (double)(2u * Y + size), T.rel0[1]);
             const double cz = fma(hc, (double)(2u * Z + size), T.rel0[2]);
-            const float t0 = (float)(cx * d0[0] + cy * d0[1] + cz * d0[2]);
+            const float t0 = (float)(cx * d0x + cy * d0y + cz * d0z);
             const double t0d = (double)t0;
             EntryRec rec;
             rec.t0 = t0;
-            rec.m0[0] = (float)(cx - t0d * d0[0]); rec.m0[1] = (float)(cy - t0d * d0[1]); rec.m0[2] = (float)(cz - t0d * d0[2]);
+            rec.m0[0] = (float)(cx - t0d * d0x); rec.m0[1] = (float)(cy - t0d * d0y); rec.m0[2] = (float)(cz - t0d * d0z);
             rec.hs = (float)(hc * (double)size);
             rec.id = id; rec.level = lv; rec.pad = 0;
             Q.ent[lane] = rec;
@@ -476,49 +514,38 @@ __global__ void __launch_bounds__(TILE_THREADS, 2) composite_tile_kernel(const C
           const float4 r0 = *reinterpret_cast<const float4 *>(&Q.ent[j]);          // t0, m0
           const uint4 r1 = *(reinterpret_cast<const uint4 *>(&Q.ent[j]) + 1);      // hs, id, level
           const float hs = __uint_as_float(r1.x);
-          bool emit = false;
-          float ca = 0.f, cb = 0.f, w0 = 0.f, w1 = 0.f, w2 = 0.f;
-          if (active && c_l <= ei) {
-            if (counters) ++q_test;
-            w0 = fmaf(r0.x, e[0], -r0.y); w1 = fmaf(r0.x, e[1], -r0.z); w2 = fmaf(r0.x, e[2], -r0.w);
-            const float c0 = w0 * inv[0], c1 = w1 * inv[1], c2 = w2 * inv[2];
-            const float sa = fmaxf(fmaxf(fmaf(-hs, kinv[0], -c0), fmaf(-hs, kinv[1], -c1)), fmaf(-hs, kinv[2], -c2));
-            const float sb = fminf(fminf(fmaf(hs, kinv[0], -c0), fmaf(hs, kinv[1], -c1)), fmaf(hs, kinv[2], -c2));
-            if (sb > sa) {
-              const float lo_r = lo - r0.x, hi_r = hi - r0.x;
-              if (sa >= hi_r) {           // the voxel starts at or beyond the interval end: gate here
-                active = false; c_l = ei;
-              } else {
-                ca = fmaxf(sa, lo_r); cb = fminf(sb, hi_r);   // R1: clip to the interval
-                emit = cb > ca;
-                if (sb > hi_r) { active = false; c_l = ei; }  // sticks out: it may own a second piece after the box
-              }
-            }
-          }
+          const float w0 = fmaf(r0.x, e[0], -r0.y), w1 = fmaf(r0.x, e[1], -r0.z), w2 = fmaf(r0.x, e[2], -r0.w);
+          const float c0 = w0 * inv[0], c1 = w1 * inv[1], c2 = w2 * inv[2];
+          const float sa = fmaxf(fmaxf(fmaf(-hs, fabsf(inv[0]), -c0), fmaf(-hs, fabsf(inv[1]), -c1)), fmaf(-hs, fabsf(inv[2]), -c2));
+          const float sb = fminf(fminf(fmaf(hs, fabsf(inv[0]), -c0), fmaf(hs, fabsf(inv[1]), -c1)), fmaf(hs, fabsf(inv[2]), -c2));
+          const float lo_r = lo - r0.x, hi_r = hi - r0.x;
+          const float ca = fmaxf(sa, lo_r), cb = fminf(sb, hi_r);       // R1: clip to the interval
+          const bool live = active != 0u && c_l <= ei && sb > sa;       // this pixel's ray meets the voxel
+          const bool emit = live && cb > ca;
+          if (CNT) q_test += (active != 0u && c_l <= ei) ? 1u : 0u;
+          // gate: the voxel reaches beyond the interval end (it may own a second piece after the box), or starts beyond it
+          if (live && sb > hi_r) { active = 0u; c_l = ei; }
           const uint32_t mk = __ballot_sync(0xffffffffu, emit);
           if (mk) {
             if (emit) {
               const int rel_at = n_items + __popc(mk & lt);
-              const int at = (head + rel_at) & (QCAP - 1);
-              Q.id[at] = r1.y; Q.meta[at] = (uint32_t)lane | (t << 8) | (r1.z << 16);
-              Q.ca[at] = ca; Q.cb[at] = cb;
-              Q.w[0][at] = w0; Q.w[1][at] = w1; Q.w[2][at] = w2;
-              Q.d[0][at] = d[0]; Q.d[1][at] = d[1]; Q.d[2][at] = d[2];
-              Q.mid[at] = r0.x + 0.5f * (ca + cb);
+              float4 *it = reinterpret_cast<float4 *>(&Q.item[(head + rel_at) & (QCAP - 1)]);
+              it[0] = make_float4(__uint_as_float(r1.y), __uint_as_float((uint32_t)lane | (t << 8) | (r1.z << 16)), ca, cb);
+              it[1] = make_float4(w0, w1, w2, r0.x + 0.5f * (ca + cb));
+              it[2] = make_float4(d[0], d[1], d[2], 0.f);
               my_bits |= 1ull << rel_at;
             }
             n_items += __popc(mk);
             if (n_items >= 32) {
               flush_batch<BWD>(A, lane, Q, n_items, head, my_bits, S);
-              active = active && !S.done;
+              if (S.done) active = 0u;
             }
           }
-          if (!__any_sync(0xffffffffu, active)) break;
         }
         __syncwarp();
         pos += 32;
       }
-      if (counters && A.eff_end && lane == 0) atomicMax(A.eff_end + bucket, min(pos, end));
+      if (CNT && A.eff_end && lane == 0) atomicMax(A.eff_end + bucket, min(pos, end));
       if (part && q == qq) {
         if (active) c_l = end;          // walked off the list: nothing left for later intervals either
         if (t == 0) cur0 = c_l;
@@ -538,7 +565,7 @@ __global__ void __launch_bounds__(TILE_THREADS, 2) composite_tile_kernel(const C
       A.sv_nused[pix] = S.n_used;
     }
   }
-  if (counters && !BWD) {
+  if (CNT && !BWD) {
     unsigned long long qt = q_test, qh = S.n_used;
     for (int o = 16; o > 0; o >>= 1) {
       qt += __shfl_xor_sync(0xffffffffu, qt, o);
@@ -556,8 +583,11 @@ __global__ void __launch_bounds__(TILE_THREADS, 2) composite_tile_kernel(const C
 void dvx_composite_tile_launch(const CompositeArgs &a, bool backward, cudaStream_t st) {
   if (a.p.n_tiles == 0) return;
   DVX_COUNT_LAUNCH(1);
+  const bool cnt = (a.p.flags & DVX_FLAG_COUNTERS) != 0;
   if (backward)
-    composite_tile_kernel<true><<<a.p.n_tiles, TILE_THREADS, 0, st>>>(a);
+    composite_tile_kernel<true, false><<<a.p.n_tiles, TILE_THREADS, 0, st>>>(a);
+  else if (cnt)
+    composite_tile_kernel<false, true><<<a.p.n_tiles, TILE_THREADS, 0, st>>>(a);
   else
-    composite_tile_kernel<false><<<a.p.n_tiles, TILE_THREADS, 0, st>>>(a);
+    composite_tile_kernel<false, false><<<a.p.n_tiles, TILE_THREADS, 0, st>>>(a);
 }
