@@ -39,6 +39,8 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing leg (profiling runs)")
     ap.add_argument("--cpu-tiles", type=int, default=0, help="tiles in the CPU-oracle sample (0 = pick for about 10-30 s)")
     ap.add_argument("--fwd-only", action="store_true", help="profiling aid: time dvx_render alone")
+    ap.add_argument("--profiler-range", action="store_true",
+                    help="bracket the first timed region with cudaProfilerStart/Stop (use with ncu --profile-from-start off)")
     return ap.parse_args()
 
 
@@ -243,7 +245,12 @@ def run_dvx(args):
     ctx.stage_ms_collect()                       # drop the stage times of the warm-up frames
     l0 = ctx.lib.dvx_launch_count()
     sampler = ClockSampler(local) if rank == 0 else None
+    if args.profiler_range:
+        torch.cuda.synchronize()
+        torch.cuda.cudart().cudaProfilerStart()
     ms_total = timed(args.steps, bwd=not args.fwd_only)
+    if args.profiler_range:
+        torch.cuda.cudart().cudaProfilerStop()
     launches = int(ctx.lib.dvx_launch_count() - l0)
     sums, n_frames = ctx.stage_ms_collect()      # CUDA-event stage times of exactly the timed steps (on the ctx stream)
     stage = {k: v / args.steps for k, v in sums.items()}

@@ -283,13 +283,16 @@ __global__ void ranges_kernel(const uint64_t *keys, uint64_t n, uint32_t rank_bi
 }
 
 // ------------------------------------------------------------------ step 5b: dL/dk_{v,i} = Y_i(dir_v) dL/drgb_v
+// SH degree 3 (the configured case): four threads per voxel, thread j owns coefficients 4j..4j+3 = 12 consecutive floats,
+// so a quad reads and writes the voxel's 192 contiguous bytes with 16-byte accesses.  Other degrees: one thread per voxel.
 __global__ void __launch_bounds__(PRE_THREADS) sh_backward_kernel(FrameParams p, const TreeFrame *trees,
                                                                   const FrameVox *fvox, const ushort4 *pxrect,
                                                                   const float *drgb) {
   __shared__ uint32_t s_base[DVX_MAX_TREES + 1];
   for (int i = threadIdx.x; i < (int)p.n_trees; i += blockDim.x) s_base[i] = trees[i].base;
   __syncthreads();
-  uint32_t g = blockIdx.x * blockDim.x + threadIdx.x;
+  const uint32_t gt = blockIdx.x * blockDim.x + threadIdx.x;
+  const uint32_t g = gt >> 2, part = gt & 3u;
   if (g >= p.v_total) return;
   ushort4 r = pxrect[g];
   if (r.x > r.z) return;
@@ -298,6 +301,7 @@ __global__ void __launch_bounds__(PRE_THREADS) sh_backward_kernel(FrameParams p,
   int t = find_tree(s_base, p.n_trees, g);
   const TreeFrame &T = trees[t];
   if (!T.dsh) return;
+  if (T.n_sh != 16 && part != 0) return;
   FrameVox fv = fvox[g];
   float dx = fv.rel[0] + 0.5f * fv.s, dy = fv.rel[1] + 0.5f * fv.s, dz = fv.rel[2] + 0.5f * fv.s;
   float inv = rsqrtf(dx * dx + dy * dy + dz * dz);
@@ -305,10 +309,28 @@ __global__ void __launch_bounds__(PRE_THREADS) sh_backward_kernel(FrameParams p,
   dvx_sh_basis(dx * inv, dy * inv, dz * inv, Y, (int)T.n_sh);
   float gch[3] = {(fv.meta & 1u) ? 0.f : d.x, (fv.meta & 2u) ? 0.f : d.y, (fv.meta & 4u) ? 0.f : d.z};
   float *out = T.dsh + (size_t)(g - s_base[t]) * T.n_sh * 3;
-  for (int i = 0; i < (int)T.n_sh; ++i) {
-    out[3 * i] += Y[i] * gch[0];
-    out[3 * i + 1] += Y[i] * gch[1];
-    out[3 * i + 2] += Y[i] * gch[2];
+  if (T.n_sh == 16) {
+    float y[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) y[k] = part == 0 ? Y[k] : part == 1 ? Y[4 + k] : part == 2 ? Y[8 + k] : Y[12 + k];
+    float v[12];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+      v[3 * k] = y[k] * gch[0]; v[3 * k + 1] = y[k] * gch[1]; v[3 * k + 2] = y[k] * gch[2];
+    }
+    float4 *o4 = reinterpret_cast<float4 *>(out) + 3 * part;
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+      float4 x = o4[k];
+      x.x += v[4 * k]; x.y += v[4 * k + 1]; x.z += v[4 * k + 2]; x.w += v[4 * k + 3];
+      o4[k] = x;
+    }
+  } else {
+    for (int i = 0; i < (int)T.n_sh; ++i) {
+      out[3 * i] += Y[i] * gch[0];
+      out[3 * i + 1] += Y[i] * gch[1];
+      out[3 * i + 2] += Y[i] * gch[2];
+    }
   }
 }
 
@@ -349,5 +371,5 @@ void dvx_ranges_launch(const uint64_t *keys, uint64_t n, uint32_t rank_bits, uin
 }
 void dvx_sh_backward_launch(const FrameParams &p, const TreeFrame *trees, const FrameVox *fvox, const ushort4 *pxrect,
                             const float *drgb, cudaStream_t st) {
-    if (p.v_total) { DVX_COUNT_LAUNCH(1); sh_backward_kernel<<<blocks_for(p.v_total, PRE_THREADS), PRE_THREADS, 0, st>>>(p, trees, fvox, pxrect, drgb); }
+    if (p.v_total) { DVX_COUNT_LAUNCH(1); sh_backward_kernel<<<blocks_for(4ull * p.v_total, PRE_THREADS), PRE_THREADS, 0, st>>>(p, trees, fvox, pxrect, drgb); }
 }

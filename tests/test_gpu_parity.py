@@ -20,16 +20,35 @@ def ctx():
     c.close()
 
 
-def _check_images(rgb, depth, alpha, ref, mask=None):
+def _pixel_errors(rgb, depth, alpha, ref):
+    e_rgb = np.abs(rgb - ref["rgb"]).max(-1) / RGB_TOL
+    e_a = np.abs(alpha - ref["alpha"]) / RGB_TOL
+    e_d = np.abs(depth - ref["depth"]) / np.maximum(np.abs(ref["depth"]), 1.0) / DEPTH_REL
+    return np.maximum(np.maximum(e_rgb, e_a), e_d)   # > 1 = out of tolerance
+
+
+def _check_images(rgb, depth, alpha, ref, mask=None, scene=None):
+    """Every compared pixel must be within the tolerances of R16.  A pixel may instead be *threshold-ambiguous* (DESIGN.md
+    section 3): its transmittance passes within fp32 rounding of t_stop, so stopping one voxel earlier or later are both
+    valid; that is established with the oracle alone (its own result changes under t_stop (1 +- 2e-3)) and the GPU result must
+    then match one of the two oracle outcomes.  Returns the number of such pixels (at most 1e-4 of the sample)."""
     rgb, depth, alpha = rgb.cpu().numpy().astype(np.float64), depth.cpu().numpy().astype(np.float64), alpha.cpu().numpy().astype(np.float64)
     m = np.ones(depth.shape, bool) if mask is None else mask.astype(bool)
-    e_rgb = np.abs(rgb - ref["rgb"])[m].max()
-    e_a = np.abs(alpha - ref["alpha"])[m].max()
-    e_d = (np.abs(depth - ref["depth"]) / np.maximum(np.abs(ref["depth"]), 1.0))[m].max()
-    assert e_rgb <= RGB_TOL, "rgb max abs error %g" % e_rgb
-    assert e_a <= RGB_TOL, "alpha max abs error %g" % e_a
-    assert e_d <= DEPTH_REL, "depth rel error %g" % e_d
-    return e_rgb, e_a, e_d
+    err = _pixel_errors(rgb, depth, alpha, ref) * m
+    bad = err > 1.0
+    n_bad = int(bad.sum())
+    if n_bad == 0:
+        return 0
+    v, u = np.unravel_index(np.argmax(err), err.shape)
+    detail = "worst pixel (%d,%d): %.2f x tolerance; %d pixels out" % (u, v, err[v, u], n_bad)
+    assert scene is not None and n_bad <= max(1, int(1e-4 * m.sum())), detail
+    lo = O.render(scene, mode=1, mask=bad.astype(np.uint8), t_stop=scene.t_stop * (1 - 2e-3))
+    hi = O.render(scene, mode=1, mask=bad.astype(np.uint8), t_stop=scene.t_stop * (1 + 2e-3))
+    ambiguous = bad & (lo["n_used"] != hi["n_used"])
+    assert np.array_equal(ambiguous, bad), "not a termination-threshold effect: " + detail
+    e2 = np.minimum(_pixel_errors(rgb, depth, alpha, lo), _pixel_errors(rgb, depth, alpha, hi))
+    assert (e2[bad] <= 1.0).all(), "threshold-ambiguous pixel matches neither outcome: " + detail
+    return n_bad
 
 
 def _check_grads(got, ref, what):
@@ -71,7 +90,7 @@ def test_t2_t3_config1_images_and_gradients(ctx, config1):
     for flags in (dvx.FLAG_NAIVE, 0):
         rgb, depth, alpha, frame = dev.render(flags=flags)
         torch.cuda.synchronize()
-        _check_images(rgb, depth, alpha, ref)
+        _check_images(rgb, depth, alpha, ref, scene=sc)
         g = [torch.from_numpy(gin[k]).cuda() for k in ("rgb", "depth", "alpha")]
         grads = frame.backward(g[0], g[1], g[2])
         torch.cuda.synchronize()
@@ -143,7 +162,7 @@ def _sampled_parity(ctx, sc, n_tiles, seed, backward):
     dev = dvx.SceneOnDevice(ctx, sc)
     rgb, depth, alpha, frame = dev.render()
     torch.cuda.synchronize()
-    errs = _check_images(rgb, depth, alpha, ref, mask)
+    errs = _check_images(rgb, depth, alpha, ref, mask, scene=sc)
     if backward:
         grads = frame.backward(torch.from_numpy(gin["rgb"]).cuda())
         torch.cuda.synchronize()
