@@ -7,8 +7,8 @@
 namespace {
 
 constexpr int SORT_THREADS = 256;
-constexpr int SORT_ITEMS = 16;                         // keys per thread
-constexpr int SORT_TILE = SORT_THREADS * SORT_ITEMS;   // 4096 keys per block
+constexpr int SORT_ITEMS = 8;                          // keys per thread
+constexpr int SORT_TILE = SORT_THREADS * SORT_ITEMS;   // 2048 keys per block
 constexpr int SORT_WARPS = SORT_THREADS / 32;
 constexpr int RADIX = 256;
 
@@ -93,28 +93,39 @@ __global__ void __launch_bounds__(SORT_THREADS) radix_hist(const uint64_t *keys,
   block_hist[(uint64_t)threadIdx.x * n_blocks + blockIdx.x] = h[threadIdx.x];  // digit-major for the scan
 }
 
+// Stable scatter of one 2048-key tile.  Ranks inside the tile come from warp-private digit counters (__match_any_sync keeps
+// equal digits in lane order); the tile is first sorted by digit INTO SHARED MEMORY and only then written out, so that
+// consecutive threads write consecutive global addresses (runs of one digit) instead of 8-byte pieces of 32 sectors.
 __global__ void __launch_bounds__(SORT_THREADS) radix_scatter(const uint64_t *__restrict__ keys_in,
                                                                const uint32_t *__restrict__ vals_in,
                                                                uint64_t *__restrict__ keys_out, uint32_t *__restrict__ vals_out,
                                                                uint64_t n, uint32_t shift, const uint32_t *__restrict__ offs,
                                                                uint32_t n_blocks) {
   __shared__ uint32_t cnt[SORT_WARPS][RADIX];
+  __shared__ uint64_t s_key[SORT_TILE];
+  __shared__ uint32_t s_val[SORT_TILE];
+  __shared__ uint32_t gbase[RADIX];
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
   for (int d = lane; d < RADIX; d += 32) cnt[w][d] = 0;
   __syncwarp();
-  // warp w owns the contiguous keys [w*512, (w+1)*512) of the tile, in 16 steps of 32: order inside the tile is kept
-  const uint64_t wbase = (uint64_t)blockIdx.x * SORT_TILE + (uint64_t)w * (32 * SORT_ITEMS);
+  // warp w owns the contiguous keys [w*256, (w+1)*256) of the tile, in 8 steps of 32: order inside the tile is kept
+  const uint64_t tbase = (uint64_t)blockIdx.x * SORT_TILE;
+  const uint64_t wbase = tbase + (uint64_t)w * (32 * SORT_ITEMS);
   uint64_t key[SORT_ITEMS];
   uint16_t rnk[SORT_ITEMS];
 #pragma unroll
   for (int i = 0; i < SORT_ITEMS; ++i) {
-    uint64_t idx = wbase + (uint64_t)i * 32 + lane;
-    bool valid = idx < n;
-    key[i] = valid ? keys_in[idx] : 0;
-    uint32_t d = valid ? ((uint32_t)(key[i] >> shift) & (RADIX - 1)) : RADIX;  // RADIX = "no key"
-    uint32_t peers = __match_any_sync(0xffffffffu, d);
-    uint32_t before = __popc(peers & ((1u << lane) - 1u));
-    int leader = __ffs(peers) - 1;
+    const uint64_t idx = wbase + (uint64_t)i * 32 + lane;
+    key[i] = idx < n ? keys_in[idx] : 0;
+  }
+#pragma unroll
+  for (int i = 0; i < SORT_ITEMS; ++i) {
+    const uint64_t idx = wbase + (uint64_t)i * 32 + lane;
+    const bool valid = idx < n;
+    const uint32_t d = valid ? ((uint32_t)(key[i] >> shift) & (RADIX - 1)) : RADIX;  // RADIX = "no key"
+    const uint32_t peers = __match_any_sync(0xffffffffu, d);
+    const uint32_t before = __popc(peers & ((1u << lane) - 1u));
+    const int leader = __ffs(peers) - 1;
     uint32_t old = 0;
     if (valid && lane == leader) {
       old = cnt[w][d];
@@ -125,26 +136,39 @@ __global__ void __launch_bounds__(SORT_THREADS) radix_scatter(const uint64_t *__
     __syncwarp();
   }
   __syncthreads();
-  {  // digit d = threadIdx.x: exclusive prefix over the warps, plus this block's global base for the digit
+  {  // digit d = threadIdx.x: prefix over the warps, the tile-local base of the digit, and the global base
     const int d = threadIdx.x;
-    uint32_t run = offs[(uint64_t)d * n_blocks + blockIdx.x];
+    uint32_t run = 0;
 #pragma unroll
     for (int ww = 0; ww < SORT_WARPS; ++ww) {
-      uint32_t c = cnt[ww][d];
+      const uint32_t c = cnt[ww][d];
       cnt[ww][d] = run;
       run += c;
     }
+    uint32_t total;
+    const uint32_t lbase = block_excl_scan(run, &total);
+#pragma unroll
+    for (int ww = 0; ww < SORT_WARPS; ++ww) cnt[ww][d] += lbase;
+    gbase[d] = offs[(uint64_t)d * n_blocks + blockIdx.x] - lbase;
   }
   __syncthreads();
 #pragma unroll
   for (int i = 0; i < SORT_ITEMS; ++i) {
-    uint64_t idx = wbase + (uint64_t)i * 32 + lane;
+    const uint64_t idx = wbase + (uint64_t)i * 32 + lane;
     if (idx < n) {
-      uint32_t d = (uint32_t)(key[i] >> shift) & (RADIX - 1);
-      uint32_t pos = cnt[w][d] + rnk[i];
-      keys_out[pos] = key[i];
-      vals_out[pos] = vals_in[idx];
+      const uint32_t d = (uint32_t)(key[i] >> shift) & (RADIX - 1);
+      const uint32_t pos = cnt[w][d] + rnk[i];
+      s_key[pos] = key[i];
+      s_val[pos] = vals_in[idx];
     }
+  }
+  __syncthreads();
+  const uint32_t nb = (uint32_t)min((uint64_t)SORT_TILE, n - tbase);
+  for (uint32_t i = threadIdx.x; i < nb; i += SORT_THREADS) {
+    const uint64_t k = s_key[i];
+    const uint32_t out = gbase[(uint32_t)(k >> shift) & (RADIX - 1)] + i;
+    keys_out[out] = k;
+    vals_out[out] = s_val[i];
   }
 }
 
