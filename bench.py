@@ -284,6 +284,14 @@ def run_dvx(args):
     except (OSError, ValueError):
         pass
     hbm_frac_step = ab["min_fwdbwd" if not args.fwd_only else "min_fwd"] / (ms_step * 1e-3) / 1e9 / peak
+    # fp32-lane roofline of the same kernel: algorithmic lane-operations from the run's own counters
+    # (slab test ~20, per composited sub-segment: cubic fold + K samples x 5 + blend ~115 forward, ~260 with the backward's
+    # moments, corner sums and reduction) against 148 SMs x 128 fp32 lanes x the SM clock sampled under load
+    K = scene.k_samples
+    lane_ops = cnt["q_test"] * 20 + cnt["q_hit"] * ((75 + 5 * K) if args.fwd_only else (220 + 5 * K))
+    sm_mhz = (clocks or {}).get("sm_mhz") or peaks.get("sm_max_mhz") or 1965.0
+    alu_peak = 148 * 128 * sm_mhz * 1e6 / 1e12
+    alu_ach = lane_ops / (dom_ms * 1e-3) / 1e12 if dom_ms > 0 else 0.0
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
@@ -299,6 +307,9 @@ def run_dvx(args):
         "roofline": {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
                      "frac": achieved / peak if peak else None, "traffic": ncu_traffic, "peak_source": peak_src,
                      "bytes_per_launch": dom_bytes, "ms_per_launch": dom_ms},
+        "alu_roofline": {"bound": "alu", "kernel": dom, "achieved": alu_ach, "peak": alu_peak, "unit": "Tlane-op/s",
+                         "frac": alu_ach / alu_peak, "lane_ops_per_launch": lane_ops,
+                         "peak_source": "148 SMs x 128 fp32 lanes x %.0f MHz (nvidia-smi, under load)" % sm_mhz},
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": (0 if args.fwd_only else 12 * px_step),
                 "d2h_bytes_per_step": 20 * px_step, "ms_per_step": ms_e2e / args.steps},
         "gpu_launches": launches, "clocks": clocks,
