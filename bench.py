@@ -145,6 +145,24 @@ def run_reference(args, scene):
     print(json.dumps(line))
 
 
+# ----------------------------------------------------------------------------------------------- replicas
+def max_over_ranks(ms, device=None):
+    """Replicas only: the job time is the slowest replica's.  all_reduce(MAX) over the default
+    process group (nccl on the GPU box, gloo in the CPU test); identity for a single process."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return float(ms)
+    t = torch.tensor([float(ms)], dtype=torch.float64, device=device if device is not None else "cpu")
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_value(px_per_step_per_replica, world, ms_per_step):
+    """Whole-job MP/s of `world` independent replicas that each finish a step of px pixels in ms_per_step (max over ranks)."""
+    return world * px_per_step_per_replica / (ms_per_step * 1e-3) / 1e6
+
+
 # ----------------------------------------------------------------------------------------------- GPU arm
 def measured_peaks():
     """Roofline denominators: MEASURED_PEAKS.json (driver-written) or the fallback B200_PROFILING.md states."""
@@ -220,12 +238,7 @@ def run_dvx(args):
             step(**kw)
         e1.record()
         barrier()
-        ms = e0.elapsed_time(e1)
-        if world > 1:
-            t = torch.tensor([ms], device=ctx.device)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ms = float(t.item())
-        return ms
+        return max_over_ranks(e0.elapsed_time(e1), ctx.device)
 
     # ---- untimed: counters of this workload (one frame per camera, counting build of the kernels)
     cnt = {"v_vis": 0, "pairs": 0, "pairs_eff": 0, "q_test": 0, "q_hit": 0}
@@ -269,9 +282,9 @@ def run_dvx(args):
             dist.destroy_process_group()
         return
     ms_step = ms_total / args.steps
-    value = world * px_step / (ms_step * 1e-3) / 1e6
-    fwd_value = world * px_step / (ms_fwd / args.steps * 1e-3) / 1e6
-    e2e_value = world * px_step / (ms_e2e / args.steps * 1e-3) / 1e6
+    value = aggregate_value(px_step, world, ms_step)
+    fwd_value = aggregate_value(px_step, world, ms_fwd / args.steps)
+    e2e_value = aggregate_value(px_step, world, ms_e2e / args.steps)
     peak, peak_src, peaks = measured_peaks()
     ab = algorithmic_bytes(scene, W, H, {k: v / 1 for k, v in cnt.items()}, touched)
     dom = "composite_bwd" if not args.fwd_only else "composite_fwd"
