@@ -301,19 +301,24 @@ __device__ __forceinline__ void flush_batch(const CompositeArgs &A, int lane, Wa
       for (int c = 0; c < 8; ++c) val[c] = dtau * cs[c];
       val[8] = Q.wg[0][at_b]; val[9] = Q.wg[1][at_b]; val[10] = Q.wg[2][at_b];
     }
-    // items of one voxel are contiguous: segmented suffix sums, the first lane of each run ends up with the run total
+    // runs of consecutive items of one voxel (the pixels one list entry hit): segmented suffix sums over the run index,
+    // the first lane of each run ends up with the run total.  (The voxel id itself is not a valid segment key: a voxel cut
+    // in two by a box is queued twice, with other voxels in between.)
+    const uint32_t prev = __shfl_up_sync(0xffffffffu, my_id, 1);
+    const bool is_head = lane == 0 || prev != my_id;
+    const uint32_t heads = __ballot_sync(0xffffffffu, is_head);
+    const uint32_t run = __popc(heads & (0xffffffffu >> (31 - lane)));
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
-      const uint32_t oid = __shfl_down_sync(0xffffffffu, my_id, o);
-      const bool take = (lane + o < 32) && oid == my_id;
+      const uint32_t orun = __shfl_down_sync(0xffffffffu, run, o);
+      const bool take = (lane + o < 32) && orun == run;
 #pragma unroll
       for (int c = 0; c < 11; ++c) {
         const float x = __shfl_down_sync(0xffffffffu, val[c], o);
         if (take) val[c] += x;
       }
     }
-    const uint32_t prev = __shfl_up_sync(0xffffffffu, my_id, 1);
-    if (my_id != NONE && (lane == 0 || prev != my_id)) {
+    if (my_id != NONE && is_head) {
       const TreeFrame &T = A.trees[(my_meta >> 8) & 0xFFu];
       if (T.dgeo) {
         float *dg = T.dgeo + (size_t)(my_id - T.base) * 8;
@@ -335,6 +340,29 @@ __device__ __forceinline__ void pixel_ray_d(const FrameParams &p, int u, int v, 
   xd = ((double)u + 0.5 - p.cx_d) * p.inv_fx;
   yd = ((double)v + 0.5 - p.cy_d) * p.inv_fy;
   rnd = rsqrt(xd * xd + yd * yd + 1.0);
+}
+
+// R20, the measure-zero case of a ray component that is exactly 0: that axis puts no constraint on tau, and the ray meets
+// the voxel only if the camera coordinate lies in [min, max) of the slab.  Decided exactly, from the voxel's integer
+// coordinates in fp64 (the staged fp32 centre is not exact enough to settle a ray lying IN a voxel face).
+__device__ __noinline__ float2 axis_parallel_fix(const TreeFrame *T, uint32_t id, uint32_t level, uint32_t zmask, float hs,
+                                                 float k0, float k1, float k2, float c0, float c1, float c2) {
+  uint32_t XYZ[3], lv;
+  dvx_decode16(__ldg(T->code + (id - T->base)), XYZ[0], XYZ[1], XYZ[2], lv);
+  const uint32_t size = 1u << (DVX_MAX_LEVEL - level);
+  const float c[3] = {c0, c1, c2}, k[3] = {k0, k1, k2};  // k = |1/d|
+  float sa = -INFINITY, sb = INFINITY;
+  bool inside = true;
+  for (int a = 0; a < 3; ++a) {
+    if ((zmask >> a) & 1u) {
+      const double mn = fma(T->cell, (double)XYZ[a], T->rel0[a]);  // slab minimum relative to the camera
+      inside = inside && mn <= 0.0 && mn + T->cell * (double)size > 0.0;
+    } else {
+      sa = fmaxf(sa, fmaf(-hs, k[a], -c[a]));
+      sb = fminf(sb, fmaf(hs, k[a], -c[a]));
+    }
+  }
+  return inside ? make_float2(sa, sb) : make_float2(INFINITY, -INFINITY);
 }
 
 template <bool BWD, bool CNT>
@@ -450,6 +478,7 @@ __global__ void __launch_bounds__(TILE_THREADS, DVX_TILE_MIN_CTAS) composite_til
     // difference e to the warp's reference direction d0 (= the direction of lane 0's pixel, kept in shared memory)
     float d[3], inv[3], e[3];
     int q = 0;
+    uint32_t zmask = 0;  // axes on which this ray is exactly axis-parallel (R20), almost always 0
     {
       double xd, yd, rnd;
       pixel_ray_d(p, u, v, xd, yd, rnd);
@@ -463,7 +492,8 @@ __global__ void __launch_bounds__(TILE_THREADS, DVX_TILE_MIN_CTAS) composite_til
         e[a] = (float)(da - d0a);
         d[a] = (float)da;
         q |= (dvx_dir_comp(T.N, a, xp, yp) < 0.f) ? (4 >> a) : 0;  // R12: s_a = (d_a < 0), same fp32 formula as step 1
-        inv[a] = d[a] != 0.f ? 1.0f / d[a] : 1.0e30f;               // axis-parallel: +-1e30 puts the slab at -+infinity
+        inv[a] = d[a] != 0.f ? 1.0f / d[a] : 0.f;
+        if (d[a] == 0.f) zmask |= 1u << a;
       }
       __syncwarp();
     }
@@ -516,8 +546,12 @@ __global__ void __launch_bounds__(TILE_THREADS, DVX_TILE_MIN_CTAS) composite_til
           const float hs = __uint_as_float(r1.x);
           const float w0 = fmaf(r0.x, e[0], -r0.y), w1 = fmaf(r0.x, e[1], -r0.z), w2 = fmaf(r0.x, e[2], -r0.w);
           const float c0 = w0 * inv[0], c1 = w1 * inv[1], c2 = w2 * inv[2];
-          const float sa = fmaxf(fmaxf(fmaf(-hs, fabsf(inv[0]), -c0), fmaf(-hs, fabsf(inv[1]), -c1)), fmaf(-hs, fabsf(inv[2]), -c2));
-          const float sb = fminf(fminf(fmaf(hs, fabsf(inv[0]), -c0), fmaf(hs, fabsf(inv[1]), -c1)), fmaf(hs, fabsf(inv[2]), -c2));
+          float sa = fmaxf(fmaxf(fmaf(-hs, fabsf(inv[0]), -c0), fmaf(-hs, fabsf(inv[1]), -c1)), fmaf(-hs, fabsf(inv[2]), -c2));
+          float sb = fminf(fminf(fmaf(hs, fabsf(inv[0]), -c0), fmaf(hs, fabsf(inv[1]), -c1)), fmaf(hs, fabsf(inv[2]), -c2));
+          if (zmask) {
+            const float2 f = axis_parallel_fix(&T, r1.y, r1.z, zmask, hs, fabsf(inv[0]), fabsf(inv[1]), fabsf(inv[2]), c0, c1, c2);
+            sa = f.x; sb = f.y;
+          }
           const float lo_r = lo - r0.x, hi_r = hi - r0.x;
           const float ca = fmaxf(sa, lo_r), cb = fminf(sb, hi_r);       // R1: clip to the interval
           const bool live = active != 0u && c_l <= ei && sb > sa;       // this pixel's ray meets the voxel

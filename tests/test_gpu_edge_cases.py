@@ -1,0 +1,145 @@
+"""GPU-vs-oracle parity on the degenerate and edge cases of the method (through the C ABI, brute-force oracle, every pixel
+and every gradient entry): other K / activation / t_stop than the configured ones, axis-parallel rays (R20), a static voxel
+cut into two pieces by a box (R1), overlapping boxes (R2), the camera inside a box (R11), empty octrees and actor lists,
+ragged and single-pixel images (R15)."""
+import numpy as np
+import pytest
+
+import dvx_scenes as S
+from oracle import oracle as O
+from helpers import tree_from_cells, empty_tree, scene, axis_camera
+from dvx_scenes.octree import C0
+
+pytestmark = pytest.mark.gpu
+
+RGB_TOL, DEPTH_REL, GRAD_REL, GRAD_ABS = 2e-4, 1e-4, 1e-3, 1e-6
+
+
+@pytest.fixture(scope="module")
+def ctx():
+    import paper_2606_23031_b200 as dvx
+    c = dvx.Context(0)
+    yield c
+    c.close()
+
+
+def _round_to_f32(sc):
+    """The library takes fp32 inputs: make every input exactly fp32-representable so both sides see the same numbers."""
+    for t in sc.octrees:
+        t.geo = np.ascontiguousarray(t.geo, dtype=np.float32)
+        t.sh = np.ascontiguousarray(t.sh, dtype=np.float32)
+        t.center = np.asarray(t.center, dtype=np.float32).astype(np.float64)
+        t.side = float(np.float32(t.side))
+    sc.poses = np.ascontiguousarray(sc.poses, dtype=np.float32)
+    sc.box_half = np.ascontiguousarray(sc.box_half, dtype=np.float32)
+    for cam in sc.cameras:
+        cam.c2w = np.asarray(cam.c2w, dtype=np.float32).reshape(12)
+        for k in ("fx", "fy", "cx", "cy", "near", "far"):
+            setattr(cam, k, float(np.float32(getattr(cam, k))))
+    return sc
+
+
+def _compare(ctx, sc, backward=True, **opt):
+    import paper_2606_23031_b200 as dvx
+    import torch
+    _round_to_f32(sc)
+    for k, v in opt.items():
+        setattr(sc, k, v)
+    cam = sc.cameras[0]
+    gin = sc.image_grads(rgb_std=1e-2, depth_std=1e-3, alpha_std=1e-2) if backward else None
+    ref = O.render(sc, mode=0, grads_in=gin)
+    dev = dvx.SceneOnDevice(ctx, sc)
+    for flags in (0, dvx.FLAG_NAIVE):
+        rgb, depth, alpha, frame = dev.render(flags=flags)
+        torch.cuda.synchronize()
+        r, d, a = (x.cpu().numpy().astype(np.float64) for x in (rgb, depth, alpha))
+        assert np.abs(r - ref["rgb"]).max() <= RGB_TOL, (flags, np.abs(r - ref["rgb"]).max())
+        assert np.abs(a - ref["alpha"]).max() <= RGB_TOL, (flags, np.abs(a - ref["alpha"]).max())
+        e_d = (np.abs(d - ref["depth"]) / np.maximum(np.abs(ref["depth"]), 1.0)).max()
+        assert e_d <= DEPTH_REL, (flags, e_d)
+        if backward:
+            g = [None if gin[k] is None else torch.from_numpy(gin[k]).cuda() for k in ("rgb", "depth", "alpha")]
+            grads = frame.backward(g[0], g[1], g[2])
+            torch.cuda.synchronize()
+            for t in range(len(sc.octrees)):
+                for got, want, name in ((grads[t][0], ref["dgeo"][t], "dgeo"), (grads[t][1], ref["dsh"][t], "dsh")):
+                    err = np.abs(got.cpu().numpy().astype(np.float64) - want)
+                    bound = GRAD_REL * np.abs(want) + GRAD_ABS
+                    assert (err <= bound).all(), "%s[%d] flags %d: worst excess %g" % (name, t, flags, (err - bound).max())
+        frame.release()
+    for t in dev.trees:
+        t.close()
+    return ref
+
+
+@pytest.mark.parametrize("seed,K,act,t_stop", [(3, 8, 0, 0.0), (5, 1, 0, 1e-4), (7, 3, 0, 1e-4), (11, 5, 1, 0.0), (13, 8, 1, 1e-4),
+                                               (17, 2, 0, 0.05)])
+def test_random_tiny_scenes_other_options(ctx, seed, K, act, t_stop):
+    """K != 8 and the exp-linear activation take the generic quadrature path of the kernels; a large t_stop makes most rays
+    terminate early (R3)."""
+    sc = S.tiny_random_scene(seed, sh_degree=1, width=24, height=20)
+    _compare(ctx, sc, k_samples=K, activation=act, t_stop=t_stop)
+
+
+def _cube8(geo, side=2.0, sh=None):
+    cells = [(i, j, k, 1) for i in (0, 1) for j in (0, 1) for k in (0, 1)]
+    return tree_from_cells(cells, geo=geo, side=side, sh=sh)
+
+
+def test_axis_parallel_rays_and_two_slabs(ctx):
+    """The centre pixel's ray is exactly the +x axis (two zero direction components, R20); static + actor voxel on the axis."""
+    cam = axis_camera(width=9, height=7)
+    sh1 = np.full((1, 1, 3), (0.8 - 0.5) / C0); sh2 = np.full((1, 1, 3), (0.3 - 0.5) / C0)
+    st = tree_from_cells([(1, 1, 1, 1)], geo=-0.5, sh=sh1)
+    act = tree_from_cells([(1, 1, 1, 1)], geo=0.25, sh=sh2, side=1.0)
+    for x_act in (4.0, -3.0):
+        pose = S.pose_yaw((x_act, 0.75, 0.75), 0.0)
+        ref = _compare(ctx, scene(st, [act], [pose], [[0.625, 0.625, 0.625]], cam=cam))
+        assert ref["alpha"][3, 4] > 0.5
+
+
+def test_box_inside_a_voxel_gives_two_pieces(ctx):
+    """R1: one large static voxel, an empty actor box strictly inside it: the voxel is composited as two clipped pieces."""
+    cam = axis_camera(width=9, height=7)
+    st = tree_from_cells([(1, 1, 1, 1)], geo=-0.25)
+    pose = S.pose_yaw((1.0, 1.0, 1.0), 0.0)
+    ref = _compare(ctx, scene(st, [empty_tree()], [pose], [[0.375, 0.25, 0.25]], cam=cam))
+    assert ref["n_used"][3, 4] == 2
+
+
+def test_overlapping_boxes_rule_r2(ctx):
+    cam = axis_camera(width=9, height=7)
+    act = _cube8(0.0)
+    pa, pb = S.pose_yaw((0.0, 1.0, 1.0), 0.0), S.pose_yaw((1.0, 1.0, 1.0), 0.0)   # boxes overlap on x in [0,1]
+    st = tree_from_cells([(0, 0, 0, 1), (1, 1, 1, 1)], geo=-1.0, side=8.0)
+    _compare(ctx, scene(st, [act, act], [pa, pb], [[1, 1, 1], [1, 1, 1]], cam=cam))
+
+
+def test_camera_inside_an_actor_box(ctx):
+    """R11: everything is clipped at `near`; tau_in of the enclosing box is negative."""
+    cam = axis_camera(position=(0.25, 1.0, 1.0), width=9, height=7)
+    act = _cube8(np.linspace(-1.0, 0.5, 64).reshape(8, 8))
+    pose = S.pose_yaw((0.5, 1.0, 1.0), 0.3)
+    st = tree_from_cells([(1, 1, 1, 1), (1, 0, 1, 1)], geo=-0.5, side=16.0, center=(4.0, 0.0, 0.0))
+    _compare(ctx, scene(st, [act], [pose], [[1, 1, 1]], cam=cam))
+
+
+@pytest.mark.parametrize("w,h", [(1, 1), (17, 33), (40, 16)])
+def test_ragged_and_single_pixel_images(ctx, w, h):
+    sc = S.tiny_random_scene(23, sh_degree=1, width=w, height=h)
+    _compare(ctx, sc)
+
+
+def test_no_actors_and_empty_trees(ctx):
+    sc = S.tiny_random_scene(29, sh_degree=1, width=16, height=12)
+    only_static = scene(sc.static, [], [], [], cam=sc.cameras[0], t_stop=0.0)
+    _compare(ctx, only_static)
+    empty_static = scene(empty_tree(sh_degree=1, side=8.0), sc.actors, sc.poses, sc.box_half, cam=sc.cameras[0], t_stop=0.0)
+    _compare(ctx, empty_static)
+    empty_actor = scene(sc.static, [empty_tree(sh_degree=1)], sc.poses, sc.box_half, cam=sc.cameras[0], t_stop=0.0)
+    _compare(ctx, empty_actor)
+
+
+def test_sh_degrees_0_2_3(ctx):
+    for deg in (0, 2, 3):
+        _compare(ctx, S.tiny_random_scene(31 + deg, sh_degree=deg, width=16, height=12))
