@@ -39,6 +39,8 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing leg (profiling runs)")
     ap.add_argument("--cpu-tiles", type=int, default=0, help="tiles in the CPU-oracle sample (0 = pick for about 10-30 s)")
     ap.add_argument("--fwd-only", action="store_true", help="profiling aid: time dvx_render alone")
+    ap.add_argument("--k-samples", type=int, default=0, help="report-only variant: override K (samples per voxel segment)")
+    ap.add_argument("--opaque", action="store_true", help="report-only variant 3b: config 3 with raw += 8 on leaves holding a LiDAR return")
     ap.add_argument("--profiler-range", action="store_true",
                     help="bracket the first timed region with cudaProfilerStart/Stop (use with ncu --profile-from-start off)")
     return ap.parse_args()
@@ -203,7 +205,7 @@ def run_dvx(args):
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
 
-    scene = dvx_scenes.make_config(args.config)
+    scene = make_scene(args)
     ctx = dvx.Context(local)
     dev = dvx.SceneOnDevice(ctx, scene)
     n_cams = len(scene.cameras)
@@ -309,7 +311,7 @@ def run_dvx(args):
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
         "data": "synthetic",
-        "config": {"workload": workload_name(args.config), "cameras": n_cams, "k_samples": scene.k_samples, "sh_degree": scene.static.sh_degree,
+        "config": {"workload": workload_name(args.config) + ("_opaque3b" if args.opaque else "") + ("_K%d" % args.k_samples if args.k_samples else ""), "cameras": n_cams, "k_samples": scene.k_samples, "sh_degree": scene.static.sh_degree,
                    "voxels": int(sum(t.n_voxels for t in scene.octrees)), "actors": len(scene.actors),
                    "l2_policy": "inputs larger than L2 (voxel records + gradient buffers >> 126 MB)", "replicas": world,
                    "passes": "fwd" if args.fwd_only else "fwd+bwd"},
@@ -341,13 +343,21 @@ def run_dvx(args):
         dist.destroy_process_group()
 
 
+def make_scene(args):
+    import dvx_scenes
+    scene = dvx_scenes.make_config(args.config, **({"opaque": True} if args.opaque and args.config == 3 else {}))
+    if args.k_samples:
+        scene.k_samples = args.k_samples
+    return scene
+
+
 def main():
     args = parse_args()
     if args.impl == "reference":
         if int(os.environ.get("RANK", "0")) != 0:
             return
         import dvx_scenes
-        run_reference(args, dvx_scenes.make_config(args.config))
+        run_reference(args, make_scene(args))
         return
     run_dvx(args)
 

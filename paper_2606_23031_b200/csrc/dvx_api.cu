@@ -354,6 +354,7 @@ dvx_status dvx_render(dvx_ctx *ctx, const dvx_camera *cam, const dvx_octree *sta
     vtot += tr->d.n_voxels;
     if (tr->d.n_voxels > vmax) vmax = tr->d.n_voxels;
   }
+  if ((uint64_t)p.n_tiles * 8u >= (1u << 24)) { frame_free(ctx, f); return fail(ctx, DVX_ERR_INVALID_ARG, "image too large (more than 2^21 tiles)"); }
   if (vtot >= 0xFFFFFFFFull) { frame_free(ctx, f); return fail(ctx, DVX_ERR_INVALID_ARG, "more than 2^32-2 voxels in total"); }
   p.v_total = (uint32_t)vtot;
   p.rank_bits = bits_for(vmax);
@@ -412,7 +413,7 @@ dvx_status dvx_render(dvx_ctx *ctx, const dvx_camera *cam, const dvx_octree *sta
     return fail(ctx, DVX_ERR_OOM, "dvx_render: allocator returned NULL");
   }
   CU(cudaEventRecord(f->ev[2], st));
-  dvx_emit_pairs_launch(p, trees_d, (const uint8_t *)f->octmask.p, (const ushort4 *)f->pxrect.p, ka, va, P, counters, st);
+  dvx_emit_pairs_launch(p, trees_d, (const uint8_t *)f->octmask.p, (const ushort4 *)f->pxrect.p, (const FrameVox *)f->fvox.p, ka, va, P, counters, st);
   int which = dvx_sort_launch(ka, va, kb, vb, P, key_bits, scr, st);
   CU(cudaMemsetAsync(f->range_beg.p, 0, sizeof(uint32_t) * (size_t)p.n_buckets, st));
   CU(cudaMemsetAsync(f->range_end.p, 0, sizeof(uint32_t) * (size_t)p.n_buckets, st));

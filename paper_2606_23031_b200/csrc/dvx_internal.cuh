@@ -91,8 +91,8 @@ void dvx_tile_masks_launch(const FrameParams &p, const TreeFrame *trees, uint8_t
 void dvx_preprocess_launch(const FrameParams &p, const TreeFrame *trees, const uint8_t *octmask, FrameVox *fvox,
                            ushort4 *pxrect, unsigned long long *counters, cudaStream_t st);
 void dvx_emit_pairs_launch(const FrameParams &p, const TreeFrame *trees, const uint8_t *octmask, const ushort4 *pxrect,
-                           uint64_t *keys, uint32_t *vals, unsigned long long capacity, unsigned long long *counters,
-                           cudaStream_t st);
+                           const FrameVox *fvox, uint64_t *keys, uint32_t *vals, unsigned long long capacity,
+                           unsigned long long *counters, cudaStream_t st);
 void dvx_ranges_launch(const uint64_t *keys, uint64_t n, uint32_t rank_bits, uint32_t *range_beg, uint32_t *range_end,
                        cudaStream_t st);
 void dvx_sh_backward_launch(const FrameParams &p, const TreeFrame *trees, const FrameVox *fvox, const ushort4 *pxrect,

@@ -146,6 +146,30 @@ __device__ __forceinline__ uint32_t count_pairs(const FrameParams &p, const uint
   return n;
 }
 
+// A voxel whose rectangle spans more than BIG_TILES tiles (ground next to the camera, a voxel around the camera) is
+// handled by its whole warp, 32 tiles per step, instead of by one thread walking up to thousands of tiles.
+constexpr int BIG_TILES = 24;
+
+__device__ __forceinline__ int rect_tiles(int x0, int y0, int x1, int y1) {
+  return ((x1 >> 4) - (x0 >> 4) + 1) * ((y1 >> 4) - (y0 >> 4) + 1);
+}
+
+// Warp-cooperative count_pairs for the voxel held by lane `src` (all lanes call; every lane gets the total).
+__device__ __forceinline__ uint32_t count_pairs_warp(const FrameParams &p, const uint8_t *octmask, int src, int t, int x0,
+                                                     int y0, int x1, int y1) {
+  t = __shfl_sync(0xffffffffu, t, src);
+  const int tx0 = __shfl_sync(0xffffffffu, x0, src) >> 4, ty0 = __shfl_sync(0xffffffffu, y0, src) >> 4;
+  const int tx1 = __shfl_sync(0xffffffffu, x1, src) >> 4, ty1 = __shfl_sync(0xffffffffu, y1, src) >> 4;
+  const int w = tx1 - tx0 + 1, n = w * (ty1 - ty0 + 1);
+  uint32_t c = 0;
+  for (int i = threadIdx.x & 31; i < n; i += 32) {
+    const int tile = (ty0 + i / w) * (int)p.tiles_x + tx0 + i % w;
+    c += __popc((uint32_t)octmask[(size_t)tile * p.n_trees + t]);
+  }
+  for (int o = 16; o > 0; o >>= 1) c += __shfl_xor_sync(0xffffffffu, c, o);
+  return c;
+}
+
 __global__ void __launch_bounds__(PRE_THREADS) preprocess_kernel(FrameParams p, const TreeFrame *trees,
                                                                  const uint8_t *octmask, FrameVox *fvox,
                                                                  ushort4 *pxrect, unsigned long long *counters) {
@@ -154,14 +178,23 @@ __global__ void __launch_bounds__(PRE_THREADS) preprocess_kernel(FrameParams p, 
   __syncthreads();
   uint32_t g = blockIdx.x * blockDim.x + threadIdx.x;
   uint32_t npairs = 0, vis = 0;
+  int t = 0, x0 = 0, y0 = 0, x1 = -1, y1 = -1;
+  float rel[3] = {0.f, 0.f, 0.f}, s = 0.f;
+  bool ok = false;
   if (g < p.v_total) {
-    int t = find_tree(s_base, p.n_trees, g);
+    t = find_tree(s_base, p.n_trees, g);
+    ok = voxel_rect(p, trees[t], trees[t].code[g - s_base[t]], rel, s, x0, y0, x1, y1);
+  }
+  const bool big = ok && rect_tiles(x0, y0, x1, y1) > BIG_TILES;
+  if (ok && !big) npairs = count_pairs(p, octmask, t, x0, y0, x1, y1);
+  for (uint32_t bm = __ballot_sync(0xffffffffu, big); bm; bm &= bm - 1) {
+    const int src = __ffs(bm) - 1;
+    const uint32_t c = count_pairs_warp(p, octmask, src, t, x0, y0, x1, y1);
+    if ((int)(threadIdx.x & 31) == src) npairs = c;
+  }
+  if (g < p.v_total) {
     const TreeFrame &T = trees[t];
-    uint32_t v = g - s_base[t];
-    float rel[3], s;
-    int x0, y0, x1, y1;
-    bool ok = voxel_rect(p, T, T.code[v], rel, s, x0, y0, x1, y1);
-    if (ok) npairs = count_pairs(p, octmask, t, x0, y0, x1, y1);
+    const uint32_t v = g - s_base[t];
     if (npairs == 0) {
       pxrect[g] = make_ushort4(0xFFFF, 0xFFFF, 0, 0);
     } else {
@@ -199,7 +232,7 @@ __global__ void __launch_bounds__(PRE_THREADS) preprocess_kernel(FrameParams p, 
         if (!(acc[ch] > 0.f)) { meta |= 1u << ch; acc[ch] = 0.f; }
         fv.rgb[ch] = acc[ch];
       }
-      fv.meta = meta;
+      fv.meta = meta | (npairs << 8);  // bits 8-31: this voxel's pair count (step 2 allocates its slots from it)
       fvox[g] = fv;
     }
   }
@@ -217,10 +250,23 @@ __global__ void __launch_bounds__(PRE_THREADS) preprocess_kernel(FrameParams p, 
 // ------------------------------------------------------------------ step 2: key generation
 // key = (bucket << rank_bits) | rank_q(v), bucket = (tile*n_trees + tree)*8 + q; value = global voxel id.
 // Every key is unique, so the order in which pairs are emitted does not matter: slots are handed out with one
-// warp-aggregated atomic per warp.
+// warp-aggregated atomic per warp from the per-voxel pair counts step 1 left in fvox.meta.  Voxels with a large
+// footprint are emitted by the whole warp, 32 tiles per step.
+__device__ __forceinline__ void emit_tile(const FrameParams &p, const TreeFrame &T, uint32_t tile, int t, uint32_t v, uint32_t g,
+                                          uint32_t m, unsigned long long pos, uint64_t *keys, uint32_t *vals) {
+  while (m) {
+    const int q = __ffs(m) - 1;
+    m &= m - 1;
+    const uint64_t bucket = ((uint64_t)tile * p.n_trees + t) * 8u + q;
+    keys[pos] = (bucket << p.rank_bits) | (uint64_t)__ldg(T.rank + (size_t)q * T.n_voxels + v);
+    vals[pos] = g;
+    ++pos;
+  }
+}
+
 __global__ void __launch_bounds__(PRE_THREADS) emit_pairs_kernel(FrameParams p, const TreeFrame *trees,
                                                                  const uint8_t *octmask, const ushort4 *pxrect,
-                                                                 uint64_t *keys, uint32_t *vals,
+                                                                 const FrameVox *fvox, uint64_t *keys, uint32_t *vals,
                                                                  unsigned long long capacity,
                                                                  unsigned long long *counters) {
   __shared__ uint32_t s_base[DVX_MAX_TREES + 1];
@@ -235,7 +281,7 @@ __global__ void __launch_bounds__(PRE_THREADS) emit_pairs_kernel(FrameParams p, 
     r = pxrect[g];
     if (r.x <= r.z) {
       t = find_tree(s_base, p.n_trees, g);
-      n = count_pairs(p, octmask, t, r.x, r.y, r.z, r.w);
+      n = fvox[g].meta >> 8;
     }
   }
   // warp exclusive scan of n, one atomic for the warp
@@ -246,30 +292,54 @@ __global__ void __launch_bounds__(PRE_THREADS) emit_pairs_kernel(FrameParams p, 
     if (lane >= o) inc += x;
   }
   uint32_t total = __shfl_sync(0xffffffffu, inc, 31);
+  if (total == 0) return;
   unsigned long long wbase = 0;
-  if (lane == 31 && total) wbase = atomicAdd(&counters[CNT_EMIT], (unsigned long long)total);
+  if (lane == 31) wbase = atomicAdd(&counters[CNT_EMIT], (unsigned long long)total);
   wbase = __shfl_sync(0xffffffffu, wbase, 31);
-  if (n == 0) return;
-  unsigned long long pos = wbase + (inc - n);
-  if (pos + n > capacity) {
-    atomicOr((unsigned int *)&counters[CNT_OVERFLOW], 1u);
+  if (wbase + total > capacity) {
+    if (lane == 0) atomicOr((unsigned int *)&counters[CNT_OVERFLOW], 1u);
     return;
   }
-  const TreeFrame &T = trees[t];
-  const uint32_t v = g - s_base[t];
-  for (int ty = r.y >> 4; ty <= (r.w >> 4); ++ty)
-    for (int tx = r.x >> 4; tx <= (r.z >> 4); ++tx) {
-      uint32_t tile = ty * p.tiles_x + tx;
-      uint32_t m = octmask[(size_t)tile * p.n_trees + t];
-      while (m) {
-        int q = __ffs(m) - 1;
-        m &= m - 1;
-        uint64_t bucket = ((uint64_t)tile * p.n_trees + t) * 8u + q;
-        keys[pos] = (bucket << p.rank_bits) | (uint64_t)__ldg(T.rank + (size_t)q * T.n_voxels + v);
-        vals[pos] = g;
-        ++pos;
+  unsigned long long pos = wbase + (inc - n);
+  const bool big = n && rect_tiles(r.x, r.y, r.z, r.w) > BIG_TILES;
+  if (n && !big) {
+    const TreeFrame &T = trees[t];
+    const uint32_t v = g - s_base[t];
+    for (int ty = r.y >> 4; ty <= (r.w >> 4); ++ty)
+      for (int tx = r.x >> 4; tx <= (r.z >> 4); ++tx) {
+        const uint32_t tile = ty * p.tiles_x + tx;
+        const uint32_t m = octmask[(size_t)tile * p.n_trees + t];
+        emit_tile(p, T, tile, t, v, g, m, pos, keys, vals);
+        pos += __popc(m);
       }
+  }
+  for (uint32_t bm = __ballot_sync(0xffffffffu, big); bm; bm &= bm - 1) {
+    const int src = __ffs(bm) - 1;
+    const int bt = __shfl_sync(0xffffffffu, t, src);
+    const uint32_t bg = __shfl_sync(0xffffffffu, g, src);
+    const int tx0 = __shfl_sync(0xffffffffu, (int)r.x, src) >> 4, ty0 = __shfl_sync(0xffffffffu, (int)r.y, src) >> 4;
+    const int tx1 = __shfl_sync(0xffffffffu, (int)r.z, src) >> 4, ty1 = __shfl_sync(0xffffffffu, (int)r.w, src) >> 4;
+    unsigned long long bpos = __shfl_sync(0xffffffffu, pos, src);
+    const TreeFrame &T = trees[bt];
+    const uint32_t v = bg - s_base[bt];
+    const int w = tx1 - tx0 + 1, nt = w * (ty1 - ty0 + 1);
+    for (int i0 = 0; i0 < nt; i0 += 32) {
+      const int i = i0 + lane;
+      uint32_t tile = 0, m = 0;
+      if (i < nt) {
+        tile = (ty0 + i / w) * p.tiles_x + tx0 + i % w;
+        m = octmask[(size_t)tile * p.n_trees + bt];
+      }
+      uint32_t c = __popc(m), ci = c;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        uint32_t x = __shfl_up_sync(0xffffffffu, ci, o);
+        if (lane >= o) ci += x;
+      }
+      emit_tile(p, T, tile, bt, v, bg, m, bpos + (ci - c), keys, vals);
+      bpos += __shfl_sync(0xffffffffu, ci, 31);
     }
+  }
 }
 
 // range[bucket] = [begin, end) in the sorted pair array, by boundary detection (buffers pre-zeroed: empty = [0,0))
@@ -360,9 +430,9 @@ void dvx_preprocess_launch(const FrameParams &p, const TreeFrame *trees, const u
     if (p.v_total) { DVX_COUNT_LAUNCH(1); preprocess_kernel<<<blocks_for(p.v_total, PRE_THREADS), PRE_THREADS, 0, st>>>(p, trees, octmask, fvox, pxrect, counters); }
 }
 void dvx_emit_pairs_launch(const FrameParams &p, const TreeFrame *trees, const uint8_t *octmask, const ushort4 *pxrect,
-                           uint64_t *keys, uint32_t *vals, unsigned long long capacity, unsigned long long *counters,
-                           cudaStream_t st) {
-    if (p.v_total) { DVX_COUNT_LAUNCH(1); emit_pairs_kernel<<<blocks_for(p.v_total, PRE_THREADS), PRE_THREADS, 0, st>>>(p, trees, octmask, pxrect, keys, vals,
+                           const FrameVox *fvox, uint64_t *keys, uint32_t *vals, unsigned long long capacity,
+                           unsigned long long *counters, cudaStream_t st) {
+    if (p.v_total) { DVX_COUNT_LAUNCH(1); emit_pairs_kernel<<<blocks_for(p.v_total, PRE_THREADS), PRE_THREADS, 0, st>>>(p, trees, octmask, pxrect, fvox, keys, vals,
                                                                                    capacity, counters); }
 }
 void dvx_ranges_launch(const uint64_t *keys, uint64_t n, uint32_t rank_bits, uint32_t *range_beg, uint32_t *range_end,
