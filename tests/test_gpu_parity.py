@@ -269,3 +269,67 @@ def test_t4_api_errors_and_inference_path(ctx, config1):
     torch.cuda.synchronize()
     assert float(a.abs().max()) == 0.0 and float(r.abs().max()) == 0.0
     f2.release()
+
+
+def test_t1_config3_tile_order_sampled(ctx, config3):
+    """T1 at the headline size: 4 seeded tiles of config 3 (the brute-force hit list costs ~10 s per tile and list)."""
+    import paper_2606_23031_b200 as dvx
+    sc = config3
+    dev = dvx.SceneOnDevice(ctx, sc)
+    _, _, _, frame = dev.render()
+    cam = sc.cameras[0]
+    tw = (cam.width + 15) // 16
+    _, tiles = _tile_mask(cam, 4, 61)
+    n_checked = 0
+    for tile in tiles:
+        ty, tx = divmod(int(tile), tw)
+        for tree in range(len(sc.octrees)):
+            for q in range(8):
+                got = frame.tile_list(int(tile), tree, q)
+                if len(got) == 0:
+                    continue
+                keys = O.order_key(sc.octrees[tree].code[got], q)
+                assert np.all(keys[1:] > keys[:-1])
+                want = O.tile_hit_list(sc, tx, ty, tree, q)
+                pos = {int(v): i for i, v in enumerate(got)}
+                idx = [pos.get(int(v), -1) for v in want]
+                assert len(idx) == 0 or min(idx) >= 0, "hit voxel missing from the tile list"
+                assert all(a < b for a, b in zip(idx, idx[1:]))
+                n_checked += len(want)
+    assert n_checked > 50
+    frame.release()
+    for t in dev.trees:
+        t.close()
+
+
+def test_multi_camera_accumulation_config5_semantics(ctx):
+    """Config 5's contract at a size the oracle handles: several cameras at one ego pose render the same octrees and
+    accumulate into ONE set of gradient buffers (R17); compared on seeded tiles of every camera, all gradient entries."""
+    import paper_2606_23031_b200 as dvx
+    import torch
+    sc = S.make_config(2)
+    cam0 = sc.cameras[0]
+    pos = np.asarray(cam0.c2w).reshape(3, 4)[:, 3]
+    sc.cameras = [S.Camera(cam0.width, cam0.height, cam0.fx, cam0.fy, cam0.cx, cam0.cy, S.look_yaw(pos, np.deg2rad(a)))
+                  for a in (0.0, 45.0, -90.0)]
+    dev = dvx.SceneOnDevice(ctx, sc)
+    grads = dev.zero_grads()
+    ref_dgeo = [np.zeros((t.n_voxels, 8)) for t in sc.octrees]
+    ref_dsh = [np.zeros((t.n_voxels, t.n_sh, 3)) for t in sc.octrees]
+    for c in range(len(sc.cameras)):
+        mask, _ = _tile_mask(sc.cameras[c], 48, 71 + c)
+        gin = sc.image_grads(c, rgb_std=1e-2)
+        gin["rgb"] = gin["rgb"] * mask[:, :, None].astype(np.float32)
+        ref = O.render(sc, cam_index=c, mode=1, mask=mask, grads_in=gin)
+        rgb, depth, alpha, frame = dev.render(c)
+        torch.cuda.synchronize()
+        _check_images(rgb, depth, alpha, ref, mask, scene=None)
+        frame.backward(torch.from_numpy(gin["rgb"]).cuda(), grads=grads)
+        frame.release()
+        for t in range(len(sc.octrees)):
+            ref_dgeo[t] += ref["dgeo"][t]
+            ref_dsh[t] += ref["dsh"][t]
+    torch.cuda.synchronize()
+    for t in range(len(sc.octrees)):
+        _check_grads(grads[t][0], ref_dgeo[t], "dgeo[%d] over 3 cameras" % t)
+        _check_grads(grads[t][1], ref_dsh[t], "dsh[%d] over 3 cameras" % t)
