@@ -19,6 +19,9 @@
  *   O8 compositing        state S=(C,D,T), weighted by accumulated transmittance, T<eps stop
  *                                                                  PAPER.md:107, :297, Alg.1 l.8-9, Eq.2 :111
  *   O9 backward           reverse-mode tape per ray
+ *   O10 sky composite     C = C_voxels + T_final C_sky, C_sky = bilinear sample of a 2-D spherical map at the
+ *                         ray's world direction, texture updated by backpropagation
+ *                                                                  PAPER.md:65 (Sky Modeling), Eq. 2 :111; R21
  *
  * Pinned by tests/test_oracle_pins.py (closed forms P1/P2/P10/P11, Morton-vs-depth order P3,
  * world-frame rewrite P4, empty box P5, finite differences P6, partition of unity P7,
@@ -67,6 +70,36 @@ typedef struct {
   double *dgeo; /* [V][8]   accumulated (+=) */
   double *dsh;  /* [V][C][3] accumulated (+=) */
 } orc_grad;
+
+/* R21: the sky is an equirectangular map tex[H][W][3] over the WORLD direction d (z up): azimuth phi = atan2(d_y, d_x),
+ * polar angle theta = acos(d_z); continuous texel coordinates s = (phi/2pi + 1/2) W - 1/2 (wraps), t = (theta/pi) H - 1/2
+ * (clamped to [0, H-1]); bilinear between the four surrounding texel centres. */
+typedef struct orc_sky_s {
+  uint32_t width, height;
+  const double *tex; /* [H][W][3] */
+  double *dtex;      /* [H][W][3] accumulated (+=), or NULL */
+} orc_sky;
+
+static const double ORC_PI = 3.14159265358979323846;
+
+/* texel indices (into [H][W]) and weights of the bilinear footprint of world direction d */
+static void sky_footprint(const orc_sky *sky, const double d[3], size_t idx[4], double wt[4]) {
+  double W = (double)sky->width, H = (double)sky->height;
+  double dz = d[2] > 1 ? 1 : (d[2] < -1 ? -1 : d[2]);
+  double s = (atan2(d[1], d[0]) / (2 * ORC_PI) + 0.5) * W - 0.5;
+  double t = acos(dz) / ORC_PI * H - 0.5;
+  if (t < 0) t = 0;
+  if (t > H - 1) t = H - 1;
+  double fs = floor(s), ft = floor(t);
+  double as = s - fs, at = t - ft;
+  long i0 = (long)fs, j0 = (long)ft, w = (long)sky->width, h = (long)sky->height;
+  long i1 = i0 + 1, j1 = j0 + 1 < h ? j0 + 1 : h - 1;
+  i0 = ((i0 % w) + w) % w; i1 = ((i1 % w) + w) % w;
+  idx[0] = (size_t)(j0 * w + i0); wt[0] = (1 - as) * (1 - at);
+  idx[1] = (size_t)(j0 * w + i1); wt[1] = as * (1 - at);
+  idx[2] = (size_t)(j1 * w + i0); wt[2] = (1 - as) * at;
+  idx[3] = (size_t)(j1 * w + i1); wt[3] = as * at;
+}
 
 /* ------------------------------------------------------------------ small helpers ---------- */
 
@@ -226,6 +259,7 @@ typedef struct {
   const double *half;        /* [N][3] */
   const orc_camera *cam;
   const orc_opts *opt;
+  const struct orc_sky_s *sky; /* NULL = no sky (Eq. 2 with C_sky = 0) */
 } scene_t;
 
 /* O3: the allowed intervals.  Sort hit actors by (tau_in, index); tau_curr never moves backwards (R2). */
@@ -377,11 +411,31 @@ static void render_ray(const scene_t *sc, int u, int v, const uint32_t *const *c
     used = n + 1;
     if (T < sc->opt->t_stop) break;
   }
+  size_t sk_idx[4] = {0, 0, 0, 0};
+  double sk_wt[4] = {0, 0, 0, 0}, sky_rgb[3] = {0, 0, 0};
+  if (sc->sky) { /* O10, Eq. 2: C = C_voxels + T_final C_sky */
+    sky_footprint(sc->sky, d, sk_idx, sk_wt);
+    for (int ch = 0; ch < 3; ++ch) {
+      for (int n = 0; n < 4; ++n) sky_rgb[ch] += sk_wt[n] * sc->sky->tex[3 * sk_idx[n] + ch];
+      C[ch] += T * sky_rgb[ch];
+    }
+  }
   out5[0] = C[0]; out5[1] = C[1]; out5[2] = C[2]; out5[3] = D; out5[4] = 1.0 - T;
   if (n_used) *n_used = (uint32_t)used;
   if (!g5 || !grads) return;
-  /* O9: reverse sweep over the tape.  Adjoint of T after the last voxel comes from alpha = 1 - T. */
+  /* O9: reverse sweep over the tape.  Adjoint of T after the last voxel comes from alpha = 1 - T and from Eq. 2. */
   double gT = -g5[4];
+  if (sc->sky) {
+    for (int ch = 0; ch < 3; ++ch) {
+      gT += g5[ch] * sky_rgb[ch];
+      if (sc->sky->dtex)
+        for (int n = 0; n < 4; ++n) {
+          double val = g5[ch] * T * sk_wt[n];
+#pragma omp atomic
+          sc->sky->dtex[3 * sk_idx[n] + ch] += val;
+        }
+    }
+  }
   int K = (int)sc->opt->k_samples;
   double raw_k[64], w_k[64 * 8];
   for (size_t n = used; n-- > 0;) {
@@ -542,12 +596,13 @@ static void build_tilelists(const scene_t *sc, tilelists *tl) {
  * doubles (untouched where masked out).  When g_rgb != NULL also runs O9 and accumulates into grads[n_trees]
  * (g_depth / g_alpha may be NULL = zero).  n_used (optional, [H][W]) = sub-segments composited per ray.
  * Returns 0, or -1 on invalid arguments. */
-int orc_render(const orc_camera *cam, int n_trees, const orc_octree *trees, const double *poses, const double *half,
-               const orc_opts *opt, const uint8_t *mask, double *rgb, double *depth, double *alpha,
-               const double *g_rgb, const double *g_depth, const double *g_alpha, orc_grad *grads,
-               uint32_t *n_used) {
+int orc_render_sky(const orc_camera *cam, int n_trees, const orc_octree *trees, const double *poses, const double *half,
+                   const orc_opts *opt, const uint8_t *mask, double *rgb, double *depth, double *alpha,
+                   const double *g_rgb, const double *g_depth, const double *g_alpha, orc_grad *grads,
+                   uint32_t *n_used, const orc_sky *sky) {
   if (!cam || !trees || !opt || n_trees < 1 || opt->k_samples < 1 || opt->k_samples > 64) return -1;
-  scene_t sc = {n_trees, trees, poses, half, cam, opt};
+  if (sky && (!sky->tex || sky->width < 1 || sky->height < 1)) return -1;
+  scene_t sc = {n_trees, trees, poses, half, cam, opt, sky};
   int W = (int)cam->width, H = (int)cam->height;
   int tw = (W + ORC_TILE - 1) / ORC_TILE, th = (H + ORC_TILE - 1) / ORC_TILE;
   tilelists tl = {0, 0};
@@ -587,6 +642,22 @@ int orc_render(const orc_camera *cam, int n_trees, const orc_octree *trees, cons
   }
   free(tl.start); free(tl.ids);
   return 0;
+}
+
+int orc_render(const orc_camera *cam, int n_trees, const orc_octree *trees, const double *poses, const double *half,
+               const orc_opts *opt, const uint8_t *mask, double *rgb, double *depth, double *alpha,
+               const double *g_rgb, const double *g_depth, const double *g_alpha, orc_grad *grads,
+               uint32_t *n_used) {
+  return orc_render_sky(cam, n_trees, trees, poses, half, opt, mask, rgb, depth, alpha, g_rgb, g_depth, g_alpha, grads,
+                        n_used, NULL);
+}
+
+/* the bilinear footprint alone (pin P14) */
+void orc_sky_footprint(uint32_t width, uint32_t height, const double d[3], int64_t idx[4], double wt[4]) {
+  orc_sky sky = {width, height, NULL, NULL};
+  size_t i4[4];
+  sky_footprint(&sky, d, i4, wt);
+  for (int n = 0; n < 4; ++n) idx[n] = (int64_t)i4[n];
 }
 
 static int key_cmp(const void *a, const void *b) {

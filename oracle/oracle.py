@@ -35,6 +35,10 @@ class _Opts(C.Structure):
     _fields_ = [("k_samples", C.c_uint32), ("activation", C.c_uint32), ("t_stop", C.c_double), ("mode", C.c_uint32)]
 
 
+class _Sky(C.Structure):
+    _fields_ = [("width", C.c_uint32), ("height", C.c_uint32), ("tex", C.c_void_p), ("dtex", C.c_void_p)]
+
+
 class _Grad(C.Structure):
     _fields_ = [("dgeo", C.c_void_p), ("dsh", C.c_void_p)]
 
@@ -96,11 +100,12 @@ class _Packed:
         self.hw = (cam.height, cam.width)
 
 
-def render(scene, cam_index=0, mode=0, mask=None, grads_in=None, want_grads=None, **opt):
+def render(scene, cam_index=0, mode=0, mask=None, grads_in=None, want_grads=None, sky=None, **opt):
     """Forward (and backward when ``grads_in`` is given) in double precision.
 
     grads_in: dict with 'rgb' [H,W,3] and optional 'depth', 'alpha' [H,W].
-    Returns dict(rgb, depth, alpha, n_used [, dgeo list, dsh list]).
+    sky: optional equirectangular map [Hs,Ws,3] (O10 / Eq. 2, reading R21); with grads_in also returns 'dsky'.
+    Returns dict(rgb, depth, alpha, n_used [, dgeo list, dsh list, dsky]).
     """
     p = _Packed(scene, cam_index, mode, **opt)
     H, W = p.hw
@@ -120,9 +125,17 @@ def render(scene, cam_index=0, mode=0, mask=None, grads_in=None, want_grads=None
             dg = np.zeros((t.n_voxels, 8)); ds = np.zeros((t.n_voxels, t.n_sh, 3))
             out["dgeo"].append(dg); out["dsh"].append(ds)
             cgrads[n].dgeo, cgrads[n].dsh = _ptr(dg), _ptr(ds)
-    rc = lib().orc_render(C.byref(p.cam), p.n_trees, p.trees, _ptr(p.poses), _ptr(p.half), C.byref(p.opts), _ptr(m),
-                          _ptr(rgb), _ptr(depth), _ptr(alpha), _ptr(g_rgb), _ptr(g_depth), _ptr(g_alpha), cgrads,
-                          _ptr(n_used))
+    csky = None
+    if sky is not None:
+        tex = np.ascontiguousarray(sky, dtype=np.float64)
+        assert tex.ndim == 3 and tex.shape[2] == 3
+        dtex = np.zeros_like(tex) if grads_in is not None else None
+        csky = C.byref(_Sky(tex.shape[1], tex.shape[0], _ptr(tex), _ptr(dtex)))
+        if dtex is not None:
+            out["dsky"] = dtex
+    rc = lib().orc_render_sky(C.byref(p.cam), p.n_trees, p.trees, _ptr(p.poses), _ptr(p.half), C.byref(p.opts), _ptr(m),
+                              _ptr(rgb), _ptr(depth), _ptr(alpha), _ptr(g_rgb), _ptr(g_depth), _ptr(g_alpha), cgrads,
+                              _ptr(n_used), csky)
     if rc != 0:
         raise ValueError("orc_render: invalid arguments")
     out.update(rgb=rgb, depth=depth, alpha=alpha, n_used=n_used)
@@ -146,6 +159,13 @@ def ray_segments(scene, u, v, cam_index=0, cap=1 << 16):
                                int(u), int(v), _ptr(tree), _ptr(vox), _ptr(a), _ptr(b), C.c_int64(cap))
     n = min(n, cap)
     return tree[:n], vox[:n], a[:n], b[:n]
+
+
+def sky_footprint(width, height, direction):
+    d = (C.c_double * 3)(*[float(x) for x in direction])
+    idx = (C.c_int64 * 4)(); wt = (C.c_double * 4)()
+    lib().orc_sky_footprint(C.c_uint32(width), C.c_uint32(height), d, idx, wt)
+    return np.array(list(idx)), np.array(list(wt))
 
 
 def order_key(code, q):

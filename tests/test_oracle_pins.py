@@ -417,3 +417,91 @@ def test_p13_culled_equals_brute_config2_sampled():
     m = mask.astype(bool)
     for k in ("rgb", "depth", "alpha", "n_used"):
         assert np.array_equal(a[k][m], b[k][m])
+
+
+# ---------------------------------------------------------------- P14 sky composite (Eq. 2; reading R21)
+def _sky_tex(h, w, seed=5):
+    rs = np.random.RandomState(seed)
+    return rs.uniform(0.0, 1.0, size=(h, w, 3))
+
+
+def test_p14_constant_sky_and_partition_of_unity():
+    """Eq. 2 with a constant map: C = C_voxels + T_final c_sky exactly, wherever the ray points; empty scene: C = c_sky."""
+    s = S.tiny_random_scene(3, sh_degree=1)
+    c_sky = np.array([0.2, 0.5, 0.9])
+    tex = np.broadcast_to(c_sky, (6, 12, 3)).copy()
+    base, with_sky = O.render(s), O.render(s, sky=tex)
+    assert np.abs(with_sky["rgb"] - (base["rgb"] + (1.0 - base["alpha"])[..., None] * c_sky)).max() < 1e-14
+    assert np.array_equal(with_sky["alpha"], base["alpha"]) and np.array_equal(with_sky["depth"], base["depth"])
+    empty = scene(empty_tree(), cam=s.cameras[0])
+    assert np.abs(O.render(empty, sky=tex)["rgb"] - c_sky).max() < 1e-15
+
+
+def test_p14_single_voxel_closed_form_with_sky():
+    """P1 + Eq. 2: one constant-density voxel of colour c in front of a constant sky: C = alpha c + (1 - alpha) c_sky."""
+    cam = axis_camera(width=1, height=1)
+    v, c = -0.4, 0.7
+    st = tree_from_cells([(1, 1, 1, 1)], geo=v, sh=np.full((1, 1, 3), (c - 0.5) / C0))
+    tex = np.broadcast_to(np.array([0.1, 0.3, 0.6]), (4, 8, 3)).copy()
+    r = O.render(scene(st, cam=cam), sky=tex)
+    alpha = 1.0 - math.exp(-math.exp(v) * 2.0)
+    assert np.abs(r["rgb"][0, 0] - (alpha * c + (1 - alpha) * tex[0, 0])).max() < 1e-13
+
+
+def test_p14_bilinear_footprint_geometry():
+    """The footprint is a bilinear one (4 texels, weights in [0,1] summing to 1), it reproduces maps that are linear in the
+    texel coordinates, the azimuth wraps, and rotating the direction by one texel of azimuth shifts the sample by one
+    column; known directions land where R21 says: +x -> column W/2, horizon -> row H/2, zenith -> row 0."""
+    W, H = 16, 8
+    rs = np.random.RandomState(1)
+    for _ in range(200):
+        d = rs.normal(size=3); d /= np.linalg.norm(d)
+        idx, wt = O.sky_footprint(W, H, d)
+        assert abs(wt.sum() - 1) < 1e-14 and wt.min() >= 0 and wt.max() <= 1
+        jj, ii = idx // W, idx % W
+        assert jj[0] == jj[1] and jj[2] == jj[3] and ii[0] == ii[2] and ii[1] == ii[3]
+        assert ii[1] == (ii[0] + 1) % W and jj[2] in (jj[0], jj[0] + 1)
+        # one texel of azimuth = rotation by 2 pi / W about z
+        a = 2 * math.pi / W
+        d2 = np.array([math.cos(a) * d[0] - math.sin(a) * d[1], math.sin(a) * d[0] + math.cos(a) * d[1], d[2]])
+        idx2, wt2 = O.sky_footprint(W, H, d2)
+        assert np.array_equal(idx2 // W, jj) and np.array_equal(idx2 % W, (ii + 1) % W) and np.abs(wt2 - wt).max() < 1e-9
+    idx, wt = O.sky_footprint(W, H, (1.0, 0.0, 0.0))       # phi = 0, theta = pi/2: between columns W/2-1, W/2 and rows H/2-1, H/2
+    assert sorted(idx.tolist()) == sorted([(H // 2 - 1) * W + W // 2 - 1, (H // 2 - 1) * W + W // 2, (H // 2) * W + W // 2 - 1,
+                                           (H // 2) * W + W // 2]) and np.abs(wt - 0.25).max() < 1e-12
+    idx, wt = O.sky_footprint(W, H, (0.0, 0.0, 1.0))       # zenith: clamped to row 0
+    assert set((idx // W)[wt > 0].tolist()) == {0}
+    idx, wt = O.sky_footprint(W, H, (0.0, 0.0, -1.0))      # nadir: row H-1
+    assert set((idx // W)[wt > 0].tolist()) == {H - 1}
+    # reproduces a map linear in the row index (away from the clamp): value = t = theta / pi * H - 1/2
+    d = np.array([0.3, -0.4, 0.2]); d /= np.linalg.norm(d)
+    idx, wt = O.sky_footprint(W, H, d)
+    assert abs((wt * (idx // W)).sum() - (math.acos(d[2]) / math.pi * H - 0.5)) < 1e-12
+
+
+def test_p14_finite_difference_gradients_with_sky():
+    """O9 + O10: analytic gradients of the texture, the corner densities and the SH coefficients with the sky on."""
+    s = S.tiny_random_scene(9, sh_degree=1, colour_floor=True)
+    for t in s.octrees:
+        t.geo = t.geo.astype(np.float64)
+        t.sh = t.sh.astype(np.float64)
+    tex = _sky_tex(5, 9)
+    g = s.image_grads(0, 1.0, 0.3, 1.0)
+    r = O.render(s, grads_in=g, sky=tex)
+
+    def loss():
+        q = O.render(s, sky=tex)
+        return (q["rgb"] * g["rgb"]).sum() + (q["depth"] * g["depth"]).sum() + (q["alpha"] * g["alpha"]).sum()
+
+    h = 1e-5
+    checks = [(tex, r["dsky"])] + [(t.geo, r["dgeo"][n]) for n, t in enumerate(s.octrees)]
+    for arr, ana in checks:
+        flat, aflat = arr.reshape(-1), ana.reshape(-1)
+        scale = max(np.abs(aflat).max(), 1e-12)
+        assert np.count_nonzero(aflat) > 10
+        for idx in range(0, flat.shape[0], 3):
+            keep = flat[idx]
+            flat[idx] = keep + h; lp = loss()
+            flat[idx] = keep - h; lm = loss()
+            flat[idx] = keep
+            assert abs((lp - lm) / (2 * h) - aflat[idx]) / scale < 1e-6
