@@ -85,11 +85,22 @@ typedef struct {
   float far_;    /* tau_max */
 } dvx_camera;
 
+/* Sky ("Sky Modeling", Eq. 2 :111): C = C_voxels + T_final * C_sky, C_sky = bilinear sample of a 2-D spherical
+ * map at the ray's WORLD direction d (z up).  Reading R21: equirectangular, phi = atan2(d_y, d_x), theta = acos(d_z), texel
+ * coordinates s = (phi/2pi + 1/2) W - 1/2 (wraps), t = (theta/pi) H - 1/2 (clamped to [0, H-1]).  Depth and alpha are not
+ * affected.  dvx_backward accumulates (+=) the texture gradient into dtex when it is not NULL. */
+typedef struct {
+  uint32_t width, height; /* W, H >= 1 */
+  const float *tex;       /* DEVICE [H][W][3], borrowed until the frame is released */
+  float *dtex;            /* DEVICE [H][W][3] or NULL */
+} dvx_sky;
+
 typedef struct {
   uint32_t k_samples;  /* K midpoint samples per clipped ray-voxel segment, 1..8 (R6) */
   uint32_t activation; /* 0 = exp (default), 1 = exp-linear with theta = 1.1 (R5) */
   float t_stop;        /* early termination T < t_stop, tested after every voxel (R3); 0 disables */
   uint32_t flags;      /* DVX_FLAG_* */
+  const dvx_sky *sky;  /* HOST pointer, read before the call returns; NULL = no sky (C_sky = 0) */
 } dvx_render_opts;
 #define DVX_FLAG_COUNTERS 1u /* maintain q_test / q_hit / pairs_eff (slower; off in timed runs) */
 #define DVX_FLAG_NAIVE 2u    /* debug: per-thread in-order walker instead of the cooperative tile kernel */

@@ -41,8 +41,13 @@ class Camera(C.Structure):
                 ("cy", C.c_float), ("c2w", C.c_float * 12), ("near_", C.c_float), ("far_", C.c_float)]
 
 
+class Sky(C.Structure):
+    _fields_ = [("width", C.c_uint32), ("height", C.c_uint32), ("tex", C.c_void_p), ("dtex", C.c_void_p)]
+
+
 class RenderOpts(C.Structure):
-    _fields_ = [("k_samples", C.c_uint32), ("activation", C.c_uint32), ("t_stop", C.c_float), ("flags", C.c_uint32)]
+    _fields_ = [("k_samples", C.c_uint32), ("activation", C.c_uint32), ("t_stop", C.c_float), ("flags", C.c_uint32),
+                ("sky", C.POINTER(Sky))]
 
 
 class Image(C.Structure):
@@ -163,10 +168,11 @@ class Context:
 
     # ------------------------------------------------------------------ render / backward
     def render(self, cam, static, actors=(), poses=None, box_half=None, k_samples=8, activation=0, t_stop=1e-4, flags=0,
-               save=True, out=None, host=False):
+               save=True, out=None, host=False, sky=None, dsky=None):
         """dvx_render (host=False: device image tensors) or dvx_render_host (host=True: ``out`` must be three pinned
         CPU tensors).  cam: binding.Camera; poses [N,12] / box_half [N,3] host float32 arrays.
-        Returns (rgb [H,W,3], depth [H,W], alpha [H,W], Frame or None)."""
+        sky: optional CUDA float32 tensor [Hs,Ws,3] (Eq. 2); dsky: tensor of the same shape that dvx_backward accumulates
+        the texture gradient into.  Returns (rgb [H,W,3], depth [H,W], alpha [H,W], Frame or None)."""
         torch = self.torch
         H, W = cam.height, cam.width
         if host and out is None:
@@ -183,7 +189,11 @@ class Context:
         poses = np.ascontiguousarray(np.zeros((0, 12)) if poses is None else poses, dtype=np.float32).reshape(-1)
         half = np.ascontiguousarray(np.zeros((0, 3)) if box_half is None else box_half, dtype=np.float32).reshape(-1)
         assert poses.size == 12 * n and half.size == 3 * n
-        opts = RenderOpts(k_samples, activation, t_stop, flags)
+        opts = RenderOpts(k_samples, activation, t_stop, flags, None)
+        if sky is not None:
+            assert sky.is_cuda and sky.dtype == torch.float32 and sky.dim() == 3 and sky.shape[2] == 3 and sky.is_contiguous()
+            csky = Sky(sky.shape[1], sky.shape[0], sky.data_ptr(), dsky.data_ptr() if dsky is not None else None)
+            opts.sky = C.pointer(csky)
         img = Image(rgb.data_ptr(), depth.data_ptr(), alpha.data_ptr())
         fh = C.c_void_p()
         fn = self.lib.dvx_render_host if host else self.lib.dvx_render
@@ -191,6 +201,8 @@ class Context:
                 half.ctypes.data_as(C.c_void_p), C.byref(opts), img, C.byref(fh) if save else None)
         self.check(rc)
         frame = Frame(self, fh, [static] + list(actors)) if save else None
+        if frame is not None:
+            frame.keep = (sky, dsky)   # the library borrows these until the frame is released
         return rgb, depth, alpha, frame
 
 
@@ -290,12 +302,12 @@ class SceneOnDevice:
         self.box_half = np.ascontiguousarray(scene.box_half, dtype=np.float32)
         self.cams = [camera_from(c) for c in scene.cameras]
 
-    def render(self, cam_index=0, save=True, flags=0, out=None, host=False, **opt):
+    def render(self, cam_index=0, save=True, flags=0, out=None, host=False, sky=None, dsky=None, **opt):
         s = self.scene
         kw = dict(k_samples=s.k_samples, activation=s.activation, t_stop=s.t_stop)
         kw.update(opt)
         return self.ctx.render(self.cams[cam_index], self.trees[0], self.trees[1:], self.poses, self.box_half, flags=flags,
-                               save=save, out=out, host=host, **kw)
+                               save=save, out=out, host=host, sky=sky, dsky=dsky, **kw)
 
     def zero_grads(self):
         torch = self.ctx.torch

@@ -46,6 +46,7 @@ struct dvx_frame {
   EventSet *es = nullptr;
   cudaEvent_t *ev = nullptr;  // = es->ev
   Buf eff_end;
+  dvx_sky sky = {0, 0, nullptr, nullptr};
   bool did_backward = false;
 };
 
@@ -307,11 +308,13 @@ dvx_status dvx_render(dvx_ctx *ctx, const dvx_camera *cam, const dvx_octree *sta
   if (!cam || !static_tree || !out.rgb || !out.depth || !out.alpha) return fail(ctx, DVX_ERR_INVALID_ARG, "NULL argument");
   if (n_actors > DVX_MAX_ACTORS) return fail(ctx, DVX_ERR_INVALID_ARG, "n_actors > 64");
   if (n_actors && (!actors || !poses_l2w || !box_half)) return fail(ctx, DVX_ERR_INVALID_ARG, "actor arrays are NULL");
-  dvx_render_opts o = {8u, 0u, 1e-4f, 0u};
+  dvx_render_opts o = {8u, 0u, 1e-4f, 0u, nullptr};
   if (opts) o = *opts;
   if (o.k_samples < 1 || o.k_samples > 8) return fail(ctx, DVX_ERR_INVALID_ARG, "k_samples must be in [1,8]");
   if (o.activation > 1) return fail(ctx, DVX_ERR_INVALID_ARG, "unknown activation");
   if (!(o.t_stop >= 0.f)) return fail(ctx, DVX_ERR_INVALID_ARG, "t_stop must be >= 0");
+  if (o.sky && (!o.sky->tex || o.sky->width == 0 || o.sky->height == 0 || o.sky->width > 65536 || o.sky->height > 32768))
+    return fail(ctx, DVX_ERR_INVALID_ARG, "bad sky map (NULL texture or size)");
   if (cam->width == 0 || cam->height == 0 || cam->width > 65535 || cam->height > 65535 || !(cam->fx > 0.f) ||
       !(cam->fy > 0.f) || !(cam->near_ > 0.f) || !(cam->far_ > cam->near_))
     return fail(ctx, DVX_ERR_INVALID_ARG, "bad camera (size, focal length, near/far)");
@@ -332,6 +335,9 @@ dvx_status dvx_render(dvx_ctx *ctx, const dvx_camera *cam, const dvx_octree *sta
   p.tiles_x = (cam->width + DVX_TILE - 1) / DVX_TILE; p.tiles_y = (cam->height + DVX_TILE - 1) / DVX_TILE;
   p.n_tiles = p.tiles_x * p.tiles_y; p.n_trees = 1 + n_actors;
   p.fx = cam->fx; p.fy = cam->fy; p.cx = cam->cx; p.cy = cam->cy; p.near_ = cam->near_; p.far_ = cam->far_;
+  for (int r = 0; r < 3; ++r)
+    for (int c = 0; c < 3; ++c) p.Rc[3 * r + c] = (double)cam->c2w[4 * r + c];
+  if (o.sky) f->sky = *o.sky;
   p.inv_fx = 1.0 / (double)cam->fx; p.inv_fy = 1.0 / (double)cam->fy; p.cx_d = (double)cam->cx; p.cy_d = (double)cam->cy;
   {  // every point of a ray at tau >= near has z_cam >= near * min_pixels cos(angle to the axis) > zclip
     double mc = 1.0;
@@ -431,6 +437,7 @@ dvx_status dvx_render(dvx_ctx *ctx, const dvx_camera *cam, const dvx_octree *sta
   A.rgb = out.rgb; A.depth = out.depth; A.alpha = out.alpha;
   A.sv_rgbd = (float *)f->sv_rgbd.p; A.sv_T = (float *)f->sv_T.p; A.sv_nused = (uint32_t *)f->sv_nused.p;
   A.counters = counters;
+  A.sky_tex = f->sky.tex; A.sky_w = f->sky.width; A.sky_h = f->sky.height;
   if (p.flags & DVX_FLAG_COUNTERS) {
     if (!buf_alloc(ctx, f->eff_end, sizeof(uint32_t) * (size_t)p.n_buckets)) { frame_free(ctx, f); return fail(ctx, DVX_ERR_OOM, "dvx_render: allocator returned NULL"); }
     CU(cudaMemsetAsync(f->eff_end.p, 0, sizeof(uint32_t) * (size_t)p.n_buckets, st));
@@ -476,6 +483,7 @@ dvx_status dvx_backward(dvx_ctx *ctx, dvx_frame *f, const float *dL_drgb, const 
   A.sv_rgbd = (float *)f->sv_rgbd.p; A.sv_T = (float *)f->sv_T.p; A.sv_nused = (uint32_t *)f->sv_nused.p;
   A.counters = (unsigned long long *)f->counters.p;
   A.g_rgb = dL_drgb; A.g_depth = dL_ddepth; A.g_alpha = dL_dalpha; A.drgb = drgb;
+  A.sky_tex = f->sky.tex; A.sky_w = f->sky.width; A.sky_h = f->sky.height; A.sky_dtex = f->sky.dtex;
   CU(cudaEventRecord(f->ev[7], st));
   dvx_composite_launch(A, true, st);
   CU(cudaEventRecord(f->ev[8], st));

@@ -120,7 +120,7 @@ __device__ __forceinline__ void walk_list(const CompositeArgs &A, const TreeFram
 }
 
 template <bool BWD>
-__global__ void __launch_bounds__(TILE_THREADS) composite_naive_kernel(const CompositeArgs A) {
+__global__ void __launch_bounds__(TILE_THREADS) composite_naive_kernel(const __grid_constant__ CompositeArgs A) {
   const FrameParams &p = A.p;
   const int tile = blockIdx.x;
   const int tx = tile % p.tiles_x, ty = tile / p.tiles_x;
@@ -140,6 +140,8 @@ __global__ void __launch_bounds__(TILE_THREADS) composite_naive_kernel(const Com
     S.Xtot = S.gC[0] * cd.x + S.gC[1] * cd.y + S.gC[2] * cd.z + S.gD * cd.w;
     S.T_final = A.sv_T[pix];
     S.n_stop = A.sv_nused[pix];
+    // Eq. 2: dL/dT_final also has g_C . C_sky; with alpha = 1 - T_final that is an alpha gradient of -(g_C . C_sky)
+    if (A.sky_tex) S.gA -= dvx_sky_backward(&A, u, v, S.gC[0], S.gC[1], S.gC[2], S.T_final);
     if (S.n_stop == 0) S.done = true;
   }
 
@@ -193,7 +195,9 @@ __global__ void __launch_bounds__(TILE_THREADS) composite_naive_kernel(const Com
   }
 
   if (!BWD && inside) {
-    A.rgb[3 * pix] = S.C[0]; A.rgb[3 * pix + 1] = S.C[1]; A.rgb[3 * pix + 2] = S.C[2];
+    float3 sky = make_float3(0.f, 0.f, 0.f);
+    if (A.sky_tex) sky = dvx_sky_forward(&A, u, v, S.T);  // Eq. 2: C = C_voxels + T_final C_sky
+    A.rgb[3 * pix] = S.C[0] + sky.x; A.rgb[3 * pix + 1] = S.C[1] + sky.y; A.rgb[3 * pix + 2] = S.C[2] + sky.z;
     A.depth[pix] = S.D;
     A.alpha[pix] = 1.0f - S.T;
     if (A.sv_rgbd) {

@@ -366,7 +366,7 @@ __device__ __noinline__ float2 axis_parallel_fix(const TreeFrame *T, uint32_t id
 }
 
 template <bool BWD, bool CNT>
-__global__ void __launch_bounds__(TILE_THREADS, DVX_TILE_MIN_CTAS) composite_tile_kernel(const CompositeArgs A) {
+__global__ void __launch_bounds__(TILE_THREADS, DVX_TILE_MIN_CTAS) composite_tile_kernel(const __grid_constant__ CompositeArgs A) {
   __shared__ WarpQueue<BWD> s_queue[TILE_WARPS];
   const FrameParams &p = A.p;
   const int tile = blockIdx.x;
@@ -391,6 +391,8 @@ __global__ void __launch_bounds__(TILE_THREADS, DVX_TILE_MIN_CTAS) composite_til
     S.Xtot = S.gC0 * cd.x + S.gC1 * cd.y + S.gC2 * cd.z + S.gD * cd.w;
     S.T_final = A.sv_T[pix];
     S.n_stop = A.sv_nused[pix];
+    // Eq. 2: dL/dT_final also has g_C . C_sky; with alpha = 1 - T_final that is an alpha gradient of -(g_C . C_sky)
+    if (A.sky_tex) S.gA -= dvx_sky_backward(&A, u, v, S.gC0, S.gC1, S.gC2, S.T_final);
     if (S.n_stop == 0) S.done = true;
   }
 
@@ -590,7 +592,9 @@ __global__ void __launch_bounds__(TILE_THREADS, DVX_TILE_MIN_CTAS) composite_til
   while (n_items > 0) flush_batch<BWD>(A, lane, Q, n_items, head, my_bits, S);
 
   if (!BWD && inside) {
-    A.rgb[3 * pix] = S.C0; A.rgb[3 * pix + 1] = S.C1; A.rgb[3 * pix + 2] = S.C2;
+    float3 sky = make_float3(0.f, 0.f, 0.f);
+    if (A.sky_tex) sky = dvx_sky_forward(&A, u, v, S.T);  // Eq. 2: C = C_voxels + T_final C_sky
+    A.rgb[3 * pix] = S.C0 + sky.x; A.rgb[3 * pix + 1] = S.C1 + sky.y; A.rgb[3 * pix + 2] = S.C2 + sky.z;
     A.depth[pix] = S.D;
     A.alpha[pix] = 1.0f - S.T;
     if (A.sv_rgbd) {

@@ -32,6 +32,7 @@ struct FrameParams {
   uint32_t width, height, tiles_x, tiles_y, n_tiles, n_trees;
   float fx, fy, cx, cy, near_, far_, zclip;
   double inv_fx, inv_fy, cx_d, cy_d;  // fp64 copies for the per-pixel ray set-up of the tile kernel
+  double Rc[9];                       // camera rotation (row-major, camera -> world): world direction of a pixel (sky)
   uint32_t k_samples, activation, flags;
   float t_stop, inv_k;  // inv_k = 1 / k_samples
   uint32_t rank_bits;   // sort key = (bucket << rank_bits) | rank ; bucket = (tile*n_trees + tree)*8 + octant
@@ -64,6 +65,9 @@ struct CompositeArgs {
   uint32_t *sv_nused;          // [H*W]
   unsigned long long *counters;
   uint32_t *eff_end;           // [n_buckets] furthest list position any warp streamed (DVX_FLAG_COUNTERS only, else NULL)
+  const float *sky_tex;        // [sky_h][sky_w][3] or NULL (Eq. 2)
+  float *sky_dtex;             // backward: texture gradient, or NULL
+  uint32_t sky_w, sky_h;
   // backward
   const float *g_rgb, *g_depth, *g_alpha;
   float *drgb;                 // [v_total][4] scratch: dL/drgb_v

@@ -75,3 +75,64 @@ __device__ __forceinline__ bool ray_box(const TreeFrame &T, const Ray &r, float 
   return true;
 }
 
+
+
+// O10 / Eq. 2 (reading R21): bilinear footprint of pixel (u, v)'s WORLD direction in the equirectangular
+// sky map.  Once per pixel, in fp64 up to the texel coordinates.  idx = texel indices into [H][W], wt = weights.
+__device__ __forceinline__ void dvx_sky_footprint(const FrameParams &p, uint32_t W, uint32_t H, int u, int v, uint32_t idx[4],
+                                                  float wt[4]) {
+  const double xd = ((double)u + 0.5 - p.cx_d) * p.inv_fx, yd = ((double)v + 0.5 - p.cy_d) * p.inv_fy;
+  const double rn = rsqrt(xd * xd + yd * yd + 1.0);
+  const double dx = (p.Rc[0] * xd + p.Rc[1] * yd + p.Rc[2]) * rn, dy = (p.Rc[3] * xd + p.Rc[4] * yd + p.Rc[5]) * rn;
+  const double dz = fmin(1.0, fmax(-1.0, (p.Rc[6] * xd + p.Rc[7] * yd + p.Rc[8]) * rn));
+  const double PI = 3.14159265358979323846;
+  const double s = (atan2(dy, dx) / (2.0 * PI) + 0.5) * (double)W - 0.5;
+  const double t = fmin((double)H - 1.0, fmax(0.0, acos(dz) / PI * (double)H - 0.5));
+  const double fs = floor(s), ft = floor(t);
+  const float as = (float)(s - fs), at = (float)(t - ft);
+  long long i0 = (long long)fs, j0 = (long long)ft;
+  const long long w = (long long)W, h = (long long)H;
+  long long i1 = i0 + 1;
+  const long long j1 = j0 + 1 < h ? j0 + 1 : h - 1;
+  i0 = ((i0 % w) + w) % w;
+  i1 = ((i1 % w) + w) % w;
+  idx[0] = (uint32_t)(j0 * w + i0); wt[0] = (1.f - as) * (1.f - at);
+  idx[1] = (uint32_t)(j0 * w + i1); wt[1] = as * (1.f - at);
+  idx[2] = (uint32_t)(j1 * w + i0); wt[2] = (1.f - as) * at;
+  idx[3] = (uint32_t)(j1 * w + i1); wt[3] = as * at;
+}
+__device__ __forceinline__ void dvx_sky_colour(const float *tex, const uint32_t idx[4], const float wt[4], float rgb[3]) {
+  rgb[0] = rgb[1] = rgb[2] = 0.f;
+#pragma unroll
+  for (int n = 0; n < 4; ++n) {
+    const float *t = tex + 3 * (size_t)idx[n];
+    rgb[0] = fmaf(wt[n], __ldg(t), rgb[0]); rgb[1] = fmaf(wt[n], __ldg(t + 1), rgb[1]); rgb[2] = fmaf(wt[n], __ldg(t + 2), rgb[2]);
+  }
+}
+
+// Forward: T_final * C_sky for pixel (u, v) (added to C_voxels by the caller, Eq. 2).
+static __device__ __noinline__ float3 dvx_sky_forward(const CompositeArgs *A, int u, int v, float T_final) {
+  uint32_t idx[4];
+  float wt[4], c[3];
+  dvx_sky_footprint(A->p, A->sky_w, A->sky_h, u, v, idx, wt);
+  dvx_sky_colour(A->sky_tex, idx, wt, c);
+  return make_float3(T_final * c[0], T_final * c[1], T_final * c[2]);
+}
+// Backward of Eq. 2 for one pixel: dL/dtex += g_C T_final w (4 texels), and returns g_C . C_sky, the part of dL/dT_final
+// that comes through the sky term (the caller folds it into the alpha gradient: alpha = 1 - T_final).
+static __device__ __noinline__ float dvx_sky_backward(const CompositeArgs *A, int u, int v, float g0, float g1, float g2, float T_final) {
+  uint32_t idx[4];
+  float wt[4], c[3];
+  dvx_sky_footprint(A->p, A->sky_w, A->sky_h, u, v, idx, wt);
+  dvx_sky_colour(A->sky_tex, idx, wt, c);
+  if (A->sky_dtex) {
+#pragma unroll
+    for (int n = 0; n < 4; ++n) {
+      if (wt[n] == 0.f) continue;
+      float *t = A->sky_dtex + 3 * (size_t)idx[n];
+      const float k = T_final * wt[n];
+      atomicAdd(t, g0 * k); atomicAdd(t + 1, g1 * k); atomicAdd(t + 2, g2 * k);
+    }
+  }
+  return g0 * c[0] + g1 * c[1] + g2 * c[2];
+}

@@ -143,3 +143,61 @@ def test_no_actors_and_empty_trees(ctx):
 def test_sh_degrees_0_2_3(ctx):
     for deg in (0, 2, 3):
         _compare(ctx, S.tiny_random_scene(31 + deg, sh_degree=deg, width=16, height=12))
+
+
+def _sky_map(h, w, seed):
+    idx = np.arange(h * w * 3, dtype=np.uint64)
+    return S.rng.uniform(seed, 950, idx).astype(np.float32).reshape(h, w, 3)
+
+
+@pytest.mark.parametrize("seed,hw", [(41, (16, 32)), (43, (5, 9)), (47, (1, 1))])
+def test_sky_composite_eq2(ctx, seed, hw):
+    """Eq. 2 (reading R21): C = C_voxels + T_final C_sky through both kernels, and the backward's texture,
+    density and SH gradients, against the oracle; depth and alpha must not change when the sky is switched on."""
+    import paper_2606_23031_b200 as dvx
+    import torch
+    sc = _round_to_f32(S.tiny_random_scene(seed, sh_degree=1, width=40, height=24))
+    tex = _sky_map(hw[0], hw[1], seed)
+    gin = sc.image_grads(rgb_std=1e-2, depth_std=1e-3, alpha_std=1e-2)
+    ref = O.render(sc, mode=0, grads_in=gin, sky=tex)
+    assert np.abs(ref["dsky"]).max() > 0
+    dev = dvx.SceneOnDevice(ctx, sc)
+    tex_d = torch.from_numpy(tex).cuda()
+    for flags in (0, dvx.FLAG_NAIVE):
+        dsky = torch.zeros_like(tex_d)
+        rgb, depth, alpha, frame = dev.render(flags=flags, sky=tex_d, dsky=dsky)
+        rgb0, depth0, alpha0, _ = dev.render(flags=flags, save=False)
+        torch.cuda.synchronize()
+        assert torch.equal(depth, depth0) and torch.equal(alpha, alpha0)
+        assert np.abs(rgb.cpu().numpy() - ref["rgb"]).max() <= RGB_TOL
+        assert np.abs(alpha.cpu().numpy() - ref["alpha"]).max() <= RGB_TOL
+        g = [torch.from_numpy(gin[k]).cuda() for k in ("rgb", "depth", "alpha")]
+        grads = frame.backward(g[0], g[1], g[2])
+        torch.cuda.synchronize()
+        pairs = [(dsky, ref["dsky"], "dsky")]
+        for t in range(len(sc.octrees)):
+            pairs += [(grads[t][0], ref["dgeo"][t], "dgeo[%d]" % t), (grads[t][1], ref["dsh"][t], "dsh[%d]" % t)]
+        for got, want, name in pairs:
+            err = np.abs(got.cpu().numpy().astype(np.float64) - want)
+            bound = GRAD_REL * np.abs(want) + GRAD_ABS
+            assert (err <= bound).all(), "%s flags %d: worst excess %g" % (name, flags, (err - bound).max())
+        frame.release()
+
+
+def test_sky_on_config1_and_empty_scene(ctx, config1):
+    """An empty scene renders the sky map itself (T_final = 1); config 1 with a sky at full tile coverage."""
+    import paper_2606_23031_b200 as dvx
+    import torch
+    tex = _sky_map(32, 64, 3)
+    tex_d = torch.from_numpy(tex).cuda()
+    sc = config1
+    dev = dvx.SceneOnDevice(ctx, sc)
+    rgb, _, _, _ = dev.render(save=False, sky=tex_d)
+    torch.cuda.synchronize()
+    assert np.abs(rgb.cpu().numpy() - O.render(sc, mode=0, sky=tex)["rgb"]).max() <= RGB_TOL
+    empty = ctx.octree(torch.zeros(0, dtype=torch.int64, device="cuda"), torch.zeros((0, 8), device="cuda"),
+                       torch.zeros((0, 1, 3), device="cuda"), (0, 0, 0), 1.0, 0)
+    r, d, a, _ = ctx.render(dev.cams[0], empty, save=False, sky=tex_d)
+    torch.cuda.synchronize()
+    es = scene(empty_tree(), cam=sc.cameras[0])
+    assert np.abs(r.cpu().numpy() - O.render(es, sky=tex)["rgb"]).max() <= 1e-5 and float(a.abs().max()) == 0.0
