@@ -63,6 +63,7 @@ struct WarpQueue {
   EntryRec ent[32];
   Item item[QCAP];              // ring
   double d0[3];                 // the warp's reference direction for the list being served
+  float4 rgbm[32];              // phase B -> C: per batch item, the voxel's RGB and clamp bits (fetched by the item's lane)
   float wg[BWD ? 3 : 1][QCAP];  // backward phase C: T alpha g_C per item, zero where the colour clamp is active
 };
 
@@ -246,7 +247,10 @@ __device__ __forceinline__ void flush_batch(const CompositeArgs &A, int lane, Wa
   float M[4];
   uint32_t my_id = NONE, my_meta = 0;
   const int at_b = (head + lane) & (QCAP - 1);
-  if (lane < count) Q.item[at_b].tau = integrate_item<BWD>(A, Q, at_b, my_id, my_meta, G, M);
+  if (lane < count) {
+    Q.item[at_b].tau = integrate_item<BWD>(A, Q, at_b, my_id, my_meta, G, M);
+    Q.rgbm[lane] = __ldg(reinterpret_cast<const float4 *>(A.fvox + my_id) + 1);  // keeps the global load out of C's serial loop
+  }
   __syncwarp();
   // -- C: lane = pixel; its own items of the batch in queue order = front-to-back order along its ray
   uint32_t mine = (uint32_t)my_bits;
@@ -256,7 +260,7 @@ __device__ __forceinline__ void flush_batch(const CompositeArgs &A, int lane, Wa
     mine &= mine - 1;
     const int at = (head + i) & (QCAP - 1);
     if (!S.done) {
-      const float4 f1 = __ldg(reinterpret_cast<const float4 *>(A.fvox + Q.item[at].id) + 1);
+      const float4 f1 = Q.rgbm[i];
       const float tau = Q.item[at].tau;
       const float mid = Q.item[at].mid;
       const float e = ex2_approx(-tau * LOG2E);
