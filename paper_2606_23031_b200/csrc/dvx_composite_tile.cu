@@ -5,7 +5,7 @@
 //           alpha = 1 - exp(-sum sigma dt), blend weighted by T
 //   step 5  the matching backward, run-reduced over the warp before the vector atomics
 //
-// One CTA per 16x16 tile, one warp per 8x4 pixel block, one lane per pixel.  The work of a warp is split into phases so
+// One CTA per 16x16 tile, one warp per 4x8 pixel block (DVX_WARP_W x 32/DVX_WARP_W; 4x8 measured best on config 3), one lane per pixel.  The work of a warp is split into phases so
 // that the expensive arithmetic always runs on full warps:
 //   A  geometry   the warp walks the tile's sorted list 32 entries at a time.  First lane = entry: coalesced id load,
 //                 pixel-rectangle pre-filter, Morton decode and - in fp64, once per (warp, entry) - the voxel centre
@@ -33,6 +33,10 @@ constexpr int TILE_WARPS = TILE_THREADS / 32;
 #ifndef DVX_TILE_MIN_CTAS
 #define DVX_TILE_MIN_CTAS 3
 #endif
+#ifndef DVX_WARP_W
+#define DVX_WARP_W 4   // a warp covers DVX_WARP_W x (32 / DVX_WARP_W) pixels
+#endif
+constexpr int WARP_W = DVX_WARP_W, WARP_H = 32 / DVX_WARP_W, WARPS_X = DVX_TILE / WARP_W;
 constexpr int QCAP = 64;              // ring capacity per warp: at most 31 left-over items + 32 of one entry
 constexpr uint32_t NONE = 0xFFFFFFFFu;
 constexpr float LOG2E = 1.4426950408889634f;
@@ -377,10 +381,10 @@ __global__ void __launch_bounds__(TILE_THREADS, DVX_TILE_MIN_CTAS) composite_til
   const int warp = threadIdx.x >> 5;
   const int lane = threadIdx.x & 31;
   const uint32_t lt = (1u << lane) - 1u;
-  const int wu0 = (tile % p.tiles_x) * DVX_TILE + (warp & 1) * 8;   // pixel of lane 0 of this warp
-  const int wv0 = (tile / p.tiles_x) * DVX_TILE + (warp >> 1) * 4;
+  const int wu0 = (tile % p.tiles_x) * DVX_TILE + (warp % WARPS_X) * WARP_W;   // pixel of lane 0 of this warp
+  const int wv0 = (tile / p.tiles_x) * DVX_TILE + (warp / WARPS_X) * WARP_H;
   WarpQueue<BWD> &Q = s_queue[warp];
-  const int u = wu0 + (lane & 7), v = wv0 + (lane >> 3);
+  const int u = wu0 + lane % WARP_W, v = wv0 + lane / WARP_W;
   const bool inside = u < (int)p.width && v < (int)p.height;
   const size_t pix = (size_t)v * p.width + u;
 
@@ -449,7 +453,7 @@ __global__ void __launch_bounds__(TILE_THREADS, DVX_TILE_MIN_CTAS) composite_til
   int n_items = 0, head = 0;
   unsigned long long my_bits = 0;
   unsigned long long q_test = 0;
-  const uint32_t ru0 = (uint32_t)wu0, rv0 = (uint32_t)wv0, ru1 = ru0 + 7u, rv1 = rv0 + 3u;
+  const uint32_t ru0 = (uint32_t)wu0, rv0 = (uint32_t)wv0, ru1 = ru0 + WARP_W - 1, rv1 = rv0 + WARP_H - 1;
   uint32_t seg_tree = NONE;  // pending segment of this lane: tree and interval [lo, hi]
   float lo = 0.f, hi = 0.f;
 
