@@ -22,6 +22,8 @@
  *   O10 sky composite     C = C_voxels + T_final C_sky, C_sky = bilinear sample of a 2-D spherical map at the
  *                         ray's world direction, texture updated by backpropagation
  *                                                                  PAPER.md:65 (Sky Modeling), Eq. 2 :111; R21
+ *   O11 normal map        N = sum_j T_j alpha_j n_j, n_j = the voxel's normal (state tuple S = (C, D, N, T, tau_curr))
+ *                                                                  PAPER.md:107, :297; R22
  *
  * Pinned by tests/test_oracle_pins.py (closed forms P1/P2/P10/P11, Morton-vs-depth order P3,
  * world-frame rewrite P4, empty box P5, finite differences P6, partition of unity P7,
@@ -350,6 +352,56 @@ static void voxel_colour(const orc_octree *t, uint32_t v, const double o_frame[3
   }
 }
 
+/* R22: the voxel's normal = minus the gradient of its trilinear raw density at the voxel centre, normalised:
+ * g_a = 1/4 sum over the four corner pairs along axis a of (geo[b_a = 1] - geo[b_a = 0]) (so a constant voxel has g = 0
+ * exactly), n_local = -g / max(|g|, ORC_NRM_EPS) (a flat voxel fades to no normal instead of a random unit vector),
+ * rotated into the WORLD frame by the actor's R_i (identity for the static octree).
+ * Outputs: nw[3] world normal; g[3] local gradient, gn = |g| (for the backward). */
+#define ORC_NRM_EPS 1e-6
+static void voxel_normal(const scene_t *sc, uint32_t tree, uint32_t v, double nw[3], double g[3], double *gn) {
+  const orc_octree *t = &sc->trees[tree];
+  for (int a = 0; a < 3; ++a) {
+    int bit = 4 >> a;
+    double acc = 0;
+    for (int c = 0; c < 8; ++c)
+      if (!(c & bit)) acc += geo_at(t, v, c | bit) - geo_at(t, v, c);
+    g[a] = 0.25 * acc;
+  }
+  *gn = sqrt(g[0] * g[0] + g[1] * g[1] + g[2] * g[2]);
+  double den = *gn > ORC_NRM_EPS ? *gn : ORC_NRM_EPS;
+  double nl[3] = {-g[0] / den, -g[1] / den, -g[2] / den};
+  if (tree == 0) { memcpy(nw, nl, sizeof nl); return; }
+  const double *P = sc->poses + 12 * (tree - 1);
+  for (int r = 0; r < 3; ++r) nw[r] = P[4 * r] * nl[0] + P[4 * r + 1] * nl[1] + P[4 * r + 2] * nl[2];
+}
+/* adjoint of voxel_normal: gnw = dL/dn_world -> accumulates dL/dgeo[v][0..8) */
+static void voxel_normal_backward(const scene_t *sc, uint32_t tree, uint32_t v, const double gnw[3], double *dgeo_v) {
+  double nw[3], g[3], gn;
+  voxel_normal(sc, tree, v, nw, g, &gn);
+  double gl[3];
+  if (tree == 0) memcpy(gl, gnw, sizeof gl);
+  else {
+    const double *P = sc->poses + 12 * (tree - 1);
+    for (int c = 0; c < 3; ++c) gl[c] = P[c] * gnw[0] + P[4 + c] * gnw[1] + P[8 + c] * gnw[2]; /* R^T */
+  }
+  double dg[3];
+  if (gn > ORC_NRM_EPS) { /* d(-g/|g|)/dg = -(I - n n^T)/|g| */
+    double nl[3] = {-g[0] / gn, -g[1] / gn, -g[2] / gn};
+    double dot = nl[0] * gl[0] + nl[1] * gl[1] + nl[2] * gl[2];
+    for (int a = 0; a < 3; ++a) dg[a] = -(gl[a] - nl[a] * dot) / gn;
+  } else {
+    for (int a = 0; a < 3; ++a) dg[a] = -gl[a] / ORC_NRM_EPS;
+  }
+  for (int a = 0; a < 3; ++a) {
+    int bit = 4 >> a;
+    for (int c = 0; c < 8; ++c) {
+      double val = 0.25 * ((c & bit) ? dg[a] : -dg[a]);
+#pragma omp atomic
+      dgeo_v[c] += val;
+    }
+  }
+}
+
 typedef struct {
   segvec segs;
   ival *bg, *actv;
@@ -369,7 +421,8 @@ static void ws_free(ray_ws *w) { free(w->segs.s); free(w->bg); free(w->actv); fr
 /* One ray: O1-O8 (+O9 when g_* given).  cand[t]/ncand[t] = candidate voxel ids of tree t (NULL = all voxels).
  * out5 = {R,G,B,depth,alpha}; *n_used = number of sub-segments composited. */
 static void render_ray(const scene_t *sc, int u, int v, const uint32_t *const *cand, const uint32_t *ncand,
-                       ray_ws *w, double out5[5], const double *g5 /* or NULL */, orc_grad *grads, uint32_t *n_used) {
+                       ray_ws *w, double out5[5], const double *g5 /* or NULL */, orc_grad *grads, uint32_t *n_used,
+                       double *nout /* [3] or NULL */, const double *gN /* [3] or NULL */) {
   double o[3], d[3];
   orc_ray(sc->cam, u, v, o, d);
   int nbg = schedule(sc, o, d, w->bg, w->actv, w->hits);
@@ -392,7 +445,7 @@ static void render_ray(const scene_t *sc, int u, int v, const uint32_t *const *c
     w->tau = (double *)realloc(w->tau, sizeof(double) * w->tape_cap);
     w->Tb = (double *)realloc(w->Tb, sizeof(double) * w->tape_cap);
   }
-  double C[3] = {0, 0, 0}, D = 0, T = 1;
+  double C[3] = {0, 0, 0}, D = 0, T = 1, Nacc[3] = {0, 0, 0};
   size_t used = 0;
   for (size_t n = 0; n < w->segs.n; ++n) { /* O8 */
     const seg_t *sg = &w->segs.s[n];
@@ -407,6 +460,11 @@ static void render_ray(const scene_t *sc, int u, int v, const uint32_t *const *c
     w->tau[n] = tau; w->Tb[n] = T;
     for (int ch = 0; ch < 3; ++ch) C[ch] += wgt * rgb[ch];
     D += wgt * 0.5 * (sg->a + sg->b);
+    if (nout) { /* O11 */
+      double nw[3], gg[3], gn;
+      voxel_normal(sc, sg->tree, sg->v, nw, gg, &gn);
+      for (int a = 0; a < 3; ++a) Nacc[a] += wgt * nw[a];
+    }
     T *= exp(-tau);
     used = n + 1;
     if (T < sc->opt->t_stop) break;
@@ -421,6 +479,7 @@ static void render_ray(const scene_t *sc, int u, int v, const uint32_t *const *c
     }
   }
   out5[0] = C[0]; out5[1] = C[1]; out5[2] = C[2]; out5[3] = D; out5[4] = 1.0 - T;
+  if (nout) memcpy(nout, Nacc, sizeof Nacc);
   if (n_used) *n_used = (uint32_t)used;
   if (!g5 || !grads) return;
   /* O9: reverse sweep over the tape.  Adjoint of T after the last voxel comes from alpha = 1 - T and from Eq. 2. */
@@ -448,6 +507,15 @@ static void render_ray(const scene_t *sc, int u, int v, const uint32_t *const *c
     voxel_colour(tr, sg->v, ol, rgb, pre, Y);
     double mid = 0.5 * (sg->a + sg->b);
     double g_w = g5[0] * rgb[0] + g5[1] * rgb[1] + g5[2] * rgb[2] + g5[3] * mid;
+    if (gN) {
+      double nw[3], gg[3], gn;
+      voxel_normal(sc, sg->tree, sg->v, nw, gg, &gn);
+      g_w += gN[0] * nw[0] + gN[1] * nw[1] + gN[2] * nw[2];
+      if (grads[sg->tree].dgeo) {
+        double gnw[3] = {wgt * gN[0], wgt * gN[1], wgt * gN[2]};
+        voxel_normal_backward(sc, sg->tree, sg->v, gnw, grads[sg->tree].dgeo + (size_t)sg->v * 8);
+      }
+    }
     double g_alpha = g_w * Tb;
     double g_Tb = g_w * alpha + gT * e;
     double g_tau = g_alpha * e - gT * Tb * e;
@@ -596,10 +664,11 @@ static void build_tilelists(const scene_t *sc, tilelists *tl) {
  * doubles (untouched where masked out).  When g_rgb != NULL also runs O9 and accumulates into grads[n_trees]
  * (g_depth / g_alpha may be NULL = zero).  n_used (optional, [H][W]) = sub-segments composited per ray.
  * Returns 0, or -1 on invalid arguments. */
-int orc_render_sky(const orc_camera *cam, int n_trees, const orc_octree *trees, const double *poses, const double *half,
-                   const orc_opts *opt, const uint8_t *mask, double *rgb, double *depth, double *alpha,
-                   const double *g_rgb, const double *g_depth, const double *g_alpha, orc_grad *grads,
-                   uint32_t *n_used, const orc_sky *sky) {
+int orc_render_full(const orc_camera *cam, int n_trees, const orc_octree *trees, const double *poses, const double *half,
+                    const orc_opts *opt, const uint8_t *mask, double *rgb, double *depth, double *alpha,
+                    const double *g_rgb, const double *g_depth, const double *g_alpha, orc_grad *grads,
+                    uint32_t *n_used, const orc_sky *sky, double *normal /* [H][W][3] or NULL */,
+                    const double *g_normal /* [H][W][3] or NULL */) {
   if (!cam || !trees || !opt || n_trees < 1 || opt->k_samples < 1 || opt->k_samples > 64) return -1;
   if (sky && (!sky->tex || sky->width < 1 || sky->height < 1)) return -1;
   scene_t sc = {n_trees, trees, poses, half, cam, opt, sky};
@@ -632,7 +701,8 @@ int orc_render_sky(const orc_camera *cam, int n_trees, const orc_octree *trees, 
             g5[3] = g_depth ? g_depth[p] : 0; g5[4] = g_alpha ? g_alpha[p] : 0;
           }
           uint32_t used;
-          render_ray(&sc, u, v, opt->mode == 1 ? cand : NULL, ncand, &w, out5, g_rgb ? g5 : NULL, grads, &used);
+          render_ray(&sc, u, v, opt->mode == 1 ? cand : NULL, ncand, &w, out5, g_rgb ? g5 : NULL, grads, &used,
+                     normal ? normal + 3 * p : NULL, (g_rgb && g_normal) ? g_normal + 3 * p : NULL);
           rgb[3 * p] = out5[0]; rgb[3 * p + 1] = out5[1]; rgb[3 * p + 2] = out5[2];
           depth[p] = out5[3]; alpha[p] = out5[4];
           if (n_used) n_used[p] = used;
@@ -642,6 +712,14 @@ int orc_render_sky(const orc_camera *cam, int n_trees, const orc_octree *trees, 
   }
   free(tl.start); free(tl.ids);
   return 0;
+}
+
+int orc_render_sky(const orc_camera *cam, int n_trees, const orc_octree *trees, const double *poses, const double *half,
+                   const orc_opts *opt, const uint8_t *mask, double *rgb, double *depth, double *alpha,
+                   const double *g_rgb, const double *g_depth, const double *g_alpha, orc_grad *grads,
+                   uint32_t *n_used, const orc_sky *sky) {
+  return orc_render_full(cam, n_trees, trees, poses, half, opt, mask, rgb, depth, alpha, g_rgb, g_depth, g_alpha, grads,
+                         n_used, sky, NULL, NULL);
 }
 
 int orc_render(const orc_camera *cam, int n_trees, const orc_octree *trees, const double *poses, const double *half,
@@ -724,7 +802,7 @@ int64_t orc_ray_segments(const orc_camera *cam, int n_trees, const orc_octree *t
   orc_opts o2 = *opt;
   o2.t_stop = 0; /* list everything */
   sc.opt = &o2;
-  render_ray(&sc, u, v, NULL, NULL, &w, out5, NULL, NULL, &used);
+  render_ray(&sc, u, v, NULL, NULL, &w, out5, NULL, NULL, &used, NULL, NULL);
   int64_t n = (int64_t)w.segs.n;
   for (int64_t i = 0; i < n && i < cap; ++i) {
     tree_out[i] = w.segs.s[i].tree; vox_out[i] = w.segs.s[i].v; a_out[i] = w.segs.s[i].a; b_out[i] = w.segs.s[i].b;

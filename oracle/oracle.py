@@ -100,11 +100,12 @@ class _Packed:
         self.hw = (cam.height, cam.width)
 
 
-def render(scene, cam_index=0, mode=0, mask=None, grads_in=None, want_grads=None, sky=None, **opt):
+def render(scene, cam_index=0, mode=0, mask=None, grads_in=None, want_grads=None, sky=None, normals=False, **opt):
     """Forward (and backward when ``grads_in`` is given) in double precision.
 
     grads_in: dict with 'rgb' [H,W,3] and optional 'depth', 'alpha' [H,W].
     sky: optional equirectangular map [Hs,Ws,3] (O10 / Eq. 2, reading R21); with grads_in also returns 'dsky'.
+    normals: also return the normal map 'normal' [H,W,3] (O11, reading R22); grads_in may then hold 'normal' [H,W,3].
     Returns dict(rgb, depth, alpha, n_used [, dgeo list, dsh list, dsky]).
     """
     p = _Packed(scene, cam_index, mode, **opt)
@@ -133,9 +134,15 @@ def render(scene, cam_index=0, mode=0, mask=None, grads_in=None, want_grads=None
         csky = C.byref(_Sky(tex.shape[1], tex.shape[0], _ptr(tex), _ptr(dtex)))
         if dtex is not None:
             out["dsky"] = dtex
-    rc = lib().orc_render_sky(C.byref(p.cam), p.n_trees, p.trees, _ptr(p.poses), _ptr(p.half), C.byref(p.opts), _ptr(m),
-                              _ptr(rgb), _ptr(depth), _ptr(alpha), _ptr(g_rgb), _ptr(g_depth), _ptr(g_alpha), cgrads,
-                              _ptr(n_used), csky)
+    normal = np.zeros((H, W, 3)) if (normals or (grads_in is not None and grads_in.get("normal") is not None)) else None
+    g_normal = None
+    if grads_in is not None and grads_in.get("normal") is not None:
+        g_normal = np.ascontiguousarray(grads_in["normal"], dtype=np.float64)
+    rc = lib().orc_render_full(C.byref(p.cam), p.n_trees, p.trees, _ptr(p.poses), _ptr(p.half), C.byref(p.opts), _ptr(m),
+                               _ptr(rgb), _ptr(depth), _ptr(alpha), _ptr(g_rgb), _ptr(g_depth), _ptr(g_alpha), cgrads,
+                               _ptr(n_used), csky, _ptr(normal), _ptr(g_normal))
+    if normal is not None:
+        out["normal"] = normal
     if rc != 0:
         raise ValueError("orc_render: invalid arguments")
     out.update(rgb=rgb, depth=depth, alpha=alpha, n_used=n_used)

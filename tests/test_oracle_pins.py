@@ -505,3 +505,92 @@ def test_p14_finite_difference_gradients_with_sky():
             flat[idx] = keep - h; lm = loss()
             flat[idx] = keep
             assert abs((lp - lm) / (2 * h) - aflat[idx]) / scale < 1e-6
+
+
+# ---------------------------------------------------------------- P15 normal map (state tuple S; reading R22)
+def _ramp_geo(axis, lo=0.0, hi=1.0):
+    """8 corner values, corner c = 4 bx + 2 by + bz, raw density = lo on the face b_axis = 0 and hi on b_axis = 1."""
+    return np.array([hi if (c >> (2 - axis)) & 1 else lo for c in range(8)], dtype=np.float64)
+
+
+@pytest.mark.parametrize("axis", [0, 1, 2])
+def test_p15_linear_density_gives_axis_normal(axis):
+    """A voxel whose raw density rises linearly along one axis has the normal -e_axis; N = alpha n (one voxel)."""
+    cam = axis_camera(width=3, height=3)
+    st = tree_from_cells([(1, 1, 1, 1)], geo=_ramp_geo(axis, -1.0, 0.5).reshape(1, 8))
+    r = O.render(scene(st, cam=cam), normals=True)
+    n = np.zeros(3); n[axis] = -1.0
+    assert r["alpha"][1, 1] > 0.3
+    assert np.abs(r["normal"] - r["alpha"][..., None] * n).max() < 1e-14
+    # falling density flips it; a constant voxel has no normal at all
+    st2 = tree_from_cells([(1, 1, 1, 1)], geo=_ramp_geo(axis, 0.5, -1.0).reshape(1, 8))
+    r2 = O.render(scene(st2, cam=cam), normals=True)
+    assert np.abs(r2["normal"] + r2["alpha"][..., None] * n).max() < 1e-14
+    r3 = O.render(scene(tree_from_cells([(1, 1, 1, 1)], geo=0.2), cam=cam), normals=True)
+    assert np.abs(r3["normal"]).max() == 0.0
+
+
+def test_p15_actor_normal_is_rotated_into_the_world_frame():
+    cam = axis_camera(width=3, height=3)
+    act = tree_from_cells([(1, 1, 1, 1)], geo=_ramp_geo(0, -1.0, 0.5).reshape(1, 8), side=1.0)
+    for yaw in (0.0, 0.7, math.pi / 2, -2.0):
+        pose = S.pose_yaw((0.0, 1.0, 1.0), yaw)
+        r = O.render(scene(empty_tree(), [act], [pose], [[0.6, 0.6, 0.6]], cam=cam), normals=True)
+        n = np.array([-math.cos(yaw), -math.sin(yaw), 0.0])
+        assert r["alpha"].max() > 0.1
+        assert np.abs(r["normal"] - r["alpha"][..., None] * n).max() < 1e-14
+
+
+def test_p15_rigid_motion_rotates_the_normal_map_and_bound():
+    """One rigid motion G applied to the camera and to every pose (P4 (d)): N' = G_R N; and |N| <= alpha everywhere."""
+    s0 = S.tiny_random_scene(5, sh_degree=1)
+    cam = s0.cameras[0]
+    from helpers import _raw
+    st = s0.static
+    st0 = _raw(st.code, st.geo, st.sh, (0, 0, 0), st.side, st.sh_degree)
+    th, ax = 0.9, np.array([0.3, -0.5, 0.8]) / np.linalg.norm([0.3, -0.5, 0.8])
+    Kx = np.array([[0, -ax[2], ax[1]], [ax[2], 0, -ax[0]], [-ax[1], ax[0], 0]])
+    G = np.eye(3) + math.sin(th) * Kx + (1 - math.cos(th)) * Kx @ Kx
+    g = np.array([0.7, -1.1, 2.0])
+    P1 = np.asarray(s0.poses[0], dtype=np.float64).reshape(3, 4)
+    P2 = S.pose_yaw((-1.0, -2.0, 0.5), -0.4)
+    acts, halves = [s0.actors[0], st0], [s0.box_half[0], [1.0, 1.0, 1.0]]
+    c2w = np.asarray(cam.c2w, dtype=np.float64).reshape(3, 4)
+    moved = lambda P: np.concatenate([G @ P[:, :3], (G @ P[:, 3] + g)[:, None]], 1)
+    cam.c2w = c2w.reshape(12)
+    A = scene(empty_tree(1), acts, [P1, P2], halves, cam=cam, t_stop=0.0)
+    cam2 = S.Camera(cam.width, cam.height, cam.fx, cam.fy, cam.cx, cam.cy, cam.c2w, cam.near, cam.far)
+    cam2.c2w = moved(c2w).reshape(12)
+    B = scene(empty_tree(1), acts, [moved(P1), moved(P2)], halves, cam=cam2, t_stop=0.0)
+    ra, rb = O.render(A, normals=True), O.render(B, normals=True)
+    assert np.abs(ra["normal"]).max() > 0.05
+    assert np.abs(ra["normal"] @ G.T - rb["normal"]).max() < 1e-10
+    assert (np.linalg.norm(ra["normal"], axis=-1) <= ra["alpha"] * (1 + 1e-6) + 1e-12).all()  # poses are fp32-rounded rotations
+
+
+def test_p15_finite_difference_gradients_with_normals():
+    s = S.tiny_random_scene(13, sh_degree=1, colour_floor=True)
+    for t in s.octrees:
+        t.geo = t.geo.astype(np.float64)
+        t.sh = t.sh.astype(np.float64)
+    g = s.image_grads(0, 1.0, 0.3, 1.0)
+    rs = np.random.RandomState(2)
+    g["normal"] = rs.normal(size=g["rgb"].shape)
+    r = O.render(s, grads_in=g)
+
+    def loss():
+        q = O.render(s, normals=True)
+        return ((q["rgb"] * g["rgb"]).sum() + (q["depth"] * g["depth"]).sum() + (q["alpha"] * g["alpha"]).sum()
+                + (q["normal"] * g["normal"]).sum())
+
+    h = 1e-6
+    for n, t in enumerate(s.octrees):
+        flat, aflat = t.geo.reshape(-1), r["dgeo"][n].reshape(-1)
+        scale = max(np.abs(aflat).max(), 1e-12)
+        assert np.count_nonzero(aflat) > 20
+        for idx in range(flat.shape[0]):
+            keep = flat[idx]
+            flat[idx] = keep + h; lp = loss()
+            flat[idx] = keep - h; lm = loss()
+            flat[idx] = keep
+            assert abs((lp - lm) / (2 * h) - aflat[idx]) / scale < 2e-6, (n, idx)
