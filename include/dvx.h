@@ -109,6 +109,9 @@ typedef struct {
   float *rgb;   /* DEVICE [H][W][3] */
   float *depth; /* DEVICE [H][W]  D = sum T_j alpha_j (a_j+b_j)/2, Euclidean ray distance (R9) */
   float *alpha; /* DEVICE [H][W]  1 - T_final */
+  float *normal; /* DEVICE [H][W][3] or NULL (not computed).  N = sum T_j alpha_j n_j, the N of the state tuple S
+                    (PAPER.md:107, :297); n_j = the voxel's normal in the WORLD frame, reading R22: minus the gradient of
+                    its trilinear raw density at the voxel centre, divided by max(|g|, 1e-6) */
 } dvx_image;
 
 /* Steps 1-4 of the hot path.  poses_l2w: HOST [N][12] row-major [R_i | t_i] local->world;
@@ -129,6 +132,12 @@ typedef struct {
  * No gradient flows to geometry (camera, poses, voxel positions) nor through the per-voxel view direction. */
 dvx_status dvx_backward(dvx_ctx *ctx, dvx_frame *saved, const float *dL_drgb, const float *dL_ddepth,
                         const float *dL_dalpha, dvx_grad static_grad, const dvx_grad *actor_grads);
+/* dvx_backward with a gradient of the normal map as well (the frame must have been rendered with out.normal != NULL):
+ * dL_dnormal DEVICE [H][W][3] or NULL.  The corner densities receive it through the compositing weights and through
+ * the voxel normals themselves (R22). */
+dvx_status dvx_backward_n(dvx_ctx *ctx, dvx_frame *saved, const float *dL_drgb, const float *dL_ddepth,
+                          const float *dL_dalpha, const float *dL_dnormal, dvx_grad static_grad,
+                          const dvx_grad *actor_grads);
 void dvx_frame_release(dvx_ctx *ctx, dvx_frame *frame);
 
 /* The same two calls with HOST image buffers (pinned memory recommended), for end-to-end use from a host

@@ -20,7 +20,7 @@ FLAG_COUNTERS = 1
 FLAG_NAIVE = 2
 
 EXPORTS = ["dvx_create", "dvx_destroy", "dvx_octree_create", "dvx_octree_refresh_structure", "dvx_octree_destroy",
-           "dvx_render", "dvx_backward", "dvx_frame_release", "dvx_debug_tile_list", "dvx_frame_counters",
+           "dvx_render", "dvx_backward", "dvx_backward_n", "dvx_frame_release", "dvx_debug_tile_list", "dvx_frame_counters",
            "dvx_frame_stage_ms", "dvx_last_error", "dvx_sort_pairs", "dvx_launch_count", "dvx_stage_ms_collect", "dvx_render_host",
            "dvx_backward_host"]
 
@@ -51,7 +51,7 @@ class RenderOpts(C.Structure):
 
 
 class Image(C.Structure):
-    _fields_ = [("rgb", C.c_void_p), ("depth", C.c_void_p), ("alpha", C.c_void_p)]
+    _fields_ = [("rgb", C.c_void_p), ("depth", C.c_void_p), ("alpha", C.c_void_p), ("normal", C.c_void_p)]
 
 
 class Grad(C.Structure):
@@ -83,6 +83,7 @@ def load():
     lib.dvx_render.argtypes = [P, C.POINTER(Camera), P, C.c_uint32, C.POINTER(P), P, P, C.POINTER(RenderOpts), Image,
                                C.POINTER(P)]
     lib.dvx_backward.argtypes = [P, P, P, P, P, Grad, C.POINTER(Grad)]
+    lib.dvx_backward_n.argtypes = [P, P, P, P, P, P, Grad, C.POINTER(Grad)]
     lib.dvx_frame_release.argtypes = [P, P]
     lib.dvx_frame_release.restype = None
     lib.dvx_debug_tile_list.argtypes = [P, P, C.c_uint32, C.c_uint32, C.c_uint32, P, C.c_uint32, C.POINTER(C.c_uint32)]
@@ -168,11 +169,12 @@ class Context:
 
     # ------------------------------------------------------------------ render / backward
     def render(self, cam, static, actors=(), poses=None, box_half=None, k_samples=8, activation=0, t_stop=1e-4, flags=0,
-               save=True, out=None, host=False, sky=None, dsky=None):
+               save=True, out=None, host=False, sky=None, dsky=None, normals=False):
         """dvx_render (host=False: device image tensors) or dvx_render_host (host=True: ``out`` must be three pinned
         CPU tensors).  cam: binding.Camera; poses [N,12] / box_half [N,3] host float32 arrays.
         sky: optional CUDA float32 tensor [Hs,Ws,3] (Eq. 2); dsky: tensor of the same shape that dvx_backward accumulates
-        the texture gradient into.  Returns (rgb [H,W,3], depth [H,W], alpha [H,W], Frame or None)."""
+        the texture gradient into.  normals=True also renders the normal map (O11) and returns
+        (rgb, depth, alpha, normal [H,W,3], Frame or None) instead of (rgb [H,W,3], depth [H,W], alpha [H,W], Frame or None)."""
         torch = self.torch
         H, W = cam.height, cam.width
         if host and out is None:
@@ -194,7 +196,11 @@ class Context:
             assert sky.is_cuda and sky.dtype == torch.float32 and sky.dim() == 3 and sky.shape[2] == 3 and sky.is_contiguous()
             csky = Sky(sky.shape[1], sky.shape[0], sky.data_ptr(), dsky.data_ptr() if dsky is not None else None)
             opts.sky = C.pointer(csky)
-        img = Image(rgb.data_ptr(), depth.data_ptr(), alpha.data_ptr())
+        normal = None
+        if normals:
+            normal = torch.empty((H, W, 3), dtype=torch.float32).pin_memory() if host else \
+                torch.empty((H, W, 3), dtype=torch.float32, device=self.device)
+        img = Image(rgb.data_ptr(), depth.data_ptr(), alpha.data_ptr(), normal.data_ptr() if normals else None)
         fh = C.c_void_p()
         fn = self.lib.dvx_render_host if host else self.lib.dvx_render
         rc = fn(self.h, C.byref(cam), static.h, n, handles, poses.ctypes.data_as(C.c_void_p),
@@ -203,6 +209,8 @@ class Context:
         frame = Frame(self, fh, [static] + list(actors)) if save else None
         if frame is not None:
             frame.keep = (sky, dsky)   # the library borrows these until the frame is released
+        if normals:
+            return rgb, depth, alpha, normal, frame
         return rgb, depth, alpha, frame
 
 
@@ -237,7 +245,7 @@ class Frame:
     def __init__(self, ctx, h, trees):
         self.ctx, self.h, self.trees = ctx, h, trees
 
-    def backward(self, dL_drgb, dL_ddepth=None, dL_dalpha=None, grads=None, host=False):
+    def backward(self, dL_drgb, dL_ddepth=None, dL_dalpha=None, grads=None, host=False, dL_dnormal=None):
         """dvx_backward (device image gradients) or dvx_backward_host (host=True: pinned CPU tensors).
         grads: list of (dgeo, dsh) tensors per octree (accumulated into); None = fresh zeros.
         Returns the list of (dgeo, dsh)."""
@@ -249,6 +257,10 @@ class Frame:
         n = len(self.trees) - 1
         arr = (Grad * max(n, 1))(*g[1:])
         ptr = lambda t: None if t is None else t.data_ptr()
+        if dL_dnormal is not None:
+            assert not host
+            ctx.check(ctx.lib.dvx_backward_n(ctx.h, self.h, ptr(dL_drgb), ptr(dL_ddepth), ptr(dL_dalpha), ptr(dL_dnormal), g[0], arr))
+            return grads
         fn = ctx.lib.dvx_backward_host if host else ctx.lib.dvx_backward
         ctx.check(fn(ctx.h, self.h, ptr(dL_drgb), ptr(dL_ddepth), ptr(dL_dalpha), g[0], arr))
         return grads
@@ -302,12 +314,12 @@ class SceneOnDevice:
         self.box_half = np.ascontiguousarray(scene.box_half, dtype=np.float32)
         self.cams = [camera_from(c) for c in scene.cameras]
 
-    def render(self, cam_index=0, save=True, flags=0, out=None, host=False, sky=None, dsky=None, **opt):
+    def render(self, cam_index=0, save=True, flags=0, out=None, host=False, sky=None, dsky=None, normals=False, **opt):
         s = self.scene
         kw = dict(k_samples=s.k_samples, activation=s.activation, t_stop=s.t_stop)
         kw.update(opt)
         return self.ctx.render(self.cams[cam_index], self.trees[0], self.trees[1:], self.poses, self.box_half, flags=flags,
-                               save=save, out=out, host=host, sky=sky, dsky=dsky, **kw)
+                               save=save, out=out, host=host, sky=sky, dsky=dsky, normals=normals, **kw)
 
     def zero_grads(self):
         torch = self.ctx.torch

@@ -45,7 +45,7 @@ struct dvx_frame {
   uint64_t n_pairs = 0, v_vis = 0;
   EventSet *es = nullptr;
   cudaEvent_t *ev = nullptr;  // = es->ev
-  Buf eff_end;
+  Buf eff_end, vnrm, sv_nrm;
   dvx_sky sky = {0, 0, nullptr, nullptr};
   bool did_backward = false;
 };
@@ -115,6 +115,8 @@ void frame_free(dvx_ctx *ctx, dvx_frame *f) {
                           &f->range_beg, &f->range_end, &f->counters, &f->sv_rgbd, &f->sv_T, &f->sv_nused};
   for (auto *b : bs) ctx_release(ctx, b->p);
   ctx_release(ctx, f->eff_end.p);
+  ctx_release(ctx, f->vnrm.p);
+  ctx_release(ctx, f->sv_nrm.p);
   if (f->es) {
     f->es->did_backward = f->did_backward;
     if (f->es->rendered) {
@@ -283,6 +285,7 @@ void setup_tree(TreeFrame &T, const dvx_octree *t, uint32_t base, bool actor, co
       T.N[3 * a + c] = (float)n;
     }
     T.half[a] = actor ? half[a] : INFINITY;
+    for (int c = 0; c < 3; ++c) T.R[3 * a + c] = (float)R[3 * a + c];
   }
 }
 
@@ -376,6 +379,10 @@ dvx_status dvx_render(dvx_ctx *ctx, const dvx_camera *cam, const dvx_octree *sta
             buf_alloc(ctx, f->counters, sizeof(unsigned long long) * CNT_N);
   if (ok && saved)
     ok = buf_alloc(ctx, f->sv_rgbd, npix * 16) && buf_alloc(ctx, f->sv_T, npix * 4) && buf_alloc(ctx, f->sv_nused, npix * 4);
+  if (ok && out.normal) {
+    if (o.flags & DVX_FLAG_NAIVE) { frame_free(ctx, f); return fail(ctx, DVX_ERR_NOT_IMPLEMENTED, "the debug walker has no normal map"); }
+    ok = buf_alloc(ctx, f->vnrm, sizeof(float4) * (size_t)p.v_total) && (!saved || buf_alloc(ctx, f->sv_nrm, npix * 16));
+  }
   if (!ok) { frame_free(ctx, f); return fail(ctx, DVX_ERR_OOM, "dvx_render: allocator returned NULL"); }
   if (!ctx->ev_free.empty()) {
     f->es = ctx->ev_free.back();
@@ -401,7 +408,7 @@ dvx_status dvx_render(dvx_ctx *ctx, const dvx_camera *cam, const dvx_octree *sta
   CU(cudaEventRecord(f->ev[0], st));
   dvx_tree_setup_launch(p, trees_d, st);
   dvx_tile_masks_launch(p, trees_d, (uint8_t *)f->octmask.p, (unsigned long long *)f->actor_mask.p, st);
-  dvx_preprocess_launch(p, trees_d, (const uint8_t *)f->octmask.p, (FrameVox *)f->fvox.p, (ushort4 *)f->pxrect.p, counters, st);
+  dvx_preprocess_launch(p, trees_d, (const uint8_t *)f->octmask.p, (FrameVox *)f->fvox.p, (ushort4 *)f->pxrect.p, (float4 *)f->vnrm.p, counters, st);
   CU(cudaEventRecord(f->ev[1], st));
   CU(cudaMemcpyAsync(ctx->h_counters, counters, sizeof(unsigned long long) * CNT_N, cudaMemcpyDeviceToHost, st));
   CU(cudaStreamSynchronize(st));
@@ -438,6 +445,7 @@ dvx_status dvx_render(dvx_ctx *ctx, const dvx_camera *cam, const dvx_octree *sta
   A.sv_rgbd = (float *)f->sv_rgbd.p; A.sv_T = (float *)f->sv_T.p; A.sv_nused = (uint32_t *)f->sv_nused.p;
   A.counters = counters;
   A.sky_tex = f->sky.tex; A.sky_w = f->sky.width; A.sky_h = f->sky.height;
+  A.normal = out.normal; A.vnrm = (const float4 *)f->vnrm.p; A.sv_nrm = (float *)f->sv_nrm.p;
   if (p.flags & DVX_FLAG_COUNTERS) {
     if (!buf_alloc(ctx, f->eff_end, sizeof(uint32_t) * (size_t)p.n_buckets)) { frame_free(ctx, f); return fail(ctx, DVX_ERR_OOM, "dvx_render: allocator returned NULL"); }
     CU(cudaMemsetAsync(f->eff_end.p, 0, sizeof(uint32_t) * (size_t)p.n_buckets, st));
@@ -454,9 +462,15 @@ dvx_status dvx_render(dvx_ctx *ctx, const dvx_camera *cam, const dvx_octree *sta
 
 dvx_status dvx_backward(dvx_ctx *ctx, dvx_frame *f, const float *dL_drgb, const float *dL_ddepth, const float *dL_dalpha,
                         dvx_grad static_grad, const dvx_grad *actor_grads) {
+  return dvx_backward_n(ctx, f, dL_drgb, dL_ddepth, dL_dalpha, nullptr, static_grad, actor_grads);
+}
+
+dvx_status dvx_backward_n(dvx_ctx *ctx, dvx_frame *f, const float *dL_drgb, const float *dL_ddepth, const float *dL_dalpha,
+                          const float *dL_dnormal, dvx_grad static_grad, const dvx_grad *actor_grads) {
   if (!ctx) return DVX_ERR_INVALID_ARG;
   if (!f || !dL_drgb) return fail(ctx, DVX_ERR_INVALID_ARG, "NULL argument");
   if (!f->sv_rgbd.p) return fail(ctx, DVX_ERR_INVALID_ARG, "frame holds no saved state");
+  if (dL_dnormal && !f->sv_nrm.p) return fail(ctx, DVX_ERR_INVALID_ARG, "the frame was rendered without a normal map");
   const FrameParams &p = f->p;
   if (p.n_trees > 1 && !actor_grads) return fail(ctx, DVX_ERR_INVALID_ARG, "actor_grads is NULL");
   cudaSetDevice(ctx->device);
@@ -467,7 +481,11 @@ dvx_status dvx_backward(dvx_ctx *ctx, dvx_frame *f, const float *dL_drgb, const 
     f->trees_h[t].dsh = g.dsh;
   }
   float *drgb = (float *)ctx_alloc(ctx, (size_t)p.v_total * 16);
-  if (!drgb) return fail(ctx, DVX_ERR_OOM, "dvx_backward: allocator returned NULL");
+  float *dnrm = dL_dnormal ? (float *)ctx_alloc(ctx, (size_t)p.v_total * 16) : nullptr;
+  if (!drgb || (dL_dnormal && !dnrm)) {
+    ctx_release(ctx, drgb); ctx_release(ctx, dnrm);
+    return fail(ctx, DVX_ERR_OOM, "dvx_backward: allocator returned NULL");
+  }
   TreeFrame *trees_d = (TreeFrame *)f->trees_d.p;
   // box_rect was filled on the device; only the gradient pointers change, so patch those fields
   for (uint32_t t = 0; t < p.n_trees; ++t)
@@ -475,6 +493,7 @@ dvx_status dvx_backward(dvx_ctx *ctx, dvx_frame *f, const float *dL_drgb, const 
                        cudaMemcpyHostToDevice, st));
   CU(cudaEventRecord(f->ev[5], st));
   CU(cudaMemsetAsync(drgb, 0, (size_t)p.v_total * 16, st));
+  if (dnrm) CU(cudaMemsetAsync(dnrm, 0, (size_t)p.v_total * 16, st));
   CompositeArgs A;
   memset(&A, 0, sizeof(A));
   A.p = p; A.trees = trees_d; A.fvox = (const FrameVox *)f->fvox.p; A.pxrect = (const ushort4 *)f->pxrect.p;
@@ -484,13 +503,16 @@ dvx_status dvx_backward(dvx_ctx *ctx, dvx_frame *f, const float *dL_drgb, const 
   A.counters = (unsigned long long *)f->counters.p;
   A.g_rgb = dL_drgb; A.g_depth = dL_ddepth; A.g_alpha = dL_dalpha; A.drgb = drgb;
   A.sky_tex = f->sky.tex; A.sky_w = f->sky.width; A.sky_h = f->sky.height; A.sky_dtex = f->sky.dtex;
+  A.g_normal = dL_dnormal; A.vnrm = (const float4 *)f->vnrm.p; A.sv_nrm = (float *)f->sv_nrm.p; A.dnrm = dnrm;
   CU(cudaEventRecord(f->ev[7], st));
   dvx_composite_launch(A, true, st);
   CU(cudaEventRecord(f->ev[8], st));
   dvx_sh_backward_launch(p, trees_d, A.fvox, A.pxrect, drgb, st);
+  if (dnrm) dvx_normal_backward_launch(p, trees_d, A.pxrect, dnrm, st);
   CU(cudaEventRecord(f->ev[6], st));
   CU(cudaGetLastError());
   ctx_release(ctx, drgb);
+  ctx_release(ctx, dnrm);
   f->did_backward = true;
   return DVX_OK;
 }
@@ -597,14 +619,15 @@ dvx_status dvx_render_host(dvx_ctx *ctx, const dvx_camera *cam, const dvx_octree
   if (!cam || !out_host.rgb || !out_host.depth || !out_host.alpha) return fail(ctx, DVX_ERR_INVALID_ARG, "NULL argument");
   cudaSetDevice(ctx->device);
   const size_t npix = (size_t)cam->width * cam->height;
-  float *stage = (float *)ctx_alloc(ctx, npix * 20);
+  float *stage = (float *)ctx_alloc(ctx, npix * 32);
   if (!stage) return fail(ctx, DVX_ERR_OOM, "dvx_render_host: allocator returned NULL");
-  dvx_image dev = {stage, stage + 3 * npix, stage + 4 * npix};
+  dvx_image dev = {stage, stage + 3 * npix, stage + 4 * npix, out_host.normal ? stage + 5 * npix : nullptr};
   dvx_status rc = dvx_render(ctx, cam, static_tree, n_actors, actors, poses_l2w, box_half, opts, dev, saved);
   if (rc == DVX_OK) {
     cudaError_t e = cudaMemcpyAsync(out_host.rgb, dev.rgb, npix * 12, cudaMemcpyDeviceToHost, ctx->st);
     if (e == cudaSuccess) e = cudaMemcpyAsync(out_host.depth, dev.depth, npix * 4, cudaMemcpyDeviceToHost, ctx->st);
     if (e == cudaSuccess) e = cudaMemcpyAsync(out_host.alpha, dev.alpha, npix * 4, cudaMemcpyDeviceToHost, ctx->st);
+    if (e == cudaSuccess && dev.normal) e = cudaMemcpyAsync(out_host.normal, dev.normal, npix * 12, cudaMemcpyDeviceToHost, ctx->st);
     if (e != cudaSuccess) rc = cuda_fail(ctx, e, "dvx_render_host: cudaMemcpyAsync");
   }
   ctx_release(ctx, stage);  // stream-ordered reuse: later users of the block are enqueued after the copies

@@ -62,13 +62,15 @@ struct __align__(16) Item {
   float tau;          // phase B: tau_v;  backward phase C overwrites it with dL/dtau_v
 };
 
-template <bool BWD>
+template <bool BWD, bool NRM>
 struct WarpQueue {
   EntryRec ent[32];
   Item item[QCAP];              // ring
   double d0[3];                 // the warp's reference direction for the list being served
   float4 rgbm[32];              // phase B -> C: per batch item, the voxel's RGB and clamp bits (fetched by the item's lane)
-  float wg[BWD ? 3 : 1][QCAP];  // backward phase C: T alpha g_C per item, zero where the colour clamp is active
+  float wg[BWD ? 3 : 1][32];    // backward phase C: T alpha g_C per batch item, zero where the colour clamp is active
+  float4 nrm[NRM ? 32 : 1];     // normal map (O11): per batch item the voxel's world normal
+  float wgn[(BWD && NRM) ? 3 : 1][32];  // backward phase C: T alpha g_N per batch item
 };
 
 struct Pix {
@@ -77,6 +79,8 @@ struct Pix {
   bool done;
   float gC0, gC1, gC2, gD, gA, Xtot, Xpre, T_final;  // backward only
   uint32_t n_stop;
+  float N0, N1, N2;     // normal map (O11), forward
+  float gN0, gN1, gN2;  // dL/dN, backward
 };
 
 __device__ __forceinline__ uint32_t warp_min_u32(uint32_t v) { return __reduce_min_sync(0xffffffffu, v); }
@@ -128,8 +132,8 @@ struct ItemGeom {
 
 // O6 for one queued item (ring slot `at`): K-point midpoint rule on the clipped segment.  Returns tau_v; with GRAD also
 // the moments M_j = sum_k act'(raw_k) lambda_k^j (j = 0..3), from which phase B2 rebuilds sum_k act'(raw_k) w_c(u_k).
-template <bool BWD>
-__device__ __forceinline__ float integrate_item(const CompositeArgs &A, const WarpQueue<BWD> &Q, int at, uint32_t &id,
+template <bool BWD, bool NRM>
+__device__ __forceinline__ float integrate_item(const CompositeArgs &A, const WarpQueue<BWD, NRM> &Q, int at, uint32_t &id,
                                                 uint32_t &meta, ItemGeom &G, float M[4]) {
   id = Q.item[at].id;
   meta = Q.item[at].meta;
@@ -241,8 +245,8 @@ __device__ __forceinline__ void red_add_v4(float *addr, float x, float y, float 
 
 // ---- phases B, C (and B2) over the first min(n_items, 32) queued items of the ring ------------------------------------
 // Ring slot of the i-th queued item: (head + i) & (QCAP-1).  my_bits: bit i set <=> queued item i belongs to this pixel.
-template <bool BWD>
-__device__ __forceinline__ void flush_batch(const CompositeArgs &A, int lane, WarpQueue<BWD> &Q, int &n_items, int &head,
+template <bool BWD, bool NRM>
+__device__ __forceinline__ void flush_batch(const CompositeArgs &A, int lane, WarpQueue<BWD, NRM> &Q, int &n_items, int &head,
                                             unsigned long long &my_bits, Pix &S) {
   const int count = n_items < 32 ? n_items : 32;
   __syncwarp();
@@ -252,8 +256,9 @@ __device__ __forceinline__ void flush_batch(const CompositeArgs &A, int lane, Wa
   uint32_t my_id = NONE, my_meta = 0;
   const int at_b = (head + lane) & (QCAP - 1);
   if (lane < count) {
-    Q.item[at_b].tau = integrate_item<BWD>(A, Q, at_b, my_id, my_meta, G, M);
+    Q.item[at_b].tau = integrate_item<BWD, NRM>(A, Q, at_b, my_id, my_meta, G, M);
     Q.rgbm[lane] = __ldg(reinterpret_cast<const float4 *>(A.fvox + my_id) + 1);  // keeps the global load out of C's serial loop
+    if (NRM) Q.nrm[lane] = __ldg(A.vnrm + my_id);
   }
   __syncwarp();
   // -- C: lane = pixel; its own items of the batch in queue order = front-to-back order along its ray
@@ -273,14 +278,23 @@ __device__ __forceinline__ void flush_batch(const CompositeArgs &A, int lane, Wa
       if (!BWD) {
         S.C0 = fmaf(w, f1.x, S.C0); S.C1 = fmaf(w, f1.y, S.C1); S.C2 = fmaf(w, f1.z, S.C2);
         S.D = fmaf(w, mid, S.D);
+        if (NRM) {
+          const float4 nv = Q.nrm[i];
+          S.N0 = fmaf(w, nv.x, S.N0); S.N1 = fmaf(w, nv.y, S.N1); S.N2 = fmaf(w, nv.z, S.N2);
+        }
       } else {
-        const float X = S.gC0 * f1.x + S.gC1 * f1.y + S.gC2 * f1.z + S.gD * mid;
+        float X = S.gC0 * f1.x + S.gC1 * f1.y + S.gC2 * f1.z + S.gD * mid;
+        if (NRM) {
+          const float4 nv = Q.nrm[i];
+          X += S.gN0 * nv.x + S.gN1 * nv.y + S.gN2 * nv.z;
+          Q.wgn[0][i] = w * S.gN0; Q.wgn[1][i] = w * S.gN1; Q.wgn[2][i] = w * S.gN2;
+        }
         S.Xpre = fmaf(w, X, S.Xpre);
         Q.item[at].tau = S.T * e * X - (S.Xtot - S.Xpre) + S.gA * S.T_final;  // dL/dtau_v
         const uint32_t cm = __float_as_uint(f1.w);
-        Q.wg[0][at] = (cm & 1u) ? 0.f : w * S.gC0;
-        Q.wg[1][at] = (cm & 2u) ? 0.f : w * S.gC1;
-        Q.wg[2][at] = (cm & 4u) ? 0.f : w * S.gC2;
+        Q.wg[0][i] = (cm & 1u) ? 0.f : w * S.gC0;
+        Q.wg[1][i] = (cm & 2u) ? 0.f : w * S.gC1;
+        Q.wg[2][i] = (cm & 4u) ? 0.f : w * S.gC2;
       }
       S.T *= e;
       S.n_used++;
@@ -291,23 +305,26 @@ __device__ __forceinline__ void flush_batch(const CompositeArgs &A, int lane, Wa
       }
     } else if (BWD) {  // queued before this pixel finished its replay: contributes nothing
       Q.item[at].tau = 0.f;
-      Q.wg[0][at] = 0.f; Q.wg[1][at] = 0.f; Q.wg[2][at] = 0.f;
+      Q.wg[0][i] = 0.f; Q.wg[1][i] = 0.f; Q.wg[2][i] = 0.f;
+      if (NRM) { Q.wgn[0][i] = 0.f; Q.wgn[1][i] = 0.f; Q.wgn[2][i] = 0.f; }
     }
   }
   my_bits >>= count;
   __syncwarp();
   // -- B2 (backward): lane = item again; corner gradients, run-reduced by voxel, vector reductions
   if (BWD) {
-    float val[11];
+    constexpr int NV = NRM ? 14 : 11;  // 8 corner gradients, 3 colour, (3 normal)
+    float val[NV];
 #pragma unroll
-    for (int c = 0; c < 11; ++c) val[c] = 0.f;
+    for (int c = 0; c < NV; ++c) val[c] = 0.f;
     if (lane < count) {
       const float dtau = Q.item[at_b].tau * G.delta;
       float cs[8];
       corner_sums(G, M, cs);
 #pragma unroll
       for (int c = 0; c < 8; ++c) val[c] = dtau * cs[c];
-      val[8] = Q.wg[0][at_b]; val[9] = Q.wg[1][at_b]; val[10] = Q.wg[2][at_b];
+      val[8] = Q.wg[0][lane]; val[9] = Q.wg[1][lane]; val[10] = Q.wg[2][lane];
+      if (NRM) { val[NV - 3] = Q.wgn[0][lane]; val[NV - 2] = Q.wgn[1][lane]; val[NV - 1] = Q.wgn[2][lane]; }
     }
     // runs of consecutive items of one voxel (the pixels one list entry hit): segmented suffix sums over the run index,
     // the first lane of each run ends up with the run total.  (The voxel id itself is not a valid segment key: a voxel cut
@@ -321,7 +338,7 @@ __device__ __forceinline__ void flush_batch(const CompositeArgs &A, int lane, Wa
       const uint32_t orun = __shfl_down_sync(0xffffffffu, run, o);
       const bool take = (lane + o < 32) && orun == run;
 #pragma unroll
-      for (int c = 0; c < 11; ++c) {
+      for (int c = 0; c < NV; ++c) {
         const float x = __shfl_down_sync(0xffffffffu, val[c], o);
         if (take) val[c] += x;
       }
@@ -334,6 +351,7 @@ __device__ __forceinline__ void flush_batch(const CompositeArgs &A, int lane, Wa
         red_add_v4(dg + 4, val[4], val[5], val[6], val[7]);
       }
       red_add_v4(A.drgb + (size_t)my_id * 4, val[8], val[9], val[10], 0.f);
+      if (NRM) red_add_v4(A.dnrm + (size_t)my_id * 4, val[NV - 3], val[NV - 2], val[NV - 1], 0.f);
     }
     __syncwarp();
   }
@@ -373,9 +391,9 @@ __device__ __noinline__ float2 axis_parallel_fix(const TreeFrame *T, uint32_t id
   return inside ? make_float2(sa, sb) : make_float2(INFINITY, -INFINITY);
 }
 
-template <bool BWD, bool CNT>
+template <bool BWD, bool CNT, bool NRM>
 __global__ void __launch_bounds__(TILE_THREADS, DVX_TILE_MIN_CTAS) composite_tile_kernel(const __grid_constant__ CompositeArgs A) {
-  __shared__ WarpQueue<BWD> s_queue[TILE_WARPS];
+  __shared__ WarpQueue<BWD, NRM> s_queue[TILE_WARPS];
   const FrameParams &p = A.p;
   const int tile = blockIdx.x;
   const int warp = threadIdx.x >> 5;
@@ -383,7 +401,7 @@ __global__ void __launch_bounds__(TILE_THREADS, DVX_TILE_MIN_CTAS) composite_til
   const uint32_t lt = (1u << lane) - 1u;
   const int wu0 = (tile % p.tiles_x) * DVX_TILE + (warp % WARPS_X) * WARP_W;   // pixel of lane 0 of this warp
   const int wv0 = (tile / p.tiles_x) * DVX_TILE + (warp / WARPS_X) * WARP_H;
-  WarpQueue<BWD> &Q = s_queue[warp];
+  WarpQueue<BWD, NRM> &Q = s_queue[warp];
   const int u = wu0 + lane % WARP_W, v = wv0 + lane / WARP_W;
   const bool inside = u < (int)p.width && v < (int)p.height;
   const size_t pix = (size_t)v * p.width + u;
@@ -391,12 +409,18 @@ __global__ void __launch_bounds__(TILE_THREADS, DVX_TILE_MIN_CTAS) composite_til
   Pix S;
   S.C0 = S.C1 = S.C2 = 0.f; S.D = 0.f; S.T = 1.f; S.n_used = 0; S.done = !inside;
   S.Xpre = 0.f; S.n_stop = 0;
+  S.N0 = S.N1 = S.N2 = 0.f; S.gN0 = S.gN1 = S.gN2 = 0.f;
   if (BWD && inside) {
     S.gC0 = A.g_rgb[3 * pix]; S.gC1 = A.g_rgb[3 * pix + 1]; S.gC2 = A.g_rgb[3 * pix + 2];
     S.gD = A.g_depth ? A.g_depth[pix] : 0.f;
     S.gA = A.g_alpha ? A.g_alpha[pix] : 0.f;
     const float4 cd = reinterpret_cast<const float4 *>(A.sv_rgbd)[pix];
     S.Xtot = S.gC0 * cd.x + S.gC1 * cd.y + S.gC2 * cd.z + S.gD * cd.w;
+    if (NRM) {
+      S.gN0 = A.g_normal[3 * pix]; S.gN1 = A.g_normal[3 * pix + 1]; S.gN2 = A.g_normal[3 * pix + 2];
+      const float4 nf = reinterpret_cast<const float4 *>(A.sv_nrm)[pix];
+      S.Xtot += S.gN0 * nf.x + S.gN1 * nf.y + S.gN2 * nf.z;
+    }
     S.T_final = A.sv_T[pix];
     S.n_stop = A.sv_nused[pix];
     // Eq. 2: dL/dT_final also has g_C . C_sky; with alpha = 1 - T_final that is an alpha gradient of -(g_C . C_sky)
@@ -581,7 +605,7 @@ __global__ void __launch_bounds__(TILE_THREADS, DVX_TILE_MIN_CTAS) composite_til
             }
             n_items += __popc(mk);
             if (n_items >= 32) {
-              flush_batch<BWD>(A, lane, Q, n_items, head, my_bits, S);
+              flush_batch<BWD, NRM>(A, lane, Q, n_items, head, my_bits, S);
               if (S.done) active = 0u;
             }
           }
@@ -597,7 +621,7 @@ __global__ void __launch_bounds__(TILE_THREADS, DVX_TILE_MIN_CTAS) composite_til
     }
     if (part) seg_tree = NONE;          // served
   }
-  while (n_items > 0) flush_batch<BWD>(A, lane, Q, n_items, head, my_bits, S);
+  while (n_items > 0) flush_batch<BWD, NRM>(A, lane, Q, n_items, head, my_bits, S);
 
   if (!BWD && inside) {
     float3 sky = make_float3(0.f, 0.f, 0.f);
@@ -605,6 +629,10 @@ __global__ void __launch_bounds__(TILE_THREADS, DVX_TILE_MIN_CTAS) composite_til
     A.rgb[3 * pix] = S.C0 + sky.x; A.rgb[3 * pix + 1] = S.C1 + sky.y; A.rgb[3 * pix + 2] = S.C2 + sky.z;
     A.depth[pix] = S.D;
     A.alpha[pix] = 1.0f - S.T;
+    if (NRM) {
+      A.normal[3 * pix] = S.N0; A.normal[3 * pix + 1] = S.N1; A.normal[3 * pix + 2] = S.N2;
+      if (A.sv_nrm) reinterpret_cast<float4 *>(A.sv_nrm)[pix] = make_float4(S.N0, S.N1, S.N2, 0.f);
+    }
     if (A.sv_rgbd) {
       reinterpret_cast<float4 *>(A.sv_rgbd)[pix] = make_float4(S.C0, S.C1, S.C2, S.D);
       A.sv_T[pix] = S.T;
@@ -630,10 +658,15 @@ void dvx_composite_tile_launch(const CompositeArgs &a, bool backward, cudaStream
   if (a.p.n_tiles == 0) return;
   DVX_COUNT_LAUNCH(1);
   const bool cnt = (a.p.flags & DVX_FLAG_COUNTERS) != 0;
-  if (backward)
-    composite_tile_kernel<true, false><<<a.p.n_tiles, TILE_THREADS, 0, st>>>(a);
-  else if (cnt)
-    composite_tile_kernel<false, true><<<a.p.n_tiles, TILE_THREADS, 0, st>>>(a);
-  else
-    composite_tile_kernel<false, false><<<a.p.n_tiles, TILE_THREADS, 0, st>>>(a);
+  const bool nrm = backward ? (a.g_normal != nullptr) : (a.normal != nullptr);  // normal map requested (O11)
+  if (backward) {
+    if (nrm) composite_tile_kernel<true, false, true><<<a.p.n_tiles, TILE_THREADS, 0, st>>>(a);
+    else composite_tile_kernel<true, false, false><<<a.p.n_tiles, TILE_THREADS, 0, st>>>(a);
+  } else if (nrm) {
+    composite_tile_kernel<false, false, true><<<a.p.n_tiles, TILE_THREADS, 0, st>>>(a);
+  } else if (cnt) {
+    composite_tile_kernel<false, true, false><<<a.p.n_tiles, TILE_THREADS, 0, st>>>(a);
+  } else {
+    composite_tile_kernel<false, false, false><<<a.p.n_tiles, TILE_THREADS, 0, st>>>(a);
+  }
 }

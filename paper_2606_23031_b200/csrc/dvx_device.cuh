@@ -100,3 +100,13 @@ __device__ __forceinline__ bool dvx_pixel_rect(const float (*pc)[3], const Frame
   y1 = ymax >= H - 1.f ? (int)p.height - 1 : (int)floorf(ymax);
   return x1 >= x0 && y1 >= y0;
 }
+
+
+// R22: a voxel's normal = minus the gradient of its trilinear raw density at the voxel centre, normalised with
+// max(|g|, 1e-6); g_a = 1/4 sum over the four corner pairs along axis a of (geo[b_a = 1] - geo[b_a = 0]).
+#define DVX_NRM_EPS 1e-6f
+__device__ __forceinline__ void dvx_centre_gradient(const float g[8], float grad[3]) {
+  grad[0] = 0.25f * ((g[4] - g[0]) + (g[5] - g[1]) + (g[6] - g[2]) + (g[7] - g[3]));
+  grad[1] = 0.25f * ((g[2] - g[0]) + (g[3] - g[1]) + (g[6] - g[4]) + (g[7] - g[5]));
+  grad[2] = 0.25f * ((g[1] - g[0]) + (g[3] - g[2]) + (g[5] - g[4]) + (g[7] - g[6]));
+}

@@ -24,6 +24,7 @@ struct TreeFrame {
   float ol_f[3];         // o_l rounded to fp32 (debug walker's ray-OBB test only)
   float inv_cell_f;      // 1 / cell rounded to fp32
   float N[9];            // R_o^T R_c: d_l[a] = N[3a] x' + N[3a+1] y' + N[3a+2];  p_cam[c] = sum_a N[3a+c] rel[a]
+  float R[9];            // local -> world rotation R_o (row-major; identity for the static tree): world normals (R22)
   float half[3];         // OBB half extents (actors)
   int box_rect[4];       // pixel rectangle of the OBB (x0,y0,x1,y1 inclusive; x1<x0 = not visible); set on device
 };
@@ -65,6 +66,11 @@ struct CompositeArgs {
   uint32_t *sv_nused;          // [H*W]
   unsigned long long *counters;
   uint32_t *eff_end;           // [n_buckets] furthest list position any warp streamed (DVX_FLAG_COUNTERS only, else NULL)
+  const float4 *vnrm;          // [v_total] per-voxel world normal (R22), or NULL when no normal map was requested
+  float *normal;               // caller's normal image [H][W][3] or NULL
+  float *sv_nrm;               // [H*W][4] saved N_final (frame-owned) or NULL
+  const float *g_normal;       // backward: dL/dN [H][W][3] or NULL
+  float *dnrm;                 // backward scratch [v_total][4]: dL/dn_v (world frame)
   const float *sky_tex;        // [sky_h][sky_w][3] or NULL (Eq. 2)
   float *sky_dtex;             // backward: texture gradient, or NULL
   uint32_t sky_w, sky_h;
@@ -93,7 +99,9 @@ void dvx_tree_setup_launch(const FrameParams &p, TreeFrame *trees, cudaStream_t 
 void dvx_tile_masks_launch(const FrameParams &p, const TreeFrame *trees, uint8_t *octmask, unsigned long long *actor_mask,
                            cudaStream_t st);
 void dvx_preprocess_launch(const FrameParams &p, const TreeFrame *trees, const uint8_t *octmask, FrameVox *fvox,
-                           ushort4 *pxrect, unsigned long long *counters, cudaStream_t st);
+                           ushort4 *pxrect, float4 *vnrm, unsigned long long *counters, cudaStream_t st);
+void dvx_normal_backward_launch(const FrameParams &p, const TreeFrame *trees, const ushort4 *pxrect, const float *dnrm,
+                                cudaStream_t st);
 void dvx_emit_pairs_launch(const FrameParams &p, const TreeFrame *trees, const uint8_t *octmask, const ushort4 *pxrect,
                            const FrameVox *fvox, uint64_t *keys, uint32_t *vals, unsigned long long capacity,
                            unsigned long long *counters, cudaStream_t st);

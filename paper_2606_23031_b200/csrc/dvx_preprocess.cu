@@ -172,7 +172,8 @@ __device__ __forceinline__ uint32_t count_pairs_warp(const FrameParams &p, const
 
 __global__ void __launch_bounds__(PRE_THREADS) preprocess_kernel(FrameParams p, const TreeFrame *trees,
                                                                  const uint8_t *octmask, FrameVox *fvox,
-                                                                 ushort4 *pxrect, unsigned long long *counters) {
+                                                                 ushort4 *pxrect, float4 *vnrm,
+                                                                 unsigned long long *counters) {
   __shared__ uint32_t s_base[DVX_MAX_TREES + 1];
   for (int i = threadIdx.x; i < (int)p.n_trees; i += blockDim.x) s_base[i] = trees[i].base;
   __syncthreads();
@@ -234,6 +235,17 @@ __global__ void __launch_bounds__(PRE_THREADS) preprocess_kernel(FrameParams p, 
       }
       fv.meta = meta | (npairs << 8);  // bits 8-31: this voxel's pair count (step 2 allocates its slots from it)
       fvox[g] = fv;
+      if (vnrm) {  // O11 / R22: world-frame voxel normal, only when a normal map was requested
+        const float4 *gp = reinterpret_cast<const float4 *>(T.geo + (size_t)v * 8);
+        const float4 g0 = __ldg(gp), g1 = __ldg(gp + 1);
+        const float gg[8] = {g0.x, g0.y, g0.z, g0.w, g1.x, g1.y, g1.z, g1.w};
+        float gr[3];
+        dvx_centre_gradient(gg, gr);
+        const float den = fmaxf(sqrtf(gr[0] * gr[0] + gr[1] * gr[1] + gr[2] * gr[2]), DVX_NRM_EPS);
+        const float nl[3] = {-gr[0] / den, -gr[1] / den, -gr[2] / den};
+        vnrm[g] = make_float4(T.R[0] * nl[0] + T.R[1] * nl[1] + T.R[2] * nl[2], T.R[3] * nl[0] + T.R[4] * nl[1] + T.R[5] * nl[2],
+                              T.R[6] * nl[0] + T.R[7] * nl[1] + T.R[8] * nl[2], 0.f);
+      }
     }
   }
   // warp-aggregated totals
@@ -404,6 +416,50 @@ __global__ void __launch_bounds__(PRE_THREADS) sh_backward_kernel(FrameParams p,
   }
 }
 
+// ------------------------------------------------------------------ step 5c: dL/dgeo through the voxel normal (R22)
+// dnrm[v] = sum over pixels of T alpha g_N (world frame).  n = -g / max(|g|, eps): dn/dg = -(I - n n^T)/|g| above eps,
+// -I/eps below; g is linear in the corners with weights +-1/4.  One thread per voxel, after the compositing replay.
+__global__ void __launch_bounds__(PRE_THREADS) normal_backward_kernel(FrameParams p, const TreeFrame *trees,
+                                                                      const ushort4 *pxrect, const float *dnrm) {
+  __shared__ uint32_t s_base[DVX_MAX_TREES + 1];
+  for (int i = threadIdx.x; i < (int)p.n_trees; i += blockDim.x) s_base[i] = trees[i].base;
+  __syncthreads();
+  const uint32_t g = blockIdx.x * blockDim.x + threadIdx.x;
+  if (g >= p.v_total) return;
+  const ushort4 r = pxrect[g];
+  if (r.x > r.z) return;
+  const float4 d = reinterpret_cast<const float4 *>(dnrm)[g];
+  if (d.x == 0.f && d.y == 0.f && d.z == 0.f) return;
+  const int t = find_tree(s_base, p.n_trees, g);
+  const TreeFrame &T = trees[t];
+  if (!T.dgeo) return;
+  const uint32_t v = g - s_base[t];
+  const float4 *gp = reinterpret_cast<const float4 *>(T.geo + (size_t)v * 8);
+  const float4 g0 = __ldg(gp), g1 = __ldg(gp + 1);
+  const float gg[8] = {g0.x, g0.y, g0.z, g0.w, g1.x, g1.y, g1.z, g1.w};
+  float gr[3];
+  dvx_centre_gradient(gg, gr);
+  const float gn = sqrtf(gr[0] * gr[0] + gr[1] * gr[1] + gr[2] * gr[2]);
+  const float gl[3] = {T.R[0] * d.x + T.R[3] * d.y + T.R[6] * d.z, T.R[1] * d.x + T.R[4] * d.y + T.R[7] * d.z,
+                       T.R[2] * d.x + T.R[5] * d.y + T.R[8] * d.z};  // R^T dL/dn_world
+  float dg[3];
+  if (gn > DVX_NRM_EPS) {
+    const float nl[3] = {-gr[0] / gn, -gr[1] / gn, -gr[2] / gn};
+    const float dot = nl[0] * gl[0] + nl[1] * gl[1] + nl[2] * gl[2];
+#pragma unroll
+    for (int a = 0; a < 3; ++a) dg[a] = -(gl[a] - nl[a] * dot) / gn;
+  } else {
+#pragma unroll
+    for (int a = 0; a < 3; ++a) dg[a] = -gl[a] / DVX_NRM_EPS;
+  }
+  float4 *o = reinterpret_cast<float4 *>(T.dgeo + (size_t)v * 8);
+  float4 o0 = o[0], o1 = o[1];
+  const float qx = 0.25f * dg[0], qy = 0.25f * dg[1], qz = 0.25f * dg[2];
+  o0.x += -qx - qy - qz; o0.y += -qx - qy + qz; o0.z += -qx + qy - qz; o0.w += -qx + qy + qz;
+  o1.x += qx - qy - qz;  o1.y += qx - qy + qz;  o1.z += qx + qy - qz;  o1.w += qx + qy + qz;
+  o[0] = o0; o[1] = o1;
+}
+
 inline unsigned blocks_for(uint64_t n, int threads) { return (unsigned)((n + threads - 1) / threads); }
 
 }  // namespace
@@ -425,9 +481,16 @@ void dvx_tile_masks_launch(const FrameParams &p, const TreeFrame *trees, uint8_t
                            cudaStream_t st) {
   { DVX_COUNT_LAUNCH(1); tile_masks_kernel<<<blocks_for(p.n_tiles, 128), 128, 0, st>>>(p, trees, octmask, actor_mask); }
 }
+void dvx_normal_backward_launch(const FrameParams &p, const TreeFrame *trees, const ushort4 *pxrect, const float *dnrm,
+                                cudaStream_t st) {
+  if (p.v_total) {
+    DVX_COUNT_LAUNCH(1);
+    normal_backward_kernel<<<blocks_for(p.v_total, PRE_THREADS), PRE_THREADS, 0, st>>>(p, trees, pxrect, dnrm);
+  }
+}
 void dvx_preprocess_launch(const FrameParams &p, const TreeFrame *trees, const uint8_t *octmask, FrameVox *fvox,
-                           ushort4 *pxrect, unsigned long long *counters, cudaStream_t st) {
-    if (p.v_total) { DVX_COUNT_LAUNCH(1); preprocess_kernel<<<blocks_for(p.v_total, PRE_THREADS), PRE_THREADS, 0, st>>>(p, trees, octmask, fvox, pxrect, counters); }
+                           ushort4 *pxrect, float4 *vnrm, unsigned long long *counters, cudaStream_t st) {
+    if (p.v_total) { DVX_COUNT_LAUNCH(1); preprocess_kernel<<<blocks_for(p.v_total, PRE_THREADS), PRE_THREADS, 0, st>>>(p, trees, octmask, fvox, pxrect, vnrm, counters); }
 }
 void dvx_emit_pairs_launch(const FrameParams &p, const TreeFrame *trees, const uint8_t *octmask, const ushort4 *pxrect,
                            const FrameVox *fvox, uint64_t *keys, uint32_t *vals, unsigned long long capacity,

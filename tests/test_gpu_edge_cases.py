@@ -201,3 +201,52 @@ def test_sky_on_config1_and_empty_scene(ctx, config1):
     torch.cuda.synchronize()
     es = scene(empty_tree(), cam=sc.cameras[0])
     assert np.abs(r.cpu().numpy() - O.render(es, sky=tex)["rgb"]).max() <= 1e-5 and float(a.abs().max()) == 0.0
+
+
+@pytest.mark.parametrize("seed,t_stop", [(51, 0.0), (53, 1e-4), (57, 0.05)])
+def test_normal_map_o11(ctx, seed, t_stop):
+    """O11 / R22: N = sum T alpha n (world frame) and its backward (through the weights and through the voxel normals),
+    every pixel and every gradient entry against the oracle; the other outputs must not change when normals are on."""
+    import paper_2606_23031_b200 as dvx
+    import torch
+    sc = _round_to_f32(S.tiny_random_scene(seed, sh_degree=1, width=40, height=24))
+    sc.t_stop = t_stop
+    gin = sc.image_grads(rgb_std=1e-2, depth_std=1e-3, alpha_std=1e-2)
+    idx = np.arange(40 * 24 * 3, dtype=np.uint64)
+    gin["normal"] = (1e-2 * S.rng.normal(seed, 960, idx)).astype(np.float32).reshape(24, 40, 3)
+    ref = O.render(sc, mode=0, grads_in=gin)
+    assert np.abs(ref["normal"]).max() > 0.05
+    dev = dvx.SceneOnDevice(ctx, sc)
+    rgb, depth, alpha, normal, frame = dev.render(normals=True)
+    rgb0, depth0, alpha0, _ = dev.render(save=False)
+    torch.cuda.synchronize()
+    assert torch.equal(rgb, rgb0) and torch.equal(depth, depth0) and torch.equal(alpha, alpha0)
+    assert np.abs(normal.cpu().numpy() - ref["normal"]).max() <= RGB_TOL
+    assert np.abs(rgb.cpu().numpy() - ref["rgb"]).max() <= RGB_TOL
+    g = {k: torch.from_numpy(v).cuda() for k, v in gin.items()}
+    grads = frame.backward(g["rgb"], g["depth"], g["alpha"], dL_dnormal=g["normal"])
+    torch.cuda.synchronize()
+    for t in range(len(sc.octrees)):
+        for got, want, name in ((grads[t][0], ref["dgeo"][t], "dgeo"), (grads[t][1], ref["dsh"][t], "dsh")):
+            err = np.abs(got.cpu().numpy().astype(np.float64) - want)
+            bound = GRAD_REL * np.abs(want) + GRAD_ABS
+            assert (err <= bound).all(), "%s[%d]: worst excess %g" % (name, t, (err - bound).max())
+    # a frame rendered without normals refuses a normal gradient
+    _, _, _, f2 = dev.render()
+    with pytest.raises(dvx.DvxError):
+        f2.backward(g["rgb"], dL_dnormal=g["normal"])
+    f2.release()
+    frame.release()
+
+
+def test_normal_map_on_config1_with_sky(ctx, config1):
+    import paper_2606_23031_b200 as dvx
+    import torch
+    sc = config1
+    tex = _sky_map(8, 16, 5)
+    ref = O.render(sc, mode=0, sky=tex, normals=True)
+    dev = dvx.SceneOnDevice(ctx, sc)
+    rgb, depth, alpha, normal, _ = dev.render(save=False, normals=True, sky=torch.from_numpy(tex).cuda())
+    torch.cuda.synchronize()
+    assert np.abs(normal.cpu().numpy() - ref["normal"]).max() <= RGB_TOL
+    assert np.abs(rgb.cpu().numpy() - ref["rgb"]).max() <= RGB_TOL
