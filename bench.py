@@ -190,6 +190,38 @@ def algorithmic_bytes(scene, W, H, cnt, touched):
     return b
 
 
+def _bits_for(n):
+    b = 1
+    while (1 << b) < n:
+        b += 1
+    return b
+
+
+def sort_throughput(ctx, n_pairs, scene, W, H, reps=5):
+    """Step 2's radix sort alone (dvx_sort_pairs: the same kernels dvx_render runs), on as many seeded random pairs as one
+    frame produces, with the frame's key width (tile | tree | octant | rank).  Mpairs/s, CUDA events, median of reps."""
+    import torch
+    n_tiles = ((W + 15) // 16) * ((H + 15) // 16)
+    key_bits = _bits_for(max(t.n_voxels for t in scene.octrees)) + _bits_for(n_tiles * len(scene.octrees) * 8)
+    n = max(int(n_pairs), 1)
+    g = torch.Generator(device="cuda").manual_seed(1)
+    base = torch.randint(0, 1 << min(key_bits, 62), (n,), dtype=torch.int64, device="cuda", generator=g)
+    vals0 = torch.arange(n, dtype=torch.int32, device="cuda")
+    times = []
+    for _ in range(reps + 1):
+        keys, vals = base.clone(), vals0.clone()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        ctx.check(ctx.lib.dvx_sort_pairs(ctx.h, keys.data_ptr(), vals.data_ptr(), n, key_bits))
+        e1.record()
+        torch.cuda.synchronize()
+        times.append(e0.elapsed_time(e1))
+    assert bool((keys[1:] >= keys[:-1]).all())
+    ms = float(np.median(times[1:]))
+    return {"pairs": n, "key_bits": key_bits, "passes": (key_bits + 7) // 8, "ms": ms, "mpairs_per_s": n / ms / 1e3,
+            "gb_per_s_moved": n * 12 * 2 * ((key_bits + 7) // 8) / ms / 1e6}
+
+
 def run_dvx(args):
     import torch
     import torch.distributed as dist
@@ -278,6 +310,7 @@ def run_dvx(args):
         step(host=True, bwd=not args.fwd_only)
     ms_e2e = timed(args.steps, host=True, bwd=not args.fwd_only)
     clocks = sampler.stop() if sampler else None
+    sort_stats = sort_throughput(ctx, cnt["pairs"] // n_cams, scene, W, H) if rank == 0 else None
 
     if rank != 0:
         if world > 1:
@@ -327,6 +360,7 @@ def run_dvx(args):
                          "peak_source": "148 SMs x 128 fp32 lanes x %.0f MHz (nvidia-smi, under load)" % sm_mhz},
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": (0 if args.fwd_only else 12 * px_step),
                 "d2h_bytes_per_step": 20 * px_step, "ms_per_step": ms_e2e / args.steps},
+        "sort": sort_stats,
         "gpu_launches": launches, "clocks": clocks,
     }
     if not args.no_cpu_baseline and world == 1:

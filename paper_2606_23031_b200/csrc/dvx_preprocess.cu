@@ -170,6 +170,7 @@ __device__ __forceinline__ uint32_t count_pairs_warp(const FrameParams &p, const
   return c;
 }
 
+template <bool NRM>
 __global__ void __launch_bounds__(PRE_THREADS) preprocess_kernel(FrameParams p, const TreeFrame *trees,
                                                                  const uint8_t *octmask, FrameVox *fvox,
                                                                  ushort4 *pxrect, float4 *vnrm,
@@ -235,7 +236,7 @@ __global__ void __launch_bounds__(PRE_THREADS) preprocess_kernel(FrameParams p, 
       }
       fv.meta = meta | (npairs << 8);  // bits 8-31: this voxel's pair count (step 2 allocates its slots from it)
       fvox[g] = fv;
-      if (vnrm) {  // O11 / R22: world-frame voxel normal, only when a normal map was requested
+      if (NRM) {  // O11 / R22: world-frame voxel normal, only when a normal map was requested
         const float4 *gp = reinterpret_cast<const float4 *>(T.geo + (size_t)v * 8);
         const float4 g0 = __ldg(gp), g1 = __ldg(gp + 1);
         const float gg[8] = {g0.x, g0.y, g0.z, g0.w, g1.x, g1.y, g1.z, g1.w};
@@ -490,7 +491,10 @@ void dvx_normal_backward_launch(const FrameParams &p, const TreeFrame *trees, co
 }
 void dvx_preprocess_launch(const FrameParams &p, const TreeFrame *trees, const uint8_t *octmask, FrameVox *fvox,
                            ushort4 *pxrect, float4 *vnrm, unsigned long long *counters, cudaStream_t st) {
-    if (p.v_total) { DVX_COUNT_LAUNCH(1); preprocess_kernel<<<blocks_for(p.v_total, PRE_THREADS), PRE_THREADS, 0, st>>>(p, trees, octmask, fvox, pxrect, vnrm, counters); }
+  if (!p.v_total) return;
+  DVX_COUNT_LAUNCH(1);
+  if (vnrm) preprocess_kernel<true><<<blocks_for(p.v_total, PRE_THREADS), PRE_THREADS, 0, st>>>(p, trees, octmask, fvox, pxrect, vnrm, counters);
+  else preprocess_kernel<false><<<blocks_for(p.v_total, PRE_THREADS), PRE_THREADS, 0, st>>>(p, trees, octmask, fvox, pxrect, vnrm, counters);
 }
 void dvx_emit_pairs_launch(const FrameParams &p, const TreeFrame *trees, const uint8_t *octmask, const ushort4 *pxrect,
                            const FrameVox *fvox, uint64_t *keys, uint32_t *vals, unsigned long long capacity,
