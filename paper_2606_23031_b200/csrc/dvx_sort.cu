@@ -172,6 +172,127 @@ __global__ void __launch_bounds__(SORT_THREADS) radix_scatter(const uint64_t *__
   }
 }
 
+// ------------------------------------------------------------------ one-sweep pass (decoupled look-back)
+// One kernel per digit instead of histogram + scan + scatter: the global base of every digit comes from one up-front
+// histogram of all digit positions (digit counts do not depend on the order of the keys), and the offset of a tile inside
+// a digit comes from a look-back over the per-tile digit counts that earlier tiles publish in `status`.  Tiles take their
+// index from a ticket counter, so a tile only ever waits for tiles that are already running (no deadlock).
+constexpr uint32_t ST_AGG = 1u << 30, ST_PREFIX = 1u << 31, ST_MASK = ST_AGG - 1u;  // counts < 2^30 (checked by the host)
+constexpr int MAX_PASSES = 8;
+
+__global__ void __launch_bounds__(SORT_THREADS) radix_digit_hist(const uint64_t *__restrict__ keys, uint64_t n, int passes,
+                                                                  uint32_t *__restrict__ ghist /* [passes][RADIX] */) {
+  __shared__ uint32_t h[MAX_PASSES][RADIX];
+  for (int p = 0; p < passes; ++p) h[p][threadIdx.x] = 0;
+  __syncthreads();
+  for (uint64_t i = (uint64_t)blockIdx.x * SORT_THREADS + threadIdx.x; i < n; i += (uint64_t)gridDim.x * SORT_THREADS) {
+    const uint64_t k = keys[i];
+    for (int p = 0; p < passes; ++p) atomicAdd(&h[p][(uint32_t)(k >> (8 * p)) & (RADIX - 1)], 1u);
+  }
+  __syncthreads();
+  for (int p = 0; p < passes; ++p)
+    if (h[p][threadIdx.x]) atomicAdd(&ghist[p * RADIX + threadIdx.x], h[p][threadIdx.x]);
+}
+// one block per pass: exclusive scan of its 256 digit counts, in place
+__global__ void __launch_bounds__(RADIX) radix_digit_scan(uint32_t *ghist) {
+  uint32_t *g = ghist + blockIdx.x * RADIX;
+  uint32_t total;
+  const uint32_t ex = block_excl_scan(g[threadIdx.x], &total);
+  g[threadIdx.x] = ex;
+}
+
+__global__ void __launch_bounds__(SORT_THREADS) radix_onesweep(const uint64_t *__restrict__ keys_in,
+                                                                const uint32_t *__restrict__ vals_in,
+                                                                uint64_t *__restrict__ keys_out, uint32_t *__restrict__ vals_out,
+                                                                uint64_t n, uint32_t shift, const uint32_t *__restrict__ dbase,
+                                                                volatile uint32_t *status /* [tiles][RADIX], zeroed */,
+                                                                uint32_t *ticket) {
+  __shared__ uint32_t cnt[SORT_WARPS][RADIX];
+  __shared__ uint64_t s_key[SORT_TILE];
+  __shared__ uint32_t s_val[SORT_TILE];
+  __shared__ uint32_t gbase[RADIX];
+  __shared__ uint32_t s_tile;
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  if (threadIdx.x == 0) s_tile = atomicAdd(ticket, 1u);
+  for (int d = lane; d < RADIX; d += 32) cnt[w][d] = 0;
+  __syncthreads();
+  const uint32_t tile = s_tile;
+  const uint64_t tbase = (uint64_t)tile * SORT_TILE;
+  const uint64_t wbase = tbase + (uint64_t)w * (32 * SORT_ITEMS);
+  uint64_t key[SORT_ITEMS];
+  uint16_t rnk[SORT_ITEMS];
+#pragma unroll
+  for (int i = 0; i < SORT_ITEMS; ++i) {
+    const uint64_t idx = wbase + (uint64_t)i * 32 + lane;
+    key[i] = idx < n ? keys_in[idx] : 0;
+  }
+#pragma unroll
+  for (int i = 0; i < SORT_ITEMS; ++i) {
+    const uint64_t idx = wbase + (uint64_t)i * 32 + lane;
+    const bool valid = idx < n;
+    const uint32_t d = valid ? ((uint32_t)(key[i] >> shift) & (RADIX - 1)) : RADIX;  // RADIX = "no key"
+    const uint32_t peers = __match_any_sync(0xffffffffu, d);
+    const uint32_t before = __popc(peers & ((1u << lane) - 1u));
+    const int leader = __ffs(peers) - 1;
+    uint32_t old = 0;
+    if (valid && lane == leader) {
+      old = cnt[w][d];
+      cnt[w][d] = old + __popc(peers);
+    }
+    old = __shfl_sync(0xffffffffu, old, leader);
+    rnk[i] = (uint16_t)(old + before);
+    __syncwarp();
+  }
+  __syncthreads();
+  {  // digit d = threadIdx.x
+    const int d = threadIdx.x;
+    uint32_t run = 0;
+#pragma unroll
+    for (int ww = 0; ww < SORT_WARPS; ++ww) {
+      const uint32_t c = cnt[ww][d];
+      cnt[ww][d] = run;
+      run += c;
+    }
+    // publish this tile's count of digit d, then look back for the number of keys with digit d in earlier tiles
+    volatile uint32_t *mine = status + (size_t)tile * RADIX + d;
+    *mine = run | (tile == 0 ? ST_PREFIX : ST_AGG);
+    uint32_t excl = 0;
+    if (tile > 0) {
+      uint32_t t = tile - 1;
+      for (;;) {
+        const uint32_t v = status[(size_t)t * RADIX + d];
+        if (v & ST_PREFIX) { excl += v & ST_MASK; break; }
+        if (v & ST_AGG) { excl += v & ST_MASK; --t; }   // tile 0 always publishes a prefix, so t never underflows
+      }
+      *mine = (excl + run) | ST_PREFIX;
+    }
+    uint32_t total;
+    const uint32_t lbase = block_excl_scan(run, &total);
+#pragma unroll
+    for (int ww = 0; ww < SORT_WARPS; ++ww) cnt[ww][d] += lbase;
+    gbase[d] = dbase[d] + excl - lbase;
+  }
+  __syncthreads();
+#pragma unroll
+  for (int i = 0; i < SORT_ITEMS; ++i) {
+    const uint64_t idx = wbase + (uint64_t)i * 32 + lane;
+    if (idx < n) {
+      const uint32_t d = (uint32_t)(key[i] >> shift) & (RADIX - 1);
+      const uint32_t pos = cnt[w][d] + rnk[i];
+      s_key[pos] = key[i];
+      s_val[pos] = vals_in[idx];
+    }
+  }
+  __syncthreads();
+  const uint32_t nb = (uint32_t)min((uint64_t)SORT_TILE, n - tbase);
+  for (uint32_t i = threadIdx.x; i < nb; i += SORT_THREADS) {
+    const uint64_t k = s_key[i];
+    const uint32_t out = gbase[(uint32_t)(k >> shift) & (RADIX - 1)] + i;
+    keys_out[out] = k;
+    vals_out[out] = s_val[i];
+  }
+}
+
 inline uint64_t ceil_div(uint64_t a, uint64_t b) { return (a + b - 1) / b; }
 
 }  // namespace
@@ -198,21 +319,48 @@ void dvx_scan_u32_launch(uint32_t *data, uint64_t n, uint32_t *scratch, cudaStre
   { DVX_COUNT_LAUNCH(1); scan_apply<<<(unsigned)nb, SCAN_THREADS, 0, st>>>(data, n, scratch); }
 }
 
+// scratch: legacy path = per-tile histograms + scan levels; one-sweep path = digit histograms, tickets, tile status
+static size_t onesweep_words(uint64_t n) {
+  uint64_t nb = ceil_div(n ? n : 1, SORT_TILE);
+  return (size_t)MAX_PASSES * RADIX + MAX_PASSES + (size_t)MAX_PASSES * nb * RADIX;
+}
 size_t dvx_sort_scratch_bytes(uint64_t n) {
   uint64_t nb = ceil_div(n ? n : 1, SORT_TILE);
   uint64_t hist = nb * RADIX;
-  return (hist + scan_scratch_elems(hist) + 64) * sizeof(uint32_t);
+  size_t legacy = hist + scan_scratch_elems(hist) + 64;
+  size_t one = onesweep_words(n) + 64;
+  return (legacy > one ? legacy : one) * sizeof(uint32_t);
 }
 
 int dvx_sort_launch(uint64_t *keys_a, uint32_t *vals_a, uint64_t *keys_b, uint32_t *vals_b, uint64_t n, uint32_t key_bits,
                     void *scratch, cudaStream_t st) {
   if (n == 0) return 0;
   uint32_t nb = (uint32_t)ceil_div(n, SORT_TILE);
-  uint32_t *hist = (uint32_t *)scratch;
-  uint32_t *scan_scr = hist + (uint64_t)nb * RADIX;
   int passes = (int)((key_bits + 7) / 8);
   if (passes < 1) passes = 1;
   int cur = 0;
+#ifndef DVX_SORT_LEGACY
+  if (n < (1ull << 30)) {  // one-sweep: 2 + passes launches
+    uint32_t *ghist = (uint32_t *)scratch;                 // [MAX_PASSES][RADIX]
+    uint32_t *ticket = ghist + MAX_PASSES * RADIX;         // [MAX_PASSES]
+    uint32_t *status = ticket + MAX_PASSES;                // [passes][nb][RADIX]
+    cudaMemsetAsync(scratch, 0, (MAX_PASSES * RADIX + MAX_PASSES + (size_t)passes * nb * RADIX) * sizeof(uint32_t), st);
+    const unsigned hb = nb < 592u ? nb : 592u;
+    { DVX_COUNT_LAUNCH(1); radix_digit_hist<<<hb, SORT_THREADS, 0, st>>>(keys_a, n, passes, ghist); }
+    { DVX_COUNT_LAUNCH(1); radix_digit_scan<<<passes, RADIX, 0, st>>>(ghist); }
+    for (int p = 0; p < passes; ++p) {
+      uint64_t *kin = cur ? keys_b : keys_a, *kout = cur ? keys_a : keys_b;
+      uint32_t *vin = cur ? vals_b : vals_a, *vout = cur ? vals_a : vals_b;
+      DVX_COUNT_LAUNCH(1);
+      radix_onesweep<<<nb, SORT_THREADS, 0, st>>>(kin, vin, kout, vout, n, 8u * p, ghist + p * RADIX,
+                                                  status + (size_t)p * nb * RADIX, ticket + p);
+      cur ^= 1;
+    }
+    return cur;
+  }
+#endif
+  uint32_t *hist = (uint32_t *)scratch;
+  uint32_t *scan_scr = hist + (uint64_t)nb * RADIX;
   for (int p = 0; p < passes; ++p) {
     uint64_t *kin = cur ? keys_b : keys_a, *kout = cur ? keys_a : keys_b;
     uint32_t *vin = cur ? vals_b : vals_a, *vout = cur ? vals_a : vals_b;
