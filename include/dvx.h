@@ -144,7 +144,10 @@ void dvx_frame_release(dvx_ctx *ctx, dvx_frame *frame);
  * data pipeline: dvx_render_host renders into device staging owned by the context and enqueues the device->host
  * copies of RGB, depth and alpha (out_host.* are HOST pointers; valid after the stream is synchronised);
  * dvx_backward_host enqueues the host->device copies of the incoming image gradients (HOST pointers; depth / alpha
- * may be NULL) and then runs step 5.  Octree arrays and gradient buffers stay DEVICE pointers (they are model
+ * may be NULL) and then runs step 5.  The copies run on a second, library-owned stream so that they overlap the compute
+ * on the context's stream (copy-out of frame i with the backward of frame i, copy-in with the forward); events order
+ * them.  The host images of dvx_render_host are valid once the context's stream has been synchronised AFTER the matching
+ * dvx_backward_host call (or directly after dvx_render_host when saved == NULL).  Octree arrays and gradient buffers stay DEVICE pointers (they are model
  * state that lives in HBM across steps).  Bytes moved per call: 20 W H out, 12 W H (+4 W H each for depth/alpha) in. */
 dvx_status dvx_render_host(dvx_ctx *ctx, const dvx_camera *cam, const dvx_octree *static_tree, uint32_t n_actors,
                            const dvx_octree *const *actors, const float *poses_l2w, const float *box_half,

@@ -29,6 +29,11 @@ struct dvx_ctx {
   std::vector<Block> all;    // every block ever obtained (freed in dvx_destroy)
   unsigned long long *h_counters = nullptr;  // pinned
   std::string err;
+  // host-buffer entry points: a second stream moves the images while the main stream computes
+  cudaStream_t cs = nullptr, cs_in = nullptr;  // copy-out and copy-in streams (one per direction: both overlap compute)
+  cudaEvent_t ev_main = nullptr, ev_d2h = nullptr, ev_h2d = nullptr, ev_bwd = nullptr;
+  float *st_out = nullptr, *st_in = nullptr;  // persistent device staging (grow-only)
+  size_t st_out_bytes = 0, st_in_bytes = 0;
 };
 
 struct dvx_octree {
@@ -212,6 +217,13 @@ void dvx_destroy(dvx_ctx *ctx) {
     else cudaFree(b.p);
   }
   cudaFreeHost(ctx->h_counters);
+  if (ctx->cs) {
+    cudaStreamSynchronize(ctx->cs);
+    cudaStreamSynchronize(ctx->cs_in);
+    cudaStreamDestroy(ctx->cs);
+    cudaStreamDestroy(ctx->cs_in);
+    cudaEventDestroy(ctx->ev_main); cudaEventDestroy(ctx->ev_d2h); cudaEventDestroy(ctx->ev_h2d); cudaEventDestroy(ctx->ev_bwd);
+  }
   for (auto *v : {&ctx->ev_free, &ctx->ev_pending})
     for (EventSet *es : *v) {
       for (auto &e : es->ev) cudaEventDestroy(e);
@@ -611,6 +623,27 @@ dvx_status dvx_stage_ms_collect(dvx_ctx *ctx, float *ms, uint32_t *n_frames) {
 
 uint64_t dvx_launch_count(void) { return (uint64_t)g_dvx_launches; }
 
+namespace {
+// lazily creates the copy stream and its events; (re)sizes a persistent staging buffer
+dvx_status host_io_setup(dvx_ctx *ctx, float **buf, size_t *have, size_t need) {
+  if (!ctx->cs) {
+    CU(cudaStreamCreateWithFlags(&ctx->cs, cudaStreamNonBlocking));
+    CU(cudaStreamCreateWithFlags(&ctx->cs_in, cudaStreamNonBlocking));
+    for (cudaEvent_t *e : {&ctx->ev_main, &ctx->ev_d2h, &ctx->ev_h2d, &ctx->ev_bwd}) CU(cudaEventCreateWithFlags(e, cudaEventDisableTiming));
+  }
+  if (*have < need) {
+    CU(cudaStreamSynchronize(ctx->cs));  // nothing in flight may still use the old buffer
+    CU(cudaStreamSynchronize(ctx->cs_in));
+    CU(cudaStreamSynchronize(ctx->st));
+    ctx_release(ctx, *buf);
+    *buf = (float *)ctx_alloc(ctx, need);
+    *have = *buf ? need : 0;
+    if (!*buf) return fail(ctx, DVX_ERR_OOM, "host staging: allocator returned NULL");
+  }
+  return DVX_OK;
+}
+}  // namespace
+
 dvx_status dvx_render_host(dvx_ctx *ctx, const dvx_camera *cam, const dvx_octree *static_tree, uint32_t n_actors,
                            const dvx_octree *const *actors, const float *poses_l2w, const float *box_half,
                            const dvx_render_opts *opts, dvx_image out_host, dvx_frame **saved) {
@@ -619,19 +652,24 @@ dvx_status dvx_render_host(dvx_ctx *ctx, const dvx_camera *cam, const dvx_octree
   if (!cam || !out_host.rgb || !out_host.depth || !out_host.alpha) return fail(ctx, DVX_ERR_INVALID_ARG, "NULL argument");
   cudaSetDevice(ctx->device);
   const size_t npix = (size_t)cam->width * cam->height;
-  float *stage = (float *)ctx_alloc(ctx, npix * 32);
-  if (!stage) return fail(ctx, DVX_ERR_OOM, "dvx_render_host: allocator returned NULL");
+  dvx_status rc = host_io_setup(ctx, &ctx->st_out, &ctx->st_out_bytes, npix * 32);
+  if (rc != DVX_OK) return rc;
+  float *stage = ctx->st_out;
   dvx_image dev = {stage, stage + 3 * npix, stage + 4 * npix, out_host.normal ? stage + 5 * npix : nullptr};
-  dvx_status rc = dvx_render(ctx, cam, static_tree, n_actors, actors, poses_l2w, box_half, opts, dev, saved);
-  if (rc == DVX_OK) {
-    cudaError_t e = cudaMemcpyAsync(out_host.rgb, dev.rgb, npix * 12, cudaMemcpyDeviceToHost, ctx->st);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(out_host.depth, dev.depth, npix * 4, cudaMemcpyDeviceToHost, ctx->st);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(out_host.alpha, dev.alpha, npix * 4, cudaMemcpyDeviceToHost, ctx->st);
-    if (e == cudaSuccess && dev.normal) e = cudaMemcpyAsync(out_host.normal, dev.normal, npix * 12, cudaMemcpyDeviceToHost, ctx->st);
-    if (e != cudaSuccess) rc = cuda_fail(ctx, e, "dvx_render_host: cudaMemcpyAsync");
-  }
-  ctx_release(ctx, stage);  // stream-ordered reuse: later users of the block are enqueued after the copies
-  return rc;
+  CU(cudaStreamWaitEvent(ctx->st, ctx->ev_d2h, 0));  // the previous frame's copy-out must have left the staging buffer
+  rc = dvx_render(ctx, cam, static_tree, n_actors, actors, poses_l2w, box_half, opts, dev, saved);
+  if (rc != DVX_OK) return rc;
+  // copy-out on the copy stream: it overlaps whatever the main stream does next (the backward of this frame)
+  CU(cudaEventRecord(ctx->ev_main, ctx->st));
+  CU(cudaStreamWaitEvent(ctx->cs, ctx->ev_main, 0));
+  CU(cudaMemcpyAsync(out_host.rgb, dev.rgb, npix * 12, cudaMemcpyDeviceToHost, ctx->cs));
+  CU(cudaMemcpyAsync(out_host.depth, dev.depth, npix * 4, cudaMemcpyDeviceToHost, ctx->cs));
+  CU(cudaMemcpyAsync(out_host.alpha, dev.alpha, npix * 4, cudaMemcpyDeviceToHost, ctx->cs));
+  if (dev.normal) CU(cudaMemcpyAsync(out_host.normal, dev.normal, npix * 12, cudaMemcpyDeviceToHost, ctx->cs));
+  CU(cudaEventRecord(ctx->ev_d2h, ctx->cs));
+  // inference (nothing saved): the caller's next synchronisation of the main stream must cover the copies
+  if (!saved) CU(cudaStreamWaitEvent(ctx->st, ctx->ev_d2h, 0));
+  return DVX_OK;
 }
 
 dvx_status dvx_backward_host(dvx_ctx *ctx, dvx_frame *f, const float *g_rgb_h, const float *g_depth_h, const float *g_alpha_h,
@@ -640,15 +678,21 @@ dvx_status dvx_backward_host(dvx_ctx *ctx, dvx_frame *f, const float *g_rgb_h, c
   if (!f || !g_rgb_h) return fail(ctx, DVX_ERR_INVALID_ARG, "NULL argument");
   cudaSetDevice(ctx->device);
   const size_t npix = (size_t)f->p.width * f->p.height;
-  float *stage = (float *)ctx_alloc(ctx, npix * 20);
-  if (!stage) return fail(ctx, DVX_ERR_OOM, "dvx_backward_host: allocator returned NULL");
+  dvx_status rc = host_io_setup(ctx, &ctx->st_in, &ctx->st_in_bytes, npix * 20);
+  if (rc != DVX_OK) return rc;
+  float *stage = ctx->st_in;
   float *d_rgb = stage, *d_depth = g_depth_h ? stage + 3 * npix : nullptr, *d_alpha = g_alpha_h ? stage + 4 * npix : nullptr;
-  cudaError_t e = cudaMemcpyAsync(d_rgb, g_rgb_h, npix * 12, cudaMemcpyHostToDevice, ctx->st);
-  if (e == cudaSuccess && d_depth) e = cudaMemcpyAsync(d_depth, g_depth_h, npix * 4, cudaMemcpyHostToDevice, ctx->st);
-  if (e == cudaSuccess && d_alpha) e = cudaMemcpyAsync(d_alpha, g_alpha_h, npix * 4, cudaMemcpyHostToDevice, ctx->st);
-  dvx_status rc = e == cudaSuccess ? dvx_backward(ctx, f, d_rgb, d_depth, d_alpha, static_grad, actor_grads)
-                                   : cuda_fail(ctx, e, "dvx_backward_host: cudaMemcpyAsync");
-  ctx_release(ctx, stage);
+  // copy-in on the copy stream (it overlaps the forward still running on the main stream), after the previous backward
+  // has finished reading the staging buffer
+  CU(cudaStreamWaitEvent(ctx->cs_in, ctx->ev_bwd, 0));
+  CU(cudaMemcpyAsync(d_rgb, g_rgb_h, npix * 12, cudaMemcpyHostToDevice, ctx->cs_in));
+  if (d_depth) CU(cudaMemcpyAsync(d_depth, g_depth_h, npix * 4, cudaMemcpyHostToDevice, ctx->cs_in));
+  if (d_alpha) CU(cudaMemcpyAsync(d_alpha, g_alpha_h, npix * 4, cudaMemcpyHostToDevice, ctx->cs_in));
+  CU(cudaEventRecord(ctx->ev_h2d, ctx->cs_in));
+  CU(cudaStreamWaitEvent(ctx->st, ctx->ev_h2d, 0));
+  rc = dvx_backward(ctx, f, d_rgb, d_depth, d_alpha, static_grad, actor_grads);
+  CU(cudaEventRecord(ctx->ev_bwd, ctx->st));
+  CU(cudaStreamWaitEvent(ctx->st, ctx->ev_d2h, 0));  // a main-stream synchronisation after this call also covers the copy-out
   return rc;
 }
 
