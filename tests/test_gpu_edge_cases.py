@@ -250,3 +250,45 @@ def test_normal_map_on_config1_with_sky(ctx, config1):
     torch.cuda.synchronize()
     assert np.abs(normal.cpu().numpy() - ref["normal"]).max() <= RGB_TOL
     assert np.abs(rgb.cpu().numpy() - ref["rgb"]).max() <= RGB_TOL
+
+
+def test_refresh_structure_and_max_actors(ctx):
+    """dvx_octree_refresh_structure after the leaf set changed = a freshly created handle; 64 actors (DVX_MAX_ACTORS) render
+    like the oracle, 65 are refused."""
+    import ctypes as C
+    import paper_2606_23031_b200 as dvx
+    import torch
+    sc = _round_to_f32(S.tiny_random_scene(61, sh_degree=1, width=24, height=16))
+    other = _round_to_f32(S.tiny_random_scene(67, sh_degree=1, width=24, height=16))
+    dev = dvx.SceneOnDevice(ctx, sc)
+    # swap the static tree's arrays for those of another scene through refresh_structure
+    t0, new = dev.trees[0], other.static
+    code = torch.from_numpy(np.ascontiguousarray(new.code).view(np.int64)).cuda()
+    geo = torch.from_numpy(np.ascontiguousarray(new.geo, dtype=np.float32)).cuda()
+    sh = torch.from_numpy(np.ascontiguousarray(new.sh, dtype=np.float32)).cuda()
+    desc = dvx.binding.OctreeDesc(new.n_voxels, new.sh_degree, (C.c_float * 3)(*[float(x) for x in new.center]), float(new.side),
+                                  code.data_ptr(), geo.data_ptr(), sh.data_ptr())
+    ctx.check(ctx.lib.dvx_octree_refresh_structure(ctx.h, t0.h, C.byref(desc)))
+    t0.code, t0.geo, t0.sh, t0.n_voxels = code, geo, sh, new.n_voxels
+    rgb, depth, alpha, _ = dev.render(save=False)
+    torch.cuda.synchronize()
+    mixed = scene(new, sc.actors, sc.poses, sc.box_half, cam=sc.cameras[0], t_stop=sc.t_stop)
+    ref = O.render(mixed, mode=0)
+    assert np.abs(rgb.cpu().numpy() - ref["rgb"]).max() <= RGB_TOL and np.abs(alpha.cpu().numpy() - ref["alpha"]).max() <= RGB_TOL
+    # 64 actors: one single-voxel actor replicated on a grid in front of the camera
+    act = tree_from_cells([(0, 0, 0, 1), (1, 1, 1, 1)], geo=np.linspace(-1, 1, 16).reshape(2, 8), side=0.5)
+    poses, halves = [], []
+    for n in range(64):
+        poses.append(S.pose_yaw((1.0 + 0.7 * (n // 8), -2.5 + 0.7 * (n % 8), 0.2 * ((n * 7) % 5)), 0.1 * n))
+        halves.append([0.25, 0.25, 0.25])
+    many = _round_to_f32(scene(sc.static, [act] * 64, poses, halves, cam=sc.cameras[0], t_stop=0.0))
+    dev2 = dvx.SceneOnDevice(ctx, many)
+    rgb, depth, alpha, _ = dev2.render(save=False)
+    torch.cuda.synchronize()
+    ref = O.render(many, mode=0)
+    assert np.abs(rgb.cpu().numpy() - ref["rgb"]).max() <= RGB_TOL
+    assert (np.abs(depth.cpu().numpy() - ref["depth"]) / np.maximum(np.abs(ref["depth"]), 1.0)).max() <= DEPTH_REL
+    with pytest.raises(dvx.DvxError) as e:
+        ctx.render(dev2.cams[0], dev2.trees[0], dev2.trees[1:] + [dev2.trees[1]], np.concatenate([dev2.poses, dev2.poses[:1]]),
+                   np.concatenate([dev2.box_half, dev2.box_half[:1]]))
+    assert e.value.status == -1
