@@ -333,3 +333,33 @@ def test_multi_camera_accumulation_config5_semantics(ctx):
     for t in range(len(sc.octrees)):
         _check_grads(grads[t][0], ref_dgeo[t], "dgeo[%d] over 3 cameras" % t)
         _check_grads(grads[t][1], ref_dsh[t], "dsh[%d] over 3 cameras" % t)
+
+
+@pytest.mark.parametrize("cfg", [2, 4])
+def test_forward_is_bit_deterministic(ctx, cfg):
+    """The forward has no atomics: two renders of the same frame must agree bit for bit (a data race between the phases of
+    the tile kernel, or an unstable sort, would show up here), and the backward twice must agree to float-atomic noise."""
+    import paper_2606_23031_b200 as dvx
+    import torch
+    sc = S.make_config(cfg)
+    dev = dvx.SceneOnDevice(ctx, sc)
+    a = dev.render(normals=True)
+    b = dev.render(normals=True)
+    torch.cuda.synchronize()
+    for x, y in zip(a[:4], b[:4]):
+        assert torch.equal(x, y)
+    cam = sc.cameras[0]
+    tw = (cam.width + 15) // 16
+    for tile in (0, tw * 20 + 31, tw * 33 + 7):
+        for tree in range(min(len(sc.octrees), 3)):
+            for q in range(8):
+                assert np.array_equal(a[4].tile_list(tile, tree, q), b[4].tile_list(tile, tree, q))
+    g = torch.from_numpy(sc.image_grads(rgb_std=1e-2)["rgb"]).cuda()
+    ga, gb = a[4].backward(g), b[4].backward(g)
+    torch.cuda.synchronize()
+    for t in range(len(sc.octrees)):
+        ref = ga[t][0].abs().max().item()
+        assert (ga[t][0] - gb[t][0]).abs().max().item() <= 1e-5 * ref + 1e-9
+    a[4].release(); b[4].release()
+    for t in dev.trees:
+        t.close()
