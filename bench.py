@@ -287,6 +287,25 @@ def run_dvx(args):
         step(bwd=not args.fwd_only)
     torch.cuda.synchronize()
     touched = int(sum(int((g[0] != 0).any(dim=1).sum().item()) for g in grads))
+    # fraction of rays that reached T < t_stop (camera 0), hits per ray; step 0 uncached; the caller's gradient zeroing
+    frac_term = float((out_dev[2] > 1.0 - scene.t_stop).float().mean().item()) if scene.t_stop > 0 else 0.0
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t = scene.octrees[0]
+    e0.record()
+    tmp = ctx.octree(dev.trees[0].code, dev.trees[0].geo, dev.trees[0].sh, t.center, t.side, t.sh_degree)  # 8 sorts of V keys
+    e1.record()
+    torch.cuda.synchronize()
+    step0_ms = e0.elapsed_time(e1)
+    tmp.close()
+    e0.record()
+    for ga, gb in grads:
+        ga.zero_(); gb.zero_()
+    e1.record()
+    torch.cuda.synchronize()
+    grad_zero_ms = e0.elapsed_time(e1)
+    for _ in range(2):  # refill the gradient buffers so that the timed steps accumulate into touched memory as before
+        step(bwd=not args.fwd_only)
+    torch.cuda.synchronize()
 
     # ---- timed region 1: device-resident inputs
     ctx.stage_ms_collect()                       # drop the stage times of the warm-up frames
@@ -350,7 +369,9 @@ def run_dvx(args):
                    "passes": "fwd" if args.fwd_only else "fwd+bwd"},
         "fwd_value": fwd_value, "fwd_ms": ms_fwd / args.steps,
         "hbm_roofline_frac_step": hbm_frac_step,
-        "stage_ms": stage, "counters": dict(cnt, touched_voxels=touched),
+        "stage_ms": stage,
+        "counters": dict(cnt, touched_voxels=touched, hits_per_ray=cnt["q_hit"] / px_step, frac_rays_terminated=frac_term),
+        "step0_uncached_ms_static_octree": step0_ms, "grad_zero_ms_excluded": grad_zero_ms,
         "algorithmic_bytes": ab,
         "roofline": {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
                      "frac": achieved / peak if peak else None, "traffic": ncu_traffic, "peak_source": peak_src,
