@@ -59,7 +59,7 @@ struct __align__(16) Item {
   float w[3];         // x(tau) - centre = s' d + w
   float mid;          // (a + b) / 2, absolute ray distance (depth, R9)
   float d[3];         // ray direction in the tree frame
-  float tau;          // phase B: tau_v;  backward phase C overwrites it with dL/dtau_v
+  float pad;
 };
 
 template <bool BWD, bool NRM>
@@ -67,10 +67,10 @@ struct WarpQueue {
   EntryRec ent[32];
   Item item[QCAP];              // ring
   double d0[3];                 // the warp's reference direction for the list being served
-  float4 rgbm[32];              // phase B -> C: per batch item, the voxel's RGB and clamp bits (fetched by the item's lane)
-  float wg[BWD ? 3 : 1][32];    // backward phase C: T alpha g_C per batch item, zero where the colour clamp is active
-  float4 nrm[NRM ? 32 : 1];     // normal map (O11): per batch item the voxel's world normal
-  float wgn[(BWD && NRM) ? 3 : 1][32];  // backward phase C: T alpha g_N per batch item
+  // phase B -> C, per batch item (written by the item's lane, read by the pixel's lane):
+  float4 eam[32];               // exp(-tau_v), alpha_v, (a+b)/2, -;  backward phase C puts dL/dtau_v into .w for phase B2
+  float4 rgbm[32];              // the voxel's RGB and clamp bits;    backward phase C overwrites .xyz with T alpha g_C
+  float4 nrm[NRM ? 32 : 1];     // the voxel's world normal (O11);    backward phase C overwrites .xyz with T alpha g_N
 };
 
 struct Pix {
@@ -256,7 +256,10 @@ __device__ __forceinline__ void flush_batch(const CompositeArgs &A, int lane, Wa
   uint32_t my_id = NONE, my_meta = 0;
   const int at_b = (head + lane) & (QCAP - 1);
   if (lane < count) {
-    Q.item[at_b].tau = integrate_item<BWD, NRM>(A, Q, at_b, my_id, my_meta, G, M);
+    const float tau = integrate_item<BWD, NRM>(A, Q, at_b, my_id, my_meta, G, M);
+    const float e = ex2_approx(-tau * LOG2E);
+    const float alpha = tau < 1e-3f ? tau * fmaf(-0.5f, tau, 1.0f) : 1.0f - e;  // 1 - exp(-tau) without cancellation
+    Q.eam[lane] = make_float4(e, alpha, Q.item[at_b].mid, 0.f);
     Q.rgbm[lane] = __ldg(reinterpret_cast<const float4 *>(A.fvox + my_id) + 1);  // keeps the global load out of C's serial loop
     if (NRM) Q.nrm[lane] = __ldg(A.vnrm + my_id);
   }
@@ -267,14 +270,11 @@ __device__ __forceinline__ void flush_batch(const CompositeArgs &A, int lane, Wa
   while (mine) {
     const int i = __ffs(mine) - 1;
     mine &= mine - 1;
-    const int at = (head + i) & (QCAP - 1);
     if (!S.done) {
       const float4 f1 = Q.rgbm[i];
-      const float tau = Q.item[at].tau;
-      const float mid = Q.item[at].mid;
-      const float e = ex2_approx(-tau * LOG2E);
-      const float alpha = tau < 1e-3f ? tau * fmaf(-0.5f, tau, 1.0f) : 1.0f - e;  // 1 - exp(-tau) without cancellation
-      const float w = S.T * alpha;
+      const float4 ea = Q.eam[i];
+      const float e = ea.x, mid = ea.z;
+      const float w = S.T * ea.y;
       if (!BWD) {
         S.C0 = fmaf(w, f1.x, S.C0); S.C1 = fmaf(w, f1.y, S.C1); S.C2 = fmaf(w, f1.z, S.C2);
         S.D = fmaf(w, mid, S.D);
@@ -287,14 +287,12 @@ __device__ __forceinline__ void flush_batch(const CompositeArgs &A, int lane, Wa
         if (NRM) {
           const float4 nv = Q.nrm[i];
           X += S.gN0 * nv.x + S.gN1 * nv.y + S.gN2 * nv.z;
-          Q.wgn[0][i] = w * S.gN0; Q.wgn[1][i] = w * S.gN1; Q.wgn[2][i] = w * S.gN2;
+          Q.nrm[i] = make_float4(w * S.gN0, w * S.gN1, w * S.gN2, 0.f);
         }
         S.Xpre = fmaf(w, X, S.Xpre);
-        Q.item[at].tau = S.T * e * X - (S.Xtot - S.Xpre) + S.gA * S.T_final;  // dL/dtau_v
-        const uint32_t cm = __float_as_uint(f1.w);
-        Q.wg[0][i] = (cm & 1u) ? 0.f : w * S.gC0;
-        Q.wg[1][i] = (cm & 2u) ? 0.f : w * S.gC1;
-        Q.wg[2][i] = (cm & 4u) ? 0.f : w * S.gC2;
+        Q.eam[i].w = S.T * e * X - (S.Xtot - S.Xpre) + S.gA * S.T_final;  // dL/dtau_v
+        const uint32_t cm = __float_as_uint(f1.w);  // colour clamp active: no gradient through that channel (O7)
+        Q.rgbm[i] = make_float4((cm & 1u) ? 0.f : w * S.gC0, (cm & 2u) ? 0.f : w * S.gC1, (cm & 4u) ? 0.f : w * S.gC2, 0.f);
       }
       S.T *= e;
       S.n_used++;
@@ -304,9 +302,9 @@ __device__ __forceinline__ void flush_batch(const CompositeArgs &A, int lane, Wa
         if (S.n_used >= S.n_stop) S.done = true;
       }
     } else if (BWD) {  // queued before this pixel finished its replay: contributes nothing
-      Q.item[at].tau = 0.f;
-      Q.wg[0][i] = 0.f; Q.wg[1][i] = 0.f; Q.wg[2][i] = 0.f;
-      if (NRM) { Q.wgn[0][i] = 0.f; Q.wgn[1][i] = 0.f; Q.wgn[2][i] = 0.f; }
+      Q.eam[i].w = 0.f;
+      Q.rgbm[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+      if (NRM) Q.nrm[i] = make_float4(0.f, 0.f, 0.f, 0.f);
     }
   }
   my_bits >>= count;
@@ -318,13 +316,14 @@ __device__ __forceinline__ void flush_batch(const CompositeArgs &A, int lane, Wa
 #pragma unroll
     for (int c = 0; c < NV; ++c) val[c] = 0.f;
     if (lane < count) {
-      const float dtau = Q.item[at_b].tau * G.delta;
+      const float dtau = Q.eam[lane].w * G.delta;
       float cs[8];
       corner_sums(G, M, cs);
 #pragma unroll
       for (int c = 0; c < 8; ++c) val[c] = dtau * cs[c];
-      val[8] = Q.wg[0][lane]; val[9] = Q.wg[1][lane]; val[10] = Q.wg[2][lane];
-      if (NRM) { val[NV - 3] = Q.wgn[0][lane]; val[NV - 2] = Q.wgn[1][lane]; val[NV - 1] = Q.wgn[2][lane]; }
+      const float4 wc = Q.rgbm[lane];
+      val[8] = wc.x; val[9] = wc.y; val[10] = wc.z;
+      if (NRM) { const float4 wn = Q.nrm[lane]; val[NV - 3] = wn.x; val[NV - 2] = wn.y; val[NV - 1] = wn.z; }
     }
     // runs of consecutive items of one voxel (the pixels one list entry hit): segmented suffix sums over the run index,
     // the first lane of each run ends up with the run total.  (The voxel id itself is not a valid segment key: a voxel cut
