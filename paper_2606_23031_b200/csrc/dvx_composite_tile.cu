@@ -33,6 +33,9 @@ constexpr int TILE_WARPS = TILE_THREADS / 32;
 #ifndef DVX_TILE_MIN_CTAS
 #define DVX_TILE_MIN_CTAS 3
 #endif
+#ifndef DVX_RUN_SPLIT
+#define DVX_RUN_SPLIT 4  // backward: runs of one voxel are reduced in pieces of at most this many lanes (1, 2, 8, 16, 32 measured slower)
+#endif
 #ifndef DVX_WARP_W
 #define DVX_WARP_W 4   // a warp covers DVX_WARP_W x (32 / DVX_WARP_W) pixels
 #endif
@@ -331,9 +334,26 @@ __device__ __forceinline__ void flush_batch(const CompositeArgs &A, int lane, Wa
     const uint32_t prev = __shfl_up_sync(0xffffffffu, my_id, 1);
     const bool is_head = lane == 0 || prev != my_id;
     const uint32_t heads = __ballot_sync(0xffffffffu, is_head);
+#if DVX_RUN_SPLIT < 32
+    // runs longer than DVX_RUN_SPLIT lanes are cut into pieces of that length (each piece issues its own reductions), so
+    // the segmented scan needs log2(DVX_RUN_SPLIT) steps instead of 5
+    uint32_t heads2 = heads;
+    {
+      const uint32_t below = heads & (0xffffffffu >> (31 - lane));       // heads at or below this lane
+      const int start = 31 - __clz(below);                                // lane of this run's head
+      const bool extra = lane > start && ((lane - start) % DVX_RUN_SPLIT) == 0;
+      heads2 |= __ballot_sync(0xffffffffu, extra);
+    }
+    const bool is_head2 = (heads2 >> lane) & 1u;
+    const uint32_t run = __popc(heads2 & (0xffffffffu >> (31 - lane)));
+#pragma unroll
+    for (int o = 1; o < DVX_RUN_SPLIT; o <<= 1) {
+#else
+    const bool is_head2 = is_head;
     const uint32_t run = __popc(heads & (0xffffffffu >> (31 - lane)));
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
+#endif
       const uint32_t orun = __shfl_down_sync(0xffffffffu, run, o);
       const bool take = (lane + o < 32) && orun == run;
 #pragma unroll
@@ -342,7 +362,7 @@ __device__ __forceinline__ void flush_batch(const CompositeArgs &A, int lane, Wa
         if (take) val[c] += x;
       }
     }
-    if (my_id != NONE && is_head) {
+    if (my_id != NONE && is_head2) {
       const TreeFrame &T = A.trees[(my_meta >> 8) & 0xFFu];
       if (T.dgeo) {
         float *dg = T.dgeo + (size_t)(my_id - T.base) * 8;
