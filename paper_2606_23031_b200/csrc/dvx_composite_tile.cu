@@ -259,12 +259,25 @@ __device__ __forceinline__ void flush_batch(const CompositeArgs &A, int lane, Wa
   uint32_t my_id = NONE, my_meta = 0;
   const int at_b = (head + lane) & (QCAP - 1);
   if (lane < count) {
+    // Storing colour and normal to shared memory keeps every global load out of C's serial loop.
+    // Forward: the colour (and normal) loads go out before the integration so their latency hides under it. Backward keeps
+    // them after it: there the four extra live registers spill (measured: forward 1.39 -> 1.35 ms, backward 1.83 -> 1.87 ms).
+    float4 f1, nv = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (!BWD) {
+      const uint32_t id0 = Q.item[at_b].id;
+      f1 = __ldg(reinterpret_cast<const float4 *>(A.fvox + id0) + 1);
+      if (NRM) nv = __ldg(A.vnrm + id0);
+    }
     const float tau = integrate_item<BWD, NRM>(A, Q, at_b, my_id, my_meta, G, M);
+    if (BWD) {
+      f1 = __ldg(reinterpret_cast<const float4 *>(A.fvox + my_id) + 1);
+      if (NRM) nv = __ldg(A.vnrm + my_id);
+    }
     const float e = ex2_approx(-tau * LOG2E);
     const float alpha = tau < 1e-3f ? tau * fmaf(-0.5f, tau, 1.0f) : 1.0f - e;  // 1 - exp(-tau) without cancellation
     Q.eam[lane] = make_float4(e, alpha, Q.item[at_b].mid, 0.f);
-    Q.rgbm[lane] = __ldg(reinterpret_cast<const float4 *>(A.fvox + my_id) + 1);  // keeps the global load out of C's serial loop
-    if (NRM) Q.nrm[lane] = __ldg(A.vnrm + my_id);
+    Q.rgbm[lane] = f1;
+    if (NRM) Q.nrm[lane] = nv;
   }
   __syncwarp();
   // -- C: lane = pixel; its own items of the batch in queue order = front-to-back order along its ray
