@@ -180,6 +180,45 @@ const char *dvx_last_error(const dvx_ctx *ctx);
  * the low key_bits bits of the key, ascending, stable.  keys / vals DEVICE arrays, sorted in place. */
 dvx_status dvx_sort_pairs(dvx_ctx *ctx, uint64_t *keys, uint32_t *vals, uint64_t n, uint32_t key_bits);
 
+/* ---- Widening row N2: shared grid-point corner densities and the optimizer step -----------------------
+ * The corner densities "are optimized during training".  Reading R23: coincident corners of
+ * neighbouring voxels are ONE parameter (a grid point), identified by the corner's integer coordinate on the level-16
+ * lattice of the octree (hanging nodes are grid points of their own); grid points are numbered in ascending order of
+ * the 51-bit Morton key of that coordinate (bit b of x at 3b+2, of y at 3b+1, of z at 3b).  Reading R24: the optimizer
+ * is Adam (Kingma & Ba 2015, Algorithm 1, with bias correction).  The [V][8] corner record stays what the rasterizer
+ * reads and what dvx_backward accumulates into; these calls tie it to the per-grid-point parameter array. */
+typedef struct dvx_grid dvx_grid; /* opaque: owns the three tables below */
+typedef struct {
+  uint32_t n_points;         /* G */
+  const uint32_t *point_of;  /* DEVICE [V][8]: grid point of corner c of voxel v */
+  const uint32_t *offsets;   /* DEVICE [G+1]: CSR row starts into slots */
+  const uint32_t *slots;     /* DEVICE [8V]: slots[offsets[p] .. offsets[p+1]) = the corner slots 8v+c that are point p, ascending */
+} dvx_grid_tables;
+
+/* Builds the tables from the leaf set (code DEVICE [V], the dvx_octree_desc format, already validated by
+ * dvx_octree_create; V < 2^27).  One radix sort of 8V keys.  tables (HOST, may be NULL) receives borrowed pointers valid
+ * until dvx_grid_destroy.  Synchronises the stream.  V = 0 gives G = 0. */
+dvx_status dvx_grid_create(dvx_ctx *ctx, const uint64_t *code, uint32_t n_voxels, dvx_grid **out, dvx_grid_tables *tables);
+void dvx_grid_destroy(dvx_ctx *ctx, dvx_grid *grid);
+/* geo[v][c] = density[point_of[v][c]].  density DEVICE [G], geo DEVICE [V][8] (overwritten). */
+dvx_status dvx_grid_gather(dvx_ctx *ctx, const dvx_grid *grid, const float *density, float *geo);
+/* ddensity[p] = sum over the slots of p of dgeo (ascending slot order, no atomics: deterministic).  dgeo DEVICE [V][8],
+ * ddensity DEVICE [G] (overwritten, not accumulated). */
+dvx_status dvx_grid_reduce(dvx_ctx *ctx, const dvx_grid *grid, const float *dgeo, float *ddensity);
+
+typedef struct {
+  float lr, beta1, beta2, eps; /* lr > 0, 0 <= beta < 1, eps >= 0 */
+  uint32_t step;               /* t >= 1: the bias corrections 1 - beta^t are taken on the host in double */
+} dvx_adam;
+/* One fused optimizer step of the corner densities of one octree: g = dvx_grid_reduce(dgeo); Adam on (density, m, v)
+ * DEVICE [G]; the new densities are written back into every corner slot of geo DEVICE [V][8]; dgeo DEVICE [V][8] is
+ * ZEROED (ready for the next dvx_backward).  Does not synchronise. */
+dvx_status dvx_grid_adam_step(dvx_ctx *ctx, const dvx_grid *grid, const dvx_adam *hp, float *density, float *m, float *v,
+                              float *dgeo, float *geo);
+/* Elementwise Adam over n floats (the SH coefficients, the sky texture): p, m, v updated in place, g ZEROED.
+ * All four DEVICE, 16-byte aligned.  Does not synchronise. */
+dvx_status dvx_adam_step(dvx_ctx *ctx, const dvx_adam *hp, uint64_t n, float *p, float *m, float *v, float *g);
+
 #ifdef __cplusplus
 }
 #endif

@@ -22,7 +22,8 @@ FLAG_NAIVE = 2
 EXPORTS = ["dvx_create", "dvx_destroy", "dvx_octree_create", "dvx_octree_refresh_structure", "dvx_octree_destroy",
            "dvx_render", "dvx_backward", "dvx_backward_n", "dvx_frame_release", "dvx_debug_tile_list", "dvx_frame_counters",
            "dvx_frame_stage_ms", "dvx_last_error", "dvx_sort_pairs", "dvx_launch_count", "dvx_stage_ms_collect", "dvx_render_host",
-           "dvx_backward_host"]
+           "dvx_backward_host", "dvx_grid_create", "dvx_grid_destroy", "dvx_grid_gather", "dvx_grid_reduce",
+           "dvx_grid_adam_step", "dvx_adam_step"]
 
 
 class DvxError(RuntimeError):
@@ -56,6 +57,14 @@ class Image(C.Structure):
 
 class Grad(C.Structure):
     _fields_ = [("dgeo", C.c_void_p), ("dsh", C.c_void_p)]
+
+
+class GridTables(C.Structure):
+    _fields_ = [("n_points", C.c_uint32), ("point_of", C.c_void_p), ("offsets", C.c_void_p), ("slots", C.c_void_p)]
+
+
+class Adam(C.Structure):
+    _fields_ = [("lr", C.c_float), ("beta1", C.c_float), ("beta2", C.c_float), ("eps", C.c_float), ("step", C.c_uint32)]
 
 
 ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_size_t, C.c_void_p)
@@ -96,8 +105,16 @@ def load():
     lib.dvx_stage_ms_collect.argtypes = [P, C.POINTER(C.c_float), C.POINTER(C.c_uint32)]
     lib.dvx_render_host.argtypes = lib.dvx_render.argtypes
     lib.dvx_backward_host.argtypes = lib.dvx_backward.argtypes
+    lib.dvx_grid_create.argtypes = [P, P, C.c_uint32, C.POINTER(P), C.POINTER(GridTables)]
+    lib.dvx_grid_destroy.argtypes = [P, P]
+    lib.dvx_grid_destroy.restype = None
+    lib.dvx_grid_gather.argtypes = [P, P, P, P]
+    lib.dvx_grid_reduce.argtypes = [P, P, P, P]
+    lib.dvx_grid_adam_step.argtypes = [P, P, C.POINTER(Adam), P, P, P, P, P]
+    lib.dvx_adam_step.argtypes = [P, C.POINTER(Adam), C.c_uint64, P, P, P, P]
     for name in EXPORTS:
-        if name not in ("dvx_destroy", "dvx_octree_destroy", "dvx_frame_release", "dvx_last_error", "dvx_launch_count"):
+        if name not in ("dvx_destroy", "dvx_octree_destroy", "dvx_frame_release", "dvx_last_error", "dvx_launch_count",
+                        "dvx_grid_destroy"):
             getattr(lib, name).restype = C.c_int32
     lib.dvx_launch_count.restype = C.c_uint64
     _lib = lib
@@ -166,6 +183,17 @@ class Context:
     # ------------------------------------------------------------------ octrees
     def octree(self, code, geo, sh, center, side, sh_degree):
         return Octree(self, code, geo, sh, center, side, sh_degree)
+
+    # ------------------------------------------------------------------ row N2: grid points + optimizer
+    def grid(self, code):
+        """dvx_grid_create for a CUDA uint64 (stored as int64) code tensor [V]."""
+        return Grid(self, code)
+
+    def adam_step(self, p, m, v, g, lr, beta1, beta2, eps, step):
+        """dvx_adam_step over contiguous CUDA float32 tensors of equal size; g is zeroed."""
+        hp = Adam(lr, beta1, beta2, eps, step)
+        self.check(self.lib.dvx_adam_step(self.h, C.byref(hp), p.numel(), p.data_ptr(), m.data_ptr(), v.data_ptr(),
+                                          g.data_ptr()))
 
     # ------------------------------------------------------------------ render / backward
     def render(self, cam, static, actors=(), poses=None, box_half=None, k_samples=8, activation=0, t_stop=1e-4, flags=0,
@@ -238,6 +266,55 @@ class Octree:
     def close(self):
         if self.h and self.ctx.h:
             self.ctx.lib.dvx_octree_destroy(self.ctx.h, self.h)
+        self.h = None
+
+
+class Grid:
+    """Grid-point tables of one octree (dvx_grid_create): argument marshalling only."""
+
+    def __init__(self, ctx, code):
+        self.ctx = ctx
+        self.n_voxels = int(code.shape[0])
+        h = C.c_void_p()
+        self.tables = GridTables()
+        ctx.check(ctx.lib.dvx_grid_create(ctx.h, code.data_ptr() if self.n_voxels else None, self.n_voxels, C.byref(h),
+                                          C.byref(self.tables)))
+        self.h = h
+        self.n_points = int(self.tables.n_points)
+
+    def _view(self, ptr, n):
+        """The library allocated the table through this context's torch allocator: view that block, no copy."""
+        torch = self.ctx.torch
+        if n == 0:
+            return torch.empty(0, dtype=torch.int32, device=self.ctx.device)
+        block = self.ctx._blocks.get(ptr)
+        if block is None:
+            raise RuntimeError("grid tables are only viewable with torch_alloc=True")
+        return block.view(torch.int32)[:n]
+
+    def point_of(self):
+        return self._view(self.tables.point_of, self.n_voxels * 8).view(self.n_voxels, 8)
+
+    def offsets(self):
+        return self._view(self.tables.offsets, self.n_points + 1)
+
+    def slots(self):
+        return self._view(self.tables.slots, self.n_voxels * 8)
+
+    def gather(self, density, geo):
+        self.ctx.check(self.ctx.lib.dvx_grid_gather(self.ctx.h, self.h, density.data_ptr(), geo.data_ptr()))
+
+    def reduce(self, dgeo, ddensity):
+        self.ctx.check(self.ctx.lib.dvx_grid_reduce(self.ctx.h, self.h, dgeo.data_ptr(), ddensity.data_ptr()))
+
+    def adam_step(self, density, m, v, dgeo, geo, lr, beta1, beta2, eps, step):
+        hp = Adam(lr, beta1, beta2, eps, step)
+        self.ctx.check(self.ctx.lib.dvx_grid_adam_step(self.ctx.h, self.h, C.byref(hp), density.data_ptr(), m.data_ptr(),
+                                                       v.data_ptr(), dgeo.data_ptr(), geo.data_ptr()))
+
+    def close(self):
+        if self.h and self.ctx.h:
+            self.ctx.lib.dvx_grid_destroy(self.ctx.h, self.h)
         self.h = None
 
 

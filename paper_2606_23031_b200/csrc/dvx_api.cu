@@ -42,6 +42,11 @@ struct dvx_octree {
   size_t rank_bytes = 0;
 };
 
+struct dvx_grid {
+  uint32_t n_voxels = 0, n_points = 0;
+  uint32_t *point_of = nullptr, *offsets = nullptr, *slots = nullptr;
+};
+
 struct dvx_frame {
   FrameParams p;
   std::vector<TreeFrame> trees_h;
@@ -718,6 +723,139 @@ dvx_status dvx_sort_pairs(dvx_ctx *ctx, uint64_t *keys, uint32_t *vals, uint64_t
   }
   ctx_release(ctx, kb); ctx_release(ctx, vb); ctx_release(ctx, scr);
   return rc;
+}
+
+// ---- row N2: grid points + optimizer (dvx_grid.cu) ---------------------------------------------------------------------
+dvx_status dvx_grid_create(dvx_ctx *ctx, const uint64_t *code, uint32_t n_voxels, dvx_grid **out, dvx_grid_tables *tables) {
+  if (!ctx) return DVX_ERR_INVALID_ARG;
+  if (!out) return fail(ctx, DVX_ERR_INVALID_ARG, "dvx_grid_create: out is NULL");
+  *out = nullptr;
+  if (n_voxels && !code) return fail(ctx, DVX_ERR_INVALID_ARG, "dvx_grid_create: code is NULL");
+  if (n_voxels >= (1u << 27)) return fail(ctx, DVX_ERR_INVALID_ARG, "dvx_grid_create: V must be below 2^27");
+  cudaSetDevice(ctx->device);
+  dvx_grid *g = new dvx_grid();
+  g->n_voxels = n_voxels;
+  const uint64_t n = (uint64_t)n_voxels * 8;
+  dvx_status rc = DVX_OK;
+  if (n == 0) {
+    g->offsets = (uint32_t *)ctx_alloc(ctx, 256);
+    if (!g->offsets) rc = fail(ctx, DVX_ERR_OOM, "dvx_grid_create: allocator returned NULL");
+    else cudaMemsetAsync(g->offsets, 0, 4, ctx->st);
+  } else {
+    uint64_t *ka = (uint64_t *)ctx_alloc(ctx, n * 8), *kb = (uint64_t *)ctx_alloc(ctx, n * 8);
+    uint32_t *va = (uint32_t *)ctx_alloc(ctx, n * 4), *vb = (uint32_t *)ctx_alloc(ctx, n * 4);
+    uint32_t *excl = (uint32_t *)ctx_alloc(ctx, n * 4);
+    void *scr = ctx_alloc(ctx, dvx_sort_scratch_bytes(n));  // also ample for the scan of n flags
+    uint32_t *cnt = (uint32_t *)ctx_alloc(ctx, 256);
+    g->point_of = (uint32_t *)ctx_alloc(ctx, n * 4);
+    g->slots = (uint32_t *)ctx_alloc(ctx, n * 4);
+    if (!ka || !kb || !va || !vb || !excl || !scr || !cnt || !g->point_of || !g->slots) {
+      rc = fail(ctx, DVX_ERR_OOM, "dvx_grid_create: allocator returned NULL");
+    } else {
+      dvx_corner_keys_launch(code, n, ka, va, ctx->st);
+      const int which = dvx_sort_launch(ka, va, kb, vb, n, 51, scr, ctx->st);
+      const uint64_t *sk = which ? kb : ka;
+      const uint32_t *sv = which ? vb : va;
+      dvx_grid_heads_launch(sk, n, excl, ctx->st);
+      dvx_scan_u32_launch(excl, n, (uint32_t *)scr, ctx->st);
+      dvx_grid_count_launch(sk, excl, n, cnt, ctx->st);
+      uint32_t G = 0;
+      cudaError_t e = cudaMemcpyAsync(&G, cnt, 4, cudaMemcpyDeviceToHost, ctx->st);
+      if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->st);
+      if (e != cudaSuccess) rc = cuda_fail(ctx, e, "dvx_grid_create");
+      else {
+        g->n_points = G;
+        g->offsets = (uint32_t *)ctx_alloc(ctx, ((size_t)G + 1) * 4);
+        if (!g->offsets) rc = fail(ctx, DVX_ERR_OOM, "dvx_grid_create: allocator returned NULL");
+        else {
+          dvx_grid_tables_launch(sk, sv, excl, n, g->point_of, g->offsets, g->slots, ctx->st);
+          e = cudaStreamSynchronize(ctx->st);
+          if (e != cudaSuccess) rc = cuda_fail(ctx, e, "dvx_grid_create");
+        }
+      }
+    }
+    ctx_release(ctx, ka); ctx_release(ctx, kb); ctx_release(ctx, va); ctx_release(ctx, vb);
+    ctx_release(ctx, excl); ctx_release(ctx, scr); ctx_release(ctx, cnt);
+  }
+  if (rc != DVX_OK) {
+    dvx_grid_destroy(ctx, g);
+    return rc;
+  }
+  if (tables) {
+    tables->n_points = g->n_points;
+    tables->point_of = g->point_of;
+    tables->offsets = g->offsets;
+    tables->slots = g->slots;
+  }
+  *out = g;
+  return DVX_OK;
+}
+
+void dvx_grid_destroy(dvx_ctx *ctx, dvx_grid *grid) {
+  if (!ctx || !grid) return;
+  ctx_release(ctx, grid->point_of);
+  ctx_release(ctx, grid->offsets);
+  ctx_release(ctx, grid->slots);
+  delete grid;
+}
+
+dvx_status dvx_grid_gather(dvx_ctx *ctx, const dvx_grid *grid, const float *density, float *geo) {
+  if (!ctx) return DVX_ERR_INVALID_ARG;
+  if (!grid) return fail(ctx, DVX_ERR_INVALID_ARG, "dvx_grid_gather: grid is NULL");
+  if (grid->n_voxels == 0) return DVX_OK;
+  if (!density || !geo) return fail(ctx, DVX_ERR_INVALID_ARG, "dvx_grid_gather: NULL argument");
+  cudaSetDevice(ctx->device);
+  dvx_grid_gather_launch(density, grid->point_of, (uint64_t)grid->n_voxels * 8, geo, ctx->st);
+  cudaError_t e = cudaGetLastError();
+  return e == cudaSuccess ? DVX_OK : cuda_fail(ctx, e, "dvx_grid_gather");
+}
+
+dvx_status dvx_grid_reduce(dvx_ctx *ctx, const dvx_grid *grid, const float *dgeo, float *ddensity) {
+  if (!ctx) return DVX_ERR_INVALID_ARG;
+  if (!grid) return fail(ctx, DVX_ERR_INVALID_ARG, "dvx_grid_reduce: grid is NULL");
+  if (grid->n_points == 0) return DVX_OK;
+  if (!dgeo || !ddensity) return fail(ctx, DVX_ERR_INVALID_ARG, "dvx_grid_reduce: NULL argument");
+  cudaSetDevice(ctx->device);
+  dvx_grid_reduce_launch(dgeo, grid->offsets, grid->slots, grid->n_points, ddensity, ctx->st);
+  cudaError_t e = cudaGetLastError();
+  return e == cudaSuccess ? DVX_OK : cuda_fail(ctx, e, "dvx_grid_reduce");
+}
+
+static dvx_status check_adam(dvx_ctx *ctx, const dvx_adam *hp) {
+  if (!hp) return fail(ctx, DVX_ERR_INVALID_ARG, "adam: hyper-parameters are NULL");
+  if (!(hp->lr > 0.f) || !(hp->beta1 >= 0.f && hp->beta1 < 1.f) || !(hp->beta2 >= 0.f && hp->beta2 < 1.f) ||
+      !(hp->eps >= 0.f) || hp->step < 1)
+    return fail(ctx, DVX_ERR_INVALID_ARG, "adam: need lr > 0, 0 <= beta < 1, eps >= 0, step >= 1");
+  return DVX_OK;
+}
+
+dvx_status dvx_grid_adam_step(dvx_ctx *ctx, const dvx_grid *grid, const dvx_adam *hp, float *density, float *m, float *v,
+                              float *dgeo, float *geo) {
+  if (!ctx) return DVX_ERR_INVALID_ARG;
+  if (!grid) return fail(ctx, DVX_ERR_INVALID_ARG, "dvx_grid_adam_step: grid is NULL");
+  dvx_status rc = check_adam(ctx, hp);
+  if (rc != DVX_OK) return rc;
+  if (grid->n_points == 0) return DVX_OK;
+  if (!density || !m || !v || !dgeo || !geo) return fail(ctx, DVX_ERR_INVALID_ARG, "dvx_grid_adam_step: NULL argument");
+  cudaSetDevice(ctx->device);
+  dvx_grid_adam_launch(hp->lr, hp->beta1, hp->beta2, hp->eps, hp->step, grid->offsets, grid->slots, grid->n_points, density,
+                       m, v, dgeo, geo, ctx->st);
+  cudaError_t e = cudaGetLastError();
+  return e == cudaSuccess ? DVX_OK : cuda_fail(ctx, e, "dvx_grid_adam_step");
+}
+
+dvx_status dvx_adam_step(dvx_ctx *ctx, const dvx_adam *hp, uint64_t n, float *p, float *m, float *v, float *g) {
+  if (!ctx) return DVX_ERR_INVALID_ARG;
+  dvx_status rc = check_adam(ctx, hp);
+  if (rc != DVX_OK) return rc;
+  if (n == 0) return DVX_OK;
+  if (!p || !m || !v || !g) return fail(ctx, DVX_ERR_INVALID_ARG, "dvx_adam_step: NULL argument");
+  if (((uintptr_t)p | (uintptr_t)m | (uintptr_t)v | (uintptr_t)g) & 15)
+    return fail(ctx, DVX_ERR_INVALID_ARG, "dvx_adam_step: arrays must be 16-byte aligned");
+  cudaSetDevice(ctx->device);
+  dvx_adam_launch(hp->lr, hp->beta1, hp->beta2, hp->eps, hp->step, n, p, m, v, g, ctx->st);
+  cudaError_t e = cudaGetLastError();
+  return e == cudaSuccess ? DVX_OK : cuda_fail(ctx, e, "dvx_adam_step");
 }
 
 }  // extern "C"

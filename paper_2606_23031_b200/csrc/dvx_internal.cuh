@@ -110,6 +110,21 @@ void dvx_ranges_launch(const uint64_t *keys, uint64_t n, uint32_t rank_bits, uin
 void dvx_sh_backward_launch(const FrameParams &p, const TreeFrame *trees, const FrameVox *fvox, const ushort4 *pxrect,
                             const float *drgb, cudaStream_t st);
 
+// ---- dvx_grid.cu (row N2: shared grid-point densities, optimizer step)
+void dvx_corner_keys_launch(const uint64_t *code, uint64_t n_slots, uint64_t *keys, uint32_t *vals, cudaStream_t st);
+void dvx_grid_heads_launch(const uint64_t *skeys, uint64_t n, uint32_t *flag, cudaStream_t st);
+void dvx_grid_count_launch(const uint64_t *skeys, const uint32_t *excl, uint64_t n, uint32_t *n_points, cudaStream_t st);
+void dvx_grid_tables_launch(const uint64_t *skeys, const uint32_t *svals, const uint32_t *excl, uint64_t n,
+                            uint32_t *point_of, uint32_t *offsets, uint32_t *slots, cudaStream_t st);
+void dvx_grid_gather_launch(const float *density, const uint32_t *point_of, uint64_t n_slots, float *geo, cudaStream_t st);
+void dvx_grid_reduce_launch(const float *dgeo, const uint32_t *offsets, const uint32_t *slots, uint32_t n_points,
+                            float *ddensity, cudaStream_t st);
+void dvx_grid_adam_launch(float lr, float beta1, float beta2, float eps, uint32_t step, const uint32_t *offsets,
+                          const uint32_t *slots, uint32_t n_points, float *density, float *m, float *v, float *dgeo,
+                          float *geo, cudaStream_t st);
+void dvx_adam_launch(float lr, float beta1, float beta2, float eps, uint32_t step, uint64_t n, float *p, float *m, float *v,
+                     float *g, cudaStream_t st);
+
 // ---- dvx_composite_tile.cu (production) / dvx_composite_naive.cu (DVX_FLAG_NAIVE: one thread walks one ray, debug)
 void dvx_composite_tile_launch(const CompositeArgs &a, bool backward, cudaStream_t st);
 void dvx_composite_naive_launch(const CompositeArgs &a, bool backward, cudaStream_t st);
