@@ -222,6 +222,58 @@ def sort_throughput(ctx, n_pairs, scene, W, H, reps=5):
             "gb_per_s_moved": n * 12 * 2 * ((key_bits + 7) // 8) / ms / 1e6}
 
 
+def optimizer_step_stats(ctx, dev, grads, peak, reps=5):
+    """Widening row N2, reported beside the headline (not part of `value`): the optimizer step that follows the
+    rasterizer's backward - dvx_grid_adam_step on the corner densities of every octree and dvx_adam_step on their SH
+    coefficients - timed with CUDA events (median of reps) against its algorithmic bytes:
+      grid Adam : per grid point 4 (CSR offset) + 12 read + 12 written (density, m, v), per corner slot 4 (slot index)
+                  + 4 (gradient read) + 4 (gradient zeroed) + 4 (corner record written)  = 28 G + 16 * 8V
+      SH Adam   : 32 bytes per coefficient (g, p, m, v read; p, m, v, g = 0 written)"""
+    import torch
+    hp = dict(lr=0.01, beta1=0.9, beta2=0.99, eps=1e-15)
+    grids, build_ms = [], 0.0
+    for t in dev.trees:
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        grids.append(ctx.grid(t.code))
+        e1.record()
+        torch.cuda.synchronize()
+        build_ms += e0.elapsed_time(e1)
+    state = []
+    for t, g in zip(dev.trees, grids):
+        d = torch.zeros(g.n_points, device=ctx.device)
+        if t.n_voxels:
+            d[g.point_of().reshape(-1).long()] = t.geo.reshape(-1)   # the scene's corner record is consistent on shared corners
+        state.append((d, torch.zeros_like(d), torch.zeros_like(d), torch.zeros_like(t.sh), torch.zeros_like(t.sh)))
+    G_total = sum(g.n_points for g in grids)
+    V_total = sum(t.n_voxels for t in dev.trees)
+    n_sh = sum(t.sh.numel() for t in dev.trees)
+    t_grid, t_sh = [], []
+    for r in range(reps + 1):
+        for (dgeo, dsh) in grads:  # the kernels zero the gradients: refill so that every repetition does the same work
+            dgeo.fill_(1e-3); dsh.fill_(1e-3)
+        e = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+        torch.cuda.synchronize()
+        e[0].record()
+        for t, g, (d, m, v, ms, vs), (dgeo, dsh) in zip(dev.trees, grids, state, grads):
+            g.adam_step(d, m, v, dgeo, t.geo, step=r + 1, **hp)
+        e[1].record()
+        for t, (d, m, v, ms, vs), (dgeo, dsh) in zip(dev.trees, state, grads):
+            if t.n_voxels:
+                ctx.adam_step(t.sh, ms, vs, dsh, step=r + 1, **hp)
+        e[2].record()
+        torch.cuda.synchronize()
+        t_grid.append(e[0].elapsed_time(e[1])); t_sh.append(e[1].elapsed_time(e[2]))
+    ms_grid, ms_sh = float(np.median(t_grid[1:])), float(np.median(t_sh[1:]))
+    b_grid, b_sh = 28 * G_total + 16 * 8 * V_total, 32 * n_sh
+    for g in grids:
+        g.close()
+    return {"grid_points": G_total, "corner_slots": 8 * V_total, "sh_coefficients": n_sh, "grid_build_ms": build_ms,
+            "grid_adam": {"ms": ms_grid, "bytes": b_grid, "gb_per_s": b_grid / ms_grid / 1e6, "hbm_frac": b_grid / ms_grid / 1e6 / peak},
+            "sh_adam": {"ms": ms_sh, "bytes": b_sh, "gb_per_s": b_sh / ms_sh / 1e6, "hbm_frac": b_sh / ms_sh / 1e6 / peak},
+            "launches": 2 * len(dev.trees)}
+
+
 def run_dvx(args):
     import torch
     import torch.distributed as dist
@@ -330,6 +382,7 @@ def run_dvx(args):
     ms_e2e = timed(args.steps, host=True, bwd=not args.fwd_only)
     clocks = sampler.stop() if sampler else None
     sort_stats = sort_throughput(ctx, cnt["pairs"] // n_cams, scene, W, H) if rank == 0 else None
+    opt_stats = optimizer_step_stats(ctx, dev, grads, measured_peaks()[0]) if rank == 0 and not args.fwd_only else None
 
     if rank != 0:
         if world > 1:
@@ -381,7 +434,7 @@ def run_dvx(args):
                          "peak_source": "148 SMs x 128 fp32 lanes x %.0f MHz (nvidia-smi, under load)" % sm_mhz},
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": (0 if args.fwd_only else 12 * px_step),
                 "d2h_bytes_per_step": 20 * px_step, "ms_per_step": ms_e2e / args.steps},
-        "sort": sort_stats,
+        "sort": sort_stats, "n2_optimizer_step": opt_stats,
         "gpu_launches": launches, "clocks": clocks,
     }
     if not args.no_cpu_baseline and world == 1:

@@ -12,6 +12,10 @@ neighbouring voxels are one parameter, and it never names the optimizer.  Readin
        of that coordinate (x most significant within a 3-bit group, like the voxel code).
   R24  the optimizer is Adam (Kingma & Ba 2015, Algorithm 1) with bias correction, one step per call.
 
+Pins: tests/test_oracle_grid_pins.py P16-P21 (closed-form counts, a hand count, brute force with exact fractions,
+adjointness + torch autograd, torch.optim.Adam in float64).  R23 and R24 are readings the paper does not fix:
+PARITY UNPINNED against the authors' implementation for the choice of parameterisation and optimizer.
+
 Plain numpy, int64/uint64 for the tables and float64 for the arithmetic.  No blocking, no fusion: each function is
 the definition written out.
 """
