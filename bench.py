@@ -225,7 +225,7 @@ def sort_throughput(ctx, n_pairs, scene, W, H, reps=5):
 def optimizer_step_stats(ctx, dev, grads, peak, reps=5):
     """Widening row N2, reported beside the headline (not part of `value`): the optimizer step that follows the
     rasterizer's backward - dvx_grid_adam_step on the corner densities of every octree and dvx_adam_step on their SH
-    coefficients - timed with CUDA events (median of reps) against its algorithmic bytes:
+    coefficients, all octrees in one launch each (dvx_*_step_n) - timed with CUDA events (median of reps) against its algorithmic bytes:
       grid Adam : per grid point 4 (CSR offset) + 12 read + 12 written (density, m, v), per corner slot 4 (slot index)
                   + 4 (gradient read) + 4 (gradient zeroed) + 4 (corner record written)  = 28 G + 16 * 8V
       SH Adam   : 32 bytes per coefficient (g, p, m, v read; p, m, v, g = 0 written)"""
@@ -255,12 +255,11 @@ def optimizer_step_stats(ctx, dev, grads, peak, reps=5):
         e = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
         torch.cuda.synchronize()
         e[0].record()
-        for t, g, (d, m, v, ms, vs), (dgeo, dsh) in zip(dev.trees, grids, state, grads):
-            g.adam_step(d, m, v, dgeo, t.geo, step=r + 1, **hp)
+        ctx.grid_adam_step_n([(g, d, m, v, dgeo, t.geo) for t, g, (d, m, v, ms, vs), (dgeo, dsh) in
+                              zip(dev.trees, grids, state, grads)], step=r + 1, **hp)
         e[1].record()
-        for t, (d, m, v, ms, vs), (dgeo, dsh) in zip(dev.trees, state, grads):
-            if t.n_voxels:
-                ctx.adam_step(t.sh, ms, vs, dsh, step=r + 1, **hp)
+        ctx.adam_step_n([(t.sh, ms, vs, dsh) for t, (d, m, v, ms, vs), (dgeo, dsh) in zip(dev.trees, state, grads)],
+                        step=r + 1, **hp)
         e[2].record()
         torch.cuda.synchronize()
         t_grid.append(e[0].elapsed_time(e[1])); t_sh.append(e[1].elapsed_time(e[2]))
@@ -271,7 +270,7 @@ def optimizer_step_stats(ctx, dev, grads, peak, reps=5):
     return {"grid_points": G_total, "corner_slots": 8 * V_total, "sh_coefficients": n_sh, "grid_build_ms": build_ms,
             "grid_adam": {"ms": ms_grid, "bytes": b_grid, "gb_per_s": b_grid / ms_grid / 1e6, "hbm_frac": b_grid / ms_grid / 1e6 / peak},
             "sh_adam": {"ms": ms_sh, "bytes": b_sh, "gb_per_s": b_sh / ms_sh / 1e6, "hbm_frac": b_sh / ms_sh / 1e6 / peak},
-            "launches": 2 * len(dev.trees)}
+            "launches": 2 * ((len(dev.trees) + 31) // 32)}
 
 
 def run_dvx(args):

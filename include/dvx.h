@@ -216,8 +216,24 @@ typedef struct {
 dvx_status dvx_grid_adam_step(dvx_ctx *ctx, const dvx_grid *grid, const dvx_adam *hp, float *density, float *m, float *v,
                               float *dgeo, float *geo);
 /* Elementwise Adam over n floats (the SH coefficients, the sky texture): p, m, v updated in place, g ZEROED.
- * All four DEVICE, 16-byte aligned.  Does not synchronise. */
+ * All four DEVICE, 16-byte aligned.  n < 2^43.  Does not synchronise. */
 dvx_status dvx_adam_step(dvx_ctx *ctx, const dvx_adam *hp, uint64_t n, float *p, float *m, float *v, float *g);
+
+/* The same two steps for SEVERAL parameter arrays in one kernel launch per 32 arrays (the static octree and the actor
+ * octrees of a scene: an actor's few thousand parameters would otherwise cost a launch of their own).  items HOST [n],
+ * read before the call returns; the fields mean what the arguments of the single-array calls mean.  Entries with an
+ * empty grid / n = 0 are skipped.  Results are identical to n single-array calls. */
+typedef struct {
+  const dvx_grid *grid;
+  float *density, *m, *v; /* DEVICE [G] */
+  float *dgeo, *geo;      /* DEVICE [V][8] */
+} dvx_grid_adam_item;
+typedef struct {
+  uint64_t n;
+  float *p, *m, *v, *g; /* DEVICE [n], 16-byte aligned */
+} dvx_adam_item;
+dvx_status dvx_grid_adam_step_n(dvx_ctx *ctx, const dvx_adam *hp, uint32_t n, const dvx_grid_adam_item *items);
+dvx_status dvx_adam_step_n(dvx_ctx *ctx, const dvx_adam *hp, uint32_t n, const dvx_adam_item *items);
 
 #ifdef __cplusplus
 }

@@ -23,7 +23,7 @@ EXPORTS = ["dvx_create", "dvx_destroy", "dvx_octree_create", "dvx_octree_refresh
            "dvx_render", "dvx_backward", "dvx_backward_n", "dvx_frame_release", "dvx_debug_tile_list", "dvx_frame_counters",
            "dvx_frame_stage_ms", "dvx_last_error", "dvx_sort_pairs", "dvx_launch_count", "dvx_stage_ms_collect", "dvx_render_host",
            "dvx_backward_host", "dvx_grid_create", "dvx_grid_destroy", "dvx_grid_gather", "dvx_grid_reduce",
-           "dvx_grid_adam_step", "dvx_adam_step"]
+           "dvx_grid_adam_step", "dvx_adam_step", "dvx_grid_adam_step_n", "dvx_adam_step_n"]
 
 
 class DvxError(RuntimeError):
@@ -65,6 +65,15 @@ class GridTables(C.Structure):
 
 class Adam(C.Structure):
     _fields_ = [("lr", C.c_float), ("beta1", C.c_float), ("beta2", C.c_float), ("eps", C.c_float), ("step", C.c_uint32)]
+
+
+class GridAdamItem(C.Structure):
+    _fields_ = [("grid", C.c_void_p), ("density", C.c_void_p), ("m", C.c_void_p), ("v", C.c_void_p), ("dgeo", C.c_void_p),
+                ("geo", C.c_void_p)]
+
+
+class AdamItem(C.Structure):
+    _fields_ = [("n", C.c_uint64), ("p", C.c_void_p), ("m", C.c_void_p), ("v", C.c_void_p), ("g", C.c_void_p)]
 
 
 ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_size_t, C.c_void_p)
@@ -112,6 +121,8 @@ def load():
     lib.dvx_grid_reduce.argtypes = [P, P, P, P]
     lib.dvx_grid_adam_step.argtypes = [P, P, C.POINTER(Adam), P, P, P, P, P]
     lib.dvx_adam_step.argtypes = [P, C.POINTER(Adam), C.c_uint64, P, P, P, P]
+    lib.dvx_grid_adam_step_n.argtypes = [P, C.POINTER(Adam), C.c_uint32, C.POINTER(GridAdamItem)]
+    lib.dvx_adam_step_n.argtypes = [P, C.POINTER(Adam), C.c_uint32, C.POINTER(AdamItem)]
     for name in EXPORTS:
         if name not in ("dvx_destroy", "dvx_octree_destroy", "dvx_frame_release", "dvx_last_error", "dvx_launch_count",
                         "dvx_grid_destroy"):
@@ -194,6 +205,19 @@ class Context:
         hp = Adam(lr, beta1, beta2, eps, step)
         self.check(self.lib.dvx_adam_step(self.h, C.byref(hp), p.numel(), p.data_ptr(), m.data_ptr(), v.data_ptr(),
                                           g.data_ptr()))
+
+    def grid_adam_step_n(self, items, lr, beta1, beta2, eps, step):
+        """dvx_grid_adam_step_n: items = [(Grid, density, m, v, dgeo, geo), ...], all octrees in one launch."""
+        hp = Adam(lr, beta1, beta2, eps, step)
+        arr = (GridAdamItem * max(len(items), 1))(*[GridAdamItem(g.h, *[t.data_ptr() for t in ts]) for g, *ts in items])
+        self.check(self.lib.dvx_grid_adam_step_n(self.h, C.byref(hp), len(items), arr))
+
+    def adam_step_n(self, items, lr, beta1, beta2, eps, step):
+        """dvx_adam_step_n: items = [(p, m, v, g), ...] contiguous CUDA float32 tensors."""
+        hp = Adam(lr, beta1, beta2, eps, step)
+        arr = (AdamItem * max(len(items), 1))(*[AdamItem(p.numel(), p.data_ptr(), m.data_ptr(), v.data_ptr(), g.data_ptr())
+                                                for p, m, v, g in items])
+        self.check(self.lib.dvx_adam_step_n(self.h, C.byref(hp), len(items), arr))
 
     # ------------------------------------------------------------------ render / backward
     def render(self, cam, static, actors=(), poses=None, box_half=None, k_samples=8, activation=0, t_stop=1e-4, flags=0,

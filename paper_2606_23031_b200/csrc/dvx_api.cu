@@ -829,33 +829,60 @@ static dvx_status check_adam(dvx_ctx *ctx, const dvx_adam *hp) {
   return DVX_OK;
 }
 
-dvx_status dvx_grid_adam_step(dvx_ctx *ctx, const dvx_grid *grid, const dvx_adam *hp, float *density, float *m, float *v,
-                              float *dgeo, float *geo) {
+dvx_status dvx_grid_adam_step_n(dvx_ctx *ctx, const dvx_adam *hp, uint32_t n, const dvx_grid_adam_item *items) {
   if (!ctx) return DVX_ERR_INVALID_ARG;
-  if (!grid) return fail(ctx, DVX_ERR_INVALID_ARG, "dvx_grid_adam_step: grid is NULL");
   dvx_status rc = check_adam(ctx, hp);
   if (rc != DVX_OK) return rc;
-  if (grid->n_points == 0) return DVX_OK;
-  if (!density || !m || !v || !dgeo || !geo) return fail(ctx, DVX_ERR_INVALID_ARG, "dvx_grid_adam_step: NULL argument");
+  if (n && !items) return fail(ctx, DVX_ERR_INVALID_ARG, "dvx_grid_adam_step_n: items is NULL");
+  std::vector<DvxGridAdamItem> v;
+  v.reserve(n);
+  for (uint32_t i = 0; i < n; ++i) {
+    const dvx_grid_adam_item &it = items[i];
+    if (!it.grid) return fail(ctx, DVX_ERR_INVALID_ARG, "dvx_grid_adam_step: grid is NULL");
+    if (it.grid->n_points == 0) continue;
+    if (!it.density || !it.m || !it.v || !it.dgeo || !it.geo)
+      return fail(ctx, DVX_ERR_INVALID_ARG, "dvx_grid_adam_step: NULL argument");
+    v.push_back({it.grid->offsets, it.grid->slots, it.grid->n_points, it.density, it.m, it.v, it.dgeo, it.geo});
+  }
+  if (v.empty()) return DVX_OK;
   cudaSetDevice(ctx->device);
-  dvx_grid_adam_launch(hp->lr, hp->beta1, hp->beta2, hp->eps, hp->step, grid->offsets, grid->slots, grid->n_points, density,
-                       m, v, dgeo, geo, ctx->st);
+  dvx_grid_adam_launch(hp->lr, hp->beta1, hp->beta2, hp->eps, hp->step, (uint32_t)v.size(), v.data(), ctx->st);
   cudaError_t e = cudaGetLastError();
   return e == cudaSuccess ? DVX_OK : cuda_fail(ctx, e, "dvx_grid_adam_step");
 }
 
-dvx_status dvx_adam_step(dvx_ctx *ctx, const dvx_adam *hp, uint64_t n, float *p, float *m, float *v, float *g) {
+dvx_status dvx_grid_adam_step(dvx_ctx *ctx, const dvx_grid *grid, const dvx_adam *hp, float *density, float *m, float *v,
+                              float *dgeo, float *geo) {
+  const dvx_grid_adam_item it = {grid, density, m, v, dgeo, geo};
+  return dvx_grid_adam_step_n(ctx, hp, 1, &it);
+}
+
+dvx_status dvx_adam_step_n(dvx_ctx *ctx, const dvx_adam *hp, uint32_t n, const dvx_adam_item *items) {
   if (!ctx) return DVX_ERR_INVALID_ARG;
   dvx_status rc = check_adam(ctx, hp);
   if (rc != DVX_OK) return rc;
-  if (n == 0) return DVX_OK;
-  if (!p || !m || !v || !g) return fail(ctx, DVX_ERR_INVALID_ARG, "dvx_adam_step: NULL argument");
-  if (((uintptr_t)p | (uintptr_t)m | (uintptr_t)v | (uintptr_t)g) & 15)
-    return fail(ctx, DVX_ERR_INVALID_ARG, "dvx_adam_step: arrays must be 16-byte aligned");
+  if (n && !items) return fail(ctx, DVX_ERR_INVALID_ARG, "dvx_adam_step_n: items is NULL");
+  std::vector<DvxAdamItem> v;
+  v.reserve(n);
+  for (uint32_t i = 0; i < n; ++i) {
+    const dvx_adam_item &it = items[i];
+    if (it.n == 0) continue;
+    if (it.n >= (1ull << 43)) return fail(ctx, DVX_ERR_INVALID_ARG, "dvx_adam_step: n must be below 2^43");
+    if (!it.p || !it.m || !it.v || !it.g) return fail(ctx, DVX_ERR_INVALID_ARG, "dvx_adam_step: NULL argument");
+    if (((uintptr_t)it.p | (uintptr_t)it.m | (uintptr_t)it.v | (uintptr_t)it.g) & 15)
+      return fail(ctx, DVX_ERR_INVALID_ARG, "dvx_adam_step: arrays must be 16-byte aligned");
+    v.push_back({it.n, it.p, it.m, it.v, it.g});
+  }
+  if (v.empty()) return DVX_OK;
   cudaSetDevice(ctx->device);
-  dvx_adam_launch(hp->lr, hp->beta1, hp->beta2, hp->eps, hp->step, n, p, m, v, g, ctx->st);
+  dvx_adam_launch(hp->lr, hp->beta1, hp->beta2, hp->eps, hp->step, (uint32_t)v.size(), v.data(), ctx->st);
   cudaError_t e = cudaGetLastError();
   return e == cudaSuccess ? DVX_OK : cuda_fail(ctx, e, "dvx_adam_step");
+}
+
+dvx_status dvx_adam_step(dvx_ctx *ctx, const dvx_adam *hp, uint64_t n, float *p, float *m, float *v, float *g) {
+  const dvx_adam_item it = {n, p, m, v, g};
+  return dvx_adam_step_n(ctx, hp, 1, &it);
 }
 
 }  // extern "C"

@@ -6,7 +6,7 @@
 // its corner slots, CSR).  They fall out of ONE radix sort of the 8V corner keys (51-bit Morton key of the corner's
 // level-16 lattice coordinate): runs of equal keys are the grid points, and the sorted payload is the CSR slot list.
 //
-// The optimizer step (reading R24: Adam) is one kernel per parameter array and is purely HBM-bound:
+// The optimizer step (reading R24: Adam) is one kernel per parameter KIND (all octrees of a scene in one launch), HBM-bound:
 //   grid_adam_kernel : thread = grid point.  GATHERS its <= 8 corner gradients (fixed order, so the step is
 //                      deterministic and needs no atomics), Adam, writes the new density back into every corner slot of
 //                      the [V][8] record the next forward reads, and zeroes the gradients it consumed.
@@ -15,6 +15,8 @@
 // summing per grid point here, once per step, replaces the scatter-add "fused into the backward atomics" that SURVEY.md
 // sketches: 8 scalar reductions per run would quadruple the reduction instructions of a kernel that is issue-bound.
 #include "dvx_internal.cuh"
+
+#include <cstring>
 
 namespace {
 
@@ -122,30 +124,48 @@ __device__ __forceinline__ void adam_update(const AdamConst &h, float g, float &
   p -= h.step_size * (m / denom);
 }
 
-__global__ void __launch_bounds__(GRID_THREADS) grid_adam_kernel(AdamConst h, const uint32_t *__restrict__ offsets,
-                                                                 const uint32_t *__restrict__ slots, uint32_t n_points,
-                                                                 float *__restrict__ density, float *__restrict__ m,
-                                                                 float *__restrict__ v, float *__restrict__ dgeo,
-                                                                 float *__restrict__ geo) {
-  const uint32_t p = blockIdx.x * GRID_THREADS + threadIdx.x;
-  if (p >= n_points) return;
-  const uint32_t b = offsets[p], e = offsets[p + 1];
+// One launch serves up to ADAM_BATCH parameter arrays (the static octree and the actor octrees of a scene): a block finds
+// its array by a short scan of the block prefix held in the kernel parameters.  Ten launches of a few hundred blocks each
+// cost ten latency chains (9 us apiece measured); batched they hide inside the static octree's launch.
+constexpr int ADAM_BATCH = 32;
+
+struct GridAdamBatch {
+  uint32_t block_start[ADAM_BATCH + 1];
+  const uint32_t *offsets[ADAM_BATCH];
+  const uint32_t *slots[ADAM_BATCH];
+  float *density[ADAM_BATCH], *m[ADAM_BATCH], *v[ADAM_BATCH], *dgeo[ADAM_BATCH], *geo[ADAM_BATCH];
+  uint32_t n_points[ADAM_BATCH];
+  int n;
+};
+
+#ifndef DVX_GA_MINB
+#define DVX_GA_MINB 8  // 32 registers, 64 warps per SM: the kernel waits on scattered 4-byte accesses
+#endif
+__global__ void __launch_bounds__(GRID_THREADS, DVX_GA_MINB) grid_adam_kernel(const __grid_constant__ AdamConst h,
+                                                                 const __grid_constant__ GridAdamBatch B) {
+  int e = 0;
+  while (e + 1 < B.n && blockIdx.x >= B.block_start[e + 1]) ++e;
+  const uint32_t p = (blockIdx.x - B.block_start[e]) * GRID_THREADS + threadIdx.x;
+  if (p >= B.n_points[e]) return;
+  const uint32_t *__restrict__ offsets = B.offsets[e];
+  const uint32_t *__restrict__ slots = B.slots[e];
+  float *__restrict__ dgeo = B.dgeo[e];
+  float *__restrict__ geo = B.geo[e];
+  const uint32_t b = offsets[p], end = offsets[p + 1];
   uint32_t sl[8];
   float gs[8];
 #pragma unroll
-  for (int i = 0; i < 8; ++i) {
-    sl[i] = b + i < e ? __ldg(slots + b + i) : 0xFFFFFFFFu;
-  }
+  for (int i = 0; i < 8; ++i) sl[i] = b + i < end ? __ldg(slots + b + i) : 0xFFFFFFFFu;
 #pragma unroll
   for (int i = 0; i < 8; ++i) gs[i] = sl[i] != 0xFFFFFFFFu ? dgeo[sl[i]] : 0.f;  // all eight loads in flight together
   float g = 0.f;
 #pragma unroll
   for (int i = 0; i < 8; ++i) g += gs[i];  // ascending slot order: deterministic
-  float pv = density[p], mv = m[p], vv = v[p];
+  float pv = B.density[e][p], mv = B.m[e][p], vv = B.v[e][p];
   adam_update(h, g, pv, mv, vv);
-  density[p] = pv;
-  m[p] = mv;
-  v[p] = vv;
+  B.density[e][p] = pv;
+  B.m[e][p] = mv;
+  B.v[e][p] = vv;
 #pragma unroll
   for (int i = 0; i < 8; ++i)
     if (sl[i] != 0xFFFFFFFFu) {
@@ -154,34 +174,63 @@ __global__ void __launch_bounds__(GRID_THREADS) grid_adam_kernel(AdamConst h, co
     }
 }
 
-// elementwise Adam over n floats, float4 lanes + scalar tail; zeroes the gradient
-__global__ void __launch_bounds__(GRID_THREADS) adam_kernel(AdamConst h, uint64_t n, float *__restrict__ p,
-                                                            float *__restrict__ m, float *__restrict__ v,
-                                                            float *__restrict__ g) {
-  const uint64_t n4 = n >> 2;
-  const uint64_t stride = (uint64_t)gridDim.x * GRID_THREADS;
-  for (uint64_t i = (uint64_t)blockIdx.x * GRID_THREADS + threadIdx.x; i < n4; i += stride) {
-    float4 gp = reinterpret_cast<float4 *>(g)[i];
-    float4 pp = reinterpret_cast<float4 *>(p)[i];
-    float4 mp = reinterpret_cast<float4 *>(m)[i];
-    float4 vp = reinterpret_cast<float4 *>(v)[i];
-    adam_update(h, gp.x, pp.x, mp.x, vp.x);
-    adam_update(h, gp.y, pp.y, mp.y, vp.y);
-    adam_update(h, gp.z, pp.z, mp.z, vp.z);
-    adam_update(h, gp.w, pp.w, mp.w, vp.w);
-    reinterpret_cast<float4 *>(p)[i] = pp;
-    reinterpret_cast<float4 *>(m)[i] = mp;
-    reinterpret_cast<float4 *>(v)[i] = vp;
-    reinterpret_cast<float4 *>(g)[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+// elementwise Adam: a block owns ADAM_CHUNK consecutive floats of one array (4 float4 per thread, 16 loads in flight),
+// the last block of an array also its scalar tail; zeroes the gradient
+constexpr int ADAM_V4 = 4;
+constexpr int ADAM_CHUNK = GRID_THREADS * ADAM_V4 * 4;  // 4096 floats
+
+struct AdamBatch {
+  uint32_t block_start[ADAM_BATCH + 1];
+  float *p[ADAM_BATCH], *m[ADAM_BATCH], *v[ADAM_BATCH], *g[ADAM_BATCH];
+  uint64_t n[ADAM_BATCH];
+  int count;
+};
+
+__global__ void __launch_bounds__(GRID_THREADS) adam_kernel(const __grid_constant__ AdamConst h,
+                                                            const __grid_constant__ AdamBatch B) {
+  int e = 0;
+  while (e + 1 < B.count && blockIdx.x >= B.block_start[e + 1]) ++e;
+  const uint64_t n = B.n[e], n4 = n >> 2;
+  float4 *__restrict__ p4 = reinterpret_cast<float4 *>(B.p[e]);
+  float4 *__restrict__ m4 = reinterpret_cast<float4 *>(B.m[e]);
+  float4 *__restrict__ v4 = reinterpret_cast<float4 *>(B.v[e]);
+  float4 *__restrict__ g4 = reinterpret_cast<float4 *>(B.g[e]);
+  const uint64_t base = (uint64_t)(blockIdx.x - B.block_start[e]) * (GRID_THREADS * ADAM_V4) + threadIdx.x;
+  float4 gp[ADAM_V4], pp[ADAM_V4], mp[ADAM_V4], vp[ADAM_V4];
+#pragma unroll
+  for (int k = 0; k < ADAM_V4; ++k) {
+    const uint64_t i = base + (uint64_t)k * GRID_THREADS;
+    if (i < n4) {
+      gp[k] = g4[i];
+      pp[k] = p4[i];
+      mp[k] = m4[i];
+      vp[k] = v4[i];
+    }
   }
-  const uint64_t t = (n4 << 2) + (uint64_t)blockIdx.x * GRID_THREADS + threadIdx.x;
-  if (t < n) {
-    float pv = p[t], mv = m[t], vv = v[t];
-    adam_update(h, g[t], pv, mv, vv);
-    p[t] = pv;
-    m[t] = mv;
-    v[t] = vv;
-    g[t] = 0.f;
+#pragma unroll
+  for (int k = 0; k < ADAM_V4; ++k) {
+    const uint64_t i = base + (uint64_t)k * GRID_THREADS;
+    if (i < n4) {
+      adam_update(h, gp[k].x, pp[k].x, mp[k].x, vp[k].x);
+      adam_update(h, gp[k].y, pp[k].y, mp[k].y, vp[k].y);
+      adam_update(h, gp[k].z, pp[k].z, mp[k].z, vp[k].z);
+      adam_update(h, gp[k].w, pp[k].w, mp[k].w, vp[k].w);
+      p4[i] = pp[k];
+      m4[i] = mp[k];
+      v4[i] = vp[k];
+      g4[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+    }
+  }
+  if (blockIdx.x + 1 == B.block_start[e + 1]) {  // scalar tail (n mod 4 floats) by the array's last block
+    const uint64_t t = (n4 << 2) + threadIdx.x;
+    if (t < n) {
+      float pv = B.p[e][t], mv = B.m[e][t], vv = B.v[e][t];
+      adam_update(h, B.g[e][t], pv, mv, vv);
+      B.p[e][t] = pv;
+      B.m[e][t] = mv;
+      B.v[e][t] = vv;
+      B.g[e][t] = 0.f;
+    }
   }
 }
 
@@ -227,20 +276,49 @@ void dvx_grid_reduce_launch(const float *dgeo, const uint32_t *offsets, const ui
   DVX_COUNT_LAUNCH(1);
   grid_reduce_kernel<<<blocks_for(n_points), GRID_THREADS, 0, st>>>(dgeo, offsets, slots, n_points, ddensity);
 }
-void dvx_grid_adam_launch(float lr, float beta1, float beta2, float eps, uint32_t step, const uint32_t *offsets,
-                          const uint32_t *slots, uint32_t n_points, float *density, float *m, float *v, float *dgeo,
-                          float *geo, cudaStream_t st) {
-  DVX_COUNT_LAUNCH(1);
-  grid_adam_kernel<<<blocks_for(n_points), GRID_THREADS, 0, st>>>(adam_const(lr, beta1, beta2, eps, step), offsets, slots,
-                                                                 n_points, density, m, v, dgeo, geo);
+void dvx_grid_adam_launch(float lr, float beta1, float beta2, float eps, uint32_t step, uint32_t n,
+                          const DvxGridAdamItem *items, cudaStream_t st) {
+  const AdamConst h = adam_const(lr, beta1, beta2, eps, step);
+  for (uint32_t at = 0; at < n;) {
+    GridAdamBatch B;
+    memset(&B, 0, sizeof(B));
+    uint32_t blocks = 0;
+    while (at < n && B.n < ADAM_BATCH) {
+      const DvxGridAdamItem &it = items[at++];
+      if (it.n_points == 0) continue;
+      const int e = B.n++;
+      B.block_start[e] = blocks;
+      blocks += blocks_for(it.n_points);
+      B.offsets[e] = it.offsets; B.slots[e] = it.slots; B.n_points[e] = it.n_points;
+      B.density[e] = it.density; B.m[e] = it.m; B.v[e] = it.v; B.dgeo[e] = it.dgeo; B.geo[e] = it.geo;
+    }
+    if (B.n == 0) continue;
+    B.block_start[B.n] = blocks;
+    DVX_COUNT_LAUNCH(1);
+    grid_adam_kernel<<<blocks, GRID_THREADS, 0, st>>>(h, B);
+  }
 }
-void dvx_adam_launch(float lr, float beta1, float beta2, float eps, uint32_t step, uint64_t n, float *p, float *m, float *v,
-                     float *g, cudaStream_t st) {
-  // grid-stride over float4 lanes; 148 SMs x 8 resident blocks of 256 threads
-  uint64_t want = ((n >> 2) + GRID_THREADS - 1) / GRID_THREADS;
-  if (want < 1) want = 1;
-  const uint64_t cap = 148ull * 8ull * 4ull;
-  DVX_COUNT_LAUNCH(1);
-  adam_kernel<<<(unsigned)(want < cap ? want : cap), GRID_THREADS, 0, st>>>(adam_const(lr, beta1, beta2, eps, step), n, p, m,
-                                                                           v, g);
+void dvx_adam_launch(float lr, float beta1, float beta2, float eps, uint32_t step, uint32_t n, const DvxAdamItem *items,
+                     cudaStream_t st) {
+  const AdamConst h = adam_const(lr, beta1, beta2, eps, step);
+  for (uint32_t at = 0; at < n;) {
+    AdamBatch B;
+    memset(&B, 0, sizeof(B));
+    uint64_t blocks = 0;
+    while (at < n && B.count < ADAM_BATCH) {
+      const DvxAdamItem &it = items[at];
+      if (it.n == 0) { ++at; continue; }
+      const uint64_t nb = (it.n + ADAM_CHUNK - 1) / ADAM_CHUNK;
+      if (blocks + nb > 0x7FFFFFFFull) break;  // grid.x limit: the rest goes into the next launch
+      ++at;
+      const int e = B.count++;
+      B.block_start[e] = (uint32_t)blocks;
+      blocks += nb;
+      B.p[e] = it.p; B.m[e] = it.m; B.v[e] = it.v; B.g[e] = it.g; B.n[e] = it.n;
+    }
+    if (B.count == 0) break;  // a single array beyond 2^31 blocks (2^43 floats) is rejected by the caller
+    B.block_start[B.count] = (uint32_t)blocks;
+    DVX_COUNT_LAUNCH(1);
+    adam_kernel<<<(unsigned)blocks, GRID_THREADS, 0, st>>>(h, B);
+  }
 }

@@ -119,11 +119,20 @@ void dvx_grid_tables_launch(const uint64_t *skeys, const uint32_t *svals, const 
 void dvx_grid_gather_launch(const float *density, const uint32_t *point_of, uint64_t n_slots, float *geo, cudaStream_t st);
 void dvx_grid_reduce_launch(const float *dgeo, const uint32_t *offsets, const uint32_t *slots, uint32_t n_points,
                             float *ddensity, cudaStream_t st);
-void dvx_grid_adam_launch(float lr, float beta1, float beta2, float eps, uint32_t step, const uint32_t *offsets,
-                          const uint32_t *slots, uint32_t n_points, float *density, float *m, float *v, float *dgeo,
-                          float *geo, cudaStream_t st);
-void dvx_adam_launch(float lr, float beta1, float beta2, float eps, uint32_t step, uint64_t n, float *p, float *m, float *v,
-                     float *g, cudaStream_t st);
+struct DvxGridAdamItem {
+  const uint32_t *offsets, *slots;
+  uint32_t n_points;
+  float *density, *m, *v, *dgeo, *geo;
+};
+struct DvxAdamItem {
+  uint64_t n;
+  float *p, *m, *v, *g;
+};
+// all items in as few launches as possible (32 arrays per launch)
+void dvx_grid_adam_launch(float lr, float beta1, float beta2, float eps, uint32_t step, uint32_t n,
+                          const DvxGridAdamItem *items, cudaStream_t st);
+void dvx_adam_launch(float lr, float beta1, float beta2, float eps, uint32_t step, uint32_t n, const DvxAdamItem *items,
+                     cudaStream_t st);
 
 // ---- dvx_composite_tile.cu (production) / dvx_composite_naive.cu (DVX_FLAG_NAIVE: one thread walks one ray, debug)
 void dvx_composite_tile_launch(const CompositeArgs &a, bool backward, cudaStream_t st);

@@ -159,6 +159,43 @@ def test_adam_step_elementwise(ctx, n):
     _close(p.cpu().numpy(), rp, 2e-7, step_size * dm / denom + 1e-6 * np.abs(rp - p_h), "p")
 
 
+def test_batched_steps_equal_single_calls(ctx, config1):
+    """dvx_grid_adam_step_n / dvx_adam_step_n over all octrees of config 1 (one launch) == one call per octree, bit for bit;
+    empty arrays in the batch are skipped."""
+    import torch
+    rs = np.random.RandomState(9)
+    hp = dict(HP, step=2)
+    grids, single, batch = [], [], []
+    for tree in config1.octrees:
+        grid = ctx.grid(_dev_code(tree.code))
+        V, Gn = tree.n_voxels, grid.n_points
+        arrs = [rs.randn(Gn), rs.randn(Gn) * 0.1, rs.rand(Gn) * 0.01, rs.randn(V, 8), np.zeros((V, 8))]
+        grids.append(grid)
+        single.append([torch.from_numpy(a.astype(np.float32)).cuda() for a in arrs])
+        batch.append([t.clone() for t in single[-1]])
+    empty = ctx.grid(torch.zeros(0, dtype=torch.int64, device="cuda"))
+    z = torch.zeros(4, device="cuda")
+    for grid, ts in zip(grids, single):
+        grid.adam_step(*ts, **hp)
+    ctx.grid_adam_step_n([(grids[0], *batch[0]), (empty, z, z, z, z, z)] + [(g, *ts) for g, ts in zip(grids[1:], batch[1:])], **hp)
+    torch.cuda.synchronize()
+    for a, b in zip(single, batch):
+        for x, y in zip(a, b):
+            assert torch.equal(x, y)
+    sizes = [5, 4096, 0, 4097, 12289, 3]
+    one = [[torch.from_numpy(rs.randn(n).astype(np.float32)).cuda().abs() * s for s in (1, 0.1, 0.01, 1)] for n in sizes]
+    many = [[t.clone() for t in ts] for ts in one]
+    for ts in one:
+        ctx.adam_step(*ts, **hp)
+    ctx.adam_step_n([tuple(ts) for ts in many], **hp)
+    torch.cuda.synchronize()
+    for a, b in zip(one, many):
+        for x, y in zip(a, b):
+            assert torch.equal(x, y)
+    for g in grids + [empty]:
+        g.close()
+
+
 def test_adam_argument_errors(ctx):
     import torch
     import paper_2606_23031_b200 as dvx
