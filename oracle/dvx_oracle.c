@@ -82,6 +82,21 @@ typedef struct orc_sky_s {
   double *dtex;      /* [H][W][3] accumulated (+=), or NULL */
 } orc_sky;
 
+/* O12 (widening row N3, "substituting the standard RGB color rendering step with a high-dimensional feature
+ * accumulation pass", and the "feature volume fuser" of :241).  Reading R25: with w_j = T_j alpha_j the compositing
+ * weight of the j-th composited sub-segment of a ray (the same weights that blend the colour, :107),
+ *   render:  F[p][c]        = sum_j w_j feat[tree_j][v_j][c]                  (no view dependence, no sky term)
+ *   fuse:    num[t][v][c]  += sum over rays p, sub-segments j of (t, v):  w_j img[p][c],   wsum[t][v] += the same sum of w_j
+ * so that num/wsum is the weight-averaged 2-D feature seen by the voxel, and fuse is the transpose of render. */
+typedef struct {
+  uint32_t n_channels;
+  const double *const *feat; /* [n_trees] -> [V_t][C], or NULL (no feature image) */
+  double *out;               /* [H][W][C] (untouched where masked out), or NULL */
+  const double *img;         /* [H][W][C] 2-D features to fuse, or NULL */
+  double *const *num;        /* [n_trees] -> [V_t][C], accumulated (+=) */
+  double *const *wsum;       /* [n_trees] -> [V_t],    accumulated (+=) */
+} orc_feat;
+
 static const double ORC_PI = 3.14159265358979323846;
 
 /* texel indices (into [H][W]) and weights of the bilinear footprint of world direction d */
@@ -262,6 +277,7 @@ typedef struct {
   const orc_camera *cam;
   const orc_opts *opt;
   const struct orc_sky_s *sky; /* NULL = no sky (Eq. 2 with C_sky = 0) */
+  const orc_feat *fx;          /* NULL = no feature pass (O12) */
 } scene_t;
 
 /* O3: the allowed intervals.  Sort hit actors by (tau_in, index); tau_curr never moves backwards (R2). */
@@ -481,6 +497,27 @@ static void render_ray(const scene_t *sc, int u, int v, const uint32_t *const *c
   out5[0] = C[0]; out5[1] = C[1]; out5[2] = C[2]; out5[3] = D; out5[4] = 1.0 - T;
   if (nout) memcpy(nout, Nacc, sizeof Nacc);
   if (n_used) *n_used = (uint32_t)used;
+  if (sc->fx) { /* O12: the tape holds T before each composited sub-segment and its tau */
+    const orc_feat *fx = sc->fx;
+    const size_t C = fx->n_channels, p = (size_t)v * sc->cam->width + (size_t)u;
+    if (fx->feat && fx->out)
+      for (size_t c = 0; c < C; ++c) fx->out[p * C + c] = 0.0;
+    for (size_t n = 0; n < used; ++n) {
+      const seg_t *sg = &w->segs.s[n];
+      const double wgt = w->Tb[n] * (1.0 - exp(-w->tau[n]));
+      if (fx->feat && fx->out)
+        for (size_t c = 0; c < C; ++c) fx->out[p * C + c] += wgt * fx->feat[sg->tree][(size_t)sg->v * C + c];
+      if (fx->img) {
+        for (size_t c = 0; c < C; ++c) {
+          const double val = wgt * fx->img[p * C + c];
+#pragma omp atomic
+          fx->num[sg->tree][(size_t)sg->v * C + c] += val;
+        }
+#pragma omp atomic
+        fx->wsum[sg->tree][sg->v] += wgt;
+      }
+    }
+  }
   if (!g5 || !grads) return;
   /* O9: reverse sweep over the tape.  Adjoint of T after the last voxel comes from alpha = 1 - T and from Eq. 2. */
   double gT = -g5[4];
@@ -664,14 +701,14 @@ static void build_tilelists(const scene_t *sc, tilelists *tl) {
  * doubles (untouched where masked out).  When g_rgb != NULL also runs O9 and accumulates into grads[n_trees]
  * (g_depth / g_alpha may be NULL = zero).  n_used (optional, [H][W]) = sub-segments composited per ray.
  * Returns 0, or -1 on invalid arguments. */
-int orc_render_full(const orc_camera *cam, int n_trees, const orc_octree *trees, const double *poses, const double *half,
-                    const orc_opts *opt, const uint8_t *mask, double *rgb, double *depth, double *alpha,
-                    const double *g_rgb, const double *g_depth, const double *g_alpha, orc_grad *grads,
-                    uint32_t *n_used, const orc_sky *sky, double *normal /* [H][W][3] or NULL */,
-                    const double *g_normal /* [H][W][3] or NULL */) {
+static int render_impl(const orc_camera *cam, int n_trees, const orc_octree *trees, const double *poses, const double *half,
+                       const orc_opts *opt, const uint8_t *mask, double *rgb, double *depth, double *alpha,
+                       const double *g_rgb, const double *g_depth, const double *g_alpha, orc_grad *grads,
+                       uint32_t *n_used, const orc_sky *sky, double *normal /* [H][W][3] or NULL */,
+                       const double *g_normal /* [H][W][3] or NULL */, const orc_feat *fx) {
   if (!cam || !trees || !opt || n_trees < 1 || opt->k_samples < 1 || opt->k_samples > 64) return -1;
   if (sky && (!sky->tex || sky->width < 1 || sky->height < 1)) return -1;
-  scene_t sc = {n_trees, trees, poses, half, cam, opt, sky};
+  scene_t sc = {n_trees, trees, poses, half, cam, opt, sky, fx};
   int W = (int)cam->width, H = (int)cam->height;
   int tw = (W + ORC_TILE - 1) / ORC_TILE, th = (H + ORC_TILE - 1) / ORC_TILE;
   tilelists tl = {0, 0};
@@ -703,8 +740,9 @@ int orc_render_full(const orc_camera *cam, int n_trees, const orc_octree *trees,
           uint32_t used;
           render_ray(&sc, u, v, opt->mode == 1 ? cand : NULL, ncand, &w, out5, g_rgb ? g5 : NULL, grads, &used,
                      normal ? normal + 3 * p : NULL, (g_rgb && g_normal) ? g_normal + 3 * p : NULL);
-          rgb[3 * p] = out5[0]; rgb[3 * p + 1] = out5[1]; rgb[3 * p + 2] = out5[2];
-          depth[p] = out5[3]; alpha[p] = out5[4];
+          if (rgb) { rgb[3 * p] = out5[0]; rgb[3 * p + 1] = out5[1]; rgb[3 * p + 2] = out5[2]; }
+          if (depth) depth[p] = out5[3];
+          if (alpha) alpha[p] = out5[4];
           if (n_used) n_used[p] = used;
         }
     }
@@ -712,6 +750,25 @@ int orc_render_full(const orc_camera *cam, int n_trees, const orc_octree *trees,
   }
   free(tl.start); free(tl.ids);
   return 0;
+}
+
+int orc_render_full(const orc_camera *cam, int n_trees, const orc_octree *trees, const double *poses, const double *half,
+                    const orc_opts *opt, const uint8_t *mask, double *rgb, double *depth, double *alpha,
+                    const double *g_rgb, const double *g_depth, const double *g_alpha, orc_grad *grads,
+                    uint32_t *n_used, const orc_sky *sky, double *normal, const double *g_normal) {
+  if (!rgb || !depth || !alpha) return -1;
+  return render_impl(cam, n_trees, trees, poses, half, opt, mask, rgb, depth, alpha, g_rgb, g_depth, g_alpha, grads, n_used,
+                     sky, normal, g_normal, NULL);
+}
+
+/* O12: feature image and / or fusion over every pixel whose mask byte is non-zero; alpha (optional) = 1 - T_final. */
+int orc_render_features(const orc_camera *cam, int n_trees, const orc_octree *trees, const double *poses,
+                        const double *half, const orc_opts *opt, const uint8_t *mask, const orc_feat *fx, double *alpha) {
+  if (!fx || fx->n_channels < 1) return -1;
+  if (fx->feat && !fx->out) return -1;
+  if (fx->img && (!fx->num || !fx->wsum)) return -1;
+  return render_impl(cam, n_trees, trees, poses, half, opt, mask, NULL, NULL, alpha, NULL, NULL, NULL, NULL, NULL, NULL, NULL,
+                     NULL, fx);
 }
 
 int orc_render_sky(const orc_camera *cam, int n_trees, const orc_octree *trees, const double *poses, const double *half,

@@ -149,6 +149,53 @@ def render(scene, cam_index=0, mode=0, mask=None, grads_in=None, want_grads=None
     return out
 
 
+class _Feat(C.Structure):
+    _fields_ = [("n_channels", C.c_uint32), ("feat", C.POINTER(C.c_void_p)), ("out", C.c_void_p), ("img", C.c_void_p),
+                ("num", C.POINTER(C.c_void_p)), ("wsum", C.POINTER(C.c_void_p))]
+
+
+def render_features(scene, feats=None, img=None, cam_index=0, mode=0, mask=None, **opt):
+    """O12 (row N3, reading R25).  feats: list of [V_t, C] arrays per octree -> 'features' [H,W,C] = sum_j T_j alpha_j f_j.
+    img: [H,W,C] 2-D features -> 'num' (list of [V_t,C]) and 'wsum' (list of [V_t]): the fuse pass, the transpose of the
+    feature render.  Also returns 'alpha'.  Double precision."""
+    p = _Packed(scene, cam_index, mode, **opt)
+    H, W = p.hw
+    nt = p.n_trees
+    fx = _Feat()
+    out = {}
+    keep = []
+    if feats is not None:
+        fs = [np.ascontiguousarray(f, dtype=np.float64) for f in feats]
+        n_ch = fs[0].shape[1] if fs[0].ndim == 2 else int(np.asarray(feats[0]).shape[-1])
+        assert all(f.shape == (t.n_voxels, n_ch) for f, t in zip(fs, scene.octrees))
+        arr = (C.c_void_p * nt)(*[f.ctypes.data for f in fs])
+        fx.feat = C.cast(arr, C.POINTER(C.c_void_p))
+        F = np.zeros((H, W, n_ch))
+        fx.out = _ptr(F)
+        out["features"] = F
+        keep += [fs, arr]
+    if img is not None:
+        im = np.ascontiguousarray(img, dtype=np.float64)
+        n_ch = im.shape[2]
+        assert im.shape == (H, W, n_ch)
+        num = [np.zeros((t.n_voxels, n_ch)) for t in scene.octrees]
+        ws = [np.zeros(t.n_voxels) for t in scene.octrees]
+        a1 = (C.c_void_p * nt)(*[a.ctypes.data for a in num])
+        a2 = (C.c_void_p * nt)(*[a.ctypes.data for a in ws])
+        fx.img, fx.num, fx.wsum = _ptr(im), C.cast(a1, C.POINTER(C.c_void_p)), C.cast(a2, C.POINTER(C.c_void_p))
+        out["num"], out["wsum"] = num, ws
+        keep += [im, a1, a2]
+    fx.n_channels = n_ch
+    alpha = np.zeros((H, W))
+    m = None if mask is None else np.ascontiguousarray(mask, dtype=np.uint8)
+    rc = lib().orc_render_features(C.byref(p.cam), p.n_trees, p.trees, _ptr(p.poses), _ptr(p.half), C.byref(p.opts), _ptr(m),
+                                   C.byref(fx), _ptr(alpha))
+    if rc != 0:
+        raise ValueError("orc_render_features: invalid arguments")
+    out["alpha"] = alpha
+    return out
+
+
 def tile_hit_list(scene, tx, ty, tree, octant, cam_index=0):
     p = _Packed(scene, cam_index, 0)
     cap = scene.octrees[tree].n_voxels
