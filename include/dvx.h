@@ -235,6 +235,33 @@ typedef struct {
 dvx_status dvx_grid_adam_step_n(dvx_ctx *ctx, const dvx_adam *hp, uint32_t n, const dvx_grid_adam_item *items);
 dvx_status dvx_adam_step_n(dvx_ctx *ctx, const dvx_adam *hp, uint32_t n, const dvx_adam_item *items);
 
+/* ---- Widening row N3: feature compositing and the feature fuser -----------------------------------------
+ * "substituting the standard RGB color rendering step with a high-dimensional feature accumulation pass" and
+ * the "feature volume fuser".  Reading R25: with w_j = T_j alpha_j the compositing weight of the j-th
+ * composited sub-segment of a pixel's ray (the weights that blend the colour; early termination as rendered),
+ *   render:  F[p][c]    = sum_j w_j feat[v_j][c]                     (no view dependence, no sky term)
+ *   fuse:    num[v][c] += sum over (p, j) with v_j = v of w_j img[p][c],   wsum[v] += the same sum of w_j
+ * so num / wsum is the weight-averaged 2-D feature a voxel saw, and fuse is the transpose of render.
+ * Voxels are addressed by their FRAME-GLOBAL index: the octrees of the dvx_render call laid end to end (static octree
+ * first, then actor 0 .. N-1), i.e. row = (sum of n_voxels of the octrees before it) + voxel index.  V_total = that sum
+ * over all octrees.  All three calls need a frame rendered with saved != NULL and still alive. */
+typedef struct {
+  uint64_t nnz;              /* = sum over pixels of the number of composited sub-segments */
+  const uint32_t *row_start; /* DEVICE [H*W + 1], row-major pixels */
+  const uint32_t *voxel;     /* DEVICE [nnz] frame-global voxel index, front to back within a row */
+  const float *weight;       /* DEVICE [nnz] w_j */
+} dvx_weights;
+/* The compositing weights of the frame as a CSR matrix [H*W x V_total].  Built on the first call by one replay of the
+ * compositing pass (the per-pixel counts were saved by dvx_render), then cached in the frame until dvx_frame_release;
+ * the pointers are borrowed.  out may be NULL (build only).  Synchronises the stream (it has to learn nnz). */
+dvx_status dvx_frame_weights(dvx_ctx *ctx, dvx_frame *frame, dvx_weights *out);
+/* F = W feat.  n_channels C in [1, 512]; feat DEVICE [V_total][C], out DEVICE [H][W][C] (overwritten), both 16-byte
+ * aligned.  Builds the weights if dvx_frame_weights has not been called.  Does not synchronise otherwise. */
+dvx_status dvx_render_features(dvx_ctx *ctx, dvx_frame *frame, uint32_t n_channels, const float *feat, float *out);
+/* num += W^T img, wsum += W^T 1.  img DEVICE [H][W][C]; num DEVICE [V_total][C] ACCUMULATED; wsum DEVICE [V_total]
+ * ACCUMULATED, or NULL.  Float atomics: the sums are order-dependent in the last bits. */
+dvx_status dvx_fuse_features(dvx_ctx *ctx, dvx_frame *frame, uint32_t n_channels, const float *img, float *num, float *wsum);
+
 #ifdef __cplusplus
 }
 #endif

@@ -23,7 +23,8 @@ EXPORTS = ["dvx_create", "dvx_destroy", "dvx_octree_create", "dvx_octree_refresh
            "dvx_render", "dvx_backward", "dvx_backward_n", "dvx_frame_release", "dvx_debug_tile_list", "dvx_frame_counters",
            "dvx_frame_stage_ms", "dvx_last_error", "dvx_sort_pairs", "dvx_launch_count", "dvx_stage_ms_collect", "dvx_render_host",
            "dvx_backward_host", "dvx_grid_create", "dvx_grid_destroy", "dvx_grid_gather", "dvx_grid_reduce",
-           "dvx_grid_adam_step", "dvx_adam_step", "dvx_grid_adam_step_n", "dvx_adam_step_n"]
+           "dvx_grid_adam_step", "dvx_adam_step", "dvx_grid_adam_step_n", "dvx_adam_step_n",
+           "dvx_frame_weights", "dvx_render_features", "dvx_fuse_features"]
 
 
 class DvxError(RuntimeError):
@@ -65,6 +66,10 @@ class GridTables(C.Structure):
 
 class Adam(C.Structure):
     _fields_ = [("lr", C.c_float), ("beta1", C.c_float), ("beta2", C.c_float), ("eps", C.c_float), ("step", C.c_uint32)]
+
+
+class Weights(C.Structure):
+    _fields_ = [("nnz", C.c_uint64), ("row_start", C.c_void_p), ("voxel", C.c_void_p), ("weight", C.c_void_p)]
 
 
 class GridAdamItem(C.Structure):
@@ -121,6 +126,9 @@ def load():
     lib.dvx_grid_reduce.argtypes = [P, P, P, P]
     lib.dvx_grid_adam_step.argtypes = [P, P, C.POINTER(Adam), P, P, P, P, P]
     lib.dvx_adam_step.argtypes = [P, C.POINTER(Adam), C.c_uint64, P, P, P, P]
+    lib.dvx_frame_weights.argtypes = [P, P, C.POINTER(Weights)]
+    lib.dvx_render_features.argtypes = [P, P, C.c_uint32, P, P]
+    lib.dvx_fuse_features.argtypes = [P, P, C.c_uint32, P, P, P]
     lib.dvx_grid_adam_step_n.argtypes = [P, C.POINTER(Adam), C.c_uint32, C.POINTER(GridAdamItem)]
     lib.dvx_adam_step_n.argtypes = [P, C.POINTER(Adam), C.c_uint32, C.POINTER(AdamItem)]
     for name in EXPORTS:
@@ -365,6 +373,34 @@ class Frame:
         fn = ctx.lib.dvx_backward_host if host else ctx.lib.dvx_backward
         ctx.check(fn(ctx.h, self.h, ptr(dL_drgb), ptr(dL_ddepth), ptr(dL_dalpha), g[0], arr))
         return grads
+
+    # ------------------------------------------------------------------ row N3: feature compositing
+    def weights(self):
+        """dvx_frame_weights -> (nnz, row_start [H*W+1], voxel [nnz], weight [nnz]) as zero-copy views of the frame's CSR."""
+        ctx, torch = self.ctx, self.ctx.torch
+        w = Weights()
+        ctx.check(ctx.lib.dvx_frame_weights(ctx.h, self.h, C.byref(w)))
+
+        def view(ptr, n, dtype):
+            if n == 0:
+                return torch.empty(0, dtype=dtype, device=ctx.device)
+            return ctx._blocks[ptr].view(dtype)[:n]
+        nnz = int(w.nnz)
+        return nnz, ctx._blocks[w.row_start].view(torch.int32), view(w.voxel, nnz, torch.int32), view(w.weight, nnz, torch.float32)
+
+    def render_features(self, feat, height, width):
+        """dvx_render_features: feat CUDA float32 [V_total, C] (octrees end to end) -> [H, W, C]."""
+        ctx, torch = self.ctx, self.ctx.torch
+        n_ch = int(feat.shape[1])
+        out = torch.empty((height, width, n_ch), dtype=torch.float32, device=ctx.device)
+        ctx.check(ctx.lib.dvx_render_features(ctx.h, self.h, n_ch, feat.data_ptr(), out.data_ptr()))
+        return out
+
+    def fuse_features(self, img, num, wsum=None):
+        """dvx_fuse_features: img [H, W, C]; num [V_total, C] and wsum [V_total] are accumulated into."""
+        ctx = self.ctx
+        ctx.check(ctx.lib.dvx_fuse_features(ctx.h, self.h, int(img.shape[2]), img.data_ptr(), num.data_ptr(),
+                                            wsum.data_ptr() if wsum is not None else None))
 
     def tile_list(self, tile, octree, octant):
         ctx = self.ctx

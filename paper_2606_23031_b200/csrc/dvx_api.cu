@@ -56,6 +56,8 @@ struct dvx_frame {
   EventSet *es = nullptr;
   cudaEvent_t *ev = nullptr;  // = es->ev
   Buf eff_end, vnrm, sv_nrm;
+  Buf w_row, w_vox, w_val;  // row N3: the compositing weights as CSR, built on demand
+  uint64_t w_nnz = 0;
   dvx_sky sky = {0, 0, nullptr, nullptr};
   bool did_backward = false;
 };
@@ -127,6 +129,7 @@ void frame_free(dvx_ctx *ctx, dvx_frame *f) {
   ctx_release(ctx, f->eff_end.p);
   ctx_release(ctx, f->vnrm.p);
   ctx_release(ctx, f->sv_nrm.p);
+  ctx_release(ctx, f->w_row.p); ctx_release(ctx, f->w_vox.p); ctx_release(ctx, f->w_val.p);
   if (f->es) {
     f->es->did_backward = f->did_backward;
     if (f->es->rendered) {
@@ -883,6 +886,77 @@ dvx_status dvx_adam_step_n(dvx_ctx *ctx, const dvx_adam *hp, uint32_t n, const d
 dvx_status dvx_adam_step(dvx_ctx *ctx, const dvx_adam *hp, uint64_t n, float *p, float *m, float *v, float *g) {
   const dvx_adam_item it = {n, p, m, v, g};
   return dvx_adam_step_n(ctx, hp, 1, &it);
+}
+
+// ---- row N3: feature compositing (dvx_features.cu) ----------------------------------------------------------------------
+dvx_status dvx_frame_weights(dvx_ctx *ctx, dvx_frame *f, dvx_weights *out) {
+  if (!ctx) return DVX_ERR_INVALID_ARG;
+  if (!f) return fail(ctx, DVX_ERR_INVALID_ARG, "dvx_frame_weights: frame is NULL");
+  if (!f->sv_rgbd.p) return fail(ctx, DVX_ERR_INVALID_ARG, "frame holds no saved state");
+  if (f->p.flags & DVX_FLAG_NAIVE) return fail(ctx, DVX_ERR_NOT_IMPLEMENTED, "weights need the tile kernel (no DVX_FLAG_NAIVE)");
+  const FrameParams &p = f->p;
+  cudaSetDevice(ctx->device);
+  cudaStream_t st = ctx->st;
+  if (!f->w_row.p) {
+    const size_t npix = (size_t)p.width * p.height;
+    if (!buf_alloc(ctx, f->w_row, (npix + 1) * 4)) return fail(ctx, DVX_ERR_OOM, "dvx_frame_weights: allocator returned NULL");
+    uint32_t *row = (uint32_t *)f->w_row.p;
+    void *scr = ctx_alloc(ctx, dvx_sort_scratch_bytes(npix + 1));
+    if (!scr) return fail(ctx, DVX_ERR_OOM, "dvx_frame_weights: allocator returned NULL");
+    CU(cudaMemcpyAsync(row, f->sv_nused.p, npix * 4, cudaMemcpyDeviceToDevice, st));
+    CU(cudaMemsetAsync(row + npix, 0, 4, st));
+    dvx_scan_u32_launch(row, npix + 1, (uint32_t *)scr, st);  // exclusive: row[npix] = nnz
+    uint32_t nnz = 0;
+    CU(cudaMemcpyAsync(&nnz, row + npix, 4, cudaMemcpyDeviceToHost, st));
+    CU(cudaStreamSynchronize(st));
+    ctx_release(ctx, scr);
+    f->w_nnz = nnz;
+    if (!buf_alloc(ctx, f->w_vox, (size_t)nnz * 4) || !buf_alloc(ctx, f->w_val, (size_t)nnz * 4))
+      return fail(ctx, DVX_ERR_OOM, "dvx_frame_weights: allocator returned NULL");
+    CompositeArgs A;
+    memset(&A, 0, sizeof(A));
+    A.p = p; A.trees = (const TreeFrame *)f->trees_d.p; A.fvox = (const FrameVox *)f->fvox.p; A.pxrect = (const ushort4 *)f->pxrect.p;
+    A.ids = (const uint32_t *)f->ids.p; A.range_beg = (const uint32_t *)f->range_beg.p; A.range_end = (const uint32_t *)f->range_end.p;
+    A.actor_mask = (const unsigned long long *)f->actor_mask.p;
+    A.counters = (unsigned long long *)f->counters.p;
+    A.exp_row = row; A.exp_vox = (uint32_t *)f->w_vox.p; A.exp_w = (float *)f->w_val.p;
+    dvx_composite_export_launch(A, st);
+    CU(cudaGetLastError());
+  }
+  if (out) {
+    out->nnz = f->w_nnz;
+    out->row_start = (const uint32_t *)f->w_row.p;
+    out->voxel = (const uint32_t *)f->w_vox.p;
+    out->weight = (const float *)f->w_val.p;
+  }
+  return DVX_OK;
+}
+
+static dvx_status features_common(dvx_ctx *ctx, dvx_frame *f, uint32_t C, const void *a, const void *b, const char *who) {
+  if (!ctx) return DVX_ERR_INVALID_ARG;
+  if (!f || !a || !b) return fail(ctx, DVX_ERR_INVALID_ARG, "NULL argument");
+  if (C < 1 || C > 512) return fail(ctx, DVX_ERR_INVALID_ARG, "n_channels must be in [1, 512]");
+  if (((uintptr_t)a | (uintptr_t)b) & 15) return fail(ctx, DVX_ERR_INVALID_ARG, "feature arrays must be 16-byte aligned");
+  (void)who;
+  return dvx_frame_weights(ctx, f, nullptr);
+}
+
+dvx_status dvx_render_features(dvx_ctx *ctx, dvx_frame *f, uint32_t n_channels, const float *feat, float *out) {
+  dvx_status rc = features_common(ctx, f, n_channels, feat, out, "dvx_render_features");
+  if (rc != DVX_OK) return rc;
+  dvx_features_launch(f->p.width, f->p.height, n_channels, (const uint32_t *)f->w_row.p, (const uint32_t *)f->w_vox.p,
+                      (const float *)f->w_val.p, feat, out, nullptr, nullptr, nullptr, ctx->st);
+  CU(cudaGetLastError());
+  return DVX_OK;
+}
+
+dvx_status dvx_fuse_features(dvx_ctx *ctx, dvx_frame *f, uint32_t n_channels, const float *img, float *num, float *wsum) {
+  dvx_status rc = features_common(ctx, f, n_channels, img, num, "dvx_fuse_features");
+  if (rc != DVX_OK) return rc;
+  dvx_features_launch(f->p.width, f->p.height, n_channels, (const uint32_t *)f->w_row.p, (const uint32_t *)f->w_vox.p,
+                      (const float *)f->w_val.p, nullptr, nullptr, img, num, wsum, ctx->st);
+  CU(cudaGetLastError());
+  return DVX_OK;
 }
 
 }  // extern "C"

@@ -87,6 +87,7 @@ struct Pix {
   uint32_t n_stop;
   float N0, N1, N2;     // normal map (O11), forward
   float gN0, gN1, gN2;  // dL/dN, backward
+  uint32_t exp_pos;     // weight export (row N3): start of this pixel's row in the CSR arrays
 };
 
 __device__ __forceinline__ uint32_t warp_min_u32(uint32_t v) { return __reduce_min_sync(0xffffffffu, v); }
@@ -251,7 +252,7 @@ __device__ __forceinline__ void red_add_v4(float *addr, float x, float y, float 
 
 // ---- phases B, C (and B2) over the first min(n_items, 32) queued items of the ring ------------------------------------
 // Ring slot of the i-th queued item: (head + i) & (QCAP-1).  my_bits: bit i set <=> queued item i belongs to this pixel.
-template <bool BWD, bool NRM>
+template <bool BWD, bool NRM, bool EXP = false>
 __device__ __forceinline__ void flush_batch(const CompositeArgs &A, int lane, WarpQueue<BWD, NRM> &Q, int &n_items, int &head,
                                             unsigned long long &my_bits, Pix &S) {
   const int count = n_items < 32 ? n_items : 32;
@@ -294,6 +295,13 @@ __device__ __forceinline__ void flush_batch(const CompositeArgs &A, int lane, Wa
       const float4 ea = Q.eam[i];
       const float e = ea.x, mid = ea.z;
       const float w = S.T * ea.y;
+      if (EXP) {  // row N3: the compositing weight of this (pixel, voxel), in the pixel's front-to-back order
+        if (S.n_used < S.n_stop) {
+          const uint32_t at = S.exp_pos + S.n_used;
+          A.exp_vox[at] = Q.item[(head + i) & (QCAP - 1)].id;
+          A.exp_w[at] = w;
+        }
+      }
       if (!BWD) {
         S.C0 = fmaf(w, f1.x, S.C0); S.C1 = fmaf(w, f1.y, S.C1); S.C2 = fmaf(w, f1.z, S.C2);
         S.D = fmaf(w, mid, S.D);
@@ -437,7 +445,7 @@ __device__ __noinline__ float2 axis_parallel_fix(const TreeFrame *T, uint32_t id
   return inside ? make_float2(sa, sb) : make_float2(INFINITY, -INFINITY);
 }
 
-template <bool BWD, bool CNT, bool NRM>
+template <bool BWD, bool CNT, bool NRM, bool EXP = false>
 __global__ void __launch_bounds__(TILE_THREADS, DVX_TILE_MIN_CTAS) composite_tile_kernel(const __grid_constant__ CompositeArgs A) {
   __shared__ WarpQueue<BWD, NRM> s_queue[TILE_WARPS];
   const FrameParams &p = A.p;
@@ -456,6 +464,11 @@ __global__ void __launch_bounds__(TILE_THREADS, DVX_TILE_MIN_CTAS) composite_til
   S.C0 = S.C1 = S.C2 = 0.f; S.D = 0.f; S.T = 1.f; S.n_used = 0; S.done = !inside;
   S.Xpre = 0.f; S.n_stop = 0;
   S.N0 = S.N1 = S.N2 = 0.f; S.gN0 = S.gN1 = S.gN2 = 0.f;
+  S.exp_pos = 0;
+  if (EXP && inside) {  // the row lengths are the n_used the rendering pass saved
+    S.exp_pos = A.exp_row[pix];
+    S.n_stop = A.exp_row[pix + 1] - S.exp_pos;
+  }
   if (BWD && inside) {
     S.gC0 = A.g_rgb[3 * pix]; S.gC1 = A.g_rgb[3 * pix + 1]; S.gC2 = A.g_rgb[3 * pix + 2];
     S.gD = A.g_depth ? A.g_depth[pix] : 0.f;
@@ -651,7 +664,7 @@ __global__ void __launch_bounds__(TILE_THREADS, DVX_TILE_MIN_CTAS) composite_til
             }
             n_items += __popc(mk);
             if (n_items >= 32) {
-              flush_batch<BWD, NRM>(A, lane, Q, n_items, head, my_bits, S);
+              flush_batch<BWD, NRM, EXP>(A, lane, Q, n_items, head, my_bits, S);
               if (S.done) active = 0u;
             }
           }
@@ -667,9 +680,9 @@ __global__ void __launch_bounds__(TILE_THREADS, DVX_TILE_MIN_CTAS) composite_til
     }
     if (part) seg_tree = NONE;          // served
   }
-  while (n_items > 0) flush_batch<BWD, NRM>(A, lane, Q, n_items, head, my_bits, S);
+  while (n_items > 0) flush_batch<BWD, NRM, EXP>(A, lane, Q, n_items, head, my_bits, S);
 
-  if (!BWD && inside) {
+  if (!BWD && !EXP && inside) {
     float3 sky = make_float3(0.f, 0.f, 0.f);
     if (A.sky_tex) sky = dvx_sky_forward(&A, u, v, S.T);  // Eq. 2: C = C_voxels + T_final C_sky
     A.rgb[3 * pix] = S.C0 + sky.x; A.rgb[3 * pix + 1] = S.C1 + sky.y; A.rgb[3 * pix + 2] = S.C2 + sky.z;
@@ -699,6 +712,14 @@ __global__ void __launch_bounds__(TILE_THREADS, DVX_TILE_MIN_CTAS) composite_til
 }
 
 }  // namespace
+
+// Row N3: the forward walk once more, writing the compositing weights (voxel, T alpha) of every pixel into the CSR rows
+// whose lengths the rendering pass saved; no image is written.
+void dvx_composite_export_launch(const CompositeArgs &a, cudaStream_t st) {
+  if (a.p.n_tiles == 0) return;
+  DVX_COUNT_LAUNCH(1);
+  composite_tile_kernel<false, false, false, true><<<a.p.n_tiles, TILE_THREADS, 0, st>>>(a);
+}
 
 void dvx_composite_tile_launch(const CompositeArgs &a, bool backward, cudaStream_t st) {
   if (a.p.n_tiles == 0) return;

@@ -77,6 +77,10 @@ struct CompositeArgs {
   // backward
   const float *g_rgb, *g_depth, *g_alpha;
   float *drgb;                 // [v_total][4] scratch: dL/drgb_v
+  // weight export (row N3)
+  const uint32_t *exp_row;     // [H*W + 1] CSR row starts
+  uint32_t *exp_vox;           // [nnz] global voxel id
+  float *exp_w;                // [nnz] T_j alpha_j
 };
 
 // Number of kernels launched by this library since it was loaded (bench.py's gpu_launches claim).
@@ -134,9 +138,15 @@ void dvx_grid_adam_launch(float lr, float beta1, float beta2, float eps, uint32_
 void dvx_adam_launch(float lr, float beta1, float beta2, float eps, uint32_t step, uint32_t n, const DvxAdamItem *items,
                      cudaStream_t st);
 
+// ---- dvx_features.cu (row N3).  img == NULL: render (feat, out);  img != NULL: fuse (img, num, wsum)
+void dvx_features_launch(uint32_t width, uint32_t height, uint32_t n_channels, const uint32_t *row_start, const uint32_t *voxel,
+                         const float *weight, const float *feat, float *out, const float *img, float *num, float *wsum,
+                         cudaStream_t st);
+
 // ---- dvx_composite_tile.cu (production) / dvx_composite_naive.cu (DVX_FLAG_NAIVE: one thread walks one ray, debug)
 void dvx_composite_tile_launch(const CompositeArgs &a, bool backward, cudaStream_t st);
 void dvx_composite_naive_launch(const CompositeArgs &a, bool backward, cudaStream_t st);
+void dvx_composite_export_launch(const CompositeArgs &a, cudaStream_t st);
 inline void dvx_composite_launch(const CompositeArgs &a, bool backward, cudaStream_t st) {
   if (a.p.flags & DVX_FLAG_NAIVE) dvx_composite_naive_launch(a, backward, st);
   else dvx_composite_tile_launch(a, backward, st);
