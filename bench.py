@@ -273,6 +273,52 @@ def optimizer_step_stats(ctx, dev, grads, peak, reps=5):
             "launches": 2 * ((len(dev.trees) + 31) // 32)}
 
 
+def feature_stats(ctx, dev, scene, peak, n_ch=64, reps=5):
+    """Widening row N3, reported beside the headline (not part of `value`): camera 0's compositing weights exported as a
+    CSR matrix (one replay of the tile kernel), then the feature render F = W feat and the fuser num += W^T img for C = 64
+    channels, CUDA events, median of reps.  Bytes: `dram_floor` = every datum once (8 nnz CSR + 4C per touched voxel row +
+    4C per pixel); `gathered` = what the SMs pull through L1/L2 (8 nnz + 4C nnz + 4C per pixel)."""
+    import torch
+    cam = scene.cameras[0]
+    H, W = cam.height, cam.width
+    _, _, _, fr = dev.render(0, save=True)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record()
+    nnz, rows, vox, w = fr.weights()
+    e1.record()
+    torch.cuda.synchronize()
+    export_ms = e0.elapsed_time(e1)
+    v_total = sum(t.n_voxels for t in dev.trees)
+    g = torch.Generator(device="cuda").manual_seed(3)
+    feat = torch.rand((v_total, n_ch), device="cuda", generator=g) * 2 - 1
+    img = torch.rand((H, W, n_ch), device="cuda", generator=g) * 2 - 1
+    num = torch.zeros((v_total, n_ch), device="cuda")
+    wsum = torch.zeros(v_total, device="cuda")
+    touched = int(torch.unique(vox).numel()) if nnz else 0
+    t_r, t_f = [], []
+    for _ in range(reps + 1):
+        e = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+        e[0].record()
+        fr.render_features(feat, H, W)
+        e[1].record()
+        fr.fuse_features(img, num, wsum)
+        e[2].record()
+        torch.cuda.synchronize()
+        t_r.append(e[0].elapsed_time(e[1])); t_f.append(e[1].elapsed_time(e[2]))
+    fr.release()
+    ms_r, ms_f = float(np.median(t_r[1:])), float(np.median(t_f[1:]))
+    floor = 8 * nnz + 4 * n_ch * touched + 4 * n_ch * H * W
+    gathered = 8 * nnz + 4 * n_ch * nnz + 4 * n_ch * H * W
+
+    def leg(ms, extra=0):
+        return {"ms": ms, "mp_per_s": H * W / ms / 1e3, "dram_floor_gb_per_s": (floor + extra) / ms / 1e6,
+                "dram_floor_hbm_frac": (floor + extra) / ms / 1e6 / peak, "gathered_gb_per_s": gathered / ms / 1e6}
+    return {"channels": n_ch, "nnz": nnz, "touched_voxels": touched, "weights_export_ms": export_ms,
+            "bytes": {"dram_floor": floor, "gathered": gathered},
+            "render": leg(ms_r), "fuse": leg(ms_f, 4 * n_ch * touched), "launches": 1 + 2 * (reps + 1) + 3}
+
+
 def run_dvx(args):
     import torch
     import torch.distributed as dist
@@ -381,6 +427,7 @@ def run_dvx(args):
     ms_e2e = timed(args.steps, host=True, bwd=not args.fwd_only)
     clocks = sampler.stop() if sampler else None
     sort_stats = sort_throughput(ctx, cnt["pairs"] // n_cams, scene, W, H) if rank == 0 else None
+    feat_stats = feature_stats(ctx, dev, scene, measured_peaks()[0]) if rank == 0 and not args.fwd_only else None
     opt_stats = optimizer_step_stats(ctx, dev, grads, measured_peaks()[0]) if rank == 0 and not args.fwd_only else None
 
     if rank != 0:
@@ -433,7 +480,7 @@ def run_dvx(args):
                          "peak_source": "148 SMs x 128 fp32 lanes x %.0f MHz (nvidia-smi, under load)" % sm_mhz},
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": (0 if args.fwd_only else 12 * px_step),
                 "d2h_bytes_per_step": 20 * px_step, "ms_per_step": ms_e2e / args.steps},
-        "sort": sort_stats, "n2_optimizer_step": opt_stats,
+        "sort": sort_stats, "n2_optimizer_step": opt_stats, "n3_features": feat_stats,
         "gpu_launches": launches, "clocks": clocks,
     }
     if not args.no_cpu_baseline and world == 1:

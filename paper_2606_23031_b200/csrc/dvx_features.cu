@@ -76,6 +76,7 @@ __global__ void __launch_bounds__(FEAT_THREADS) feature_kernel(const __grid_cons
         my_w = __ldg(A.weight + j0 + lane);
       }
       if (FUSE && A.wsum && (uint32_t)lane < n) atomicAdd(A.wsum + my_vox, my_w);
+#pragma unroll 4
       for (uint32_t i = 0; i < n; ++i) {
         const uint32_t id = __shfl_sync(0xffffffffu, my_vox, (int)i);
         const float w = __shfl_sync(0xffffffffu, my_w, (int)i);
@@ -117,6 +118,71 @@ __global__ void __launch_bounds__(FEAT_THREADS) feature_kernel(const __grid_cons
   }
 }
 
+// C = 4 LPR with LPR | 32 (C = 4 .. 128): a row is LPR float4 lanes, so the warp serves 32 / LPR non-zeros at once - every
+// lane busy - each lane group with its own accumulator, summed across the groups by shuffles when the pixel is done.
+template <int LPR, bool FUSE>
+__global__ void __launch_bounds__(FEAT_THREADS) feature_grouped_kernel(const __grid_constant__ FeatArgs A) {
+  constexpr int NG = 32 / LPR;
+  const int tile = blockIdx.x, warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int grp = lane / LPR, sub = lane % LPR;
+  const int u0 = (tile % A.tiles_x) * DVX_TILE + (warp & 3) * 4;
+  const int v0 = (tile / A.tiles_x) * DVX_TILE + (warp >> 2) * 8;
+  constexpr uint32_t C = 4 * LPR;
+  for (int px = 0; px < 32; ++px) {
+    const int u = u0 + (px & 3), v = v0 + (px >> 2);
+    if (u >= (int)A.width || v >= (int)A.height) continue;  // warp-uniform
+    const size_t pix = (size_t)v * A.width + u;
+    const uint32_t b = A.row_start[pix], e = A.row_start[pix + 1];
+    float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (FUSE) acc = *reinterpret_cast<const float4 *>(A.img + pix * C + 4 * sub);
+    for (uint32_t j0 = b; j0 < e; j0 += 32) {
+      const uint32_t n = min(32u, e - j0);
+      uint32_t my_vox = 0;
+      float my_w = 0.f;
+      if ((uint32_t)lane < n) {
+        my_vox = __ldg(A.voxel + j0 + lane);
+        my_w = __ldg(A.weight + j0 + lane);
+      }
+      if (FUSE && A.wsum && (uint32_t)lane < n) atomicAdd(A.wsum + my_vox, my_w);
+#pragma unroll 4
+      for (uint32_t i0 = 0; i0 < n; i0 += NG) {
+        const uint32_t i = i0 + grp;
+        const uint32_t id = __shfl_sync(0xffffffffu, my_vox, (int)(i & 31u));
+        const float w = __shfl_sync(0xffffffffu, my_w, (int)(i & 31u));
+        if (i < n) {
+          if (!FUSE) {
+            const float4 f = __ldg(reinterpret_cast<const float4 *>(A.feat + (size_t)id * C) + sub);
+            acc.x = fmaf(w, f.x, acc.x); acc.y = fmaf(w, f.y, acc.y); acc.z = fmaf(w, f.z, acc.z); acc.w = fmaf(w, f.w, acc.w);
+          } else {
+            red_add_v4f(A.num + (size_t)id * C + 4 * sub, make_float4(w * acc.x, w * acc.y, w * acc.z, w * acc.w));
+          }
+        }
+      }
+    }
+    if (!FUSE) {
+#pragma unroll
+      for (int o = LPR; o < 32; o <<= 1) {
+        acc.x += __shfl_xor_sync(0xffffffffu, acc.x, o); acc.y += __shfl_xor_sync(0xffffffffu, acc.y, o);
+        acc.z += __shfl_xor_sync(0xffffffffu, acc.z, o); acc.w += __shfl_xor_sync(0xffffffffu, acc.w, o);
+      }
+      if (grp == 0) *(reinterpret_cast<float4 *>(A.out + pix * C) + sub) = acc;
+    }
+  }
+}
+
+template <bool FUSE>
+bool launch_grouped(const FeatArgs &A, unsigned tiles, cudaStream_t st) {
+  switch (A.n_channels) {
+    case 4: feature_grouped_kernel<1, FUSE><<<tiles, FEAT_THREADS, 0, st>>>(A); return true;
+    case 8: feature_grouped_kernel<2, FUSE><<<tiles, FEAT_THREADS, 0, st>>>(A); return true;
+    case 16: feature_grouped_kernel<4, FUSE><<<tiles, FEAT_THREADS, 0, st>>>(A); return true;
+    case 32: feature_grouped_kernel<8, FUSE><<<tiles, FEAT_THREADS, 0, st>>>(A); return true;
+    case 64: feature_grouped_kernel<16, FUSE><<<tiles, FEAT_THREADS, 0, st>>>(A); return true;
+    case 128: feature_grouped_kernel<32, FUSE><<<tiles, FEAT_THREADS, 0, st>>>(A); return true;
+    default: return false;
+  }
+}
+
 }  // namespace
 
 void dvx_features_launch(uint32_t width, uint32_t height, uint32_t n_channels, const uint32_t *row_start, const uint32_t *voxel,
@@ -131,6 +197,7 @@ void dvx_features_launch(uint32_t width, uint32_t height, uint32_t n_channels, c
   const bool fuse = img != nullptr;
   const bool v4 = (n_channels % 4) == 0;
   DVX_COUNT_LAUNCH(1);
+  if (fuse ? launch_grouped<true>(A, tiles, st) : launch_grouped<false>(A, tiles, st)) return;
   if (fuse) {
     if (v4) feature_kernel<4, true><<<tiles, FEAT_THREADS, 0, st>>>(A);
     else feature_kernel<1, true><<<tiles, FEAT_THREADS, 0, st>>>(A);
