@@ -262,6 +262,38 @@ dvx_status dvx_render_features(dvx_ctx *ctx, dvx_frame *frame, uint32_t n_channe
  * ACCUMULATED, or NULL.  Float atomics: the sums are order-dependent in the last bits. */
 dvx_status dvx_fuse_features(dvx_ctx *ctx, dvx_frame *frame, uint32_t n_channels, const float *img, float *num, float *wsum);
 
+/* ---- Widening row N4: LiDAR-guided structure operations of the static octree ------------
+ * "Proximity-Based Voxel Subdivision: ... In each round, voxels closer than a distance threshold to a LiDAR point are
+ * subdivided" (:87) and "Soft Density Initialization Prior: ... For each grid corner, the euclidean distance d to the
+ * nearest LiDAR point is computed and mapped to an initial density" v = v_far + (v_close - v_far) exp(-2 d^2 / s^2) (Eq. 1,
+ * :91; the paper sets v_close = -2, v_far = -10, s = the minimum voxel size).  Readings R26-R28: the distance
+ * of a point to a voxel is the Euclidean distance to its closed box (0 inside), "closer than" is <=; Eq. 1 is evaluated per
+ * grid point of R23; a leaf is pruned when the largest of its 8 raw corner densities is below a threshold.  Geometry is
+ * evaluated in fp64 from the fp32 inputs, so split / keep decisions are exact.  After a structure change the caller rebuilds
+ * the step-0 tables (dvx_octree_refresh_structure) and the grid tables (dvx_grid_create). */
+typedef struct dvx_cloud dvx_cloud; /* opaque: the LiDAR points binned into a uniform cell grid */
+/* points DEVICE [n][3] fp32 in the octree's frame (copied, not borrowed), n < 2^31.  cell > 0: the edge of the binning
+ * cells; queries cost least when it is about the query radius (the subdivision threshold, 3.1 s for Eq. 1).
+ * Synchronises the stream.  n = 0 is valid (nothing is ever near). */
+dvx_status dvx_cloud_create(dvx_ctx *ctx, const float *points, uint64_t n, float cell, dvx_cloud **out);
+void dvx_cloud_destroy(dvx_ctx *ctx, dvx_cloud *cloud);
+/* Eq. 1 for every grid point of `grid` (built from desc->code): density DEVICE [G] overwritten.  desc supplies center,
+ * side and code; geo / sh are not read.  Points further than 3.1 s_min from a grid point cannot change its fp32 result and
+ * are not searched.  Does not synchronise. */
+dvx_status dvx_density_prior(dvx_ctx *ctx, const dvx_cloud *cloud, const dvx_octree_desc *desc, const dvx_grid *grid,
+                             float s_min, float v_close, float v_far, float *density);
+/* One subdivision round: every leaf with level < max_level that has a point within `threshold` of its box is replaced by its
+ * 8 children (octant order 4x+2y+z), the others are kept; input order is preserved.  *n_out (HOST) = number of leaves of
+ * the result; code_out DEVICE [capacity] is written only if capacity >= *n_out (8 V always suffices).  split DEVICE [V]
+ * bytes (1 = was subdivided) or NULL.  Synchronises the stream. */
+dvx_status dvx_subdivide_near(dvx_ctx *ctx, const dvx_cloud *cloud, const dvx_octree_desc *desc, float threshold,
+                              uint32_t max_level, uint64_t *code_out, uint64_t capacity, uint64_t *n_out, uint8_t *split);
+/* Pruning: keeps the leaves whose largest raw corner density is >= threshold, in order.  code DEVICE [V], geo DEVICE
+ * [V][8] (32-byte aligned); code_out DEVICE [V]; index_out DEVICE [V] (the kept leaves' old indices, for gathering geo and
+ * sh) or NULL; *n_out HOST.  Synchronises the stream. */
+dvx_status dvx_prune(dvx_ctx *ctx, uint32_t n_voxels, const uint64_t *code, const float *geo, float threshold,
+                     uint64_t *code_out, uint32_t *index_out, uint32_t *n_out);
+
 #ifdef __cplusplus
 }
 #endif

@@ -24,7 +24,8 @@ EXPORTS = ["dvx_create", "dvx_destroy", "dvx_octree_create", "dvx_octree_refresh
            "dvx_frame_stage_ms", "dvx_last_error", "dvx_sort_pairs", "dvx_launch_count", "dvx_stage_ms_collect", "dvx_render_host",
            "dvx_backward_host", "dvx_grid_create", "dvx_grid_destroy", "dvx_grid_gather", "dvx_grid_reduce",
            "dvx_grid_adam_step", "dvx_adam_step", "dvx_grid_adam_step_n", "dvx_adam_step_n",
-           "dvx_frame_weights", "dvx_render_features", "dvx_fuse_features"]
+           "dvx_frame_weights", "dvx_render_features", "dvx_fuse_features",
+           "dvx_cloud_create", "dvx_cloud_destroy", "dvx_density_prior", "dvx_subdivide_near", "dvx_prune"]
 
 
 class DvxError(RuntimeError):
@@ -129,11 +130,17 @@ def load():
     lib.dvx_frame_weights.argtypes = [P, P, C.POINTER(Weights)]
     lib.dvx_render_features.argtypes = [P, P, C.c_uint32, P, P]
     lib.dvx_fuse_features.argtypes = [P, P, C.c_uint32, P, P, P]
+    lib.dvx_cloud_create.argtypes = [P, P, C.c_uint64, C.c_float, C.POINTER(P)]
+    lib.dvx_cloud_destroy.argtypes = [P, P]
+    lib.dvx_cloud_destroy.restype = None
+    lib.dvx_density_prior.argtypes = [P, P, C.POINTER(OctreeDesc), P, C.c_float, C.c_float, C.c_float, P]
+    lib.dvx_subdivide_near.argtypes = [P, P, C.POINTER(OctreeDesc), C.c_float, C.c_uint32, P, C.c_uint64, C.POINTER(C.c_uint64), P]
+    lib.dvx_prune.argtypes = [P, C.c_uint32, P, P, C.c_float, P, P, C.POINTER(C.c_uint32)]
     lib.dvx_grid_adam_step_n.argtypes = [P, C.POINTER(Adam), C.c_uint32, C.POINTER(GridAdamItem)]
     lib.dvx_adam_step_n.argtypes = [P, C.POINTER(Adam), C.c_uint32, C.POINTER(AdamItem)]
     for name in EXPORTS:
         if name not in ("dvx_destroy", "dvx_octree_destroy", "dvx_frame_release", "dvx_last_error", "dvx_launch_count",
-                        "dvx_grid_destroy"):
+                        "dvx_grid_destroy", "dvx_cloud_destroy"):
             getattr(lib, name).restype = C.c_int32
     lib.dvx_launch_count.restype = C.c_uint64
     _lib = lib
@@ -213,6 +220,46 @@ class Context:
         hp = Adam(lr, beta1, beta2, eps, step)
         self.check(self.lib.dvx_adam_step(self.h, C.byref(hp), p.numel(), p.data_ptr(), m.data_ptr(), v.data_ptr(),
                                           g.data_ptr()))
+
+    # ------------------------------------------------------------------ row N4: LiDAR-guided structure operations
+    def cloud(self, points, cell):
+        """dvx_cloud_create for a CUDA float32 [n, 3] tensor of points in the octree's frame."""
+        return Cloud(self, points, cell)
+
+    @staticmethod
+    def _structure_desc(code, center, side):
+        n = int(code.shape[0])
+        return OctreeDesc(n, 0, (C.c_float * 3)(*[float(x) for x in center]), float(side), code.data_ptr() if n else None, None, None)
+
+    def density_prior(self, cloud, code, center, side, grid, s_min, v_close=-2.0, v_far=-10.0):
+        """dvx_density_prior (Eq. 1) -> CUDA float32 [G]."""
+        out = self.torch.empty(grid.n_points, dtype=self.torch.float32, device=self.device)
+        desc = self._structure_desc(code, center, side)
+        self.check(self.lib.dvx_density_prior(self.h, cloud.h, C.byref(desc), grid.h, s_min, v_close, v_far, out.data_ptr()))
+        return out
+
+    def subdivide_near(self, cloud, code, center, side, threshold, max_level=16):
+        """dvx_subdivide_near -> (new codes int64 [V'], split uint8 [V])."""
+        torch = self.torch
+        n = int(code.shape[0])
+        desc = self._structure_desc(code, center, side)
+        out = torch.empty(8 * n, dtype=torch.int64, device=self.device)
+        split = torch.zeros(n, dtype=torch.uint8, device=self.device)
+        n_out = C.c_uint64()
+        self.check(self.lib.dvx_subdivide_near(self.h, cloud.h, C.byref(desc), threshold, max_level, out.data_ptr(), 8 * n,
+                                               C.byref(n_out), split.data_ptr()))
+        return out[:n_out.value], split
+
+    def prune(self, code, geo, threshold):
+        """dvx_prune -> (kept codes int64 [V'], kept indices int32 [V'])."""
+        torch = self.torch
+        n = int(code.shape[0])
+        out = torch.empty(n, dtype=torch.int64, device=self.device)
+        idx = torch.empty(n, dtype=torch.int32, device=self.device)
+        n_out = C.c_uint32()
+        self.check(self.lib.dvx_prune(self.h, n, code.data_ptr(), geo.data_ptr(), threshold, out.data_ptr(), idx.data_ptr(),
+                                      C.byref(n_out)))
+        return out[:n_out.value], idx[:n_out.value]
 
     def grid_adam_step_n(self, items, lr, beta1, beta2, eps, step):
         """dvx_grid_adam_step_n: items = [(Grid, density, m, v, dgeo, geo), ...], all octrees in one launch."""
@@ -298,6 +345,23 @@ class Octree:
     def close(self):
         if self.h and self.ctx.h:
             self.ctx.lib.dvx_octree_destroy(self.ctx.h, self.h)
+        self.h = None
+
+
+class Cloud:
+    """LiDAR points binned into a uniform cell grid (dvx_cloud_create)."""
+
+    def __init__(self, ctx, points, cell):
+        self.ctx = ctx
+        points = points.contiguous()
+        h = C.c_void_p()
+        n = int(points.shape[0])
+        ctx.check(ctx.lib.dvx_cloud_create(ctx.h, points.data_ptr() if n else None, n, cell, C.byref(h)))
+        self.h = h
+
+    def close(self):
+        if self.h and self.ctx.h:
+            self.ctx.lib.dvx_cloud_destroy(self.ctx.h, self.h)
         self.h = None
 
 

@@ -138,6 +138,32 @@ void dvx_grid_adam_launch(float lr, float beta1, float beta2, float eps, uint32_
 void dvx_adam_launch(float lr, float beta1, float beta2, float eps, uint32_t step, uint32_t n, const DvxAdamItem *items,
                      cudaStream_t st);
 
+// ---- dvx_structure.cu (row N4: LiDAR-guided structure operations)
+struct DvxCloudData {
+  double origin[3];            // lower corner of cell (0,0,0)
+  double cell;                 // cell edge
+  uint32_t dims[3];            // cells per axis
+  uint32_t n_cells;            // occupied cells
+  uint64_t n;                  // points
+  const uint64_t *cell_key;    // [n_cells] ascending linear index (z * ny + y) * nx + x
+  const uint32_t *cell_start;  // [n_cells + 1]
+  const float4 *pts;           // [n] in cell order
+};
+void dvx_cloud_bounds_launch(const float *pts, uint64_t n, uint32_t *minmax6, cudaStream_t st);
+void dvx_cloud_keys_launch(const float *pts, uint64_t n, const DvxCloudData &d, uint64_t *keys, uint32_t *vals, cudaStream_t st);
+void dvx_cloud_gather_launch(const float *pts, const uint32_t *perm, uint64_t n, float4 *out, cudaStream_t st);
+void dvx_cloud_cells_launch(const uint64_t *skeys, const uint32_t *excl, uint64_t n, uint64_t *cell_key, uint32_t *cell_start,
+                            cudaStream_t st);
+void dvx_density_prior_launch(const DvxCloudData &d, const uint64_t *code, const uint32_t *offsets, const uint32_t *slots,
+                              uint32_t n_points, const double center[3], double side, double s_min, double reach,
+                              double v_close, double v_far, float *density, cudaStream_t st);
+void dvx_near_flags_launch(const DvxCloudData &d, const uint64_t *code, uint32_t n_voxels, const double center[3], double side,
+                           double threshold, uint32_t max_level, uint32_t *count, uint8_t *split, cudaStream_t st);
+void dvx_expand_launch(const uint64_t *code, uint32_t n_voxels, const uint32_t *offsets, uint64_t *out, cudaStream_t st);
+void dvx_prune_flags_launch(const float *geo, uint32_t n_voxels, float threshold, uint32_t *keep, cudaStream_t st);
+void dvx_prune_scatter_launch(const uint64_t *code, uint32_t n_voxels, const uint32_t *offsets, uint64_t *code_out,
+                              uint32_t *index_out, cudaStream_t st);
+
 // ---- dvx_features.cu (row N3).  img == NULL: render (feat, out);  img != NULL: fuse (img, num, wsum)
 void dvx_features_launch(uint32_t width, uint32_t height, uint32_t n_channels, const uint32_t *row_start, const uint32_t *voxel,
                          const float *weight, const float *feat, float *out, const float *img, float *num, float *wsum,
