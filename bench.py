@@ -319,6 +319,64 @@ def feature_stats(ctx, dev, scene, peak, n_ch=64, reps=5):
             "render": leg(ms_r), "fuse": leg(ms_f, 4 * n_ch * touched), "launches": 1 + 2 * (reps + 1) + 3}
 
 
+def structure_stats(ctx, dev, scene, n_points=2_000_000):
+    """Widening row N4, reported beside the headline (not part of `value`): the LiDAR-guided structure operations on the
+    static octree with a seeded synthetic cloud (points scattered around the centres of randomly chosen leaves, sigma = 2
+    minimum voxel sizes): cloud binning, one proximity-subdivision round (threshold 1.5 s), grid tables + Eq. 1 prior on the
+    result, pruning at v < -9.5.  One-off operations, search- and fp64-bound: times and rates only, no roofline claim."""
+    import torch
+    t = dev.trees[0]
+    tree = scene.octrees[0]
+    if t.n_voxels == 0:
+        return None
+    code = t.code
+    level = (code >> 48) & 31
+    lmax = int(level.max())
+    side = float(tree.side)
+    s_min = side / (1 << lmax)
+    g = torch.Generator(device="cuda").manual_seed(11)
+    pick = torch.randint(0, t.n_voxels, (n_points,), device="cuda", generator=g)
+    # leaf centres from the code (input generation only: 3-bit groups -> lattice coordinates)
+    c = code[pick]
+    xyz = torch.zeros((n_points, 3), dtype=torch.float64, device="cuda")
+    for m in range(16):
+        grp = (c >> (45 - 3 * m)) & 7
+        for a, sh in enumerate((2, 1, 0)):
+            xyz[:, a] += ((grp >> sh) & 1).double() * (1 << (15 - m))
+    size = (1 << (16 - ((c >> 48) & 31))).double()
+    centre = torch.tensor([float(x) for x in tree.center], dtype=torch.float64, device="cuda")
+    pos = centre - 0.5 * side + (xyz + 0.5 * size[:, None]) * (side / 65536.0)
+    pts = (pos + torch.randn((n_points, 3), dtype=torch.float64, device="cuda", generator=g) * (2.0 * s_min)).float().contiguous()
+
+    def timed(fn):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record()
+        r = fn()
+        e1.record()
+        torch.cuda.synchronize()
+        return r, e0.elapsed_time(e1)
+    thr = 1.5 * s_min
+    cloud, ms_cloud = timed(lambda: ctx.cloud(pts, thr))
+    (new, split), ms_sub = timed(lambda: ctx.subdivide_near(cloud, code, tree.center, side, thr, min(lmax + 1, 16)))
+    new = new.contiguous()
+    grid, ms_grid = timed(lambda: ctx.grid(new))
+    s2 = 0.5 * s_min
+    cloud2, ms_cloud2 = timed(lambda: ctx.cloud(pts, 3.1 * s2))
+    dens, ms_prior = timed(lambda: ctx.density_prior(cloud2, new, tree.center, side, grid, s2))
+    geo = torch.empty((new.shape[0], 8), device="cuda")
+    grid.gather(dens, geo)
+    (kept, idx), ms_prune = timed(lambda: ctx.prune(new, geo, -9.5))
+    out = {"points": n_points, "leaves_in": t.n_voxels, "leaves_split": int(split.sum().item()), "leaves_out": int(new.shape[0]),
+           "grid_points": grid.n_points, "leaves_after_prune": int(kept.shape[0]),
+           "cloud_build_ms": ms_cloud, "subdivide_round_ms": ms_sub, "mleaves_per_s": t.n_voxels / ms_sub / 1e3,
+           "grid_tables_ms": ms_grid, "density_prior_ms": ms_prior, "mpoints_per_s": grid.n_points / ms_prior / 1e3,
+           "prune_ms": ms_prune}
+    for o in (cloud, cloud2, grid):
+        o.close()
+    return out
+
+
 def run_dvx(args):
     import torch
     import torch.distributed as dist
@@ -428,6 +486,7 @@ def run_dvx(args):
     clocks = sampler.stop() if sampler else None
     sort_stats = sort_throughput(ctx, cnt["pairs"] // n_cams, scene, W, H) if rank == 0 else None
     feat_stats = feature_stats(ctx, dev, scene, measured_peaks()[0]) if rank == 0 and not args.fwd_only else None
+    struct_stats = structure_stats(ctx, dev, scene) if rank == 0 and not args.fwd_only else None
     opt_stats = optimizer_step_stats(ctx, dev, grads, measured_peaks()[0]) if rank == 0 and not args.fwd_only else None
 
     if rank != 0:
@@ -480,7 +539,7 @@ def run_dvx(args):
                          "peak_source": "148 SMs x 128 fp32 lanes x %.0f MHz (nvidia-smi, under load)" % sm_mhz},
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": (0 if args.fwd_only else 12 * px_step),
                 "d2h_bytes_per_step": 20 * px_step, "ms_per_step": ms_e2e / args.steps},
-        "sort": sort_stats, "n2_optimizer_step": opt_stats, "n3_features": feat_stats,
+        "sort": sort_stats, "n2_optimizer_step": opt_stats, "n3_features": feat_stats, "n4_structure": struct_stats,
         "gpu_launches": launches, "clocks": clocks,
     }
     if not args.no_cpu_baseline and world == 1:

@@ -101,6 +101,16 @@ __device__ __forceinline__ int find_cell(const CloudView &c, uint64_t key) {
   return -1;
 }
 
+__device__ __forceinline__ uint32_t lower_cell(const CloudView &c, uint64_t key) {  // first occupied cell with key >= `key`
+  uint32_t lo = 0, hi = c.n_cells;
+  while (lo < hi) {
+    const uint32_t mid = (lo + hi) >> 1;
+    if (__ldg(c.cell_key + mid) < key) lo = mid + 1;
+    else hi = mid;
+  }
+  return lo;
+}
+
 // lattice coordinate -> octree frame, in R26's order of operations: (centre - side/2) + X * (side / 65536)
 __device__ __forceinline__ double lattice_pos(double center, double side, uint32_t X) {
   return __dadd_rn(__dsub_rn(center, __dmul_rn(0.5, side)), __dmul_rn((double)X, __ddiv_rn(side, 65536.0)));
@@ -135,8 +145,10 @@ __device__ double warp_min_box_dist2(const CloudView &c, const double lo[3], con
   int c0[3], c1[3];
   bool empty = c.n_cells == 0;
   for (int a = 0; a < 3; ++a) {
-    c0[a] = cell_of(lo[a] - reach, c.origin[a], c.cell) - 1;  // one cell of slack absorbs rounding in the cell index
-    c1[a] = cell_of(hi[a] + reach, c.origin[a], c.cell) + 1;
+    // a relative slack of 1e-9 (fp64 rounds at 1e-16) keeps a point at exactly `reach` on a cell boundary inside the range
+    const double eps = 1e-9 * (fabs(lo[a]) + fabs(hi[a]) + reach + c.cell);
+    c0[a] = cell_of(lo[a] - reach - eps, c.origin[a], c.cell);
+    c1[a] = cell_of(hi[a] + reach + eps, c.origin[a], c.cell);
     c0[a] = max(c0[a], 0);
     c1[a] = min(c1[a], (int)c.dims[a] - 1);
     if (c1[a] < c0[a]) empty = true;
@@ -146,16 +158,24 @@ __device__ double warp_min_box_dist2(const CloudView &c, const double lo[3], con
   const double reach2 = reach * reach;
   const uint64_t nx = (uint64_t)(c1[0] - c0[0] + 1), ny = (uint64_t)(c1[1] - c0[1] + 1), nz = (uint64_t)(c1[2] - c0[2] + 1);
   const uint64_t range = nx * ny * nz;
-  const bool by_list = range > (uint64_t)c.n_cells;  // fewer occupied cells than cells in the search box: walk the list
-  const uint64_t total = by_list ? (uint64_t)c.n_cells : range;
+  // the occupied cells of the z-slab [c0z, c1z] are one contiguous run of the sorted cell list: when that run is shorter
+  // than the search box has cells (coarse leaves, sparse clouds), walk the run instead of probing every cell of the box
+  const uint64_t plane = (uint64_t)c.dims[0] * c.dims[1];
+  uint32_t run_lo = 0, run_hi = 0xFFFFFFFFu;
+  if (range > 256) {  // small boxes (fine leaves, grid points) are probed cell by cell without looking at the run
+    run_lo = lower_cell(c, (uint64_t)c0[2] * plane);
+    run_hi = lower_cell(c, (uint64_t)(c1[2] + 1) * plane);
+  }
+  const bool by_list = range > (uint64_t)(run_hi - run_lo);
+  const uint64_t total = by_list ? (uint64_t)(run_hi - run_lo) : range;
   for (uint64_t base = 0; base < total; base += 32) {
     const uint64_t i = base + lane;
     int idx = -1;
     if (i < total) {
       if (by_list) {
-        const uint64_t key = __ldg(c.cell_key + i);
+        const uint64_t key = __ldg(c.cell_key + run_lo + i);
         const int cx = (int)(key % c.dims[0]), cy = (int)((key / c.dims[0]) % c.dims[1]), cz = (int)(key / ((uint64_t)c.dims[0] * c.dims[1]));
-        if (cx >= c0[0] && cx <= c1[0] && cy >= c0[1] && cy <= c1[1] && cz >= c0[2] && cz <= c1[2]) idx = (int)i;
+        if (cx >= c0[0] && cx <= c1[0] && cy >= c0[1] && cy <= c1[1] && cz >= c0[2] && cz <= c1[2]) idx = (int)(run_lo + i);
       } else {
         const int cx = c0[0] + (int)(i % nx), cy = c0[1] + (int)((i / nx) % ny), cz = c0[2] + (int)(i / (nx * ny));
         idx = find_cell(c, ((uint64_t)cz * c.dims[1] + cy) * c.dims[0] + cx);
