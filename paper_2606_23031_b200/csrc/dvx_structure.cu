@@ -40,11 +40,17 @@ __global__ void __launch_bounds__(ST_THREADS) cloud_bounds_kernel(const float *_
     lo[a] = __reduce_min_sync(0xffffffffu, lo[a]);
     hi[a] = __reduce_max_sync(0xffffffffu, hi[a]);
   }
+  __shared__ uint32_t s_mm[6];  // one set of global atomics per block, not per warp
+  if (threadIdx.x < 6) s_mm[threadIdx.x] = threadIdx.x < 3 ? 0xFFFFFFFFu : 0u;
+  __syncthreads();
   if ((threadIdx.x & 31) == 0)
     for (int a = 0; a < 3; ++a) {
-      atomicMin(mm + a, lo[a]);
-      atomicMax(mm + 3 + a, hi[a]);
+      atomicMin(s_mm + a, lo[a]);
+      atomicMax(s_mm + 3 + a, hi[a]);
     }
+  __syncthreads();
+  if (threadIdx.x < 3) atomicMin(mm + threadIdx.x, s_mm[threadIdx.x]);
+  else if (threadIdx.x < 6) atomicMax(mm + threadIdx.x, s_mm[threadIdx.x]);
 }
 
 __device__ __forceinline__ int cell_of(double x, double origin, double cell) {
