@@ -5,6 +5,7 @@
 #include <string.h>
 
 #include <string>
+#include <cstdlib>
 #include <vector>
 
 #include "dvx_internal.cuh"
@@ -61,6 +62,7 @@ struct dvx_frame {
   EventSet *es = nullptr;
   cudaEvent_t *ev = nullptr;  // = es->ev
   Buf eff_end, vnrm, sv_nrm;
+  Buf tile_cost, tile_order;  // pairs per tile [n_tiles]; the CTA -> tile launch order derived from it [2 n_tiles: result, intermediate]
   Buf w_row, w_vox, w_val;  // row N3: the compositing weights as CSR, built on demand
   uint64_t w_nnz = 0;
   dvx_sky sky = {0, 0, nullptr, nullptr};
@@ -68,6 +70,9 @@ struct dvx_frame {
 };
 
 namespace {
+
+// Experiments only: DVX_TILE_ORDER=0 launches the compositing CTAs in raster order instead of heaviest tile first.
+const bool g_tile_order_on = [] { const char *e = getenv("DVX_TILE_ORDER"); return !(e && e[0] == '0'); }();
 
 dvx_status fail(dvx_ctx *ctx, dvx_status code, const char *msg) {
   if (ctx) ctx->err = msg;
@@ -134,6 +139,7 @@ void frame_free(dvx_ctx *ctx, dvx_frame *f) {
   ctx_release(ctx, f->eff_end.p);
   ctx_release(ctx, f->vnrm.p);
   ctx_release(ctx, f->sv_nrm.p);
+  ctx_release(ctx, f->tile_cost.p); ctx_release(ctx, f->tile_order.p);
   ctx_release(ctx, f->w_row.p); ctx_release(ctx, f->w_vox.p); ctx_release(ctx, f->w_val.p);
   if (f->es) {
     f->es->did_backward = f->did_backward;
@@ -401,7 +407,8 @@ dvx_status dvx_render(dvx_ctx *ctx, const dvx_camera *cam, const dvx_octree *sta
             buf_alloc(ctx, f->actor_mask, sizeof(unsigned long long) * p.n_tiles) &&
             buf_alloc(ctx, f->range_beg, sizeof(uint32_t) * (size_t)p.n_buckets) &&
             buf_alloc(ctx, f->range_end, sizeof(uint32_t) * (size_t)p.n_buckets) &&
-            buf_alloc(ctx, f->counters, sizeof(unsigned long long) * CNT_N);
+            buf_alloc(ctx, f->counters, sizeof(unsigned long long) * CNT_N) &&
+            buf_alloc(ctx, f->tile_cost, sizeof(uint32_t) * (size_t)p.n_tiles) && buf_alloc(ctx, f->tile_order, sizeof(uint32_t) * 2 * (size_t)p.n_tiles);
   if (ok && saved)
     ok = buf_alloc(ctx, f->sv_rgbd, npix * 16) && buf_alloc(ctx, f->sv_T, npix * 4) && buf_alloc(ctx, f->sv_nused, npix * 4);
   if (ok && out.normal) {
@@ -455,7 +462,10 @@ dvx_status dvx_render(dvx_ctx *ctx, const dvx_camera *cam, const dvx_octree *sta
   int which = dvx_sort_launch(ka, va, kb, vb, P, key_bits, scr, st);
   CU(cudaMemsetAsync(f->range_beg.p, 0, sizeof(uint32_t) * (size_t)p.n_buckets, st));
   CU(cudaMemsetAsync(f->range_end.p, 0, sizeof(uint32_t) * (size_t)p.n_buckets, st));
-  dvx_ranges_launch(which ? kb : ka, P, p.rank_bits, (uint32_t *)f->range_beg.p, (uint32_t *)f->range_end.p, st);
+  CU(cudaMemsetAsync(f->tile_cost.p, 0, sizeof(uint32_t) * (size_t)p.n_tiles, st));
+  dvx_ranges_launch(which ? kb : ka, P, p.rank_bits, p.n_trees * 8u, (uint32_t *)f->range_beg.p, (uint32_t *)f->range_end.p,
+                    (uint32_t *)f->tile_cost.p, st);
+  dvx_tile_order_launch((const uint32_t *)f->tile_cost.p, p.n_tiles, (uint32_t *)f->tile_order.p, st);
   CU(cudaEventRecord(f->ev[3], st));
   f->ids.p = which ? vb : va;
   f->ids.bytes = P * 4;
@@ -466,6 +476,7 @@ dvx_status dvx_render(dvx_ctx *ctx, const dvx_camera *cam, const dvx_octree *sta
   A.p = p; A.trees = trees_d; A.fvox = (const FrameVox *)f->fvox.p; A.pxrect = (const ushort4 *)f->pxrect.p;
   A.ids = (const uint32_t *)f->ids.p; A.range_beg = (const uint32_t *)f->range_beg.p; A.range_end = (const uint32_t *)f->range_end.p;
   A.actor_mask = (const unsigned long long *)f->actor_mask.p;
+  A.tile_order = g_tile_order_on ? (const uint32_t *)f->tile_order.p : nullptr;
   A.rgb = out.rgb; A.depth = out.depth; A.alpha = out.alpha;
   A.sv_rgbd = (float *)f->sv_rgbd.p; A.sv_T = (float *)f->sv_T.p; A.sv_nused = (uint32_t *)f->sv_nused.p;
   A.counters = counters;
@@ -524,6 +535,7 @@ dvx_status dvx_backward_n(dvx_ctx *ctx, dvx_frame *f, const float *dL_drgb, cons
   A.p = p; A.trees = trees_d; A.fvox = (const FrameVox *)f->fvox.p; A.pxrect = (const ushort4 *)f->pxrect.p;
   A.ids = (const uint32_t *)f->ids.p; A.range_beg = (const uint32_t *)f->range_beg.p; A.range_end = (const uint32_t *)f->range_end.p;
   A.actor_mask = (const unsigned long long *)f->actor_mask.p;
+  A.tile_order = g_tile_order_on ? (const uint32_t *)f->tile_order.p : nullptr;
   A.sv_rgbd = (float *)f->sv_rgbd.p; A.sv_T = (float *)f->sv_T.p; A.sv_nused = (uint32_t *)f->sv_nused.p;
   A.counters = (unsigned long long *)f->counters.p;
   A.g_rgb = dL_drgb; A.g_depth = dL_ddepth; A.g_alpha = dL_dalpha; A.drgb = drgb;
@@ -923,6 +935,7 @@ dvx_status dvx_frame_weights(dvx_ctx *ctx, dvx_frame *f, dvx_weights *out) {
     A.p = p; A.trees = (const TreeFrame *)f->trees_d.p; A.fvox = (const FrameVox *)f->fvox.p; A.pxrect = (const ushort4 *)f->pxrect.p;
     A.ids = (const uint32_t *)f->ids.p; A.range_beg = (const uint32_t *)f->range_beg.p; A.range_end = (const uint32_t *)f->range_end.p;
     A.actor_mask = (const unsigned long long *)f->actor_mask.p;
+  A.tile_order = g_tile_order_on ? (const uint32_t *)f->tile_order.p : nullptr;
     A.counters = (unsigned long long *)f->counters.p;
     A.exp_row = row; A.exp_vox = (uint32_t *)f->w_vox.p; A.exp_w = (float *)f->w_val.p;
     dvx_composite_export_launch(A, st);

@@ -28,10 +28,14 @@
 
 namespace {
 
-constexpr int TILE_THREADS = 256;
+#ifndef DVX_TILE_SPLIT
+#define DVX_TILE_SPLIT 1  // CTAs per 16x16 tile (1, 2, 4 or 8): a CTA holds 8 / DVX_TILE_SPLIT of the tile's warps
+#endif
+constexpr int TILE_SPLIT = DVX_TILE_SPLIT;
+constexpr int TILE_THREADS = 256 / TILE_SPLIT;
 constexpr int TILE_WARPS = TILE_THREADS / 32;
 #ifndef DVX_TILE_MIN_CTAS
-#define DVX_TILE_MIN_CTAS 3
+#define DVX_TILE_MIN_CTAS (3 * DVX_TILE_SPLIT)
 #endif
 #ifndef DVX_RUN_SPLIT
 #define DVX_RUN_SPLIT 4  // backward: runs of one voxel are reduced in pieces of at most this many lanes (1, 2, 8, 16, 32 measured slower)
@@ -449,13 +453,14 @@ template <bool BWD, bool CNT, bool NRM, bool EXP = false>
 __global__ void __launch_bounds__(TILE_THREADS, DVX_TILE_MIN_CTAS) composite_tile_kernel(const __grid_constant__ CompositeArgs A) {
   __shared__ WarpQueue<BWD, NRM> s_queue[TILE_WARPS];
   const FrameParams &p = A.p;
-  const int tile = blockIdx.x;
-  const int warp = threadIdx.x >> 5;
+  const int tile = A.tile_order ? (int)__ldg(A.tile_order + blockIdx.x / TILE_SPLIT) : (int)(blockIdx.x / TILE_SPLIT);
+  const int warp_l = threadIdx.x >> 5;                                  // warp of this CTA
+  const int warp = (int)(blockIdx.x % TILE_SPLIT) * TILE_WARPS + warp_l;  // warp of the tile: which 4x8 pixel block
   const int lane = threadIdx.x & 31;
   const uint32_t lt = (1u << lane) - 1u;
   const int wu0 = (tile % p.tiles_x) * DVX_TILE + (warp % WARPS_X) * WARP_W;   // pixel of lane 0 of this warp
   const int wv0 = (tile / p.tiles_x) * DVX_TILE + (warp / WARPS_X) * WARP_H;
-  WarpQueue<BWD, NRM> &Q = s_queue[warp];
+  WarpQueue<BWD, NRM> &Q = s_queue[warp_l];
   const int u = wu0 + lane % WARP_W, v = wv0 + lane / WARP_W;
   const bool inside = u < (int)p.width && v < (int)p.height;
   const size_t pix = (size_t)v * p.width + u;
@@ -718,7 +723,7 @@ __global__ void __launch_bounds__(TILE_THREADS, DVX_TILE_MIN_CTAS) composite_til
 void dvx_composite_export_launch(const CompositeArgs &a, cudaStream_t st) {
   if (a.p.n_tiles == 0) return;
   DVX_COUNT_LAUNCH(1);
-  composite_tile_kernel<false, false, false, true><<<a.p.n_tiles, TILE_THREADS, 0, st>>>(a);
+  composite_tile_kernel<false, false, false, true><<<a.p.n_tiles * TILE_SPLIT, TILE_THREADS, 0, st>>>(a);
 }
 
 void dvx_composite_tile_launch(const CompositeArgs &a, bool backward, cudaStream_t st) {
@@ -727,13 +732,13 @@ void dvx_composite_tile_launch(const CompositeArgs &a, bool backward, cudaStream
   const bool cnt = (a.p.flags & DVX_FLAG_COUNTERS) != 0;
   const bool nrm = backward ? (a.g_normal != nullptr) : (a.normal != nullptr);  // normal map requested (O11)
   if (backward) {
-    if (nrm) composite_tile_kernel<true, false, true><<<a.p.n_tiles, TILE_THREADS, 0, st>>>(a);
-    else composite_tile_kernel<true, false, false><<<a.p.n_tiles, TILE_THREADS, 0, st>>>(a);
+    if (nrm) composite_tile_kernel<true, false, true><<<a.p.n_tiles * TILE_SPLIT, TILE_THREADS, 0, st>>>(a);
+    else composite_tile_kernel<true, false, false><<<a.p.n_tiles * TILE_SPLIT, TILE_THREADS, 0, st>>>(a);
   } else if (nrm) {
-    composite_tile_kernel<false, false, true><<<a.p.n_tiles, TILE_THREADS, 0, st>>>(a);
+    composite_tile_kernel<false, false, true><<<a.p.n_tiles * TILE_SPLIT, TILE_THREADS, 0, st>>>(a);
   } else if (cnt) {
-    composite_tile_kernel<false, true, false><<<a.p.n_tiles, TILE_THREADS, 0, st>>>(a);
+    composite_tile_kernel<false, true, false><<<a.p.n_tiles * TILE_SPLIT, TILE_THREADS, 0, st>>>(a);
   } else {
-    composite_tile_kernel<false, false, false><<<a.p.n_tiles, TILE_THREADS, 0, st>>>(a);
+    composite_tile_kernel<false, false, false><<<a.p.n_tiles * TILE_SPLIT, TILE_THREADS, 0, st>>>(a);
   }
 }

@@ -60,6 +60,7 @@ struct CompositeArgs {
   const uint32_t *range_beg;   // [n_buckets]
   const uint32_t *range_end;   // [n_buckets]
   const unsigned long long *actor_mask;  // [n_tiles]
+  const uint32_t *tile_order;  // [n_tiles] CTA -> tile, heaviest tiles first, or NULL (CTA i serves tile i)
   float *rgb, *depth, *alpha;  // caller's images
   float *sv_rgbd;              // [H*W][4] saved C_final, D_final (frame-owned; may be NULL when nothing is saved)
   float *sv_T;                 // [H*W]
@@ -109,8 +110,9 @@ void dvx_normal_backward_launch(const FrameParams &p, const TreeFrame *trees, co
 void dvx_emit_pairs_launch(const FrameParams &p, const TreeFrame *trees, const uint8_t *octmask, const ushort4 *pxrect,
                            const FrameVox *fvox, uint64_t *keys, uint32_t *vals, unsigned long long capacity,
                            unsigned long long *counters, cudaStream_t st);
-void dvx_ranges_launch(const uint64_t *keys, uint64_t n, uint32_t rank_bits, uint32_t *range_beg, uint32_t *range_end,
-                       cudaStream_t st);
+void dvx_ranges_launch(const uint64_t *keys, uint64_t n, uint32_t rank_bits, uint32_t buckets_per_tile, uint32_t *range_beg,
+                       uint32_t *range_end, uint32_t *tile_cost, cudaStream_t st);
+void dvx_tile_order_launch(const uint32_t *tile_cost, uint32_t n_tiles, uint32_t *tile_order /* [2 n_tiles] */, cudaStream_t st);
 void dvx_sh_backward_launch(const FrameParams &p, const TreeFrame *trees, const FrameVox *fvox, const ushort4 *pxrect,
                             const float *drgb, cudaStream_t st);
 

@@ -355,14 +355,84 @@ __global__ void __launch_bounds__(PRE_THREADS) emit_pairs_kernel(FrameParams p, 
   }
 }
 
-// range[bucket] = [begin, end) in the sorted pair array, by boundary detection (buffers pre-zeroed: empty = [0,0))
-__global__ void ranges_kernel(const uint64_t *keys, uint64_t n, uint32_t rank_bits, uint32_t *range_beg,
-                              uint32_t *range_end) {
+// range[bucket] = [begin, end) in the sorted pair array, by boundary detection (buffers pre-zeroed: empty = [0,0)).
+// tile_cost[tile] (pre-zeroed) receives the tile's pair count as sum(end) - sum(begin) over its buckets, in u32 arithmetic.
+__global__ void ranges_kernel(const uint64_t *keys, uint64_t n, uint32_t rank_bits, uint32_t buckets_per_tile,
+                              uint32_t *range_beg, uint32_t *range_end, uint32_t *tile_cost) {
   uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
   uint64_t b = keys[i] >> rank_bits;
-  if (i == 0 || (keys[i - 1] >> rank_bits) != b) range_beg[b] = (uint32_t)i;
-  if (i + 1 == n || (keys[i + 1] >> rank_bits) != b) range_end[b] = (uint32_t)(i + 1);
+  const bool first = i == 0 || (keys[i - 1] >> rank_bits) != b, last = i + 1 == n || (keys[i + 1] >> rank_bits) != b;
+  if (first) range_beg[b] = (uint32_t)i;
+  if (last) range_end[b] = (uint32_t)(i + 1);
+  if (tile_cost && (first || last)) {
+    const uint32_t tile = (uint32_t)b / buckets_per_tile;
+    if (first && last) atomicAdd(tile_cost + tile, 1u);
+    else atomicAdd(tile_cost + tile, first ? 0u - (uint32_t)i : (uint32_t)(i + 1));
+  }
+}
+
+// Launch order of the compositing CTAs: tiles by descending pair count (longest processing time first), so that the heavy
+// tiles do not end up as the kernel's tail.  One CTA; the cost is quantised to 12 bits and sorted by a stable two-pass
+// LSD counting sort (6 bits each), so equal-cost tiles keep raster order and the result is deterministic.
+// tile_order holds 2 n_tiles entries: the second half is the intermediate order, the first half the result.
+constexpr int ORDER_THREADS = 1024, ORDER_DIGITS = 64;
+__global__ void __launch_bounds__(ORDER_THREADS) tile_order_kernel(const uint32_t *tile_cost, uint32_t n_tiles, uint32_t *tile_order) {
+  __shared__ uint32_t s_cnt[32][ORDER_DIGITS + 1];
+  __shared__ uint32_t s_base[ORDER_DIGITS];
+  __shared__ uint32_t s_warp[32];
+  __shared__ uint32_t s_max;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  uint32_t mx = 0;
+  for (uint32_t t = tid; t < n_tiles; t += ORDER_THREADS) mx = max(mx, tile_cost[t]);
+  mx = __reduce_max_sync(0xffffffffu, mx);
+  if (lane == 0) s_warp[warp] = mx;
+  __syncthreads();
+  if (warp == 0) {
+    mx = __reduce_max_sync(0xffffffffu, s_warp[lane]);
+    if (lane == 0) s_max = mx;
+  }
+  __syncthreads();
+  const unsigned long long den = (unsigned long long)s_max + 1ull;
+  for (int pass = 0; pass < 2; ++pass) {
+    const uint32_t shift = 6u * pass;
+    const uint32_t *src = pass ? tile_order + n_tiles : nullptr;  // pass 0 reads the tiles in raster order
+    uint32_t *dst = pass ? tile_order : tile_order + n_tiles;
+    if (tid < ORDER_DIGITS) s_base[tid] = 0;
+    __syncthreads();
+    for (uint32_t t = tid; t < n_tiles; t += ORDER_THREADS) {  // key 0 = the most expensive tiles
+      const uint32_t key = 4095u - (uint32_t)(((unsigned long long)tile_cost[t] * 4096ull) / den);
+      atomicAdd(&s_base[(key >> shift) & 63u], 1u);
+    }
+    __syncthreads();
+    if (tid == 0) {
+      uint32_t run = 0;
+      for (int c = 0; c < ORDER_DIGITS; ++c) { const uint32_t v = s_base[c]; s_base[c] = run; run += v; }
+    }
+    for (uint32_t c0 = 0; c0 < n_tiles; c0 += ORDER_THREADS) {
+      for (int i = tid; i < 32 * (ORDER_DIGITS + 1); i += ORDER_THREADS) (&s_cnt[0][0])[i] = 0;
+      __syncthreads();
+      const bool valid = c0 + tid < n_tiles;
+      uint32_t t = 0, dig = ORDER_DIGITS;
+      if (valid) {
+        t = src ? src[c0 + tid] : c0 + tid;
+        dig = ((4095u - (uint32_t)(((unsigned long long)tile_cost[t] * 4096ull) / den)) >> shift) & 63u;
+      }
+      const uint32_t same = __match_any_sync(0xffffffffu, dig);
+      const uint32_t rank = __popc(same & ((1u << lane) - 1u));
+      if (rank == 0) s_cnt[warp][dig] = __popc(same);
+      __syncthreads();
+      if (tid < ORDER_DIGITS) {
+        uint32_t run = s_base[tid];
+        for (int w = 0; w < 32; ++w) { const uint32_t v = s_cnt[w][tid]; s_cnt[w][tid] = run; run += v; }
+        s_base[tid] = run;
+      }
+      __syncthreads();
+      if (valid) dst[s_cnt[warp][dig] + rank] = t;
+      __syncthreads();
+    }
+    __threadfence_block();
+  }
 }
 
 // ------------------------------------------------------------------ step 5b: dL/dk_{v,i} = Y_i(dir_v) dL/drgb_v
@@ -502,9 +572,12 @@ void dvx_emit_pairs_launch(const FrameParams &p, const TreeFrame *trees, const u
     if (p.v_total) { DVX_COUNT_LAUNCH(1); emit_pairs_kernel<<<blocks_for(p.v_total, PRE_THREADS), PRE_THREADS, 0, st>>>(p, trees, octmask, pxrect, fvox, keys, vals,
                                                                                    capacity, counters); }
 }
-void dvx_ranges_launch(const uint64_t *keys, uint64_t n, uint32_t rank_bits, uint32_t *range_beg, uint32_t *range_end,
-                       cudaStream_t st) {
-  if (n) { DVX_COUNT_LAUNCH(1); ranges_kernel<<<blocks_for(n, 256), 256, 0, st>>>(keys, n, rank_bits, range_beg, range_end); }
+void dvx_ranges_launch(const uint64_t *keys, uint64_t n, uint32_t rank_bits, uint32_t buckets_per_tile, uint32_t *range_beg,
+                       uint32_t *range_end, uint32_t *tile_cost, cudaStream_t st) {
+  if (n) { DVX_COUNT_LAUNCH(1); ranges_kernel<<<blocks_for(n, 256), 256, 0, st>>>(keys, n, rank_bits, buckets_per_tile, range_beg, range_end, tile_cost); }
+}
+void dvx_tile_order_launch(const uint32_t *tile_cost, uint32_t n_tiles, uint32_t *tile_order, cudaStream_t st) {
+  if (n_tiles) { DVX_COUNT_LAUNCH(1); tile_order_kernel<<<1, ORDER_THREADS, 0, st>>>(tile_cost, n_tiles, tile_order); }
 }
 void dvx_sh_backward_launch(const FrameParams &p, const TreeFrame *trees, const FrameVox *fvox, const ushort4 *pxrect,
                             const float *drgb, cudaStream_t st) {
