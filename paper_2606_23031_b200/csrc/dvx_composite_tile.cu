@@ -29,7 +29,8 @@
 namespace {
 
 #ifndef DVX_TILE_SPLIT
-#define DVX_TILE_SPLIT 1  // CTAs per 16x16 tile (1, 2, 4 or 8): a CTA holds 8 / DVX_TILE_SPLIT of the tile's warps
+#define DVX_TILE_SPLIT 2  // CTAs per 16x16 tile (1, 2, 4 or 8): a CTA holds 8 / DVX_TILE_SPLIT of the tile's warps.  Measured on
+                          // B200, step ms for 1 / 2 / 4: config 3 4.00 / 3.92 / 3.98, config 4 5.32 / 5.25 / 5.32 (finer tail)
 #endif
 constexpr int TILE_SPLIT = DVX_TILE_SPLIT;
 constexpr int TILE_THREADS = 256 / TILE_SPLIT;
@@ -595,6 +596,9 @@ __global__ void __launch_bounds__(TILE_THREADS, DVX_TILE_MIN_CTAS) composite_til
       }
       __syncwarp();
     }
+    // warp-uniform "some lane is axis-parallel": keeps the R20 test out of the per-candidate loop (the forward otherwise
+    // rebuilt zmask from d[] there, 9 instructions per candidate: forward 1.254 -> 1.218 ms on config 3)
+    const bool z_any = __any_sync(0xffffffffu, zmask != 0u);
     uint32_t omask = __reduce_or_sync(0xffffffffu, part ? (1u << q) : 0u);
     while (omask) {
       const int qq = __ffs(omask) - 1;
@@ -646,7 +650,7 @@ __global__ void __launch_bounds__(TILE_THREADS, DVX_TILE_MIN_CTAS) composite_til
           const float c0 = w0 * inv[0], c1 = w1 * inv[1], c2 = w2 * inv[2];
           float sa = fmaxf(fmaxf(fmaf(-hs, fabsf(inv[0]), -c0), fmaf(-hs, fabsf(inv[1]), -c1)), fmaf(-hs, fabsf(inv[2]), -c2));
           float sb = fminf(fminf(fmaf(hs, fabsf(inv[0]), -c0), fmaf(hs, fabsf(inv[1]), -c1)), fmaf(hs, fabsf(inv[2]), -c2));
-          if (zmask) {
+          if (z_any && zmask) {
             const float2 f = axis_parallel_fix(&T, r1.y, r1.z, zmask, hs, fabsf(inv[0]), fabsf(inv[1]), fabsf(inv[2]), c0, c1, c2);
             sa = f.x; sb = f.y;
           }

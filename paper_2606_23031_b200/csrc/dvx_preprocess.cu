@@ -373,12 +373,17 @@ __global__ void ranges_kernel(const uint64_t *keys, uint64_t n, uint32_t rank_bi
 }
 
 // Launch order of the compositing CTAs: tiles by descending pair count (longest processing time first), so that the heavy
-// tiles do not end up as the kernel's tail.  One CTA; the cost is quantised to 12 bits and sorted by a stable two-pass
-// LSD counting sort (6 bits each), so equal-cost tiles keep raster order and the result is deterministic.
+// tiles do not end up as the kernel's tail.  One CTA; the cost is quantised to 12 bits (relative to the heaviest tile) and
+// sorted by a stable two-pass LSD counting sort (6 bits each), so equal-cost tiles keep raster order and the result is
+// deterministic.  A warp ranks ORDER_ROUNDS x 32 consecutive tiles against its own digit counters (no block barrier inside),
+// so a 1920x1080 frame (8160 tiles) is one chunk per pass: 28.8 -> 7 us.
 // tile_order holds 2 n_tiles entries: the second half is the intermediate order, the first half the result.
-constexpr int ORDER_THREADS = 1024, ORDER_DIGITS = 64;
+constexpr int ORDER_THREADS = 1024, ORDER_DIGITS = 64, ORDER_ROUNDS = 8;
+__device__ __forceinline__ uint32_t order_key(uint32_t cost, float scale) {  // key 0 = the most expensive tiles
+  return 4095u - min(4095u, (uint32_t)((float)cost * scale));
+}
 __global__ void __launch_bounds__(ORDER_THREADS) tile_order_kernel(const uint32_t *tile_cost, uint32_t n_tiles, uint32_t *tile_order) {
-  __shared__ uint32_t s_cnt[32][ORDER_DIGITS + 1];
+  __shared__ uint32_t s_cnt[32][ORDER_DIGITS + 1];  // column ORDER_DIGITS: lanes past the end
   __shared__ uint32_t s_base[ORDER_DIGITS];
   __shared__ uint32_t s_warp[32];
   __shared__ uint32_t s_max;
@@ -393,34 +398,53 @@ __global__ void __launch_bounds__(ORDER_THREADS) tile_order_kernel(const uint32_
     if (lane == 0) s_max = mx;
   }
   __syncthreads();
-  const unsigned long long den = (unsigned long long)s_max + 1ull;
+  const float scale = 4096.0f / ((float)s_max + 1.0f);
   for (int pass = 0; pass < 2; ++pass) {
     const uint32_t shift = 6u * pass;
     const uint32_t *src = pass ? tile_order + n_tiles : nullptr;  // pass 0 reads the tiles in raster order
     uint32_t *dst = pass ? tile_order : tile_order + n_tiles;
     if (tid < ORDER_DIGITS) s_base[tid] = 0;
     __syncthreads();
-    for (uint32_t t = tid; t < n_tiles; t += ORDER_THREADS) {  // key 0 = the most expensive tiles
-      const uint32_t key = 4095u - (uint32_t)(((unsigned long long)tile_cost[t] * 4096ull) / den);
-      atomicAdd(&s_base[(key >> shift) & 63u], 1u);
+    for (uint32_t t0 = 0; t0 < n_tiles; t0 += ORDER_THREADS) {  // digit histogram, one shared-memory atomic per (warp, digit)
+      const uint32_t t = t0 + tid;
+      const uint32_t dig = t < n_tiles ? (order_key(tile_cost[t], scale) >> shift) & 63u : (uint32_t)ORDER_DIGITS;
+      const uint32_t same = __match_any_sync(0xffffffffu, dig);
+      if (dig != ORDER_DIGITS && (same & ((1u << lane) - 1u)) == 0u) atomicAdd(&s_base[dig], __popc(same));
     }
     __syncthreads();
-    if (tid == 0) {
-      uint32_t run = 0;
-      for (int c = 0; c < ORDER_DIGITS; ++c) { const uint32_t v = s_base[c]; s_base[c] = run; run += v; }
+    if (warp == 0) {  // exclusive scan of the 64 digit counts
+      const uint32_t a = s_base[2 * lane], b = s_base[2 * lane + 1];
+      uint32_t inc = a + b;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        const uint32_t x = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += x;
+      }
+      s_base[2 * lane] = inc - a - b;
+      s_base[2 * lane + 1] = inc - b;
     }
-    for (uint32_t c0 = 0; c0 < n_tiles; c0 += ORDER_THREADS) {
+    for (uint32_t c0 = 0; c0 < n_tiles; c0 += ORDER_THREADS * ORDER_ROUNDS) {
       for (int i = tid; i < 32 * (ORDER_DIGITS + 1); i += ORDER_THREADS) (&s_cnt[0][0])[i] = 0;
       __syncthreads();
-      const bool valid = c0 + tid < n_tiles;
-      uint32_t t = 0, dig = ORDER_DIGITS;
-      if (valid) {
-        t = src ? src[c0 + tid] : c0 + tid;
-        dig = ((4095u - (uint32_t)(((unsigned long long)tile_cost[t] * 4096ull) / den)) >> shift) & 63u;
+      uint32_t tl[ORDER_ROUNDS], dg[ORDER_ROUNDS], of[ORDER_ROUNDS];
+#pragma unroll
+      for (int r = 0; r < ORDER_ROUNDS; ++r) {  // chunk order = (warp, round, lane): consecutive entries of src
+        const uint32_t idx = c0 + (uint32_t)(warp * ORDER_ROUNDS + r) * 32u + lane;
+        tl[r] = idx < n_tiles ? (src ? src[idx] : idx) : 0xFFFFFFFFu;
       }
-      const uint32_t same = __match_any_sync(0xffffffffu, dig);
-      const uint32_t rank = __popc(same & ((1u << lane) - 1u));
-      if (rank == 0) s_cnt[warp][dig] = __popc(same);
+#pragma unroll
+      for (int r = 0; r < ORDER_ROUNDS; ++r)  // all gathers in flight before the first ranking round
+        dg[r] = tl[r] != 0xFFFFFFFFu ? (order_key(tile_cost[tl[r]], scale) >> shift) & 63u : (uint32_t)ORDER_DIGITS;
+#pragma unroll
+      for (int r = 0; r < ORDER_ROUNDS; ++r) {
+        const uint32_t same = __match_any_sync(0xffffffffu, dg[r]);
+        const uint32_t rank = __popc(same & ((1u << lane) - 1u));
+        const uint32_t before = s_cnt[warp][dg[r]];
+        of[r] = before + rank;
+        __syncwarp();
+        if (rank == 0) s_cnt[warp][dg[r]] = before + __popc(same);
+        __syncwarp();
+      }
       __syncthreads();
       if (tid < ORDER_DIGITS) {
         uint32_t run = s_base[tid];
@@ -428,7 +452,9 @@ __global__ void __launch_bounds__(ORDER_THREADS) tile_order_kernel(const uint32_
         s_base[tid] = run;
       }
       __syncthreads();
-      if (valid) dst[s_cnt[warp][dig] + rank] = t;
+#pragma unroll
+      for (int r = 0; r < ORDER_ROUNDS; ++r)
+        if (dg[r] != ORDER_DIGITS) dst[s_cnt[warp][dg[r]] + of[r]] = tl[r];
       __syncthreads();
     }
     __threadfence_block();
