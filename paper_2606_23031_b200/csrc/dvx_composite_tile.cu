@@ -58,14 +58,14 @@ struct __align__(16) EntryRec {
   float m0[3];    // centre - t0 d0 (tree frame)
   float hs;       // half edge length
   uint32_t id;    // global voxel id
-  uint32_t level;
+  uint32_t meta;  // tree << 8 | level << 16: the item's meta word, composed once per (warp, entry)
   uint32_t pad;
 };
 
 // One queued (pixel, voxel) hit: 48 bytes, written with three 16-byte stores in phase A.
 struct __align__(16) Item {
   uint32_t id;        // global voxel id
-  uint32_t meta;      // pixel lane | tree << 8 | level << 16
+  uint32_t meta;      // tree << 8 | level << 16
   float ca, cb;       // clipped sub-segment, relative to t0 (O4, R1)
   float w[3];         // x(tau) - centre = s' d + w
   float mid;          // (a + b) / 2, absolute ray distance (depth, R9)
@@ -100,6 +100,11 @@ __device__ __forceinline__ float ex2_approx(float x) {
   float y;
   asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
   return y;
+}
+__device__ __forceinline__ uint32_t lanemask_lt() {  // one S2R where it is used; kept in a register it was rebuilt from tid.x
+  uint32_t m;
+  asm("mov.u32 %0, %%lanemask_lt;" : "=r"(m));
+  return m;
 }
 __device__ __forceinline__ double shfl_double(double v, int src) {
   int lo = __double2loint(v), hi = __double2hiint(v);
@@ -458,7 +463,6 @@ __global__ void __launch_bounds__(TILE_THREADS, DVX_TILE_MIN_CTAS) composite_til
   const int warp_l = threadIdx.x >> 5;                                  // warp of this CTA
   const int warp = (int)(blockIdx.x % TILE_SPLIT) * TILE_WARPS + warp_l;  // warp of the tile: which 4x8 pixel block
   const int lane = threadIdx.x & 31;
-  const uint32_t lt = (1u << lane) - 1u;
   const int wu0 = (tile % p.tiles_x) * DVX_TILE + (warp % WARPS_X) * WARP_W;   // pixel of lane 0 of this warp
   const int wv0 = (tile / p.tiles_x) * DVX_TILE + (warp / WARPS_X) * WARP_H;
   WarpQueue<BWD, NRM> &Q = s_queue[warp_l];
@@ -605,11 +609,11 @@ __global__ void __launch_bounds__(TILE_THREADS, DVX_TILE_MIN_CTAS) composite_til
       omask &= omask - 1;
       const size_t bucket = ((size_t)tile * p.n_trees + t) * 8 + qq;
       const uint32_t beg = __ldg(A.range_beg + bucket), end = __ldg(A.range_end + bucket);
-      uint32_t active = (part && q == qq) ? 1u : 0u;
       uint32_t c_l = beg;
       if (t == 0 && cur0 != NONE) c_l = cur0;
-      uint32_t pos = warp_min_u32(active ? c_l : NONE);
-      while (pos < end && __any_sync(0xffffffffu, active != 0u)) {
+      uint32_t c_t = (part && q == qq) ? c_l : NONE;  // first entry this pixel still tests; NONE = not (or no longer) walking
+      uint32_t pos = warp_min_u32(c_t);
+      while (pos < end && __any_sync(0xffffffffu, c_t != NONE)) {
         const uint32_t n = min(32u, end - pos);
         // -- lane = entry: pre-filter and fp64 centre decomposition
         bool c = false;
@@ -632,7 +636,7 @@ __global__ void __launch_bounds__(TILE_THREADS, DVX_TILE_MIN_CTAS) composite_til
             rec.t0 = t0;
             rec.m0[0] = (float)(cx - t0d * d0x); rec.m0[1] = (float)(cy - t0d * d0y); rec.m0[2] = (float)(cz - t0d * d0z);
             rec.hs = (float)(hc * (double)size);
-            rec.id = id; rec.level = lv; rec.pad = 0;
+            rec.id = id; rec.meta = (t << 8) | (lv << 16); rec.pad = 0;
             Q.ent[lane] = rec;
           }
         }
@@ -644,29 +648,29 @@ __global__ void __launch_bounds__(TILE_THREADS, DVX_TILE_MIN_CTAS) composite_til
           cand &= cand - 1;
           const uint32_t ei = pos + j;
           const float4 r0 = *reinterpret_cast<const float4 *>(&Q.ent[j]);          // t0, m0
-          const uint4 r1 = *(reinterpret_cast<const uint4 *>(&Q.ent[j]) + 1);      // hs, id, level
+          const uint4 r1 = *(reinterpret_cast<const uint4 *>(&Q.ent[j]) + 1);      // hs, id, meta
           const float hs = __uint_as_float(r1.x);
           const float w0 = fmaf(r0.x, e[0], -r0.y), w1 = fmaf(r0.x, e[1], -r0.z), w2 = fmaf(r0.x, e[2], -r0.w);
           const float c0 = w0 * inv[0], c1 = w1 * inv[1], c2 = w2 * inv[2];
           float sa = fmaxf(fmaxf(fmaf(-hs, fabsf(inv[0]), -c0), fmaf(-hs, fabsf(inv[1]), -c1)), fmaf(-hs, fabsf(inv[2]), -c2));
           float sb = fminf(fminf(fmaf(hs, fabsf(inv[0]), -c0), fmaf(hs, fabsf(inv[1]), -c1)), fmaf(hs, fabsf(inv[2]), -c2));
           if (z_any && zmask) {
-            const float2 f = axis_parallel_fix(&T, r1.y, r1.z, zmask, hs, fabsf(inv[0]), fabsf(inv[1]), fabsf(inv[2]), c0, c1, c2);
+            const float2 f = axis_parallel_fix(&T, r1.y, r1.z >> 16, zmask, hs, fabsf(inv[0]), fabsf(inv[1]), fabsf(inv[2]), c0, c1, c2);
             sa = f.x; sb = f.y;
           }
           const float lo_r = lo - r0.x, hi_r = hi - r0.x;
           const float ca = fmaxf(sa, lo_r), cb = fminf(sb, hi_r);       // R1: clip to the interval
-          const bool live = active != 0u && c_l <= ei && sb > sa;       // this pixel's ray meets the voxel
+          const bool live = c_t <= ei && sb > sa;                       // this pixel's ray meets the voxel
           const bool emit = live && cb > ca;
-          if (CNT) q_test += (active != 0u && c_l <= ei) ? 1u : 0u;
+          if (CNT) q_test += (c_t <= ei) ? 1u : 0u;
           // gate: the voxel reaches beyond the interval end (it may own a second piece after the box), or starts beyond it
-          if (live && sb > hi_r) { active = 0u; c_l = ei; }
+          if (live && sb > hi_r) { c_t = NONE; c_l = ei; }
           const uint32_t mk = __ballot_sync(0xffffffffu, emit);
           if (mk) {
             if (emit) {
-              const int rel_at = n_items + __popc(mk & lt);
+              const int rel_at = n_items + __popc(mk & lanemask_lt());
               float4 *it = reinterpret_cast<float4 *>(&Q.item[(head + rel_at) & (QCAP - 1)]);
-              it[0] = make_float4(__uint_as_float(r1.y), __uint_as_float((uint32_t)lane | (t << 8) | (r1.z << 16)), ca, cb);
+              it[0] = make_float4(__uint_as_float(r1.y), __uint_as_float(r1.z), ca, cb);
               it[1] = make_float4(w0, w1, w2, r0.x + 0.5f * (ca + cb));
               it[2] = make_float4(d[0], d[1], d[2], 0.f);
               my_bits |= 1ull << rel_at;
@@ -674,7 +678,7 @@ __global__ void __launch_bounds__(TILE_THREADS, DVX_TILE_MIN_CTAS) composite_til
             n_items += __popc(mk);
             if (n_items >= 32) {
               flush_batch<BWD, NRM, EXP>(A, lane, Q, n_items, head, my_bits, S);
-              if (S.done) active = 0u;
+              if (S.done) c_t = NONE;
             }
           }
         }
@@ -683,7 +687,7 @@ __global__ void __launch_bounds__(TILE_THREADS, DVX_TILE_MIN_CTAS) composite_til
       }
       if (CNT && A.eff_end && lane == 0) atomicMax(A.eff_end + bucket, min(pos, end));
       if (part && q == qq) {
-        if (active) c_l = end;          // walked off the list: nothing left for later intervals either
+        if (c_t != NONE) c_l = end;     // walked off the list: nothing left for later intervals either
         if (t == 0) cur0 = c_l;
       }
     }
