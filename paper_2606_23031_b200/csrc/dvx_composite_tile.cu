@@ -56,9 +56,9 @@ constexpr float LOG2E = 1.4426950408889634f;
 struct __align__(16) EntryRec {
   float t0;       // distance of the voxel centre along the warp's reference direction d0
   float m0[3];    // centre - t0 d0 (tree frame)
+  uint32_t id;    // global voxel id                 } same order as the head of Item: phase A's item store takes the
+  uint32_t meta;  // tree << 8 | level << 16         } pair as it was loaded
   float hs;       // half edge length
-  uint32_t id;    // global voxel id
-  uint32_t meta;  // tree << 8 | level << 16: the item's meta word, composed once per (warp, entry)
   uint32_t pad;
 };
 
@@ -87,7 +87,7 @@ struct WarpQueue {
 struct Pix {
   float C0, C1, C2, D, T;
   uint32_t n_used;
-  bool done;
+  uint32_t done;  // 0 / 1 (a full register: as a bool it was packed into a byte lane with PRMT)
   float gC0, gC1, gC2, gD, gA, Xtot, Xpre, T_final;  // backward only
   uint32_t n_stop;
   float N0, N1, N2;     // normal map (O11), forward
@@ -648,14 +648,14 @@ __global__ void __launch_bounds__(TILE_THREADS, DVX_TILE_MIN_CTAS) composite_til
           cand &= cand - 1;
           const uint32_t ei = pos + j;
           const float4 r0 = *reinterpret_cast<const float4 *>(&Q.ent[j]);          // t0, m0
-          const uint4 r1 = *(reinterpret_cast<const uint4 *>(&Q.ent[j]) + 1);      // hs, id, meta
-          const float hs = __uint_as_float(r1.x);
+          const uint4 r1 = *(reinterpret_cast<const uint4 *>(&Q.ent[j]) + 1);      // id, meta, hs
+          const float hs = __uint_as_float(r1.z);
           const float w0 = fmaf(r0.x, e[0], -r0.y), w1 = fmaf(r0.x, e[1], -r0.z), w2 = fmaf(r0.x, e[2], -r0.w);
           const float c0 = w0 * inv[0], c1 = w1 * inv[1], c2 = w2 * inv[2];
           float sa = fmaxf(fmaxf(fmaf(-hs, fabsf(inv[0]), -c0), fmaf(-hs, fabsf(inv[1]), -c1)), fmaf(-hs, fabsf(inv[2]), -c2));
           float sb = fminf(fminf(fmaf(hs, fabsf(inv[0]), -c0), fmaf(hs, fabsf(inv[1]), -c1)), fmaf(hs, fabsf(inv[2]), -c2));
           if (z_any && zmask) {
-            const float2 f = axis_parallel_fix(&T, r1.y, r1.z >> 16, zmask, hs, fabsf(inv[0]), fabsf(inv[1]), fabsf(inv[2]), c0, c1, c2);
+            const float2 f = axis_parallel_fix(&T, r1.x, r1.y >> 16, zmask, hs, fabsf(inv[0]), fabsf(inv[1]), fabsf(inv[2]), c0, c1, c2);
             sa = f.x; sb = f.y;
           }
           const float lo_r = lo - r0.x, hi_r = hi - r0.x;
@@ -670,7 +670,7 @@ __global__ void __launch_bounds__(TILE_THREADS, DVX_TILE_MIN_CTAS) composite_til
             if (emit) {
               const int rel_at = n_items + __popc(mk & lanemask_lt());
               float4 *it = reinterpret_cast<float4 *>(&Q.item[(head + rel_at) & (QCAP - 1)]);
-              it[0] = make_float4(__uint_as_float(r1.y), __uint_as_float(r1.z), ca, cb);
+              it[0] = make_float4(__uint_as_float(r1.x), __uint_as_float(r1.y), ca, cb);
               it[1] = make_float4(w0, w1, w2, r0.x + 0.5f * (ca + cb));
               it[2] = make_float4(d[0], d[1], d[2], 0.f);
               my_bits |= 1ull << rel_at;

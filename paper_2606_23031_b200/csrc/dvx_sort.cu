@@ -11,6 +11,10 @@ constexpr int SORT_ITEMS = 8;                          // keys per thread
 constexpr int SORT_TILE = SORT_THREADS * SORT_ITEMS;   // 2048 keys per block
 constexpr int SORT_WARPS = SORT_THREADS / 32;
 constexpr int RADIX = 256;
+#ifndef DVX_SORT_LOOK
+#define DVX_SORT_LOOK 8
+#endif
+constexpr int SORT_LOOK = DVX_SORT_LOOK;  // one-sweep look-back: predecessor tiles read per round trip
 
 constexpr int SCAN_THREADS = 512;
 constexpr int SCAN_ITEMS = 8;
@@ -258,11 +262,20 @@ __global__ void __launch_bounds__(SORT_THREADS) radix_onesweep(const uint64_t *_
     *mine = run | (tile == 0 ? ST_PREFIX : ST_AGG);
     uint32_t excl = 0;
     if (tile > 0) {
-      uint32_t t = tile - 1;
-      for (;;) {
-        const uint32_t v = status[(size_t)t * RADIX + d];
-        if (v & ST_PREFIX) { excl += v & ST_MASK; break; }
-        if (v & ST_AGG) { excl += v & ST_MASK; --t; }   // tile 0 always publishes a prefix, so t never underflows
+      // LOOK predecessors are read at once (independent loads, one L2 round trip) and then consumed front to back up to the
+      // first prefix or the first one not yet published: a walk of h tiles costs h / LOOK round trips instead of h.
+      uint32_t t = tile;  // the next tile to consume is t - 1
+      for (bool found = false; !found;) {
+        uint32_t v[SORT_LOOK];
+#pragma unroll
+        for (int j = 0; j < SORT_LOOK; ++j) v[j] = t > (uint32_t)j ? status[(size_t)(t - 1 - j) * RADIX + d] : 0u;
+#pragma unroll
+        for (int j = 0; j < SORT_LOOK; ++j) {
+          if (found || !(v[j] & (ST_PREFIX | ST_AGG))) break;  // not yet published: poll again from here
+          excl += v[j] & ST_MASK;
+          if (v[j] & ST_PREFIX) found = true;   // tile 0 always publishes a prefix, so the walk never passes it
+          else --t;
+        }
       }
       *mine = (excl + run) | ST_PREFIX;
     }
