@@ -14,6 +14,9 @@ constexpr int RADIX = 256;
 #ifndef DVX_SORT_LOOK
 #define DVX_SORT_LOOK 4  // measured on config 3 (6 passes over 2.9 M pairs), sort stage ms for 1 / 4 / 8 / 16: 0.386 / 0.356 / 0.359 / 0.378
 #endif
+#ifndef DVX_SORT_EARLY_VALS
+#define DVX_SORT_EARLY_VALS 1  // payload loads issued with the key loads.  Same box, config 3 sort stage ms: look-back 1 wide 0.446,
+#endif                          // 4 wide 0.395, 4 wide + early payload loads at 4 CTAs per SM 0.351
 constexpr int SORT_LOOK = DVX_SORT_LOOK;  // one-sweep look-back: predecessor tiles read per round trip
 
 constexpr int SCAN_THREADS = 512;
@@ -205,7 +208,10 @@ __global__ void __launch_bounds__(RADIX) radix_digit_scan(uint32_t *ghist) {
   g[threadIdx.x] = ex;
 }
 
-__global__ void __launch_bounds__(SORT_THREADS) radix_onesweep(const uint64_t *__restrict__ keys_in,
+#ifndef DVX_SORT_MIN_CTAS
+#define DVX_SORT_MIN_CTAS 4  // 64 registers with the payload loads issued early (80 and 3 CTAs per SM without the cap)
+#endif
+__global__ void __launch_bounds__(SORT_THREADS, DVX_SORT_MIN_CTAS) radix_onesweep(const uint64_t *__restrict__ keys_in,
                                                                 const uint32_t *__restrict__ vals_in,
                                                                 uint64_t *__restrict__ keys_out, uint32_t *__restrict__ vals_out,
                                                                 uint64_t n, uint32_t shift, const uint32_t *__restrict__ dbase,
@@ -230,6 +236,14 @@ __global__ void __launch_bounds__(SORT_THREADS) radix_onesweep(const uint64_t *_
     const uint64_t idx = wbase + (uint64_t)i * 32 + lane;
     key[i] = idx < n ? keys_in[idx] : 0;
   }
+#if DVX_SORT_EARLY_VALS
+  uint32_t val[SORT_ITEMS];  // payload loads in flight under the ranking and the look-back
+#pragma unroll
+  for (int i = 0; i < SORT_ITEMS; ++i) {
+    const uint64_t idx = wbase + (uint64_t)i * 32 + lane;
+    val[i] = idx < n ? vals_in[idx] : 0;
+  }
+#endif
 #pragma unroll
   for (int i = 0; i < SORT_ITEMS; ++i) {
     const uint64_t idx = wbase + (uint64_t)i * 32 + lane;
@@ -293,7 +307,11 @@ __global__ void __launch_bounds__(SORT_THREADS) radix_onesweep(const uint64_t *_
       const uint32_t d = (uint32_t)(key[i] >> shift) & (RADIX - 1);
       const uint32_t pos = cnt[w][d] + rnk[i];
       s_key[pos] = key[i];
+#if DVX_SORT_EARLY_VALS
+      s_val[pos] = val[i];
+#else
       s_val[pos] = vals_in[idx];
+#endif
     }
   }
   __syncthreads();
