@@ -7,8 +7,11 @@
 namespace {
 
 constexpr int SORT_THREADS = 256;
-constexpr int SORT_ITEMS = 8;                          // keys per thread
-constexpr int SORT_TILE = SORT_THREADS * SORT_ITEMS;   // 2048 keys per block
+#ifndef DVX_SORT_ITEMS
+#define DVX_SORT_ITEMS 12  // keys per thread: 3072-key tiles (45 KB of shared memory, 3 CTAs per SM). Config 3 sort stage ms for 6 / 8 / 12: 0.381 / 0.353 / 0.341
+#endif
+constexpr int SORT_ITEMS = DVX_SORT_ITEMS;
+constexpr int SORT_TILE = SORT_THREADS * SORT_ITEMS;   // 3072 keys per block
 constexpr int SORT_WARPS = SORT_THREADS / 32;
 constexpr int RADIX = 256;
 #ifndef DVX_SORT_LOOK
@@ -100,7 +103,7 @@ __global__ void __launch_bounds__(SORT_THREADS) radix_hist(const uint64_t *keys,
   block_hist[(uint64_t)threadIdx.x * n_blocks + blockIdx.x] = h[threadIdx.x];  // digit-major for the scan
 }
 
-// Stable scatter of one 2048-key tile.  Ranks inside the tile come from warp-private digit counters (__match_any_sync keeps
+// Stable scatter of one SORT_TILE-key tile.  Ranks inside the tile come from warp-private digit counters (__match_any_sync keeps
 // equal digits in lane order); the tile is first sorted by digit INTO SHARED MEMORY and only then written out, so that
 // consecutive threads write consecutive global addresses (runs of one digit) instead of 8-byte pieces of 32 sectors.
 __global__ void __launch_bounds__(SORT_THREADS) radix_scatter(const uint64_t *__restrict__ keys_in,
@@ -209,7 +212,7 @@ __global__ void __launch_bounds__(RADIX) radix_digit_scan(uint32_t *ghist) {
 }
 
 #ifndef DVX_SORT_MIN_CTAS
-#define DVX_SORT_MIN_CTAS 4  // 64 registers with the payload loads issued early (80 and 3 CTAs per SM without the cap)
+#define DVX_SORT_MIN_CTAS 3  // register cap with the payload loads issued early (12 keys per thread at 4 CTAs per SM: 0.363 ms)
 #endif
 __global__ void __launch_bounds__(SORT_THREADS, DVX_SORT_MIN_CTAS) radix_onesweep(const uint64_t *__restrict__ keys_in,
                                                                 const uint32_t *__restrict__ vals_in,
