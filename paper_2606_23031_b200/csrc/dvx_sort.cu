@@ -17,9 +17,8 @@ constexpr int RADIX = 256;
 #ifndef DVX_SORT_LOOK
 #define DVX_SORT_LOOK 4  // measured on config 3 (6 passes over 2.9 M pairs), sort stage ms for 1 / 4 / 8 / 16: 0.386 / 0.356 / 0.359 / 0.378
 #endif
-#ifndef DVX_SORT_EARLY_VALS
-#define DVX_SORT_EARLY_VALS 1  // payload loads issued with the key loads.  Same box, config 3 sort stage ms: look-back 1 wide 0.446,
-#endif                          // 4 wide 0.395, 4 wide + early payload loads at 4 CTAs per SM 0.351
+// Payload loads are issued with the key loads.  Same box, config 3 sort stage ms: look-back 1 wide 0.446, 4 wide 0.395,
+// 4 wide + early payload loads 0.351, + 3072-key tiles 0.341.
 constexpr int SORT_LOOK = DVX_SORT_LOOK;  // one-sweep look-back: predecessor tiles read per round trip
 
 constexpr int SCAN_THREADS = 512;
@@ -239,14 +238,12 @@ __global__ void __launch_bounds__(SORT_THREADS, DVX_SORT_MIN_CTAS) radix_oneswee
     const uint64_t idx = wbase + (uint64_t)i * 32 + lane;
     key[i] = idx < n ? keys_in[idx] : 0;
   }
-#if DVX_SORT_EARLY_VALS
   uint32_t val[SORT_ITEMS];  // payload loads in flight under the ranking and the look-back
 #pragma unroll
   for (int i = 0; i < SORT_ITEMS; ++i) {
     const uint64_t idx = wbase + (uint64_t)i * 32 + lane;
     val[i] = idx < n ? vals_in[idx] : 0;
   }
-#endif
 #pragma unroll
   for (int i = 0; i < SORT_ITEMS; ++i) {
     const uint64_t idx = wbase + (uint64_t)i * 32 + lane;
@@ -310,11 +307,7 @@ __global__ void __launch_bounds__(SORT_THREADS, DVX_SORT_MIN_CTAS) radix_oneswee
       const uint32_t d = (uint32_t)(key[i] >> shift) & (RADIX - 1);
       const uint32_t pos = cnt[w][d] + rnk[i];
       s_key[pos] = key[i];
-#if DVX_SORT_EARLY_VALS
       s_val[pos] = val[i];
-#else
-      s_val[pos] = vals_in[idx];
-#endif
     }
   }
   __syncthreads();
