@@ -150,17 +150,18 @@ struct ItemGeom {
 // O6 for one queued item (ring slot `at`): K-point midpoint rule on the clipped segment.  Returns tau_v; with GRAD also
 // the moments M_j = sum_k act'(raw_k) lambda_k^j (j = 0..3), from which phase B2 rebuilds sum_k act'(raw_k) w_c(u_k).
 template <bool BWD, bool NRM>
-__device__ __forceinline__ float integrate_item(const CompositeArgs &A, const WarpQueue<BWD, NRM> &Q, int at, uint32_t &id,
-                                                uint32_t &meta, ItemGeom &G, float M[4]) {
+__device__ __forceinline__ float integrate_item(const CompositeArgs &A, const WarpQueue<BWD, NRM> &Q, const uint4 *s_tree, int at,
+                                                uint32_t &id, uint32_t &meta, ItemGeom &G, float M[4]) {
   id = Q.item[at].id;
   meta = Q.item[at].meta;
-  const TreeFrame &T = A.trees[(meta >> 8) & 0xFFu];
+  const uint4 tf = s_tree[(meta >> 8) & 0xFFu];  // geo pointer, base, 1 / cell of the item's octree (per-CTA table)
   const uint32_t level = meta >> 16;
-  const float4 *gp = reinterpret_cast<const float4 *>(T.geo + (size_t)(id - T.base) * 8);
+  const float *geo = reinterpret_cast<const float *>(((unsigned long long)tf.y << 32) | tf.x);
+  const float4 *gp = reinterpret_cast<const float4 *>(geo + (size_t)(id - tf.z) * 8);
   const float4 g0 = __ldg(gp), g1 = __ldg(gp + 1);
   const float g[8] = {g0.x, g0.y, g0.z, g0.w, g1.x, g1.y, g1.z, g1.w};
   // 1 / edge length = (1 / level-16 cell) * 2^(level - 16): exact power-of-two scaling
-  const float inv_s = T.inv_cell_f * __uint_as_float((111u + level) << 23);
+  const float inv_s = __uint_as_float(tf.w) * __uint_as_float((111u + level) << 23);
   const float4 i0 = *reinterpret_cast<const float4 *>(&Q.item[at]);        // id, meta, ca, cb
   const float4 i1 = *(reinterpret_cast<const float4 *>(&Q.item[at]) + 1);  // w, mid
   const float4 i2 = *(reinterpret_cast<const float4 *>(&Q.item[at]) + 2);  // d, tau
@@ -263,8 +264,8 @@ __device__ __forceinline__ void red_add_v4(float *addr, float x, float y, float 
 // ---- phases B, C (and B2) over the first min(n_items, 32) queued items of the ring ------------------------------------
 // Ring slot of the i-th queued item: (head + i) & (QCAP-1).  my_bits: bit i set <=> queued item i belongs to this pixel.
 template <bool BWD, bool NRM, bool EXP = false>
-__device__ __forceinline__ void flush_batch(const CompositeArgs &A, int lane, WarpQueue<BWD, NRM> &Q, int &n_items, int &head,
-                                            unsigned long long &my_bits, Pix &S) {
+__device__ __forceinline__ void flush_batch(const CompositeArgs &A, int lane, WarpQueue<BWD, NRM> &Q, const uint4 *s_tree,
+                                            float *const *s_dgeo, int &n_items, int &head, unsigned long long &my_bits, Pix &S) {
   const int count = n_items < 32 ? n_items : 32;
   __syncwarp();
   // -- B: lane = item
@@ -282,7 +283,7 @@ __device__ __forceinline__ void flush_batch(const CompositeArgs &A, int lane, Wa
       f1 = __ldg(reinterpret_cast<const float4 *>(A.fvox + id0) + 1);
       if (NRM) nv = __ldg(A.vnrm + id0);
     }
-    const float tau = integrate_item<BWD, NRM>(A, Q, at_b, my_id, my_meta, G, M);
+    const float tau = integrate_item<BWD, NRM>(A, Q, s_tree, at_b, my_id, my_meta, G, M);
     if (BWD) {
       f1 = __ldg(reinterpret_cast<const float4 *>(A.fvox + my_id) + 1);
       if (NRM) nv = __ldg(A.vnrm + my_id);
@@ -408,9 +409,9 @@ __device__ __forceinline__ void flush_batch(const CompositeArgs &A, int lane, Wa
       }
     }
     if (my_id != NONE && is_head2) {
-      const TreeFrame &T = A.trees[(my_meta >> 8) & 0xFFu];
-      if (T.dgeo) {
-        float *dg = T.dgeo + (size_t)(my_id - T.base) * 8;
+      const uint32_t ti = (my_meta >> 8) & 0xFFu;
+      if (s_dgeo[ti]) {
+        float *dg = s_dgeo[ti] + (size_t)(my_id - s_tree[ti].z) * 8;
         red_add_v4(dg, val[0], val[1], val[2], val[3]);
         red_add_v4(dg + 4, val[4], val[5], val[6], val[7]);
       }
@@ -458,7 +459,16 @@ __device__ __noinline__ float2 axis_parallel_fix(const TreeFrame *T, uint32_t id
 template <bool BWD, bool CNT, bool NRM, bool EXP = false>
 __global__ void __launch_bounds__(TILE_THREADS, DVX_TILE_MIN_CTAS) composite_tile_kernel(const __grid_constant__ CompositeArgs A) {
   __shared__ WarpQueue<BWD, NRM> s_queue[TILE_WARPS];
+  // what phase B needs of an item's octree, 16 bytes each: one shared-memory load instead of three dependent global ones
+  __shared__ uint4 s_tree[DVX_MAX_ACTORS + 1];
+  __shared__ float *s_dgeo[BWD ? DVX_MAX_ACTORS + 1 : 1];
   const FrameParams &p = A.p;
+  for (uint32_t i = threadIdx.x; i < p.n_trees; i += TILE_THREADS) {
+    const TreeFrame &Ti = A.trees[i];
+    const unsigned long long ga = reinterpret_cast<unsigned long long>(Ti.geo);
+    s_tree[i] = make_uint4((uint32_t)ga, (uint32_t)(ga >> 32), Ti.base, __float_as_uint(Ti.inv_cell_f));
+    if (BWD) s_dgeo[i] = Ti.dgeo;
+  }
   const int tile = A.tile_order ? (int)__ldg(A.tile_order + blockIdx.x / TILE_SPLIT) : (int)(blockIdx.x / TILE_SPLIT);
   const int warp_l = threadIdx.x >> 5;                                  // warp of this CTA
   const int warp = (int)(blockIdx.x % TILE_SPLIT) * TILE_WARPS + warp_l;  // warp of the tile: which 4x8 pixel block
@@ -538,6 +548,7 @@ __global__ void __launch_bounds__(TILE_THREADS, DVX_TILE_MIN_CTAS) composite_til
     }
   }
 
+  __syncthreads();  // s_tree / s_dgeo
   // ---- step 4: Algorithm 1 as a per-lane state machine; the warp serves one (tree, octant) list at a time
   float cur = p.near_;   // tau_curr
   int h = 0;             // next entry of the hit list
@@ -677,7 +688,7 @@ __global__ void __launch_bounds__(TILE_THREADS, DVX_TILE_MIN_CTAS) composite_til
             }
             n_items += __popc(mk);
             if (n_items >= 32) {
-              flush_batch<BWD, NRM, EXP>(A, lane, Q, n_items, head, my_bits, S);
+              flush_batch<BWD, NRM, EXP>(A, lane, Q, s_tree, s_dgeo, n_items, head, my_bits, S);
               if (S.done) c_t = NONE;
             }
           }
@@ -693,7 +704,7 @@ __global__ void __launch_bounds__(TILE_THREADS, DVX_TILE_MIN_CTAS) composite_til
     }
     if (part) seg_tree = NONE;          // served
   }
-  while (n_items > 0) flush_batch<BWD, NRM, EXP>(A, lane, Q, n_items, head, my_bits, S);
+  while (n_items > 0) flush_batch<BWD, NRM, EXP>(A, lane, Q, s_tree, s_dgeo, n_items, head, my_bits, S);
 
   if (!BWD && !EXP && inside) {
     float3 sky = make_float3(0.f, 0.f, 0.f);
