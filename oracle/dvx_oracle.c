@@ -27,7 +27,10 @@
  *
  * Pinned by tests/test_oracle_pins.py (closed forms P1/P2/P10/P11, Morton-vs-depth order P3,
  * world-frame rewrite P4, empty box P5, finite differences P6, partition of unity P7,
- * subdivision P8, dense-sampling ray-box P9, SH orthonormality P12, culled==brute P13).
+ * subdivision P8, dense-sampling ray-box P9, SH orthonormality P12, culled==brute P13; early termination
+ * P32 (threshold crossed / not crossed closed forms, crossing voxel included, strict '<'), the exp-linear
+ * derivative and the truncated tape P33 (finite differences), orc_tile_hit_list P34 (hand-written lists and a
+ * dense-sampling cross-check)).  tests/test_oracle_sanitizers.py runs this file under ASan + UBSan.
  * Parity-unpinned against the AUTHORS' implementation: readings R1, R2, R5, R8, R9 (the paper
  * prints no worked numeric example); see DESIGN.md.
  */
@@ -455,7 +458,7 @@ static void render_ray(const scene_t *sc, int u, int v, const uint32_t *const *c
     if (cand && cand[t]) for (uint32_t n = 0; n < ncand[t]; ++n) candidate(tr, (uint32_t)t, cand[t][n], ol, dl, iv, niv, &w->segs);
     else if (!cand) for (uint32_t vx = 0; vx < tr->n_voxels; ++vx) candidate(tr, (uint32_t)t, vx, ol, dl, iv, niv, &w->segs);
   }
-  qsort(w->segs.s, w->segs.n, sizeof(seg_t), seg_cmp); /* O5 */
+  if (w->segs.n > 1) qsort(w->segs.s, w->segs.n, sizeof(seg_t), seg_cmp); /* O5 (guard: no NULL base for an empty list) */
   if (w->segs.n > w->tape_cap) {
     w->tape_cap = w->segs.n * 2;
     w->tau = (double *)realloc(w->tau, sizeof(double) * w->tape_cap);

@@ -594,3 +594,208 @@ def test_p15_finite_difference_gradients_with_normals():
             flat[idx] = keep - h; lm = loss()
             flat[idx] = keep
             assert abs((lp - lm) / (2 * h) - aflat[idx]) / scale < 2e-6, (n, idx)
+
+
+# ---------------------------------------------------------------- P32 early termination (Alg. 1 l.8-9; R3)
+def _two_slab_scene(v1, t_stop, v2=0.2, c1=0.8, c2=0.3):
+    """P10's geometry: static voxel [0,2]^3 (chord 2 on the optical axis, entered at tau = 5) in front of one actor voxel
+    (chord 0.5, entered at tau = 9)."""
+    cam = axis_camera(width=1, height=1)
+    sh1 = np.full((1, 1, 3), (c1 - 0.5) / C0); sh2 = np.full((1, 1, 3), (c2 - 0.5) / C0)
+    st = tree_from_cells([(1, 1, 1, 1)], geo=v1, sh=sh1)
+    act = tree_from_cells([(1, 1, 1, 1)], geo=v2, sh=sh2, side=1.0)
+    pose = S.pose_yaw((4.0, 0.75, 0.75), 0.0)
+    return scene(st, [act], [pose], [[0.6, 0.6, 0.6]], cam=cam, t_stop=t_stop)
+
+
+def test_p32_early_termination_after_the_crossing_voxel():
+    """north_star (4) 'early termination at T < 1e-4', Alg. 1 l.8-9, reading R3: T is tested AFTER each
+    voxel, the voxel that crosses the threshold is composited, everything behind it is not.  t_stop = 0.05:
+      T1 = 0.04 -> the second slab must be ABSENT  (alpha = 1 - T1, C = c1 (1 - T1), n_used = 1);
+      T1 = 0.06 -> the second slab must be PRESENT (closed form of P10, n_used = 2).
+    Fails under: no termination at all (first case), a threshold compared against alpha or against tau instead of T
+    (second case: alpha1 = 0.94, tau1 = 2.8), termination that drops the crossing voxel as 3DGS-style rasterizers do
+    (test_p32_crossing_voxel_is_included), `<=` instead of `<` (test_p32_threshold_is_strict)."""
+    c1, c2, v2, l2 = 0.8, 0.3, 0.2, 0.5
+    e2 = math.exp(-math.exp(v2) * l2)
+    for T1, second in ((0.04, False), (0.06, True)):
+        v1 = math.log(-math.log(T1) / 2.0)          # sigma1 * 2 = -ln T1
+        r = O.render(_two_slab_scene(v1, 0.05))
+        if second:
+            assert r["n_used"][0, 0] == 2
+            assert abs(r["alpha"][0, 0] - (1 - T1 * e2)) < 1e-12
+            assert abs(r["rgb"][0, 0, 0] - (c1 * (1 - T1) + T1 * c2 * (1 - e2))) < 1e-12
+            assert abs(r["depth"][0, 0] - ((1 - T1) * 6.0 + T1 * (1 - e2) * 9.25)) < 1e-11
+        else:
+            assert r["n_used"][0, 0] == 1
+            assert abs(r["alpha"][0, 0] - (1 - T1)) < 1e-12
+            assert abs(r["rgb"][0, 0, 0] - c1 * (1 - T1)) < 1e-12
+            assert abs(r["depth"][0, 0] - (1 - T1) * 6.0) < 1e-11
+        # t_stop = 0 disables the test: both slabs, whatever T1
+        r0 = O.render(_two_slab_scene(v1, 0.0))
+        assert r0["n_used"][0, 0] == 2 and abs(r0["alpha"][0, 0] - (1 - T1 * e2)) < 1e-12
+
+
+def test_p32_crossing_voxel_is_included():
+    """One slab whose own transmittance (0.01) is already below t_stop = 0.05: it is composited in full (R3).  A renderer
+    that tests T * exp(-tau) BEFORE blending and skips the voxel returns alpha = 0 here."""
+    T1 = 0.01
+    cam = axis_camera(width=1, height=1)
+    sc = scene(tree_from_cells([(1, 1, 1, 1)], geo=math.log(-math.log(T1) / 2.0)), cam=cam, t_stop=0.05)
+    r = O.render(sc)
+    assert r["n_used"][0, 0] == 1
+    assert abs(r["alpha"][0, 0] - 0.99) < 1e-12 and abs(r["depth"][0, 0] - 0.99 * 6.0) < 1e-11
+
+
+def test_p32_threshold_is_strict():
+    """'T < eps_stop' (Alg. 1 l.8): with t_stop EXACTLY the transmittance after the first slab the ray goes
+    on.  T1 is taken from a t_stop = 0 render of the first slab alone; for T1 in [1/2, 1] both 1 - T1 and 1 - (1 - T1)
+    are exact in binary floating point (Sterbenz), so 1 - alpha is the T the oracle holds, bit for bit."""
+    v1 = math.log(-math.log(0.6) / 2.0)
+    cam = axis_camera(width=1, height=1)
+    alone = O.render(scene(tree_from_cells([(1, 1, 1, 1)], geo=v1), cam=cam, t_stop=0.0))
+    T1 = 1.0 - alone["alpha"][0, 0]
+    assert 0.5 < T1 < 0.7
+    assert O.render(_two_slab_scene(v1, T1))["n_used"][0, 0] == 2              # T1 < T1 is false: continue
+    assert O.render(_two_slab_scene(v1, np.nextafter(T1, 1.0)))["n_used"][0, 0] == 1
+
+
+# ---------------------------------------------------------------- P33 exp-linear derivative and the truncated tape
+def _fd_check(s, g, opt, h, tol, stride=1):
+    """Central differences of the loss <g, render> against the analytic gradients, every `stride`-th parameter; every
+    perturbed render must composite exactly the sub-segments the base render did (n_used unchanged)."""
+    r = O.render(s, grads_in=g, **opt)
+
+    def loss():
+        q = O.render(s, **opt)
+        assert np.array_equal(q["n_used"], r["n_used"]), "perturbation moved a ray across the termination threshold"
+        return (q["rgb"] * g["rgb"]).sum() + (q["depth"] * g["depth"]).sum() + (q["alpha"] * g["alpha"]).sum()
+
+    worst, n_nonzero = 0.0, 0
+    for n, t in enumerate(s.octrees):
+        for arr, ana in ((t.geo, r["dgeo"][n]), (t.sh, r["dsh"][n])):
+            flat, aflat = arr.reshape(-1), ana.reshape(-1)
+            scale = max(np.abs(aflat).max(), 1e-12)
+            for idx in range(0, flat.shape[0], stride):
+                keep = flat[idx]
+                flat[idx] = keep + h; lp = loss()
+                flat[idx] = keep - h; lm = loss()
+                flat[idx] = keep
+                worst = max(worst, abs((lp - lm) / (2 * h) - aflat[idx]) / scale)
+                n_nonzero += abs(aflat[idx]) > 1e-9 * scale
+    assert worst < tol, worst
+    return r, n_nonzero
+
+
+def _fd_scene(seed, gain, shift):
+    s = S.tiny_random_scene(seed, sh_degree=1, colour_floor=True)
+    for t in s.octrees:
+        t.geo = t.geo.astype(np.float64) * gain + shift
+        t.sh = t.sh.astype(np.float64)
+    return s
+
+
+def test_p33_finite_differences_exp_linear_activation():
+    """R5 option 1 (PAPER.md:107 'exponential-linear density activation'): act(x) = x above theta = 1.1, exp(x/theta - 1 +
+    ln theta) below; its derivative is 1 above and act/theta below.  P6's loop with activation = 1 on raw densities spread
+    over both branches.  Fails when dact forgets the 1/theta factor, uses the wrong branch, or returns act itself."""
+    s = _fd_scene(7, 1.5, 1.8)
+    raw = np.concatenate([t.geo.reshape(-1) for t in s.octrees])
+    assert (raw > 1.3).mean() > 0.2 and (raw < 0.9).mean() > 0.2      # both branches of the activation are exercised
+    g = s.image_grads(0, 1.0, 0.3, 1.0)
+    r, n_nonzero = _fd_check(s, g, dict(activation=1, t_stop=0.0), 1e-5, 1e-6)
+    assert n_nonzero > 100 and r["alpha"].max() > 0.5
+
+
+@pytest.mark.parametrize("activation", [0, 1])
+def test_p33_finite_differences_of_the_truncated_tape(activation):
+    """O9 with early termination ON (the configured case, t_stop = 1e-4): the gradient of what was composited is the
+    gradient of the image as long as no ray changes its stopping voxel.  Dense scene (raw shifted up) so that many rays
+    terminate early; voxels behind the stopping point must get exactly zero gradient from those rays."""
+    s = _fd_scene(7, 1.0, 3.2)
+    g = s.image_grads(0, 1.0, 0.3, 1.0)
+    full = O.render(s, t_stop=0.0, activation=activation)
+    r, n_nonzero = _fd_check(s, g, dict(activation=activation, t_stop=1e-4), 1e-6, 2e-6)
+    stopped = (r["n_used"] < full["n_used"])
+    assert stopped.sum() >= 10, stopped.sum()                       # the truncation really fires
+    assert (r["alpha"][stopped] > 1 - 1e-4).all() and n_nonzero > 60
+
+
+# ---------------------------------------------------------------- P34 the T1 reference list (orc_tile_hit_list)
+def _p34_scene():
+    """One 16x16 tile, camera at (-5,0,0) looking down +x with the optical axis on the pixel corner (8,8): the four pixel
+    quadrants are the four ray octants q = 2 (d_y<0) + (d_z<0) in {0,1,2,3} (d_x > 0 always).  Static 4 m cube centred at
+    the origin, leaves given in scrambled order (ids = positions in this list):
+       id 0  L1 (1,1,1)   x in [0,2],   y,z in [0,2]            seen by q = 0 only
+       id 1  L2 (1,1,1)   x in [-1,0],  y,z in [-1,0]           q = 3
+       id 2  L1 (0,1,0)   x in [-2,0],  y in [0,2], z in [-2,0] q = 1
+       id 3  L2 (0,3,3)   x in [-2,-1], y,z in [1,2]            q = 0
+       id 4  L2 (0,0,0)   x in [-2,-1], y,z in [-2,-1]          q = 3
+       id 5  L1 (1,0,0)   x in [0,2],   y,z in [-2,0]           q = 3, but masked by the box except a 1.4e-5 m sliver
+       id 6  L2 (1,3,2)   x in [-1,0],  y in [1,2], z in [0,1]  q = 0
+       id 7  L2 (0,2,2)   x in [-2,-1], y,z in [0,1]            q = 0
+       id 8  L1 (0,0,1)   x in [-2,0],  y in [-2,0], z in [0,2] q = 2
+       id 9  L2 (0,1,1)   x in [-2,-1], y,z in [-1,0]           q = 3
+       id 10 L2 (1,2,2)   x in [-1,0],  y,z in [0,1]            q = 0
+    Actor: 4 m cube, box half 1.5, pose = translation (1.5 + 1.4e-5, -1.5, -1.5): world box x in [1.4e-5, 3.000014],
+    y,z in [-3,0].  Leaves  id 0  L3 (0,3,3): local x in [-2,-1.5] -> OUTSIDE the box (R18), on the path of ray (14,14);
+                            id 1  L3 (1,3,3): local x in [-1.5,-1], y,z in [-0.5,0] -> inside, world x in [0,0.5], y,z in [-2,-1.5]."""
+    cells = [(1, 1, 1, 1), (1, 1, 1, 2), (0, 1, 0, 1), (0, 3, 3, 2), (0, 0, 0, 2), (1, 0, 0, 1), (1, 3, 2, 2), (0, 2, 2, 2),
+             (0, 0, 1, 1), (0, 1, 1, 2), (1, 2, 2, 2)]
+    st = tree_from_cells(cells, geo=-1.0, center=(0, 0, 0), side=4.0)
+    act = tree_from_cells([(0, 3, 3, 3), (1, 3, 3, 3)], geo=-1.0, center=(0, 0, 0), side=4.0)
+    cam = S.Camera(16, 16, 16.0, 16.0, 8.0, 8.0, S.look_yaw((-5.0, 0.0, 0.0), 0.0))
+    cam.c2w = np.asarray(S.look_yaw((-5.0, 0.0, 0.0), 0.0), dtype=np.float64).reshape(12)
+    pose = S.pose_yaw((1.5 + 1.4e-5, -1.5, -1.5), 0.0)
+    return scene(st, [act], [pose], [[1.5, 1.5, 1.5]], cam=cam, t_stop=0.0), cells
+
+
+def test_p34_tile_hit_list_hand_case():
+    """T1's reference: per (tile, octree, octant) the voxels hit by a pixel of that octant with a sub-segment
+    longer than 1e-5 s_l, sorted by the R14b key.  Expected lists written out by hand (see _p34_scene):
+      q = 0: plain Morton order                 -> L2 (0,2,2), (0,3,3), (1,2,2), (1,3,2), then L1 (1,1,1)  = ids 7, 3, 10, 6, 0
+      q = 3: y and z bits flipped in every group -> L2 (0,1,1) [group 011 -> 000], (0,0,0) [000 -> 011], (1,1,1) [111 -> 100]
+                                                   = ids 9, 4, 1   (plain Morton order would give 4, 9, 1)
+      id 5 is absent from q = 3: its only pieces are 1.4e-5..1.7e-5 m long, below 1e-5 * 2 m but above an absolute 1e-5.
+    Fails under: a wrong octant formula (bit order), a missing or unscaled length cut, the static intervals used for the
+    actor (its outside-the-box leaf would appear), an unsorted or plain-Morton-sorted list."""
+    sc, cells = _p34_scene()
+    want0 = {0: [7, 3, 10, 6, 0], 1: [2], 2: [8], 3: [9, 4, 1]}
+    for q in range(8):
+        assert O.tile_hit_list(sc, 0, 0, 0, q).tolist() == want0.get(q, []), q
+        assert O.tile_hit_list(sc, 0, 0, 1, q).tolist() == ([1] if q == 3 else []), q
+    # without the box, id 5 and the actor-masked part come back: the sliver cut is what removed it
+    sc2 = scene(sc.static, cam=sc.cameras[0], t_stop=0.0)
+    assert O.tile_hit_list(sc2, 0, 0, 0, 3).tolist() == [9, 4, 1, 5]
+
+
+def test_p34_tile_hit_list_against_dense_ray_sampling():
+    """The same lists from a method that shares nothing with the slab test: 40 000 points along every ray of the tile,
+    point-in-box membership, masked where the point is inside the actor box (static) or outside it (actor)."""
+    sc, cells = _p34_scene()
+    cam = sc.cameras[0]
+    ts = np.linspace(0.05, 12.0, 40001)
+    dt = ts[1] - ts[0]
+    hit = {(tree, q): {} for tree in (0, 1) for q in range(8)}
+    bx_lo, bx_hi = np.array([1.4e-5, -3.0, -3.0]), np.array([3.0 + 1.4e-5, 0.0, 0.0])
+    a_cells = [(0, 3, 3, 3), (1, 3, 3, 3)]
+    for v in range(16):
+        for u in range(16):
+            dc = np.array([(u + 0.5 - 8.0) / 16.0, (v + 0.5 - 8.0) / 16.0, 1.0])
+            d = np.array([dc[2], -dc[0], -dc[1]]) / np.linalg.norm(dc)      # R10: x right = -y_world, y down = -z_world
+            q = 4 * (d[0] < 0) + 2 * (d[1] < 0) + (d[2] < 0)
+            p = np.array([-5.0, 0.0, 0.0])[None] + ts[:, None] * d[None]
+            in_box = np.all((p >= bx_lo) & (p <= bx_hi), axis=1)
+            for tree, cl, origin in ((0, cells, np.array([-2.0, -2.0, -2.0])),
+                                     (1, a_cells, np.array([-2.0, -2.0, -2.0]) + np.array([1.5 + 1.4e-5, -1.5, -1.5]))):
+                for n, (i, j, k, l) in enumerate(cl):
+                    s_l = 4.0 / (1 << l)
+                    lo = origin + np.array([i, j, k]) * s_l
+                    inside = np.all((p >= lo) & (p <= lo + s_l), axis=1) & (in_box if tree else ~in_box)
+                    if inside.sum() * dt > 10 * dt:     # far above the sampling step, far above the 1e-5 s_l cut
+                        hit[(tree, q)][n] = True
+    for tree in (0, 1):
+        codes = sc.octrees[tree].code
+        for q in range(8):
+            ids = sorted(hit[(tree, q)], key=lambda n: int(O.order_key([codes[n]], q)[0]))
+            assert O.tile_hit_list(sc, 0, 0, tree, q).tolist() == ids, (tree, q)
