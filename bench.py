@@ -41,6 +41,8 @@ def parse_args():
     ap.add_argument("--fwd-only", action="store_true", help="profiling aid: time dvx_render alone")
     ap.add_argument("--k-samples", type=int, default=0, help="report-only variant: override K (samples per voxel segment)")
     ap.add_argument("--opaque", action="store_true", help="report-only variant 3b: config 3 with raw += 8 on leaves holding a LiDAR return")
+    ap.add_argument("--no-records", action="store_true",
+                    help="A/B aid: DVX_FLAG_NO_RECORDS (the backward walks the tile lists again instead of replaying hit records)")
     ap.add_argument("--profiler-range", action="store_true",
                     help="bracket the first timed region with cudaProfilerStart/Stop (use with ncu --profile-from-start off)")
     return ap.parse_args()
@@ -408,7 +410,8 @@ def run_dvx(args):
 
     def step(host=False, bwd=True):
         for c in range(n_cams):
-            _, _, _, fr = dev.render(c, save=bwd, out=out_host if host else out_dev, host=host)
+            _, _, _, fr = dev.render(c, save=bwd, out=out_host if host else out_dev, host=host,
+                                     flags=dvx.FLAG_NO_RECORDS if args.no_records else 0)
             if bwd:
                 fr.backward(g_host[c] if host else g_dev[c], grads=grads, host=host)
                 fr.release()

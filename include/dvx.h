@@ -104,6 +104,8 @@ typedef struct {
 } dvx_render_opts;
 #define DVX_FLAG_COUNTERS 1u /* maintain q_test / q_hit / pairs_eff (slower; off in timed runs) */
 #define DVX_FLAG_NAIVE 2u    /* debug: per-thread in-order walker instead of the cooperative tile kernel */
+#define DVX_FLAG_NO_RECORDS 4u /* saved frames only: keep no hit records; dvx_backward then walks the tile lists again
+                                  (same gradients up to the order of the float reductions; slower, no record pool) */
 
 typedef struct {
   float *rgb;   /* DEVICE [H][W][3] */
@@ -139,6 +141,19 @@ dvx_status dvx_backward_n(dvx_ctx *ctx, dvx_frame *saved, const float *dL_drgb, 
                           const float *dL_dalpha, const float *dL_dnormal, dvx_grad static_grad,
                           const dvx_grad *actor_grads);
 void dvx_frame_release(dvx_ctx *ctx, dvx_frame *frame);
+
+/* Hit records.  When dvx_render is given a `saved` handle, the compositing kernel also writes what it composited -
+ * per (pixel, voxel) hit 40 bytes: voxel, octree, the clipped segment in the voxel's local coordinates, its length / K
+ * and midpoint, in the order the pixel blended them (Alg. 1's sequence) - into a pool obtained from
+ * the caller's allocator, and dvx_backward streams those records instead of walking the sorted tile
+ * lists and testing every candidate voxel a second time.  The pool is sized from the hit counts of the context's recent
+ * frames (first frame: 48 hits per pixel); a frame that needs more falls back to the list walk on the device, without
+ * a host round trip, with identical results up to float summation order.  dvx_set_record_budget fixes the pool size
+ * instead (bytes per frame; 0 = back to automatic sizing).  dvx_frame_record_stats (synchronises the stream) reports
+ * what one frame used. */
+dvx_status dvx_set_record_budget(dvx_ctx *ctx, uint64_t bytes_per_frame);
+dvx_status dvx_frame_record_stats(dvx_ctx *ctx, const dvx_frame *frame, uint64_t *bytes_used, uint64_t *bytes_capacity,
+                                  uint32_t *overflowed);
 
 /* The same two calls with HOST image buffers (pinned memory recommended), for end-to-end use from a host
  * data pipeline: dvx_render_host renders into device staging owned by the context and enqueues the device->host

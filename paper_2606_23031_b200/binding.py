@@ -18,6 +18,7 @@ ERRORS = {-1: "DVX_ERR_INVALID_ARG", -2: "DVX_ERR_BAD_OCTREE", -3: "DVX_ERR_OOM"
 STAGES = ("preprocess", "sort", "composite", "backward", "backward_composite", "backward_sh")
 FLAG_COUNTERS = 1
 FLAG_NAIVE = 2
+FLAG_NO_RECORDS = 4
 
 EXPORTS = ["dvx_create", "dvx_destroy", "dvx_octree_create", "dvx_octree_refresh_structure", "dvx_octree_destroy",
            "dvx_render", "dvx_backward", "dvx_backward_n", "dvx_frame_release", "dvx_debug_tile_list", "dvx_frame_counters",
@@ -25,7 +26,8 @@ EXPORTS = ["dvx_create", "dvx_destroy", "dvx_octree_create", "dvx_octree_refresh
            "dvx_backward_host", "dvx_grid_create", "dvx_grid_destroy", "dvx_grid_gather", "dvx_grid_reduce",
            "dvx_grid_adam_step", "dvx_adam_step", "dvx_grid_adam_step_n", "dvx_adam_step_n",
            "dvx_frame_weights", "dvx_render_features", "dvx_fuse_features",
-           "dvx_cloud_create", "dvx_cloud_destroy", "dvx_density_prior", "dvx_subdivide_near", "dvx_prune"]
+           "dvx_cloud_create", "dvx_cloud_destroy", "dvx_density_prior", "dvx_subdivide_near", "dvx_prune",
+           "dvx_set_record_budget", "dvx_frame_record_stats"]
 
 
 class DvxError(RuntimeError):
@@ -138,6 +140,8 @@ def load():
     lib.dvx_prune.argtypes = [P, C.c_uint32, P, P, C.c_float, P, P, C.POINTER(C.c_uint32)]
     lib.dvx_grid_adam_step_n.argtypes = [P, C.POINTER(Adam), C.c_uint32, C.POINTER(GridAdamItem)]
     lib.dvx_adam_step_n.argtypes = [P, C.POINTER(Adam), C.c_uint32, C.POINTER(AdamItem)]
+    lib.dvx_set_record_budget.argtypes = [P, C.c_uint64]
+    lib.dvx_frame_record_stats.argtypes = [P, P, C.POINTER(C.c_uint64), C.POINTER(C.c_uint64), C.POINTER(C.c_uint32)]
     for name in EXPORTS:
         if name not in ("dvx_destroy", "dvx_octree_destroy", "dvx_frame_release", "dvx_last_error", "dvx_launch_count",
                         "dvx_grid_destroy", "dvx_cloud_destroy"):
@@ -190,6 +194,10 @@ class Context:
         n = C.c_uint32()
         self.check(self.lib.dvx_stage_ms_collect(self.h, ms, C.byref(n)))
         return dict(zip(STAGES, list(ms)[:6])), n.value
+
+    def set_record_budget(self, nbytes):
+        """dvx_set_record_budget: bytes of hit records per saved frame (0 = automatic sizing)."""
+        self.check(self.lib.dvx_set_record_budget(self.h, int(nbytes)))
 
     def check(self, rc):
         if rc != DVX_OK:
@@ -480,6 +488,13 @@ class Frame:
         v = [C.c_uint64() for _ in range(5)]
         ctx.check(ctx.lib.dvx_frame_counters(ctx.h, self.h, *[C.byref(x) for x in v]))
         return dict(zip(("v_vis", "pairs", "pairs_eff", "q_test", "q_hit"), [x.value for x in v]))
+
+    def record_stats(self):
+        """dvx_frame_record_stats -> dict(bytes_used, bytes_capacity, overflowed)."""
+        ctx = self.ctx
+        used, cap, over = C.c_uint64(), C.c_uint64(), C.c_uint32()
+        ctx.check(ctx.lib.dvx_frame_record_stats(ctx.h, self.h, C.byref(used), C.byref(cap), C.byref(over)))
+        return {"bytes_used": used.value, "bytes_capacity": cap.value, "overflowed": bool(over.value)}
 
     def stage_ms(self):
         ctx = self.ctx

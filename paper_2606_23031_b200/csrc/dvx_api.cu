@@ -35,6 +35,13 @@ struct dvx_ctx {
   cudaEvent_t ev_main = nullptr, ev_d2h = nullptr, ev_h2d = nullptr, ev_bwd = nullptr;
   float *st_out = nullptr, *st_in = nullptr;  // persistent device staging (grow-only)
   size_t st_out_bytes = 0, st_in_bytes = 0;
+  // hit-record pool sizing: chunks per pixel used by the last frames (read back lazily, never waited for)
+  uint64_t rec_budget = 0;             // dvx_set_record_budget: bytes per frame, 0 = automatic
+  double rec_seen[8] = {0, 0, 0, 0, 0, 0, 0, 0};  // chunks per pixel of the last 8 frames whose count has arrived
+  int rec_seen_n = 0;
+  unsigned long long *h_rec = nullptr;  // pinned: [0] chunks handed out by the frame in flight
+  cudaEvent_t ev_rec = nullptr;
+  double rec_pending_npix = 0;          // > 0: a read-back is in flight for a frame of that many pixels
 };
 
 struct dvx_octree {
@@ -63,6 +70,8 @@ struct dvx_frame {
   cudaEvent_t *ev = nullptr;  // = es->ev
   Buf eff_end, vnrm, sv_nrm;
   Buf tile_cost, tile_order;  // pairs per tile [n_tiles]; the CTA -> tile launch order derived from it [2 n_tiles: result, intermediate]
+  Buf rec_pool, rec_next, rec_tab;  // hit records of the forward (dvx_internal.cuh); rec_pool.p == NULL: none kept
+  uint32_t rec_cap = 0;             // chunks in rec_pool
   Buf w_row, w_vox, w_val;  // row N3: the compositing weights as CSR, built on demand
   uint64_t w_nnz = 0;
   dvx_sky sky = {0, 0, nullptr, nullptr};
@@ -141,6 +150,7 @@ void frame_free(dvx_ctx *ctx, dvx_frame *f) {
   ctx_release(ctx, f->sv_nrm.p);
   ctx_release(ctx, f->tile_cost.p); ctx_release(ctx, f->tile_order.p);
   ctx_release(ctx, f->w_row.p); ctx_release(ctx, f->w_vox.p); ctx_release(ctx, f->w_val.p);
+  ctx_release(ctx, f->rec_pool.p); ctx_release(ctx, f->rec_next.p); ctx_release(ctx, f->rec_tab.p);
   if (f->es) {
     f->es->did_backward = f->did_backward;
     if (f->es->rendered) {
@@ -219,7 +229,13 @@ dvx_status dvx_create(int device, void *cuda_stream, dvx_alloc_fn alloc, dvx_fre
   ctx->device = device;
   ctx->st = (cudaStream_t)cuda_stream;
   ctx->alloc = alloc; ctx->free_ = free_; ctx->user = user;
-  if (cudaMallocHost((void **)&ctx->h_counters, CNT_N * sizeof(unsigned long long)) != cudaSuccess) {
+  if (cudaMallocHost((void **)&ctx->h_counters, (CNT_N + 1) * sizeof(unsigned long long)) != cudaSuccess) {
+    delete ctx;
+    return DVX_ERR_CUDA;
+  }
+  ctx->h_rec = ctx->h_counters + CNT_N;
+  if (cudaEventCreateWithFlags(&ctx->ev_rec, cudaEventDisableTiming) != cudaSuccess) {
+    cudaFreeHost(ctx->h_counters);
     delete ctx;
     return DVX_ERR_CUDA;
   }
@@ -236,6 +252,7 @@ void dvx_destroy(dvx_ctx *ctx) {
     else cudaFree(b.p);
   }
   cudaFreeHost(ctx->h_counters);
+  cudaEventDestroy(ctx->ev_rec);
   if (ctx->cs) {
     cudaStreamSynchronize(ctx->cs);
     cudaStreamSynchronize(ctx->cs_in);
@@ -318,6 +335,34 @@ void setup_tree(TreeFrame &T, const dvx_octree *t, uint32_t base, bool actor, co
     T.half[a] = actor ? half[a] : INFINITY;
     for (int c = 0; c < 3; ++c) T.R[3 * a + c] = (float)R[3 * a + c];
   }
+}
+
+// ---- hit-record pool sizing (dvx.h "Hit records") ------------------------------------------------------------------------
+// The chunk count of a frame is copied to pinned memory behind its forward and picked up here, without waiting, by a later
+// dvx_render; the pool of the next frame is 1.25 x the largest count per pixel among the last 8 frames seen.
+void rec_collect(dvx_ctx *ctx) {
+  if (ctx->rec_pending_npix > 0 && cudaEventQuery(ctx->ev_rec) == cudaSuccess) {
+    ctx->rec_seen[ctx->rec_seen_n % 8] = (double)ctx->h_rec[0] / ctx->rec_pending_npix;
+    ctx->rec_seen_n++;
+    ctx->rec_pending_npix = 0;
+  } else {
+    cudaGetLastError();  // cudaErrorNotReady is not an error
+  }
+}
+uint64_t rec_capacity(const dvx_ctx *ctx, const FrameParams &p) {
+  const double chunk_bytes = (double)DVX_REC_CHUNK * DVX_REC_BATCH_BYTES;
+  const double npix = (double)p.width * p.height, n_warps = (double)p.n_tiles * 8.0;
+  double cap;
+  if (ctx->rec_budget) {
+    cap = floor((double)ctx->rec_budget / chunk_bytes);
+  } else if (ctx->rec_seen_n == 0) {
+    cap = ceil(npix * 48.0 / 32.0 / DVX_REC_CHUNK) + n_warps;  // 48 hits per pixel + one partly filled chunk per warp
+  } else {
+    double m = 0;
+    for (int i = 0; i < 8 && i < ctx->rec_seen_n; ++i) m = fmax(m, ctx->rec_seen[i]);
+    cap = ceil(1.25 * m * npix) + 0.125 * n_warps + 16.0;
+  }
+  return cap > 4.0e9 ? 4000000000ull : (uint64_t)cap;
 }
 
 bool rigid(const float *m, int stride) {  // rows of a 3x3 inside a row-major matrix with `stride` columns
@@ -487,8 +532,32 @@ dvx_status dvx_render(dvx_ctx *ctx, const dvx_camera *cam, const dvx_octree *sta
     CU(cudaMemsetAsync(f->eff_end.p, 0, sizeof(uint32_t) * (size_t)p.n_buckets, st));
     A.eff_end = (uint32_t *)f->eff_end.p;
   }
+  // ---- hit records for the backward (dvx.h): only for saved frames rendered by the tile kernel
+  bool rec = false;
+  if (saved && !(p.flags & (DVX_FLAG_NAIVE | DVX_FLAG_NO_RECORDS))) {
+    rec_collect(ctx);
+    const uint64_t cap = rec_capacity(ctx, p);
+    if (cap > 0) {
+      // a pool the allocator cannot give is not an error: the frame then keeps no records and the backward walks the lists
+      if (buf_alloc(ctx, f->rec_tab, sizeof(uint32_t) * 2 * 8 * (size_t)p.n_tiles) && buf_alloc(ctx, f->rec_next, sizeof(uint32_t) * cap) &&
+          buf_alloc(ctx, f->rec_pool, (size_t)cap * DVX_REC_CHUNK * DVX_REC_BATCH_BYTES)) {
+        rec = true;
+        f->rec_cap = (uint32_t)cap;
+        A.rec_pool = (unsigned char *)f->rec_pool.p; A.rec_next = (uint32_t *)f->rec_next.p; A.rec_tab = (uint32_t *)f->rec_tab.p;
+        A.rec_cap = f->rec_cap;
+      } else {
+        ctx_release(ctx, f->rec_tab.p); ctx_release(ctx, f->rec_next.p); ctx_release(ctx, f->rec_pool.p);
+        f->rec_tab.p = f->rec_next.p = f->rec_pool.p = nullptr;
+      }
+    }
+  }
   dvx_composite_launch(A, false, st);
   CU(cudaEventRecord(f->ev[4], st));
+  if (rec && !ctx->rec_budget) {
+    CU(cudaMemcpyAsync(ctx->h_rec, counters + CNT_REC_CHUNKS, sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
+    CU(cudaEventRecord(ctx->ev_rec, st));
+    ctx->rec_pending_npix = (double)npix;
+  }
   f->es->rendered = true;
   CU(cudaGetLastError());
   if (saved) *saved = f;
@@ -542,6 +611,11 @@ dvx_status dvx_backward_n(dvx_ctx *ctx, dvx_frame *f, const float *dL_drgb, cons
   A.sky_tex = f->sky.tex; A.sky_w = f->sky.width; A.sky_h = f->sky.height; A.sky_dtex = f->sky.dtex;
   A.g_normal = dL_dnormal; A.vnrm = (const float4 *)f->vnrm.p; A.sv_nrm = (float *)f->sv_nrm.p; A.dnrm = dnrm;
   CU(cudaEventRecord(f->ev[7], st));
+  if (f->rec_pool.p) {  // replay the forward's hit records; the list walk behind it runs only if the pool overflowed
+    A.rec_pool = (unsigned char *)f->rec_pool.p; A.rec_next = (uint32_t *)f->rec_next.p; A.rec_tab = (uint32_t *)f->rec_tab.p;
+    A.rec_cap = f->rec_cap;
+    dvx_composite_replay_launch(A, st);
+  }
   dvx_composite_launch(A, true, st);
   CU(cudaEventRecord(f->ev[8], st));
   dvx_sh_backward_launch(p, trees_d, A.fvox, A.pxrect, drgb, st);
@@ -605,6 +679,28 @@ dvx_status dvx_frame_counters(dvx_ctx *ctx, const dvx_frame *f, uint64_t *v_vis,
   }
   if (q_test) *q_test = h[CNT_QTEST];
   if (q_hit) *q_hit = h[CNT_QHIT];
+  return DVX_OK;
+}
+
+dvx_status dvx_set_record_budget(dvx_ctx *ctx, uint64_t bytes_per_frame) {
+  if (!ctx) return DVX_ERR_INVALID_ARG;
+  ctx->rec_budget = bytes_per_frame;
+  return DVX_OK;
+}
+
+dvx_status dvx_frame_record_stats(dvx_ctx *ctx, const dvx_frame *f, uint64_t *bytes_used, uint64_t *bytes_capacity,
+                                  uint32_t *overflowed) {
+  if (!ctx) return DVX_ERR_INVALID_ARG;
+  if (!f) return fail(ctx, DVX_ERR_INVALID_ARG, "NULL argument");
+  cudaSetDevice(ctx->device);
+  unsigned long long h[CNT_N];
+  CU(cudaMemcpyAsync(h, f->counters.p, sizeof(h), cudaMemcpyDeviceToHost, ctx->st));
+  CU(cudaStreamSynchronize(ctx->st));
+  const uint64_t chunk_bytes = (uint64_t)DVX_REC_CHUNK * DVX_REC_BATCH_BYTES;
+  const bool on = f->rec_pool.p != nullptr;
+  if (bytes_used) *bytes_used = on ? (h[CNT_REC_CHUNKS] < f->rec_cap ? h[CNT_REC_CHUNKS] : f->rec_cap) * chunk_bytes : 0;
+  if (bytes_capacity) *bytes_capacity = on ? (uint64_t)f->rec_cap * chunk_bytes : 0;
+  if (overflowed) *overflowed = on ? (h[CNT_REC_OVERFLOW] != 0) : 0;
   return DVX_OK;
 }
 

@@ -73,15 +73,34 @@ struct __align__(16) Item {
   float pad;
 };
 
-template <bool BWD, bool NRM>
+// phase B -> C (-> B2), per batch item (written by the item's lane, read by the pixel's lane):
+template <bool NRM>
+struct BatchShared {
+  float4 eam[32];               // exp(-tau_v), alpha_v, (a+b)/2, voxel id (forward; the weight export reads it);
+                                // backward phase C puts dL/dtau_v into .w for phase B2
+  float4 rgbm[32];              // the voxel's RGB and clamp bits;    backward phase C overwrites .xyz with T alpha g_C
+  float4 nrm[NRM ? 32 : 1];     // the voxel's world normal (O11);    backward phase C overwrites .xyz with T alpha g_N
+};
+
+// Everything only the batch phases touch lives in shared memory, not in registers: the candidate loop of phase A runs
+// under an 80-register cap, and what it does not need must not be live across it (the compiler otherwise re-derives lane,
+// warp and queue addresses from tid.x inside the loop: 6 % of the forward's instructions in profiles/r02a).
+template <bool NRM>
 struct WarpQueue {
   EntryRec ent[32];
   Item item[QCAP];              // ring
   double d0[3];                 // the warp's reference direction for the list being served
-  // phase B -> C, per batch item (written by the item's lane, read by the pixel's lane):
-  float4 eam[32];               // exp(-tau_v), alpha_v, (a+b)/2, -;  backward phase C puts dL/dtau_v into .w for phase B2
-  float4 rgbm[32];              // the voxel's RGB and clamp bits;    backward phase C overwrites .xyz with T alpha g_C
-  float4 nrm[NRM ? 32 : 1];     // the voxel's world normal (O11);    backward phase C overwrites .xyz with T alpha g_N
+  BatchShared<NRM> b;
+  float4 dir[32];               // per pixel: its ray direction in the frame of the list being served (copied into every item)
+  float4 acc[32];               // forward, per pixel between batches: C (rgb) and D
+  float2 tn[32];                //          T and n_used (as bits)
+  float4 nacc[NRM ? 32 : 1];    //          N (O11)
+  // the warp's position in its hit-record stream (dvx_internal.cuh)
+  unsigned long long rec_ptr;   // next batch slot
+  uint32_t rec_left;            // slots left in the current chunk
+  uint32_t rec_n;               // batches written so far
+  uint32_t rec_chunk;           // current chunk
+  uint32_t rec_ok;              // 0 once the pool is exhausted
 };
 
 struct Pix {
@@ -147,39 +166,47 @@ struct ItemGeom {
   float delta;       // (b - a) / K
 };
 
-// O6 for one queued item (ring slot `at`): K-point midpoint rule on the clipped segment.  Returns tau_v; with GRAD also
-// the moments M_j = sum_k act'(raw_k) lambda_k^j (j = 0..3), from which phase B2 rebuilds sum_k act'(raw_k) w_c(u_k).
-template <bool BWD, bool NRM>
-__device__ __forceinline__ float integrate_item(const CompositeArgs &A, const WarpQueue<BWD, NRM> &Q, const uint4 *s_tree, int at,
-                                                uint32_t &id, uint32_t &meta, ItemGeom &G, float M[4]) {
-  id = Q.item[at].id;
-  meta = Q.item[at].meta;
-  const uint4 tf = s_tree[(meta >> 8) & 0xFFu];  // geo pointer, base, 1 / cell of the item's octree (per-CTA table)
-  const uint32_t level = meta >> 16;
-  const float *geo = reinterpret_cast<const float *>(((unsigned long long)tf.y << 32) | tf.x);
-  const float4 *gp = reinterpret_cast<const float4 *>(geo + (size_t)(id - tf.z) * 8);
-  const float4 g0 = __ldg(gp), g1 = __ldg(gp + 1);
-  const float g[8] = {g0.x, g0.y, g0.z, g0.w, g1.x, g1.y, g1.z, g1.w};
-  // 1 / edge length = (1 / level-16 cell) * 2^(level - 16): exact power-of-two scaling
-  const float inv_s = __uint_as_float(tf.w) * __uint_as_float((111u + level) << 23);
+// One queued item (ring slot `at`) as phase B needs it: voxel, tree / level, and the clipped segment in the voxel's local
+// coordinates, u(lambda) = p + q lambda with u clamped to [0,1]^3 (O6).
+template <bool NRM>
+__device__ __forceinline__ void item_geom(const CompositeArgs &A, const WarpQueue<NRM> &Q, const uint4 *s_tree, int at,
+                                          uint32_t &id, uint32_t &meta, ItemGeom &G, float &mid) {
   const float4 i0 = *reinterpret_cast<const float4 *>(&Q.item[at]);        // id, meta, ca, cb
   const float4 i1 = *(reinterpret_cast<const float4 *>(&Q.item[at]) + 1);  // w, mid
-  const float4 i2 = *(reinterpret_cast<const float4 *>(&Q.item[at]) + 2);  // d, tau
+  const float4 i2 = *(reinterpret_cast<const float4 *>(&Q.item[at]) + 2);  // d
+  id = __float_as_uint(i0.x);
+  meta = __float_as_uint(i0.y);
+  mid = i1.w;
+  const uint32_t level = meta >> 16;
+  // 1 / edge length = (1 / level-16 cell) * 2^(level - 16): exact power-of-two scaling
+  const float inv_s = __uint_as_float(s_tree[(meta >> 8) & 0xFFu].w) * __uint_as_float((111u + level) << 23);
   const float ca = i0.z, cb = i0.w;
   const float dd[3] = {i2.x, i2.y, i2.z}, ww[3] = {i1.x, i1.y, i1.z};
 #pragma unroll
   for (int ax = 0; ax < 3; ++ax) {
     const float d = dd[ax], w = ww[ax];
-    const float pa = __saturatef(fmaf(fmaf(ca, d, w), inv_s, 0.5f));   // u clamped to [0,1]^3 (O6)
+    const float pa = __saturatef(fmaf(fmaf(ca, d, w), inv_s, 0.5f));
     const float pb = __saturatef(fmaf(fmaf(cb, d, w), inv_s, 0.5f));
     G.p[ax] = pa;
     G.q[ax] = pb - pa;
   }
+  G.delta = (cb - ca) * A.p.inv_k;
+}
+
+// O6 for one item: K-point midpoint rule on the clipped segment.  Returns tau_v; with BWD also the moments
+// M_j = sum_k act'(raw_k) lambda_k^j (j = 0..3), from which phase B2 rebuilds sum_k act'(raw_k) w_c(u_k).
+template <bool BWD>
+__device__ __forceinline__ float integrate_geom(const CompositeArgs &A, const uint4 *s_tree, uint32_t id, uint32_t meta,
+                                                const ItemGeom &G, float M[4]) {
+  const uint4 tf = s_tree[(meta >> 8) & 0xFFu];  // geo pointer, base, 1 / cell of the item's octree (per-CTA table)
+  const float *geo = reinterpret_cast<const float *>(((unsigned long long)tf.y << 32) | tf.x);
+  const float4 *gp = reinterpret_cast<const float4 *>(geo + (size_t)(id - tf.z) * 8);
+  const float4 g0 = __ldg(gp), g1 = __ldg(gp + 1);
+  const float g[8] = {g0.x, g0.y, g0.z, g0.w, g1.x, g1.y, g1.z, g1.w};
   float c[4];
   cubic_coeffs(g, G.p, G.q, c);
   const uint32_t K = A.p.k_samples, kind = A.p.activation;
   const float invK = A.p.inv_k;
-  G.delta = (cb - ca) * invK;
   float S = 0.f;
   if (BWD) M[0] = M[1] = M[2] = M[3] = 0.f;
   float lam = 0.5f * invK;
@@ -187,16 +214,16 @@ __device__ __forceinline__ float integrate_item(const CompositeArgs &A, const Wa
     const float c0 = c[0] * LOG2E, c1 = c[1] * LOG2E, c2 = c[2] * LOG2E, c3 = c[3] * LOG2E;
 #pragma unroll
     for (int k = 0; k < 8; ++k) {
-      const float l8 = (float)(2 * k + 1) * 0.0625f;
+      const float l8 = (float)(2 * k + 1) * 0.0625f;   // lambda_k and its powers are exact in fp32 (odd / 16, / 256, / 4096)
       const float sig = ex2_approx(fmaf(fmaf(fmaf(c3, l8, c2), l8, c1), l8, c0));
       S += sig;
-      if (BWD) {
-        M[0] += sig;
-        float t = sig * l8; M[1] += t;
-        t *= l8; M[2] += t;
-        t *= l8; M[3] += t;
+      if (BWD) {  // one FFMA per moment with an immediate power of lambda_k
+        M[1] = fmaf(sig, l8, M[1]);
+        M[2] = fmaf(sig, l8 * l8, M[2]);
+        M[3] = fmaf(sig, l8 * l8 * l8, M[3]);
       }
     }
+    if (BWD) M[0] = S;  // act' = act for exp
   } else if (kind == 0) {  // exp: sigma = ex2(raw * log2 e), act' = act
     const float c0 = c[0] * LOG2E, c1 = c[1] * LOG2E, c2 = c[2] * LOG2E, c3 = c[3] * LOG2E;
 #pragma unroll 4
@@ -261,55 +288,51 @@ __device__ __forceinline__ void red_add_v4(float *addr, float x, float y, float 
   asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(addr), "f"(x), "f"(y), "f"(z), "f"(w) : "memory");
 }
 
-// ---- phases B, C (and B2) over the first min(n_items, 32) queued items of the ring ------------------------------------
-// Ring slot of the i-th queued item: (head + i) & (QCAP-1).  my_bits: bit i set <=> queued item i belongs to this pixel.
-template <bool BWD, bool NRM, bool EXP = false>
-__device__ __forceinline__ void flush_batch(const CompositeArgs &A, int lane, WarpQueue<BWD, NRM> &Q, const uint4 *s_tree,
-                                            float *const *s_dgeo, int &n_items, int &head, unsigned long long &my_bits, Pix &S) {
-  const int count = n_items < 32 ? n_items : 32;
-  __syncwarp();
-  // -- B: lane = item
-  ItemGeom G;
-  float M[4];
-  uint32_t my_id = NONE, my_meta = 0;
-  const int at_b = (head + lane) & (QCAP - 1);
-  if (lane < count) {
-    // Storing colour and normal to shared memory keeps every global load out of C's serial loop.
-    // Forward: the colour (and normal) loads go out before the integration so their latency hides under it. Backward keeps
-    // them after it: there the four extra live registers spill (measured: forward 1.39 -> 1.35 ms, backward 1.83 -> 1.87 ms).
-    float4 f1, nv = make_float4(0.f, 0.f, 0.f, 0.f);
-    if (!BWD) {
-      const uint32_t id0 = Q.item[at_b].id;
-      f1 = __ldg(reinterpret_cast<const float4 *>(A.fvox + id0) + 1);
-      if (NRM) nv = __ldg(A.vnrm + id0);
-    }
-    const float tau = integrate_item<BWD, NRM>(A, Q, s_tree, at_b, my_id, my_meta, G, M);
-    if (BWD) {
-      f1 = __ldg(reinterpret_cast<const float4 *>(A.fvox + my_id) + 1);
-      if (NRM) nv = __ldg(A.vnrm + my_id);
-    }
-    const float e = ex2_approx(-tau * LOG2E);
-    const float alpha = tau < 1e-3f ? tau * fmaf(-0.5f, tau, 1.0f) : 1.0f - e;  // 1 - exp(-tau) without cancellation
-    Q.eam[lane] = make_float4(e, alpha, Q.item[at_b].mid, 0.f);
-    Q.rgbm[lane] = f1;
-    if (NRM) Q.nrm[lane] = nv;
+// ---- phases B, C and B2 of one batch of up to 32 items ---------------------------------------------------------------
+// The list-walking kernels take the batch from the head of the warp's ring (flush_batch), the replay kernel from the hit
+// records the forward wrote (composite_replay_kernel); from there on both run the same three phases.
+
+// -- B: lane = item (lanes < count).  tau_v, exp(-tau_v), alpha_v, the voxel's colour (and normal) -> shared memory, so that
+// C's serial per-pixel loop contains no transcendental and no global load.
+// Forward: the colour (and normal) loads go out before the integration so their latency hides under it.  Backward keeps
+// them after it: there the four extra live registers spill (measured: forward 1.39 -> 1.35 ms, backward 1.83 -> 1.87 ms).
+template <bool BWD, bool NRM>
+__device__ __forceinline__ void phase_B(const CompositeArgs &A, const uint4 *s_tree, int lane, BatchShared<NRM> &bs, uint32_t id,
+                                        uint32_t meta, const ItemGeom &G, float mid, float M[4]) {
+  float4 f1, nv = make_float4(0.f, 0.f, 0.f, 0.f);
+  if (!BWD) {
+    f1 = __ldg(reinterpret_cast<const float4 *>(A.fvox + id) + 1);
+    if (NRM) nv = __ldg(A.vnrm + id);
   }
-  __syncwarp();
-  // -- C: lane = pixel; its own items of the batch in queue order = front-to-back order along its ray
-  uint32_t mine = (uint32_t)my_bits;
-  if (count < 32) mine &= (1u << count) - 1u;
+  const float tau = integrate_geom<BWD>(A, s_tree, id, meta, G, M);
+  if (BWD) {
+    f1 = __ldg(reinterpret_cast<const float4 *>(A.fvox + id) + 1);
+    if (NRM) nv = __ldg(A.vnrm + id);
+  }
+  const float e = ex2_approx(-tau * LOG2E);
+  const float alpha = tau < 1e-3f ? tau * fmaf(-0.5f, tau, 1.0f) : 1.0f - e;  // 1 - exp(-tau) without cancellation
+  bs.eam[lane] = make_float4(e, alpha, mid, __uint_as_float(id));
+  bs.rgbm[lane] = f1;
+  if (NRM) bs.nrm[lane] = nv;
+}
+
+// -- C: lane = pixel; its own items of the batch (bit i of `mine` = item i) in batch order = front-to-back order along its
+// ray: T, C, D update and the T < t_stop test after every voxel (R3).  The backward leaves dL/dtau_v and T alpha g_C (g_N)
+// per item in shared memory for B2.
+template <bool BWD, bool NRM, bool EXP>
+__device__ __forceinline__ void phase_C(const CompositeArgs &A, BatchShared<NRM> &bs, uint32_t mine, Pix &S) {
   while (mine) {
     const int i = __ffs(mine) - 1;
     mine &= mine - 1;
     if (!S.done) {
-      const float4 f1 = Q.rgbm[i];
-      const float4 ea = Q.eam[i];
+      const float4 f1 = bs.rgbm[i];
+      const float4 ea = bs.eam[i];
       const float e = ea.x, mid = ea.z;
       const float w = S.T * ea.y;
       if (EXP) {  // row N3: the compositing weight of this (pixel, voxel), in the pixel's front-to-back order
         if (S.n_used < S.n_stop) {
           const uint32_t at = S.exp_pos + S.n_used;
-          A.exp_vox[at] = Q.item[(head + i) & (QCAP - 1)].id;
+          A.exp_vox[at] = __float_as_uint(ea.w);
           A.exp_w[at] = w;
         }
       }
@@ -317,20 +340,20 @@ __device__ __forceinline__ void flush_batch(const CompositeArgs &A, int lane, Wa
         S.C0 = fmaf(w, f1.x, S.C0); S.C1 = fmaf(w, f1.y, S.C1); S.C2 = fmaf(w, f1.z, S.C2);
         S.D = fmaf(w, mid, S.D);
         if (NRM) {
-          const float4 nv = Q.nrm[i];
+          const float4 nv = bs.nrm[i];
           S.N0 = fmaf(w, nv.x, S.N0); S.N1 = fmaf(w, nv.y, S.N1); S.N2 = fmaf(w, nv.z, S.N2);
         }
       } else {
         float X = S.gC0 * f1.x + S.gC1 * f1.y + S.gC2 * f1.z + S.gD * mid;
         if (NRM) {
-          const float4 nv = Q.nrm[i];
+          const float4 nv = bs.nrm[i];
           X += S.gN0 * nv.x + S.gN1 * nv.y + S.gN2 * nv.z;
-          Q.nrm[i] = make_float4(w * S.gN0, w * S.gN1, w * S.gN2, 0.f);
+          bs.nrm[i] = make_float4(w * S.gN0, w * S.gN1, w * S.gN2, 0.f);
         }
         S.Xpre = fmaf(w, X, S.Xpre);
-        Q.eam[i].w = S.T * e * X - (S.Xtot - S.Xpre) + S.gA * S.T_final;  // dL/dtau_v
+        bs.eam[i].w = S.T * e * X - (S.Xtot - S.Xpre) + S.gA * S.T_final;  // dL/dtau_v
         const uint32_t cm = __float_as_uint(f1.w);  // colour clamp active: no gradient through that channel (O7)
-        Q.rgbm[i] = make_float4((cm & 1u) ? 0.f : w * S.gC0, (cm & 2u) ? 0.f : w * S.gC1, (cm & 4u) ? 0.f : w * S.gC2, 0.f);
+        bs.rgbm[i] = make_float4((cm & 1u) ? 0.f : w * S.gC0, (cm & 2u) ? 0.f : w * S.gC1, (cm & 4u) ? 0.f : w * S.gC2, 0.f);
       }
       S.T *= e;
       S.n_used++;
@@ -340,84 +363,168 @@ __device__ __forceinline__ void flush_batch(const CompositeArgs &A, int lane, Wa
         if (S.n_used >= S.n_stop) S.done = true;
       }
     } else if (BWD) {  // queued before this pixel finished its replay: contributes nothing
-      Q.eam[i].w = 0.f;
-      Q.rgbm[i] = make_float4(0.f, 0.f, 0.f, 0.f);
-      if (NRM) Q.nrm[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+      bs.eam[i].w = 0.f;
+      bs.rgbm[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+      if (NRM) bs.nrm[i] = make_float4(0.f, 0.f, 0.f, 0.f);
     }
   }
-  my_bits >>= count;
-  __syncwarp();
-  // -- B2 (backward): lane = item again; corner gradients, run-reduced by voxel, vector reductions
-  if (BWD) {
-    constexpr int NV = NRM ? 14 : 11;  // 8 corner gradients, 3 colour, (3 normal)
-    float val[NV];
+}
+
+// -- B2 (backward): lane = item again; corner gradients, run-reduced by voxel, vector reductions
+template <bool NRM>
+__device__ __forceinline__ void phase_B2(const CompositeArgs &A, int lane, int count, const BatchShared<NRM> &bs, const uint4 *s_tree,
+                                         float *const *s_dgeo, uint32_t my_id, uint32_t my_meta, const ItemGeom &G, const float M[4]) {
+  constexpr int NV = NRM ? 14 : 11;  // 8 corner gradients, 3 colour, (3 normal)
+  float val[NV];
 #pragma unroll
-    for (int c = 0; c < NV; ++c) val[c] = 0.f;
-    if (lane < count) {
-      const float dtau = Q.eam[lane].w * G.delta;
-      float cs[8];
-      corner_sums(G, M, cs);
+  for (int c = 0; c < NV; ++c) val[c] = 0.f;
+  if (lane < count) {
+    const float dtau = bs.eam[lane].w * G.delta;
+    float cs[8];
+    corner_sums(G, M, cs);
 #pragma unroll
-      for (int c = 0; c < 8; ++c) val[c] = dtau * cs[c];
-      const float4 wc = Q.rgbm[lane];
-      val[8] = wc.x; val[9] = wc.y; val[10] = wc.z;
-      if (NRM) { const float4 wn = Q.nrm[lane]; val[NV - 3] = wn.x; val[NV - 2] = wn.y; val[NV - 1] = wn.z; }
+    for (int c = 0; c < 8; ++c) val[c] = dtau * cs[c];
+    const float4 wc = bs.rgbm[lane];
+    val[8] = wc.x; val[9] = wc.y; val[10] = wc.z;
+    if (NRM) { const float4 wn = bs.nrm[lane]; val[NV - 3] = wn.x; val[NV - 2] = wn.y; val[NV - 1] = wn.z; }
+  }
+  // runs of consecutive items of one voxel (the pixels one list entry hit): segmented suffix sums over the run index,
+  // the first lane of each run ends up with the run total.  (The voxel id itself is not a valid segment key: a voxel cut
+  // in two by a box is queued twice, with other voxels in between.)
+  const uint32_t prev = __shfl_up_sync(0xffffffffu, my_id, 1);
+  const bool is_head = lane == 0 || prev != my_id;
+  const uint32_t heads = __ballot_sync(0xffffffffu, is_head);
+  // Runs longer than DVX_RUN_SPLIT lanes are first reduced in pieces of that length (log2(DVX_RUN_SPLIT) scan steps
+  // instead of 5) and each piece issues its own reductions: the L2 absorbs ~3x more of them cheaper than three more
+  // shuffle rounds.  Not so where many warps hammer the same voxel: when the whole batch is one run (count >= DVX_RUN_LONG
+  // x runs; a voxel that covers the warp's 4x8 pixels covers its neighbours' too) the pieces are merged with the remaining
+  // scan steps, keyed by the true run.  Measured (backward compositing, ms): config 4 3.29 -> 2.78, config 3 1.83 -> 1.85;
+  // thresholds 6, 8, 12, 16, 24: config 4 2.98, 2.96, 2.89, 2.89, 2.78, config 3 1.98, 1.97, 1.91, 1.91, 1.85.  Warp-uniform.
+  uint32_t heads2 = heads;
+  {
+    const uint32_t below = heads & (0xffffffffu >> (31 - lane));       // heads at or below this lane
+    const int start = 31 - __clz(below);                                // lane of this run's head
+    const bool extra = lane > start && ((lane - start) % DVX_RUN_SPLIT) == 0;
+    heads2 |= __ballot_sync(0xffffffffu, extra);
+  }
+  const bool merge = count >= DVX_RUN_LONG * __popc(heads);
+  const bool is_head2 = ((merge ? heads : heads2) >> lane) & 1u;
+  const uint32_t run2 = __popc(heads2 & (0xffffffffu >> (31 - lane)));
+#pragma unroll
+  for (int o = 1; o < DVX_RUN_SPLIT; o <<= 1) {
+    const uint32_t orun = __shfl_down_sync(0xffffffffu, run2, o);
+    const bool take = (lane + o < 32) && orun == run2;
+#pragma unroll
+    for (int c = 0; c < NV; ++c) {
+      const float x = __shfl_down_sync(0xffffffffu, val[c], o);
+      if (take) val[c] += x;
     }
-    // runs of consecutive items of one voxel (the pixels one list entry hit): segmented suffix sums over the run index,
-    // the first lane of each run ends up with the run total.  (The voxel id itself is not a valid segment key: a voxel cut
-    // in two by a box is queued twice, with other voxels in between.)
-    const uint32_t prev = __shfl_up_sync(0xffffffffu, my_id, 1);
-    const bool is_head = lane == 0 || prev != my_id;
-    const uint32_t heads = __ballot_sync(0xffffffffu, is_head);
-    // Runs longer than DVX_RUN_SPLIT lanes are first reduced in pieces of that length (log2(DVX_RUN_SPLIT) scan steps
-    // instead of 5) and each piece issues its own reductions: the L2 absorbs ~3x more of them cheaper than three more
-    // shuffle rounds.  Not so where many warps hammer the same voxel: when the whole batch is one run (count >= DVX_RUN_LONG
-    // x runs; a voxel that covers the warp's 4x8 pixels covers its neighbours' too) the pieces are merged with the remaining
-    // scan steps, keyed by the true run.  Measured (backward compositing, ms): config 4 3.29 -> 2.78, config 3 1.83 -> 1.85;
-    // thresholds 6, 8, 12, 16, 24: config 4 2.98, 2.96, 2.89, 2.89, 2.78, config 3 1.98, 1.97, 1.91, 1.91, 1.85.  Warp-uniform.
-    uint32_t heads2 = heads;
-    {
-      const uint32_t below = heads & (0xffffffffu >> (31 - lane));       // heads at or below this lane
-      const int start = 31 - __clz(below);                                // lane of this run's head
-      const bool extra = lane > start && ((lane - start) % DVX_RUN_SPLIT) == 0;
-      heads2 |= __ballot_sync(0xffffffffu, extra);
-    }
-    const bool merge = count >= DVX_RUN_LONG * __popc(heads);
-    const bool is_head2 = ((merge ? heads : heads2) >> lane) & 1u;
-    const uint32_t run2 = __popc(heads2 & (0xffffffffu >> (31 - lane)));
+  }
+  if (merge) {  // piece heads sit DVX_RUN_SPLIT lanes apart within a run: the scan continues over them
+    const uint32_t run1 = __popc(heads & (0xffffffffu >> (31 - lane)));
 #pragma unroll
-    for (int o = 1; o < DVX_RUN_SPLIT; o <<= 1) {
-      const uint32_t orun = __shfl_down_sync(0xffffffffu, run2, o);
-      const bool take = (lane + o < 32) && orun == run2;
+    for (int o = DVX_RUN_SPLIT; o < 32; o <<= 1) {
+      const uint32_t orun = __shfl_down_sync(0xffffffffu, run1, o);
+      const bool take = (lane + o < 32) && orun == run1;
 #pragma unroll
       for (int c = 0; c < NV; ++c) {
         const float x = __shfl_down_sync(0xffffffffu, val[c], o);
         if (take) val[c] += x;
       }
     }
-    if (merge) {  // piece heads sit DVX_RUN_SPLIT lanes apart within a run: the scan continues over them
-      const uint32_t run1 = __popc(heads & (0xffffffffu >> (31 - lane)));
-#pragma unroll
-      for (int o = DVX_RUN_SPLIT; o < 32; o <<= 1) {
-        const uint32_t orun = __shfl_down_sync(0xffffffffu, run1, o);
-        const bool take = (lane + o < 32) && orun == run1;
-#pragma unroll
-        for (int c = 0; c < NV; ++c) {
-          const float x = __shfl_down_sync(0xffffffffu, val[c], o);
-          if (take) val[c] += x;
-        }
-      }
+  }
+  if (my_id != NONE && is_head2) {
+    const uint32_t ti = (my_meta >> 8) & 0xFFu;
+    if (s_dgeo[ti]) {
+      float *dg = s_dgeo[ti] + (size_t)(my_id - s_tree[ti].z) * 8;
+      red_add_v4(dg, val[0], val[1], val[2], val[3]);
+      red_add_v4(dg + 4, val[4], val[5], val[6], val[7]);
     }
-    if (my_id != NONE && is_head2) {
-      const uint32_t ti = (my_meta >> 8) & 0xFFu;
-      if (s_dgeo[ti]) {
-        float *dg = s_dgeo[ti] + (size_t)(my_id - s_tree[ti].z) * 8;
-        red_add_v4(dg, val[0], val[1], val[2], val[3]);
-        red_add_v4(dg + 4, val[4], val[5], val[6], val[7]);
+    red_add_v4(A.drgb + (size_t)my_id * 4, val[8], val[9], val[10], 0.f);
+    if (NRM) red_add_v4(A.dnrm + (size_t)my_id * 4, val[NV - 3], val[NV - 2], val[NV - 1], 0.f);
+  }
+}
+
+// The next batch slot of this warp's hit-record stream, or NULL once the pool is exhausted (warp-uniform).  A new chunk is
+// taken from the pool every DVX_REC_CHUNK batches with one atomic and linked behind the previous one.
+template <bool NRM>
+__device__ __forceinline__ unsigned char *rec_next_block(const CompositeArgs &A, int lane, uint32_t warp_global, WarpQueue<NRM> &Q) {
+  if (Q.rec_left == 0) {  // rare path: first batch, chunk boundary, or no pool left
+    if (!Q.rec_ok) return nullptr;
+    uint32_t c = 0;
+    if (lane == 0) c = (uint32_t)atomicAdd(&A.counters[CNT_REC_CHUNKS], 1ull);
+    c = __shfl_sync(0xffffffffu, c, 0);
+    if (c >= A.rec_cap) {
+      if (lane == 0) {
+        Q.rec_ok = 0;
+        atomicOr(reinterpret_cast<unsigned int *>(&A.counters[CNT_REC_OVERFLOW]), 1u);
       }
-      red_add_v4(A.drgb + (size_t)my_id * 4, val[8], val[9], val[10], 0.f);
-      if (NRM) red_add_v4(A.dnrm + (size_t)my_id * 4, val[NV - 3], val[NV - 2], val[NV - 1], 0.f);
+      __syncwarp();
+      return nullptr;
     }
+    if (lane == 0) {
+      if (Q.rec_n == 0) A.rec_tab[2 * warp_global] = c;
+      else A.rec_next[Q.rec_chunk] = c;
+      Q.rec_chunk = c;
+      Q.rec_left = DVX_REC_CHUNK;
+      Q.rec_ptr = reinterpret_cast<unsigned long long>(A.rec_pool) + (unsigned long long)c * (DVX_REC_CHUNK * DVX_REC_BATCH_BYTES);
+    }
+    __syncwarp();
+  }
+  unsigned char *blk = reinterpret_cast<unsigned char *>(Q.rec_ptr);
+  __syncwarp();
+  if (lane == 0) {
+    Q.rec_ptr += DVX_REC_BATCH_BYTES;
+    Q.rec_left -= 1;
+    Q.rec_n += 1;
+  }
+  return blk;
+}
+
+// Phases B, C (and B2) over the first min(n_items, 32) queued items of the ring.
+// Ring slot of the i-th queued item: (head + i) & (QCAP-1).  my_bits: bit i set <=> queued item i belongs to this pixel.
+template <bool BWD, bool NRM, bool EXP, bool REC>
+__device__ __forceinline__ void flush_batch(const CompositeArgs &A, int lane, WarpQueue<NRM> &Q, const uint4 *s_tree,
+                                            float *const *s_dgeo, int &n_items, int &head, unsigned long long &my_bits, Pix &S,
+                                            uint32_t warp_global) {
+  const int count = n_items < 32 ? n_items : 32;
+  unsigned char *blk = nullptr;
+  if (REC) blk = rec_next_block<NRM>(A, lane, warp_global, Q);
+  __syncwarp();
+  ItemGeom G;
+  float M[4];
+  uint32_t my_id = NONE, my_meta = 0;
+  if (lane < count) {
+    float mid;
+    item_geom<NRM>(A, Q, s_tree, (head + lane) & (QCAP - 1), my_id, my_meta, G, mid);
+    if (REC && blk) {
+      unsigned char *mine_rec = blk + 16 * lane;
+      __stcs(reinterpret_cast<float4 *>(mine_rec), make_float4(__uint_as_float(my_id), __uint_as_float(my_meta), G.delta, mid));
+      __stcs(reinterpret_cast<float4 *>(mine_rec + 512), make_float4(G.p[0], G.p[1], G.p[2], G.q[0]));
+      __stcs(reinterpret_cast<float2 *>(blk + 1024 + 8 * lane), make_float2(G.q[1], G.q[2]));
+    }
+    phase_B<BWD, NRM>(A, s_tree, lane, Q.b, my_id, my_meta, G, mid, M);
+  }
+  uint32_t mine = (uint32_t)my_bits;
+  if (count < 32) mine &= (1u << count) - 1u;
+  if (REC && blk) __stcs(reinterpret_cast<uint32_t *>(blk + 1280) + lane, mine);
+  __syncwarp();
+  if (!BWD) {  // the pixel's running sums live in shared memory between batches
+    const float4 a4 = Q.acc[lane];
+    const float2 t2 = Q.tn[lane];
+    S.C0 = a4.x; S.C1 = a4.y; S.C2 = a4.z; S.D = a4.w; S.T = t2.x; S.n_used = __float_as_uint(t2.y);
+    if (NRM) { const float4 n4 = Q.nacc[lane]; S.N0 = n4.x; S.N1 = n4.y; S.N2 = n4.z; }
+  }
+  phase_C<BWD, NRM, EXP>(A, Q.b, mine, S);
+  if (!BWD) {
+    Q.acc[lane] = make_float4(S.C0, S.C1, S.C2, S.D);
+    Q.tn[lane] = make_float2(S.T, __uint_as_float(S.n_used));
+    if (NRM) Q.nacc[lane] = make_float4(S.N0, S.N1, S.N2, 0.f);
+  }
+  my_bits >>= count;
+  __syncwarp();
+  if (BWD) {
+    phase_B2<NRM>(A, lane, count, Q.b, s_tree, s_dgeo, my_id, my_meta, G, M);
     __syncwarp();
   }
   head = (head + count) & (QCAP - 1);
@@ -456,9 +563,40 @@ __device__ __noinline__ float2 axis_parallel_fix(const TreeFrame *T, uint32_t id
   return inside ? make_float2(sa, sb) : make_float2(INFINITY, -INFINITY);
 }
 
-template <bool BWD, bool CNT, bool NRM, bool EXP = false>
+// Per-pixel state of a backward pass: incoming gradients, the forward's saved totals, where the replay stops (R3).
+template <bool NRM>
+__device__ __forceinline__ void backward_pixel_init(const CompositeArgs &A, int u, int v, size_t pix, Pix &S) {
+  S.gC0 = A.g_rgb[3 * pix]; S.gC1 = A.g_rgb[3 * pix + 1]; S.gC2 = A.g_rgb[3 * pix + 2];
+  S.gD = A.g_depth ? A.g_depth[pix] : 0.f;
+  S.gA = A.g_alpha ? A.g_alpha[pix] : 0.f;
+  const float4 cd = reinterpret_cast<const float4 *>(A.sv_rgbd)[pix];
+  S.Xtot = S.gC0 * cd.x + S.gC1 * cd.y + S.gC2 * cd.z + S.gD * cd.w;
+  if (NRM) {
+    S.gN0 = A.g_normal[3 * pix]; S.gN1 = A.g_normal[3 * pix + 1]; S.gN2 = A.g_normal[3 * pix + 2];
+    const float4 nf = reinterpret_cast<const float4 *>(A.sv_nrm)[pix];
+    S.Xtot += S.gN0 * nf.x + S.gN1 * nf.y + S.gN2 * nf.z;
+  }
+  S.T_final = A.sv_T[pix];
+  S.n_stop = A.sv_nused[pix];
+  // Eq. 2: dL/dT_final also has g_C . C_sky; with alpha = 1 - T_final that is an alpha gradient of -(g_C . C_sky)
+  if (A.sky_tex) S.gA -= dvx_sky_backward(&A, u, v, S.gC0, S.gC1, S.gC2, S.T_final);
+  if (S.n_stop == 0) S.done = true;
+}
+
+__device__ __forceinline__ void pixel_state_zero(Pix &S, bool inside) {
+  S.C0 = S.C1 = S.C2 = 0.f; S.D = 0.f; S.T = 1.f; S.n_used = 0; S.done = !inside;
+  S.gC0 = S.gC1 = S.gC2 = S.gD = S.gA = S.Xtot = S.T_final = 0.f;
+  S.Xpre = 0.f; S.n_stop = 0;
+  S.N0 = S.N1 = S.N2 = 0.f; S.gN0 = S.gN1 = S.gN2 = 0.f;
+  S.exp_pos = 0;
+}
+
+// REC (forward, frame saved for a backward): every batch is also appended to the warp's hit-record stream.
+// A BWD launch with a record pool attached is the fall-back of the replay kernel: it only runs when the pool overflowed.
+template <bool BWD, bool CNT, bool NRM, bool EXP = false, bool REC = false>
 __global__ void __launch_bounds__(TILE_THREADS, DVX_TILE_MIN_CTAS) composite_tile_kernel(const __grid_constant__ CompositeArgs A) {
-  __shared__ WarpQueue<BWD, NRM> s_queue[TILE_WARPS];
+  if (BWD && A.rec_pool && A.counters[CNT_REC_OVERFLOW] == 0ull) return;  // the replay kernel did this frame's backward
+  __shared__ WarpQueue<NRM> s_queue[TILE_WARPS];
   // what phase B needs of an item's octree, 16 bytes each: one shared-memory load instead of three dependent global ones
   __shared__ uint4 s_tree[DVX_MAX_ACTORS + 1];
   __shared__ float *s_dgeo[BWD ? DVX_MAX_ACTORS + 1 : 1];
@@ -475,37 +613,25 @@ __global__ void __launch_bounds__(TILE_THREADS, DVX_TILE_MIN_CTAS) composite_til
   const int lane = threadIdx.x & 31;
   const int wu0 = (tile % p.tiles_x) * DVX_TILE + (warp % WARPS_X) * WARP_W;   // pixel of lane 0 of this warp
   const int wv0 = (tile / p.tiles_x) * DVX_TILE + (warp / WARPS_X) * WARP_H;
-  WarpQueue<BWD, NRM> &Q = s_queue[warp_l];
+  WarpQueue<NRM> &Q = s_queue[warp_l];
   const int u = wu0 + lane % WARP_W, v = wv0 + lane / WARP_W;
   const bool inside = u < (int)p.width && v < (int)p.height;
   const size_t pix = (size_t)v * p.width + u;
 
   Pix S;
-  S.C0 = S.C1 = S.C2 = 0.f; S.D = 0.f; S.T = 1.f; S.n_used = 0; S.done = !inside;
-  S.Xpre = 0.f; S.n_stop = 0;
-  S.N0 = S.N1 = S.N2 = 0.f; S.gN0 = S.gN1 = S.gN2 = 0.f;
-  S.exp_pos = 0;
+  pixel_state_zero(S, inside);
   if (EXP && inside) {  // the row lengths are the n_used the rendering pass saved
     S.exp_pos = A.exp_row[pix];
     S.n_stop = A.exp_row[pix + 1] - S.exp_pos;
   }
-  if (BWD && inside) {
-    S.gC0 = A.g_rgb[3 * pix]; S.gC1 = A.g_rgb[3 * pix + 1]; S.gC2 = A.g_rgb[3 * pix + 2];
-    S.gD = A.g_depth ? A.g_depth[pix] : 0.f;
-    S.gA = A.g_alpha ? A.g_alpha[pix] : 0.f;
-    const float4 cd = reinterpret_cast<const float4 *>(A.sv_rgbd)[pix];
-    S.Xtot = S.gC0 * cd.x + S.gC1 * cd.y + S.gC2 * cd.z + S.gD * cd.w;
-    if (NRM) {
-      S.gN0 = A.g_normal[3 * pix]; S.gN1 = A.g_normal[3 * pix + 1]; S.gN2 = A.g_normal[3 * pix + 2];
-      const float4 nf = reinterpret_cast<const float4 *>(A.sv_nrm)[pix];
-      S.Xtot += S.gN0 * nf.x + S.gN1 * nf.y + S.gN2 * nf.z;
-    }
-    S.T_final = A.sv_T[pix];
-    S.n_stop = A.sv_nused[pix];
-    // Eq. 2: dL/dT_final also has g_C . C_sky; with alpha = 1 - T_final that is an alpha gradient of -(g_C . C_sky)
-    if (A.sky_tex) S.gA -= dvx_sky_backward(&A, u, v, S.gC0, S.gC1, S.gC2, S.T_final);
-    if (S.n_stop == 0) S.done = true;
+  if (BWD && inside) backward_pixel_init<NRM>(A, u, v, pix, S);
+  const uint32_t warp_global = (uint32_t)tile * 8u + (uint32_t)warp;
+  if (!BWD) {
+    Q.acc[lane] = make_float4(0.f, 0.f, 0.f, 0.f);
+    Q.tn[lane] = make_float2(1.f, __uint_as_float(0u));
+    if (NRM) Q.nacc[lane] = make_float4(0.f, 0.f, 0.f, 0.f);
   }
+  if (REC && lane == 0) { Q.rec_left = 0; Q.rec_n = 0; Q.rec_chunk = 0; Q.rec_ok = 1; Q.rec_ptr = 0; }
 
   // ---- step 3: intervals of the actors in this tile's mask, insertion-sorted by (tau_in, actor index) (O2, O3)
   float h_in[DVX_MAX_ACTORS], h_out[DVX_MAX_ACTORS];
@@ -590,7 +716,7 @@ __global__ void __launch_bounds__(TILE_THREADS, DVX_TILE_MIN_CTAS) composite_til
     const TreeFrame &T = A.trees[t];
     // ray of this pixel in the frame of tree t: fp64 direction, its fp32 rounding, reciprocal, octant, and the small
     // difference e to the warp's reference direction d0 (= the direction of lane 0's pixel, kept in shared memory)
-    float d[3], inv[3], e[3];
+    float inv[3], e[3];
     int q = 0;
     uint32_t zmask = 0;  // axes on which this ray is exactly axis-parallel (R20), almost always 0
     {
@@ -598,6 +724,7 @@ __global__ void __launch_bounds__(TILE_THREADS, DVX_TILE_MIN_CTAS) composite_til
       pixel_ray_d(p, u, v, xd, yd, rnd);
       const float xp = dvx_cam_x(p, u), yp = dvx_cam_y(p, v);  // fp32 copy: only the octant decision uses it (R12)
       __syncwarp();
+      float d[3];
 #pragma unroll
       for (int a = 0; a < 3; ++a) {
         const double da = (T.Nd[3 * a] * xd + T.Nd[3 * a + 1] * yd + T.Nd[3 * a + 2]) * rnd;
@@ -609,6 +736,7 @@ __global__ void __launch_bounds__(TILE_THREADS, DVX_TILE_MIN_CTAS) composite_til
         inv[a] = d[a] != 0.f ? 1.0f / d[a] : 0.f;
         if (d[a] == 0.f) zmask |= 1u << a;
       }
+      Q.dir[lane] = make_float4(d[0], d[1], d[2], 0.f);  // read back by this lane only, at every emit
       __syncwarp();
     }
     // warp-uniform "some lane is axis-parallel": keeps the R20 test out of the per-candidate loop (the forward otherwise
@@ -683,12 +811,12 @@ __global__ void __launch_bounds__(TILE_THREADS, DVX_TILE_MIN_CTAS) composite_til
               float4 *it = reinterpret_cast<float4 *>(&Q.item[(head + rel_at) & (QCAP - 1)]);
               it[0] = make_float4(__uint_as_float(r1.x), __uint_as_float(r1.y), ca, cb);
               it[1] = make_float4(w0, w1, w2, r0.x + 0.5f * (ca + cb));
-              it[2] = make_float4(d[0], d[1], d[2], 0.f);
+              it[2] = Q.dir[lane];
               my_bits |= 1ull << rel_at;
             }
             n_items += __popc(mk);
             if (n_items >= 32) {
-              flush_batch<BWD, NRM, EXP>(A, lane, Q, s_tree, s_dgeo, n_items, head, my_bits, S);
+              flush_batch<BWD, NRM, EXP, REC>(A, lane, Q, s_tree, s_dgeo, n_items, head, my_bits, S, warp_global);
               if (S.done) c_t = NONE;
             }
           }
@@ -704,8 +832,15 @@ __global__ void __launch_bounds__(TILE_THREADS, DVX_TILE_MIN_CTAS) composite_til
     }
     if (part) seg_tree = NONE;          // served
   }
-  while (n_items > 0) flush_batch<BWD, NRM, EXP>(A, lane, Q, s_tree, s_dgeo, n_items, head, my_bits, S);
+  while (n_items > 0) flush_batch<BWD, NRM, EXP, REC>(A, lane, Q, s_tree, s_dgeo, n_items, head, my_bits, S, warp_global);
 
+  if (REC && lane == 0) A.rec_tab[2 * warp_global + 1] = Q.rec_ok ? Q.rec_n : 0u;
+  if (!BWD) {
+    const float4 a4 = Q.acc[lane];
+    const float2 t2 = Q.tn[lane];
+    S.C0 = a4.x; S.C1 = a4.y; S.C2 = a4.z; S.D = a4.w; S.T = t2.x; S.n_used = __float_as_uint(t2.y);
+    if (NRM) { const float4 n4 = Q.nacc[lane]; S.N0 = n4.x; S.N1 = n4.y; S.N2 = n4.z; }
+  }
   if (!BWD && !EXP && inside) {
     float3 sky = make_float3(0.f, 0.f, 0.f);
     if (A.sky_tex) sky = dvx_sky_forward(&A, u, v, S.T);  // Eq. 2: C = C_voxels + T_final C_sky
@@ -735,6 +870,91 @@ __global__ void __launch_bounds__(TILE_THREADS, DVX_TILE_MIN_CTAS) composite_til
   }
 }
 
+
+// ---- backward from the hit records -------------------------------------------------------------------------------------
+// Step 5 without steps 3-4's geometry: the forward left every batch it composited (voxel, local segment, owner masks) in the
+// warp's record stream, so the backward needs no list walk, no slab test, no interval schedule and no queue: per batch it
+// loads the records (three coalesced loads, the next batch prefetched under the current one), integrates with moments
+// (phase B), replays the pixels' blend order (phase C) and reduces the gradients (phase B2).
+// Same grid and warp -> pixel-block mapping as the forward.
+#ifndef DVX_REPLAY_MIN_CTAS
+#define DVX_REPLAY_MIN_CTAS (4 * DVX_TILE_SPLIT)
+#endif
+struct RecBatch {
+  uint4 a;      // id, meta, delta, mid
+  float4 b;     // p, q_x
+  float2 c;     // q_y, q_z
+  uint32_t mask;
+};
+__device__ __forceinline__ RecBatch rec_load(const unsigned char *blk, int lane) {
+  RecBatch r;
+  r.a = __ldcs(reinterpret_cast<const uint4 *>(blk) + lane);
+  r.b = __ldcs(reinterpret_cast<const float4 *>(blk + 512) + lane);
+  r.c = __ldcs(reinterpret_cast<const float2 *>(blk + 1024) + lane);
+  r.mask = __ldcs(reinterpret_cast<const uint32_t *>(blk + 1280) + lane);
+  return r;
+}
+
+template <bool NRM>
+__global__ void __launch_bounds__(TILE_THREADS, DVX_REPLAY_MIN_CTAS) composite_replay_kernel(const __grid_constant__ CompositeArgs A) {
+  if (A.counters[CNT_REC_OVERFLOW] != 0ull) return;  // incomplete records: the list-walking backward runs instead
+  __shared__ BatchShared<NRM> s_b[TILE_WARPS];
+  __shared__ uint4 s_tree[DVX_MAX_ACTORS + 1];
+  __shared__ float *s_dgeo[DVX_MAX_ACTORS + 1];
+  const FrameParams &p = A.p;
+  for (uint32_t i = threadIdx.x; i < p.n_trees; i += TILE_THREADS) {
+    const TreeFrame &Ti = A.trees[i];
+    const unsigned long long ga = reinterpret_cast<unsigned long long>(Ti.geo);
+    s_tree[i] = make_uint4((uint32_t)ga, (uint32_t)(ga >> 32), Ti.base, __float_as_uint(Ti.inv_cell_f));
+    s_dgeo[i] = Ti.dgeo;
+  }
+  const int tile = A.tile_order ? (int)__ldg(A.tile_order + blockIdx.x / TILE_SPLIT) : (int)(blockIdx.x / TILE_SPLIT);
+  const int warp_l = threadIdx.x >> 5;
+  const int warp = (int)(blockIdx.x % TILE_SPLIT) * TILE_WARPS + warp_l;
+  const int lane = threadIdx.x & 31;
+  const int u = (tile % p.tiles_x) * DVX_TILE + (warp % WARPS_X) * WARP_W + lane % WARP_W;
+  const int v = (tile / p.tiles_x) * DVX_TILE + (warp / WARPS_X) * WARP_H + lane / WARP_W;
+  const bool inside = u < (int)p.width && v < (int)p.height;
+  const size_t pix = (size_t)v * p.width + u;
+  BatchShared<NRM> &bs = s_b[warp_l];
+  Pix S;
+  pixel_state_zero(S, inside);
+  if (inside) backward_pixel_init<NRM>(A, u, v, pix, S);
+  const uint32_t warp_global = (uint32_t)tile * 8u + (uint32_t)warp;
+  const uint32_t nb = A.rec_tab[2 * warp_global + 1];
+  uint32_t chunk = nb ? A.rec_tab[2 * warp_global] : 0u;
+  __syncthreads();  // s_tree / s_dgeo
+  if (nb == 0) return;
+  RecBatch cur = rec_load(A.rec_pool + (size_t)chunk * DVX_REC_CHUNK * DVX_REC_BATCH_BYTES, lane);
+  for (uint32_t b = 0; b < nb; ++b) {
+    if (__all_sync(0xffffffffu, S.done)) break;  // every pixel of the block has replayed its n_used voxels
+    // -- prefetch the next batch (a chunk's successor is read when its last slot is reached)
+    RecBatch nxt = cur;
+    if (b + 1 < nb) {
+      const uint32_t slot = (b + 1) & (DVX_REC_CHUNK - 1u);
+      if (slot == 0) chunk = __ldg(A.rec_next + chunk);
+      nxt = rec_load(A.rec_pool + ((size_t)chunk * DVX_REC_CHUNK + slot) * DVX_REC_BATCH_BYTES, lane);
+    }
+    const int count = __popc(__reduce_or_sync(0xffffffffu, cur.mask));  // every item of the batch has one owner
+    ItemGeom G;
+    float M[4];
+    uint32_t my_id = NONE, my_meta = 0;
+    if (lane < count) {
+      my_id = cur.a.x; my_meta = cur.a.y;
+      G.delta = __uint_as_float(cur.a.z);
+      G.p[0] = cur.b.x; G.p[1] = cur.b.y; G.p[2] = cur.b.z;
+      G.q[0] = cur.b.w; G.q[1] = cur.c.x; G.q[2] = cur.c.y;
+      phase_B<true, NRM>(A, s_tree, lane, bs, my_id, my_meta, G, __uint_as_float(cur.a.w), M);
+    }
+    __syncwarp();
+    phase_C<true, NRM, false>(A, bs, cur.mask, S);
+    __syncwarp();
+    phase_B2<NRM>(A, lane, count, bs, s_tree, s_dgeo, my_id, my_meta, G, M);
+    __syncwarp();
+    cur = nxt;
+  }
+}
+
 }  // namespace
 
 // Row N3: the forward walk once more, writing the compositing weights (voxel, T alpha) of every pixel into the CSR rows
@@ -750,14 +970,27 @@ void dvx_composite_tile_launch(const CompositeArgs &a, bool backward, cudaStream
   DVX_COUNT_LAUNCH(1);
   const bool cnt = (a.p.flags & DVX_FLAG_COUNTERS) != 0;
   const bool nrm = backward ? (a.g_normal != nullptr) : (a.normal != nullptr);  // normal map requested (O11)
+  const bool rec = !backward && a.rec_pool != nullptr;                           // forward of a saved frame: write hit records
+  const unsigned grid = a.p.n_tiles * TILE_SPLIT;
   if (backward) {
-    if (nrm) composite_tile_kernel<true, false, true><<<a.p.n_tiles * TILE_SPLIT, TILE_THREADS, 0, st>>>(a);
-    else composite_tile_kernel<true, false, false><<<a.p.n_tiles * TILE_SPLIT, TILE_THREADS, 0, st>>>(a);
+    if (nrm) composite_tile_kernel<true, false, true><<<grid, TILE_THREADS, 0, st>>>(a);
+    else composite_tile_kernel<true, false, false><<<grid, TILE_THREADS, 0, st>>>(a);
   } else if (nrm) {
-    composite_tile_kernel<false, false, true><<<a.p.n_tiles * TILE_SPLIT, TILE_THREADS, 0, st>>>(a);
+    if (rec) composite_tile_kernel<false, false, true, false, true><<<grid, TILE_THREADS, 0, st>>>(a);
+    else composite_tile_kernel<false, false, true><<<grid, TILE_THREADS, 0, st>>>(a);
   } else if (cnt) {
-    composite_tile_kernel<false, true, false><<<a.p.n_tiles * TILE_SPLIT, TILE_THREADS, 0, st>>>(a);
+    if (rec) composite_tile_kernel<false, true, false, false, true><<<grid, TILE_THREADS, 0, st>>>(a);
+    else composite_tile_kernel<false, true, false><<<grid, TILE_THREADS, 0, st>>>(a);
   } else {
-    composite_tile_kernel<false, false, false><<<a.p.n_tiles * TILE_SPLIT, TILE_THREADS, 0, st>>>(a);
+    if (rec) composite_tile_kernel<false, false, false, false, true><<<grid, TILE_THREADS, 0, st>>>(a);
+    else composite_tile_kernel<false, false, false><<<grid, TILE_THREADS, 0, st>>>(a);
   }
+}
+
+void dvx_composite_replay_launch(const CompositeArgs &a, cudaStream_t st) {
+  if (a.p.n_tiles == 0) return;
+  DVX_COUNT_LAUNCH(1);
+  const unsigned grid = a.p.n_tiles * TILE_SPLIT;
+  if (a.g_normal) composite_replay_kernel<true><<<grid, TILE_THREADS, 0, st>>>(a);
+  else composite_replay_kernel<false><<<grid, TILE_THREADS, 0, st>>>(a);
 }

@@ -49,7 +49,27 @@ struct __align__(16) FrameVox {
   uint32_t meta;  // bits 0-2: colour channel clamped at 0 (gradient blocked)
 };
 
-enum { CNT_PAIRS = 0, CNT_VVIS = 1, CNT_QTEST = 2, CNT_QHIT = 3, CNT_PAIRS_EFF = 4, CNT_OVERFLOW = 5, CNT_EMIT = 6, CNT_N = 8 };
+enum { CNT_PAIRS = 0, CNT_VVIS = 1, CNT_QTEST = 2, CNT_QHIT = 3, CNT_PAIRS_EFF = 4, CNT_OVERFLOW = 5, CNT_EMIT = 6,
+       CNT_REC_CHUNKS = 7,    // hit-record chunks handed out by the forward (may exceed the capacity: then CNT_REC_OVERFLOW is set)
+       CNT_REC_OVERFLOW = 8,  // != 0: the record pool was too small, the backward re-walks the lists instead of replaying
+       CNT_N = 12 };
+
+// ---- hit records (forward -> backward): what the forward composited, in the order it composited it ------------------
+// The forward kernel processes its (pixel, voxel) hits in batches of up to 32 per warp (phase B/C of dvx_composite_tile.cu).
+// When a frame is saved for a backward pass, every batch is also written to a per-warp stream in HBM, so that the
+// backward replays the batches instead of walking the tile lists and testing every candidate voxel again.
+// One batch = DVX_REC_BATCH_BYTES, structure-of-arrays so that each of the three record stores / loads of a warp is one
+// contiguous run:
+//   [   0,  512)  32 x {id, meta, delta, mid}      voxel, tree << 8 | level << 16, (b - a) / K, (a + b) / 2
+//   [ 512, 1024)  32 x {p_x, p_y, p_z, q_x}        local coordinates u(lambda) = p + q lambda on the clipped segment
+//   [1024, 1280)  32 x {q_y, q_z}
+//   [1280, 1408)  32 x ownership mask              bit i of word l: item i of the batch belongs to the warp's pixel l
+// Batches are grouped in chunks of DVX_REC_CHUNK, handed out from one pool by an atomic counter; rec_next links a warp's
+// chunks, rec_tab[2 * warp] = first chunk, rec_tab[2 * warp + 1] = number of batches (warp = tile * 8 + 4x8 block).
+#define DVX_REC_BATCH_BYTES 1408u
+#ifndef DVX_REC_CHUNK
+#define DVX_REC_CHUNK 8u
+#endif
 
 struct CompositeArgs {
   FrameParams p;
@@ -78,6 +98,11 @@ struct CompositeArgs {
   // backward
   const float *g_rgb, *g_depth, *g_alpha;
   float *drgb;                 // [v_total][4] scratch: dL/drgb_v
+  // hit records (see above); rec_pool == NULL: nothing is recorded / the backward walks the lists
+  unsigned char *rec_pool;     // [rec_cap chunks][DVX_REC_CHUNK][DVX_REC_BATCH_BYTES]
+  uint32_t *rec_next;          // [rec_cap]
+  uint32_t *rec_tab;           // [n_tiles * 8][2]
+  uint32_t rec_cap;            // chunks in the pool
   // weight export (row N3)
   const uint32_t *exp_row;     // [H*W + 1] CSR row starts
   uint32_t *exp_vox;           // [nnz] global voxel id
@@ -175,6 +200,9 @@ void dvx_features_launch(uint32_t width, uint32_t height, uint32_t n_channels, c
 void dvx_composite_tile_launch(const CompositeArgs &a, bool backward, cudaStream_t st);
 void dvx_composite_naive_launch(const CompositeArgs &a, bool backward, cudaStream_t st);
 void dvx_composite_export_launch(const CompositeArgs &a, cudaStream_t st);
+// Backward from the hit records (returns at once when the frame's record pool overflowed); a list-walking backward launched
+// with a.rec_pool != NULL is its complement (it returns at once unless the pool overflowed).
+void dvx_composite_replay_launch(const CompositeArgs &a, cudaStream_t st);
 inline void dvx_composite_launch(const CompositeArgs &a, bool backward, cudaStream_t st) {
   if (a.p.flags & DVX_FLAG_NAIVE) dvx_composite_naive_launch(a, backward, st);
   else dvx_composite_tile_launch(a, backward, st);

@@ -87,7 +87,7 @@ def test_t2_t3_config1_images_and_gradients(ctx, config1):
     gin = sc.image_grads(rgb_std=1e-2, depth_std=1e-3, alpha_std=1e-2)
     ref = O.render(sc, mode=0, grads_in=gin)
     dev = dvx.SceneOnDevice(ctx, sc)
-    for flags in (dvx.FLAG_NAIVE, 0):
+    for flags in (dvx.FLAG_NAIVE, 0, dvx.FLAG_NO_RECORDS):   # debug walker; tile kernel + record replay; tile kernel + list walk
         rgb, depth, alpha, frame = dev.render(flags=flags)
         torch.cuda.synchronize()
         _check_images(rgb, depth, alpha, ref, scene=sc)
@@ -160,16 +160,26 @@ def _sampled_parity(ctx, sc, n_tiles, seed, backward):
         gin["rgb"] = gin["rgb"] * mask[:, :, None].astype(np.float32)
     ref = O.render(sc, mode=1, mask=mask, grads_in=gin)
     dev = dvx.SceneOnDevice(ctx, sc)
-    rgb, depth, alpha, frame = dev.render()
-    torch.cuda.synchronize()
-    errs = _check_images(rgb, depth, alpha, ref, mask, scene=sc)
-    if backward:
-        grads = frame.backward(torch.from_numpy(gin["rgb"]).cuda())
+    errs = 0
+    for flags in ((0, dvx.FLAG_NO_RECORDS) if backward else (0,)):   # backward from the hit records, then by the list walk
+        rgb, depth, alpha, frame = dev.render(flags=flags)
         torch.cuda.synchronize()
-        for t in range(len(sc.octrees)):
-            _check_grads(grads[t][0], ref["dgeo"][t], "dgeo[%d]" % t)
-            _check_grads(grads[t][1], ref["dsh"][t], "dsh[%d]" % t)
-    frame.release()
+        errs = _check_images(rgb, depth, alpha, ref, mask, scene=sc)
+        if backward:
+            if flags == 0:
+                st = frame.record_stats()
+                if st["overflowed"]:   # the context's history came from a lighter workload: this frame would fall back
+                    frame.release()    # to the list walk (covered below); its count sizes the pool of the next one
+                    rgb, depth, alpha, frame = dev.render(flags=flags)
+                    st = frame.record_stats()
+                assert st["bytes_used"] > 0 and not st["overflowed"], st
+            grads = frame.backward(torch.from_numpy(gin["rgb"]).cuda())
+            torch.cuda.synchronize()
+            for t in range(len(sc.octrees)):
+                _check_grads(grads[t][0], ref["dgeo"][t], "dgeo[%d] flags %d" % (t, flags))
+                _check_grads(grads[t][1], ref["dsh"][t], "dsh[%d] flags %d" % (t, flags))
+            del grads
+        frame.release()
     for t in dev.trees:
         t.close()
     return errs
