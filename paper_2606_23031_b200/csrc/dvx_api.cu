@@ -72,6 +72,7 @@ struct dvx_frame {
   Buf tile_cost, tile_order;  // pairs per tile [n_tiles]; the CTA -> tile launch order derived from it [2 n_tiles: result, intermediate]
   Buf rec_pool, rec_next, rec_tab;  // hit records of the forward (dvx_internal.cuh); rec_pool.p == NULL: none kept
   uint32_t rec_cap = 0;             // chunks in rec_pool
+  unsigned char *rec_base = nullptr; // rec_pool.p rounded up to the chunk stride
   Buf w_row, w_vox, w_val;  // row N3: the compositing weights as CSR, built on demand
   uint64_t w_nnz = 0;
   dvx_sky sky = {0, 0, nullptr, nullptr};
@@ -350,13 +351,13 @@ void rec_collect(dvx_ctx *ctx) {
   }
 }
 uint64_t rec_capacity(const dvx_ctx *ctx, const FrameParams &p) {
-  const double chunk_bytes = (double)DVX_REC_CHUNK * DVX_REC_BATCH_BYTES;
+  const double chunk_bytes = (double)DVX_REC_CHUNK_STRIDE;
   const double npix = (double)p.width * p.height, n_warps = (double)p.n_tiles * 8.0;
   double cap;
   if (ctx->rec_budget) {
     cap = floor((double)ctx->rec_budget / chunk_bytes);
   } else if (ctx->rec_seen_n == 0) {
-    cap = ceil(npix * 48.0 / 32.0 / DVX_REC_CHUNK) + n_warps;  // 48 hits per pixel + one partly filled chunk per warp
+    cap = ceil(npix * 48.0 / 32.0 / DVX_REC_CHUNK) + 0.5 * n_warps;  // 48 hits per pixel + half a chunk per warp unfilled
   } else {
     double m = 0;
     for (int i = 0; i < 8 && i < ctx->rec_seen_n; ++i) m = fmax(m, ctx->rec_seen[i]);
@@ -540,10 +541,11 @@ dvx_status dvx_render(dvx_ctx *ctx, const dvx_camera *cam, const dvx_octree *sta
     if (cap > 0) {
       // a pool the allocator cannot give is not an error: the frame then keeps no records and the backward walks the lists
       if (buf_alloc(ctx, f->rec_tab, sizeof(uint32_t) * 2 * 8 * (size_t)p.n_tiles) && buf_alloc(ctx, f->rec_next, sizeof(uint32_t) * cap) &&
-          buf_alloc(ctx, f->rec_pool, (size_t)cap * DVX_REC_CHUNK * DVX_REC_BATCH_BYTES)) {
+          buf_alloc(ctx, f->rec_pool, ((size_t)cap + 1) * DVX_REC_CHUNK_STRIDE)) {  // + 1: the chunks start at a multiple of the stride
         rec = true;
         f->rec_cap = (uint32_t)cap;
-        A.rec_pool = (unsigned char *)f->rec_pool.p; A.rec_next = (uint32_t *)f->rec_next.p; A.rec_tab = (uint32_t *)f->rec_tab.p;
+        f->rec_base = (unsigned char *)(((uintptr_t)f->rec_pool.p + DVX_REC_CHUNK_STRIDE - 1) & ~(uintptr_t)(DVX_REC_CHUNK_STRIDE - 1));
+        A.rec_pool = f->rec_base; A.rec_next = (uint32_t *)f->rec_next.p; A.rec_tab = (uint32_t *)f->rec_tab.p;
         A.rec_cap = f->rec_cap;
       } else {
         ctx_release(ctx, f->rec_tab.p); ctx_release(ctx, f->rec_next.p); ctx_release(ctx, f->rec_pool.p);
@@ -612,7 +614,7 @@ dvx_status dvx_backward_n(dvx_ctx *ctx, dvx_frame *f, const float *dL_drgb, cons
   A.g_normal = dL_dnormal; A.vnrm = (const float4 *)f->vnrm.p; A.sv_nrm = (float *)f->sv_nrm.p; A.dnrm = dnrm;
   CU(cudaEventRecord(f->ev[7], st));
   if (f->rec_pool.p) {  // replay the forward's hit records; the list walk behind it runs only if the pool overflowed
-    A.rec_pool = (unsigned char *)f->rec_pool.p; A.rec_next = (uint32_t *)f->rec_next.p; A.rec_tab = (uint32_t *)f->rec_tab.p;
+    A.rec_pool = f->rec_base; A.rec_next = (uint32_t *)f->rec_next.p; A.rec_tab = (uint32_t *)f->rec_tab.p;
     A.rec_cap = f->rec_cap;
     dvx_composite_replay_launch(A, st);
   }
@@ -696,7 +698,7 @@ dvx_status dvx_frame_record_stats(dvx_ctx *ctx, const dvx_frame *f, uint64_t *by
   unsigned long long h[CNT_N];
   CU(cudaMemcpyAsync(h, f->counters.p, sizeof(h), cudaMemcpyDeviceToHost, ctx->st));
   CU(cudaStreamSynchronize(ctx->st));
-  const uint64_t chunk_bytes = (uint64_t)DVX_REC_CHUNK * DVX_REC_BATCH_BYTES;
+  const uint64_t chunk_bytes = (uint64_t)DVX_REC_CHUNK_STRIDE;
   const bool on = f->rec_pool.p != nullptr;
   if (bytes_used) *bytes_used = on ? (h[CNT_REC_CHUNKS] < f->rec_cap ? h[CNT_REC_CHUNKS] : f->rec_cap) * chunk_bytes : 0;
   if (bytes_capacity) *bytes_capacity = on ? (uint64_t)f->rec_cap * chunk_bytes : 0;

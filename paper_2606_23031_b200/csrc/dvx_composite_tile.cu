@@ -95,12 +95,7 @@ struct WarpQueue {
   float4 acc[32];               // forward, per pixel between batches: C (rgb) and D
   float2 tn[32];                //          T and n_used (as bits)
   float4 nacc[NRM ? 32 : 1];    //          N (O11)
-  // the warp's position in its hit-record stream (dvx_internal.cuh)
-  unsigned long long rec_ptr;   // next batch slot
-  uint32_t rec_left;            // slots left in the current chunk
-  uint32_t rec_n;               // batches written so far
-  uint32_t rec_chunk;           // current chunk
-  uint32_t rec_ok;              // 0 once the pool is exhausted
+  uint32_t rec_n;               // chunks this warp has taken for its hit-record stream (dvx_internal.cuh); lane 0 only
 };
 
 struct Pix {
@@ -445,39 +440,35 @@ __device__ __forceinline__ void phase_B2(const CompositeArgs &A, int lane, int c
   }
 }
 
-// The next batch slot of this warp's hit-record stream, or NULL once the pool is exhausted (warp-uniform).  A new chunk is
-// taken from the pool every DVX_REC_CHUNK batches with one atomic and linked behind the previous one.
+// The next batch slot of this warp's hit-record stream, or NULL once the pool is exhausted (warp-uniform).
+// `ptr` is the warp's write pointer: REC_PTR_START before the first batch, REC_PTR_OFF after the pool ran out (both have a
+// zero high word, which no device address has), else the address of the next slot.  Chunks start at multiples of
+// DVX_REC_CHUNK_STRIDE and hold DVX_REC_CHUNK batches, so the low bits of the pointer say when a new chunk is due; it is
+// taken from the pool with one atomic and linked behind the previous one.  The fast path is two 32-bit tests and an add.
+constexpr uint32_t REC_CHUNK_USED = DVX_REC_CHUNK * DVX_REC_BATCH_BYTES;
+constexpr unsigned long long REC_PTR_START = REC_CHUNK_USED, REC_PTR_OFF = 1ull;
 template <bool NRM>
-__device__ __forceinline__ unsigned char *rec_next_block(const CompositeArgs &A, int lane, uint32_t warp_global, WarpQueue<NRM> &Q) {
-  if (Q.rec_left == 0) {  // rare path: first batch, chunk boundary, or no pool left
-    if (!Q.rec_ok) return nullptr;
+__device__ __forceinline__ unsigned char *rec_next_block(const CompositeArgs &A, int lane, int tile, int warp, WarpQueue<NRM> &Q,
+                                                         unsigned long long &ptr) {
+  if (((uint32_t)ptr & (DVX_REC_CHUNK_STRIDE - 1u)) == REC_CHUNK_USED) {  // rare path: first batch or chunk boundary
     uint32_t c = 0;
     if (lane == 0) c = (uint32_t)atomicAdd(&A.counters[CNT_REC_CHUNKS], 1ull);
     c = __shfl_sync(0xffffffffu, c, 0);
     if (c >= A.rec_cap) {
+      if (lane == 0) atomicOr(reinterpret_cast<unsigned int *>(&A.counters[CNT_REC_OVERFLOW]), 1u);
+      ptr = REC_PTR_OFF;
+    } else {
       if (lane == 0) {
-        Q.rec_ok = 0;
-        atomicOr(reinterpret_cast<unsigned int *>(&A.counters[CNT_REC_OVERFLOW]), 1u);
+        if (ptr == REC_PTR_START) A.rec_tab[2 * ((uint32_t)tile * 8u + (uint32_t)warp)] = c;
+        else A.rec_next[(ptr - reinterpret_cast<unsigned long long>(A.rec_pool)) / DVX_REC_CHUNK_STRIDE] = c;
+        Q.rec_n += 1;  // chunks taken so far
       }
-      __syncwarp();
-      return nullptr;
+      ptr = reinterpret_cast<unsigned long long>(A.rec_pool) + (unsigned long long)c * DVX_REC_CHUNK_STRIDE;
     }
-    if (lane == 0) {
-      if (Q.rec_n == 0) A.rec_tab[2 * warp_global] = c;
-      else A.rec_next[Q.rec_chunk] = c;
-      Q.rec_chunk = c;
-      Q.rec_left = DVX_REC_CHUNK;
-      Q.rec_ptr = reinterpret_cast<unsigned long long>(A.rec_pool) + (unsigned long long)c * (DVX_REC_CHUNK * DVX_REC_BATCH_BYTES);
-    }
-    __syncwarp();
   }
-  unsigned char *blk = reinterpret_cast<unsigned char *>(Q.rec_ptr);
-  __syncwarp();
-  if (lane == 0) {
-    Q.rec_ptr += DVX_REC_BATCH_BYTES;
-    Q.rec_left -= 1;
-    Q.rec_n += 1;
-  }
+  if ((uint32_t)(ptr >> 32) == 0u) return nullptr;
+  unsigned char *blk = reinterpret_cast<unsigned char *>(ptr);
+  ptr += DVX_REC_BATCH_BYTES;
   return blk;
 }
 
@@ -486,10 +477,10 @@ __device__ __forceinline__ unsigned char *rec_next_block(const CompositeArgs &A,
 template <bool BWD, bool NRM, bool EXP, bool REC>
 __device__ __forceinline__ void flush_batch(const CompositeArgs &A, int lane, WarpQueue<NRM> &Q, const uint4 *s_tree,
                                             float *const *s_dgeo, int &n_items, int &head, unsigned long long &my_bits, Pix &S,
-                                            uint32_t warp_global) {
+                                            int tile, int warp, unsigned long long &rec_ptr) {
   const int count = n_items < 32 ? n_items : 32;
   unsigned char *blk = nullptr;
-  if (REC) blk = rec_next_block<NRM>(A, lane, warp_global, Q);
+  if (REC) blk = rec_next_block<NRM>(A, lane, tile, warp, Q, rec_ptr);
   __syncwarp();
   ItemGeom G;
   float M[4];
@@ -625,13 +616,13 @@ __global__ void __launch_bounds__(TILE_THREADS, DVX_TILE_MIN_CTAS) composite_til
     S.n_stop = A.exp_row[pix + 1] - S.exp_pos;
   }
   if (BWD && inside) backward_pixel_init<NRM>(A, u, v, pix, S);
-  const uint32_t warp_global = (uint32_t)tile * 8u + (uint32_t)warp;
+  unsigned long long rec_ptr = REC_PTR_START;
   if (!BWD) {
     Q.acc[lane] = make_float4(0.f, 0.f, 0.f, 0.f);
     Q.tn[lane] = make_float2(1.f, __uint_as_float(0u));
     if (NRM) Q.nacc[lane] = make_float4(0.f, 0.f, 0.f, 0.f);
   }
-  if (REC && lane == 0) { Q.rec_left = 0; Q.rec_n = 0; Q.rec_chunk = 0; Q.rec_ok = 1; Q.rec_ptr = 0; }
+  if (REC && lane == 0) Q.rec_n = 0;
 
   // ---- step 3: intervals of the actors in this tile's mask, insertion-sorted by (tau_in, actor index) (O2, O3)
   float h_in[DVX_MAX_ACTORS], h_out[DVX_MAX_ACTORS];
@@ -816,7 +807,7 @@ __global__ void __launch_bounds__(TILE_THREADS, DVX_TILE_MIN_CTAS) composite_til
             }
             n_items += __popc(mk);
             if (n_items >= 32) {
-              flush_batch<BWD, NRM, EXP, REC>(A, lane, Q, s_tree, s_dgeo, n_items, head, my_bits, S, warp_global);
+              flush_batch<BWD, NRM, EXP, REC>(A, lane, Q, s_tree, s_dgeo, n_items, head, my_bits, S, tile, warp, rec_ptr);
               if (S.done) c_t = NONE;
             }
           }
@@ -832,9 +823,12 @@ __global__ void __launch_bounds__(TILE_THREADS, DVX_TILE_MIN_CTAS) composite_til
     }
     if (part) seg_tree = NONE;          // served
   }
-  while (n_items > 0) flush_batch<BWD, NRM, EXP, REC>(A, lane, Q, s_tree, s_dgeo, n_items, head, my_bits, S, warp_global);
+  while (n_items > 0) flush_batch<BWD, NRM, EXP, REC>(A, lane, Q, s_tree, s_dgeo, n_items, head, my_bits, S, tile, warp, rec_ptr);
 
-  if (REC && lane == 0) A.rec_tab[2 * warp_global + 1] = Q.rec_ok ? Q.rec_n : 0u;
+  if (REC && lane == 0) {  // batches written = full chunks + the slots used of the last one
+    const uint32_t used = ((uint32_t)rec_ptr & (DVX_REC_CHUNK_STRIDE - 1u)) / DVX_REC_BATCH_BYTES;
+    A.rec_tab[2 * ((uint32_t)tile * 8u + (uint32_t)warp) + 1] = Q.rec_n ? (Q.rec_n - 1u) * DVX_REC_CHUNK + used : 0u;
+  }
   if (!BWD) {
     const float4 a4 = Q.acc[lane];
     const float2 t2 = Q.tn[lane];
@@ -878,7 +872,7 @@ __global__ void __launch_bounds__(TILE_THREADS, DVX_TILE_MIN_CTAS) composite_til
 // (phase B), replays the pixels' blend order (phase C) and reduces the gradients (phase B2).
 // Same grid and warp -> pixel-block mapping as the forward.
 #ifndef DVX_REPLAY_MIN_CTAS
-#define DVX_REPLAY_MIN_CTAS (4 * DVX_TILE_SPLIT)
+#define DVX_REPLAY_MIN_CTAS 7   // 72 registers, no spills; config 3 replay ms at 6 / 7 / 8 CTAs per SM: 1.272 / 1.189 / 1.207 (config 4: 2.114 / 1.996 / 2.045)
 #endif
 struct RecBatch {
   uint4 a;      // id, meta, delta, mid
@@ -917,6 +911,8 @@ __global__ void __launch_bounds__(TILE_THREADS, DVX_REPLAY_MIN_CTAS) composite_r
   const bool inside = u < (int)p.width && v < (int)p.height;
   const size_t pix = (size_t)v * p.width + u;
   BatchShared<NRM> &bs = s_b[warp_l];
+  // The per-pixel state stays in registers here (unlike in the forward): parked in shared memory between batches, with
+  // two batch buffers in flight, the same loop ran 1.43-1.63 ms instead of 1.21 ms (config 3, 6-8 CTAs per SM).
   Pix S;
   pixel_state_zero(S, inside);
   if (inside) backward_pixel_init<NRM>(A, u, v, pix, S);
@@ -925,15 +921,21 @@ __global__ void __launch_bounds__(TILE_THREADS, DVX_REPLAY_MIN_CTAS) composite_r
   uint32_t chunk = nb ? A.rec_tab[2 * warp_global] : 0u;
   __syncthreads();  // s_tree / s_dgeo
   if (nb == 0) return;
-  RecBatch cur = rec_load(A.rec_pool + (size_t)chunk * DVX_REC_CHUNK * DVX_REC_BATCH_BYTES, lane);
+  const unsigned char *blk = A.rec_pool + (size_t)chunk * DVX_REC_CHUNK_STRIDE;
+  uint32_t slot = 0;
+  RecBatch cur = rec_load(blk, lane);
   for (uint32_t b = 0; b < nb; ++b) {
     if (__all_sync(0xffffffffu, S.done)) break;  // every pixel of the block has replayed its n_used voxels
-    // -- prefetch the next batch (a chunk's successor is read when its last slot is reached)
+    // -- prefetch the next batch (a chunk's successor is read when its last slot has been used)
     RecBatch nxt = cur;
     if (b + 1 < nb) {
-      const uint32_t slot = (b + 1) & (DVX_REC_CHUNK - 1u);
-      if (slot == 0) chunk = __ldg(A.rec_next + chunk);
-      nxt = rec_load(A.rec_pool + ((size_t)chunk * DVX_REC_CHUNK + slot) * DVX_REC_BATCH_BYTES, lane);
+      blk += DVX_REC_BATCH_BYTES;
+      if (++slot == DVX_REC_CHUNK) {
+        slot = 0;
+        chunk = __ldg(A.rec_next + chunk);
+        blk = A.rec_pool + (size_t)chunk * DVX_REC_CHUNK_STRIDE;
+      }
+      nxt = rec_load(blk, lane);
     }
     const int count = __popc(__reduce_or_sync(0xffffffffu, cur.mask));  // every item of the batch has one owner
     ItemGeom G;

@@ -64,12 +64,13 @@ enum { CNT_PAIRS = 0, CNT_VVIS = 1, CNT_QTEST = 2, CNT_QHIT = 3, CNT_PAIRS_EFF =
 //   [ 512, 1024)  32 x {p_x, p_y, p_z, q_x}        local coordinates u(lambda) = p + q lambda on the clipped segment
 //   [1024, 1280)  32 x {q_y, q_z}
 //   [1280, 1408)  32 x ownership mask              bit i of word l: item i of the batch belongs to the warp's pixel l
-// Batches are grouped in chunks of DVX_REC_CHUNK, handed out from one pool by an atomic counter; rec_next links a warp's
-// chunks, rec_tab[2 * warp] = first chunk, rec_tab[2 * warp + 1] = number of batches (warp = tile * 8 + 4x8 block).
+// Batches are grouped in chunks of DVX_REC_CHUNK, handed out from one pool by an atomic counter; chunk c starts at
+// rec_pool + c * DVX_REC_CHUNK_STRIDE (a power of two, pool base aligned to it, so that "the chunk is full" is a test on the
+// low bits of the write pointer); rec_next links a warp's chunks, rec_tab[2 * warp] = first chunk, rec_tab[2 * warp + 1] =
+// number of batches (warp = tile * 8 + 4x8 block).
 #define DVX_REC_BATCH_BYTES 1408u
-#ifndef DVX_REC_CHUNK
-#define DVX_REC_CHUNK 8u
-#endif
+#define DVX_REC_CHUNK 11u
+#define DVX_REC_CHUNK_STRIDE 16384u   // 11 * 1408 = 15488 bytes used
 
 struct CompositeArgs {
   FrameParams p;

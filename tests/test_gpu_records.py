@@ -46,14 +46,14 @@ def test_replay_walk_and_overflow_fallback_agree_with_the_oracle(ctx, config1):
     dev = dvx.SceneOnDevice(ctx, sc)
     img_r, g_r, st_r = _backward_all(dev, sc, gin)                                    # records + replay
     img_w, g_w, st_w = _backward_all(dev, sc, gin, flags=dvx.FLAG_NO_RECORDS)         # list walk
-    ctx.set_record_budget(3 * 8 * 1408)                                               # three chunks: certain overflow
+    ctx.set_record_budget(3 * 16384)                                                  # three chunks: certain overflow
     try:
         img_o, g_o, st_o = _backward_all(dev, sc, gin)                                # replay refuses, the walk runs
     finally:
         ctx.set_record_budget(0)
     assert st_r["bytes_used"] > 0 and st_r["bytes_used"] <= st_r["bytes_capacity"] and not st_r["overflowed"]
     assert st_w == {"bytes_used": 0, "bytes_capacity": 0, "overflowed": False}
-    assert st_o["overflowed"] and st_o["bytes_capacity"] == 3 * 8 * 1408
+    assert st_o["overflowed"] and st_o["bytes_capacity"] == 3 * 16384
     for a, b, c in zip(img_r, img_w, img_o):   # writing records must not change a bit of the image
         assert torch.equal(a, b) and torch.equal(a, c)
     for t in range(len(sc.octrees)):
