@@ -54,6 +54,10 @@ typedef void (*dvx_free_fn)(void *ptr, void *user);
 /* device: CUDA ordinal.  cuda_stream: a cudaStream_t (NULL = the legacy default stream). */
 dvx_status dvx_create(int device, void *cuda_stream, dvx_alloc_fn alloc, dvx_free_fn free_, void *user, dvx_ctx **out);
 void dvx_destroy(dvx_ctx *ctx);
+/* The context keeps released scratch blocks (sort buffers, per-frame tables, record pools) for reuse, matched by size, so a
+ * steady-state loop allocates nothing.  A workload whose sizes keep growing (subdivision rounds) leaves the smaller blocks
+ * behind: dvx_trim synchronises the stream and returns every cached block to the allocator.  bytes_freed may be NULL. */
+dvx_status dvx_trim(dvx_ctx *ctx, uint64_t *bytes_freed);
 
 /* One leaf-only octree.  All three arrays are DEVICE pointers, borrowed until dvx_octree_destroy;
  * geo and sh may change in place between renders (they are re-read every frame), code may not (see refresh). */

@@ -27,7 +27,7 @@ EXPORTS = ["dvx_create", "dvx_destroy", "dvx_octree_create", "dvx_octree_refresh
            "dvx_grid_adam_step", "dvx_adam_step", "dvx_grid_adam_step_n", "dvx_adam_step_n",
            "dvx_frame_weights", "dvx_render_features", "dvx_fuse_features",
            "dvx_cloud_create", "dvx_cloud_destroy", "dvx_density_prior", "dvx_subdivide_near", "dvx_prune",
-           "dvx_set_record_budget", "dvx_frame_record_stats"]
+           "dvx_set_record_budget", "dvx_frame_record_stats", "dvx_trim"]
 
 
 class DvxError(RuntimeError):
@@ -140,6 +140,7 @@ def load():
     lib.dvx_prune.argtypes = [P, C.c_uint32, P, P, C.c_float, P, P, C.POINTER(C.c_uint32)]
     lib.dvx_grid_adam_step_n.argtypes = [P, C.POINTER(Adam), C.c_uint32, C.POINTER(GridAdamItem)]
     lib.dvx_adam_step_n.argtypes = [P, C.POINTER(Adam), C.c_uint32, C.POINTER(AdamItem)]
+    lib.dvx_trim.argtypes = [P, C.POINTER(C.c_uint64)]
     lib.dvx_set_record_budget.argtypes = [P, C.c_uint64]
     lib.dvx_frame_record_stats.argtypes = [P, P, C.POINTER(C.c_uint64), C.POINTER(C.c_uint64), C.POINTER(C.c_uint32)]
     for name in EXPORTS:
@@ -194,6 +195,12 @@ class Context:
         n = C.c_uint32()
         self.check(self.lib.dvx_stage_ms_collect(self.h, ms, C.byref(n)))
         return dict(zip(STAGES, list(ms)[:6])), n.value
+
+    def trim(self):
+        """dvx_trim: hand every cached scratch block back to the allocator -> bytes freed."""
+        n = C.c_uint64()
+        self.check(self.lib.dvx_trim(self.h, C.byref(n)))
+        return n.value
 
     def set_record_budget(self, nbytes):
         """dvx_set_record_budget: bytes of hit records per saved frame (0 = automatic sizing)."""

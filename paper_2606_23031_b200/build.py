@@ -35,7 +35,7 @@ def _stale(target, deps):
 def build(force=False, verbose=False):
     os.makedirs(OBJ, exist_ok=True)
     nvcc = _nvcc()
-    extra = (["-Xptxas", "-v"] if verbose else []) + os.environ.get("DVX_NVCC_EXTRA", "").split()  # experiments only
+    extra = ["-Xptxas", "-v"] if verbose else []
     jobs = []
     for src in SOURCES:
         s = os.path.join(CSRC, src)

@@ -10,7 +10,7 @@
 
 #include "dvx_internal.cuh"
 
-unsigned long long g_dvx_launches = 0;
+std::atomic<unsigned long long> g_dvx_launches{0};
 
 // The CUDA events of one render (+ backward) call.  Owned by the context and recycled, so the steady state creates none.
 struct EventSet {
@@ -80,9 +80,6 @@ struct dvx_frame {
 };
 
 namespace {
-
-// Experiments only: DVX_TILE_ORDER=0 launches the compositing CTAs in raster order instead of heaviest tile first.
-const bool g_tile_order_on = [] { const char *e = getenv("DVX_TILE_ORDER"); return !(e && e[0] == '0'); }();
 
 dvx_status fail(dvx_ctx *ctx, dvx_status code, const char *msg) {
   if (ctx) ctx->err = msg;
@@ -167,6 +164,22 @@ void frame_free(dvx_ctx *ctx, dvx_frame *f) {
   delete f;
 }
 
+// Releases what a call holds when it leaves early (a CU() failure, an allocation that came back NULL): the frame unless it
+// was handed to the caller, and any scratch blocks registered with it.
+struct CallGuard {
+  dvx_ctx *ctx;
+  dvx_frame *frame = nullptr;
+  std::vector<void *> scratch;
+  explicit CallGuard(dvx_ctx *c) : ctx(c) {}
+  void *add(void *p) { scratch.push_back(p); return p; }
+  void drop(void *p) { for (auto &q : scratch) if (q == p) q = nullptr; }  // ownership moved elsewhere
+  void keep_frame() { frame = nullptr; }
+  ~CallGuard() {
+    for (void *p : scratch) ctx_release(ctx, p);
+    if (frame) frame_free(ctx, frame);
+  }
+};
+
 dvx_status build_rank_tables(dvx_ctx *ctx, dvx_octree *t) {
   const uint32_t V = t->d.n_voxels;
   if (t->rank) { ctx_release(ctx, t->rank); t->rank = nullptr; }
@@ -206,6 +219,7 @@ dvx_status check_desc(dvx_ctx *ctx, const dvx_octree_desc *d) {
   if (!d) return fail(ctx, DVX_ERR_INVALID_ARG, "octree desc is NULL");
   if (d->sh_degree > 3) return fail(ctx, DVX_ERR_INVALID_ARG, "sh_degree > 3");
   if (!(d->side > 0.f) || !isfinite(d->side)) return fail(ctx, DVX_ERR_INVALID_ARG, "side must be positive");
+  if (d->n_voxels >= (1u << 30)) return fail(ctx, DVX_ERR_INVALID_ARG, "2^30 or more voxels in one octree");
   if (d->n_voxels && (!d->code || !d->geo || !d->sh)) return fail(ctx, DVX_ERR_INVALID_ARG, "octree array pointer is NULL");
   if (((uintptr_t)d->geo & 31) || ((uintptr_t)d->sh & 15) || ((uintptr_t)d->code & 7))
     return fail(ctx, DVX_ERR_INVALID_ARG, "octree arrays must be aligned (code 8, geo 32, sh 16 bytes)");
@@ -270,6 +284,24 @@ void dvx_destroy(dvx_ctx *ctx) {
 }
 
 const char *dvx_last_error(const dvx_ctx *ctx) { return ctx ? ctx->err.c_str() : "context is NULL"; }
+
+dvx_status dvx_trim(dvx_ctx *ctx, uint64_t *bytes_freed) {
+  if (bytes_freed) *bytes_freed = 0;
+  if (!ctx) return DVX_ERR_INVALID_ARG;
+  cudaSetDevice(ctx->device);
+  CU(cudaStreamSynchronize(ctx->st));  // cached blocks may still be read by work in flight
+  uint64_t freed = 0;
+  for (auto &c : ctx->cache) {
+    for (size_t i = 0; i < ctx->all.size(); ++i)
+      if (ctx->all[i].p == c.p) { ctx->all.erase(ctx->all.begin() + i); break; }
+    if (ctx->free_) ctx->free_(c.p, ctx->user);
+    else cudaFree(c.p);
+    freed += c.bytes;
+  }
+  ctx->cache.clear();
+  if (bytes_freed) *bytes_freed = freed;
+  return DVX_OK;
+}
 
 dvx_status dvx_octree_create(dvx_ctx *ctx, const dvx_octree_desc *desc, dvx_octree **out) {
   if (!ctx || !out) return fail(ctx, DVX_ERR_INVALID_ARG, "NULL argument");
@@ -409,6 +441,8 @@ dvx_status dvx_render(dvx_ctx *ctx, const dvx_camera *cam, const dvx_octree *sta
   cudaStream_t st = ctx->st;
 
   dvx_frame *f = new dvx_frame();
+  CallGuard guard(ctx);
+  guard.frame = f;  // freed on every early return below
   FrameParams &p = f->p;
   memset(&p, 0, sizeof(p));
   p.width = cam->width; p.height = cam->height;
@@ -440,8 +474,8 @@ dvx_status dvx_render(dvx_ctx *ctx, const dvx_camera *cam, const dvx_octree *sta
     vtot += tr->d.n_voxels;
     if (tr->d.n_voxels > vmax) vmax = tr->d.n_voxels;
   }
-  if ((uint64_t)p.n_tiles * 8u >= (1u << 24)) { frame_free(ctx, f); return fail(ctx, DVX_ERR_INVALID_ARG, "image too large (more than 2^21 tiles)"); }
-  if (vtot >= 0xFFFFFFFFull) { frame_free(ctx, f); return fail(ctx, DVX_ERR_INVALID_ARG, "more than 2^32-2 voxels in total"); }
+  if ((uint64_t)p.n_tiles * 8u >= (1u << 24)) return fail(ctx, DVX_ERR_INVALID_ARG, "image too large (more than 2^21 tiles)");
+  if (vtot >= 0xFFFFFFFFull) return fail(ctx, DVX_ERR_INVALID_ARG, "more than 2^32-2 voxels in total");
   p.v_total = (uint32_t)vtot;
   p.rank_bits = bits_for(vmax);
   p.n_buckets = p.n_tiles * p.n_trees * 8u;
@@ -458,10 +492,10 @@ dvx_status dvx_render(dvx_ctx *ctx, const dvx_camera *cam, const dvx_octree *sta
   if (ok && saved)
     ok = buf_alloc(ctx, f->sv_rgbd, npix * 16) && buf_alloc(ctx, f->sv_T, npix * 4) && buf_alloc(ctx, f->sv_nused, npix * 4);
   if (ok && out.normal) {
-    if (o.flags & DVX_FLAG_NAIVE) { frame_free(ctx, f); return fail(ctx, DVX_ERR_NOT_IMPLEMENTED, "the debug walker has no normal map"); }
+    if (o.flags & DVX_FLAG_NAIVE) return fail(ctx, DVX_ERR_NOT_IMPLEMENTED, "the debug walker has no normal map");
     ok = buf_alloc(ctx, f->vnrm, sizeof(float4) * (size_t)p.v_total) && (!saved || buf_alloc(ctx, f->sv_nrm, npix * 16));
   }
-  if (!ok) { frame_free(ctx, f); return fail(ctx, DVX_ERR_OOM, "dvx_render: allocator returned NULL"); }
+  if (!ok) return fail(ctx, DVX_ERR_OOM, "dvx_render: allocator returned NULL");
   if (!ctx->ev_free.empty()) {
     f->es = ctx->ev_free.back();
     ctx->ev_free.pop_back();
@@ -471,7 +505,6 @@ dvx_status dvx_render(dvx_ctx *ctx, const dvx_camera *cam, const dvx_octree *sta
       if (cudaEventCreate(&e) != cudaSuccess) {
         for (auto &e2 : f->es->ev) if (e2) cudaEventDestroy(e2);
         delete f->es; f->es = nullptr;
-        frame_free(ctx, f);
         return fail(ctx, DVX_ERR_CUDA, "cudaEventCreate failed");
       }
   }
@@ -492,17 +525,13 @@ dvx_status dvx_render(dvx_ctx *ctx, const dvx_camera *cam, const dvx_octree *sta
   CU(cudaStreamSynchronize(st));
   f->n_pairs = ctx->h_counters[CNT_PAIRS];
   f->v_vis = ctx->h_counters[CNT_VVIS];
-  if (f->n_pairs >= 0xFFFFFFFFull) { frame_free(ctx, f); return fail(ctx, DVX_ERR_INVALID_ARG, "more than 2^32-2 (tile, voxel) pairs"); }
+  if (f->n_pairs >= (1ull << 30)) return fail(ctx, DVX_ERR_INVALID_ARG, "2^30 or more (tile, octant, voxel) pairs");
   // ---- step 2
   const uint64_t P = f->n_pairs;
-  uint64_t *ka = (uint64_t *)ctx_alloc(ctx, P * 8), *kb = (uint64_t *)ctx_alloc(ctx, P * 8);
-  uint32_t *va = (uint32_t *)ctx_alloc(ctx, P * 4), *vb = (uint32_t *)ctx_alloc(ctx, P * 4);
-  void *scr = ctx_alloc(ctx, dvx_sort_scratch_bytes(P));
-  if (!ka || !kb || !va || !vb || !scr) {
-    ctx_release(ctx, ka); ctx_release(ctx, kb); ctx_release(ctx, va); ctx_release(ctx, vb); ctx_release(ctx, scr);
-    frame_free(ctx, f);
-    return fail(ctx, DVX_ERR_OOM, "dvx_render: allocator returned NULL");
-  }
+  uint64_t *ka = (uint64_t *)guard.add(ctx_alloc(ctx, P * 8)), *kb = (uint64_t *)guard.add(ctx_alloc(ctx, P * 8));
+  uint32_t *va = (uint32_t *)guard.add(ctx_alloc(ctx, P * 4)), *vb = (uint32_t *)guard.add(ctx_alloc(ctx, P * 4));
+  void *scr = guard.add(ctx_alloc(ctx, dvx_sort_scratch_bytes(P)));
+  if (!ka || !kb || !va || !vb || !scr) return fail(ctx, DVX_ERR_OOM, "dvx_render: allocator returned NULL");
   CU(cudaEventRecord(f->ev[2], st));
   dvx_emit_pairs_launch(p, trees_d, (const uint8_t *)f->octmask.p, (const ushort4 *)f->pxrect.p, (const FrameVox *)f->fvox.p, ka, va, P, counters, st);
   int which = dvx_sort_launch(ka, va, kb, vb, P, key_bits, scr, st);
@@ -513,23 +542,23 @@ dvx_status dvx_render(dvx_ctx *ctx, const dvx_camera *cam, const dvx_octree *sta
                     (uint32_t *)f->tile_cost.p, st);
   dvx_tile_order_launch((const uint32_t *)f->tile_cost.p, p.n_tiles, (uint32_t *)f->tile_order.p, st);
   CU(cudaEventRecord(f->ev[3], st));
-  f->ids.p = which ? vb : va;
+  f->ids.p = which ? vb : va;   // the frame owns the sorted ids from here on; the other buffers go back with the guard
   f->ids.bytes = P * 4;
-  ctx_release(ctx, ka); ctx_release(ctx, kb); ctx_release(ctx, which ? va : vb); ctx_release(ctx, scr);
+  guard.drop(f->ids.p);
   // ---- steps 3 + 4
   CompositeArgs A;
   memset(&A, 0, sizeof(A));
   A.p = p; A.trees = trees_d; A.fvox = (const FrameVox *)f->fvox.p; A.pxrect = (const ushort4 *)f->pxrect.p;
   A.ids = (const uint32_t *)f->ids.p; A.range_beg = (const uint32_t *)f->range_beg.p; A.range_end = (const uint32_t *)f->range_end.p;
   A.actor_mask = (const unsigned long long *)f->actor_mask.p;
-  A.tile_order = g_tile_order_on ? (const uint32_t *)f->tile_order.p : nullptr;
+  A.tile_order = (const uint32_t *)f->tile_order.p;
   A.rgb = out.rgb; A.depth = out.depth; A.alpha = out.alpha;
   A.sv_rgbd = (float *)f->sv_rgbd.p; A.sv_T = (float *)f->sv_T.p; A.sv_nused = (uint32_t *)f->sv_nused.p;
   A.counters = counters;
   A.sky_tex = f->sky.tex; A.sky_w = f->sky.width; A.sky_h = f->sky.height;
   A.normal = out.normal; A.vnrm = (const float4 *)f->vnrm.p; A.sv_nrm = (float *)f->sv_nrm.p;
   if (p.flags & DVX_FLAG_COUNTERS) {
-    if (!buf_alloc(ctx, f->eff_end, sizeof(uint32_t) * (size_t)p.n_buckets)) { frame_free(ctx, f); return fail(ctx, DVX_ERR_OOM, "dvx_render: allocator returned NULL"); }
+    if (!buf_alloc(ctx, f->eff_end, sizeof(uint32_t) * (size_t)p.n_buckets)) return fail(ctx, DVX_ERR_OOM, "dvx_render: allocator returned NULL");
     CU(cudaMemsetAsync(f->eff_end.p, 0, sizeof(uint32_t) * (size_t)p.n_buckets, st));
     A.eff_end = (uint32_t *)f->eff_end.p;
   }
@@ -562,8 +591,7 @@ dvx_status dvx_render(dvx_ctx *ctx, const dvx_camera *cam, const dvx_octree *sta
   }
   f->es->rendered = true;
   CU(cudaGetLastError());
-  if (saved) *saved = f;
-  else frame_free(ctx, f);
+  if (saved) { *saved = f; guard.keep_frame(); }
   return DVX_OK;
 }
 
@@ -587,12 +615,14 @@ dvx_status dvx_backward_n(dvx_ctx *ctx, dvx_frame *f, const float *dL_drgb, cons
     f->trees_h[t].dgeo = g.dgeo;
     f->trees_h[t].dsh = g.dsh;
   }
-  float *drgb = (float *)ctx_alloc(ctx, (size_t)p.v_total * 16);
-  float *dnrm = dL_dnormal ? (float *)ctx_alloc(ctx, (size_t)p.v_total * 16) : nullptr;
-  if (!drgb || (dL_dnormal && !dnrm)) {
-    ctx_release(ctx, drgb); ctx_release(ctx, dnrm);
-    return fail(ctx, DVX_ERR_OOM, "dvx_backward: allocator returned NULL");
+  for (uint32_t t = 0; t < p.n_trees; ++t) {  // red.global.add.v4.f32 and the float4 read-modify-writes need 16-byte alignment
+    const dvx_grad g = t == 0 ? static_grad : actor_grads[t - 1];
+    if (((uintptr_t)g.dgeo | (uintptr_t)g.dsh) & 15) return fail(ctx, DVX_ERR_INVALID_ARG, "gradient buffers must be 16-byte aligned");
   }
+  CallGuard guard(ctx);
+  float *drgb = (float *)guard.add(ctx_alloc(ctx, (size_t)p.v_total * 16));
+  float *dnrm = dL_dnormal ? (float *)guard.add(ctx_alloc(ctx, (size_t)p.v_total * 16)) : nullptr;
+  if (!drgb || (dL_dnormal && !dnrm)) return fail(ctx, DVX_ERR_OOM, "dvx_backward: allocator returned NULL");
   TreeFrame *trees_d = (TreeFrame *)f->trees_d.p;
   // box_rect was filled on the device; only the gradient pointers change, so patch those fields
   for (uint32_t t = 0; t < p.n_trees; ++t)
@@ -606,7 +636,7 @@ dvx_status dvx_backward_n(dvx_ctx *ctx, dvx_frame *f, const float *dL_drgb, cons
   A.p = p; A.trees = trees_d; A.fvox = (const FrameVox *)f->fvox.p; A.pxrect = (const ushort4 *)f->pxrect.p;
   A.ids = (const uint32_t *)f->ids.p; A.range_beg = (const uint32_t *)f->range_beg.p; A.range_end = (const uint32_t *)f->range_end.p;
   A.actor_mask = (const unsigned long long *)f->actor_mask.p;
-  A.tile_order = g_tile_order_on ? (const uint32_t *)f->tile_order.p : nullptr;
+  A.tile_order = (const uint32_t *)f->tile_order.p;
   A.sv_rgbd = (float *)f->sv_rgbd.p; A.sv_T = (float *)f->sv_T.p; A.sv_nused = (uint32_t *)f->sv_nused.p;
   A.counters = (unsigned long long *)f->counters.p;
   A.g_rgb = dL_drgb; A.g_depth = dL_ddepth; A.g_alpha = dL_dalpha; A.drgb = drgb;
@@ -624,8 +654,6 @@ dvx_status dvx_backward_n(dvx_ctx *ctx, dvx_frame *f, const float *dL_drgb, cons
   if (dnrm) dvx_normal_backward_launch(p, trees_d, A.pxrect, dnrm, st);
   CU(cudaEventRecord(f->ev[6], st));
   CU(cudaGetLastError());
-  ctx_release(ctx, drgb);
-  ctx_release(ctx, dnrm);
   f->did_backward = true;
   return DVX_OK;
 }
@@ -744,7 +772,7 @@ dvx_status dvx_stage_ms_collect(dvx_ctx *ctx, float *ms, uint32_t *n_frames) {
   return DVX_OK;
 }
 
-uint64_t dvx_launch_count(void) { return (uint64_t)g_dvx_launches; }
+uint64_t dvx_launch_count(void) { return (uint64_t)g_dvx_launches.load(std::memory_order_relaxed); }
 
 namespace {
 // lazily creates the copy stream and its events; (re)sizes a persistent staging buffer
@@ -822,7 +850,7 @@ dvx_status dvx_backward_host(dvx_ctx *ctx, dvx_frame *f, const float *g_rgb_h, c
 dvx_status dvx_sort_pairs(dvx_ctx *ctx, uint64_t *keys, uint32_t *vals, uint64_t n, uint32_t key_bits) {
   if (!ctx) return DVX_ERR_INVALID_ARG;
   if (n && (!keys || !vals)) return fail(ctx, DVX_ERR_INVALID_ARG, "NULL argument");
-  if (key_bits < 1 || key_bits > 64 || n >= 0xFFFFFFFFull) return fail(ctx, DVX_ERR_INVALID_ARG, "key_bits must be in [1,64], n < 2^32-1");
+  if (key_bits < 1 || key_bits > 64 || n >= (1ull << 30)) return fail(ctx, DVX_ERR_INVALID_ARG, "key_bits must be in [1,64], n < 2^30");
   if (n == 0) return DVX_OK;
   cudaSetDevice(ctx->device);
   uint64_t *kb = (uint64_t *)ctx_alloc(ctx, n * 8);
@@ -1015,8 +1043,19 @@ dvx_status dvx_frame_weights(dvx_ctx *ctx, dvx_frame *f, dvx_weights *out) {
   if (!f->w_row.p) {
     const size_t npix = (size_t)p.width * p.height;
     if (!buf_alloc(ctx, f->w_row, (npix + 1) * 4)) return fail(ctx, DVX_ERR_OOM, "dvx_frame_weights: allocator returned NULL");
+    // a failure below must not leave a half-built CSR behind: the next call would skip the build and hand out NULL arrays
+    struct Undo {
+      dvx_ctx *ctx; dvx_frame *f; bool armed = true;
+      ~Undo() {
+        if (!armed) return;
+        ctx_release(ctx, f->w_row.p); ctx_release(ctx, f->w_vox.p); ctx_release(ctx, f->w_val.p);
+        f->w_row.p = f->w_vox.p = f->w_val.p = nullptr;
+        f->w_nnz = 0;
+      }
+    } undo{ctx, f};
+    CallGuard guard(ctx);
     uint32_t *row = (uint32_t *)f->w_row.p;
-    void *scr = ctx_alloc(ctx, dvx_sort_scratch_bytes(npix + 1));
+    void *scr = guard.add(ctx_alloc(ctx, dvx_sort_scratch_bytes(npix + 1)));
     if (!scr) return fail(ctx, DVX_ERR_OOM, "dvx_frame_weights: allocator returned NULL");
     CU(cudaMemcpyAsync(row, f->sv_nused.p, npix * 4, cudaMemcpyDeviceToDevice, st));
     CU(cudaMemsetAsync(row + npix, 0, 4, st));
@@ -1024,7 +1063,6 @@ dvx_status dvx_frame_weights(dvx_ctx *ctx, dvx_frame *f, dvx_weights *out) {
     uint32_t nnz = 0;
     CU(cudaMemcpyAsync(&nnz, row + npix, 4, cudaMemcpyDeviceToHost, st));
     CU(cudaStreamSynchronize(st));
-    ctx_release(ctx, scr);
     f->w_nnz = nnz;
     if (!buf_alloc(ctx, f->w_vox, (size_t)nnz * 4) || !buf_alloc(ctx, f->w_val, (size_t)nnz * 4))
       return fail(ctx, DVX_ERR_OOM, "dvx_frame_weights: allocator returned NULL");
@@ -1033,11 +1071,12 @@ dvx_status dvx_frame_weights(dvx_ctx *ctx, dvx_frame *f, dvx_weights *out) {
     A.p = p; A.trees = (const TreeFrame *)f->trees_d.p; A.fvox = (const FrameVox *)f->fvox.p; A.pxrect = (const ushort4 *)f->pxrect.p;
     A.ids = (const uint32_t *)f->ids.p; A.range_beg = (const uint32_t *)f->range_beg.p; A.range_end = (const uint32_t *)f->range_end.p;
     A.actor_mask = (const unsigned long long *)f->actor_mask.p;
-  A.tile_order = g_tile_order_on ? (const uint32_t *)f->tile_order.p : nullptr;
+  A.tile_order = (const uint32_t *)f->tile_order.p;
     A.counters = (unsigned long long *)f->counters.p;
     A.exp_row = row; A.exp_vox = (uint32_t *)f->w_vox.p; A.exp_w = (float *)f->w_val.p;
     dvx_composite_export_launch(A, st);
     CU(cudaGetLastError());
+    undo.armed = false;
   }
   if (out) {
     out->nnz = f->w_nnz;
@@ -1089,7 +1128,7 @@ dvx_status dvx_cloud_create(dvx_ctx *ctx, const float *points, uint64_t n, float
   *out = nullptr;
   if (n && !points) return fail(ctx, DVX_ERR_INVALID_ARG, "dvx_cloud_create: points is NULL");
   if (!(cell > 0.f) || !isfinite(cell)) return fail(ctx, DVX_ERR_INVALID_ARG, "dvx_cloud_create: cell must be positive");
-  if (n >= (1ull << 31)) return fail(ctx, DVX_ERR_INVALID_ARG, "dvx_cloud_create: n must be below 2^31");
+  if (n >= (1ull << 30)) return fail(ctx, DVX_ERR_INVALID_ARG, "dvx_cloud_create: n must be below 2^30");
   cudaSetDevice(ctx->device);
   cudaStream_t st = ctx->st;
   dvx_cloud *c = new dvx_cloud();

@@ -3,6 +3,8 @@
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
+
+#include <atomic>
 #include "../../include/dvx.h"
 
 #define DVX_MAX_TREES (DVX_MAX_ACTORS + 1)
@@ -111,8 +113,8 @@ struct CompositeArgs {
 };
 
 // Number of kernels launched by this library since it was loaded (bench.py's gpu_launches claim).
-extern unsigned long long g_dvx_launches;
-#define DVX_COUNT_LAUNCH(n) (g_dvx_launches += (unsigned long long)(n))
+extern std::atomic<unsigned long long> g_dvx_launches;
+#define DVX_COUNT_LAUNCH(n) (g_dvx_launches.fetch_add((unsigned long long)(n), std::memory_order_relaxed))
 
 // ---- dvx_sort.cu
 size_t dvx_sort_scratch_bytes(uint64_t n);

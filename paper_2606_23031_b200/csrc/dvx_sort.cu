@@ -1,7 +1,8 @@
 // dvx_sort.cu - hot-path step 2: LSD radix sort of (64-bit key, 32-bit value) pairs, plus the exclusive scan it needs.
 // "per-tile key generation and radix sort in direction-dependent Morton order" (BASELINE.json north_star (2));
-// the paper only says the traversal is "Morton-ordered".  HBM-bound: per 8-bit pass the keys are
-// read twice and written once (histogram kernel + scatter kernel), values read once and written once.
+// the paper only says the traversal is "Morton-ordered".  One kernel per 8-bit digit (one-sweep with
+// decoupled look-back): per pass keys and values are read once and written once; one up-front kernel histograms every
+// digit position.  n < 2^30 pairs (the status word of the look-back keeps a 30-bit count).
 #include "dvx_internal.cuh"
 
 namespace {
@@ -83,101 +84,6 @@ __global__ void scan_apply(uint32_t *data, uint64_t n, const uint32_t *block_off
   for (int i = 0; i < SCAN_ITEMS; ++i) {
     if (base + i < n) data[base + i] = off;
     off += v[i];
-  }
-}
-
-// ------------------------------------------------------------------ radix pass
-__global__ void __launch_bounds__(SORT_THREADS) radix_hist(const uint64_t *keys, uint64_t n, uint32_t shift,
-                                                            uint32_t *block_hist, uint32_t n_blocks) {
-  __shared__ uint32_t h[RADIX];
-  h[threadIdx.x] = 0;
-  __syncthreads();
-  uint64_t base = (uint64_t)blockIdx.x * SORT_TILE;
-#pragma unroll 4
-  for (int i = 0; i < SORT_ITEMS; ++i) {
-    uint64_t idx = base + (uint64_t)i * SORT_THREADS + threadIdx.x;
-    if (idx < n) atomicAdd(&h[(uint32_t)(keys[idx] >> shift) & (RADIX - 1)], 1u);
-  }
-  __syncthreads();
-  block_hist[(uint64_t)threadIdx.x * n_blocks + blockIdx.x] = h[threadIdx.x];  // digit-major for the scan
-}
-
-// Stable scatter of one SORT_TILE-key tile.  Ranks inside the tile come from warp-private digit counters (__match_any_sync keeps
-// equal digits in lane order); the tile is first sorted by digit INTO SHARED MEMORY and only then written out, so that
-// consecutive threads write consecutive global addresses (runs of one digit) instead of 8-byte pieces of 32 sectors.
-__global__ void __launch_bounds__(SORT_THREADS) radix_scatter(const uint64_t *__restrict__ keys_in,
-                                                               const uint32_t *__restrict__ vals_in,
-                                                               uint64_t *__restrict__ keys_out, uint32_t *__restrict__ vals_out,
-                                                               uint64_t n, uint32_t shift, const uint32_t *__restrict__ offs,
-                                                               uint32_t n_blocks) {
-  __shared__ uint32_t cnt[SORT_WARPS][RADIX];
-  __shared__ uint64_t s_key[SORT_TILE];
-  __shared__ uint32_t s_val[SORT_TILE];
-  __shared__ uint32_t gbase[RADIX];
-  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-  for (int d = lane; d < RADIX; d += 32) cnt[w][d] = 0;
-  __syncwarp();
-  // warp w owns the contiguous keys [w*256, (w+1)*256) of the tile, in 8 steps of 32: order inside the tile is kept
-  const uint64_t tbase = (uint64_t)blockIdx.x * SORT_TILE;
-  const uint64_t wbase = tbase + (uint64_t)w * (32 * SORT_ITEMS);
-  uint64_t key[SORT_ITEMS];
-  uint16_t rnk[SORT_ITEMS];
-#pragma unroll
-  for (int i = 0; i < SORT_ITEMS; ++i) {
-    const uint64_t idx = wbase + (uint64_t)i * 32 + lane;
-    key[i] = idx < n ? keys_in[idx] : 0;
-  }
-#pragma unroll
-  for (int i = 0; i < SORT_ITEMS; ++i) {
-    const uint64_t idx = wbase + (uint64_t)i * 32 + lane;
-    const bool valid = idx < n;
-    const uint32_t d = valid ? ((uint32_t)(key[i] >> shift) & (RADIX - 1)) : RADIX;  // RADIX = "no key"
-    const uint32_t peers = __match_any_sync(0xffffffffu, d);
-    const uint32_t before = __popc(peers & ((1u << lane) - 1u));
-    const int leader = __ffs(peers) - 1;
-    uint32_t old = 0;
-    if (valid && lane == leader) {
-      old = cnt[w][d];
-      cnt[w][d] = old + __popc(peers);
-    }
-    old = __shfl_sync(0xffffffffu, old, leader);
-    rnk[i] = (uint16_t)(old + before);
-    __syncwarp();
-  }
-  __syncthreads();
-  {  // digit d = threadIdx.x: prefix over the warps, the tile-local base of the digit, and the global base
-    const int d = threadIdx.x;
-    uint32_t run = 0;
-#pragma unroll
-    for (int ww = 0; ww < SORT_WARPS; ++ww) {
-      const uint32_t c = cnt[ww][d];
-      cnt[ww][d] = run;
-      run += c;
-    }
-    uint32_t total;
-    const uint32_t lbase = block_excl_scan(run, &total);
-#pragma unroll
-    for (int ww = 0; ww < SORT_WARPS; ++ww) cnt[ww][d] += lbase;
-    gbase[d] = offs[(uint64_t)d * n_blocks + blockIdx.x] - lbase;
-  }
-  __syncthreads();
-#pragma unroll
-  for (int i = 0; i < SORT_ITEMS; ++i) {
-    const uint64_t idx = wbase + (uint64_t)i * 32 + lane;
-    if (idx < n) {
-      const uint32_t d = (uint32_t)(key[i] >> shift) & (RADIX - 1);
-      const uint32_t pos = cnt[w][d] + rnk[i];
-      s_key[pos] = key[i];
-      s_val[pos] = vals_in[idx];
-    }
-  }
-  __syncthreads();
-  const uint32_t nb = (uint32_t)min((uint64_t)SORT_TILE, n - tbase);
-  for (uint32_t i = threadIdx.x; i < nb; i += SORT_THREADS) {
-    const uint64_t k = s_key[i];
-    const uint32_t out = gbase[(uint32_t)(k >> shift) & (RADIX - 1)] + i;
-    keys_out[out] = k;
-    vals_out[out] = s_val[i];
   }
 }
 
@@ -346,19 +252,18 @@ void dvx_scan_u32_launch(uint32_t *data, uint64_t n, uint32_t *scratch, cudaStre
   { DVX_COUNT_LAUNCH(1); scan_apply<<<(unsigned)nb, SCAN_THREADS, 0, st>>>(data, n, scratch); }
 }
 
-// scratch: legacy path = per-tile histograms + scan levels; one-sweep path = digit histograms, tickets, tile status
+// scratch: digit histograms, tickets, tile status
 static size_t onesweep_words(uint64_t n) {
   uint64_t nb = ceil_div(n ? n : 1, SORT_TILE);
   return (size_t)MAX_PASSES * RADIX + MAX_PASSES + (size_t)MAX_PASSES * nb * RADIX;
 }
 size_t dvx_sort_scratch_bytes(uint64_t n) {
-  uint64_t nb = ceil_div(n ? n : 1, SORT_TILE);
-  uint64_t hist = nb * RADIX;
-  size_t legacy = hist + scan_scratch_elems(hist) + 64;
-  size_t one = onesweep_words(n) + 64;
-  return (legacy > one ? legacy : one) * sizeof(uint32_t);
+  // also used as the scratch of dvx_scan_u32_launch over n counters (the chain of block-sum levels is far smaller)
+  const size_t one = onesweep_words(n) + 64, scan = scan_scratch_elems(n) + 64;
+  return (one > scan ? one : scan) * sizeof(uint32_t);
 }
 
+// n must be below 2^30 (callers check).  2 + passes launches.
 int dvx_sort_launch(uint64_t *keys_a, uint32_t *vals_a, uint64_t *keys_b, uint32_t *vals_b, uint64_t n, uint32_t key_bits,
                     void *scratch, cudaStream_t st) {
   if (n == 0) return 0;
@@ -366,34 +271,19 @@ int dvx_sort_launch(uint64_t *keys_a, uint32_t *vals_a, uint64_t *keys_b, uint32
   int passes = (int)((key_bits + 7) / 8);
   if (passes < 1) passes = 1;
   int cur = 0;
-#ifndef DVX_SORT_LEGACY
-  if (n < (1ull << 30)) {  // one-sweep: 2 + passes launches
-    uint32_t *ghist = (uint32_t *)scratch;                 // [MAX_PASSES][RADIX]
-    uint32_t *ticket = ghist + MAX_PASSES * RADIX;         // [MAX_PASSES]
-    uint32_t *status = ticket + MAX_PASSES;                // [passes][nb][RADIX]
-    cudaMemsetAsync(scratch, 0, (MAX_PASSES * RADIX + MAX_PASSES + (size_t)passes * nb * RADIX) * sizeof(uint32_t), st);
-    const unsigned hb = nb < 592u ? nb : 592u;
-    { DVX_COUNT_LAUNCH(1); radix_digit_hist<<<hb, SORT_THREADS, 0, st>>>(keys_a, n, passes, ghist); }
-    { DVX_COUNT_LAUNCH(1); radix_digit_scan<<<passes, RADIX, 0, st>>>(ghist); }
-    for (int p = 0; p < passes; ++p) {
-      uint64_t *kin = cur ? keys_b : keys_a, *kout = cur ? keys_a : keys_b;
-      uint32_t *vin = cur ? vals_b : vals_a, *vout = cur ? vals_a : vals_b;
-      DVX_COUNT_LAUNCH(1);
-      radix_onesweep<<<nb, SORT_THREADS, 0, st>>>(kin, vin, kout, vout, n, 8u * p, ghist + p * RADIX,
-                                                  status + (size_t)p * nb * RADIX, ticket + p);
-      cur ^= 1;
-    }
-    return cur;
-  }
-#endif
-  uint32_t *hist = (uint32_t *)scratch;
-  uint32_t *scan_scr = hist + (uint64_t)nb * RADIX;
+  uint32_t *ghist = (uint32_t *)scratch;                 // [MAX_PASSES][RADIX]
+  uint32_t *ticket = ghist + MAX_PASSES * RADIX;         // [MAX_PASSES]
+  uint32_t *status = ticket + MAX_PASSES;                // [passes][nb][RADIX]
+  cudaMemsetAsync(scratch, 0, (MAX_PASSES * RADIX + MAX_PASSES + (size_t)passes * nb * RADIX) * sizeof(uint32_t), st);
+  const unsigned hb = nb < 592u ? nb : 592u;
+  { DVX_COUNT_LAUNCH(1); radix_digit_hist<<<hb, SORT_THREADS, 0, st>>>(keys_a, n, passes, ghist); }
+  { DVX_COUNT_LAUNCH(1); radix_digit_scan<<<passes, RADIX, 0, st>>>(ghist); }
   for (int p = 0; p < passes; ++p) {
     uint64_t *kin = cur ? keys_b : keys_a, *kout = cur ? keys_a : keys_b;
     uint32_t *vin = cur ? vals_b : vals_a, *vout = cur ? vals_a : vals_b;
-    { DVX_COUNT_LAUNCH(1); radix_hist<<<nb, SORT_THREADS, 0, st>>>(kin, n, 8u * p, hist, nb); }
-    dvx_scan_u32_launch(hist, (uint64_t)nb * RADIX, scan_scr, st);
-    { DVX_COUNT_LAUNCH(1); radix_scatter<<<nb, SORT_THREADS, 0, st>>>(kin, vin, kout, vout, n, 8u * p, hist, nb); }
+    DVX_COUNT_LAUNCH(1);
+    radix_onesweep<<<nb, SORT_THREADS, 0, st>>>(kin, vin, kout, vout, n, 8u * p, ghist + p * RADIX,
+                                                status + (size_t)p * nb * RADIX, ticket + p);
     cur ^= 1;
   }
   return cur;

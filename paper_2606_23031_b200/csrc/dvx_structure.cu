@@ -213,7 +213,7 @@ __global__ void __launch_bounds__(ST_THREADS) density_prior_kernel(CloudView c, 
                                                                    double cx, double cy, double cz, double side, double s_min,
                                                                    double reach, double v_close, double v_far,
                                                                    float *__restrict__ density) {
-  const uint32_t p = (blockIdx.x * ST_THREADS + threadIdx.x) >> 5;
+  const uint32_t p = (uint32_t)(((uint64_t)blockIdx.x * ST_THREADS + threadIdx.x) >> 5);  // 64-bit: n_points * 32 threads exceeds 2^32
   if (p >= n_points) return;
   const uint32_t slot = __ldg(slots + __ldg(offsets + p));
   const uint64_t cd = __ldg(code + (slot >> 3));
@@ -236,7 +236,7 @@ __global__ void __launch_bounds__(ST_THREADS) near_flags_kernel(CloudView c, con
                                                                 double cx, double cy, double cz, double side,
                                                                 double threshold, uint32_t max_level,
                                                                 uint32_t *__restrict__ count, uint8_t *__restrict__ split) {
-  const uint32_t v = (blockIdx.x * ST_THREADS + threadIdx.x) >> 5;
+  const uint32_t v = (uint32_t)(((uint64_t)blockIdx.x * ST_THREADS + threadIdx.x) >> 5);  // 64-bit: n_voxels * 32 threads exceeds 2^32
   if (v >= n_voxels) return;
   const uint64_t cd = __ldg(code + v);
   const uint32_t level = (uint32_t)(cd >> 48) & 31u;

@@ -22,3 +22,15 @@ def config1():
 def config3():
     import dvx_scenes
     return dvx_scenes.make_config(3)
+
+
+def pytest_terminal_summary(terminalreporter):
+    """Parity notes (how many pixels each test compared and how many threshold-ambiguous pixels it had to use)."""
+    try:
+        from helpers import NOTES
+    except ImportError:
+        return
+    if NOTES:
+        terminalreporter.write_sep("-", "parity notes")
+        for line in NOTES:
+            terminalreporter.write_line(line)

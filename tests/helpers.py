@@ -1,6 +1,14 @@
 """Small scene builders used by the pin tests (inputs only)."""
 import numpy as np
 import dvx_scenes as S
+
+NOTES = []   # one line per parity test (pixels compared, threshold-ambiguous pixels used); conftest prints them at the end
+
+
+def note(line):
+    NOTES.append(line)
+    print(line)
+
 from dvx_scenes.octree import Octree, encode, sort_morton, C0
 
 

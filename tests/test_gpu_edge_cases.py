@@ -292,3 +292,36 @@ def test_refresh_structure_and_max_actors(ctx):
         ctx.render(dev2.cams[0], dev2.trees[0], dev2.trees[1:] + [dev2.trees[1]], np.concatenate([dev2.poses, dev2.poses[:1]]),
                    np.concatenate([dev2.box_half, dev2.box_half[:1]]))
     assert e.value.status == -1
+
+
+def test_unaligned_gradient_buffers_are_rejected_and_trim_frees_the_cache(ctx):
+    """red.global.add.v4.f32 and the float4 read-modify-writes of the SH / normal post-passes fault on gradient
+    pointers that are not 16-byte aligned -> DVX_ERR_INVALID_ARG instead.  dvx_trim returns the scratch cache to the
+    allocator; the next frame renders the same image."""
+    import paper_2606_23031_b200 as dvx
+    import torch
+    sc = S.tiny_random_scene(3, sh_degree=1, width=40, height=24)
+    dev = dvx.SceneOnDevice(ctx, sc)
+    rgb0, _, _, fr = dev.render()
+    g = torch.from_numpy(sc.image_grads(0, 1e-2)["rgb"]).cuda()
+    good = dev.zero_grads()
+    for which in (0, 1):
+        bad = [list(x) for x in good]
+        t = dev.trees[0]
+        shape = (t.n_voxels, 8) if which == 0 else (t.n_voxels, t.n_sh, 3)
+        numel = int(np.prod(shape))
+        bad[0][which] = torch.zeros(numel + 1, device="cuda")[1:].view(shape)      # 4 bytes off a 16-byte boundary
+        assert bad[0][which].data_ptr() % 16 == 4
+        with pytest.raises(dvx.DvxError) as e:
+            fr.backward(g, grads=[tuple(x) for x in bad])
+        assert e.value.status == -1
+    fr.backward(g, grads=good)
+    torch.cuda.synchronize()
+    assert float(good[0][0].abs().max()) > 0
+    fr.release()
+    freed = ctx.trim()
+    assert freed > 0 and ctx.trim() == 0
+    rgb1, _, _, fr = dev.render()
+    torch.cuda.synchronize()
+    assert torch.equal(rgb0, rgb1)
+    fr.release()

@@ -62,7 +62,11 @@ def test_weights_rows_sum_to_alpha(ctx, config1):
     # composited sub-segments per ray: equal except where a grazing hit of ~zero length (weight ~0) is decided differently
     # in fp32 and fp64 - what is unique is the sum of the weights, checked below
     d = np.abs(np.diff(rows).reshape(H, W) - ref["n_used"].astype(np.int64))
-    assert (d != 0).mean() <= 0.1, (int(d.max()), float((d != 0).mean()))
+    from helpers import note
+    note("config 1 weight rows: n_used differs from the oracle on %.5f of the pixels (largest difference %d)" % (float((d != 0).mean()), int(d.max())))
+    # observed 2.6 % on B200 (config 1 is an axis-aligned uniform 1 m grid seen from a camera standing on its lattice planes:
+    # zero-length grazing hits are common); bound = twice the observation
+    assert (d != 0).mean() <= 0.052, (int(d.max()), float((d != 0).mean()))
     v_total = sum(t.n_voxels for t in config1.octrees)
     assert int(vox.max()) < v_total and float(w.min()) >= 0.0
     sums = np.add.reduceat(np.concatenate([w.cpu().numpy().astype(np.float64), [0.0]]), np.minimum(rows[:-1], nnz))

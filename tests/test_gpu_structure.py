@@ -181,3 +181,40 @@ def test_structure_argument_errors(ctx):
         ctx.density_prior(cloud, code, (0, 0, 0), 4.0, grid, 0.0)
     grid.close()
     cloud.close()
+
+
+def test_subdivide_near_beyond_2_27_leaves(ctx):
+    """the flag kernels index warps as (block * threads + thread) >> 5; with one warp per leaf that product passes
+    2^32 at 2^27 leaves, inside the documented range V < 2^28.  2^27 + 8192 level-10 leaves (a dense Morton prefix of the
+    cube), a handful of points inside the LAST leaves: only leaves with an index above 2^27 may be flagged, and they must be
+    flagged exactly as the oracle flags them on that tail (the head is checked to be all clear)."""
+    import torch
+    n = (1 << 27) + 8192
+    idx = torch.arange(n, dtype=torch.int64, device="cuda")
+    code = (idx << 18) | (10 << 48)               # 30-bit Morton path left-aligned in 48 bits, level 10
+    side, center = 1024.0, (0.0, 0.0, 0.0)        # level-10 cells of 1 m
+    tail = code[-64:].cpu().numpy().view(np.uint64)
+    lo, hi = T.voxel_boxes(tail, center, side)
+    rs = np.random.RandomState(5)
+    pts = (0.5 * (lo[::7] + hi[::7]) + rs.uniform(-0.2, 0.2, size=lo[::7].shape)).astype(np.float32)
+    thr = 0.45
+    cloud = ctx.cloud(_dev_pts(pts), 1.0)
+    desc_code = code.contiguous()
+    split = torch.zeros(n, dtype=torch.uint8, device="cuda")
+    import ctypes as C
+    import paper_2606_23031_b200.binding as B
+    desc = B.OctreeDesc(n, 0, (C.c_float * 3)(*center), side, desc_code.data_ptr(), None, None)
+    n_out = C.c_uint64()
+    ctx.check(ctx.lib.dvx_subdivide_near(ctx.h, cloud.h, C.byref(desc), thr, 11, None, 0, C.byref(n_out), split.data_ptr()))
+    torch.cuda.synchronize()
+    # reference on the last 4096 leaves (every point is inside one of the last 64), zero elsewhere
+    m = 4096
+    ref_new, ref_split = T.subdivide_near(code[-m:].cpu().numpy().view(np.uint64), np.asarray(center, np.float64), side,
+                                          pts.astype(np.float64), float(np.float32(thr)), 11)
+    got = split[-m:].cpu().numpy().astype(bool)
+    assert ref_split.sum() >= 10 and np.array_equal(got, ref_split)
+    assert int(split[:-m].sum().item()) == 0
+    assert n_out.value == n + 7 * int(ref_split.sum())
+    cloud.close()
+    del code, split, idx
+    ctx.trim()
