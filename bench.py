@@ -43,6 +43,7 @@ def parse_args():
     ap.add_argument("--opaque", action="store_true", help="report-only variant 3b: config 3 with raw += 8 on leaves holding a LiDAR return")
     ap.add_argument("--no-records", action="store_true",
                     help="A/B aid: DVX_FLAG_NO_RECORDS (the backward walks the tile lists again instead of replaying hit records)")
+    ap.add_argument("--no-extra", action="store_true", help="skip the extra workloads (configs 4 and 5) reported beside the headline")
     ap.add_argument("--profiler-range", action="store_true",
                     help="bracket the first timed region with cudaProfilerStart/Stop (use with ncu --profile-from-start off)")
     return ap.parse_args()
@@ -93,6 +94,15 @@ class ClockSampler:
                 "samples": len(sm), "power_w_max": max(power)}
 
 
+def config_dict(args, scene, world):
+    """The `config` object of the JSON line: the same keys from both arms (the driver compares them)."""
+    return {"workload": workload_name(args.config) + ("_opaque3b" if args.opaque else "") + ("_K%d" % args.k_samples if args.k_samples else ""),
+            "cameras": len(scene.cameras), "k_samples": scene.k_samples, "sh_degree": scene.static.sh_degree,
+            "voxels": int(sum(t.n_voxels for t in scene.octrees)), "actors": len(scene.actors),
+            "l2_policy": "inputs larger than L2 (voxel records + gradient buffers >> 126 MB)", "replicas": world,
+            "passes": "fwd" if args.fwd_only else "fwd+bwd"}
+
+
 # ----------------------------------------------------------------------------------------------- CPU oracle leg
 def oracle_sample(scene, n_tiles_sample, backward, seed=7):
     """Times the oracle (tile-culled mode, validated bit-identical to brute force by pin P13), as it stands, on a seeded
@@ -129,21 +139,25 @@ def pick_cpu_tiles(scene, backward):
 
 
 def run_reference(args, scene):
-    """--impl reference: the oracle as it stands on the host cores, each step a bounded sample of the workload."""
+    """--impl reference: the oracle as it stands on the host cores, each step a bounded sample of the workload.
+    `ms_per_step` is the wall time one step really took (so steps x ms_per_step is what the driver's clock saw); the
+    full-frame time the metric needs is extrapolated from it (binning + per-pixel time x W*H) under its own key."""
     n_tiles = args.cpu_tiles or max(4, pick_cpu_tiles(scene, True) // max(args.steps + args.warmup, 1))
-    vals = []
+    vals, wall = [], []
     for it in range(args.warmup + args.steps):
+        t0 = time.perf_counter()
         r = oracle_sample(scene, n_tiles, True, seed=100 + it)
         if it >= args.warmup:
             vals.append(r)
+            wall.append(time.perf_counter() - t0)
     mp = float(np.mean([r["mp_s_full_frame"] for r in vals]))
     cam = scene.cameras[0]
-    ms = cam.width * cam.height / (mp * 1e6) * 1e3
     sample = "%d seeded 16x16 tiles (%d px) of camera 0 per step, fwd+bwd, tile-culled oracle; full-frame time = binning + per-pixel time x W*H" % (
         vals[0]["tiles"], vals[0]["pixels"])
     line = {"impl": "reference", "metric": METRIC, "value": mp, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "f64", "data": "synthetic", "config": {"workload": workload_name(args.config), "inputs_exceed_l2": True},
+            "warmup": args.warmup, "ms_per_step": float(np.mean(wall)) * 1e3, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": config_dict(args, scene, args.gpus),
+            "full_frame_ms_extrapolated": cam.width * cam.height / (mp * 1e6) * 1e3,
             "cpu_baseline": {"value": mp, "unit": UNIT, "cores": vals[0]["threads"], "kind": "oracle", "sample": sample},
             "e2e": {"value": mp, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}
     print(json.dumps(line))
@@ -283,6 +297,9 @@ def feature_stats(ctx, dev, scene, peak, n_ch=64, reps=5):
     import torch
     cam = scene.cameras[0]
     H, W = cam.height, cam.width
+    _, _, _, fr = dev.render(0, save=True)   # warm call: first-use allocations of the CSR arrays go through the caching allocator
+    fr.weights()
+    fr.release()
     _, _, _, fr = dev.render(0, save=True)
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     torch.cuda.synchronize()
@@ -379,6 +396,56 @@ def structure_stats(ctx, dev, scene, n_points=2_000_000):
     return out
 
 
+def time_workload(ctx, dvx, cfg, steps, warmup):
+    """fwd+bwd step time of another BASELINE.json config on this context: every camera of the scene rendered and
+    back-propagated into one gradient set, inputs resident in HBM, CUDA events around `steps` steps after `warmup`."""
+    import torch
+    import dvx_scenes
+    scene = dvx_scenes.make_config(cfg)
+    dev = dvx.SceneOnDevice(ctx, scene)
+    grads = dev.zero_grads()
+    n_cams = len(scene.cameras)
+    cam0 = scene.cameras[0]
+    g_dev = [torch.from_numpy(scene.image_grads(c, rgb_std=1e-2)["rgb"]).to(ctx.device) for c in range(n_cams)]
+    out = (torch.empty((cam0.height, cam0.width, 3), device=ctx.device), torch.empty((cam0.height, cam0.width), device=ctx.device),
+           torch.empty((cam0.height, cam0.width), device=ctx.device))
+
+    outs = [tuple(torch.empty_like(t) for t in out) for _ in range(n_cams)] if n_cams > 1 else None
+
+    def step():
+        if n_cams > 1:   # the batched entry points: one host round trip, steps 1-2 and the SH post-pass on the second stream
+            _, frames = dev.render_batch(save=True, outs=outs)
+            ctx.backward_batch(frames, g_dev, grads)
+            for fr in frames:
+                fr.release()
+            return
+        _, _, _, fr = dev.render(0, save=True, out=out)
+        fr.backward(g_dev[0], grads=grads)
+        fr.release()
+    for _ in range(warmup):
+        step()
+    ctx.stage_ms_collect()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record()
+    for _ in range(steps):
+        step()
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / steps
+    sums, _ = ctx.stage_ms_collect()
+    px = n_cams * cam0.width * cam0.height
+    res = {"ms_per_step": ms, "value": px / ms / 1e3, "unit": UNIT, "cameras": n_cams, "steps": steps, "warmup": warmup,
+           "api": "dvx_render_batch + dvx_backward_batch" if n_cams > 1 else "dvx_render + dvx_backward",
+           "voxels": int(sum(t.n_voxels for t in scene.octrees)), "actors": len(scene.actors),
+           "stage_ms": {k: v / steps for k, v in sums.items()}}
+    for t in dev.trees:
+        t.close()
+    del dev, grads, g_dev, out
+    ctx.trim()
+    return res
+
+
 def run_dvx(args):
     import torch
     import torch.distributed as dist
@@ -408,7 +475,16 @@ def run_dvx(args):
                torch.empty((H, W), dtype=torch.float32, device=ctx.device))
     out_host = tuple(t.cpu().pin_memory() for t in out_dev)
 
+    outs_b = [tuple(torch.empty_like(t) for t in out_dev) for _ in range(n_cams)] if n_cams > 1 else None
+
     def step(host=False, bwd=True):
+        if n_cams > 1 and not host and not args.no_records:   # config 5: the batched entry points
+            _, frames = dev.render_batch(save=bwd, outs=outs_b)
+            if bwd:
+                ctx.backward_batch(frames, g_dev, grads)
+                for fr in frames:
+                    fr.release()
+            return
         for c in range(n_cams):
             _, _, _, fr = dev.render(c, save=bwd, out=out_host if host else out_dev, host=host,
                                      flags=dvx.FLAG_NO_RECORDS if args.no_records else 0)
@@ -491,6 +567,17 @@ def run_dvx(args):
     feat_stats = feature_stats(ctx, dev, scene, measured_peaks()[0]) if rank == 0 and not args.fwd_only else None
     struct_stats = structure_stats(ctx, dev, scene) if rank == 0 and not args.fwd_only else None
     opt_stats = optimizer_step_stats(ctx, dev, grads, measured_peaks()[0]) if rank == 0 and not args.fwd_only else None
+    rec_stats = None
+    if rank == 0 and not args.fwd_only and not args.no_records:   # what the hit records of one frame take (camera 0)
+        _, _, _, fr = dev.render(0, save=True)
+        rec_stats = fr.record_stats()
+        rec_stats["bytes_per_hit"] = rec_stats["bytes_used"] / max(cnt["q_hit"] / n_cams, 1)
+        fr.release()
+    extra = None
+    if rank == 0 and args.config == 3 and not (args.no_extra or args.fwd_only or args.opaque or args.k_samples or args.no_records):
+        extra = {}
+        for cfg_x in (4, 5):   # BASELINE.json configs[3] (crowded) and configs[4] (6-camera training batch), device-resident
+            extra[workload_name(cfg_x)] = time_workload(ctx, dvx, cfg_x, steps=max(3, min(args.steps, 10)), warmup=3)
 
     if rank != 0:
         if world > 1:
@@ -502,47 +589,71 @@ def run_dvx(args):
     e2e_value = aggregate_value(px_step, world, ms_e2e / args.steps)
     peak, peak_src, peaks = measured_peaks()
     ab = algorithmic_bytes(scene, W, H, {k: v / 1 for k, v in cnt.items()}, touched)
-    dom = "composite_bwd" if not args.fwd_only else "composite_fwd"
-    dom_ms = stage.get("backward_composite" if not args.fwd_only else "composite", 0.0)
+    # ---- rooflines.  [NS] names the HBM roofline; the compositing kernels are bound by instruction issue,
+    # so both are reported: HBM for the dominant kernel (the one with the largest share of the step in THIS run), and the issue
+    # rate against the FMA / issue peak measured a moment ago by dvx_microbench_fma on this device.
+    kernels = {"composite_fwd": stage.get("composite", 0.0)}
+    if not args.fwd_only:
+        kernels["composite_bwd"] = stage.get("backward_composite", 0.0)
+    dom = max(kernels, key=kernels.get)
+    dom_ms = kernels[dom]
     dom_bytes = ab[dom]
     achieved = dom_bytes / (dom_ms * 1e-3) / 1e9 if dom_ms > 0 else 0.0
-    ncu_traffic = None
-    try:  # per-launch DRAM bytes of the dominant kernel from the committed ncu --set full capture, if present
-        ncu_traffic = json.load(open(os.path.join(ROOT, "profiles", "traffic.json"))).get(dom)
+    prof = {}
+    try:  # ncu --set full capture of the two compositing kernels (profiles/traffic.json names its commit and source hash)
+        prof = json.load(open(os.path.join(ROOT, "profiles", "traffic.json")))
     except (OSError, ValueError):
         pass
-    hbm_frac_step = ab["min_fwdbwd" if not args.fwd_only else "min_fwd"] / (ms_step * 1e-3) / 1e9 / peak
-    # fp32-lane roofline of the same kernel: algorithmic lane-operations from the run's own counters
-    # (slab test ~20, per composited sub-segment: cubic fold + K samples x 5 + blend ~115 forward, ~260 with the backward's
-    # moments, corner sums and reduction) against 148 SMs x 128 fp32 lanes x the SM clock sampled under load
-    K = scene.k_samples
-    lane_ops = cnt["q_test"] * 20 + cnt["q_hit"] * ((75 + 5 * K) if args.fwd_only else (220 + 5 * K))
-    sm_mhz = (clocks or {}).get("sm_mhz") or peaks.get("sm_max_mhz") or 1965.0
-    alu_peak = 148 * 128 * sm_mhz * 1e6 / 1e12
-    alu_ach = lane_ops / (dom_ms * 1e-3) / 1e12 if dom_ms > 0 else 0.0
+    src = os.path.join(ROOT, "paper_2606_23031_b200", "csrc", "dvx_composite_tile.cu")
+    try:
+        import hashlib
+        src_sha = hashlib.sha256(open(src, "rb").read()).hexdigest()
+    except OSError:
+        src_sha = None
+    stale = (not prof) or prof.get("source_sha256") != src_sha or prof.get("workload") != workload_name(args.config)
+    pk = prof.get("kernels", {})
+    hbm_floor_ms = ab["min_fwdbwd" if not args.fwd_only else "min_fwd"] / peak / 1e6
+    hbm_frac_step = hbm_floor_ms / ms_step
+    mb = ctx.microbench_fma()
+    issue_peak = mb["warp_instr_per_s"]
+    issue = {"peak_warp_instr_per_s": issue_peak, "peak_lane_fma_per_s": mb["lane_fma_per_s"],
+             "peak_source": "dvx_microbench_fma in this run (%.3f ms, 16 FFMA chains per thread on every warp slot)" % mb["ms"],
+             "nominal_warp_instr_per_s": 148 * 4 * ((clocks or {}).get("sm_mhz") or peaks.get("sm_max_mhz") or 1965.0) * 1e6,
+             "kernels": {}}
+    issue_floor_ms = None
+    if pk and not stale:
+        issue_floor_ms = 0.0
+        for k, ms_k in kernels.items():
+            if k in pk and ms_k > 0:
+                wi = pk[k]["warp_instructions"]
+                floor = wi / issue_peak * 1e3
+                issue_floor_ms += floor
+                issue["kernels"][k] = {"warp_instructions": wi, "ms": ms_k, "achieved_warp_instr_per_s": wi / (ms_k * 1e-3),
+                                       "frac": wi / (ms_k * 1e-3) / issue_peak, "issue_floor_ms": floor}
+    binding = max(hbm_floor_ms, issue_floor_ms or 0.0)
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
-        "data": "synthetic",
-        "config": {"workload": workload_name(args.config) + ("_opaque3b" if args.opaque else "") + ("_K%d" % args.k_samples if args.k_samples else ""), "cameras": n_cams, "k_samples": scene.k_samples, "sh_degree": scene.static.sh_degree,
-                   "voxels": int(sum(t.n_voxels for t in scene.octrees)), "actors": len(scene.actors),
-                   "l2_policy": "inputs larger than L2 (voxel records + gradient buffers >> 126 MB)", "replicas": world,
-                   "passes": "fwd" if args.fwd_only else "fwd+bwd"},
+        "data": "synthetic", "config": config_dict(args, scene, world),
         "fwd_value": fwd_value, "fwd_ms": ms_fwd / args.steps,
-        "hbm_roofline_frac_step": hbm_frac_step,
+        "hbm_roofline_frac_step": hbm_frac_step,       # the [NS] definition: B_min / peak / step time (target 0.5: NOT met)
+        "hbm_floor_ms": hbm_floor_ms, "issue_floor_ms": issue_floor_ms,
+        "frac_of_binding_floor": binding / ms_step if ms_step > 0 else None,
         "stage_ms": stage,
         "counters": dict(cnt, touched_voxels=touched, hits_per_ray=cnt["q_hit"] / px_step, frac_rays_terminated=frac_term),
+        "records": rec_stats,
         "step0_uncached_ms_static_octree": step0_ms, "grad_zero_ms_excluded": grad_zero_ms,
         "algorithmic_bytes": ab,
         "roofline": {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
-                     "frac": achieved / peak if peak else None, "traffic": ncu_traffic, "peak_source": peak_src,
-                     "bytes_per_launch": dom_bytes, "ms_per_launch": dom_ms},
-        "alu_roofline": {"bound": "alu", "kernel": dom, "achieved": alu_ach, "peak": alu_peak, "unit": "Tlane-op/s",
-                         "frac": alu_ach / alu_peak, "lane_ops_per_launch": lane_ops,
-                         "peak_source": "148 SMs x 128 fp32 lanes x %.0f MHz (nvidia-smi, under load)" % sm_mhz},
+                     "frac": achieved / peak if peak else None,
+                     "traffic": (pk.get(dom) or {}).get("dram_bytes"), "traffic_commit": prof.get("commit"),
+                     "traffic_stale": bool(stale), "peak_source": peak_src, "bytes_per_launch": dom_bytes, "ms_per_launch": dom_ms,
+                     "all_kernels_ms": kernels},
+        "issue_roofline": dict(issue, bound="alu", unit="warp-instr/s", profile_commit=prof.get("commit"), profile_stale=bool(stale)),
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": (0 if args.fwd_only else 12 * px_step),
                 "d2h_bytes_per_step": 20 * px_step, "ms_per_step": ms_e2e / args.steps},
         "sort": sort_stats, "n2_optimizer_step": opt_stats, "n3_features": feat_stats, "n4_structure": struct_stats,
+        "extra_workloads": extra,
         "gpu_launches": launches, "clocks": clocks,
     }
     if not args.no_cpu_baseline and world == 1:

@@ -120,7 +120,9 @@ typedef struct {
                     its trilinear raw density at the voxel centre, divided by max(|g|, 1e-6) */
 } dvx_image;
 
-/* Steps 1-4 of the hot path.  poses_l2w: HOST [N][12] row-major [R_i | t_i] local->world;
+/* Steps 1-4 of the hot path.  All work is enqueued on the context's stream; the call blocks the host ONCE, between step 1
+ * and step 2, to read the number of (tile, octant, voxel) pairs that sizes the sort buffers (dvx_render_batch amortises
+ * that round trip over its cameras).  poses_l2w: HOST [N][12] row-major [R_i | t_i] local->world;
  * box_half: HOST [N][3] half extents of the oriented box in the actor frame.  opts NULL = defaults
  * (K=8, exp, t_stop=1e-4, flags 0).  saved: if non-NULL receives a frame handle for dvx_backward / introspection
  * (release with dvx_frame_release); NULL = inference, nothing kept. */
@@ -145,6 +147,23 @@ dvx_status dvx_backward_n(dvx_ctx *ctx, dvx_frame *saved, const float *dL_drgb, 
                           const float *dL_dalpha, const float *dL_dnormal, dvx_grad static_grad,
                           const dvx_grad *actor_grads);
 void dvx_frame_release(dvx_ctx *ctx, dvx_frame *frame);
+
+/* Several cameras at once (BASELINE.json configs[4]: six surround cameras sharing the octrees, the poses of one timestamp
+ * and ONE gradient set, one forward + backward per training iteration).  Results are those of n_cams
+ * dvx_render / n_frames dvx_backward calls in the same order (gradients up to float summation order).  What differs is the
+ * schedule: step 1 of every camera is enqueued first and the pair counts of all of them come back in ONE host round trip
+ * instead of one per camera; camera c's key generation and sort (step 2) run on a second, library-owned high-priority
+ * stream under camera c-1's compositing kernel; in the backward, frame c's per-voxel SH post-pass runs there under frame
+ * c+1's replay.  Events order the two streams against the context's stream on entry and on exit, so the caller sees one
+ * stream as before.  cams: HOST [n_cams]; outs: HOST [n_cams] of DEVICE image pointers; saved: HOST [n_cams] frame handles
+ * out, or NULL (inference); dL_drgb: HOST [n_frames] of DEVICE pointers, dL_ddepth / dL_dalpha likewise or NULL (arrays
+ * or their entries).  Frames rendered with a normal map take dvx_backward_n, one by one (its post-pass writes dgeo). */
+dvx_status dvx_render_batch(dvx_ctx *ctx, uint32_t n_cams, const dvx_camera *cams, const dvx_octree *static_tree,
+                            uint32_t n_actors, const dvx_octree *const *actors, const float *poses_l2w,
+                            const float *box_half, const dvx_render_opts *opts, const dvx_image *outs, dvx_frame **saved);
+dvx_status dvx_backward_batch(dvx_ctx *ctx, uint32_t n_frames, dvx_frame *const *frames, const float *const *dL_drgb,
+                              const float *const *dL_ddepth, const float *const *dL_dalpha, dvx_grad static_grad,
+                              const dvx_grad *actor_grads);
 
 /* Hit records.  When dvx_render is given a `saved` handle, the compositing kernel also writes what it composited -
  * per (pixel, voxel) hit 40 bytes: voxel, octree, the clipped segment in the voxel's local coordinates, its length / K
@@ -191,6 +210,12 @@ dvx_status dvx_frame_stage_ms(dvx_ctx *ctx, const dvx_frame *frame, float *ms_ou
  * *n_frames = how many.  Lets a benchmark time the stages of the very steps it measures without keeping frames alive.
  * HOST ms_out8[8], HOST n_frames.  Synchronises the stream. */
 dvx_status dvx_stage_ms_collect(dvx_ctx *ctx, float *ms_out8, uint32_t *n_frames);
+/* The device's fp32 FMA rate, measured now: a kernel of independent FFMA chains on every warp slot of every SM, timed
+ * with CUDA events on the context's stream (synchronises).  One FFMA per lane per clock per SM sub-partition is both the
+ * fp32 peak and the instruction-issue peak, so this is the denominator of the issue-rate roofline that bounds the
+ * compositing kernels (SURVEY.md 8(d) asks for a measured FMA peak from the same run).  iters: loop trips of 64 FFMA per
+ * thread (1 << 14 runs for about a millisecond).  Any output pointer may be NULL. */
+dvx_status dvx_microbench_fma(dvx_ctx *ctx, uint32_t iters, double *lane_fma_per_s, double *warp_instr_per_s, float *ms);
 /* Kernels launched by the library in this process so far (all contexts). */
 uint64_t dvx_launch_count(void);
 const char *dvx_last_error(const dvx_ctx *ctx);

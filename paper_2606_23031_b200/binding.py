@@ -27,7 +27,7 @@ EXPORTS = ["dvx_create", "dvx_destroy", "dvx_octree_create", "dvx_octree_refresh
            "dvx_grid_adam_step", "dvx_adam_step", "dvx_grid_adam_step_n", "dvx_adam_step_n",
            "dvx_frame_weights", "dvx_render_features", "dvx_fuse_features",
            "dvx_cloud_create", "dvx_cloud_destroy", "dvx_density_prior", "dvx_subdivide_near", "dvx_prune",
-           "dvx_set_record_budget", "dvx_frame_record_stats", "dvx_trim"]
+           "dvx_set_record_budget", "dvx_frame_record_stats", "dvx_trim", "dvx_microbench_fma", "dvx_render_batch", "dvx_backward_batch"]
 
 
 class DvxError(RuntimeError):
@@ -140,7 +140,11 @@ def load():
     lib.dvx_prune.argtypes = [P, C.c_uint32, P, P, C.c_float, P, P, C.POINTER(C.c_uint32)]
     lib.dvx_grid_adam_step_n.argtypes = [P, C.POINTER(Adam), C.c_uint32, C.POINTER(GridAdamItem)]
     lib.dvx_adam_step_n.argtypes = [P, C.POINTER(Adam), C.c_uint32, C.POINTER(AdamItem)]
+    lib.dvx_render_batch.argtypes = [P, C.c_uint32, C.POINTER(Camera), P, C.c_uint32, C.POINTER(P), P, P, C.POINTER(RenderOpts),
+                                     C.POINTER(Image), C.POINTER(P)]
+    lib.dvx_backward_batch.argtypes = [P, C.c_uint32, C.POINTER(P), C.POINTER(P), C.POINTER(P), C.POINTER(P), Grad, C.POINTER(Grad)]
     lib.dvx_trim.argtypes = [P, C.POINTER(C.c_uint64)]
+    lib.dvx_microbench_fma.argtypes = [P, C.c_uint32, C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_float)]
     lib.dvx_set_record_budget.argtypes = [P, C.c_uint64]
     lib.dvx_frame_record_stats.argtypes = [P, P, C.POINTER(C.c_uint64), C.POINTER(C.c_uint64), C.POINTER(C.c_uint32)]
     for name in EXPORTS:
@@ -195,6 +199,12 @@ class Context:
         n = C.c_uint32()
         self.check(self.lib.dvx_stage_ms_collect(self.h, ms, C.byref(n)))
         return dict(zip(STAGES, list(ms)[:6])), n.value
+
+    def microbench_fma(self, iters=1 << 14):
+        """dvx_microbench_fma -> dict(lane_fma_per_s, warp_instr_per_s, ms)."""
+        a, b, ms = C.c_double(), C.c_double(), C.c_float()
+        self.check(self.lib.dvx_microbench_fma(self.h, iters, C.byref(a), C.byref(b), C.byref(ms)))
+        return {"lane_fma_per_s": a.value, "warp_instr_per_s": b.value, "ms": ms.value}
 
     def trim(self):
         """dvx_trim: hand every cached scratch block back to the allocator -> bytes freed."""
@@ -288,6 +298,41 @@ class Context:
         arr = (AdamItem * max(len(items), 1))(*[AdamItem(p.numel(), p.data_ptr(), m.data_ptr(), v.data_ptr(), g.data_ptr())
                                                 for p, m, v, g in items])
         self.check(self.lib.dvx_adam_step_n(self.h, C.byref(hp), len(items), arr))
+
+    # ------------------------------------------------------------------ batched render / backward (config 5)
+    def render_batch(self, cams, static, actors=(), poses=None, box_half=None, k_samples=8, activation=0, t_stop=1e-4, flags=0,
+                     save=True, outs=None):
+        """dvx_render_batch: cams = list of binding.Camera; outs = list of (rgb, depth, alpha) device tensors or None.
+        Returns (list of (rgb, depth, alpha), list of Frame or None)."""
+        torch = self.torch
+        n_c = len(cams)
+        if outs is None:
+            outs = [(torch.empty((c.height, c.width, 3), dtype=torch.float32, device=self.device),
+                     torch.empty((c.height, c.width), dtype=torch.float32, device=self.device),
+                     torch.empty((c.height, c.width), dtype=torch.float32, device=self.device)) for c in cams]
+        n = len(actors)
+        handles = (C.c_void_p * max(n, 1))(*[a.h for a in actors])
+        poses = np.ascontiguousarray(np.zeros((0, 12)) if poses is None else poses, dtype=np.float32).reshape(-1)
+        half = np.ascontiguousarray(np.zeros((0, 3)) if box_half is None else box_half, dtype=np.float32).reshape(-1)
+        assert poses.size == 12 * n and half.size == 3 * n
+        opts = RenderOpts(k_samples, activation, t_stop, flags, None)
+        cam_arr = (Camera * n_c)(*cams)
+        img_arr = (Image * n_c)(*[Image(o[0].data_ptr(), o[1].data_ptr(), o[2].data_ptr(), None) for o in outs])
+        fh = (C.c_void_p * n_c)()
+        self.check(self.lib.dvx_render_batch(self.h, n_c, cam_arr, static.h, n, handles, poses.ctypes.data_as(C.c_void_p),
+                                             half.ctypes.data_as(C.c_void_p), C.byref(opts), img_arr, fh if save else None))
+        frames = [Frame(self, C.c_void_p(fh[i]), [static] + list(actors)) for i in range(n_c)] if save else None
+        return outs, frames
+
+    def backward_batch(self, frames, dL_drgb, grads, dL_ddepth=None, dL_dalpha=None):
+        """dvx_backward_batch: frames / dL_drgb lists of equal length; grads = list of (dgeo, dsh) per octree (accumulated)."""
+        n_f = len(frames)
+        ptrs = lambda ts: None if ts is None else (C.c_void_p * n_f)(*[None if t is None else t.data_ptr() for t in ts])
+        g = [Grad(a.data_ptr() if a is not None else None, b.data_ptr() if b is not None else None) for a, b in grads]
+        arr = (Grad * max(len(g) - 1, 1))(*g[1:])
+        fr = (C.c_void_p * n_f)(*[f.h for f in frames])
+        self.check(self.lib.dvx_backward_batch(self.h, n_f, fr, ptrs(dL_drgb), ptrs(dL_ddepth), ptrs(dL_dalpha), g[0], arr))
+        return grads
 
     # ------------------------------------------------------------------ render / backward
     def render(self, cam, static, actors=(), poses=None, box_half=None, k_samples=8, activation=0, t_stop=1e-4, flags=0,
@@ -543,6 +588,14 @@ class SceneOnDevice:
         kw.update(opt)
         return self.ctx.render(self.cams[cam_index], self.trees[0], self.trees[1:], self.poses, self.box_half, flags=flags,
                                save=save, out=out, host=host, sky=sky, dsky=dsky, normals=normals, **kw)
+
+    def render_batch(self, cam_indices=None, save=True, flags=0, outs=None, **opt):
+        s = self.scene
+        kw = dict(k_samples=s.k_samples, activation=s.activation, t_stop=s.t_stop)
+        kw.update(opt)
+        cams = [self.cams[c] for c in (range(len(self.cams)) if cam_indices is None else cam_indices)]
+        return self.ctx.render_batch(cams, self.trees[0], self.trees[1:], self.poses, self.box_half, flags=flags, save=save,
+                                     outs=outs, **kw)
 
     def zero_grads(self):
         torch = self.ctx.torch

@@ -11,7 +11,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libdvx.so")
-SOURCES = ["dvx_sort.cu", "dvx_preprocess.cu", "dvx_composite_naive.cu", "dvx_composite_tile.cu", "dvx_grid.cu", "dvx_features.cu", "dvx_structure.cu", "dvx_api.cu"]
+SOURCES = ["dvx_sort.cu", "dvx_preprocess.cu", "dvx_composite_naive.cu", "dvx_composite_tile.cu", "dvx_grid.cu", "dvx_features.cu", "dvx_structure.cu", "dvx_microbench.cu", "dvx_api.cu"]
 HEADERS = [os.path.join(CSRC, "dvx_internal.cuh"), os.path.join(CSRC, "dvx_device.cuh"), os.path.join(CSRC, "dvx_ray.cuh"),
            os.path.join(HERE, "..", "include", "dvx.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",

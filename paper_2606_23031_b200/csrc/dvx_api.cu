@@ -14,7 +14,7 @@ std::atomic<unsigned long long> g_dvx_launches{0};
 
 // The CUDA events of one render (+ backward) call.  Owned by the context and recycled, so the steady state creates none.
 struct EventSet {
-  cudaEvent_t ev[9] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+  cudaEvent_t ev[10] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
   bool rendered = false, did_backward = false;
 };
 
@@ -37,11 +37,19 @@ struct dvx_ctx {
   size_t st_out_bytes = 0, st_in_bytes = 0;
   // hit-record pool sizing: chunks per pixel used by the last frames (read back lazily, never waited for)
   uint64_t rec_budget = 0;             // dvx_set_record_budget: bytes per frame, 0 = automatic
-  double rec_seen[8] = {0, 0, 0, 0, 0, 0, 0, 0};  // chunks per pixel of the last 8 frames whose count has arrived
+  static constexpr int REC_SLOTS = 16;
+  double rec_seen[REC_SLOTS] = {};      // chunks per pixel of the last frames whose count has arrived
   int rec_seen_n = 0;
-  unsigned long long *h_rec = nullptr;  // pinned: [0] chunks handed out by the frame in flight
-  cudaEvent_t ev_rec = nullptr;
-  double rec_pending_npix = 0;          // > 0: a read-back is in flight for a frame of that many pixels
+  unsigned long long *h_rec = nullptr;  // pinned [REC_SLOTS]: chunks handed out by a frame in flight
+  cudaEvent_t ev_rec[REC_SLOTS] = {};
+  double rec_pending_npix[REC_SLOTS] = {};  // > 0: a read-back is in flight in this slot for a frame of that many pixels
+  int rec_slot = 0;                     // next slot to use (a batch of cameras has one read-back per camera in flight)
+  // batched entry points: a second, high-priority stream for steps 1-2 and the per-voxel post-passes
+  cudaStream_t ps = nullptr;
+  cudaEvent_t ev_entry = nullptr;
+  std::vector<cudaEvent_t> ev_batch;
+  unsigned long long *h_batch = nullptr;  // pinned [h_batch_n][CNT_N]
+  uint32_t h_batch_n = 0;
 };
 
 struct dvx_octree {
@@ -66,6 +74,7 @@ struct dvx_frame {
   struct Buf { void *p = nullptr; size_t bytes = 0; };
   Buf trees_d, fvox, pxrect, octmask, actor_mask, ids, range_beg, range_end, counters, sv_rgbd, sv_T, sv_nused;
   uint64_t n_pairs = 0, v_vis = 0;
+  const unsigned long long *h_cnt = nullptr;  // pinned copy of the counters after step 1 (valid until step 2 has read it)
   EventSet *es = nullptr;
   cudaEvent_t *ev = nullptr;  // = es->ev
   Buf eff_end, vnrm, sv_nrm;
@@ -244,16 +253,18 @@ dvx_status dvx_create(int device, void *cuda_stream, dvx_alloc_fn alloc, dvx_fre
   ctx->device = device;
   ctx->st = (cudaStream_t)cuda_stream;
   ctx->alloc = alloc; ctx->free_ = free_; ctx->user = user;
-  if (cudaMallocHost((void **)&ctx->h_counters, (CNT_N + 1) * sizeof(unsigned long long)) != cudaSuccess) {
+  if (cudaMallocHost((void **)&ctx->h_counters, (CNT_N + dvx_ctx::REC_SLOTS) * sizeof(unsigned long long)) != cudaSuccess) {
     delete ctx;
     return DVX_ERR_CUDA;
   }
   ctx->h_rec = ctx->h_counters + CNT_N;
-  if (cudaEventCreateWithFlags(&ctx->ev_rec, cudaEventDisableTiming) != cudaSuccess) {
-    cudaFreeHost(ctx->h_counters);
-    delete ctx;
-    return DVX_ERR_CUDA;
-  }
+  for (int i = 0; i < dvx_ctx::REC_SLOTS; ++i)
+    if (cudaEventCreateWithFlags(&ctx->ev_rec[i], cudaEventDisableTiming) != cudaSuccess) {
+      for (int j = 0; j < i; ++j) cudaEventDestroy(ctx->ev_rec[j]);
+      cudaFreeHost(ctx->h_counters);
+      delete ctx;
+      return DVX_ERR_CUDA;
+    }
   *out = ctx;
   return DVX_OK;
 }
@@ -267,7 +278,10 @@ void dvx_destroy(dvx_ctx *ctx) {
     else cudaFree(b.p);
   }
   cudaFreeHost(ctx->h_counters);
-  cudaEventDestroy(ctx->ev_rec);
+  for (cudaEvent_t e : ctx->ev_rec) cudaEventDestroy(e);
+  if (ctx->ps) { cudaStreamSynchronize(ctx->ps); cudaStreamDestroy(ctx->ps); cudaEventDestroy(ctx->ev_entry); }
+  for (cudaEvent_t e : ctx->ev_batch) cudaEventDestroy(e);
+  if (ctx->h_batch) cudaFreeHost(ctx->h_batch);
   if (ctx->cs) {
     cudaStreamSynchronize(ctx->cs);
     cudaStreamSynchronize(ctx->cs_in);
@@ -372,14 +386,17 @@ void setup_tree(TreeFrame &T, const dvx_octree *t, uint32_t base, bool actor, co
 
 // ---- hit-record pool sizing (dvx.h "Hit records") ------------------------------------------------------------------------
 // The chunk count of a frame is copied to pinned memory behind its forward and picked up here, without waiting, by a later
-// dvx_render; the pool of the next frame is 1.25 x the largest count per pixel among the last 8 frames seen.
+// dvx_render; the pool of the next frame is 1.25 x the largest count per pixel among the last 16 frames seen.
 void rec_collect(dvx_ctx *ctx) {
-  if (ctx->rec_pending_npix > 0 && cudaEventQuery(ctx->ev_rec) == cudaSuccess) {
-    ctx->rec_seen[ctx->rec_seen_n % 8] = (double)ctx->h_rec[0] / ctx->rec_pending_npix;
-    ctx->rec_seen_n++;
-    ctx->rec_pending_npix = 0;
-  } else {
-    cudaGetLastError();  // cudaErrorNotReady is not an error
+  for (int i = 0; i < dvx_ctx::REC_SLOTS; ++i) {
+    if (ctx->rec_pending_npix[i] <= 0) continue;
+    if (cudaEventQuery(ctx->ev_rec[i]) == cudaSuccess) {
+      ctx->rec_seen[ctx->rec_seen_n % dvx_ctx::REC_SLOTS] = (double)ctx->h_rec[i] / ctx->rec_pending_npix[i];
+      ctx->rec_seen_n++;
+      ctx->rec_pending_npix[i] = 0;
+    } else {
+      cudaGetLastError();  // cudaErrorNotReady is not an error
+    }
   }
 }
 uint64_t rec_capacity(const dvx_ctx *ctx, const FrameParams &p) {
@@ -392,7 +409,7 @@ uint64_t rec_capacity(const dvx_ctx *ctx, const FrameParams &p) {
     cap = ceil(npix * 48.0 / 32.0 / DVX_REC_CHUNK) + 0.5 * n_warps;  // 48 hits per pixel + half a chunk per warp unfilled
   } else {
     double m = 0;
-    for (int i = 0; i < 8 && i < ctx->rec_seen_n; ++i) m = fmax(m, ctx->rec_seen[i]);
+    for (int i = 0; i < dvx_ctx::REC_SLOTS && i < ctx->rec_seen_n; ++i) m = fmax(m, ctx->rec_seen[i]);
     cap = ceil(1.25 * m * npix) + 0.125 * n_warps + 16.0;
   }
   return cap > 4.0e9 ? 4000000000ull : (uint64_t)cap;
@@ -412,16 +429,16 @@ bool rigid(const float *m, int stride) {  // rows of a 3x3 inside a row-major ma
 
 extern "C" {
 
-dvx_status dvx_render(dvx_ctx *ctx, const dvx_camera *cam, const dvx_octree *static_tree, uint32_t n_actors,
-                      const dvx_octree *const *actors, const float *poses_l2w, const float *box_half,
-                      const dvx_render_opts *opts, dvx_image out, dvx_frame **saved) {
-  if (saved) *saved = nullptr;
-  if (!ctx) return DVX_ERR_INVALID_ARG;
+}  // extern "C"
+
+namespace {
+
+dvx_status render_check_args(dvx_ctx *ctx, const dvx_camera *cam, const dvx_octree *static_tree, uint32_t n_actors,
+                             const dvx_octree *const *actors, const float *poses_l2w, const float *box_half,
+                             const dvx_render_opts &o, const dvx_image &out) {
   if (!cam || !static_tree || !out.rgb || !out.depth || !out.alpha) return fail(ctx, DVX_ERR_INVALID_ARG, "NULL argument");
   if (n_actors > DVX_MAX_ACTORS) return fail(ctx, DVX_ERR_INVALID_ARG, "n_actors > 64");
   if (n_actors && (!actors || !poses_l2w || !box_half)) return fail(ctx, DVX_ERR_INVALID_ARG, "actor arrays are NULL");
-  dvx_render_opts o = {8u, 0u, 1e-4f, 0u, nullptr};
-  if (opts) o = *opts;
   if (o.k_samples < 1 || o.k_samples > 8) return fail(ctx, DVX_ERR_INVALID_ARG, "k_samples must be in [1,8]");
   if (o.activation > 1) return fail(ctx, DVX_ERR_INVALID_ARG, "unknown activation");
   if (!(o.t_stop >= 0.f)) return fail(ctx, DVX_ERR_INVALID_ARG, "t_stop must be >= 0");
@@ -437,9 +454,15 @@ dvx_status dvx_render(dvx_ctx *ctx, const dvx_camera *cam, const dvx_octree *sta
     for (int a = 0; a < 3; ++a)
       if (!(box_half[3 * i + a] >= 0.f)) return fail(ctx, DVX_ERR_INVALID_ARG, "negative box half extent");
   }
-  cudaSetDevice(ctx->device);
-  cudaStream_t st = ctx->st;
+  return DVX_OK;
+}
 
+// Step 1 of one frame enqueued on stream s: frame tables, projection + binning, and the counters copied to `h_cnt` (pinned).
+// *out_f is the new frame (the caller frees it with frame_free on a later failure).
+dvx_status render_step1(dvx_ctx *ctx, const dvx_camera *cam, const dvx_octree *static_tree, uint32_t n_actors,
+                        const dvx_octree *const *actors, const float *poses_l2w, const float *box_half,
+                        const dvx_render_opts &o, const dvx_image &out, bool save, cudaStream_t st,
+                        unsigned long long *h_cnt, dvx_frame **out_f) {
   dvx_frame *f = new dvx_frame();
   CallGuard guard(ctx);
   guard.frame = f;  // freed on every early return below
@@ -479,7 +502,6 @@ dvx_status dvx_render(dvx_ctx *ctx, const dvx_camera *cam, const dvx_octree *sta
   p.v_total = (uint32_t)vtot;
   p.rank_bits = bits_for(vmax);
   p.n_buckets = p.n_tiles * p.n_trees * 8u;
-  const uint32_t key_bits = p.rank_bits + bits_for(p.n_buckets);
   const size_t npix = (size_t)p.width * p.height;
 
   bool ok = buf_alloc(ctx, f->trees_d, sizeof(TreeFrame) * p.n_trees) && buf_alloc(ctx, f->fvox, sizeof(FrameVox) * (size_t)p.v_total) &&
@@ -489,11 +511,11 @@ dvx_status dvx_render(dvx_ctx *ctx, const dvx_camera *cam, const dvx_octree *sta
             buf_alloc(ctx, f->range_end, sizeof(uint32_t) * (size_t)p.n_buckets) &&
             buf_alloc(ctx, f->counters, sizeof(unsigned long long) * CNT_N) &&
             buf_alloc(ctx, f->tile_cost, sizeof(uint32_t) * (size_t)p.n_tiles) && buf_alloc(ctx, f->tile_order, sizeof(uint32_t) * 2 * (size_t)p.n_tiles);
-  if (ok && saved)
+  if (ok && save)
     ok = buf_alloc(ctx, f->sv_rgbd, npix * 16) && buf_alloc(ctx, f->sv_T, npix * 4) && buf_alloc(ctx, f->sv_nused, npix * 4);
   if (ok && out.normal) {
     if (o.flags & DVX_FLAG_NAIVE) return fail(ctx, DVX_ERR_NOT_IMPLEMENTED, "the debug walker has no normal map");
-    ok = buf_alloc(ctx, f->vnrm, sizeof(float4) * (size_t)p.v_total) && (!saved || buf_alloc(ctx, f->sv_nrm, npix * 16));
+    ok = buf_alloc(ctx, f->vnrm, sizeof(float4) * (size_t)p.v_total) && (!save || buf_alloc(ctx, f->sv_nrm, npix * 16));
   }
   if (!ok) return fail(ctx, DVX_ERR_OOM, "dvx_render: allocator returned NULL");
   if (!ctx->ev_free.empty()) {
@@ -521,12 +543,23 @@ dvx_status dvx_render(dvx_ctx *ctx, const dvx_camera *cam, const dvx_octree *sta
   dvx_tile_masks_launch(p, trees_d, (uint8_t *)f->octmask.p, (unsigned long long *)f->actor_mask.p, st);
   dvx_preprocess_launch(p, trees_d, (const uint8_t *)f->octmask.p, (FrameVox *)f->fvox.p, (ushort4 *)f->pxrect.p, (float4 *)f->vnrm.p, counters, st);
   CU(cudaEventRecord(f->ev[1], st));
-  CU(cudaMemcpyAsync(ctx->h_counters, counters, sizeof(unsigned long long) * CNT_N, cudaMemcpyDeviceToHost, st));
-  CU(cudaStreamSynchronize(st));
-  f->n_pairs = ctx->h_counters[CNT_PAIRS];
-  f->v_vis = ctx->h_counters[CNT_VVIS];
+  CU(cudaMemcpyAsync(h_cnt, counters, sizeof(unsigned long long) * CNT_N, cudaMemcpyDeviceToHost, st));
+  f->h_cnt = h_cnt;
+  guard.keep_frame();
+  *out_f = f;
+  return DVX_OK;
+}
+
+// Step 2 on stream s, after the stream that ran step 1 has been synchronised (the pair count sizes the sort buffers).
+dvx_status render_step2(dvx_ctx *ctx, dvx_frame *f, cudaStream_t st) {
+  const FrameParams &p = f->p;
+  f->n_pairs = f->h_cnt[CNT_PAIRS];
+  f->v_vis = f->h_cnt[CNT_VVIS];
   if (f->n_pairs >= (1ull << 30)) return fail(ctx, DVX_ERR_INVALID_ARG, "2^30 or more (tile, octant, voxel) pairs");
-  // ---- step 2
+  const uint32_t key_bits = p.rank_bits + bits_for(p.n_buckets);
+  TreeFrame *trees_d = (TreeFrame *)f->trees_d.p;
+  unsigned long long *counters = (unsigned long long *)f->counters.p;
+  CallGuard guard(ctx);
   const uint64_t P = f->n_pairs;
   uint64_t *ka = (uint64_t *)guard.add(ctx_alloc(ctx, P * 8)), *kb = (uint64_t *)guard.add(ctx_alloc(ctx, P * 8));
   uint32_t *va = (uint32_t *)guard.add(ctx_alloc(ctx, P * 4)), *vb = (uint32_t *)guard.add(ctx_alloc(ctx, P * 4));
@@ -545,10 +578,17 @@ dvx_status dvx_render(dvx_ctx *ctx, const dvx_camera *cam, const dvx_octree *sta
   f->ids.p = which ? vb : va;   // the frame owns the sorted ids from here on; the other buffers go back with the guard
   f->ids.bytes = P * 4;
   guard.drop(f->ids.p);
-  // ---- steps 3 + 4
+  return DVX_OK;
+}
+
+// Steps 3 + 4 on stream s (ordered after step 2 by the caller): the compositing kernel, with hit records for a saved frame.
+dvx_status render_step34(dvx_ctx *ctx, dvx_frame *f, const dvx_image &out, bool save, cudaStream_t st) {
+  const FrameParams &p = f->p;
+  const size_t npix = (size_t)p.width * p.height;
+  unsigned long long *counters = (unsigned long long *)f->counters.p;
   CompositeArgs A;
   memset(&A, 0, sizeof(A));
-  A.p = p; A.trees = trees_d; A.fvox = (const FrameVox *)f->fvox.p; A.pxrect = (const ushort4 *)f->pxrect.p;
+  A.p = p; A.trees = (const TreeFrame *)f->trees_d.p; A.fvox = (const FrameVox *)f->fvox.p; A.pxrect = (const ushort4 *)f->pxrect.p;
   A.ids = (const uint32_t *)f->ids.p; A.range_beg = (const uint32_t *)f->range_beg.p; A.range_end = (const uint32_t *)f->range_end.p;
   A.actor_mask = (const unsigned long long *)f->actor_mask.p;
   A.tile_order = (const uint32_t *)f->tile_order.p;
@@ -564,7 +604,7 @@ dvx_status dvx_render(dvx_ctx *ctx, const dvx_camera *cam, const dvx_octree *sta
   }
   // ---- hit records for the backward (dvx.h): only for saved frames rendered by the tile kernel
   bool rec = false;
-  if (saved && !(p.flags & (DVX_FLAG_NAIVE | DVX_FLAG_NO_RECORDS))) {
+  if (save && !(p.flags & (DVX_FLAG_NAIVE | DVX_FLAG_NO_RECORDS))) {
     rec_collect(ctx);
     const uint64_t cap = rec_capacity(ctx, p);
     if (cap > 0) {
@@ -582,16 +622,119 @@ dvx_status dvx_render(dvx_ctx *ctx, const dvx_camera *cam, const dvx_octree *sta
       }
     }
   }
+  CU(cudaEventRecord(f->ev[9], st));
   dvx_composite_launch(A, false, st);
   CU(cudaEventRecord(f->ev[4], st));
   if (rec && !ctx->rec_budget) {
-    CU(cudaMemcpyAsync(ctx->h_rec, counters + CNT_REC_CHUNKS, sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
-    CU(cudaEventRecord(ctx->ev_rec, st));
-    ctx->rec_pending_npix = (double)npix;
+    const int slot = ctx->rec_slot;   // a slot still pending is simply overwritten (its frame's count is lost, not wrong)
+    ctx->rec_slot = (slot + 1) % dvx_ctx::REC_SLOTS;
+    CU(cudaMemcpyAsync(ctx->h_rec + slot, counters + CNT_REC_CHUNKS, sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
+    CU(cudaEventRecord(ctx->ev_rec[slot], st));
+    ctx->rec_pending_npix[slot] = (double)npix;
   }
   f->es->rendered = true;
   CU(cudaGetLastError());
+  return DVX_OK;
+}
+
+#ifndef DVX_BATCH_OVERLAP
+#define DVX_BATCH_OVERLAP 1  // 0: the batched calls keep everything on the context's stream (only the host round trips are merged)
+#endif
+#ifndef DVX_BATCH_PRIO
+#define DVX_BATCH_PRIO 1     // 1: the second stream has the highest priority, 0: the default one
+#endif
+// Library-owned second stream for the batched entry points, and its pinned counter slots.
+dvx_status batch_setup(dvx_ctx *ctx, uint32_t n) {
+  if (!ctx->ps) {
+    int lo = 0, hi = 0;
+    CU(cudaDeviceGetStreamPriorityRange(&lo, &hi));
+    CU(cudaStreamCreateWithPriority(&ctx->ps, cudaStreamNonBlocking, DVX_BATCH_PRIO ? hi : lo));
+    CU(cudaEventCreateWithFlags(&ctx->ev_entry, cudaEventDisableTiming));
+  }
+  if (ctx->h_batch_n < n) {
+    if (ctx->h_batch) cudaFreeHost(ctx->h_batch);
+    ctx->h_batch = nullptr; ctx->h_batch_n = 0;
+    CU(cudaMallocHost((void **)&ctx->h_batch, (size_t)n * CNT_N * sizeof(unsigned long long)));
+    ctx->h_batch_n = n;
+  }
+  while (ctx->ev_batch.size() < n) {
+    cudaEvent_t e;
+    CU(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+    ctx->ev_batch.push_back(e);
+  }
+  return DVX_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+dvx_status dvx_render(dvx_ctx *ctx, const dvx_camera *cam, const dvx_octree *static_tree, uint32_t n_actors,
+                      const dvx_octree *const *actors, const float *poses_l2w, const float *box_half,
+                      const dvx_render_opts *opts, dvx_image out, dvx_frame **saved) {
+  if (saved) *saved = nullptr;
+  if (!ctx) return DVX_ERR_INVALID_ARG;
+  dvx_render_opts o = {8u, 0u, 1e-4f, 0u, nullptr};
+  if (opts) o = *opts;
+  dvx_status rc = render_check_args(ctx, cam, static_tree, n_actors, actors, poses_l2w, box_half, o, out);
+  if (rc != DVX_OK) return rc;
+  cudaSetDevice(ctx->device);
+  cudaStream_t st = ctx->st;
+  dvx_frame *f = nullptr;
+  rc = render_step1(ctx, cam, static_tree, n_actors, actors, poses_l2w, box_half, o, out, saved != nullptr, st, ctx->h_counters, &f);
+  if (rc != DVX_OK) return rc;
+  CallGuard guard(ctx);
+  guard.frame = f;
+  CU(cudaStreamSynchronize(st));  // the one host round trip of a frame: the pair count sizes the sort buffers
+  rc = render_step2(ctx, f, st);
+  if (rc == DVX_OK) rc = render_step34(ctx, f, out, saved != nullptr, st);
+  if (rc != DVX_OK) return rc;
   if (saved) { *saved = f; guard.keep_frame(); }
+  return DVX_OK;
+}
+
+dvx_status dvx_render_batch(dvx_ctx *ctx, uint32_t n_cams, const dvx_camera *cams, const dvx_octree *static_tree,
+                            uint32_t n_actors, const dvx_octree *const *actors, const float *poses_l2w, const float *box_half,
+                            const dvx_render_opts *opts, const dvx_image *outs, dvx_frame **saved) {
+  if (saved) for (uint32_t c = 0; c < n_cams; ++c) saved[c] = nullptr;
+  if (!ctx) return DVX_ERR_INVALID_ARG;
+  if (n_cams == 0) return DVX_OK;
+  if (!cams || !outs) return fail(ctx, DVX_ERR_INVALID_ARG, "NULL argument");
+  if (n_cams > 1024) return fail(ctx, DVX_ERR_INVALID_ARG, "more than 1024 cameras in one batch");
+  dvx_render_opts o = {8u, 0u, 1e-4f, 0u, nullptr};
+  if (opts) o = *opts;
+  for (uint32_t c = 0; c < n_cams; ++c) {
+    dvx_status rc = render_check_args(ctx, cams + c, static_tree, n_actors, actors, poses_l2w, box_half, o, outs[c]);
+    if (rc != DVX_OK) return rc;
+  }
+  cudaSetDevice(ctx->device);
+  dvx_status rc = batch_setup(ctx, n_cams);
+  if (rc != DVX_OK) return rc;
+  std::vector<dvx_frame *> fr(n_cams, nullptr);
+  struct FreeAll {  // frames not handed to the caller are freed on every exit
+    dvx_ctx *ctx; std::vector<dvx_frame *> &v;
+    ~FreeAll() { for (dvx_frame *f : v) if (f) frame_free(ctx, f); }
+  } free_all{ctx, fr};
+  // the second stream starts after whatever the caller has enqueued on the context's stream (inputs, the previous step)
+  cudaStream_t side = DVX_BATCH_OVERLAP ? ctx->ps : ctx->st;
+  CU(cudaEventRecord(ctx->ev_entry, ctx->st));
+  CU(cudaStreamWaitEvent(side, ctx->ev_entry, 0));
+  for (uint32_t c = 0; c < n_cams; ++c) {
+    rc = render_step1(ctx, cams + c, static_tree, n_actors, actors, poses_l2w, box_half, o, outs[c], saved != nullptr, side,
+                      ctx->h_batch + (size_t)c * CNT_N, &fr[c]);
+    if (rc != DVX_OK) { cudaStreamSynchronize(side); return rc; }
+  }
+  cudaError_t e = cudaStreamSynchronize(side);  // ONE host round trip for the pair counts of all cameras
+  if (e != cudaSuccess) return cuda_fail(ctx, e, "dvx_render_batch");
+  for (uint32_t c = 0; c < n_cams; ++c) {
+    // camera c's key generation + sort run on the second stream, under camera c-1's compositing on the context's stream
+    rc = render_step2(ctx, fr[c], side);
+    if (rc == DVX_OK && cudaEventRecord(ctx->ev_batch[c], side) != cudaSuccess) rc = fail(ctx, DVX_ERR_CUDA, "cudaEventRecord failed");
+    if (rc == DVX_OK && cudaStreamWaitEvent(ctx->st, ctx->ev_batch[c], 0) != cudaSuccess) rc = fail(ctx, DVX_ERR_CUDA, "cudaStreamWaitEvent failed");
+    if (rc == DVX_OK) rc = render_step34(ctx, fr[c], outs[c], saved != nullptr, ctx->st);
+    if (rc != DVX_OK) { cudaStreamSynchronize(side); cudaStreamSynchronize(ctx->st); return rc; }
+  }
+  if (saved) for (uint32_t c = 0; c < n_cams; ++c) { saved[c] = fr[c]; fr[c] = nullptr; }
   return DVX_OK;
 }
 
@@ -600,28 +743,33 @@ dvx_status dvx_backward(dvx_ctx *ctx, dvx_frame *f, const float *dL_drgb, const 
   return dvx_backward_n(ctx, f, dL_drgb, dL_ddepth, dL_dalpha, nullptr, static_grad, actor_grads);
 }
 
-dvx_status dvx_backward_n(dvx_ctx *ctx, dvx_frame *f, const float *dL_drgb, const float *dL_ddepth, const float *dL_dalpha,
-                          const float *dL_dnormal, dvx_grad static_grad, const dvx_grad *actor_grads) {
-  if (!ctx) return DVX_ERR_INVALID_ARG;
+}  // extern "C"
+
+namespace {
+
+// Step 5 of one frame.  The replay (or list walk) runs on the context's stream; the per-voxel SH post-pass runs on `post`
+// (the context's stream itself, or the second stream behind an event).  `hold` receives the scratch that must stay alive
+// until the post-pass has been joined (the caller releases it).
+dvx_status backward_core(dvx_ctx *ctx, dvx_frame *f, const float *dL_drgb, const float *dL_ddepth, const float *dL_dalpha,
+                         const float *dL_dnormal, dvx_grad static_grad, const dvx_grad *actor_grads, cudaStream_t post,
+                         cudaEvent_t ev_post, CallGuard &hold) {
   if (!f || !dL_drgb) return fail(ctx, DVX_ERR_INVALID_ARG, "NULL argument");
   if (!f->sv_rgbd.p) return fail(ctx, DVX_ERR_INVALID_ARG, "frame holds no saved state");
   if (dL_dnormal && !f->sv_nrm.p) return fail(ctx, DVX_ERR_INVALID_ARG, "the frame was rendered without a normal map");
   const FrameParams &p = f->p;
   if (p.n_trees > 1 && !actor_grads) return fail(ctx, DVX_ERR_INVALID_ARG, "actor_grads is NULL");
-  cudaSetDevice(ctx->device);
   cudaStream_t st = ctx->st;
+  for (uint32_t t = 0; t < p.n_trees; ++t) {  // red.global.add.v4.f32 and the float4 read-modify-writes need 16-byte alignment
+    const dvx_grad g = t == 0 ? static_grad : actor_grads[t - 1];
+    if (((uintptr_t)g.dgeo | (uintptr_t)g.dsh) & 15) return fail(ctx, DVX_ERR_INVALID_ARG, "gradient buffers must be 16-byte aligned");
+  }
   for (uint32_t t = 0; t < p.n_trees; ++t) {
     const dvx_grad g = t == 0 ? static_grad : actor_grads[t - 1];
     f->trees_h[t].dgeo = g.dgeo;
     f->trees_h[t].dsh = g.dsh;
   }
-  for (uint32_t t = 0; t < p.n_trees; ++t) {  // red.global.add.v4.f32 and the float4 read-modify-writes need 16-byte alignment
-    const dvx_grad g = t == 0 ? static_grad : actor_grads[t - 1];
-    if (((uintptr_t)g.dgeo | (uintptr_t)g.dsh) & 15) return fail(ctx, DVX_ERR_INVALID_ARG, "gradient buffers must be 16-byte aligned");
-  }
-  CallGuard guard(ctx);
-  float *drgb = (float *)guard.add(ctx_alloc(ctx, (size_t)p.v_total * 16));
-  float *dnrm = dL_dnormal ? (float *)guard.add(ctx_alloc(ctx, (size_t)p.v_total * 16)) : nullptr;
+  float *drgb = (float *)hold.add(ctx_alloc(ctx, (size_t)p.v_total * 16));
+  float *dnrm = dL_dnormal ? (float *)hold.add(ctx_alloc(ctx, (size_t)p.v_total * 16)) : nullptr;
   if (!drgb || (dL_dnormal && !dnrm)) return fail(ctx, DVX_ERR_OOM, "dvx_backward: allocator returned NULL");
   TreeFrame *trees_d = (TreeFrame *)f->trees_d.p;
   // box_rect was filled on the device; only the gradient pointers change, so patch those fields
@@ -650,12 +798,58 @@ dvx_status dvx_backward_n(dvx_ctx *ctx, dvx_frame *f, const float *dL_drgb, cons
   }
   dvx_composite_launch(A, true, st);
   CU(cudaEventRecord(f->ev[8], st));
-  dvx_sh_backward_launch(p, trees_d, A.fvox, A.pxrect, drgb, st);
-  if (dnrm) dvx_normal_backward_launch(p, trees_d, A.pxrect, dnrm, st);
-  CU(cudaEventRecord(f->ev[6], st));
+  if (post != st) {  // the post-pass of this frame runs beside the next frame's replay
+    CU(cudaEventRecord(ev_post, st));
+    CU(cudaStreamWaitEvent(post, ev_post, 0));
+  }
+  dvx_sh_backward_launch(p, trees_d, A.fvox, A.pxrect, drgb, post);
+  if (dnrm) dvx_normal_backward_launch(p, trees_d, A.pxrect, dnrm, post);
+  CU(cudaEventRecord(f->ev[6], post));
   CU(cudaGetLastError());
   f->did_backward = true;
   return DVX_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+dvx_status dvx_backward_n(dvx_ctx *ctx, dvx_frame *f, const float *dL_drgb, const float *dL_ddepth, const float *dL_dalpha,
+                          const float *dL_dnormal, dvx_grad static_grad, const dvx_grad *actor_grads) {
+  if (!ctx) return DVX_ERR_INVALID_ARG;
+  cudaSetDevice(ctx->device);
+  CallGuard hold(ctx);  // stream-ordered reuse: the scratch goes back to the cache as soon as the work is enqueued
+  return backward_core(ctx, f, dL_drgb, dL_ddepth, dL_dalpha, dL_dnormal, static_grad, actor_grads, ctx->st, nullptr, hold);
+}
+
+dvx_status dvx_backward_batch(dvx_ctx *ctx, uint32_t n_frames, dvx_frame *const *frames, const float *const *dL_drgb,
+                              const float *const *dL_ddepth, const float *const *dL_dalpha, dvx_grad static_grad,
+                              const dvx_grad *actor_grads) {
+  if (!ctx) return DVX_ERR_INVALID_ARG;
+  if (n_frames == 0) return DVX_OK;
+  if (!frames || !dL_drgb) return fail(ctx, DVX_ERR_INVALID_ARG, "NULL argument");
+  if (n_frames > 1024) return fail(ctx, DVX_ERR_INVALID_ARG, "more than 1024 frames in one batch");
+  cudaSetDevice(ctx->device);
+  dvx_status rc = batch_setup(ctx, n_frames);
+  if (rc != DVX_OK) return rc;
+  // every frame's dL/drgb_v scratch stays allocated until the second stream has been joined below: a block handed back
+  // earlier could be given to the next frame's replay while this frame's post-pass still reads it
+  CallGuard hold(ctx);
+  cudaStream_t side = DVX_BATCH_OVERLAP ? ctx->ps : ctx->st;
+  CU(cudaEventRecord(ctx->ev_entry, ctx->st));
+  CU(cudaStreamWaitEvent(side, ctx->ev_entry, 0));
+  for (uint32_t c = 0; c < n_frames && rc == DVX_OK; ++c) {
+    // frames of one batch accumulate into the same dsh: their post-passes are ordered on the second stream; dgeo only
+    // receives reductions from the replays (a frame with a normal map would read-modify-write dgeo: not batched)
+    if (frames[c] && frames[c]->sv_nrm.p) rc = fail(ctx, DVX_ERR_NOT_IMPLEMENTED, "dvx_backward_batch: frames with a normal map go through dvx_backward_n");
+    else rc = backward_core(ctx, frames[c], dL_drgb[c], dL_ddepth ? dL_ddepth[c] : nullptr, dL_dalpha ? dL_dalpha[c] : nullptr,
+                            nullptr, static_grad, actor_grads, side, ctx->ev_batch[c], hold);
+  }
+  // join: whatever follows on the context's stream sees the gradients of every frame
+  cudaError_t e = cudaEventRecord(ctx->ev_entry, side);
+  if (e == cudaSuccess) e = cudaStreamWaitEvent(ctx->st, ctx->ev_entry, 0);
+  if (e != cudaSuccess && rc == DVX_OK) rc = cuda_fail(ctx, e, "dvx_backward_batch");
+  return rc;
 }
 
 void dvx_frame_release(dvx_ctx *ctx, dvx_frame *frame) {
@@ -742,7 +936,7 @@ dvx_status dvx_frame_stage_ms(dvx_ctx *ctx, const dvx_frame *f, float *ms) {
   for (int i = 0; i < 8; ++i) ms[i] = 0.f;
   CU(cudaEventElapsedTime(&ms[0], f->ev[0], f->ev[1]));
   CU(cudaEventElapsedTime(&ms[1], f->ev[2], f->ev[3]));
-  CU(cudaEventElapsedTime(&ms[2], f->ev[3], f->ev[4]));
+  CU(cudaEventElapsedTime(&ms[2], f->ev[9], f->ev[4]));
   if (f->did_backward) {
     CU(cudaEventElapsedTime(&ms[3], f->ev[5], f->ev[6]));
     CU(cudaEventElapsedTime(&ms[4], f->ev[7], f->ev[8]));
@@ -758,7 +952,7 @@ dvx_status dvx_stage_ms_collect(dvx_ctx *ctx, float *ms, uint32_t *n_frames) {
   CU(cudaStreamSynchronize(ctx->st));
   for (int i = 0; i < 8; ++i) ms[i] = 0.f;
   *n_frames = (uint32_t)ctx->ev_pending.size();
-  static const int pairs[6][2] = {{0, 1}, {2, 3}, {3, 4}, {5, 6}, {7, 8}, {8, 6}};
+  static const int pairs[6][2] = {{0, 1}, {2, 3}, {9, 4}, {5, 6}, {7, 8}, {8, 6}};
   for (EventSet *es : ctx->ev_pending) {
     for (int i = 0; i < 6; ++i) {
       if (i >= 3 && !es->did_backward) break;
@@ -769,6 +963,35 @@ dvx_status dvx_stage_ms_collect(dvx_ctx *ctx, float *ms, uint32_t *n_frames) {
     ctx->ev_free.push_back(es);
   }
   ctx->ev_pending.clear();
+  return DVX_OK;
+}
+
+dvx_status dvx_microbench_fma(dvx_ctx *ctx, uint32_t iters, double *lane_fma_per_s, double *warp_instr_per_s, float *ms_out) {
+  if (!ctx) return DVX_ERR_INVALID_ARG;
+  if (iters == 0 || iters > (1u << 24)) return fail(ctx, DVX_ERR_INVALID_ARG, "dvx_microbench_fma: iters must be in [1, 2^24]");
+  cudaSetDevice(ctx->device);
+  int sms = 0;
+  CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, ctx->device));
+  const uint32_t threads = dvx_microbench_threads(), blocks = (uint32_t)sms * (2048u / threads);  // every warp slot of every SM
+  CallGuard guard(ctx);
+  float *out = (float *)guard.add(ctx_alloc(ctx, (size_t)blocks * threads * sizeof(float)));
+  if (!out) return fail(ctx, DVX_ERR_OOM, "dvx_microbench_fma: allocator returned NULL");
+  cudaEvent_t e0, e1;
+  CU(cudaEventCreate(&e0));
+  if (cudaEventCreate(&e1) != cudaSuccess) { cudaEventDestroy(e0); return fail(ctx, DVX_ERR_CUDA, "cudaEventCreate failed"); }
+  dvx_microbench_fma_launch(out, blocks, iters > 64 ? 64 : iters, ctx->st);  // warm-up (clocks, instruction cache)
+  cudaEventRecord(e0, ctx->st);
+  const uint64_t per_thread = dvx_microbench_fma_launch(out, blocks, iters, ctx->st);
+  cudaEventRecord(e1, ctx->st);
+  cudaError_t e = cudaEventSynchronize(e1);
+  float ms = 0.f;
+  if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, e0, e1);
+  cudaEventDestroy(e0); cudaEventDestroy(e1);
+  if (e != cudaSuccess) return cuda_fail(ctx, e, "dvx_microbench_fma");
+  const double lanes = (double)per_thread * blocks * threads;
+  if (lane_fma_per_s) *lane_fma_per_s = lanes / ((double)ms * 1e-3);
+  if (warp_instr_per_s) *warp_instr_per_s = lanes / 32.0 / ((double)ms * 1e-3);
+  if (ms_out) *ms_out = ms;
   return DVX_OK;
 }
 

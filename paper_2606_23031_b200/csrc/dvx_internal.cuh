@@ -194,6 +194,10 @@ void dvx_prune_flags_launch(const float *geo, uint32_t n_voxels, float threshold
 void dvx_prune_scatter_launch(const uint64_t *code, uint32_t n_voxels, const uint32_t *offsets, uint64_t *code_out,
                               uint32_t *index_out, cudaStream_t st);
 
+// ---- dvx_microbench.cu
+uint64_t dvx_microbench_fma_launch(float *out, uint32_t blocks, uint32_t iters, cudaStream_t st);
+uint32_t dvx_microbench_threads(void);
+
 // ---- dvx_features.cu (row N3).  img == NULL: render (feat, out);  img != NULL: fuse (img, num, wsum)
 void dvx_features_launch(uint32_t width, uint32_t height, uint32_t n_channels, const uint32_t *row_start, const uint32_t *voxel,
                          const float *weight, const float *feat, float *out, const float *img, float *num, float *wsum,
