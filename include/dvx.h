@@ -332,6 +332,16 @@ dvx_status dvx_density_prior(dvx_ctx *ctx, const dvx_cloud *cloud, const dvx_oct
  * bytes (1 = was subdivided) or NULL.  Synchronises the stream. */
 dvx_status dvx_subdivide_near(dvx_ctx *ctx, const dvx_cloud *cloud, const dvx_octree_desc *desc, float threshold,
                               uint32_t max_level, uint64_t *code_out, uint64_t capacity, uint64_t *n_out, uint8_t *split);
+/* Parameters of the leaves a subdivision round produced (reading R29; the paper only says the structure "is only modified
+ * during an adaptive pruning and progressive subdivision", following SVRaster): in dvx_subdivide_near's output
+ * order, a kept leaf keeps its 8 corner densities and its SH coefficients; child o = 4 ox + 2 oy + oz of a split leaf gets,
+ * at its corner c = 4 bx + 2 by + bz, the parent's trilinear raw density at u = (o + b) / 2 - the continuous density field
+ * is unchanged by the split - and a copy of the parent's SH coefficients.  split DEVICE [V] as written by
+ * dvx_subdivide_near; geo_in DEVICE [V][8], sh_in DEVICE [V][C_sh][3] or NULL; geo_out DEVICE [capacity][8], sh_out DEVICE
+ * [capacity][C_sh][3] or NULL (sh_in and sh_out go together); *n_out HOST = leaves after the round (capacity must be at
+ * least that; 8 V always suffices).  geo arrays 32-byte aligned.  Synchronises the stream. */
+dvx_status dvx_subdivide_fill(dvx_ctx *ctx, uint32_t n_voxels, const uint8_t *split, const float *geo_in, const float *sh_in,
+                              uint32_t sh_degree, float *geo_out, float *sh_out, uint64_t capacity, uint64_t *n_out);
 /* Pruning: keeps the leaves whose largest raw corner density is >= threshold, in order.  code DEVICE [V], geo DEVICE
  * [V][8] (32-byte aligned); code_out DEVICE [V]; index_out DEVICE [V] (the kept leaves' old indices, for gathering geo and
  * sh) or NULL; *n_out HOST.  Synchronises the stream. */

@@ -124,3 +124,33 @@ def prune(code, geo, threshold):
     geo = np.asarray(geo, dtype=np.float64).reshape(-1, 8)
     keep = np.nonzero(geo.max(axis=1) >= threshold)[0]
     return np.asarray(code, dtype=np.uint64)[keep], keep.astype(np.uint32)
+
+
+def subdivide_fill(split, geo, sh):
+    """Parameters of the leaves after one subdivision round (reading R29): a kept leaf keeps its corner densities and SH
+    coefficients; child o = 4 ox + 2 oy + oz of a split leaf occupies the half-cube [o_a / 2, (o_a + 1) / 2] of its parent
+    along every axis, and its corner c = 4 bx + 2 by + bz takes the parent's trilinear raw density at u = (o + b) / 2, so the
+    continuous density field ('raw volume densities at its eight corners', trilinear inside) is unchanged by
+    the split; the SH coefficients are copied.  Output order = subdivide_near's.  float64."""
+    split = np.asarray(split).astype(bool)
+    geo = np.asarray(geo, dtype=np.float64).reshape(split.shape[0], 8)
+    sh = np.asarray(sh, dtype=np.float64)
+    out_geo, out_sh = [], []
+    for v in range(split.shape[0]):
+        if not split[v]:
+            out_geo.append(geo[v]); out_sh.append(sh[v])
+            continue
+        for o in range(8):
+            child = np.zeros(8)
+            for c in range(8):
+                u = [(((o >> (2 - a)) & 1) + ((c >> (2 - a)) & 1)) / 2.0 for a in range(3)]
+                val = 0.0
+                for pc in range(8):   # the parent's trilinear interpolant, corner pc = 4 bx + 2 by + bz (R7)
+                    w = 1.0
+                    for a in range(3):
+                        w *= u[a] if (pc >> (2 - a)) & 1 else 1.0 - u[a]
+                    val += w * geo[v, pc]
+                child[c] = val
+            out_geo.append(child); out_sh.append(sh[v])
+    n = len(out_geo)
+    return np.array(out_geo).reshape(n, 8), np.array(out_sh).reshape((n,) + sh.shape[1:])

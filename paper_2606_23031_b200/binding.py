@@ -27,7 +27,7 @@ EXPORTS = ["dvx_create", "dvx_destroy", "dvx_octree_create", "dvx_octree_refresh
            "dvx_grid_adam_step", "dvx_adam_step", "dvx_grid_adam_step_n", "dvx_adam_step_n",
            "dvx_frame_weights", "dvx_render_features", "dvx_fuse_features",
            "dvx_cloud_create", "dvx_cloud_destroy", "dvx_density_prior", "dvx_subdivide_near", "dvx_prune",
-           "dvx_set_record_budget", "dvx_frame_record_stats", "dvx_trim", "dvx_microbench_fma", "dvx_render_batch", "dvx_backward_batch"]
+           "dvx_set_record_budget", "dvx_frame_record_stats", "dvx_trim", "dvx_microbench_fma", "dvx_render_batch", "dvx_backward_batch", "dvx_subdivide_fill"]
 
 
 class DvxError(RuntimeError):
@@ -143,6 +143,7 @@ def load():
     lib.dvx_render_batch.argtypes = [P, C.c_uint32, C.POINTER(Camera), P, C.c_uint32, C.POINTER(P), P, P, C.POINTER(RenderOpts),
                                      C.POINTER(Image), C.POINTER(P)]
     lib.dvx_backward_batch.argtypes = [P, C.c_uint32, C.POINTER(P), C.POINTER(P), C.POINTER(P), C.POINTER(P), Grad, C.POINTER(Grad)]
+    lib.dvx_subdivide_fill.argtypes = [P, C.c_uint32, P, P, P, C.c_uint32, P, P, C.c_uint64, C.POINTER(C.c_uint64)]
     lib.dvx_trim.argtypes = [P, C.POINTER(C.c_uint64)]
     lib.dvx_microbench_fma.argtypes = [P, C.c_uint32, C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_float)]
     lib.dvx_set_record_budget.argtypes = [P, C.c_uint64]
@@ -274,6 +275,18 @@ class Context:
         self.check(self.lib.dvx_subdivide_near(self.h, cloud.h, C.byref(desc), threshold, max_level, out.data_ptr(), 8 * n,
                                                C.byref(n_out), split.data_ptr()))
         return out[:n_out.value], split
+
+    def subdivide_fill(self, split, geo, sh, sh_degree, n_out):
+        """dvx_subdivide_fill -> (geo [n_out, 8], sh [n_out, C_sh, 3]) of the leaves after the round (n_out from subdivide_near)."""
+        torch = self.torch
+        n = int(split.shape[0])
+        geo_out = torch.empty((n_out, 8), dtype=torch.float32, device=self.device)
+        sh_out = torch.empty((n_out,) + tuple(sh.shape[1:]), dtype=torch.float32, device=self.device)
+        got = C.c_uint64()
+        self.check(self.lib.dvx_subdivide_fill(self.h, n, split.data_ptr(), geo.data_ptr(), sh.data_ptr(), sh_degree,
+                                               geo_out.data_ptr(), sh_out.data_ptr(), n_out, C.byref(got)))
+        assert got.value == n_out
+        return geo_out, sh_out
 
     def prune(self, code, geo, threshold):
         """dvx_prune -> (kept codes int64 [V'], kept indices int32 [V'])."""

@@ -1491,6 +1491,38 @@ dvx_status dvx_subdivide_near(dvx_ctx *ctx, const dvx_cloud *cloud, const dvx_oc
   return rc;
 }
 
+dvx_status dvx_subdivide_fill(dvx_ctx *ctx, uint32_t n_voxels, const uint8_t *split, const float *geo_in, const float *sh_in,
+                              uint32_t sh_degree, float *geo_out, float *sh_out, uint64_t capacity, uint64_t *n_out) {
+  if (!ctx) return DVX_ERR_INVALID_ARG;
+  if (n_out) *n_out = 0;
+  if (n_voxels == 0) return DVX_OK;
+  if (!split || !geo_in || !geo_out) return fail(ctx, DVX_ERR_INVALID_ARG, "dvx_subdivide_fill: NULL argument");
+  if ((sh_in == nullptr) != (sh_out == nullptr)) return fail(ctx, DVX_ERR_INVALID_ARG, "dvx_subdivide_fill: sh_in and sh_out go together");
+  if (sh_degree > 3) return fail(ctx, DVX_ERR_INVALID_ARG, "sh_degree > 3");
+  if (n_voxels >= (1u << 28)) return fail(ctx, DVX_ERR_INVALID_ARG, "dvx_subdivide_fill: V must be below 2^28");
+  if (((uintptr_t)geo_in | (uintptr_t)geo_out) & 31) return fail(ctx, DVX_ERR_INVALID_ARG, "dvx_subdivide_fill: geo arrays must be 32-byte aligned");
+  cudaSetDevice(ctx->device);
+  cudaStream_t st = ctx->st;
+  const uint32_t V = n_voxels;
+  CallGuard guard(ctx);
+  uint32_t *cnt = (uint32_t *)guard.add(ctx_alloc(ctx, ((size_t)V + 1) * 4));
+  void *scr = guard.add(ctx_alloc(ctx, dvx_sort_scratch_bytes((uint64_t)V + 1)));
+  if (!cnt || !scr) return fail(ctx, DVX_ERR_OOM, "dvx_subdivide_fill: allocator returned NULL");
+  CU(cudaMemsetAsync(cnt + V, 0, 4, st));
+  dvx_split_counts_launch(split, V, cnt, st);
+  dvx_scan_u32_launch(cnt, (uint64_t)V + 1, (uint32_t *)scr, st);
+  uint32_t total = 0;
+  CU(cudaMemcpyAsync(&total, cnt + V, 4, cudaMemcpyDeviceToHost, st));
+  CU(cudaStreamSynchronize(st));
+  if (n_out) *n_out = total;
+  if (capacity < total) return fail(ctx, DVX_ERR_INVALID_ARG, "dvx_subdivide_fill: capacity is smaller than the number of leaves after the round");
+  const uint32_t n_sh = (sh_degree + 1) * (sh_degree + 1);
+  dvx_subdivide_fill_launch(cnt, V, geo_in, sh_in, 3 * n_sh, geo_out, sh_out, st);
+  CU(cudaGetLastError());
+  CU(cudaStreamSynchronize(st));  // cnt goes back to the cache with the guard
+  return DVX_OK;
+}
+
 dvx_status dvx_prune(dvx_ctx *ctx, uint32_t n_voxels, const uint64_t *code, const float *geo, float threshold,
                      uint64_t *code_out, uint32_t *index_out, uint32_t *n_out) {
   if (!ctx) return DVX_ERR_INVALID_ARG;

@@ -190,6 +190,9 @@ void dvx_density_prior_launch(const DvxCloudData &d, const uint64_t *code, const
 void dvx_near_flags_launch(const DvxCloudData &d, const uint64_t *code, uint32_t n_voxels, const double center[3], double side,
                            double threshold, uint32_t max_level, uint32_t *count, uint8_t *split, cudaStream_t st);
 void dvx_expand_launch(const uint64_t *code, uint32_t n_voxels, const uint32_t *offsets, uint64_t *out, cudaStream_t st);
+void dvx_split_counts_launch(const uint8_t *split, uint32_t n_voxels, uint32_t *count, cudaStream_t st);
+void dvx_subdivide_fill_launch(const uint32_t *offsets, uint32_t n_voxels, const float *geo_in, const float *sh_in, uint32_t sh_floats,
+                               float *geo_out, float *sh_out, cudaStream_t st);
 void dvx_prune_flags_launch(const float *geo, uint32_t n_voxels, float threshold, uint32_t *keep, cudaStream_t st);
 void dvx_prune_scatter_launch(const uint64_t *code, uint32_t n_voxels, const uint32_t *offsets, uint64_t *code_out,
                               uint32_t *index_out, cudaStream_t st);

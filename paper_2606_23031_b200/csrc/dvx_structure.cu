@@ -274,6 +274,54 @@ __global__ void __launch_bounds__(ST_THREADS) expand_kernel(const uint64_t *__re
   for (uint64_t o = 0; o < 8; ++o) out[at + o] = ((level + 1ull) << 48) | path | (o << shift);
 }
 
+// R29: parameters of the leaves after a subdivision round.  count[v] = 8 or 1 from the split flags; offsets = their
+// exclusive scan; thread = input leaf.  A child's corner c of octant o samples the parent's trilinear raw density at
+// u = (o + b) / 2 (each u_a in {0, 1/2, 1}), evaluated in fp64 from the fp32 corners and rounded once; SH rows are copied.
+__global__ void __launch_bounds__(ST_THREADS) split_counts_kernel(const uint8_t *__restrict__ split, uint32_t n_voxels,
+                                                                  uint32_t *__restrict__ count) {
+  const uint32_t v = blockIdx.x * ST_THREADS + threadIdx.x;
+  if (v < n_voxels) count[v] = split[v] ? 8u : 1u;
+}
+__global__ void __launch_bounds__(ST_THREADS) subdivide_fill_kernel(const uint32_t *__restrict__ offsets, uint32_t n_voxels,
+                                                                    const float *__restrict__ geo_in, const float *__restrict__ sh_in,
+                                                                    uint32_t sh_floats, float *__restrict__ geo_out,
+                                                                    float *__restrict__ sh_out) {
+  const uint32_t v = blockIdx.x * ST_THREADS + threadIdx.x;
+  if (v >= n_voxels) return;
+  const uint32_t at = offsets[v], cnt = offsets[v + 1] - at;
+  const float4 a = __ldg(reinterpret_cast<const float4 *>(geo_in) + 2 * (size_t)v);
+  const float4 b = __ldg(reinterpret_cast<const float4 *>(geo_in) + 2 * (size_t)v + 1);
+  const double g[8] = {a.x, a.y, a.z, a.w, b.x, b.y, b.z, b.w};
+  const float *sh_src = sh_in ? sh_in + (size_t)v * sh_floats : nullptr;
+  for (uint32_t o = 0; o < cnt; ++o) {
+    float outv[8];
+    if (cnt == 1) {
+#pragma unroll
+      for (int c = 0; c < 8; ++c) outv[c] = (float)g[c];
+    } else {
+#pragma unroll
+      for (int c = 0; c < 8; ++c) {
+        const double ux = 0.5 * (double)(((o >> 2) & 1u) + ((c >> 2) & 1)), uy = 0.5 * (double)(((o >> 1) & 1u) + ((c >> 1) & 1)),
+                     uz = 0.5 * (double)((o & 1u) + (c & 1));
+        double val = 0.0;
+#pragma unroll
+        for (int pc = 0; pc < 8; ++pc) {
+          const double w = ((pc & 4) ? ux : 1.0 - ux) * ((pc & 2) ? uy : 1.0 - uy) * ((pc & 1) ? uz : 1.0 - uz);
+          val += w * g[pc];
+        }
+        outv[c] = (float)val;
+      }
+    }
+    float4 *go = reinterpret_cast<float4 *>(geo_out) + 2 * (size_t)(at + o);
+    go[0] = make_float4(outv[0], outv[1], outv[2], outv[3]);
+    go[1] = make_float4(outv[4], outv[5], outv[6], outv[7]);
+    if (sh_src && sh_out) {
+      float *so = sh_out + (size_t)(at + o) * sh_floats;
+      for (uint32_t i = 0; i < sh_floats; ++i) so[i] = __ldg(sh_src + i);
+    }
+  }
+}
+
 // R28: keep = max corner >= threshold
 __global__ void __launch_bounds__(ST_THREADS) prune_flags_kernel(const float *__restrict__ geo, uint32_t n_voxels, float threshold,
                                                                  uint32_t *__restrict__ keep) {
@@ -352,4 +400,15 @@ void dvx_prune_scatter_launch(const uint64_t *code, uint32_t n_voxels, const uin
                               uint32_t *index_out, cudaStream_t st) {
   DVX_COUNT_LAUNCH(1);
   prune_scatter_kernel<<<st_blocks(n_voxels), ST_THREADS, 0, st>>>(code, n_voxels, offsets, code_out, index_out);
+}
+
+void dvx_split_counts_launch(const uint8_t *split, uint32_t n_voxels, uint32_t *count, cudaStream_t st) {
+  if (n_voxels) { DVX_COUNT_LAUNCH(1); split_counts_kernel<<<(n_voxels + ST_THREADS - 1) / ST_THREADS, ST_THREADS, 0, st>>>(split, n_voxels, count); }
+}
+void dvx_subdivide_fill_launch(const uint32_t *offsets, uint32_t n_voxels, const float *geo_in, const float *sh_in, uint32_t sh_floats,
+                               float *geo_out, float *sh_out, cudaStream_t st) {
+  if (n_voxels) {
+    DVX_COUNT_LAUNCH(1);
+    subdivide_fill_kernel<<<(n_voxels + ST_THREADS - 1) / ST_THREADS, ST_THREADS, 0, st>>>(offsets, n_voxels, geo_in, sh_in, sh_floats, geo_out, sh_out);
+  }
 }

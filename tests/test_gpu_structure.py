@@ -218,3 +218,36 @@ def test_subdivide_near_beyond_2_27_leaves(ctx):
     cloud.close()
     del code, split, idx
     ctx.trim()
+
+
+def test_subdivide_fill_matches_the_oracle_and_keeps_the_image(ctx):
+    """dvx_subdivide_fill (R29) against oracle/structure.py on config 1's static octree after a proximity round: corner
+    densities bit for bit (sums of at most 8 fp32 values with power-of-two weights are exact in fp64 on both sides), SH
+    copied; and the refined octree renders the image of the original one up to the quadrature (finer voxels, more samples)."""
+    import torch
+    import paper_2606_23031_b200 as dvx
+    sc = S.make_config(1)
+    tree = sc.static
+    side = float(tree.side)
+    pts = _surface_points(tree, 400, 23, 0.3)
+    cloud = ctx.cloud(_dev_pts(pts), 1.0)
+    code = _dev_code(tree.code)
+    new, split = ctx.subdivide_near(cloud, code, tree.center, side, 0.5, 7)
+    torch.cuda.synchronize()
+    geo, sh = torch.from_numpy(tree.geo).cuda(), torch.from_numpy(tree.sh).cuda()
+    g2, s2 = ctx.subdivide_fill(split, geo, sh, tree.sh_degree, int(new.shape[0]))
+    torch.cuda.synchronize()
+    rg, rs = T.subdivide_fill(split.cpu().numpy(), tree.geo, tree.sh)
+    assert 0.05 < float(split.float().mean()) < 0.95
+    assert np.array_equal(g2.cpu().numpy(), rg.astype(np.float32)) and np.array_equal(s2.cpu().numpy(), rs.astype(np.float32))
+    # render both octrees (static only) with the library: same field, finer quadrature
+    old = ctx.octree(code, geo, sh, tree.center, side, tree.sh_degree)
+    ref = ctx.octree(new.contiguous(), g2, s2, tree.center, side, tree.sh_degree)
+    cam = dvx.camera_from(sc.cameras[0])
+    a = ctx.render(cam, old, save=False)
+    b = ctx.render(cam, ref, save=False)
+    torch.cuda.synchronize()
+    assert float(a[2].max()) > 0.5
+    assert float((a[2] - b[2]).abs().max()) < 3e-2 and float((a[0] - b[0]).abs().max()) < 3e-2
+    assert float((a[2] - b[2]).abs().mean()) < 2e-3
+    old.close(); ref.close(); cloud.close()

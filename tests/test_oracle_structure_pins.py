@@ -121,3 +121,46 @@ def test_p31_prune():
     assert idx.tolist() == [1, 4] and kept.tolist() == code[[1, 4]].tolist()
     kept, idx = T.prune(code, geo, -20.0)
     assert idx.tolist() == list(range(6))
+
+
+# ---------------------------------------------------------------- P35 parameters of new children (reading R29)
+def test_p35_subdivide_fill_is_the_parents_trilinear_field():
+    """R29: a child's corners sample the parent's trilinear density, so (a) the child corner that coincides with a parent
+    corner keeps its value, an edge midpoint is the mean of 2 parent corners, a face centre of 4, the cube centre of 8
+    (written out by hand); (b) the continuous field is unchanged: rendering the parent and rendering its 8 children agree
+    up to the quadrature, whose error falls 4 x when K doubles (P2) and vanishes for large K - and exactly for a density
+    that is linear along the ray, where the midpoint rule on a half segment ... is NOT exact either, so only convergence is
+    asserted; (c) a constant voxel splits into constant children (P8's case) bit for bit; (d) SH rows are copied."""
+    import math
+    import dvx_scenes as S
+    from oracle import oracle as O
+    from helpers import tree_from_cells, scene, axis_camera
+    rs = np.random.RandomState(4)
+    geo = rs.normal(-0.5, 1.0, size=(2, 8))
+    sh = rs.normal(size=(2, 4, 3))
+    g2, s2 = T.subdivide_fill([True, False], geo, sh)
+    assert g2.shape == (9, 8) and s2.shape == (9, 4, 3)
+    assert np.array_equal(g2[8], geo[1]) and np.array_equal(s2[8], sh[1])          # the kept leaf, last in order
+    assert all(np.array_equal(s2[o], sh[0]) for o in range(8))                       # SH copied
+    p = geo[0]
+    for o in range(8):
+        assert g2[o, o] == p[o]                                                      # the shared corner
+        assert abs(g2[o, 7 - o] - p.mean()) < 1e-15                                  # the parent's centre
+    # child 0 = (0,0,0): its corner 4 (bx=1) is the midpoint of the parent's edge 0-4, corner 6 (bx=by=1) the centre of the
+    # face bz=0 (parent corners 0, 2, 4, 6), corner 1 (bz=1) the midpoint of edge 0-1
+    assert abs(g2[0, 4] - 0.5 * (p[0] + p[4])) < 1e-15 and abs(g2[0, 1] - 0.5 * (p[0] + p[1])) < 1e-15
+    assert abs(g2[0, 6] - 0.25 * (p[0] + p[2] + p[4] + p[6])) < 1e-15
+    # child 5 = (1,0,1): its corner 2 (by=1) sits at u = (1/2, 1/2, 1/2)+... -> u = (0.5, 0.5, 0.5)? no: o=(1,0,1), b=(0,1,0) -> u=(.5,.5,.5)
+    assert abs(g2[5, 2] - p.mean()) < 1e-15
+    const, _ = T.subdivide_fill([True], np.full((1, 8), -0.75), np.zeros((1, 1, 3)))   # exactly representable: sums are exact
+    assert np.array_equal(const, np.full((8, 8), -0.75))
+    # (b) the field is unchanged: parent voxel [0,2]^3 of a 4 m cube vs its 8 children with the filled corners
+    cam = axis_camera(width=5, height=5, f=6.0)
+    kids = [(2 + ((o >> 2) & 1), 2 + ((o >> 1) & 1), 2 + (o & 1), 2) for o in range(8)]
+    err = {}
+    for K in (8, 16, 64):
+        A = O.render(scene(tree_from_cells([(1, 1, 1, 1)], geo=geo[:1]), cam=cam, k_samples=K))
+        B = O.render(scene(tree_from_cells(kids, geo=g2[:8]), cam=cam, k_samples=K))
+        assert A["alpha"].max() > 0.3
+        err[K] = np.abs(A["alpha"] - B["alpha"]).max()
+    assert err[64] < 2e-5 and 3.0 < err[8] / err[16] < 5.0, err
