@@ -48,6 +48,9 @@ constexpr int TILE_WARPS = TILE_THREADS / 32;
 #define DVX_CAND_GROUPS 8  // phase A: bands of rows of the warp's pixel block that walk their candidates independently.  Forward
                            // compositing of a saved frame, config 3 / config 4, ms, for 1, 2, 4, 8 bands: 1.378 1.377 1.354 1.312 / 1.934 1.943 1.935 1.888
 #endif
+#ifndef DVX_STAGE_PREFETCH
+#define DVX_STAGE_PREFETCH 1
+#endif
 #ifndef DVX_WARP_W
 #define DVX_WARP_W 4   // a warp covers DVX_WARP_W x (32 / DVX_WARP_W) pixels
 #endif
@@ -747,19 +750,38 @@ __global__ void __launch_bounds__(TILE_THREADS, DVX_TILE_MIN_CTAS) composite_til
       if (t == 0 && cur0 != NONE) c_l = cur0;
       uint32_t c_t = (part && q == qq) ? c_l : NONE;  // first entry this pixel still tests; NONE = not (or no longer) walking
       uint32_t pos = warp_min_u32(c_t);
+#if DVX_STAGE_PREFETCH
+      // the id of this lane's entry of the NEXT round is loaded one round ahead, and an entry's pixel rectangle and code are
+      // loaded together (the code of an entry that fails the rectangle test is wasted, 8 bytes from L2): one exposed load
+      // latency per round of 32 entries instead of three dependent ones
+      uint32_t id_next = pos + lane < end ? __ldg(A.ids + pos + lane) : 0u;
+#endif
       while (pos < end && __any_sync(0xffffffffu, c_t != NONE)) {
         const uint32_t n = min(32u, end - pos);
         // -- lane = entry: pre-filter and fp64 centre decomposition
         bool c = false;
         uint32_t ry0 = 1u, ry1 = 0u;  // rows of the entry's pixel rectangle
+#if DVX_STAGE_PREFETCH
+        const uint32_t id_cur = id_next;
+        if (pos + 32u + lane < end) id_next = __ldg(A.ids + pos + 32u + lane);
+#endif
         if ((uint32_t)lane < n) {
+#if DVX_STAGE_PREFETCH
+          const uint32_t id = id_cur;
+          const uint64_t code_v = __ldg(T.code + (id - T.base));
+#else
           const uint32_t id = __ldg(A.ids + pos + lane);
+#endif
           const ushort4 rc = __ldg(A.pxrect + id);
           c = rc.x <= ru1 && rc.z >= ru0 && rc.y <= rv1 && rc.w >= rv0;
           ry0 = rc.y; ry1 = rc.w;
           if (c) {
             uint32_t X, Y, Z, lv;
+#if DVX_STAGE_PREFETCH
+            dvx_decode16(code_v, X, Y, Z, lv);
+#else
             dvx_decode16(__ldg(T.code + (id - T.base)), X, Y, Z, lv);
+#endif
             const uint32_t size = 1u << (DVX_MAX_LEVEL - lv);
             const double hc = 0.5 * T.cell;
             const double d0x = Q.d0[0], d0y = Q.d0[1], d0z = Q.d0[2];
