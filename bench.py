@@ -638,7 +638,8 @@ def run_dvx(args):
         "fwd_value": fwd_value, "fwd_ms": ms_fwd / args.steps,
         "hbm_roofline_frac_step": hbm_frac_step,       # the [NS] definition: B_min / peak / step time (target 0.5: NOT met)
         "hbm_floor_ms": hbm_floor_ms, "issue_floor_ms": issue_floor_ms,
-        "frac_of_binding_floor": binding / ms_step if ms_step > 0 else None,
+        # the larger of the two floors over the step time; None when no fresh ncu instruction count exists for this workload
+        "frac_of_binding_floor": binding / ms_step if (ms_step > 0 and issue_floor_ms is not None) else None,
         "stage_ms": stage,
         "counters": dict(cnt, touched_voxels=touched, hits_per_ray=cnt["q_hit"] / px_step, frac_rays_terminated=frac_term),
         "records": rec_stats,
