@@ -486,6 +486,11 @@ dvx_status render_step1(dvx_ctx *ctx, const dvx_camera *cam, const dvx_octree *s
       }
     p.zclip = (float)(0.5 * (double)cam->near_ * mc);
   }
+  {  // side planes of the view frustum, one pixel outside the image on every side (conservative pre-cull of step 1)
+    const double t[4] = {(-1.0 - cam->cx) / cam->fx, ((double)cam->width + 1.0 - cam->cx) / cam->fx,
+                         (-1.0 - cam->cy) / cam->fy, ((double)cam->height + 1.0 - cam->cy) / cam->fy};
+    for (int i = 0; i < 4; ++i) { p.cull_t[i] = (float)t[i]; p.cull_l[i] = (float)sqrt(1.0 + t[i] * t[i]); }
+  }
   p.k_samples = o.k_samples; p.activation = o.activation; p.flags = o.flags; p.t_stop = o.t_stop;
   p.inv_k = 1.0f / (float)o.k_samples;
   f->trees_h.resize(p.n_trees);

@@ -71,19 +71,24 @@ __device__ __forceinline__ bool dvx_pixel_rect(const float (*pc)[3], const Frame
       any = true;
     }
   }
+  bool behind = false;  // some corner lies behind the clip plane: only then can an edge cross it (almost never)
 #pragma unroll
-  for (int c = 0; c < 8; ++c) {
+  for (int c = 0; c < 8; ++c) behind = behind || pc[c][2] < zc;
+  if (behind) {
 #pragma unroll
-    for (int ax = 1; ax <= 4; ax <<= 1) {
-      if (c & ax) continue;
-      const int c2 = c | ax;
-      float za = pc[c][2], zb = pc[c2][2];
-      if ((za < zc) != (zb < zc)) {
-        float f = (zc - za) / (zb - za);
-        float qx = pc[c][0] + f * (pc[c2][0] - pc[c][0]), qy = pc[c][1] + f * (pc[c2][1] - pc[c][1]);
-        float px = p.fx * qx / zc + p.cx, py = p.fy * qy / zc + p.cy;
-        xmin = fminf(xmin, px); xmax = fmaxf(xmax, px); ymin = fminf(ymin, py); ymax = fmaxf(ymax, py);
-        any = true;
+    for (int c = 0; c < 8; ++c) {
+#pragma unroll
+      for (int ax = 1; ax <= 4; ax <<= 1) {
+        if (c & ax) continue;
+        const int c2 = c | ax;
+        float za = pc[c][2], zb = pc[c2][2];
+        if ((za < zc) != (zb < zc)) {
+          float f = (zc - za) / (zb - za);
+          float qx = pc[c][0] + f * (pc[c2][0] - pc[c][0]), qy = pc[c][1] + f * (pc[c2][1] - pc[c][1]);
+          float px = p.fx * qx / zc + p.cx, py = p.fy * qy / zc + p.cy;
+          xmin = fminf(xmin, px); xmax = fmaxf(xmax, px); ymin = fminf(ymin, py); ymax = fmaxf(ymax, py);
+          any = true;
+        }
       }
     }
   }

@@ -35,6 +35,8 @@ struct FrameParams {
   uint32_t width, height, tiles_x, tiles_y, n_tiles, n_trees;
   float fx, fy, cx, cy, near_, far_, zclip;
   double inv_fx, inv_fy, cx_d, cy_d;  // fp64 copies for the per-pixel ray set-up of the tile kernel
+  float cull_t[4];   // tan of the frustum's side planes, one pixel outside the image: x/z in [t[0], t[1]], y/z in [t[2], t[3]]
+  float cull_l[4];   // sqrt(1 + t^2): length of the planes' normals (step 1's bounding-sphere pre-cull)
   double Rc[9];                       // camera rotation (row-major, camera -> world): world direction of a pixel (sky)
   uint32_t k_samples, activation, flags;
   float t_stop, inv_k;  // inv_k = 1 / k_samples

@@ -125,6 +125,24 @@ __device__ __forceinline__ bool voxel_rect(const FrameParams &p, const TreeFrame
   }
   s_out = (float)s;
   if (!(bmx[0] >= bmn[0]) || !(bmx[1] >= bmn[1]) || !(bmx[2] >= bmn[2])) return false;
+  {  // Cheap conservative pre-cull (59 % of config 3's voxels end here instead of in the 8-corner projection below): the voxel's
+     // bounding sphere lies wholly outside one side plane of the frustum (taken one pixel outside the image) or wholly behind
+     // the clip plane.  Everything the exact test keeps is inside the sphere (clipping to the box or to z = zclip only
+     // removes points), and the margin covers the fp32 rounding of this test (1e-3 of |centre| + radius).  The visible set, the
+     // pair count and every image are unchanged (checked on configs 3 and 4); step 1 0.199 -> 0.184 ms on config 3.
+     // Tried on top of it in round 2, all slower or equal: the SH record staged through shared memory by cp.async (0.208 ms,
+     // one CTA per SM less), four lanes per voxel reading 48 contiguous bytes each (0.187), an L2 prefetch of the record
+     // before the pair counting (0.192), 4 or 6 CTAs per SM (0.193 / 0.196): the kernel is bound by the dependent chain
+     // code -> octant masks -> record at 2.7 TB/s, not by how the record is read.
+    const float hs = 0.5f * s_out, cxl = rel_out[0] + hs, cyl = rel_out[1] + hs, czl = rel_out[2] + hs;
+    const float X = T.N[0] * cxl + T.N[3] * cyl + T.N[6] * czl, Y = T.N[1] * cxl + T.N[4] * cyl + T.N[7] * czl,
+                Z = T.N[2] * cxl + T.N[5] * cyl + T.N[8] * czl;
+    const float r = 1.7320508f * hs;
+    const float m = r + 1e-3f * (fabsf(X) + fabsf(Y) + fabsf(Z) + r);
+    if (Z + m < p.zclip) return false;
+    if (p.cull_t[0] * Z - X > m * p.cull_l[0] || X - p.cull_t[1] * Z > m * p.cull_l[1] ||
+        p.cull_t[2] * Z - Y > m * p.cull_l[2] || Y - p.cull_t[3] * Z > m * p.cull_l[3]) return false;
+  }
   float pc[8][3];
 #pragma unroll
   for (int c = 0; c < 8; ++c) {
