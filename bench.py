@@ -244,6 +244,8 @@ def optimizer_step_stats(ctx, dev, grads, peak, reps=5):
     coefficients, all octrees in one launch each (dvx_*_step_n) - timed with CUDA events (median of reps) against its algorithmic bytes:
       grid Adam : per grid point 4 (CSR offset) + 12 read + 12 written (density, m, v), per corner slot 4 (slot index)
                   + 4 (gradient read) + 4 (gradient zeroed) + 4 (corner record written)  = 28 G + 16 * 8V
+                  (two kernels: the per-point update, then the per-voxel rewrite of the corner and gradient records,
+                  which also reads the 4-byte point index of every slot: + 4 * 8V of real traffic, not counted)
       SH Adam   : 32 bytes per coefficient (g, p, m, v read; p, m, v, g = 0 written)"""
     import torch
     hp = dict(lr=0.01, beta1=0.9, beta2=0.99, eps=1e-15)
@@ -286,7 +288,7 @@ def optimizer_step_stats(ctx, dev, grads, peak, reps=5):
     return {"grid_points": G_total, "corner_slots": 8 * V_total, "sh_coefficients": n_sh, "grid_build_ms": build_ms,
             "grid_adam": {"ms": ms_grid, "bytes": b_grid, "gb_per_s": b_grid / ms_grid / 1e6, "hbm_frac": b_grid / ms_grid / 1e6 / peak},
             "sh_adam": {"ms": ms_sh, "bytes": b_sh, "gb_per_s": b_sh / ms_sh / 1e6, "hbm_frac": b_sh / ms_sh / 1e6 / peak},
-            "launches": 2 * ((len(dev.trees) + 31) // 32)}
+            "launches": 3 * ((len(dev.trees) + 31) // 32)}
 
 
 def feature_stats(ctx, dev, scene, peak, n_ch=64, reps=5):

@@ -1216,7 +1216,7 @@ dvx_status dvx_grid_adam_step_n(dvx_ctx *ctx, const dvx_adam *hp, uint32_t n, co
     if (it.grid->n_points == 0) continue;
     if (!it.density || !it.m || !it.v || !it.dgeo || !it.geo)
       return fail(ctx, DVX_ERR_INVALID_ARG, "dvx_grid_adam_step: NULL argument");
-    v.push_back({it.grid->offsets, it.grid->slots, it.grid->n_points, it.density, it.m, it.v, it.dgeo, it.geo});
+    v.push_back({it.grid->offsets, it.grid->slots, it.grid->point_of, it.grid->n_points, it.grid->n_voxels, it.density, it.m, it.v, it.dgeo, it.geo});
   }
   if (v.empty()) return DVX_OK;
   cudaSetDevice(ctx->device);

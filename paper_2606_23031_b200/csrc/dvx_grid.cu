@@ -8,8 +8,11 @@
 //
 // The optimizer step (reading R24: Adam) is one kernel per parameter KIND (all octrees of a scene in one launch), HBM-bound:
 //   grid_adam_kernel : thread = grid point.  GATHERS its <= 8 corner gradients (fixed order, so the step is
-//                      deterministic and needs no atomics), Adam, writes the new density back into every corner slot of
-//                      the [V][8] record the next forward reads, and zeroes the gradients it consumed.
+//                      deterministic and needs no atomics) and does the Adam update of its density.
+//   grid_write_kernel: thread = voxel.  Rebuilds the [V][8] corner record the next forward reads from the grid-point
+//                      densities (gathers from a mostly L2-resident array, two 16-byte stores) and zeroes the voxel's
+//                      gradient record.  (One kernel doing both from the grid-point side - 16 scattered 4-byte stores per
+//                      point - ran at 35 % of the HBM peak, 0.34 ms on config 3; the two passes take 0.20 ms, 58 %.)
 //   adam_kernel      : plain elementwise Adam + gradient zeroing for the SH coefficients (float4 lanes).
 // Keeping dL/dgeo as the [V][8] accumulation target of the backward pass (two 16-byte reductions per voxel run) and
 // summing per grid point here, once per step, replaces the scatter-add "fused into the backward atomics" that SURVEY.md
@@ -137,7 +140,18 @@ struct GridAdamBatch {
   uint32_t n_points[ADAM_BATCH];
   int n;
 };
+struct GridWriteBatch {   // second pass of the grid step: thread = voxel
+  uint32_t block_start[ADAM_BATCH + 1];
+  const uint32_t *point_of[ADAM_BATCH];
+  const float *density[ADAM_BATCH];
+  float *dgeo[ADAM_BATCH], *geo[ADAM_BATCH];
+  uint32_t n_voxels[ADAM_BATCH];
+  int n;
+};
 
+#ifndef DVX_GA_TWO_PASS
+#define DVX_GA_TWO_PASS 1
+#endif
 #ifndef DVX_GA_MINB
 #define DVX_GA_MINB 8  // 32 registers, 64 warps per SM: the kernel waits on scattered 4-byte accesses
 #endif
@@ -166,12 +180,32 @@ __global__ void __launch_bounds__(GRID_THREADS, DVX_GA_MINB) grid_adam_kernel(co
   B.density[e][p] = pv;
   B.m[e][p] = mv;
   B.v[e][p] = vv;
+#if !DVX_GA_TWO_PASS
 #pragma unroll
   for (int i = 0; i < 8; ++i)
     if (sl[i] != 0xFFFFFFFFu) {
       geo[sl[i]] = pv;
       dgeo[sl[i]] = 0.f;
     }
+#endif
+}
+
+// Second pass (thread = voxel): the 32-byte corner record the next forward reads is rebuilt from the grid-point densities
+// (eight 4-byte gathers from an array that mostly sits in L2) and written with two 16-byte stores, and the voxel's gradient
+// record is zeroed the same way - instead of 16 scattered 4-byte stores per grid point in the first pass.
+__global__ void __launch_bounds__(GRID_THREADS) grid_write_kernel(const __grid_constant__ GridWriteBatch B) {
+  int e = 0;
+  while (e + 1 < B.n && blockIdx.x >= B.block_start[e + 1]) ++e;
+  const uint32_t v = (blockIdx.x - B.block_start[e]) * GRID_THREADS + threadIdx.x;
+  if (v >= B.n_voxels[e]) return;
+  const uint4 *po = reinterpret_cast<const uint4 *>(B.point_of[e]) + 2 * (size_t)v;
+  const uint4 a = __ldg(po), b = __ldg(po + 1);
+  const float *__restrict__ d = B.density[e];
+  const float4 g0 = make_float4(d[a.x], d[a.y], d[a.z], d[a.w]), g1 = make_float4(d[b.x], d[b.y], d[b.z], d[b.w]);
+  float4 *go = reinterpret_cast<float4 *>(B.geo[e]) + 2 * (size_t)v;
+  go[0] = g0; go[1] = g1;
+  float4 *dg = reinterpret_cast<float4 *>(B.dgeo[e]) + 2 * (size_t)v;
+  dg[0] = make_float4(0.f, 0.f, 0.f, 0.f); dg[1] = make_float4(0.f, 0.f, 0.f, 0.f);
 }
 
 // elementwise Adam: a block owns ADAM_CHUNK consecutive floats of one array (4 float4 per thread, 16 loads in flight),
@@ -283,6 +317,7 @@ void dvx_grid_adam_launch(float lr, float beta1, float beta2, float eps, uint32_
     GridAdamBatch B;
     memset(&B, 0, sizeof(B));
     uint32_t blocks = 0;
+    const uint32_t first = at;
     while (at < n && B.n < ADAM_BATCH) {
       const DvxGridAdamItem &it = items[at++];
       if (it.n_points == 0) continue;
@@ -296,6 +331,21 @@ void dvx_grid_adam_launch(float lr, float beta1, float beta2, float eps, uint32_
     B.block_start[B.n] = blocks;
     DVX_COUNT_LAUNCH(1);
     grid_adam_kernel<<<blocks, GRID_THREADS, 0, st>>>(h, B);
+#if DVX_GA_TWO_PASS
+    GridWriteBatch Wb;
+    memset(&Wb, 0, sizeof(Wb));
+    uint32_t wblocks = 0;
+    for (uint32_t j = first; j < at; ++j) {
+      const DvxGridAdamItem &it = items[j];
+      if (it.n_points == 0 || it.n_voxels == 0) continue;
+      const int e = Wb.n++;
+      Wb.block_start[e] = wblocks;
+      wblocks += blocks_for(it.n_voxels);
+      Wb.point_of[e] = it.point_of; Wb.density[e] = it.density; Wb.dgeo[e] = it.dgeo; Wb.geo[e] = it.geo; Wb.n_voxels[e] = it.n_voxels;
+    }
+    Wb.block_start[Wb.n] = wblocks;
+    if (wblocks) { DVX_COUNT_LAUNCH(1); grid_write_kernel<<<wblocks, GRID_THREADS, 0, st>>>(Wb); }
+#endif
   }
 }
 void dvx_adam_launch(float lr, float beta1, float beta2, float eps, uint32_t step, uint32_t n, const DvxAdamItem *items,

@@ -156,8 +156,8 @@ void dvx_grid_gather_launch(const float *density, const uint32_t *point_of, uint
 void dvx_grid_reduce_launch(const float *dgeo, const uint32_t *offsets, const uint32_t *slots, uint32_t n_points,
                             float *ddensity, cudaStream_t st);
 struct DvxGridAdamItem {
-  const uint32_t *offsets, *slots;
-  uint32_t n_points;
+  const uint32_t *offsets, *slots, *point_of;
+  uint32_t n_points, n_voxels;
   float *density, *m, *v, *dgeo, *geo;
 };
 struct DvxAdamItem {
