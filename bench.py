@@ -566,9 +566,12 @@ def run_dvx(args):
     ms_e2e = timed(args.steps, host=True, bwd=not args.fwd_only)
     clocks = sampler.stop() if sampler else None
     sort_stats = sort_throughput(ctx, cnt["pairs"] // n_cams, scene, W, H) if rank == 0 else None
-    feat_stats = feature_stats(ctx, dev, scene, measured_peaks()[0]) if rank == 0 and not args.fwd_only else None
-    struct_stats = structure_stats(ctx, dev, scene) if rank == 0 and not args.fwd_only else None
-    opt_stats = optimizer_step_stats(ctx, dev, grads, measured_peaks()[0]) if rank == 0 and not args.fwd_only else None
+    # the widening rows and the extra workloads are single-process reports: with replicas the other ranks would sit in the
+    # process-group teardown while rank 0 measures them
+    solo = rank == 0 and world == 1 and not args.fwd_only
+    feat_stats = feature_stats(ctx, dev, scene, measured_peaks()[0]) if solo else None
+    struct_stats = structure_stats(ctx, dev, scene) if solo else None
+    opt_stats = optimizer_step_stats(ctx, dev, grads, measured_peaks()[0]) if solo else None
     rec_stats = None
     if rank == 0 and not args.fwd_only and not args.no_records:   # what the hit records of one frame take (camera 0)
         _, _, _, fr = dev.render(0, save=True)
@@ -576,7 +579,7 @@ def run_dvx(args):
         rec_stats["bytes_per_hit"] = rec_stats["bytes_used"] / max(cnt["q_hit"] / n_cams, 1)
         fr.release()
     extra = None
-    if rank == 0 and args.config == 3 and not (args.no_extra or args.fwd_only or args.opaque or args.k_samples or args.no_records):
+    if rank == 0 and world == 1 and args.config == 3 and not (args.no_extra or args.fwd_only or args.opaque or args.k_samples or args.no_records):
         extra = {}
         for cfg_x in (4, 5):   # BASELINE.json configs[3] (crowded) and configs[4] (6-camera training batch), device-resident
             extra[workload_name(cfg_x)] = time_workload(ctx, dvx, cfg_x, steps=max(3, min(args.steps, 10)), warmup=3)
