@@ -636,6 +636,7 @@ def run_dvx(args):
                 issue["kernels"][k] = {"warp_instructions": wi, "ms": ms_k, "achieved_warp_instr_per_s": wi / (ms_k * 1e-3),
                                        "frac": wi / (ms_k * 1e-3) / issue_peak, "issue_floor_ms": floor}
     binding = max(hbm_floor_ms, issue_floor_ms or 0.0)
+    rec_bytes = 0 if (args.fwd_only or args.no_records) else 44 * cnt["q_hit"] / n_cams
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
@@ -652,6 +653,10 @@ def run_dvx(args):
         "algorithmic_bytes": ab,
         "roofline": {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
                      "frac": achieved / peak if peak else None,
+                     # the same kernel with the hit records it streams counted as well (this design's own traffic, 44 B per
+                     # composited hit in each direction; not part of SURVEY 8(d)'s algorithmic bytes)
+                     "achieved_with_records": (dom_bytes + rec_bytes) / (dom_ms * 1e-3) / 1e9 if dom_ms > 0 else 0.0,
+                     "frac_with_records": (dom_bytes + rec_bytes) / (dom_ms * 1e-3) / 1e9 / peak if (dom_ms > 0 and peak) else None,
                      "traffic": (pk.get(dom) or {}).get("dram_bytes"), "traffic_commit": prof.get("commit"),
                      "traffic_stale": bool(stale), "peak_source": peak_src, "bytes_per_launch": dom_bytes, "ms_per_launch": dom_ms,
                      "all_kernels_ms": kernels},
