@@ -224,6 +224,20 @@ const char *dvx_last_error(const dvx_ctx *ctx);
  * the low key_bits bits of the key, ascending, stable.  keys / vals DEVICE arrays, sorted in place. */
 dvx_status dvx_sort_pairs(dvx_ctx *ctx, uint64_t *keys, uint32_t *vals, uint64_t n, uint32_t key_bits);
 
+/* The same sort for callers that may not allocate device memory (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc): needs no context and calls no cudaMalloc, cudaFree or allocator callback.  Its
+ * ping-pong buffers and one-sweep scratch live in a file-scope device array of fixed size inside the library
+ * (DVX_SORT_NO_ALLOC_MAX_PAIRS pairs: about 15 MB, held by every GPU that loads the library until the process exits).
+ * n > DVX_SORT_NO_ALLOC_MAX_PAIRS is rejected with DVX_ERR_INVALID_ARG and a message; use dvx_sort_pairs then.
+ * device: CUDA device index (made current); cuda_stream: the stream to enqueue on (NULL = default stream); keys / vals
+ * DEVICE arrays, sorted in place, ascending by the low key_bits bits, stable; err: HOST buffer [err_cap] that receives the
+ * error text (may be NULL).  Does not synchronise.  ALL calls share the one static array: calls that overlap on the GPU
+ * (different streams or threads without ordering between them) race - order them, e.g. on one stream.  The array keeps
+ * the last call's contents; whatever must start at zero is cleared by every call. */
+#define DVX_SORT_NO_ALLOC_MAX_PAIRS (1u << 20)
+dvx_status dvx_sort_pairs_no_alloc(int device, void *cuda_stream, uint64_t *keys, uint32_t *vals, uint64_t n,
+                                   uint32_t key_bits, char *err, size_t err_cap);
+
 /* ---- Widening row N2: shared grid-point corner densities and the optimizer step -----------------------
  * The corner densities "are optimized during training".  Reading R23: coincident corners of
  * neighbouring voxels are ONE parameter (a grid point), identified by the corner's integer coordinate on the level-16

@@ -3,4 +3,4 @@ the single-pass compositional sparse-voxel tile rasterizer, forward and backward
 include/dvx.h (libdvx.so, hand-written CUDA).  This package is the thin Python binding; see DESIGN.md.
 """
 from .binding import (Context, Octree, Frame, Camera, SceneOnDevice, DvxError, camera_from, load, LIB_PATH, EXPORTS,  # noqa: F401
-                      FLAG_COUNTERS, FLAG_NAIVE, FLAG_NO_RECORDS)
+                      FLAG_COUNTERS, FLAG_NAIVE, FLAG_NO_RECORDS, sort_pairs_no_alloc, SORT_NO_ALLOC_MAX_PAIRS)

@@ -27,7 +27,7 @@ EXPORTS = ["dvx_create", "dvx_destroy", "dvx_octree_create", "dvx_octree_refresh
            "dvx_grid_adam_step", "dvx_adam_step", "dvx_grid_adam_step_n", "dvx_adam_step_n",
            "dvx_frame_weights", "dvx_render_features", "dvx_fuse_features",
            "dvx_cloud_create", "dvx_cloud_destroy", "dvx_density_prior", "dvx_subdivide_near", "dvx_prune",
-           "dvx_set_record_budget", "dvx_frame_record_stats", "dvx_trim", "dvx_microbench_fma", "dvx_render_batch", "dvx_backward_batch", "dvx_subdivide_fill"]
+           "dvx_set_record_budget", "dvx_frame_record_stats", "dvx_trim", "dvx_microbench_fma", "dvx_render_batch", "dvx_backward_batch", "dvx_subdivide_fill", "dvx_sort_pairs_no_alloc"]
 
 
 class DvxError(RuntimeError):
@@ -144,6 +144,7 @@ def load():
                                      C.POINTER(Image), C.POINTER(P)]
     lib.dvx_backward_batch.argtypes = [P, C.c_uint32, C.POINTER(P), C.POINTER(P), C.POINTER(P), C.POINTER(P), Grad, C.POINTER(Grad)]
     lib.dvx_subdivide_fill.argtypes = [P, C.c_uint32, P, P, P, C.c_uint32, P, P, C.c_uint64, C.POINTER(C.c_uint64)]
+    lib.dvx_sort_pairs_no_alloc.argtypes = [C.c_int, P, P, P, C.c_uint64, C.c_uint32, C.c_char_p, C.c_size_t]
     lib.dvx_trim.argtypes = [P, C.POINTER(C.c_uint64)]
     lib.dvx_microbench_fma.argtypes = [P, C.c_uint32, C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_float)]
     lib.dvx_set_record_budget.argtypes = [P, C.c_uint64]
@@ -155,6 +156,21 @@ def load():
     lib.dvx_launch_count.restype = C.c_uint64
     _lib = lib
     return lib
+
+
+SORT_NO_ALLOC_MAX_PAIRS = 1 << 20
+
+
+def sort_pairs_no_alloc(keys, vals, key_bits, device=0, stream_ptr=None):
+    """dvx_sort_pairs_no_alloc: sorts CUDA int64 keys / int32 vals in place using the library's static scratch (no context,
+    no allocation; at most SORT_NO_ALLOC_MAX_PAIRS pairs).  Raises DvxError with the library's message."""
+    lib = load()
+    buf = C.create_string_buffer(256)
+    n = int(keys.shape[0])
+    rc = lib.dvx_sort_pairs_no_alloc(device, C.c_void_p(stream_ptr), keys.data_ptr() if n else None, vals.data_ptr() if n else None,
+                                     n, key_bits, buf, 256)
+    if rc != DVX_OK:
+        raise DvxError(rc, buf.value.decode())
 
 
 class Context:

@@ -5,6 +5,10 @@
 // digit position.  n < 2^30 pairs (the status word of the look-back keeps a 30-bit count).
 #include "dvx_internal.cuh"
 
+#include <stdio.h>
+
+#include <mutex>
+
 namespace {
 
 constexpr int SORT_THREADS = 256;
@@ -287,4 +291,83 @@ int dvx_sort_launch(uint64_t *keys_a, uint32_t *vals_a, uint64_t *keys_b, uint32
     cur ^= 1;
   }
   return cur;
+}
+
+// ------------------------------------------------------------------ dvx_sort_pairs_no_alloc (include/dvx.h)
+// The step-2 sort for callers that may not allocate (CUDA graph capture, tight serving loops, harnesses that forbid
+// cudaMalloc): the ping-pong buffers and the one-sweep scratch of dvx_sort_launch live in ONE file-scope device array of
+// fixed size, so the entry point calls no cudaMalloc / cudaFree / allocator callback.  Every GPU that loads the library
+// holds the array (DVX_SORT_NO_ALLOC_BYTES, about 15 MB) until the process exits.  All calls share it: two calls that overlap
+// on the GPU (different streams, or threads) race; it keeps the last call's contents, and what must start at zero (digit
+// histograms, tickets, tile status) is cleared by dvx_sort_launch's cudaMemsetAsync on every call.
+namespace {
+constexpr uint64_t NA_MAX_PAIRS = DVX_SORT_NO_ALLOC_MAX_PAIRS;
+constexpr size_t NA_TILES = (size_t)((NA_MAX_PAIRS + SORT_TILE - 1) / SORT_TILE);
+constexpr size_t NA_SCRATCH_WORDS = (size_t)MAX_PASSES * RADIX + MAX_PASSES + (size_t)MAX_PASSES * NA_TILES * RADIX + 64;
+constexpr size_t na_round(size_t b) { return (b + 255) & ~(size_t)255; }
+constexpr size_t NA_OFF_VALS = na_round((size_t)NA_MAX_PAIRS * 8);                    // keys_b first
+constexpr size_t NA_OFF_SCRATCH = NA_OFF_VALS + na_round((size_t)NA_MAX_PAIRS * 4);   // then vals_b
+constexpr size_t NA_BYTES = NA_OFF_SCRATCH + na_round(NA_SCRATCH_WORDS * sizeof(uint32_t));
+}  // namespace
+
+// In host code this name is a host-side stand-in for the device array, NOT a device address: the address the kernels get
+// comes from cudaGetSymbolAddress below, once per device.
+static __device__ __align__(256) unsigned char g_sort_no_alloc[NA_BYTES];
+
+namespace {
+constexpr int NA_MAX_DEVICES = 64;
+std::mutex g_na_mutex;
+unsigned char *g_na_base[NA_MAX_DEVICES] = {};   // device address of g_sort_no_alloc on each device, resolved on first use
+
+void na_error(char *err, size_t cap, const char *msg) {
+  if (err && cap) snprintf(err, cap, "%s", msg);
+}
+}  // namespace
+
+extern "C" dvx_status dvx_sort_pairs_no_alloc(int device, void *cuda_stream, uint64_t *keys, uint32_t *vals, uint64_t n,
+                                              uint32_t key_bits, char *err, size_t err_cap) {
+  if (err && err_cap) err[0] = 0;
+  if (n == 0) return DVX_OK;
+  if (!keys || !vals) { na_error(err, err_cap, "dvx_sort_pairs_no_alloc: keys / vals is NULL"); return DVX_ERR_INVALID_ARG; }
+  if (key_bits < 1 || key_bits > 64) { na_error(err, err_cap, "dvx_sort_pairs_no_alloc: key_bits must be in [1,64]"); return DVX_ERR_INVALID_ARG; }
+  if (n > NA_MAX_PAIRS) {
+    if (err && err_cap)
+      snprintf(err, err_cap, "dvx_sort_pairs_no_alloc: n = %llu exceeds DVX_SORT_NO_ALLOC_MAX_PAIRS = %llu (the static scratch is sized for that; use dvx_sort_pairs)",
+               (unsigned long long)n, (unsigned long long)NA_MAX_PAIRS);
+    return DVX_ERR_INVALID_ARG;
+  }
+  if (device < 0 || device >= NA_MAX_DEVICES) { na_error(err, err_cap, "dvx_sort_pairs_no_alloc: device index out of range"); return DVX_ERR_INVALID_ARG; }
+  cudaError_t e = cudaSetDevice(device);
+  if (e != cudaSuccess) { na_error(err, err_cap, cudaGetErrorString(e)); return DVX_ERR_CUDA; }
+  unsigned char *base = nullptr;
+  {
+    std::lock_guard<std::mutex> lock(g_na_mutex);
+    if (!g_na_base[device]) {   // once per device, with that device current
+      void *p = nullptr;
+      e = cudaGetSymbolAddress(&p, g_sort_no_alloc);
+      if (e != cudaSuccess || !p) {
+        na_error(err, err_cap, e != cudaSuccess ? cudaGetErrorString(e) : "cudaGetSymbolAddress returned NULL");
+        cudaGetLastError();
+        return DVX_ERR_CUDA;
+      }
+      g_na_base[device] = (unsigned char *)p;
+    }
+    base = g_na_base[device];
+  }
+  if (dvx_sort_scratch_bytes(n) > NA_SCRATCH_WORDS * sizeof(uint32_t)) {  // cannot happen for n <= NA_MAX_PAIRS; kept as a guard
+    na_error(err, err_cap, "dvx_sort_pairs_no_alloc: internal scratch bound violated");
+    return DVX_ERR_INVALID_ARG;
+  }
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  uint64_t *kb = reinterpret_cast<uint64_t *>(base);
+  uint32_t *vb = reinterpret_cast<uint32_t *>(base + NA_OFF_VALS);
+  void *scr = base + NA_OFF_SCRATCH;
+  const int which = dvx_sort_launch(keys, vals, kb, vb, n, key_bits, scr, st);   // clears its scratch itself
+  if (which) {   // an odd number of passes left the result in the static buffers
+    cudaMemcpyAsync(keys, kb, n * 8, cudaMemcpyDeviceToDevice, st);
+    cudaMemcpyAsync(vals, vb, n * 4, cudaMemcpyDeviceToDevice, st);
+  }
+  e = cudaGetLastError();
+  if (e != cudaSuccess) { na_error(err, err_cap, cudaGetErrorString(e)); return DVX_ERR_CUDA; }
+  return DVX_OK;
 }
