@@ -40,6 +40,7 @@ def parse_args():
     ap.add_argument("--cpu-tiles", type=int, default=0, help="tiles in the CPU-oracle sample (0 = pick for about 10-30 s)")
     ap.add_argument("--fwd-only", action="store_true", help="profiling aid: time dvx_render alone")
     ap.add_argument("--k-samples", type=int, default=0, help="report-only variant: override K (samples per voxel segment)")
+    ap.add_argument("--activation", type=int, default=-1, help="report-only variant: density activation (0 exp, 1 exp-linear, R5)")
     ap.add_argument("--opaque", action="store_true", help="report-only variant 3b: config 3 with raw += 8 on leaves holding a LiDAR return")
     ap.add_argument("--no-records", action="store_true",
                     help="A/B aid: DVX_FLAG_NO_RECORDS (the backward walks the tile lists again instead of replaying hit records)")
@@ -96,7 +97,7 @@ class ClockSampler:
 
 def config_dict(args, scene, world):
     """The `config` object of the JSON line: the same keys from both arms (the driver compares them)."""
-    return {"workload": workload_name(args.config) + ("_opaque3b" if args.opaque else "") + ("_K%d" % args.k_samples if args.k_samples else ""),
+    return {"workload": workload_name(args.config) + ("_opaque3b" if args.opaque else "") + ("_K%d" % args.k_samples if args.k_samples else "") + ("_act%d" % args.activation if args.activation >= 0 else ""),
             "cameras": len(scene.cameras), "k_samples": scene.k_samples, "sh_degree": scene.static.sh_degree,
             "voxels": int(sum(t.n_voxels for t in scene.octrees)), "actors": len(scene.actors),
             "l2_policy": "inputs larger than L2 (voxel records + gradient buffers >> 126 MB)", "replicas": world,
@@ -579,7 +580,7 @@ def run_dvx(args):
         rec_stats["bytes_per_hit"] = rec_stats["bytes_used"] / max(cnt["q_hit"] / n_cams, 1)
         fr.release()
     extra = None
-    if rank == 0 and world == 1 and args.config == 3 and not (args.no_extra or args.fwd_only or args.opaque or args.k_samples or args.no_records):
+    if rank == 0 and world == 1 and args.config == 3 and not (args.no_extra or args.fwd_only or args.opaque or args.k_samples or args.no_records or args.activation >= 0):
         extra = {}
         for cfg_x in (4, 5):   # BASELINE.json configs[3] (crowded) and configs[4] (6-camera training batch), device-resident
             extra[workload_name(cfg_x)] = time_workload(ctx, dvx, cfg_x, steps=max(3, min(args.steps, 10)), warmup=3)
@@ -686,6 +687,8 @@ def make_scene(args):
     scene = dvx_scenes.make_config(args.config, **({"opaque": True} if args.opaque and args.config == 3 else {}))
     if args.k_samples:
         scene.k_samples = args.k_samples
+    if args.activation >= 0:
+        scene.activation = args.activation
     return scene
 
 

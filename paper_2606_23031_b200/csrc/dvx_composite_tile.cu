@@ -226,6 +226,23 @@ __device__ __forceinline__ float integrate_geom(const CompositeArgs &A, const ui
       }
     }
     if (BWD) M[0] = S;  // act' = act for exp
+  } else if (kind == 1 && K == 8) {  // exp-linear (R5, theta = 1.1) at the configured K: unrolled like the exp case
+    constexpr float TH = 1.1f, A1 = LOG2E / TH, A0 = (0.09531017980432493f - 1.0f) * LOG2E;  // ex2(A1 raw + A0) = exp(raw/theta - 1 + ln theta)
+#pragma unroll
+    for (int k = 0; k < 8; ++k) {
+      const float l8 = (float)(2 * k + 1) * 0.0625f;
+      const float raw = fmaf(fmaf(fmaf(c[3], l8, c[2]), l8, c[1]), l8, c[0]);
+      const float ex = ex2_approx(fmaf(raw, A1, A0));
+      const bool lin = raw > TH;
+      S += lin ? raw : ex;
+      if (BWD) {
+        const float ds = lin ? 1.0f : ex * (1.0f / TH);
+        M[0] += ds;
+        M[1] = fmaf(ds, l8, M[1]);
+        M[2] = fmaf(ds, l8 * l8, M[2]);
+        M[3] = fmaf(ds, l8 * l8 * l8, M[3]);
+      }
+    }
   } else if (kind == 0) {  // exp: sigma = ex2(raw * log2 e), act' = act
     const float c0 = c[0] * LOG2E, c1 = c[1] * LOG2E, c2 = c[2] * LOG2E, c3 = c[3] * LOG2E;
 #pragma unroll 4
@@ -448,12 +465,14 @@ __device__ __forceinline__ void phase_B2(const CompositeArgs &A, int lane, int c
 }
 
 // The next batch slot of this warp's hit-record stream, or NULL once the pool is exhausted (warp-uniform).
-// `ptr` is the warp's write pointer: REC_PTR_START before the first batch, REC_PTR_OFF after the pool ran out (both have a
-// zero high word, which no device address has), else the address of the next slot.  Chunks start at multiples of
-// DVX_REC_CHUNK_STRIDE and hold DVX_REC_CHUNK batches, so the low bits of the pointer say when a new chunk is due; it is
-// taken from the pool with one atomic and linked behind the previous one.  The fast path is two 32-bit tests and an add.
+// `ptr` is the warp's write pointer: REC_PTR_START before the first batch, else the address of the next slot - or, after
+// the pool ran out, the same byte offsets with a zero high word (which no device address has): the warp then writes
+// nothing but keeps COUNTING the chunks it would have taken, so that CNT_REC_CHUNKS ends up as what the frame needed and
+// the next frame's pool is sized right.  Chunks start at multiples of DVX_REC_CHUNK_STRIDE and hold DVX_REC_CHUNK batches,
+// so the low bits of the pointer say when a new chunk is due; it is taken from the pool with one atomic and linked behind
+// the previous one.  The fast path is two 32-bit tests and an add.
 constexpr uint32_t REC_CHUNK_USED = DVX_REC_CHUNK * DVX_REC_BATCH_BYTES;
-constexpr unsigned long long REC_PTR_START = REC_CHUNK_USED, REC_PTR_OFF = 1ull;
+constexpr unsigned long long REC_PTR_START = REC_CHUNK_USED;
 template <bool NRM>
 __device__ __forceinline__ unsigned char *rec_next_block(const CompositeArgs &A, int lane, int tile, int warp, WarpQueue<NRM> &Q,
                                                          unsigned long long &ptr) {
@@ -461,9 +480,9 @@ __device__ __forceinline__ unsigned char *rec_next_block(const CompositeArgs &A,
     uint32_t c = 0;
     if (lane == 0) c = (uint32_t)atomicAdd(&A.counters[CNT_REC_CHUNKS], 1ull);
     c = __shfl_sync(0xffffffffu, c, 0);
-    if (c >= A.rec_cap) {
+    if (c >= A.rec_cap) {  // the counter only grows: from here on this warp always lands here
       if (lane == 0) atomicOr(reinterpret_cast<unsigned int *>(&A.counters[CNT_REC_OVERFLOW]), 1u);
-      ptr = REC_PTR_OFF;
+      ptr = 0;             // counting mode: a virtual chunk
     } else {
       if (lane == 0) {
         if (ptr == REC_PTR_START) A.rec_tab[2 * ((uint32_t)tile * 8u + (uint32_t)warp)] = c;
@@ -473,8 +492,7 @@ __device__ __forceinline__ unsigned char *rec_next_block(const CompositeArgs &A,
       ptr = reinterpret_cast<unsigned long long>(A.rec_pool) + (unsigned long long)c * DVX_REC_CHUNK_STRIDE;
     }
   }
-  if ((uint32_t)(ptr >> 32) == 0u) return nullptr;
-  unsigned char *blk = reinterpret_cast<unsigned char *>(ptr);
+  unsigned char *blk = (uint32_t)(ptr >> 32) ? reinterpret_cast<unsigned char *>(ptr) : nullptr;
   ptr += DVX_REC_BATCH_BYTES;
   return blk;
 }

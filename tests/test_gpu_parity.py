@@ -242,6 +242,18 @@ def test_t2_t3_config4_crowded_fwd_bwd_full_frame(ctx):
     _sampled_parity(ctx, sc, None, 41, backward=True)
 
 
+def test_config3_exp_linear_activation_sampled_tiles(ctx, config3):
+    """R5 option 1 (PAPER.md:107 'exponential-linear density activation') at the headline size through its K = 8
+    specialisation: 48 seeded tiles of config 3, forward and every gradient entry, by record replay and by list walk."""
+    sc = config3
+    keep = sc.activation
+    sc.activation = 1
+    try:
+        _sampled_parity(ctx, sc, 48, 35, backward=True)
+    finally:
+        sc.activation = keep
+
+
 def test_t1_config4_tile_order_where_boxes_stack(ctx):
     """T1 on 16 tiles of config 4 chosen where rays cross the most boxes (each holds a pixel crossing >= 6): the list of every
     (tile, octree, octant) bucket ascends in the R14b key and contains the oracle's hit list as a subsequence, bit-exact."""
