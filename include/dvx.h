@@ -183,15 +183,18 @@ dvx_status dvx_frame_record_stats(dvx_ctx *ctx, const dvx_frame *frame, uint64_t
  * copies of RGB, depth and alpha (out_host.* are HOST pointers; valid after the stream is synchronised);
  * dvx_backward_host enqueues the host->device copies of the incoming image gradients (HOST pointers; depth / alpha
  * may be NULL) and then runs step 5.  The copies run on a second, library-owned stream so that they overlap the compute
- * on the context's stream (copy-out of frame i with the backward of frame i, copy-in with the forward); events order
- * them.  The host images of dvx_render_host are valid once the context's stream has been synchronised AFTER the matching
- * dvx_backward_host call (or directly after dvx_render_host when saved == NULL).  Octree arrays and gradient buffers stay DEVICE pointers (they are model
+ * on the context's stream (copy-out of frame i with the backward of frame i and the start of frame i+1 - the staging is
+ * double-buffered -, copy-in with the forward); events order them.  The host images of dvx_render_host are valid once the
+ * context's stream has been synchronised after dvx_host_io_wait(ctx), which makes that stream wait for every copy-out still
+ * in flight (a device-wide synchronisation covers them too; with saved == NULL the render call itself orders the stream
+ * behind its copies).  Octree arrays and gradient buffers stay DEVICE pointers (they are model
  * state that lives in HBM across steps).  Bytes moved per call: 20 W H out, 12 W H (+4 W H each for depth/alpha) in. */
 dvx_status dvx_render_host(dvx_ctx *ctx, const dvx_camera *cam, const dvx_octree *static_tree, uint32_t n_actors,
                            const dvx_octree *const *actors, const float *poses_l2w, const float *box_half,
                            const dvx_render_opts *opts, dvx_image out_host, dvx_frame **saved);
 dvx_status dvx_backward_host(dvx_ctx *ctx, dvx_frame *saved, const float *dL_drgb_host, const float *dL_ddepth_host,
                              const float *dL_dalpha_host, dvx_grad static_grad, const dvx_grad *actor_grads);
+dvx_status dvx_host_io_wait(dvx_ctx *ctx);
 
 /* Introspection for the parity tests and the benchmark (each synchronises the stream).
  * dvx_debug_tile_list: the sorted voxel list (voxel indices within octree `octree`, 0 = static, i = actor i-1) of
@@ -204,9 +207,11 @@ dvx_status dvx_frame_counters(dvx_ctx *ctx, const dvx_frame *frame, uint64_t *v_
 /* Device milliseconds (CUDA events on the context's stream) of the stages of the frame's dvx_render call:
  * [0] preprocess (step 1), [1] key generation + sort + ranges (step 2), [2] compositing kernel (steps 3+4);
  * after dvx_backward also [3] all of step 5, [4] its compositing-replay kernel alone, [5] its per-voxel SH
- * post-pass alone.  [6], [7] reserved (0).  HOST out[8].  Synchronises the stream. */
+ * post-pass alone; [6] the gap between the end of step 1 and the start of step 2 (the host round trip that reads the pair
+ * count: the GPU idles), [7] the gap between the end of compositing and the start of step 5 (whatever the caller or a copy
+ * put in between).  HOST out[8].  Synchronises the stream. */
 dvx_status dvx_frame_stage_ms(dvx_ctx *ctx, const dvx_frame *frame, float *ms_out8);
-/* The same six stage times SUMMED over every frame released (or rendered with saved = NULL) since the last call;
+/* The same eight times SUMMED over every frame released (or rendered with saved = NULL) since the last call;
  * *n_frames = how many.  Lets a benchmark time the stages of the very steps it measures without keeping frames alive.
  * HOST ms_out8[8], HOST n_frames.  Synchronises the stream. */
 dvx_status dvx_stage_ms_collect(dvx_ctx *ctx, float *ms_out8, uint32_t *n_frames);

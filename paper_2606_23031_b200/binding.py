@@ -15,7 +15,7 @@ LIB_PATH = os.path.join(_HERE, "libdvx.so")
 DVX_OK = 0
 ERRORS = {-1: "DVX_ERR_INVALID_ARG", -2: "DVX_ERR_BAD_OCTREE", -3: "DVX_ERR_OOM", -4: "DVX_ERR_CUDA",
           -5: "DVX_ERR_NOT_IMPLEMENTED"}
-STAGES = ("preprocess", "sort", "composite", "backward", "backward_composite", "backward_sh")
+STAGES = ("preprocess", "sort", "composite", "backward", "backward_composite", "backward_sh", "gap_host_sync", "gap_fwd_bwd")
 FLAG_COUNTERS = 1
 FLAG_NAIVE = 2
 FLAG_NO_RECORDS = 4
@@ -27,7 +27,7 @@ EXPORTS = ["dvx_create", "dvx_destroy", "dvx_octree_create", "dvx_octree_refresh
            "dvx_grid_adam_step", "dvx_adam_step", "dvx_grid_adam_step_n", "dvx_adam_step_n",
            "dvx_frame_weights", "dvx_render_features", "dvx_fuse_features",
            "dvx_cloud_create", "dvx_cloud_destroy", "dvx_density_prior", "dvx_subdivide_near", "dvx_prune",
-           "dvx_set_record_budget", "dvx_frame_record_stats", "dvx_trim", "dvx_microbench_fma", "dvx_render_batch", "dvx_backward_batch", "dvx_subdivide_fill", "dvx_sort_pairs_no_alloc"]
+           "dvx_set_record_budget", "dvx_frame_record_stats", "dvx_trim", "dvx_microbench_fma", "dvx_render_batch", "dvx_backward_batch", "dvx_subdivide_fill", "dvx_sort_pairs_no_alloc", "dvx_host_io_wait"]
 
 
 class DvxError(RuntimeError):
@@ -145,6 +145,7 @@ def load():
     lib.dvx_backward_batch.argtypes = [P, C.c_uint32, C.POINTER(P), C.POINTER(P), C.POINTER(P), C.POINTER(P), Grad, C.POINTER(Grad)]
     lib.dvx_subdivide_fill.argtypes = [P, C.c_uint32, P, P, P, C.c_uint32, P, P, C.c_uint64, C.POINTER(C.c_uint64)]
     lib.dvx_sort_pairs_no_alloc.argtypes = [C.c_int, P, P, P, C.c_uint64, C.c_uint32, C.c_char_p, C.c_size_t]
+    lib.dvx_host_io_wait.argtypes = [P]
     lib.dvx_trim.argtypes = [P, C.POINTER(C.c_uint64)]
     lib.dvx_microbench_fma.argtypes = [P, C.c_uint32, C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_float)]
     lib.dvx_set_record_budget.argtypes = [P, C.c_uint64]
@@ -215,13 +216,17 @@ class Context:
         ms = (C.c_float * 8)()
         n = C.c_uint32()
         self.check(self.lib.dvx_stage_ms_collect(self.h, ms, C.byref(n)))
-        return dict(zip(STAGES, list(ms)[:6])), n.value
+        return dict(zip(STAGES, list(ms)[:8])), n.value
 
     def microbench_fma(self, iters=1 << 14):
         """dvx_microbench_fma -> dict(lane_fma_per_s, warp_instr_per_s, ms)."""
         a, b, ms = C.c_double(), C.c_double(), C.c_float()
         self.check(self.lib.dvx_microbench_fma(self.h, iters, C.byref(a), C.byref(b), C.byref(ms)))
         return {"lane_fma_per_s": a.value, "warp_instr_per_s": b.value, "ms": ms.value}
+
+    def host_io_wait(self):
+        """dvx_host_io_wait: the context's stream waits for every host copy-out still in flight."""
+        self.check(self.lib.dvx_host_io_wait(self.h))
 
     def trim(self):
         """dvx_trim: hand every cached scratch block back to the allocator -> bytes freed."""
@@ -581,7 +586,7 @@ class Frame:
         ctx = self.ctx
         ms = (C.c_float * 8)()
         ctx.check(ctx.lib.dvx_frame_stage_ms(ctx.h, self.h, ms))
-        return dict(zip(("preprocess", "sort", "composite", "backward", "backward_composite", "backward_sh"), list(ms)[:6]))
+        return dict(zip(STAGES, list(ms)[:8]))
 
     def release(self):
         if self.h and self.ctx.h:

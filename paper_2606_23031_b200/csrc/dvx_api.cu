@@ -32,9 +32,10 @@ struct dvx_ctx {
   std::string err;
   // host-buffer entry points: a second stream moves the images while the main stream computes
   cudaStream_t cs = nullptr, cs_in = nullptr;  // copy-out and copy-in streams (one per direction: both overlap compute)
-  cudaEvent_t ev_main = nullptr, ev_d2h = nullptr, ev_h2d = nullptr, ev_bwd = nullptr;
-  float *st_out = nullptr, *st_in = nullptr;  // persistent device staging (grow-only)
-  size_t st_out_bytes = 0, st_in_bytes = 0;
+  cudaEvent_t ev_main = nullptr, ev_d2h[2] = {nullptr, nullptr}, ev_h2d = nullptr, ev_bwd = nullptr;
+  float *st_out[2] = {nullptr, nullptr}, *st_in = nullptr;  // persistent device staging (grow-only); the copy-out is double-buffered
+  size_t st_out_bytes[2] = {0, 0}, st_in_bytes = 0;
+  int out_idx = 0;  // staging buffer of the latest dvx_render_host
   // hit-record pool sizing: chunks per pixel used by the last frames (read back lazily, never waited for)
   uint64_t rec_budget = 0;             // dvx_set_record_budget: bytes per frame, 0 = automatic
   static constexpr int REC_SLOTS = 16;
@@ -287,7 +288,7 @@ void dvx_destroy(dvx_ctx *ctx) {
     cudaStreamSynchronize(ctx->cs_in);
     cudaStreamDestroy(ctx->cs);
     cudaStreamDestroy(ctx->cs_in);
-    cudaEventDestroy(ctx->ev_main); cudaEventDestroy(ctx->ev_d2h); cudaEventDestroy(ctx->ev_h2d); cudaEventDestroy(ctx->ev_bwd);
+    cudaEventDestroy(ctx->ev_main); cudaEventDestroy(ctx->ev_d2h[0]); cudaEventDestroy(ctx->ev_d2h[1]); cudaEventDestroy(ctx->ev_h2d); cudaEventDestroy(ctx->ev_bwd);
   }
   for (auto *v : {&ctx->ev_free, &ctx->ev_pending})
     for (EventSet *es : *v) {
@@ -942,10 +943,12 @@ dvx_status dvx_frame_stage_ms(dvx_ctx *ctx, const dvx_frame *f, float *ms) {
   CU(cudaEventElapsedTime(&ms[0], f->ev[0], f->ev[1]));
   CU(cudaEventElapsedTime(&ms[1], f->ev[2], f->ev[3]));
   CU(cudaEventElapsedTime(&ms[2], f->ev[9], f->ev[4]));
+  CU(cudaEventElapsedTime(&ms[6], f->ev[1], f->ev[2]));
   if (f->did_backward) {
     CU(cudaEventElapsedTime(&ms[3], f->ev[5], f->ev[6]));
     CU(cudaEventElapsedTime(&ms[4], f->ev[7], f->ev[8]));
     CU(cudaEventElapsedTime(&ms[5], f->ev[8], f->ev[6]));
+    CU(cudaEventElapsedTime(&ms[7], f->ev[4], f->ev[5]));
   }
   return DVX_OK;
 }
@@ -957,10 +960,10 @@ dvx_status dvx_stage_ms_collect(dvx_ctx *ctx, float *ms, uint32_t *n_frames) {
   CU(cudaStreamSynchronize(ctx->st));
   for (int i = 0; i < 8; ++i) ms[i] = 0.f;
   *n_frames = (uint32_t)ctx->ev_pending.size();
-  static const int pairs[6][2] = {{0, 1}, {2, 3}, {9, 4}, {5, 6}, {7, 8}, {8, 6}};
+  static const int pairs[8][2] = {{0, 1}, {2, 3}, {9, 4}, {5, 6}, {7, 8}, {8, 6}, {1, 2}, {4, 5}};
   for (EventSet *es : ctx->ev_pending) {
-    for (int i = 0; i < 6; ++i) {
-      if (i >= 3 && !es->did_backward) break;
+    for (int i = 0; i < 8; ++i) {
+      if ((i >= 3 && i != 6) && !es->did_backward) continue;
       float t = 0.f;
       if (cudaEventElapsedTime(&t, es->ev[pairs[i][0]], es->ev[pairs[i][1]]) == cudaSuccess) ms[i] += t;
       else cudaGetLastError();
@@ -1008,7 +1011,7 @@ dvx_status host_io_setup(dvx_ctx *ctx, float **buf, size_t *have, size_t need) {
   if (!ctx->cs) {
     CU(cudaStreamCreateWithFlags(&ctx->cs, cudaStreamNonBlocking));
     CU(cudaStreamCreateWithFlags(&ctx->cs_in, cudaStreamNonBlocking));
-    for (cudaEvent_t *e : {&ctx->ev_main, &ctx->ev_d2h, &ctx->ev_h2d, &ctx->ev_bwd}) CU(cudaEventCreateWithFlags(e, cudaEventDisableTiming));
+    for (cudaEvent_t *e : {&ctx->ev_main, &ctx->ev_d2h[0], &ctx->ev_d2h[1], &ctx->ev_h2d, &ctx->ev_bwd}) CU(cudaEventCreateWithFlags(e, cudaEventDisableTiming));
   }
   if (*have < need) {
     CU(cudaStreamSynchronize(ctx->cs));  // nothing in flight may still use the old buffer
@@ -1031,23 +1034,35 @@ dvx_status dvx_render_host(dvx_ctx *ctx, const dvx_camera *cam, const dvx_octree
   if (!cam || !out_host.rgb || !out_host.depth || !out_host.alpha) return fail(ctx, DVX_ERR_INVALID_ARG, "NULL argument");
   cudaSetDevice(ctx->device);
   const size_t npix = (size_t)cam->width * cam->height;
-  dvx_status rc = host_io_setup(ctx, &ctx->st_out, &ctx->st_out_bytes, npix * 32);
+  // two staging buffers, used in turn: frame i+1 renders into the other one while frame i's copy-out is still on the bus
+  // (with one buffer the next frame waited for it: 41 MB per 1920x1080 frame take longer than the backward they hide under)
+  const int k = ctx->out_idx ^= 1;
+  dvx_status rc = host_io_setup(ctx, &ctx->st_out[k], &ctx->st_out_bytes[k], npix * 32);
   if (rc != DVX_OK) return rc;
-  float *stage = ctx->st_out;
+  float *stage = ctx->st_out[k];
   dvx_image dev = {stage, stage + 3 * npix, stage + 4 * npix, out_host.normal ? stage + 5 * npix : nullptr};
-  CU(cudaStreamWaitEvent(ctx->st, ctx->ev_d2h, 0));  // the previous frame's copy-out must have left the staging buffer
+  CU(cudaStreamWaitEvent(ctx->st, ctx->ev_d2h[k], 0));  // the copy-out of the frame before last must have left this buffer
   rc = dvx_render(ctx, cam, static_tree, n_actors, actors, poses_l2w, box_half, opts, dev, saved);
   if (rc != DVX_OK) return rc;
-  // copy-out on the copy stream: it overlaps whatever the main stream does next (the backward of this frame)
+  // copy-out on the copy stream: it overlaps whatever the main stream does next (this frame's backward, the next frame)
   CU(cudaEventRecord(ctx->ev_main, ctx->st));
   CU(cudaStreamWaitEvent(ctx->cs, ctx->ev_main, 0));
   CU(cudaMemcpyAsync(out_host.rgb, dev.rgb, npix * 12, cudaMemcpyDeviceToHost, ctx->cs));
   CU(cudaMemcpyAsync(out_host.depth, dev.depth, npix * 4, cudaMemcpyDeviceToHost, ctx->cs));
   CU(cudaMemcpyAsync(out_host.alpha, dev.alpha, npix * 4, cudaMemcpyDeviceToHost, ctx->cs));
   if (dev.normal) CU(cudaMemcpyAsync(out_host.normal, dev.normal, npix * 12, cudaMemcpyDeviceToHost, ctx->cs));
-  CU(cudaEventRecord(ctx->ev_d2h, ctx->cs));
+  CU(cudaEventRecord(ctx->ev_d2h[k], ctx->cs));
   // inference (nothing saved): the caller's next synchronisation of the main stream must cover the copies
-  if (!saved) CU(cudaStreamWaitEvent(ctx->st, ctx->ev_d2h, 0));
+  if (!saved) CU(cudaStreamWaitEvent(ctx->st, ctx->ev_d2h[k], 0));
+  return DVX_OK;
+}
+
+dvx_status dvx_host_io_wait(dvx_ctx *ctx) {
+  if (!ctx) return DVX_ERR_INVALID_ARG;
+  if (!ctx->cs) return DVX_OK;  // no host-buffer call yet
+  cudaSetDevice(ctx->device);
+  CU(cudaStreamWaitEvent(ctx->st, ctx->ev_d2h[0], 0));
+  CU(cudaStreamWaitEvent(ctx->st, ctx->ev_d2h[1], 0));
   return DVX_OK;
 }
 
@@ -1071,7 +1086,6 @@ dvx_status dvx_backward_host(dvx_ctx *ctx, dvx_frame *f, const float *g_rgb_h, c
   CU(cudaStreamWaitEvent(ctx->st, ctx->ev_h2d, 0));
   rc = dvx_backward(ctx, f, d_rgb, d_depth, d_alpha, static_grad, actor_grads);
   CU(cudaEventRecord(ctx->ev_bwd, ctx->st));
-  CU(cudaStreamWaitEvent(ctx->st, ctx->ev_d2h, 0));  // a main-stream synchronisation after this call also covers the copy-out
   return rc;
 }
 
