@@ -643,18 +643,12 @@ dvx_status render_step34(dvx_ctx *ctx, dvx_frame *f, const dvx_image &out, bool 
   return DVX_OK;
 }
 
-#ifndef DVX_BATCH_OVERLAP
-#define DVX_BATCH_OVERLAP 1  // 0: the batched calls keep everything on the context's stream (only the host round trips are merged)
-#endif
-#ifndef DVX_BATCH_PRIO
-#define DVX_BATCH_PRIO 1     // 1: the second stream has the highest priority, 0: the default one
-#endif
 // Library-owned second stream for the batched entry points, and its pinned counter slots.
 dvx_status batch_setup(dvx_ctx *ctx, uint32_t n) {
   if (!ctx->ps) {
     int lo = 0, hi = 0;
     CU(cudaDeviceGetStreamPriorityRange(&lo, &hi));
-    CU(cudaStreamCreateWithPriority(&ctx->ps, cudaStreamNonBlocking, DVX_BATCH_PRIO ? hi : lo));
+    CU(cudaStreamCreateWithPriority(&ctx->ps, cudaStreamNonBlocking, hi));  // highest priority: its small kernels slip in between the compositing CTAs
     CU(cudaEventCreateWithFlags(&ctx->ev_entry, cudaEventDisableTiming));
   }
   if (ctx->h_batch_n < n) {
@@ -722,7 +716,7 @@ dvx_status dvx_render_batch(dvx_ctx *ctx, uint32_t n_cams, const dvx_camera *cam
     ~FreeAll() { for (dvx_frame *f : v) if (f) frame_free(ctx, f); }
   } free_all{ctx, fr};
   // the second stream starts after whatever the caller has enqueued on the context's stream (inputs, the previous step)
-  cudaStream_t side = DVX_BATCH_OVERLAP ? ctx->ps : ctx->st;
+  cudaStream_t side = ctx->ps;
   CU(cudaEventRecord(ctx->ev_entry, ctx->st));
   CU(cudaStreamWaitEvent(side, ctx->ev_entry, 0));
   for (uint32_t c = 0; c < n_cams; ++c) {
@@ -841,7 +835,7 @@ dvx_status dvx_backward_batch(dvx_ctx *ctx, uint32_t n_frames, dvx_frame *const 
   // every frame's dL/drgb_v scratch stays allocated until the second stream has been joined below: a block handed back
   // earlier could be given to the next frame's replay while this frame's post-pass still reads it
   CallGuard hold(ctx);
-  cudaStream_t side = DVX_BATCH_OVERLAP ? ctx->ps : ctx->st;
+  cudaStream_t side = ctx->ps;
   CU(cudaEventRecord(ctx->ev_entry, ctx->st));
   CU(cudaStreamWaitEvent(side, ctx->ev_entry, 0));
   for (uint32_t c = 0; c < n_frames && rc == DVX_OK; ++c) {

@@ -28,32 +28,17 @@
 
 namespace {
 
-#ifndef DVX_TILE_SPLIT
-#define DVX_TILE_SPLIT 2  // CTAs per 16x16 tile (1, 2, 4 or 8): a CTA holds 8 / DVX_TILE_SPLIT of the tile's warps.  Measured on
+constexpr int DVX_TILE_SPLIT = 2;  // CTAs per 16x16 tile (1, 2, 4 or 8): a CTA holds 8 / DVX_TILE_SPLIT of the tile's warps.  Measured on
                           // B200, step ms for 1 / 2 / 4: config 3 4.00 / 3.92 / 3.98, config 4 5.32 / 5.25 / 5.32 (finer tail)
-#endif
 constexpr int TILE_SPLIT = DVX_TILE_SPLIT;
 constexpr int TILE_THREADS = 256 / TILE_SPLIT;
 constexpr int TILE_WARPS = TILE_THREADS / 32;
-#ifndef DVX_TILE_MIN_CTAS
-#define DVX_TILE_MIN_CTAS (3 * DVX_TILE_SPLIT)
-#endif
-#ifndef DVX_RUN_SPLIT
-#define DVX_RUN_SPLIT 4  // backward: runs of one voxel are reduced in pieces of at most this many lanes (1, 2, 8, 16, 32 measured slower)
-#endif
-#ifndef DVX_RUN_LONG
-#define DVX_RUN_LONG 32  // ... unless the batch averages at least this many lanes per run (32: the whole batch is ONE voxel): then the run is reduced whole
-#endif
-#ifndef DVX_CAND_GROUPS
-#define DVX_CAND_GROUPS 8  // phase A: bands of rows of the warp's pixel block that walk their candidates independently.  Forward
+constexpr int DVX_TILE_MIN_CTAS = (3 * DVX_TILE_SPLIT);
+constexpr int DVX_RUN_SPLIT = 4;  // backward: runs of one voxel are reduced in pieces of at most this many lanes (1, 2, 8, 16, 32 measured slower)
+constexpr int DVX_RUN_LONG = 32;  // ... unless the batch averages at least this many lanes per run (32: the whole batch is ONE voxel): then the run is reduced whole
+constexpr int DVX_CAND_GROUPS = 8;  // phase A: bands of rows of the warp's pixel block that walk their candidates independently.  Forward
                            // compositing of a saved frame, config 3 / config 4, ms, for 1, 2, 4, 8 bands: 1.378 1.377 1.354 1.312 / 1.934 1.943 1.935 1.888
-#endif
-#ifndef DVX_STAGE_PREFETCH
-#define DVX_STAGE_PREFETCH 1
-#endif
-#ifndef DVX_WARP_W
-#define DVX_WARP_W 4   // a warp covers DVX_WARP_W x (32 / DVX_WARP_W) pixels
-#endif
+constexpr int DVX_WARP_W = 4;  // a warp covers DVX_WARP_W x (32 / DVX_WARP_W) pixels
 constexpr int WARP_W = DVX_WARP_W, WARP_H = 32 / DVX_WARP_W, WARPS_X = DVX_TILE / WARP_W;
 constexpr int QCAP = 64;              // ring capacity per warp: at most 31 left-over items + 32 of one entry
 constexpr uint32_t NONE = 0xFFFFFFFFu;
@@ -768,38 +753,26 @@ __global__ void __launch_bounds__(TILE_THREADS, DVX_TILE_MIN_CTAS) composite_til
       if (t == 0 && cur0 != NONE) c_l = cur0;
       uint32_t c_t = (part && q == qq) ? c_l : NONE;  // first entry this pixel still tests; NONE = not (or no longer) walking
       uint32_t pos = warp_min_u32(c_t);
-#if DVX_STAGE_PREFETCH
       // the id of this lane's entry of the NEXT round is loaded one round ahead, and an entry's pixel rectangle and code are
       // loaded together (the code of an entry that fails the rectangle test is wasted, 8 bytes from L2): one exposed load
       // latency per round of 32 entries instead of three dependent ones
       uint32_t id_next = pos + lane < end ? __ldg(A.ids + pos + lane) : 0u;
-#endif
       while (pos < end && __any_sync(0xffffffffu, c_t != NONE)) {
         const uint32_t n = min(32u, end - pos);
         // -- lane = entry: pre-filter and fp64 centre decomposition
         bool c = false;
         uint32_t ry0 = 1u, ry1 = 0u;  // rows of the entry's pixel rectangle
-#if DVX_STAGE_PREFETCH
         const uint32_t id_cur = id_next;
         if (pos + 32u + lane < end) id_next = __ldg(A.ids + pos + 32u + lane);
-#endif
         if ((uint32_t)lane < n) {
-#if DVX_STAGE_PREFETCH
           const uint32_t id = id_cur;
           const uint64_t code_v = __ldg(T.code + (id - T.base));
-#else
-          const uint32_t id = __ldg(A.ids + pos + lane);
-#endif
           const ushort4 rc = __ldg(A.pxrect + id);
           c = rc.x <= ru1 && rc.z >= ru0 && rc.y <= rv1 && rc.w >= rv0;
           ry0 = rc.y; ry1 = rc.w;
           if (c) {
             uint32_t X, Y, Z, lv;
-#if DVX_STAGE_PREFETCH
             dvx_decode16(code_v, X, Y, Z, lv);
-#else
-            dvx_decode16(__ldg(T.code + (id - T.base)), X, Y, Z, lv);
-#endif
             const uint32_t size = 1u << (DVX_MAX_LEVEL - lv);
             const double hc = 0.5 * T.cell;
             const double d0x = Q.d0[0], d0y = Q.d0[1], d0z = Q.d0[2];
@@ -816,15 +789,6 @@ __global__ void __launch_bounds__(TILE_THREADS, DVX_TILE_MIN_CTAS) composite_til
             Q.ent[lane] = rec;
           }
         }
-#if DVX_CAND_GROUPS == 1
-        uint32_t cand = __ballot_sync(0xffffffffu, c);
-        __syncwarp();
-        // -- lane = pixel
-        while (cand) {
-          const int j = __ffs(cand) - 1;
-          cand &= cand - 1;
-          const bool act = true;
-#else
         // The warp's 4x8 pixel block is cut into DVX_CAND_GROUPS bands of rows; every band walks its own candidates (the
         // entries whose pixel rectangle reaches into the band), so one trip of the loop below tests up to DVX_CAND_GROUPS
         // different entries.  A pixel still meets its entries in list order, and items are queued in (trip, lane) order,
@@ -844,7 +808,6 @@ __global__ void __launch_bounds__(TILE_THREADS, DVX_TILE_MIN_CTAS) composite_til
           const bool act = cand != 0u;
           const int j = act ? __ffs(cand) - 1 : 0;
           cand &= cand - 1;
-#endif
           const uint32_t ei = pos + j;
           const float4 r0 = *reinterpret_cast<const float4 *>(&Q.ent[j]);          // t0, m0
           const uint4 r1 = *(reinterpret_cast<const uint4 *>(&Q.ent[j]) + 1);      // id, meta, hs
@@ -940,9 +903,7 @@ __global__ void __launch_bounds__(TILE_THREADS, DVX_TILE_MIN_CTAS) composite_til
 // loads the records (three coalesced loads, the next batch prefetched under the current one), integrates with moments
 // (phase B), replays the pixels' blend order (phase C) and reduces the gradients (phase B2).
 // Same grid and warp -> pixel-block mapping as the forward.
-#ifndef DVX_REPLAY_MIN_CTAS
-#define DVX_REPLAY_MIN_CTAS 7   // 72 registers, no spills; config 3 replay ms at 6 / 7 / 8 CTAs per SM: 1.272 / 1.189 / 1.207 (config 4: 2.114 / 1.996 / 2.045)
-#endif
+constexpr int DVX_REPLAY_MIN_CTAS = 7;  // 72 registers, no spills; config 3 replay ms at 6 / 7 / 8 CTAs per SM: 1.272 / 1.189 / 1.207 (config 4: 2.114 / 1.996 / 2.045)
 struct RecBatch {
   uint4 a;      // id, meta, delta, mid
   float4 b;     // p, q_x

@@ -149,12 +149,7 @@ struct GridWriteBatch {   // second pass of the grid step: thread = voxel
   int n;
 };
 
-#ifndef DVX_GA_TWO_PASS
-#define DVX_GA_TWO_PASS 1
-#endif
-#ifndef DVX_GA_MINB
-#define DVX_GA_MINB 8  // 32 registers, 64 warps per SM: the kernel waits on scattered 4-byte accesses
-#endif
+constexpr int DVX_GA_MINB = 8;  // 32 registers, 64 warps per SM: the kernel waits on scattered 4-byte accesses
 __global__ void __launch_bounds__(GRID_THREADS, DVX_GA_MINB) grid_adam_kernel(const __grid_constant__ AdamConst h,
                                                                  const __grid_constant__ GridAdamBatch B) {
   int e = 0;
@@ -180,14 +175,6 @@ __global__ void __launch_bounds__(GRID_THREADS, DVX_GA_MINB) grid_adam_kernel(co
   B.density[e][p] = pv;
   B.m[e][p] = mv;
   B.v[e][p] = vv;
-#if !DVX_GA_TWO_PASS
-#pragma unroll
-  for (int i = 0; i < 8; ++i)
-    if (sl[i] != 0xFFFFFFFFu) {
-      geo[sl[i]] = pv;
-      dgeo[sl[i]] = 0.f;
-    }
-#endif
 }
 
 // Second pass (thread = voxel): the 32-byte corner record the next forward reads is rebuilt from the grid-point densities
@@ -331,7 +318,6 @@ void dvx_grid_adam_launch(float lr, float beta1, float beta2, float eps, uint32_
     B.block_start[B.n] = blocks;
     DVX_COUNT_LAUNCH(1);
     grid_adam_kernel<<<blocks, GRID_THREADS, 0, st>>>(h, B);
-#if DVX_GA_TWO_PASS
     GridWriteBatch Wb;
     memset(&Wb, 0, sizeof(Wb));
     uint32_t wblocks = 0;
@@ -345,7 +331,6 @@ void dvx_grid_adam_launch(float lr, float beta1, float beta2, float eps, uint32_
     }
     Wb.block_start[Wb.n] = wblocks;
     if (wblocks) { DVX_COUNT_LAUNCH(1); grid_write_kernel<<<wblocks, GRID_THREADS, 0, st>>>(Wb); }
-#endif
   }
 }
 void dvx_adam_launch(float lr, float beta1, float beta2, float eps, uint32_t step, uint32_t n, const DvxAdamItem *items,

@@ -188,10 +188,8 @@ __device__ __forceinline__ uint32_t count_pairs_warp(const FrameParams &p, const
   return c;
 }
 
+constexpr int DVX_PRE_MIN_CTAS = 5;  // 48 registers, no spills; config 3 step-1 ms for 4 / 5 / 6 CTAs per SM: 0.203 / 0.199 / 0.203
 template <bool NRM>
-#ifndef DVX_PRE_MIN_CTAS
-#define DVX_PRE_MIN_CTAS 5  // 48 registers, no spills; config 3 step-1 ms for 4 / 5 / 6 CTAs per SM: 0.203 / 0.199 / 0.203
-#endif
 __global__ void __launch_bounds__(PRE_THREADS, DVX_PRE_MIN_CTAS) preprocess_kernel(FrameParams p, const TreeFrame *trees,
                                                                  const uint8_t *octmask, FrameVox *fvox,
                                                                  ushort4 *pxrect, float4 *vnrm,

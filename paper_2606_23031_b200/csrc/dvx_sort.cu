@@ -12,16 +12,12 @@
 namespace {
 
 constexpr int SORT_THREADS = 256;
-#ifndef DVX_SORT_ITEMS
-#define DVX_SORT_ITEMS 12  // keys per thread: 3072-key tiles (45 KB of shared memory, 3 CTAs per SM). Config 3 sort stage ms for 6 / 8 / 12: 0.381 / 0.353 / 0.341
-#endif
+constexpr int DVX_SORT_ITEMS = 12;  // keys per thread: 3072-key tiles (45 KB of shared memory, 3 CTAs per SM). Config 3 sort stage ms for 6 / 8 / 12: 0.381 / 0.353 / 0.341
 constexpr int SORT_ITEMS = DVX_SORT_ITEMS;
 constexpr int SORT_TILE = SORT_THREADS * SORT_ITEMS;   // 3072 keys per block
 constexpr int SORT_WARPS = SORT_THREADS / 32;
 constexpr int RADIX = 256;
-#ifndef DVX_SORT_LOOK
-#define DVX_SORT_LOOK 4  // measured on config 3 (6 passes over 2.9 M pairs), sort stage ms for 1 / 4 / 8 / 16: 0.386 / 0.356 / 0.359 / 0.378
-#endif
+constexpr int DVX_SORT_LOOK = 4;  // measured on config 3 (6 passes over 2.9 M pairs), sort stage ms for 1 / 4 / 8 / 16: 0.386 / 0.356 / 0.359 / 0.378
 // Payload loads are issued with the key loads.  Same box, config 3 sort stage ms: look-back 1 wide 0.446, 4 wide 0.395,
 // 4 wide + early payload loads 0.351, + 3072-key tiles 0.341.
 constexpr int SORT_LOOK = DVX_SORT_LOOK;  // one-sweep look-back: predecessor tiles read per round trip
@@ -120,9 +116,7 @@ __global__ void __launch_bounds__(RADIX) radix_digit_scan(uint32_t *ghist) {
   g[threadIdx.x] = ex;
 }
 
-#ifndef DVX_SORT_MIN_CTAS
-#define DVX_SORT_MIN_CTAS 3  // register cap with the payload loads issued early (12 keys per thread at 4 CTAs per SM: 0.363 ms)
-#endif
+constexpr int DVX_SORT_MIN_CTAS = 3;  // register cap with the payload loads issued early (12 keys per thread at 4 CTAs per SM: 0.363 ms)
 __global__ void __launch_bounds__(SORT_THREADS, DVX_SORT_MIN_CTAS) radix_onesweep(const uint64_t *__restrict__ keys_in,
                                                                 const uint32_t *__restrict__ vals_in,
                                                                 uint64_t *__restrict__ keys_out, uint32_t *__restrict__ vals_out,
