@@ -661,6 +661,8 @@ def run_dvx(args):
                      "achieved_with_records": (dom_bytes + rec_bytes) / (dom_ms * 1e-3) / 1e9 if dom_ms > 0 else 0.0,
                      "frac_with_records": (dom_bytes + rec_bytes) / (dom_ms * 1e-3) / 1e9 / peak if (dom_ms > 0 and peak) else None,
                      "traffic": (pk.get(dom) or {}).get("dram_bytes"), "traffic_commit": prof.get("commit"),
+                     "traffic_note": "traffic above the algorithmic bytes is the hit-record stream (44 B per composited hit, written by "
+                                     "the forward, read by the backward instead of re-walking the tile lists; DESIGN.md section 6), not re-reads",
                      "traffic_stale": bool(stale), "peak_source": peak_src, "bytes_per_launch": dom_bytes, "ms_per_launch": dom_ms,
                      "all_kernels_ms": kernels},
         "issue_roofline": dict(issue, bound="alu", unit="warp-instr/s", profile_commit=prof.get("commit"), profile_stale=bool(stale)),
