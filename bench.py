@@ -216,10 +216,10 @@ def _bits_for(n):
 
 def sort_throughput(ctx, n_pairs, scene, W, H, reps=5):
     """Step 2's radix sort alone (dvx_sort_pairs: the same kernels dvx_render runs), on as many seeded random pairs as one
-    frame produces, with the frame's key width (tile | tree | octant | rank).  Mpairs/s, CUDA events, median of reps."""
+    frame produces, with the frame's key width (tile | octant | combined rank of all octrees).  Mpairs/s, CUDA events, median of reps."""
     import torch
     n_tiles = ((W + 15) // 16) * ((H + 15) // 16)
-    key_bits = _bits_for(max(t.n_voxels for t in scene.octrees)) + _bits_for(n_tiles * len(scene.octrees) * 8)
+    key_bits = _bits_for(sum(t.n_voxels for t in scene.octrees)) + _bits_for(n_tiles * 8)   # combined rank | tile, octant
     n = max(int(n_pairs), 1)
     g = torch.Generator(device="cuda").manual_seed(1)
     base = torch.randint(0, 1 << min(key_bits, 62), (n,), dtype=torch.int64, device="cuda", generator=g)

@@ -495,18 +495,17 @@ dvx_status render_step1(dvx_ctx *ctx, const dvx_camera *cam, const dvx_octree *s
   p.k_samples = o.k_samples; p.activation = o.activation; p.flags = o.flags; p.t_stop = o.t_stop;
   p.inv_k = 1.0f / (float)o.k_samples;
   f->trees_h.resize(p.n_trees);
-  uint64_t vtot = 0, vmax = 1;
+  uint64_t vtot = 0;
   for (uint32_t t = 0; t < p.n_trees; ++t) {
     const dvx_octree *tr = t == 0 ? static_tree : actors[t - 1];
     setup_tree(f->trees_h[t], tr, (uint32_t)vtot, t > 0, t ? poses_l2w + 12 * (t - 1) : nullptr,
                t ? box_half + 3 * (t - 1) : nullptr, cam);
     vtot += tr->d.n_voxels;
-    if (tr->d.n_voxels > vmax) vmax = tr->d.n_voxels;
   }
   if ((uint64_t)p.n_tiles * 8u >= (1u << 24)) return fail(ctx, DVX_ERR_INVALID_ARG, "image too large (more than 2^21 tiles)");
   if (vtot >= 0xFFFFFFFFull) return fail(ctx, DVX_ERR_INVALID_ARG, "more than 2^32-2 voxels in total");
   p.v_total = (uint32_t)vtot;
-  p.rank_bits = bits_for(vmax);
+  p.rank_bits = bits_for(vtot > 1 ? vtot : 1);   // combined rank space of all octrees (see emit_pairs_kernel)
   p.n_buckets = p.n_tiles * p.n_trees * 8u;
   const size_t npix = (size_t)p.width * p.height;
 
@@ -562,7 +561,7 @@ dvx_status render_step2(dvx_ctx *ctx, dvx_frame *f, cudaStream_t st) {
   f->n_pairs = f->h_cnt[CNT_PAIRS];
   f->v_vis = f->h_cnt[CNT_VVIS];
   if (f->n_pairs >= (1ull << 30)) return fail(ctx, DVX_ERR_INVALID_ARG, "2^30 or more (tile, octant, voxel) pairs");
-  const uint32_t key_bits = p.rank_bits + bits_for(p.n_buckets);
+  const uint32_t key_bits = p.rank_bits + bits_for((uint64_t)p.n_tiles * 8u);
   TreeFrame *trees_d = (TreeFrame *)f->trees_d.p;
   unsigned long long *counters = (unsigned long long *)f->counters.p;
   CallGuard guard(ctx);
@@ -577,7 +576,7 @@ dvx_status render_step2(dvx_ctx *ctx, dvx_frame *f, cudaStream_t st) {
   CU(cudaMemsetAsync(f->range_beg.p, 0, sizeof(uint32_t) * (size_t)p.n_buckets, st));
   CU(cudaMemsetAsync(f->range_end.p, 0, sizeof(uint32_t) * (size_t)p.n_buckets, st));
   CU(cudaMemsetAsync(f->tile_cost.p, 0, sizeof(uint32_t) * (size_t)p.n_tiles, st));
-  dvx_ranges_launch(which ? kb : ka, P, p.rank_bits, p.n_trees * 8u, (uint32_t *)f->range_beg.p, (uint32_t *)f->range_end.p,
+  dvx_ranges_launch(which ? kb : ka, P, p.rank_bits, trees_d, p.n_trees, (uint32_t *)f->range_beg.p, (uint32_t *)f->range_end.p,
                     (uint32_t *)f->tile_cost.p, st);
   dvx_tile_order_launch((const uint32_t *)f->tile_cost.p, p.n_tiles, (uint32_t *)f->tile_order.p, st);
   CU(cudaEventRecord(f->ev[3], st));

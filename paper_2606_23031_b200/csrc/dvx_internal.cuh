@@ -40,7 +40,7 @@ struct FrameParams {
   double Rc[9];                       // camera rotation (row-major, camera -> world): world direction of a pixel (sky)
   uint32_t k_samples, activation, flags;
   float t_stop, inv_k;  // inv_k = 1 / k_samples
-  uint32_t rank_bits;   // sort key = (bucket << rank_bits) | rank ; bucket = (tile*n_trees + tree)*8 + octant
+  uint32_t rank_bits;   // sort key = ((tile*8 + octant) << rank_bits) | (tree base + rank); rank_bits = bits_for(v_total)
   uint32_t v_total;     // sum of n_voxels
   uint32_t n_buckets;   // n_tiles * n_trees * 8
 };
@@ -140,8 +140,8 @@ void dvx_normal_backward_launch(const FrameParams &p, const TreeFrame *trees, co
 void dvx_emit_pairs_launch(const FrameParams &p, const TreeFrame *trees, const uint8_t *octmask, const ushort4 *pxrect,
                            const FrameVox *fvox, uint64_t *keys, uint32_t *vals, unsigned long long capacity,
                            unsigned long long *counters, cudaStream_t st);
-void dvx_ranges_launch(const uint64_t *keys, uint64_t n, uint32_t rank_bits, uint32_t buckets_per_tile, uint32_t *range_beg,
-                       uint32_t *range_end, uint32_t *tile_cost, cudaStream_t st);
+void dvx_ranges_launch(const uint64_t *keys, uint64_t n, uint32_t rank_bits, const TreeFrame *trees, uint32_t n_trees,
+                       uint32_t *range_beg, uint32_t *range_end, uint32_t *tile_cost, cudaStream_t st);
 void dvx_tile_order_launch(const uint32_t *tile_cost, uint32_t n_tiles, uint32_t *tile_order /* [2 n_tiles] */, cudaStream_t st);
 void dvx_sh_backward_launch(const FrameParams &p, const TreeFrame *trees, const FrameVox *fvox, const ushort4 *pxrect,
                             const float *drgb, cudaStream_t st);

@@ -280,7 +280,11 @@ __global__ void __launch_bounds__(PRE_THREADS, DVX_PRE_MIN_CTAS) preprocess_kern
 }
 
 // ------------------------------------------------------------------ step 2: key generation
-// key = (bucket << rank_bits) | rank_q(v), bucket = (tile*n_trees + tree)*8 + q; value = global voxel id.
+// key = ((tile * 8 + q) << rank_bits) | (base_tree + rank_q(v)); value = global voxel id.  The octree is not a key field of
+// its own: base_tree (the octree's first global voxel id) puts the ranks of all octrees into one number space of
+// bits_for(v_total) bits, so the key is tile | octant | combined rank = 39 bits for config 3 (5 radix passes) instead of
+// tile | tree | octant | rank = 42 (6 passes).  Within a tile the sorted order is (octant, tree, rank); every
+// (tile, tree, octant) bucket is still one contiguous run, found by ranges_kernel.
 // Every key is unique, so the order in which pairs are emitted does not matter: slots are handed out with one
 // warp-aggregated atomic per warp from the per-voxel pair counts step 1 left in fvox.meta.  Voxels with a large
 // footprint are emitted by the whole warp, 32 tiles per step.
@@ -289,8 +293,7 @@ __device__ __forceinline__ void emit_tile(const FrameParams &p, const TreeFrame 
   while (m) {
     const int q = __ffs(m) - 1;
     m &= m - 1;
-    const uint64_t bucket = ((uint64_t)tile * p.n_trees + t) * 8u + q;
-    keys[pos] = (bucket << p.rank_bits) | (uint64_t)__ldg(T.rank + (size_t)q * T.n_voxels + v);
+    keys[pos] = (((uint64_t)tile * 8u + q) << p.rank_bits) | (uint64_t)(T.base + __ldg(T.rank + (size_t)q * T.n_voxels + v));
     vals[pos] = g;
     ++pos;
   }
@@ -374,18 +377,37 @@ __global__ void __launch_bounds__(PRE_THREADS) emit_pairs_kernel(FrameParams p, 
   }
 }
 
-// range[bucket] = [begin, end) in the sorted pair array, by boundary detection (buffers pre-zeroed: empty = [0,0)).
+// range[bucket] = [begin, end) in the sorted pair array, by boundary detection (buffers pre-zeroed: empty = [0,0)); bucket =
+// (tile * n_trees + tree) * 8 + octant, with the tree recovered from the combined rank by a search over the trees' bases.
 // tile_cost[tile] (pre-zeroed) receives the tile's pair count as sum(end) - sum(begin) over its buckets, in u32 arithmetic.
-__global__ void ranges_kernel(const uint64_t *keys, uint64_t n, uint32_t rank_bits, uint32_t buckets_per_tile,
+__device__ __forceinline__ uint32_t bucket_of(uint64_t key, uint32_t rank_bits, const uint32_t *s_base, int n_trees) {
+  const uint32_t tq = (uint32_t)(key >> rank_bits), comb = (uint32_t)(key & ((1ull << rank_bits) - 1ull));
+  int lo = 0, hi = n_trees - 1;       // last tree whose base <= comb
+  while (lo < hi) {
+    const int mid = (lo + hi + 1) >> 1;
+    if (s_base[mid] <= comb) lo = mid; else hi = mid - 1;
+  }
+  return ((tq >> 3) * (uint32_t)n_trees + (uint32_t)lo) * 8u + (tq & 7u);
+}
+__global__ void ranges_kernel(const uint64_t *keys, uint64_t n, uint32_t rank_bits, const TreeFrame *trees, uint32_t n_trees,
                               uint32_t *range_beg, uint32_t *range_end, uint32_t *tile_cost) {
-  uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= n) return;
-  uint64_t b = keys[i] >> rank_bits;
-  const bool first = i == 0 || (keys[i - 1] >> rank_bits) != b, last = i + 1 == n || (keys[i + 1] >> rank_bits) != b;
+  __shared__ uint32_t s_base[DVX_MAX_TREES + 1];
+  for (int i = threadIdx.x; i < (int)n_trees; i += blockDim.x) s_base[i] = trees[i].base;
+  __syncthreads();
+  const uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const int lane = threadIdx.x & 31;
+  const bool valid = i < n;
+  // one search per element; the neighbours' buckets come by shuffle, only the warp's edge lanes look at a second key
+  const uint32_t b = valid ? bucket_of(keys[i], rank_bits, s_base, (int)n_trees) : 0xFFFFFFFFu;
+  uint32_t prev = __shfl_up_sync(0xffffffffu, b, 1), next = __shfl_down_sync(0xffffffffu, b, 1);
+  if (!valid) return;
+  if (lane == 0) prev = i == 0 ? 0xFFFFFFFFu : bucket_of(keys[i - 1], rank_bits, s_base, (int)n_trees);
+  if (lane == 31) next = i + 1 == n ? 0xFFFFFFFFu : bucket_of(keys[i + 1], rank_bits, s_base, (int)n_trees);
+  const bool first = prev != b, last = next != b;
   if (first) range_beg[b] = (uint32_t)i;
   if (last) range_end[b] = (uint32_t)(i + 1);
   if (tile_cost && (first || last)) {
-    const uint32_t tile = (uint32_t)b / buckets_per_tile;
+    const uint32_t tile = b / (n_trees * 8u);
     if (first && last) atomicAdd(tile_cost + tile, 1u);
     else atomicAdd(tile_cost + tile, first ? 0u - (uint32_t)i : (uint32_t)(i + 1));
   }
@@ -617,9 +639,9 @@ void dvx_emit_pairs_launch(const FrameParams &p, const TreeFrame *trees, const u
     if (p.v_total) { DVX_COUNT_LAUNCH(1); emit_pairs_kernel<<<blocks_for(p.v_total, PRE_THREADS), PRE_THREADS, 0, st>>>(p, trees, octmask, pxrect, fvox, keys, vals,
                                                                                    capacity, counters); }
 }
-void dvx_ranges_launch(const uint64_t *keys, uint64_t n, uint32_t rank_bits, uint32_t buckets_per_tile, uint32_t *range_beg,
-                       uint32_t *range_end, uint32_t *tile_cost, cudaStream_t st) {
-  if (n) { DVX_COUNT_LAUNCH(1); ranges_kernel<<<blocks_for(n, 256), 256, 0, st>>>(keys, n, rank_bits, buckets_per_tile, range_beg, range_end, tile_cost); }
+void dvx_ranges_launch(const uint64_t *keys, uint64_t n, uint32_t rank_bits, const TreeFrame *trees, uint32_t n_trees,
+                       uint32_t *range_beg, uint32_t *range_end, uint32_t *tile_cost, cudaStream_t st) {
+  if (n) { DVX_COUNT_LAUNCH(1); ranges_kernel<<<blocks_for(n, 256), 256, 0, st>>>(keys, n, rank_bits, trees, n_trees, range_beg, range_end, tile_cost); }
 }
 void dvx_tile_order_launch(const uint32_t *tile_cost, uint32_t n_tiles, uint32_t *tile_order, cudaStream_t st) {
   if (n_tiles) { DVX_COUNT_LAUNCH(1); tile_order_kernel<<<1, ORDER_THREADS, 0, st>>>(tile_cost, n_tiles, tile_order); }
