@@ -146,8 +146,11 @@ __device__ __forceinline__ double box_dist2(const double lo[3], const double hi[
 
 // min over the cloud's points of box_dist2, restricted to the cells overlapping the box inflated by `reach`; lanes of the
 // warp share the cells.  early = stop as soon as a point within reach is found (returns any value <= reach^2 then).
+// G = lanes that share one query (32: a warp per leaf; 8: four grid points per warp, for queries whose search box has only
+// a handful of rows); early exits need G = 32 (the warp-wide vote).
+template <int G>
 __device__ double warp_min_box_dist2(const CloudView &c, const double lo[3], const double hi[3], double reach, bool early) {
-  const int lane = threadIdx.x & 31;
+  const int lane = threadIdx.x & (G - 1);
   int c0[3], c1[3];
   bool empty = c.n_cells == 0;
   for (int a = 0; a < 3; ++a) {
@@ -160,9 +163,11 @@ __device__ double warp_min_box_dist2(const CloudView &c, const double lo[3], con
     if (c1[a] < c0[a]) empty = true;
   }
   double best = 1.0e300;
-  if (empty) return best;
+  // an empty search box does not return here: it has no rows below and falls through to the shuffles (with G < 32 the other
+  // groups of the warp go on, and a full-mask shuffle needs every lane)
   const double reach2 = reach * reach;
-  const uint64_t nx = (uint64_t)(c1[0] - c0[0] + 1), ny = (uint64_t)(c1[1] - c0[1] + 1), nz = (uint64_t)(c1[2] - c0[2] + 1);
+  const uint64_t nx = empty ? 0 : (uint64_t)(c1[0] - c0[0] + 1), ny = empty ? 0 : (uint64_t)(c1[1] - c0[1] + 1),
+                 nz = empty ? 0 : (uint64_t)(c1[2] - c0[2] + 1);
   const uint64_t range = nx * ny * nz;
   // the occupied cells of the z-slab [c0z, c1z] are one contiguous run of the sorted cell list: when that run is shorter
   // than the search box has cells (coarse leaves, sparse clouds), walk the run instead of probing every cell of the box
@@ -173,31 +178,52 @@ __device__ double warp_min_box_dist2(const CloudView &c, const double lo[3], con
     run_hi = lower_cell(c, (uint64_t)(c1[2] + 1) * plane);
   }
   const bool by_list = range > (uint64_t)(run_hi - run_lo);
-  const uint64_t total = by_list ? (uint64_t)(run_hi - run_lo) : range;
-  for (uint64_t base = 0; base < total; base += 32) {
-    const uint64_t i = base + lane;
-    int idx = -1;
-    if (i < total) {
-      if (by_list) {
+  if (by_list) {
+    const uint64_t total = (uint64_t)(run_hi - run_lo);
+    for (uint64_t base = 0; base < total; base += G) {
+      const uint64_t i = base + lane;
+      int idx = -1;
+      if (i < total) {
         const uint64_t key = __ldg(c.cell_key + run_lo + i);
         const int cx = (int)(key % c.dims[0]), cy = (int)((key / c.dims[0]) % c.dims[1]), cz = (int)(key / ((uint64_t)c.dims[0] * c.dims[1]));
         if (cx >= c0[0] && cx <= c1[0] && cy >= c0[1] && cy <= c1[1] && cz >= c0[2] && cz <= c1[2]) idx = (int)(run_lo + i);
-      } else {
-        const int cx = c0[0] + (int)(i % nx), cy = c0[1] + (int)((i / nx) % ny), cz = c0[2] + (int)(i / (nx * ny));
-        idx = find_cell(c, ((uint64_t)cz * c.dims[1] + cy) * c.dims[0] + cx);
       }
-    }
-    if (idx >= 0) {
-      const uint32_t b = __ldg(c.cell_start + idx), e = __ldg(c.cell_start + idx + 1);
-      for (uint32_t j = b; j < e; ++j) {
-        const double d2 = box_dist2(lo, hi, __ldg(c.pts + j));
-        best = fmin(best, d2);
-        if (early && d2 <= reach2) break;
+      if (idx >= 0) {
+        const uint32_t b = __ldg(c.cell_start + idx), e = __ldg(c.cell_start + idx + 1);
+        for (uint32_t j = b; j < e; ++j) {
+          const double d2 = box_dist2(lo, hi, __ldg(c.pts + j));
+          best = fmin(best, d2);
+          if (early && d2 <= reach2) break;
+        }
       }
+      if (G == 32 && early && __any_sync(0xffffffffu, best <= reach2)) break;
     }
-    if (early && __any_sync(0xffffffffu, best <= reach2)) break;
+  } else {
+    // lane = one x-row of the search box: its occupied cells are ONE contiguous run of the sorted cell list (keys are
+    // (z * ny + y) * nx + x), found by one binary search per row instead of one per cell, and their points are one
+    // contiguous range of the binned cloud
+    const uint64_t rows = ny * nz;
+    for (uint64_t base = 0; base < rows; base += G) {
+      const uint64_t i = base + lane;
+      if (i < rows) {
+        const int cy = c0[1] + (int)(i % ny), cz = c0[2] + (int)(i / ny);
+        const uint64_t row = ((uint64_t)cz * c.dims[1] + cy) * c.dims[0];
+        const uint32_t i0 = lower_cell(c, row + (uint64_t)c0[0]);
+        uint32_t i1 = i0;
+        while (i1 < c.n_cells && __ldg(c.cell_key + i1) <= row + (uint64_t)c1[0]) ++i1;
+        if (i1 > i0) {
+          const uint32_t b = __ldg(c.cell_start + i0), e = __ldg(c.cell_start + i1);
+          for (uint32_t j = b; j < e; ++j) {
+            const double d2 = box_dist2(lo, hi, __ldg(c.pts + j));
+            best = fmin(best, d2);
+            if (early && d2 <= reach2) break;
+          }
+        }
+      }
+      if (G == 32 && early && __any_sync(0xffffffffu, best <= reach2)) break;
+    }
   }
-  for (int o = 16; o > 0; o >>= 1) {
+  for (int o = G / 2; o > 0; o >>= 1) {
     const double other = __hiloint2double(__shfl_xor_sync(0xffffffffu, __double2hiint(best), o),
                                           __shfl_xor_sync(0xffffffffu, __double2loint(best), o));
     best = fmin(best, other);
@@ -213,8 +239,11 @@ __global__ void __launch_bounds__(ST_THREADS) density_prior_kernel(CloudView c, 
                                                                    double cx, double cy, double cz, double side, double s_min,
                                                                    double reach, double v_close, double v_far,
                                                                    float *__restrict__ density) {
-  const uint32_t p = (uint32_t)(((uint64_t)blockIdx.x * ST_THREADS + threadIdx.x) >> 5);  // 64-bit: n_points * 32 threads exceeds 2^32
-  if (p >= n_points) return;
+  // eight lanes per grid point (its search box has about 3 x 3 rows); a point index beyond the end keeps its lanes in the
+  // warp's shuffles with a clamped, harmless query
+  const uint64_t pg = ((uint64_t)blockIdx.x * ST_THREADS + threadIdx.x) >> 3;  // 64-bit: n_points * 8 threads may exceed 2^32
+  const bool live = pg < n_points;
+  const uint32_t p = live ? (uint32_t)pg : n_points - 1u;
   const uint32_t slot = __ldg(slots + __ldg(offsets + p));
   const uint64_t cd = __ldg(code + (slot >> 3));
   const uint32_t cn = slot & 7u, level = (uint32_t)(cd >> 48) & 31u;
@@ -224,8 +253,8 @@ __global__ void __launch_bounds__(ST_THREADS) density_prior_kernel(CloudView c, 
   const uint32_t Y = (uint32_t)compact3s(path >> 1) + ((cn >> 1) & 1u) * size;
   const uint32_t Z = (uint32_t)compact3s(path) + (cn & 1u) * size;
   const double q[3] = {lattice_pos(cx, side, X), lattice_pos(cy, side, Y), lattice_pos(cz, side, Z)};
-  const double d2 = warp_min_box_dist2(c, q, q, reach, false);
-  if ((threadIdx.x & 31) == 0) {
+  const double d2 = warp_min_box_dist2<8>(c, q, q, reach, false);
+  if (live && (threadIdx.x & 7) == 0) {
     const double v = d2 > reach * reach ? v_far : v_far + (v_close - v_far) * exp(-2.0 * d2 / (s_min * s_min));
     density[p] = (float)v;
   }
@@ -247,7 +276,7 @@ __global__ void __launch_bounds__(ST_THREADS) near_flags_kernel(CloudView c, con
   const double hi[3] = {lattice_pos(cx, side, X + size), lattice_pos(cy, side, Y + size), lattice_pos(cz, side, Z + size)};
   bool near = false;
   if (level < max_level) {
-    const double d2 = warp_min_box_dist2(c, lo, hi, threshold, true);
+    const double d2 = warp_min_box_dist2<32>(c, lo, hi, threshold, true);
     near = __dsqrt_rn(d2) <= threshold;  // R26 compares the distance, not its square
   }
   if ((threadIdx.x & 31) == 0) {
@@ -378,7 +407,7 @@ void dvx_density_prior_launch(const DvxCloudData &d, const uint64_t *code, const
                               uint32_t n_points, const double center[3], double side, double s_min, double reach,
                               double v_close, double v_far, float *density, cudaStream_t st) {
   DVX_COUNT_LAUNCH(1);
-  density_prior_kernel<<<st_blocks((uint64_t)n_points * 32), ST_THREADS, 0, st>>>(make_view(d), code, offsets, slots, n_points,
+  density_prior_kernel<<<st_blocks((uint64_t)n_points * 8), ST_THREADS, 0, st>>>(make_view(d), code, offsets, slots, n_points,
                                                                                  center[0], center[1], center[2], side, s_min,
                                                                                  reach, v_close, v_far, density);
 }
