@@ -125,3 +125,59 @@ def test_pool_sizing_follows_the_previous_frames(ctx):
             t.close()
     finally:
         c2.close()
+
+
+def test_a_pool_the_allocator_cannot_give_is_not_an_error(ctx, config1):
+    """dvx.h 'Hit records': when the allocator returns NULL for the record pool the frame simply keeps no records and the
+    backward walks the tile lists - same gradients."""
+    import torch
+    sc = config1
+    gin = sc.image_grads(rgb_std=1e-2, depth_std=1e-3, alpha_std=1e-2)
+    ref = O.render(sc, mode=0, grads_in=gin)
+    import paper_2606_23031_b200 as dvx
+    dev = dvx.SceneOnDevice(ctx, sc)
+    ctx.set_record_budget(1 << 46)          # 64 TiB: torch's allocator refuses, the callback returns NULL
+    try:
+        img, grads, st = _backward_all(dev, sc, gin)
+    finally:
+        ctx.set_record_budget(0)
+    assert st == {"bytes_used": 0, "bytes_capacity": 0, "overflowed": False}
+    for t in range(len(sc.octrees)):
+        _check(grads[t][0], ref["dgeo"][t], "dgeo[%d] without a pool" % t)
+        _check(grads[t][1], ref["dsh"][t], "dsh[%d] without a pool" % t)
+    for t in dev.trees:
+        t.close()
+
+
+def test_batch_entry_points_argument_errors(ctx, config1):
+    """dvx_render_batch / dvx_backward_batch: an invalid camera anywhere in the batch fails the whole call with
+    DVX_ERR_INVALID_ARG and hands out no frame; empty batches are no-ops; frames with a normal map are refused by the batched
+    backward (their post-pass writes dgeo)."""
+    import ctypes as C
+    import torch
+    import paper_2606_23031_b200 as dvx
+    sc = config1
+    dev = dvx.SceneOnDevice(ctx, sc)
+    good = dev.cams[0]
+    bad = dvx.camera_from(sc.cameras[0]); bad.fx = 0.0
+    with pytest.raises(dvx.DvxError) as e:
+        ctx.render_batch([good, bad], dev.trees[0], dev.trees[1:], dev.poses, dev.box_half)
+    assert e.value.status == -1
+    outs, frames = ctx.render_batch([], dev.trees[0], dev.trees[1:], dev.poses, dev.box_half)
+    assert outs == [] and frames == []
+    ctx.backward_batch([], [], dev.zero_grads())
+    # a frame with a normal map goes through dvx_backward_n, not the batch
+    rgb, depth, alpha, normal, fr = dev.render(normals=True)
+    g = torch.zeros_like(rgb)
+    with pytest.raises(dvx.DvxError) as e:
+        ctx.backward_batch([fr], [g], dev.zero_grads())
+    assert e.value.status == -5
+    fr.release()
+    # and the context still works
+    outs, frames = ctx.render_batch([good, good], dev.trees[0], dev.trees[1:], dev.poses, dev.box_half)
+    torch.cuda.synchronize()
+    assert torch.equal(outs[0][0], outs[1][0]) and torch.equal(outs[0][0], rgb)
+    for f in frames:
+        f.release()
+    for t in dev.trees:
+        t.close()
