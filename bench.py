@@ -664,7 +664,13 @@ def run_dvx(args):
                      "traffic_note": "traffic above the algorithmic bytes is the hit-record stream (44 B per composited hit, written by "
                                      "the forward, read by the backward instead of re-walking the tile lists; DESIGN.md section 6), not re-reads",
                      "traffic_stale": bool(stale), "peak_source": peak_src, "bytes_per_launch": dom_bytes, "ms_per_launch": dom_ms,
-                     "all_kernels_ms": kernels},
+                     "all_kernels_ms": kernels,
+                     # both compositing kernels (the forward writes the hit records, the backward reads them)
+                     "per_kernel": {k: {"ms": ms_k, "algorithmic_bytes": ab[k],
+                                        "achieved": ab[k] / (ms_k * 1e-3) / 1e9 if ms_k > 0 else 0.0,
+                                        "frac": ab[k] / (ms_k * 1e-3) / 1e9 / peak if (ms_k > 0 and peak) else None,
+                                        "frac_with_records": (ab[k] + rec_bytes) / (ms_k * 1e-3) / 1e9 / peak if (ms_k > 0 and peak) else None,
+                                        "traffic": (pk.get(k) or {}).get("dram_bytes")} for k, ms_k in kernels.items()}},
         "issue_roofline": dict(issue, bound="alu", unit="warp-instr/s", profile_commit=prof.get("commit"), profile_stale=bool(stale)),
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": (0 if args.fwd_only else 12 * px_step),
                 "d2h_bytes_per_step": 20 * px_step, "ms_per_step": ms_e2e / args.steps},
