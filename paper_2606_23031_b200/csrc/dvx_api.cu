@@ -771,10 +771,13 @@ dvx_status backward_core(dvx_ctx *ctx, dvx_frame *f, const float *dL_drgb, const
   float *dnrm = dL_dnormal ? (float *)hold.add(ctx_alloc(ctx, (size_t)p.v_total * 16)) : nullptr;
   if (!drgb || (dL_dnormal && !dnrm)) return fail(ctx, DVX_ERR_OOM, "dvx_backward: allocator returned NULL");
   TreeFrame *trees_d = (TreeFrame *)f->trees_d.p;
-  // box_rect was filled on the device; only the gradient pointers change, so patch those fields
-  for (uint32_t t = 0; t < p.n_trees; ++t)
-    CU(cudaMemcpyAsync((char *)(trees_d + t) + offsetof(TreeFrame, dgeo), &f->trees_h[t].dgeo, 2 * sizeof(float *),
-                       cudaMemcpyHostToDevice, st));
+  // box_rect was filled on the device; only the gradient pointers change: a one-block kernel patches those fields
+  {
+    DvxGradTable tbl;
+    memset(&tbl, 0, sizeof(tbl));
+    for (uint32_t t = 0; t < p.n_trees; ++t) { tbl.dgeo[t] = f->trees_h[t].dgeo; tbl.dsh[t] = f->trees_h[t].dsh; }
+    dvx_patch_grads_launch(trees_d, p.n_trees, tbl, st);
+  }
   CU(cudaEventRecord(f->ev[5], st));
   CU(cudaMemsetAsync(drgb, 0, (size_t)p.v_total * 16, st));
   if (dnrm) CU(cudaMemsetAsync(dnrm, 0, (size_t)p.v_total * 16, st));

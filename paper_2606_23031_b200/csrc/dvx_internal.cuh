@@ -143,6 +143,8 @@ void dvx_emit_pairs_launch(const FrameParams &p, const TreeFrame *trees, const u
 void dvx_ranges_launch(const uint64_t *keys, uint64_t n, uint32_t rank_bits, const TreeFrame *trees, uint32_t n_trees,
                        uint32_t *range_beg, uint32_t *range_end, uint32_t *tile_cost, cudaStream_t st);
 void dvx_tile_order_launch(const uint32_t *tile_cost, uint32_t n_tiles, uint32_t *tile_order /* [2 n_tiles] */, cudaStream_t st);
+struct DvxGradTable { float *dgeo[DVX_MAX_TREES]; float *dsh[DVX_MAX_TREES]; };
+void dvx_patch_grads_launch(TreeFrame *trees, uint32_t n_trees, const DvxGradTable &tbl, cudaStream_t st);
 void dvx_sh_backward_launch(const FrameParams &p, const TreeFrame *trees, const FrameVox *fvox, const ushort4 *pxrect,
                             const float *drgb, cudaStream_t st);
 

@@ -598,6 +598,14 @@ __global__ void __launch_bounds__(PRE_THREADS) normal_backward_kernel(FrameParam
   o[0] = o0; o[1] = o1;
 }
 
+// The gradient pointers of a backward call go into the frame's tree table by a one-block kernel with the table in its
+// parameters - not by one small host-to-device copy per octree: those queue on the copy engine behind whatever image copy is in
+// flight there (the host-buffer entry points) and each costs a driver round trip.
+__global__ void patch_grads_kernel(TreeFrame *trees, uint32_t n_trees, const __grid_constant__ DvxGradTable tbl) {
+  const uint32_t t = threadIdx.x;
+  if (t < n_trees) { trees[t].dgeo = tbl.dgeo[t]; trees[t].dsh = tbl.dsh[t]; }
+}
+
 inline unsigned blocks_for(uint64_t n, int threads) { return (unsigned)((n + threads - 1) / threads); }
 
 }  // namespace
@@ -649,4 +657,8 @@ void dvx_tile_order_launch(const uint32_t *tile_cost, uint32_t n_tiles, uint32_t
 void dvx_sh_backward_launch(const FrameParams &p, const TreeFrame *trees, const FrameVox *fvox, const ushort4 *pxrect,
                             const float *drgb, cudaStream_t st) {
     if (p.v_total) { DVX_COUNT_LAUNCH(1); sh_backward_kernel<<<blocks_for(4ull * p.v_total, PRE_THREADS), PRE_THREADS, 0, st>>>(p, trees, fvox, pxrect, drgb); }
+}
+void dvx_patch_grads_launch(TreeFrame *trees, uint32_t n_trees, const DvxGradTable &tbl, cudaStream_t st) {
+  DVX_COUNT_LAUNCH(1);
+  patch_grads_kernel<<<1, DVX_MAX_TREES, 0, st>>>(trees, n_trees, tbl);
 }
