@@ -39,12 +39,9 @@ struct dvx_ctx {
   // hit-record pool sizing: chunks per pixel used by the last frames (read back lazily, never waited for)
   uint64_t rec_budget = 0;             // dvx_set_record_budget: bytes per frame, 0 = automatic
   static constexpr int REC_SLOTS = 16;
-  double rec_seen[REC_SLOTS] = {};      // chunks per pixel of the last frames whose count has arrived
+  double rec_seen[REC_SLOTS] = {};      // chunks per pixel the last frames needed
   int rec_seen_n = 0;
-  unsigned long long *h_rec = nullptr;  // pinned [REC_SLOTS]: chunks handed out by a frame in flight
-  cudaEvent_t ev_rec[REC_SLOTS] = {};
-  double rec_pending_npix[REC_SLOTS] = {};  // > 0: a read-back is in flight in this slot for a frame of that many pixels
-  int rec_slot = 0;                     // next slot to use (a batch of cameras has one read-back per camera in flight)
+  unsigned long long *d_rec_last = nullptr;  // device {chunks, pixels} of the latest frame whose count was published
   // batched entry points: a second, high-priority stream for steps 1-2 and the per-voxel post-passes
   cudaStream_t ps = nullptr;
   cudaEvent_t ev_entry = nullptr;
@@ -150,6 +147,9 @@ uint32_t bits_for(uint64_t n_values) {  // bits needed to hold values 0..n_value
 
 void frame_free(dvx_ctx *ctx, dvx_frame *f) {
   if (!f) return;
+  // a frame that kept hit records but never had a backward still tells the context what its records needed
+  if (f->rec_pool.p && !f->did_backward && f->es && f->es->rendered && ctx->d_rec_last)
+    dvx_publish_rec_launch((const unsigned long long *)f->counters.p, ctx->d_rec_last, (unsigned long long)f->p.width * f->p.height, ctx->st);
   dvx_frame::Buf *bs[] = {&f->trees_d, &f->fvox, &f->pxrect, &f->octmask, &f->actor_mask, &f->ids,
                           &f->range_beg, &f->range_end, &f->counters, &f->sv_rgbd, &f->sv_T, &f->sv_nused};
   for (auto *b : bs) ctx_release(ctx, b->p);
@@ -254,18 +254,10 @@ dvx_status dvx_create(int device, void *cuda_stream, dvx_alloc_fn alloc, dvx_fre
   ctx->device = device;
   ctx->st = (cudaStream_t)cuda_stream;
   ctx->alloc = alloc; ctx->free_ = free_; ctx->user = user;
-  if (cudaMallocHost((void **)&ctx->h_counters, (CNT_N + dvx_ctx::REC_SLOTS) * sizeof(unsigned long long)) != cudaSuccess) {
+  if (cudaMallocHost((void **)&ctx->h_counters, CNT_N * sizeof(unsigned long long)) != cudaSuccess) {
     delete ctx;
     return DVX_ERR_CUDA;
   }
-  ctx->h_rec = ctx->h_counters + CNT_N;
-  for (int i = 0; i < dvx_ctx::REC_SLOTS; ++i)
-    if (cudaEventCreateWithFlags(&ctx->ev_rec[i], cudaEventDisableTiming) != cudaSuccess) {
-      for (int j = 0; j < i; ++j) cudaEventDestroy(ctx->ev_rec[j]);
-      cudaFreeHost(ctx->h_counters);
-      delete ctx;
-      return DVX_ERR_CUDA;
-    }
   *out = ctx;
   return DVX_OK;
 }
@@ -279,7 +271,6 @@ void dvx_destroy(dvx_ctx *ctx) {
     else cudaFree(b.p);
   }
   cudaFreeHost(ctx->h_counters);
-  for (cudaEvent_t e : ctx->ev_rec) cudaEventDestroy(e);
   if (ctx->ps) { cudaStreamSynchronize(ctx->ps); cudaStreamDestroy(ctx->ps); cudaEventDestroy(ctx->ev_entry); }
   for (cudaEvent_t e : ctx->ev_batch) cudaEventDestroy(e);
   if (ctx->h_batch) cudaFreeHost(ctx->h_batch);
@@ -386,19 +377,14 @@ void setup_tree(TreeFrame &T, const dvx_octree *t, uint32_t base, bool actor, co
 }
 
 // ---- hit-record pool sizing (dvx.h "Hit records") ------------------------------------------------------------------------
-// The chunk count of a frame is copied to pinned memory behind its forward and picked up here, without waiting, by a later
-// dvx_render; the pool of the next frame is 1.25 x the largest count per pixel among the last 16 frames seen.
-void rec_collect(dvx_ctx *ctx) {
-  for (int i = 0; i < dvx_ctx::REC_SLOTS; ++i) {
-    if (ctx->rec_pending_npix[i] <= 0) continue;
-    if (cudaEventQuery(ctx->ev_rec[i]) == cudaSuccess) {
-      ctx->rec_seen[ctx->rec_seen_n % dvx_ctx::REC_SLOTS] = (double)ctx->h_rec[i] / ctx->rec_pending_npix[i];
-      ctx->rec_seen_n++;
-      ctx->rec_pending_npix[i] = 0;
-    } else {
-      cudaGetLastError();  // cudaErrorNotReady is not an error
-    }
-  }
+// The chunk count of a frame is published on the device when its backward starts (or when it is released without one) and
+// travels to the host with the NEXT frame's pair count, at the one synchronisation dvx_render has anyway: no extra copy, no
+// polling, and the pool size of a frame depends only on the frames before it, not on timing.  The pool of the next frame is
+// 1.25 x the largest count per pixel among the last 16 values seen.
+void rec_learn(dvx_ctx *ctx, const unsigned long long *h_cnt) {
+  if (h_cnt[CNT_PREV_NPIX] == 0) return;
+  ctx->rec_seen[ctx->rec_seen_n % dvx_ctx::REC_SLOTS] = (double)h_cnt[CNT_PREV_REC] / (double)h_cnt[CNT_PREV_NPIX];
+  ctx->rec_seen_n++;
 }
 uint64_t rec_capacity(const dvx_ctx *ctx, const FrameParams &p) {
   const double chunk_bytes = (double)DVX_REC_CHUNK_STRIDE;
@@ -544,7 +530,12 @@ dvx_status render_step1(dvx_ctx *ctx, const dvx_camera *cam, const dvx_octree *s
   CU(cudaMemsetAsync(counters, 0, sizeof(unsigned long long) * CNT_N, st));
   // ---- step 1
   CU(cudaEventRecord(f->ev[0], st));
-  dvx_tree_setup_launch(p, trees_d, st);
+  if (!ctx->d_rec_last) {  // lives as long as the context
+    ctx->d_rec_last = (unsigned long long *)ctx_alloc(ctx, 256);
+    if (!ctx->d_rec_last) return fail(ctx, DVX_ERR_OOM, "dvx_render: allocator returned NULL");
+    CU(cudaMemsetAsync(ctx->d_rec_last, 0, 256, st));
+  }
+  dvx_tree_setup_launch(p, trees_d, counters, ctx->d_rec_last, st);
   dvx_tile_masks_launch(p, trees_d, (uint8_t *)f->octmask.p, (unsigned long long *)f->actor_mask.p, st);
   dvx_preprocess_launch(p, trees_d, (const uint8_t *)f->octmask.p, (FrameVox *)f->fvox.p, (ushort4 *)f->pxrect.p, (float4 *)f->vnrm.p, counters, st);
   CU(cudaEventRecord(f->ev[1], st));
@@ -610,7 +601,6 @@ dvx_status render_step34(dvx_ctx *ctx, dvx_frame *f, const dvx_image &out, bool 
   // ---- hit records for the backward (dvx.h): only for saved frames rendered by the tile kernel
   bool rec = false;
   if (save && !(p.flags & (DVX_FLAG_NAIVE | DVX_FLAG_NO_RECORDS))) {
-    rec_collect(ctx);
     const uint64_t cap = rec_capacity(ctx, p);
     if (cap > 0) {
       // a pool the allocator cannot give is not an error: the frame then keeps no records and the backward walks the lists
@@ -630,13 +620,6 @@ dvx_status render_step34(dvx_ctx *ctx, dvx_frame *f, const dvx_image &out, bool 
   CU(cudaEventRecord(f->ev[9], st));
   dvx_composite_launch(A, false, st);
   CU(cudaEventRecord(f->ev[4], st));
-  if (rec && !ctx->rec_budget) {
-    const int slot = ctx->rec_slot;   // a slot still pending is simply overwritten (its frame's count is lost, not wrong)
-    ctx->rec_slot = (slot + 1) % dvx_ctx::REC_SLOTS;
-    CU(cudaMemcpyAsync(ctx->h_rec + slot, counters + CNT_REC_CHUNKS, sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
-    CU(cudaEventRecord(ctx->ev_rec[slot], st));
-    ctx->rec_pending_npix[slot] = (double)npix;
-  }
   f->es->rendered = true;
   CU(cudaGetLastError());
   return DVX_OK;
@@ -685,6 +668,7 @@ dvx_status dvx_render(dvx_ctx *ctx, const dvx_camera *cam, const dvx_octree *sta
   CallGuard guard(ctx);
   guard.frame = f;
   CU(cudaStreamSynchronize(st));  // the one host round trip of a frame: the pair count sizes the sort buffers
+  rec_learn(ctx, f->h_cnt);
   rc = render_step2(ctx, f, st);
   if (rc == DVX_OK) rc = render_step34(ctx, f, out, saved != nullptr, st);
   if (rc != DVX_OK) return rc;
@@ -725,6 +709,7 @@ dvx_status dvx_render_batch(dvx_ctx *ctx, uint32_t n_cams, const dvx_camera *cam
   }
   cudaError_t e = cudaStreamSynchronize(side);  // ONE host round trip for the pair counts of all cameras
   if (e != cudaSuccess) return cuda_fail(ctx, e, "dvx_render_batch");
+  rec_learn(ctx, fr[0]->h_cnt);
   for (uint32_t c = 0; c < n_cams; ++c) {
     // camera c's key generation + sort run on the second stream, under camera c-1's compositing on the context's stream
     rc = render_step2(ctx, fr[c], side);
@@ -776,7 +761,9 @@ dvx_status backward_core(dvx_ctx *ctx, dvx_frame *f, const float *dL_drgb, const
     DvxGradTable tbl;
     memset(&tbl, 0, sizeof(tbl));
     for (uint32_t t = 0; t < p.n_trees; ++t) { tbl.dgeo[t] = f->trees_h[t].dgeo; tbl.dsh[t] = f->trees_h[t].dsh; }
-    dvx_patch_grads_launch(trees_d, p.n_trees, tbl, st);
+    const bool publish = f->rec_pool.p && !f->did_backward;
+    dvx_patch_grads_launch(trees_d, p.n_trees, tbl, publish ? (const unsigned long long *)f->counters.p : nullptr, ctx->d_rec_last,
+                           (unsigned long long)p.width * p.height, st);
   }
   CU(cudaEventRecord(f->ev[5], st));
   CU(cudaMemsetAsync(drgb, 0, (size_t)p.v_total * 16, st));

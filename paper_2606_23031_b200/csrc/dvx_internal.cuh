@@ -56,6 +56,8 @@ struct __align__(16) FrameVox {
 enum { CNT_PAIRS = 0, CNT_VVIS = 1, CNT_QTEST = 2, CNT_QHIT = 3, CNT_PAIRS_EFF = 4, CNT_OVERFLOW = 5, CNT_EMIT = 6,
        CNT_REC_CHUNKS = 7,    // hit-record chunks handed out by the forward (may exceed the capacity: then CNT_REC_OVERFLOW is set)
        CNT_REC_OVERFLOW = 8,  // != 0: the record pool was too small, the backward re-walks the lists instead of replaying
+       CNT_PREV_REC = 9,      // chunks the context's latest frame with a backward (or released without one) needed ...
+       CNT_PREV_NPIX = 10,    // ... and its pixel count: copied in by step 1, read by the host with the pair count (pool sizing)
        CNT_N = 12 };
 
 // ---- hit records (forward -> backward): what the forward composited, in the order it composited it ------------------
@@ -130,7 +132,8 @@ void dvx_rank_keys_launch(const uint64_t *code, uint32_t n, int q, uint64_t *key
 void dvx_rank_scatter_launch(const uint32_t *perm, uint32_t n, uint32_t *rank, cudaStream_t st);
 void dvx_validate_launch(const uint64_t *code_sorted_keys, const uint32_t *perm, const uint64_t *code, uint32_t n,
                          uint32_t *bad_flag, cudaStream_t st);
-void dvx_tree_setup_launch(const FrameParams &p, TreeFrame *trees, cudaStream_t st);
+void dvx_tree_setup_launch(const FrameParams &p, TreeFrame *trees, unsigned long long *counters, const unsigned long long *rec_last,
+                           cudaStream_t st);
 void dvx_tile_masks_launch(const FrameParams &p, const TreeFrame *trees, uint8_t *octmask, unsigned long long *actor_mask,
                            cudaStream_t st);
 void dvx_preprocess_launch(const FrameParams &p, const TreeFrame *trees, const uint8_t *octmask, FrameVox *fvox,
@@ -144,7 +147,10 @@ void dvx_ranges_launch(const uint64_t *keys, uint64_t n, uint32_t rank_bits, con
                        uint32_t *range_beg, uint32_t *range_end, uint32_t *tile_cost, cudaStream_t st);
 void dvx_tile_order_launch(const uint32_t *tile_cost, uint32_t n_tiles, uint32_t *tile_order /* [2 n_tiles] */, cudaStream_t st);
 struct DvxGradTable { float *dgeo[DVX_MAX_TREES]; float *dsh[DVX_MAX_TREES]; };
-void dvx_patch_grads_launch(TreeFrame *trees, uint32_t n_trees, const DvxGradTable &tbl, cudaStream_t st);
+// also publishes the frame's record-chunk count to the context's rec_last[2] = {chunks, pixels} (either may be NULL)
+void dvx_patch_grads_launch(TreeFrame *trees, uint32_t n_trees, const DvxGradTable &tbl, const unsigned long long *counters,
+                            unsigned long long *rec_last, unsigned long long npix, cudaStream_t st);
+void dvx_publish_rec_launch(const unsigned long long *counters, unsigned long long *rec_last, unsigned long long npix, cudaStream_t st);
 void dvx_sh_backward_launch(const FrameParams &p, const TreeFrame *trees, const FrameVox *fvox, const ushort4 *pxrect,
                             const float *drgb, cudaStream_t st);
 

@@ -47,8 +47,12 @@ __global__ void validate_kernel(const uint64_t *skeys, const uint32_t *perm, con
 
 // ------------------------------------------------------------------ per-frame set-up
 // One thread per tree: pixel rectangle of the actor's oriented box.
-__global__ void tree_setup_kernel(FrameParams p, TreeFrame *trees) {
+__global__ void tree_setup_kernel(FrameParams p, TreeFrame *trees, unsigned long long *counters, const unsigned long long *rec_last) {
   int t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t == 0 && rec_last) {  // what the latest frame's hit records needed: travels to the host with this frame's pair count
+    counters[CNT_PREV_REC] = rec_last[0];
+    counters[CNT_PREV_NPIX] = rec_last[1];
+  }
   if (t >= (int)p.n_trees) return;
   TreeFrame &T = trees[t];
   if (!T.is_actor) {
@@ -601,9 +605,15 @@ __global__ void __launch_bounds__(PRE_THREADS) normal_backward_kernel(FrameParam
 // The gradient pointers of a backward call go into the frame's tree table by a one-block kernel with the table in its
 // parameters - not by one small host-to-device copy per octree: those queue on the copy engine behind whatever image copy is in
 // flight there (the host-buffer entry points) and each costs a driver round trip.
-__global__ void patch_grads_kernel(TreeFrame *trees, uint32_t n_trees, const __grid_constant__ DvxGradTable tbl) {
+__global__ void patch_grads_kernel(TreeFrame *trees, uint32_t n_trees, const __grid_constant__ DvxGradTable tbl,
+                                   const unsigned long long *counters, unsigned long long *rec_last, unsigned long long npix) {
   const uint32_t t = threadIdx.x;
   if (t < n_trees) { trees[t].dgeo = tbl.dgeo[t]; trees[t].dsh = tbl.dsh[t]; }
+  if (t == 0 && rec_last && counters) { rec_last[0] = counters[CNT_REC_CHUNKS]; rec_last[1] = npix; }
+}
+__global__ void publish_rec_kernel(const unsigned long long *counters, unsigned long long *rec_last, unsigned long long npix) {
+  rec_last[0] = counters[CNT_REC_CHUNKS];
+  rec_last[1] = npix;
 }
 
 inline unsigned blocks_for(uint64_t n, int threads) { return (unsigned)((n + threads - 1) / threads); }
@@ -620,8 +630,9 @@ void dvx_validate_launch(const uint64_t *skeys, const uint32_t *perm, const uint
                          uint32_t *bad_flag, cudaStream_t st) {
   if (n) { DVX_COUNT_LAUNCH(1); validate_kernel<<<blocks_for(n, 256), 256, 0, st>>>(skeys, perm, code, n, bad_flag); }
 }
-void dvx_tree_setup_launch(const FrameParams &p, TreeFrame *trees, cudaStream_t st) {
-  { DVX_COUNT_LAUNCH(1); tree_setup_kernel<<<1, 128, 0, st>>>(p, trees); }
+void dvx_tree_setup_launch(const FrameParams &p, TreeFrame *trees, unsigned long long *counters, const unsigned long long *rec_last,
+                           cudaStream_t st) {
+  { DVX_COUNT_LAUNCH(1); tree_setup_kernel<<<1, 128, 0, st>>>(p, trees, counters, rec_last); }
 }
 void dvx_tile_masks_launch(const FrameParams &p, const TreeFrame *trees, uint8_t *octmask, unsigned long long *actor_mask,
                            cudaStream_t st) {
@@ -658,7 +669,12 @@ void dvx_sh_backward_launch(const FrameParams &p, const TreeFrame *trees, const 
                             const float *drgb, cudaStream_t st) {
     if (p.v_total) { DVX_COUNT_LAUNCH(1); sh_backward_kernel<<<blocks_for(4ull * p.v_total, PRE_THREADS), PRE_THREADS, 0, st>>>(p, trees, fvox, pxrect, drgb); }
 }
-void dvx_patch_grads_launch(TreeFrame *trees, uint32_t n_trees, const DvxGradTable &tbl, cudaStream_t st) {
+void dvx_patch_grads_launch(TreeFrame *trees, uint32_t n_trees, const DvxGradTable &tbl, const unsigned long long *counters,
+                            unsigned long long *rec_last, unsigned long long npix, cudaStream_t st) {
   DVX_COUNT_LAUNCH(1);
-  patch_grads_kernel<<<1, DVX_MAX_TREES, 0, st>>>(trees, n_trees, tbl);
+  patch_grads_kernel<<<1, DVX_MAX_TREES, 0, st>>>(trees, n_trees, tbl, counters, rec_last, npix);
+}
+void dvx_publish_rec_launch(const unsigned long long *counters, unsigned long long *rec_last, unsigned long long npix, cudaStream_t st) {
+  DVX_COUNT_LAUNCH(1);
+  publish_rec_kernel<<<1, 1, 0, st>>>(counters, rec_last, npix);
 }
