@@ -121,8 +121,10 @@ typedef struct {
 } dvx_image;
 
 /* Steps 1-4 of the hot path.  All work is enqueued on the context's stream; the call blocks the host ONCE, between step 1
- * and step 2, to read the number of (tile, octant, voxel) pairs that sizes the sort buffers (dvx_render_batch amortises
- * that round trip over its cameras).  poses_l2w: HOST [N][12] row-major [R_i | t_i] local->world;
+ * and step 2, to read the number of (tile, octant, voxel) pairs that sizes the sort buffers and the sort's grid (dvx_render_batch
+ * amortises that round trip over its cameras).  The GPU does not idle meanwhile: key generation only needs a capacity, which
+ * the context takes from its recent frames (x 1.25), and is enqueued before the wait; a frame with more pairs than that
+ * repeats it.  poses_l2w: HOST [N][12] row-major [R_i | t_i] local->world;
  * box_half: HOST [N][3] half extents of the oriented box in the actor frame.  opts NULL = defaults
  * (K=8, exp, t_stop=1e-4, flags 0).  saved: if non-NULL receives a frame handle for dvx_backward / introspection
  * (release with dvx_frame_release); NULL = inference, nothing kept. */
@@ -207,8 +209,8 @@ dvx_status dvx_frame_counters(dvx_ctx *ctx, const dvx_frame *frame, uint64_t *v_
 /* Device milliseconds (CUDA events on the context's stream) of the stages of the frame's dvx_render call:
  * [0] preprocess (step 1), [1] key generation + sort + ranges (step 2), [2] compositing kernel (steps 3+4);
  * after dvx_backward also [3] all of step 5, [4] its compositing-replay kernel alone, [5] its per-voxel SH
- * post-pass alone; [6] the gap between the end of step 1 and the start of step 2 (the host round trip that reads the pair
- * count: the GPU idles), [7] the gap between the end of compositing and the start of step 5 (whatever the caller or a copy
+ * post-pass alone; [6] the gap between the end of step 1 and the start of step 2 (near zero when key generation could be
+ * enqueued before the pair count was known, see dvx_render; else the host round trip, during which the GPU idles), [7] the gap between the end of compositing and the start of step 5 (whatever the caller or a copy
  * put in between).  HOST out[8].  Synchronises the stream. */
 dvx_status dvx_frame_stage_ms(dvx_ctx *ctx, const dvx_frame *frame, float *ms_out8);
 /* The same eight times SUMMED over every frame released (or rendered with saved = NULL) since the last call;

@@ -14,7 +14,7 @@ std::atomic<unsigned long long> g_dvx_launches{0};
 
 // The CUDA events of one render (+ backward) call.  Owned by the context and recycled, so the steady state creates none.
 struct EventSet {
-  cudaEvent_t ev[10] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+  cudaEvent_t ev[11] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};  // [10]: step 1's counters are on the host
   bool rendered = false, did_backward = false;
 };
 
@@ -42,6 +42,9 @@ struct dvx_ctx {
   double rec_seen[REC_SLOTS] = {};      // chunks per pixel the last frames needed
   int rec_seen_n = 0;
   unsigned long long *d_rec_last = nullptr;  // device {chunks, pixels} of the latest frame whose count was published
+  cudaStream_t qs = nullptr;            // carries step 1's counters to the host beside the frame's stream
+  uint64_t pairs_seen[8] = {};          // pair counts of the last frames: capacity of the optimistic key generation
+  int pairs_seen_n = 0;
   // batched entry points: a second, high-priority stream for steps 1-2 and the per-voxel post-passes
   cudaStream_t ps = nullptr;
   cudaEvent_t ev_entry = nullptr;
@@ -73,6 +76,8 @@ struct dvx_frame {
   Buf trees_d, fvox, pxrect, octmask, actor_mask, ids, range_beg, range_end, counters, sv_rgbd, sv_T, sv_nused;
   uint64_t n_pairs = 0, v_vis = 0;
   const unsigned long long *h_cnt = nullptr;  // pinned copy of the counters after step 1 (valid until step 2 has read it)
+  void *opt_ka = nullptr, *opt_va = nullptr;  // key generation launched before the pair count was known (capacity opt_cap)
+  uint64_t opt_cap = 0;
   EventSet *es = nullptr;
   cudaEvent_t *ev = nullptr;  // = es->ev
   Buf eff_end, vnrm, sv_nrm;
@@ -159,6 +164,7 @@ void frame_free(dvx_ctx *ctx, dvx_frame *f) {
   ctx_release(ctx, f->tile_cost.p); ctx_release(ctx, f->tile_order.p);
   ctx_release(ctx, f->w_row.p); ctx_release(ctx, f->w_vox.p); ctx_release(ctx, f->w_val.p);
   ctx_release(ctx, f->rec_pool.p); ctx_release(ctx, f->rec_next.p); ctx_release(ctx, f->rec_tab.p);
+  ctx_release(ctx, f->opt_ka); ctx_release(ctx, f->opt_va);
   if (f->es) {
     f->es->did_backward = f->did_backward;
     if (f->es->rendered) {
@@ -272,6 +278,7 @@ void dvx_destroy(dvx_ctx *ctx) {
   }
   cudaFreeHost(ctx->h_counters);
   if (ctx->ps) { cudaStreamSynchronize(ctx->ps); cudaStreamDestroy(ctx->ps); cudaEventDestroy(ctx->ev_entry); }
+  if (ctx->qs) { cudaStreamSynchronize(ctx->qs); cudaStreamDestroy(ctx->qs); }
   for (cudaEvent_t e : ctx->ev_batch) cudaEventDestroy(e);
   if (ctx->h_batch) cudaFreeHost(ctx->h_batch);
   if (ctx->cs) {
@@ -539,8 +546,32 @@ dvx_status render_step1(dvx_ctx *ctx, const dvx_camera *cam, const dvx_octree *s
   dvx_tile_masks_launch(p, trees_d, (uint8_t *)f->octmask.p, (unsigned long long *)f->actor_mask.p, st);
   dvx_preprocess_launch(p, trees_d, (const uint8_t *)f->octmask.p, (FrameVox *)f->fvox.p, (ushort4 *)f->pxrect.p, (float4 *)f->vnrm.p, counters, st);
   CU(cudaEventRecord(f->ev[1], st));
-  CU(cudaMemcpyAsync(h_cnt, counters, sizeof(unsigned long long) * CNT_N, cudaMemcpyDeviceToHost, st));
+  // the counters travel to the host on a stream of their own: a copy enqueued on the frame's stream would sit between step 1
+  // and the key generation below for the 14 us a 96-byte device-to-host copy takes
+  if (!ctx->qs) CU(cudaStreamCreateWithFlags(&ctx->qs, cudaStreamNonBlocking));
+  CU(cudaStreamWaitEvent(ctx->qs, f->ev[1], 0));
+  CU(cudaMemcpyAsync(h_cnt, counters, sizeof(unsigned long long) * CNT_N, cudaMemcpyDeviceToHost, ctx->qs));
+  CU(cudaEventRecord(f->ev[10], ctx->qs));
   f->h_cnt = h_cnt;
+  // Key generation does not need the pair count, only a capacity: with the recent frames' counts as a guide it is enqueued
+  // right here, so the GPU works while the host waits for the count, wakes up and sizes the sort (the one host round trip of
+  // a frame; 0.02 ms of idle GPU otherwise).  A frame with more pairs than the capacity repeats it in step 2.
+  if (ctx->pairs_seen_n > 0) {
+    uint64_t m = 0;
+    for (int i = 0; i < 8 && i < ctx->pairs_seen_n; ++i) m = ctx->pairs_seen[i] > m ? ctx->pairs_seen[i] : m;
+    const uint64_t cap = m + m / 4 + 4096;
+    f->opt_ka = ctx_alloc(ctx, cap * 8);
+    f->opt_va = ctx_alloc(ctx, cap * 4);
+    if (f->opt_ka && f->opt_va) {
+      f->opt_cap = cap;
+      CU(cudaEventRecord(f->ev[2], st));
+      dvx_emit_pairs_launch(p, trees_d, (const uint8_t *)f->octmask.p, (const ushort4 *)f->pxrect.p, (const FrameVox *)f->fvox.p,
+                            (uint64_t *)f->opt_ka, (uint32_t *)f->opt_va, cap, counters, st);
+    } else {
+      ctx_release(ctx, f->opt_ka); ctx_release(ctx, f->opt_va);
+      f->opt_ka = f->opt_va = nullptr;
+    }
+  }
   guard.keep_frame();
   *out_f = f;
   return DVX_OK;
@@ -557,12 +588,28 @@ dvx_status render_step2(dvx_ctx *ctx, dvx_frame *f, cudaStream_t st) {
   unsigned long long *counters = (unsigned long long *)f->counters.p;
   CallGuard guard(ctx);
   const uint64_t P = f->n_pairs;
-  uint64_t *ka = (uint64_t *)guard.add(ctx_alloc(ctx, P * 8)), *kb = (uint64_t *)guard.add(ctx_alloc(ctx, P * 8));
-  uint32_t *va = (uint32_t *)guard.add(ctx_alloc(ctx, P * 4)), *vb = (uint32_t *)guard.add(ctx_alloc(ctx, P * 4));
+  ctx->pairs_seen[ctx->pairs_seen_n++ % 8] = P;
+  const bool emitted = f->opt_cap >= P && f->opt_ka;   // step 1's optimistic key generation had room for every pair
+  uint64_t *ka, *kb;
+  uint32_t *va, *vb;
+  if (emitted) {
+    ka = (uint64_t *)guard.add(f->opt_ka); va = (uint32_t *)guard.add(f->opt_va);
+    f->opt_ka = f->opt_va = nullptr;
+    // the second pair of buffers only ever holds P entries
+    kb = (uint64_t *)guard.add(ctx_alloc(ctx, P * 8)); vb = (uint32_t *)guard.add(ctx_alloc(ctx, P * 4));
+  } else {
+    ctx_release(ctx, f->opt_ka); ctx_release(ctx, f->opt_va);   // stream-ordered: the overflowed attempt has finished before any reuse
+    f->opt_ka = f->opt_va = nullptr;
+    ka = (uint64_t *)guard.add(ctx_alloc(ctx, P * 8)); kb = (uint64_t *)guard.add(ctx_alloc(ctx, P * 8));
+    va = (uint32_t *)guard.add(ctx_alloc(ctx, P * 4)); vb = (uint32_t *)guard.add(ctx_alloc(ctx, P * 4));
+  }
   void *scr = guard.add(ctx_alloc(ctx, dvx_sort_scratch_bytes(P)));
   if (!ka || !kb || !va || !vb || !scr) return fail(ctx, DVX_ERR_OOM, "dvx_render: allocator returned NULL");
-  CU(cudaEventRecord(f->ev[2], st));
-  dvx_emit_pairs_launch(p, trees_d, (const uint8_t *)f->octmask.p, (const ushort4 *)f->pxrect.p, (const FrameVox *)f->fvox.p, ka, va, P, counters, st);
+  if (!emitted) {
+    if (f->opt_cap) CU(cudaMemsetAsync(counters + CNT_EMIT, 0, sizeof(unsigned long long), st));  // the attempt left its cursor behind
+    CU(cudaEventRecord(f->ev[2], st));
+    dvx_emit_pairs_launch(p, trees_d, (const uint8_t *)f->octmask.p, (const ushort4 *)f->pxrect.p, (const FrameVox *)f->fvox.p, ka, va, P, counters, st);
+  }
   int which = dvx_sort_launch(ka, va, kb, vb, P, key_bits, scr, st);
   CU(cudaMemsetAsync(f->range_beg.p, 0, sizeof(uint32_t) * (size_t)p.n_buckets, st));
   CU(cudaMemsetAsync(f->range_end.p, 0, sizeof(uint32_t) * (size_t)p.n_buckets, st));
@@ -667,7 +714,7 @@ dvx_status dvx_render(dvx_ctx *ctx, const dvx_camera *cam, const dvx_octree *sta
   if (rc != DVX_OK) return rc;
   CallGuard guard(ctx);
   guard.frame = f;
-  CU(cudaStreamSynchronize(st));  // the one host round trip of a frame: the pair count sizes the sort buffers
+  CU(cudaEventSynchronize(f->ev[10]));  // the one host round trip of a frame: the pair count sizes the sort buffers and the sort's grid
   rec_learn(ctx, f->h_cnt);
   rc = render_step2(ctx, f, st);
   if (rc == DVX_OK) rc = render_step34(ctx, f, out, saved != nullptr, st);
@@ -707,7 +754,7 @@ dvx_status dvx_render_batch(dvx_ctx *ctx, uint32_t n_cams, const dvx_camera *cam
                       ctx->h_batch + (size_t)c * CNT_N, &fr[c]);
     if (rc != DVX_OK) { cudaStreamSynchronize(side); return rc; }
   }
-  cudaError_t e = cudaStreamSynchronize(side);  // ONE host round trip for the pair counts of all cameras
+  cudaError_t e = cudaEventSynchronize(fr[n_cams - 1]->ev[10]);  // ONE host round trip for the pair counts of all cameras (one stream: the last count is the latest)
   if (e != cudaSuccess) return cuda_fail(ctx, e, "dvx_render_batch");
   rec_learn(ctx, fr[0]->h_cnt);
   for (uint32_t c = 0; c < n_cams; ++c) {
