@@ -386,10 +386,13 @@ __global__ void __launch_bounds__(PRE_THREADS) emit_pairs_kernel(FrameParams p, 
 // tile_cost[tile] (pre-zeroed) receives the tile's pair count as sum(end) - sum(begin) over its buckets, in u32 arithmetic.
 __device__ __forceinline__ uint32_t bucket_of(uint64_t key, uint32_t rank_bits, const uint32_t *s_base, int n_trees) {
   const uint32_t tq = (uint32_t)(key >> rank_bits), comb = (uint32_t)(key & ((1ull << rank_bits) - 1ull));
-  int lo = 0, hi = n_trees - 1;       // last tree whose base <= comb
-  while (lo < hi) {
-    const int mid = (lo + hi + 1) >> 1;
-    if (s_base[mid] <= comb) lo = mid; else hi = mid - 1;
+  int lo = 0;                         // last tree whose base <= comb
+  if (n_trees > 1 && comb >= s_base[1]) {   // most pairs belong to the static octree (tree 0): one compare
+#pragma unroll
+    for (int step = 64; step >= 1; step >>= 1) {   // branch-free: n_trees <= 65
+      const int m = lo + step;
+      if (m < n_trees && s_base[m] <= comb) lo = m;
+    }
   }
   return ((tq >> 3) * (uint32_t)n_trees + (uint32_t)lo) * 8u + (tq & 7u);
 }
