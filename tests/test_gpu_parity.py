@@ -524,6 +524,45 @@ def test_multi_camera_accumulation_config5_semantics(ctx):
         _check_grads(grads[t][1], ref_dsh[t], "dsh[%d] over 3 cameras" % t)
 
 
+def test_key_generation_ahead_of_the_pair_count_is_repeated_when_it_did_not_fit(config1):
+    """Step 2's key generation is enqueued before the host knows the frame's pair count, with a capacity taken from the
+    context's recent frames (include/dvx.h, "one host round trip").  A context that has only seen a tiny scene guesses far too
+    small for config 2: the frame must repeat the key generation at the true size and come out bit-identical to the same
+    frame rendered by a context with no history (which sizes from the count) and by one with the right history."""
+    import paper_2606_23031_b200 as dvx
+    import torch
+    big = S.make_config(2)
+    fresh = dvx.Context(0)
+    dev_f = dvx.SceneOnDevice(fresh, big)
+    ref = dev_f.render()                       # no history: sized from the count
+    ref2 = dev_f.render()                      # history = this frame: the guess fits
+    torch.cuda.synchronize()
+    pairs_ref = ref[3].counters()["pairs"]
+    lists_ref = [ref[3].tile_list(t, 0, q) for t in (5, 700, 1500) for q in range(8)]
+    small_ctx = dvx.Context(0)
+    dev_s = dvx.SceneOnDevice(small_ctx, config1)
+    for _ in range(3):
+        dev_s.render()[3].release()            # history: a few thousand pairs
+    pairs_small = dev_s.render()
+    n_small = pairs_small[3].counters()["pairs"]
+    pairs_small[3].release()
+    dev_b = dvx.SceneOnDevice(small_ctx, big)
+    got = dev_b.render()                       # the guess (1.25 x a few thousand) cannot hold config 2's pairs
+    torch.cuda.synchronize()
+    assert pairs_ref > 8 * (n_small + n_small // 4 + 4096), (pairs_ref, n_small)
+    assert got[3].counters()["pairs"] == pairs_ref
+    for a, b, c in zip(ref[:3], ref2[:3], got[:3]):
+        assert torch.equal(a, b) and torch.equal(a, c)
+    lists_got = [got[3].tile_list(t, 0, q) for t in (5, 700, 1500) for q in range(8)]
+    assert sum(len(x) for x in lists_ref) > 0
+    for a, b in zip(lists_ref, lists_got):
+        assert np.array_equal(a, b)
+    for fr in (ref[3], ref2[3], got[3]):
+        fr.release()
+    fresh.close()
+    small_ctx.close()
+
+
 @pytest.mark.parametrize("cfg", [2, 4])
 def test_forward_is_bit_deterministic(ctx, cfg):
     """The forward has no atomics: two renders of the same frame must agree bit for bit (a data race between the phases of
