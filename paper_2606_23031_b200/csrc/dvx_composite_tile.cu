@@ -68,10 +68,16 @@ struct __align__(16) Item {
 // phase B -> C (-> B2), per batch item (written by the item's lane, read by the pixel's lane):
 template <bool NRM>
 struct BatchShared {
-  float4 eam[32];               // exp(-tau_v), alpha_v, (a+b)/2, voxel id (forward; the weight export reads it);
-                                // backward phase C puts dL/dtau_v into .w for phase B2
-  float4 rgbm[32];              // the voxel's RGB and clamp bits;    backward phase C overwrites .xyz with T alpha g_C
-  float4 nrm[NRM ? 32 : 1];     // the voxel's world normal (O11);    backward phase C overwrites .xyz with T alpha g_N
+  float4 eam[32];               // forward: exp(-tau_v), alpha_v, (a+b)/2, voxel id (the weight export reads it);
+                                // backward: exp(-tau_v), alpha_v, X_v = g_C . rgb_v + g_D mid_v (+ g_N . n_v); phase C then
+                                // overwrites .z with dL/dtau_v and .w with the blend weight T alpha for phase B2
+  float4 rgbm[32];              // forward: the voxel's RGB and clamp bits
+  float4 nrm[NRM ? 32 : 1];     // the voxel's world normal (O11)
+  // backward: the incoming gradients of the warp's 32 pixels (g_C, g_D) and (g_N), filled once per kernel.  An item's lane
+  // reads its pixel's entry in phase B (the pixel's lane index travels in the low byte of the item's meta word), so that
+  // everything of dL/dtau_v that does not depend on the blend order is computed with all lanes busy
+  float4 pg[32];
+  float4 pn[NRM ? 32 : 1];
 };
 
 // Everything only the batch phases touch lives in shared memory, not in registers: the candidate loop of phase A runs
@@ -83,7 +89,8 @@ struct WarpQueue {
   Item item[QCAP];              // ring
   double d0[3];                 // the warp's reference direction for the list being served
   BatchShared<NRM> b;
-  float4 dir[32];               // per pixel: its ray direction in the frame of the list being served (copied into every item)
+  float4 dir[32];               // per pixel: its ray direction in the frame of the list being served, .w = the pixel's lane
+                                // index as bits (copied into every item)
   float4 acc[32];               // forward, per pixel between batches: C (rgb) and D
   float2 tn[32];                //          T and n_used (as bits)
   float4 nacc[NRM ? 32 : 1];    //          N (O11)
@@ -162,9 +169,9 @@ __device__ __forceinline__ void item_geom(const CompositeArgs &A, const WarpQueu
   const float4 i1 = *(reinterpret_cast<const float4 *>(&Q.item[at]) + 1);  // w, mid
   const float4 i2 = *(reinterpret_cast<const float4 *>(&Q.item[at]) + 2);  // d
   id = __float_as_uint(i0.x);
-  meta = __float_as_uint(i0.y);
+  meta = __float_as_uint(i0.y) | __float_as_uint(i2.w);  // low byte: lane of the pixel that owns the item
   mid = i1.w;
-  const uint32_t level = meta >> 16;
+  const uint32_t level = __float_as_uint(i0.y) >> 16;
   // 1 / edge length = (1 / level-16 cell) * 2^(level - 16): exact power-of-two scaling
   const float inv_s = __uint_as_float(s_tree[(meta >> 8) & 0xFFu].w) * __uint_as_float((111u + level) << 23);
   const float ca = i0.z, cb = i0.w;
@@ -302,7 +309,7 @@ __device__ __forceinline__ void red_add_v4(float *addr, float x, float y, float 
 // them after it: there the four extra live registers spill (measured: forward 1.39 -> 1.35 ms, backward 1.83 -> 1.87 ms).
 template <bool BWD, bool NRM>
 __device__ __forceinline__ void phase_B(const CompositeArgs &A, const uint4 *s_tree, int lane, BatchShared<NRM> &bs, uint32_t id,
-                                        uint32_t meta, const ItemGeom &G, float mid, float M[4]) {
+                                        uint32_t meta, const ItemGeom &G, float mid, float M[4], float gv[NRM ? 6 : 3]) {
   float4 f1, nv = make_float4(0.f, 0.f, 0.f, 0.f);
   if (!BWD) {
     f1 = __ldg(reinterpret_cast<const float4 *>(A.fvox + id) + 1);
@@ -315,9 +322,25 @@ __device__ __forceinline__ void phase_B(const CompositeArgs &A, const uint4 *s_t
   }
   const float e = ex2_approx(-tau * LOG2E);
   const float alpha = tau < 1e-3f ? tau * fmaf(-0.5f, tau, 1.0f) : 1.0f - e;  // 1 - exp(-tau) without cancellation
-  bs.eam[lane] = make_float4(e, alpha, mid, __uint_as_float(id));
-  bs.rgbm[lane] = f1;
-  if (NRM) bs.nrm[lane] = nv;
+  if (!BWD) {
+    bs.eam[lane] = make_float4(e, alpha, mid, __uint_as_float(id));
+    bs.rgbm[lane] = f1;
+    if (NRM) bs.nrm[lane] = nv;
+  } else {
+    // what phase C needs of this item besides the blend order: X_v = g_C . rgb_v + g_D mid_v (+ g_N . n_v) with the gradients
+    // of the item's pixel; what phase B2 needs: the pixel's g_C with the clamped channels zeroed (O7) (and g_N)
+    const uint32_t pl = meta & 31u;
+    const float4 g = bs.pg[pl];
+    float X = g.x * f1.x + g.y * f1.y + g.z * f1.z + g.w * mid;
+    const uint32_t cm = __float_as_uint(f1.w);  // colour clamp active: no gradient through that channel (O7)
+    gv[0] = (cm & 1u) ? 0.f : g.x; gv[1] = (cm & 2u) ? 0.f : g.y; gv[2] = (cm & 4u) ? 0.f : g.z;
+    if (NRM) {
+      const float4 gn = bs.pn[pl];
+      X += gn.x * nv.x + gn.y * nv.y + gn.z * nv.z;
+      gv[3] = gn.x; gv[4] = gn.y; gv[5] = gn.z;
+    }
+    bs.eam[lane] = make_float4(e, alpha, X, 0.f);
+  }
 }
 
 // -- C: lane = pixel; its own items of the batch (bit i of `mine` = item i) in batch order = front-to-back order along its
@@ -329,9 +352,8 @@ __device__ __forceinline__ void phase_C(const CompositeArgs &A, BatchShared<NRM>
     const int i = __ffs(mine) - 1;
     mine &= mine - 1;
     if (!S.done) {
-      const float4 f1 = bs.rgbm[i];
       const float4 ea = bs.eam[i];
-      const float e = ea.x, mid = ea.z;
+      const float e = ea.x;
       const float w = S.T * ea.y;
       if (EXP) {  // row N3: the compositing weight of this (pixel, voxel), in the pixel's front-to-back order
         if (S.n_used < S.n_stop) {
@@ -341,6 +363,8 @@ __device__ __forceinline__ void phase_C(const CompositeArgs &A, BatchShared<NRM>
         }
       }
       if (!BWD) {
+        const float4 f1 = bs.rgbm[i];
+        const float mid = ea.z;
         S.C0 = fmaf(w, f1.x, S.C0); S.C1 = fmaf(w, f1.y, S.C1); S.C2 = fmaf(w, f1.z, S.C2);
         S.D = fmaf(w, mid, S.D);
         if (NRM) {
@@ -348,16 +372,10 @@ __device__ __forceinline__ void phase_C(const CompositeArgs &A, BatchShared<NRM>
           S.N0 = fmaf(w, nv.x, S.N0); S.N1 = fmaf(w, nv.y, S.N1); S.N2 = fmaf(w, nv.z, S.N2);
         }
       } else {
-        float X = S.gC0 * f1.x + S.gC1 * f1.y + S.gC2 * f1.z + S.gD * mid;
-        if (NRM) {
-          const float4 nv = bs.nrm[i];
-          X += S.gN0 * nv.x + S.gN1 * nv.y + S.gN2 * nv.z;
-          bs.nrm[i] = make_float4(w * S.gN0, w * S.gN1, w * S.gN2, 0.f);
-        }
+        const float X = ea.z;  // phase B: g_C . rgb_v + g_D mid_v (+ g_N . n_v)
         S.Xpre = fmaf(w, X, S.Xpre);
-        bs.eam[i].w = S.T * e * X - (S.Xtot - S.Xpre) + S.gA * S.T_final;  // dL/dtau_v
-        const uint32_t cm = __float_as_uint(f1.w);  // colour clamp active: no gradient through that channel (O7)
-        bs.rgbm[i] = make_float4((cm & 1u) ? 0.f : w * S.gC0, (cm & 2u) ? 0.f : w * S.gC1, (cm & 4u) ? 0.f : w * S.gC2, 0.f);
+        const float dtau = S.T * e * X - (S.Xtot - S.Xpre) + S.gA * S.T_final;  // dL/dtau_v
+        *reinterpret_cast<float2 *>(&bs.eam[i].z) = make_float2(dtau, w);
       }
       S.T *= e;
       S.n_used++;
@@ -367,9 +385,7 @@ __device__ __forceinline__ void phase_C(const CompositeArgs &A, BatchShared<NRM>
         if (S.n_used >= S.n_stop) S.done = true;
       }
     } else if (BWD) {  // queued before this pixel finished its replay: contributes nothing
-      bs.eam[i].w = 0.f;
-      bs.rgbm[i] = make_float4(0.f, 0.f, 0.f, 0.f);
-      if (NRM) bs.nrm[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+      *reinterpret_cast<float2 *>(&bs.eam[i].z) = make_float2(0.f, 0.f);
     }
   }
 }
@@ -377,20 +393,21 @@ __device__ __forceinline__ void phase_C(const CompositeArgs &A, BatchShared<NRM>
 // -- B2 (backward): lane = item again; corner gradients, run-reduced by voxel, vector reductions
 template <bool NRM>
 __device__ __forceinline__ void phase_B2(const CompositeArgs &A, int lane, int count, const BatchShared<NRM> &bs, const uint4 *s_tree,
-                                         float *const *s_dgeo, uint32_t my_id, uint32_t my_meta, const ItemGeom &G, const float M[4]) {
+                                         float *const *s_dgeo, uint32_t my_id, uint32_t my_meta, const ItemGeom &G, const float M[4],
+                                         const float gv[NRM ? 6 : 3]) {
   constexpr int NV = NRM ? 14 : 11;  // 8 corner gradients, 3 colour, (3 normal)
   float val[NV];
 #pragma unroll
   for (int c = 0; c < NV; ++c) val[c] = 0.f;
   if (lane < count) {
-    const float dtau = bs.eam[lane].w * G.delta;
+    const float2 dw = *reinterpret_cast<const float2 *>(&bs.eam[lane].z);  // phase C: dL/dtau_v, T alpha
+    const float dtau = dw.x * G.delta;
     float cs[8];
     corner_sums(G, M, cs);
 #pragma unroll
     for (int c = 0; c < 8; ++c) val[c] = dtau * cs[c];
-    const float4 wc = bs.rgbm[lane];
-    val[8] = wc.x; val[9] = wc.y; val[10] = wc.z;
-    if (NRM) { const float4 wn = bs.nrm[lane]; val[NV - 3] = wn.x; val[NV - 2] = wn.y; val[NV - 1] = wn.z; }
+    val[8] = dw.y * gv[0]; val[9] = dw.y * gv[1]; val[10] = dw.y * gv[2];
+    if (NRM) { val[NV - 3] = dw.y * gv[3]; val[NV - 2] = dw.y * gv[4]; val[NV - 1] = dw.y * gv[5]; }
   }
   // runs of consecutive items of one voxel (the pixels one list entry hit): segmented suffix sums over the run index,
   // the first lane of each run ends up with the run total.  (The voxel id itself is not a valid segment key: a voxel cut
@@ -493,7 +510,7 @@ __device__ __forceinline__ void flush_batch(const CompositeArgs &A, int lane, Wa
   if (REC) blk = rec_next_block<NRM>(A, lane, tile, warp, Q, rec_ptr);
   __syncwarp();
   ItemGeom G;
-  float M[4];
+  float M[4], gv[NRM ? 6 : 3];
   uint32_t my_id = NONE, my_meta = 0;
   if (lane < count) {
     float mid;
@@ -504,7 +521,7 @@ __device__ __forceinline__ void flush_batch(const CompositeArgs &A, int lane, Wa
       __stcs(reinterpret_cast<float4 *>(mine_rec + 512), make_float4(G.p[0], G.p[1], G.p[2], G.q[0]));
       __stcs(reinterpret_cast<float2 *>(blk + 1024 + 8 * lane), make_float2(G.q[1], G.q[2]));
     }
-    phase_B<BWD, NRM>(A, s_tree, lane, Q.b, my_id, my_meta, G, mid, M);
+    phase_B<BWD, NRM>(A, s_tree, lane, Q.b, my_id, my_meta, G, mid, M, gv);
   }
   uint32_t mine = (uint32_t)my_bits;
   if (count < 32) mine &= (1u << count) - 1u;
@@ -525,7 +542,7 @@ __device__ __forceinline__ void flush_batch(const CompositeArgs &A, int lane, Wa
   my_bits >>= count;
   __syncwarp();
   if (BWD) {
-    phase_B2<NRM>(A, lane, count, Q.b, s_tree, s_dgeo, my_id, my_meta, G, M);
+    phase_B2<NRM>(A, lane, count, Q.b, s_tree, s_dgeo, my_id, my_meta, G, M, gv);
     __syncwarp();
   }
   head = (head + count) & (QCAP - 1);
@@ -626,6 +643,10 @@ __global__ void __launch_bounds__(TILE_THREADS, DVX_TILE_MIN_CTAS) composite_til
     S.n_stop = A.exp_row[pix + 1] - S.exp_pos;
   }
   if (BWD && inside) backward_pixel_init<NRM>(A, u, v, pix, S);
+  if (BWD) {  // pixels outside the image own no items; their entries are zero
+    Q.b.pg[lane] = make_float4(S.gC0, S.gC1, S.gC2, S.gD);
+    if (NRM) Q.b.pn[lane] = make_float4(S.gN0, S.gN1, S.gN2, 0.f);
+  }
   unsigned long long rec_ptr = REC_PTR_START;
   if (!BWD) {
     Q.acc[lane] = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -737,7 +758,7 @@ __global__ void __launch_bounds__(TILE_THREADS, DVX_TILE_MIN_CTAS) composite_til
         inv[a] = d[a] != 0.f ? 1.0f / d[a] : 0.f;
         if (d[a] == 0.f) zmask |= 1u << a;
       }
-      Q.dir[lane] = make_float4(d[0], d[1], d[2], 0.f);  // read back by this lane only, at every emit
+      Q.dir[lane] = make_float4(d[0], d[1], d[2], __uint_as_float((uint32_t)lane));  // read back by this lane only, at every emit
       __syncwarp();
     }
     // warp-uniform "some lane is axis-parallel": keeps the R20 test out of the per-candidate loop (the forward otherwise
@@ -946,6 +967,8 @@ __global__ void __launch_bounds__(TILE_THREADS, DVX_REPLAY_MIN_CTAS) composite_r
   Pix S;
   pixel_state_zero(S, inside);
   if (inside) backward_pixel_init<NRM>(A, u, v, pix, S);
+  bs.pg[lane] = make_float4(S.gC0, S.gC1, S.gC2, S.gD);
+  if (NRM) bs.pn[lane] = make_float4(S.gN0, S.gN1, S.gN2, 0.f);
   const uint32_t warp_global = (uint32_t)tile * 8u + (uint32_t)warp;
   const uint32_t nb = A.rec_tab[2 * warp_global + 1];
   uint32_t chunk = nb ? A.rec_tab[2 * warp_global] : 0u;
@@ -969,19 +992,19 @@ __global__ void __launch_bounds__(TILE_THREADS, DVX_REPLAY_MIN_CTAS) composite_r
     }
     const int count = __popc(__reduce_or_sync(0xffffffffu, cur.mask));  // every item of the batch has one owner
     ItemGeom G;
-    float M[4];
+    float M[4], gv[NRM ? 6 : 3];
     uint32_t my_id = NONE, my_meta = 0;
     if (lane < count) {
       my_id = cur.a.x; my_meta = cur.a.y;
       G.delta = __uint_as_float(cur.a.z);
       G.p[0] = cur.b.x; G.p[1] = cur.b.y; G.p[2] = cur.b.z;
       G.q[0] = cur.b.w; G.q[1] = cur.c.x; G.q[2] = cur.c.y;
-      phase_B<true, NRM>(A, s_tree, lane, bs, my_id, my_meta, G, __uint_as_float(cur.a.w), M);
+      phase_B<true, NRM>(A, s_tree, lane, bs, my_id, my_meta, G, __uint_as_float(cur.a.w), M, gv);
     }
     __syncwarp();
     phase_C<true, NRM, false>(A, bs, cur.mask, S);
     __syncwarp();
-    phase_B2<NRM>(A, lane, count, bs, s_tree, s_dgeo, my_id, my_meta, G, M);
+    phase_B2<NRM>(A, lane, count, bs, s_tree, s_dgeo, my_id, my_meta, G, M, gv);
     __syncwarp();
     cur = nxt;
   }
