@@ -34,8 +34,8 @@ constexpr int TILE_SPLIT = DVX_TILE_SPLIT;
 constexpr int TILE_THREADS = 256 / TILE_SPLIT;
 constexpr int TILE_WARPS = TILE_THREADS / 32;
 constexpr int DVX_TILE_MIN_CTAS = (3 * DVX_TILE_SPLIT);
-constexpr int DVX_RUN_SPLIT = 4;  // backward: runs of one voxel are reduced in pieces of at most this many lanes (1, 2, 8, 16, 32 measured slower)
-constexpr int DVX_RUN_LONG = 32;  // ... unless the batch averages at least this many lanes per run (32: the whole batch is ONE voxel): then the run is reduced whole
+// Backward run reduction: runs of one voxel are reduced in pieces of at most 4 lanes (1, 2, 8, 16, 32 measured slower) unless the
+// whole batch is ONE voxel: then the run is reduced whole (phase_B2).
 constexpr int DVX_CAND_GROUPS = 8;  // phase A: bands of rows of the warp's pixel block that walk their candidates independently.  Forward
                            // compositing of a saved frame, config 3 / config 4, ms, for 1, 2, 4, 8 bands: 1.378 1.377 1.354 1.312 / 1.934 1.943 1.935 1.888
 constexpr int DVX_WARP_W = 4;  // a warp covers DVX_WARP_W x (32 / DVX_WARP_W) pixels
@@ -409,49 +409,39 @@ __device__ __forceinline__ void phase_B2(const CompositeArgs &A, int lane, int c
     val[8] = dw.y * gv[0]; val[9] = dw.y * gv[1]; val[10] = dw.y * gv[2];
     if (NRM) { val[NV - 3] = dw.y * gv[3]; val[NV - 2] = dw.y * gv[4]; val[NV - 1] = dw.y * gv[5]; }
   }
-  // runs of consecutive items of one voxel (the pixels one list entry hit): segmented suffix sums over the run index,
-  // the first lane of each run ends up with the run total.  (The voxel id itself is not a valid segment key: a voxel cut
-  // in two by a box is queued twice, with other voxels in between.)
+  // Items of one voxel sit next to each other in the batch (the pixels one list entry hit in one trip of phase A).  They are
+  // summed in pieces: ADJACENT lanes with the same voxel id inside one aligned group of 4 lanes - two segmented shuffle steps,
+  // no ballots and no run numbering, the piece a lane belongs to follows from its neighbours' ids alone (adjacency matters: a
+  // voxel cut in two by a box is queued twice, with other voxels in between, and those stay separate pieces).  The first
+  // lane of a piece issues its reductions; a run that straddles a group boundary, or is longer than 4, issues several: the L2
+  // absorbs ~3x more reductions cheaper than three more shuffle rounds (pieces of 1, 2, 8, 16, 32 lanes measured slower).
+  // Not so where many warps hammer the same voxel: when the whole batch is ONE voxel (it covers the warp's 4x8 pixels, so
+  // its neighbours' too) the group sums are merged into lane 0 with the three remaining steps.  Warp-uniform choice.
+  // Round 2: pieces were first defined relative to the run's start (a ballot of run heads, clz, a second ballot, popc):
+  // ten more instructions per batch, fewer reductions; the aligned form is faster on config 3 (replay 1.152 -> 1.133 ms)
+  // and on config 4 (1.932 -> 1.890 ms).
   const uint32_t prev = __shfl_up_sync(0xffffffffu, my_id, 1);
-  const bool is_head = lane == 0 || prev != my_id;
-  const uint32_t heads = __ballot_sync(0xffffffffu, is_head);
-  // Runs longer than DVX_RUN_SPLIT lanes are first reduced in pieces of that length (log2(DVX_RUN_SPLIT) scan steps
-  // instead of 5) and each piece issues its own reductions: the L2 absorbs ~3x more of them cheaper than three more
-  // shuffle rounds.  Not so where many warps hammer the same voxel: when the whole batch is one run (count >= DVX_RUN_LONG
-  // x runs; a voxel that covers the warp's 4x8 pixels covers its neighbours' too) the pieces are merged with the remaining
-  // scan steps, keyed by the true run.  Measured (backward compositing, ms): config 4 3.29 -> 2.78, config 3 1.83 -> 1.85;
-  // thresholds 6, 8, 12, 16, 24: config 4 2.98, 2.96, 2.89, 2.89, 2.78, config 3 1.98, 1.97, 1.91, 1.91, 1.85.  Warp-uniform.
-  uint32_t heads2 = heads;
-  {
-    const uint32_t below = heads & (0xffffffffu >> (31 - lane));       // heads at or below this lane
-    const int start = 31 - __clz(below);                                // lane of this run's head
-    const bool extra = lane > start && ((lane - start) % DVX_RUN_SPLIT) == 0;
-    heads2 |= __ballot_sync(0xffffffffu, extra);
+  const uint32_t id1 = __shfl_down_sync(0xffffffffu, my_id, 1), id2 = __shfl_down_sync(0xffffffffu, my_id, 2);
+  const int sub = lane & 3;
+  const bool take1 = sub < 3 && id1 == my_id;
+  const bool take2 = sub < 2 && take1 && id2 == my_id;
+  const bool merge = __all_sync(0xffffffffu, my_id == __shfl_sync(0xffffffffu, my_id, 0));  // the whole batch is ONE voxel
+  const bool is_head2 = merge ? lane == 0 : (sub == 0 || prev != my_id);
+#pragma unroll
+  for (int c = 0; c < NV; ++c) {
+    const float x = __shfl_down_sync(0xffffffffu, val[c], 1);
+    if (take1) val[c] += x;
   }
-  const bool merge = count >= DVX_RUN_LONG * __popc(heads);
-  const bool is_head2 = ((merge ? heads : heads2) >> lane) & 1u;
-  const uint32_t run2 = __popc(heads2 & (0xffffffffu >> (31 - lane)));
 #pragma unroll
-  for (int o = 1; o < DVX_RUN_SPLIT; o <<= 1) {
-    const uint32_t orun = __shfl_down_sync(0xffffffffu, run2, o);
-    const bool take = (lane + o < 32) && orun == run2;
-#pragma unroll
-    for (int c = 0; c < NV; ++c) {
-      const float x = __shfl_down_sync(0xffffffffu, val[c], o);
-      if (take) val[c] += x;
-    }
+  for (int c = 0; c < NV; ++c) {
+    const float x = __shfl_down_sync(0xffffffffu, val[c], 2);
+    if (take2) val[c] += x;
   }
-  if (merge) {  // piece heads sit DVX_RUN_SPLIT lanes apart within a run: the scan continues over them
-    const uint32_t run1 = __popc(heads & (0xffffffffu >> (31 - lane)));
+  if (merge) {  // all 32 lanes one run: the group heads (every fourth lane) are summed into lane 0
 #pragma unroll
-    for (int o = DVX_RUN_SPLIT; o < 32; o <<= 1) {
-      const uint32_t orun = __shfl_down_sync(0xffffffffu, run1, o);
-      const bool take = (lane + o < 32) && orun == run1;
+    for (int o = 4; o < 32; o <<= 1) {
 #pragma unroll
-      for (int c = 0; c < NV; ++c) {
-        const float x = __shfl_down_sync(0xffffffffu, val[c], o);
-        if (take) val[c] += x;
-      }
+      for (int c = 0; c < NV; ++c) val[c] += __shfl_down_sync(0xffffffffu, val[c], o);
     }
   }
   if (my_id != NONE && is_head2) {
