@@ -305,21 +305,16 @@ __device__ __forceinline__ void red_add_v4(float *addr, float x, float y, float 
 
 // -- B: lane = item (lanes < count).  tau_v, exp(-tau_v), alpha_v, the voxel's colour (and normal) -> shared memory, so that
 // C's serial per-pixel loop contains no transcendental and no global load.
-// Forward: the colour (and normal) loads go out before the integration so their latency hides under it.  Backward keeps
-// them after it: there the four extra live registers spill (measured: forward 1.39 -> 1.35 ms, backward 1.83 -> 1.87 ms).
+// The colour (and normal) loads go out before the integration so their latency hides under it - in the backward too since
+// the pixels' gradients left the registers for the shared-memory table (before that the four extra live registers spilled
+// there; end of round 2: replay 1.114 -> 1.083 ms with the early load).
 template <bool BWD, bool NRM>
 __device__ __forceinline__ void phase_B(const CompositeArgs &A, const uint4 *s_tree, int lane, BatchShared<NRM> &bs, uint32_t id,
                                         uint32_t meta, const ItemGeom &G, float mid, float M[4], float gv[NRM ? 6 : 3]) {
   float4 f1, nv = make_float4(0.f, 0.f, 0.f, 0.f);
-  if (!BWD) {
-    f1 = __ldg(reinterpret_cast<const float4 *>(A.fvox + id) + 1);
-    if (NRM) nv = __ldg(A.vnrm + id);
-  }
+  f1 = __ldg(reinterpret_cast<const float4 *>(A.fvox + id) + 1);
+  if (NRM) nv = __ldg(A.vnrm + id);
   const float tau = integrate_geom<BWD>(A, s_tree, id, meta, G, M);
-  if (BWD) {
-    f1 = __ldg(reinterpret_cast<const float4 *>(A.fvox + id) + 1);
-    if (NRM) nv = __ldg(A.vnrm + id);
-  }
   const float e = ex2_approx(-tau * LOG2E);
   const float alpha = tau < 1e-3f ? tau * fmaf(-0.5f, tau, 1.0f) : 1.0f - e;  // 1 - exp(-tau) without cancellation
   if (!BWD) {
@@ -396,10 +391,11 @@ __device__ __forceinline__ void phase_B2(const CompositeArgs &A, int lane, int c
                                          float *const *s_dgeo, uint32_t my_id, uint32_t my_meta, const ItemGeom &G, const float M[4],
                                          const float gv[NRM ? 6 : 3]) {
   constexpr int NV = NRM ? 14 : 11;  // 8 corner gradients, 3 colour, (3 normal)
+  // Every lane computes: lanes past the batch's items (my_id == NONE, only in a warp's last batch) hold defined but
+  // meaningless G / M / gv (the caller initialises them), form pieces of their own and issue no reduction.  (With the
+  // values zeroed first and the arithmetic under `lane < count`: replay 1.114 -> 1.095 ms without.)
   float val[NV];
-#pragma unroll
-  for (int c = 0; c < NV; ++c) val[c] = 0.f;
-  if (lane < count) {
+  {
     const float2 dw = *reinterpret_cast<const float2 *>(&bs.eam[lane].z);  // phase C: dL/dtau_v, T alpha
     const float dtau = dw.x * G.delta;
     float cs[8];
@@ -499,8 +495,8 @@ __device__ __forceinline__ void flush_batch(const CompositeArgs &A, int lane, Wa
   unsigned char *blk = nullptr;
   if (REC) blk = rec_next_block<NRM>(A, lane, tile, warp, Q, rec_ptr);
   __syncwarp();
-  ItemGeom G;
-  float M[4], gv[NRM ? 6 : 3];
+  ItemGeom G = {};
+  float M[4] = {}, gv[NRM ? 6 : 3] = {};
   uint32_t my_id = NONE, my_meta = 0;
   if (lane < count) {
     float mid;
@@ -967,6 +963,8 @@ __global__ void __launch_bounds__(TILE_THREADS, DVX_REPLAY_MIN_CTAS) composite_r
   const unsigned char *blk = A.rec_pool + (size_t)chunk * DVX_REC_CHUNK_STRIDE;
   uint32_t slot = 0;
   RecBatch cur = rec_load(blk, lane);
+  ItemGeom G = {};                        // lanes past a short batch's items keep these (phase B2 computes on every lane)
+  float M[4] = {}, gv[NRM ? 6 : 3] = {};
   // No early exit once every pixel of the block has replayed its n_used voxels: the forward stops walking as soon as all of
   // a warp's pixels are done, so at most the batches still queued at that moment follow, and phase C gives their items zero
   // weight; the vote that tested for it cost more (replay 1.133 -> 1.114 ms on config 3, 1.890 -> 1.853 on config 4).
@@ -983,8 +981,6 @@ __global__ void __launch_bounds__(TILE_THREADS, DVX_REPLAY_MIN_CTAS) composite_r
       nxt = rec_load(blk, lane);
     }
     const int count = __popc(__reduce_or_sync(0xffffffffu, cur.mask));  // every item of the batch has one owner
-    ItemGeom G;
-    float M[4], gv[NRM ? 6 : 3];
     uint32_t my_id = NONE, my_meta = 0;
     if (lane < count) {
       my_id = cur.a.x; my_meta = cur.a.y;
