@@ -838,8 +838,8 @@ dvx_status backward_core(dvx_ctx *ctx, dvx_frame *f, const float *dL_drgb, const
     CU(cudaEventRecord(ev_post, st));
     CU(cudaStreamWaitEvent(post, ev_post, 0));
   }
-  dvx_sh_backward_launch(p, trees_d, A.fvox, A.pxrect, drgb, post);
-  if (dnrm) dvx_normal_backward_launch(p, trees_d, A.pxrect, dnrm, post);
+  dvx_sh_backward_launch(p, trees_d, A.fvox, drgb, post);
+  if (dnrm) dvx_normal_backward_launch(p, trees_d, dnrm, post);
   CU(cudaEventRecord(f->ev[6], post));
   CU(cudaGetLastError());
   f->did_backward = true;

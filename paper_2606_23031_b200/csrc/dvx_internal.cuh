@@ -138,8 +138,7 @@ void dvx_tile_masks_launch(const FrameParams &p, const TreeFrame *trees, uint8_t
                            cudaStream_t st);
 void dvx_preprocess_launch(const FrameParams &p, const TreeFrame *trees, const uint8_t *octmask, FrameVox *fvox,
                            ushort4 *pxrect, float4 *vnrm, unsigned long long *counters, cudaStream_t st);
-void dvx_normal_backward_launch(const FrameParams &p, const TreeFrame *trees, const ushort4 *pxrect, const float *dnrm,
-                                cudaStream_t st);
+void dvx_normal_backward_launch(const FrameParams &p, const TreeFrame *trees, const float *dnrm, cudaStream_t st);
 void dvx_emit_pairs_launch(const FrameParams &p, const TreeFrame *trees, const uint8_t *octmask, const ushort4 *pxrect,
                            const FrameVox *fvox, uint64_t *keys, uint32_t *vals, unsigned long long capacity,
                            unsigned long long *counters, cudaStream_t st);
@@ -151,8 +150,8 @@ struct DvxGradTable { float *dgeo[DVX_MAX_TREES]; float *dsh[DVX_MAX_TREES]; };
 void dvx_patch_grads_launch(TreeFrame *trees, uint32_t n_trees, const DvxGradTable &tbl, const unsigned long long *counters,
                             unsigned long long *rec_last, unsigned long long npix, cudaStream_t st);
 void dvx_publish_rec_launch(const unsigned long long *counters, unsigned long long *rec_last, unsigned long long npix, cudaStream_t st);
-void dvx_sh_backward_launch(const FrameParams &p, const TreeFrame *trees, const FrameVox *fvox, const ushort4 *pxrect,
-                            const float *drgb, cudaStream_t st);
+void dvx_sh_backward_launch(const FrameParams &p, const TreeFrame *trees, const FrameVox *fvox, const float *drgb,
+                            cudaStream_t st);
 
 // ---- dvx_grid.cu (row N2: shared grid-point densities, optimizer step)
 void dvx_corner_keys_launch(const uint64_t *code, uint64_t n_slots, uint64_t *keys, uint32_t *vals, cudaStream_t st);

@@ -513,16 +513,14 @@ __global__ void __launch_bounds__(ORDER_THREADS) tile_order_kernel(const uint32_
 // SH degree 3 (the configured case): four threads per voxel, thread j owns coefficients 4j..4j+3 = 12 consecutive floats,
 // so a quad reads and writes the voxel's 192 contiguous bytes with 16-byte accesses.  Other degrees: one thread per voxel.
 __global__ void __launch_bounds__(PRE_THREADS) sh_backward_kernel(FrameParams p, const TreeFrame *trees,
-                                                                  const FrameVox *fvox, const ushort4 *pxrect,
-                                                                  const float *drgb) {
+                                                                  const FrameVox *fvox, const float *drgb) {
   __shared__ uint32_t s_base[DVX_MAX_TREES + 1];
   for (int i = threadIdx.x; i < (int)p.n_trees; i += blockDim.x) s_base[i] = trees[i].base;
   __syncthreads();
   const uint32_t gt = blockIdx.x * blockDim.x + threadIdx.x;
   const uint32_t g = gt >> 2, part = gt & 3u;
   if (g >= p.v_total) return;
-  ushort4 r = pxrect[g];
-  if (r.x > r.z) return;
+  // drgb was zeroed before the compositing backward: a voxel no ray composited (culled, hidden, or off screen) still holds zeros
   float4 d = reinterpret_cast<const float4 *>(drgb)[g];
   if (d.x == 0.f && d.y == 0.f && d.z == 0.f) return;
   int t = find_tree(s_base, p.n_trees, g);
@@ -564,16 +562,13 @@ __global__ void __launch_bounds__(PRE_THREADS) sh_backward_kernel(FrameParams p,
 // ------------------------------------------------------------------ step 5c: dL/dgeo through the voxel normal (R22)
 // dnrm[v] = sum over pixels of T alpha g_N (world frame).  n = -g / max(|g|, eps): dn/dg = -(I - n n^T)/|g| above eps,
 // -I/eps below; g is linear in the corners with weights +-1/4.  One thread per voxel, after the compositing replay.
-__global__ void __launch_bounds__(PRE_THREADS) normal_backward_kernel(FrameParams p, const TreeFrame *trees,
-                                                                      const ushort4 *pxrect, const float *dnrm) {
+__global__ void __launch_bounds__(PRE_THREADS) normal_backward_kernel(FrameParams p, const TreeFrame *trees, const float *dnrm) {
   __shared__ uint32_t s_base[DVX_MAX_TREES + 1];
   for (int i = threadIdx.x; i < (int)p.n_trees; i += blockDim.x) s_base[i] = trees[i].base;
   __syncthreads();
   const uint32_t g = blockIdx.x * blockDim.x + threadIdx.x;
   if (g >= p.v_total) return;
-  const ushort4 r = pxrect[g];
-  if (r.x > r.z) return;
-  const float4 d = reinterpret_cast<const float4 *>(dnrm)[g];
+  const float4 d = reinterpret_cast<const float4 *>(dnrm)[g];   // zeroed before the compositing backward, like drgb
   if (d.x == 0.f && d.y == 0.f && d.z == 0.f) return;
   const int t = find_tree(s_base, p.n_trees, g);
   const TreeFrame &T = trees[t];
@@ -641,11 +636,10 @@ void dvx_tile_masks_launch(const FrameParams &p, const TreeFrame *trees, uint8_t
                            cudaStream_t st) {
   { DVX_COUNT_LAUNCH(1); tile_masks_kernel<<<blocks_for(p.n_tiles, 128), 128, 0, st>>>(p, trees, octmask, actor_mask); }
 }
-void dvx_normal_backward_launch(const FrameParams &p, const TreeFrame *trees, const ushort4 *pxrect, const float *dnrm,
-                                cudaStream_t st) {
+void dvx_normal_backward_launch(const FrameParams &p, const TreeFrame *trees, const float *dnrm, cudaStream_t st) {
   if (p.v_total) {
     DVX_COUNT_LAUNCH(1);
-    normal_backward_kernel<<<blocks_for(p.v_total, PRE_THREADS), PRE_THREADS, 0, st>>>(p, trees, pxrect, dnrm);
+    normal_backward_kernel<<<blocks_for(p.v_total, PRE_THREADS), PRE_THREADS, 0, st>>>(p, trees, dnrm);
   }
 }
 void dvx_preprocess_launch(const FrameParams &p, const TreeFrame *trees, const uint8_t *octmask, FrameVox *fvox,
@@ -668,9 +662,9 @@ void dvx_ranges_launch(const uint64_t *keys, uint64_t n, uint32_t rank_bits, con
 void dvx_tile_order_launch(const uint32_t *tile_cost, uint32_t n_tiles, uint32_t *tile_order, cudaStream_t st) {
   if (n_tiles) { DVX_COUNT_LAUNCH(1); tile_order_kernel<<<1, ORDER_THREADS, 0, st>>>(tile_cost, n_tiles, tile_order); }
 }
-void dvx_sh_backward_launch(const FrameParams &p, const TreeFrame *trees, const FrameVox *fvox, const ushort4 *pxrect,
-                            const float *drgb, cudaStream_t st) {
-    if (p.v_total) { DVX_COUNT_LAUNCH(1); sh_backward_kernel<<<blocks_for(4ull * p.v_total, PRE_THREADS), PRE_THREADS, 0, st>>>(p, trees, fvox, pxrect, drgb); }
+void dvx_sh_backward_launch(const FrameParams &p, const TreeFrame *trees, const FrameVox *fvox, const float *drgb,
+                            cudaStream_t st) {
+    if (p.v_total) { DVX_COUNT_LAUNCH(1); sh_backward_kernel<<<blocks_for(4ull * p.v_total, PRE_THREADS), PRE_THREADS, 0, st>>>(p, trees, fvox, drgb); }
 }
 void dvx_patch_grads_launch(TreeFrame *trees, uint32_t n_trees, const DvxGradTable &tbl, const unsigned long long *counters,
                             unsigned long long *rec_last, unsigned long long npix, cudaStream_t st) {
