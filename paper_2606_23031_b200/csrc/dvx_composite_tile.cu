@@ -411,18 +411,50 @@ __device__ __forceinline__ void phase_B2(const CompositeArgs &A, int lane, int c
   // voxel cut in two by a box is queued twice, with other voxels in between, and those stay separate pieces).  The first
   // lane of a piece issues its reductions; a run that straddles a group boundary, or is longer than 4, issues several: the L2
   // absorbs ~3x more reductions cheaper than three more shuffle rounds (pieces of 1, 2, 8, 16, 32 lanes measured slower).
-  // Not so where many warps hammer the same voxel: when the whole batch is ONE voxel (it covers the warp's 4x8 pixels, so
-  // its neighbours' too) the group sums are merged into lane 0 with the three remaining steps.  Warp-uniform choice.
+  // Not so where many warps hammer the same voxel: a batch that is ONE voxel (it covers the warp's 4x8 pixels, so its
+  // neighbours' too) is summed whole, see below.  Warp-uniform choice.
   // Round 2: pieces were first defined relative to the run's start (a ballot of run heads, clz, a second ballot, popc):
   // ten more instructions per batch, fewer reductions; the aligned form is faster on config 3 (replay 1.152 -> 1.133 ms)
   // and on config 4 (1.932 -> 1.890 ms).
+  if (__all_sync(0xffffffffu, my_id == __shfl_sync(0xffffffffu, my_id, 0))) {
+    // The whole batch is ONE voxel (coarse voxels near the camera cover whole 4x8 blocks, trip after trip; common on config 4's
+    // coarse static octree).  All 32 lanes are summed, by a transposing butterfly: at the step over lane bit b a lane keeps the half of its
+    // values whose index has the matching bit, gets the partner's copy of that half and hands over the other half, so the
+    // number of values per lane halves as the number of lanes per sum doubles - 8 + 4 + 2 + 1 + 1 shuffles instead of 5 x NV.
+    // Lane 2 i then holds the total of value i and issues one scalar reduction (the 11 or 14 of them are one instruction).
+    // Against five plain shuffle steps into lane 0: replay 1.781 -> 1.742 ms on config 4, unchanged on config 3 (1.06 ms).
+    float v[16];
+#pragma unroll
+    for (int c = 0; c < 16; ++c) v[c] = c < NV ? val[c] : 0.f;
+#pragma unroll
+    for (int h = 8; h >= 1; h >>= 1) {      // h values survive the step over lane bit 2 h
+      const bool up = (lane & (2 * h)) != 0;
+#pragma unroll
+      for (int c = 0; c < h; ++c) {
+        const float keep = up ? v[c + h] : v[c], send = up ? v[c] : v[c + h];
+        v[c] = keep + __shfl_xor_sync(0xffffffffu, send, 2 * h);
+      }
+    }
+    v[0] += __shfl_xor_sync(0xffffffffu, v[0], 1);
+    const int idx = lane >> 1;             // bits 4..1 of the lane = bits 3..0 of the value's index
+    if (!(lane & 1) && idx < NV && my_id != NONE) {
+      if (idx < 8) {
+        const uint32_t ti = (my_meta >> 8) & 0xFFu;
+        if (s_dgeo[ti]) atomicAdd(s_dgeo[ti] + (size_t)(my_id - s_tree[ti].z) * 8 + idx, v[0]);
+      } else if (idx < 11) {
+        atomicAdd(A.drgb + (size_t)my_id * 4 + (idx - 8), v[0]);
+      } else if (NRM) {
+        atomicAdd(A.dnrm + (size_t)my_id * 4 + (idx - 11), v[0]);
+      }
+    }
+    return;
+  }
   const uint32_t prev = __shfl_up_sync(0xffffffffu, my_id, 1);
   const uint32_t id1 = __shfl_down_sync(0xffffffffu, my_id, 1), id2 = __shfl_down_sync(0xffffffffu, my_id, 2);
   const int sub = lane & 3;
   const bool take1 = sub < 3 && id1 == my_id;
   const bool take2 = sub < 2 && take1 && id2 == my_id;
-  const bool merge = __all_sync(0xffffffffu, my_id == __shfl_sync(0xffffffffu, my_id, 0));  // the whole batch is ONE voxel
-  const bool is_head2 = merge ? lane == 0 : (sub == 0 || prev != my_id);
+  const bool is_head2 = sub == 0 || prev != my_id;
 #pragma unroll
   for (int c = 0; c < NV; ++c) {
     const float x = __shfl_down_sync(0xffffffffu, val[c], 1);
@@ -432,13 +464,6 @@ __device__ __forceinline__ void phase_B2(const CompositeArgs &A, int lane, int c
   for (int c = 0; c < NV; ++c) {
     const float x = __shfl_down_sync(0xffffffffu, val[c], 2);
     if (take2) val[c] += x;
-  }
-  if (merge) {  // all 32 lanes one run: the group heads (every fourth lane) are summed into lane 0
-#pragma unroll
-    for (int o = 4; o < 32; o <<= 1) {
-#pragma unroll
-      for (int c = 0; c < NV; ++c) val[c] += __shfl_down_sync(0xffffffffu, val[c], o);
-    }
   }
   if (my_id != NONE && is_head2) {
     const uint32_t ti = (my_meta >> 8) & 0xFFu;
