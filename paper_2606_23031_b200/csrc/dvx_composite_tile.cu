@@ -269,30 +269,33 @@ __device__ __forceinline__ float integrate_geom(const CompositeArgs &A, const ui
 // sum_k act'(raw_k) w_c(u_k) for the 8 corners from the moments: w_c(lambda) = X_bx Y_by Z_bz with
 // X_1 = p_x + q_x lambda, X_0 = (1 - p_x) - q_x lambda, ...  Contract the moments with Z, then Y, then X.
 __device__ __forceinline__ void corner_sums(const ItemGeom &G, const float M[4], float out[8]) {
+  // the b = 1 factor of an axis is u = p + q lambda, the b = 0 factor is 1 - u: contract with u, get the other half by
+  // subtracting from the uncontracted sums: 33 instructions instead of 44.  Every term is a sum of non-negative products
+  // (act' >= 0, u in [0,1]), so a difference loses accuracy only relative to a corner weight that is itself ~0: the error
+  // stays ~1e-7 of the voxel's largest corner gradient (parity tolerance 1e-3 relative, 1e-6 absolute).
+  // Replay 1.062 -> 1.044 ms on config 3, 1.742 -> 1.705 on config 4.
   float Nz[2][3];
 #pragma unroll
-  for (int bz = 0; bz < 2; ++bz) {
-    const float z0 = bz ? G.p[2] : 1.0f - G.p[2], z1 = bz ? G.q[2] : -G.q[2];
-#pragma unroll
-    for (int j = 0; j < 3; ++j) Nz[bz][j] = fmaf(z1, M[j + 1], z0 * M[j]);
+  for (int j = 0; j < 3; ++j) {
+    Nz[1][j] = fmaf(G.q[2], M[j + 1], G.p[2] * M[j]);
+    Nz[0][j] = M[j] - Nz[1][j];
   }
   float Oy[2][2][2];
 #pragma unroll
-  for (int by = 0; by < 2; ++by) {
-    const float y0 = by ? G.p[1] : 1.0f - G.p[1], y1 = by ? G.q[1] : -G.q[1];
+  for (int bz = 0; bz < 2; ++bz)
 #pragma unroll
-    for (int bz = 0; bz < 2; ++bz)
+    for (int j = 0; j < 2; ++j) {
+      Oy[1][bz][j] = fmaf(G.q[1], Nz[bz][j + 1], G.p[1] * Nz[bz][j]);
+      Oy[0][bz][j] = Nz[bz][j] - Oy[1][bz][j];
+    }
 #pragma unroll
-      for (int j = 0; j < 2; ++j) Oy[by][bz][j] = fmaf(y1, Nz[bz][j + 1], y0 * Nz[bz][j]);
-  }
+  for (int by = 0; by < 2; ++by)
 #pragma unroll
-  for (int bx = 0; bx < 2; ++bx) {
-    const float x0 = bx ? G.p[0] : 1.0f - G.p[0], x1 = bx ? G.q[0] : -G.q[0];
-#pragma unroll
-    for (int by = 0; by < 2; ++by)
-#pragma unroll
-      for (int bz = 0; bz < 2; ++bz) out[4 * bx + 2 * by + bz] = fmaf(x1, Oy[by][bz][1], x0 * Oy[by][bz][0]);
-  }
+    for (int bz = 0; bz < 2; ++bz) {
+      const float hi = fmaf(G.q[0], Oy[by][bz][1], G.p[0] * Oy[by][bz][0]);
+      out[4 + 2 * by + bz] = hi;
+      out[2 * by + bz] = Oy[by][bz][0] - hi;
+    }
 }
 
 __device__ __forceinline__ void red_add_v4(float *addr, float x, float y, float z, float w) {
