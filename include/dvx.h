@@ -168,7 +168,7 @@ dvx_status dvx_backward_batch(dvx_ctx *ctx, uint32_t n_frames, dvx_frame *const 
                               const dvx_grad *actor_grads);
 
 /* Hit records.  When dvx_render is given a `saved` handle, the compositing kernel also writes what it composited -
- * per (pixel, voxel) hit 40 bytes: voxel, octree, the clipped segment in the voxel's local coordinates, its length / K
+ * per (pixel, voxel) hit 44 bytes: voxel, octree, owning pixel, the clipped segment in the voxel's local coordinates, its length / K
  * and midpoint, in the order the pixel blended them (Alg. 1's sequence) - into a pool obtained from
  * the caller's allocator, and dvx_backward streams those records instead of walking the sorted tile
  * lists and testing every candidate voxel a second time.  The pool is sized from the hit counts of the context's recent

@@ -57,12 +57,12 @@ struct __align__(16) EntryRec {
 // One queued (pixel, voxel) hit: 48 bytes, written with three 16-byte stores in phase A.
 struct __align__(16) Item {
   uint32_t id;        // global voxel id
-  uint32_t meta;      // tree << 8 | level << 16
+  uint32_t meta;      // tree << 8 | level << 16 (the low byte is free here; see pad)
   float ca, cb;       // clipped sub-segment, relative to t0 (O4, R1)
   float w[3];         // x(tau) - centre = s' d + w
   float mid;          // (a + b) / 2, absolute ray distance (depth, R9)
   float d[3];         // ray direction in the tree frame
-  float pad;
+  float pad;          // as bits: the lane (0..31) of the pixel that owns the item; item_geom ORs it into the low byte of meta
 };
 
 // phase B -> C (-> B2), per batch item (written by the item's lane, read by the pixel's lane):

@@ -66,7 +66,7 @@ enum { CNT_PAIRS = 0, CNT_VVIS = 1, CNT_QTEST = 2, CNT_QHIT = 3, CNT_PAIRS_EFF =
 // backward replays the batches instead of walking the tile lists and testing every candidate voxel again.
 // One batch = DVX_REC_BATCH_BYTES, structure-of-arrays so that each of the three record stores / loads of a warp is one
 // contiguous run:
-//   [   0,  512)  32 x {id, meta, delta, mid}      voxel, tree << 8 | level << 16, (b - a) / K, (a + b) / 2
+//   [   0,  512)  32 x {id, meta, delta, mid}      voxel, owning pixel's lane | tree << 8 | level << 16, (b - a) / K, (a + b) / 2
 //   [ 512, 1024)  32 x {p_x, p_y, p_z, q_x}        local coordinates u(lambda) = p + q lambda on the clipped segment
 //   [1024, 1280)  32 x {q_y, q_z}
 //   [1280, 1408)  32 x ownership mask              bit i of word l: item i of the batch belongs to the warp's pixel l
